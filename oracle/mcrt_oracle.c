@@ -1,0 +1,840 @@
+/*
+ * mcrt_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, single-file CPU implementation (fp64, no blocking, no fusion) of the photon-packet
+ * transport of Heymann & Siebenmorgen, "GPU-based Monte Carlo dust radiative transfer scheme applied
+ * to AGN" (arxiv 1203.2941; text in /root/reference/PAPER.md).  It exists only so that tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs can check and time the
+ * CUDA path against it.  It shares no code, header, table generator or constant with the CUDA
+ * library under paper_1203_2941_b200/csrc/, and the product never calls it.
+ *
+ * The method is a stochastic simulation, so the oracle is the algorithm written out step by step in
+ * the paper's order, with a fixed counter-based random-number contract so that a packet's trajectory
+ * depends only on (seed, packet id, temperature-index field).  Each function cites the passage it
+ * follows; where the paper is silent the reading is the one listed in DESIGN.md ("Readings").
+ *
+ * Parity pins (tests/test_oracle_pins.py): Philox known-answer vectors, DDA vs brute-force slab
+ * intersections, exp(-tau) transmission, Henyey-Greenstein moments, isotropy, exact packet/energy
+ * conservation, constant-albedo ratio, optically thin temperature, Planck/zeta closed forms,
+ * 2x2x2 brute-force quadrature, per-cell redraw equivalence (paper fn. 1), epoch vs serial B&W.
+ * Parity UNPINNED: agreement with DUSTY / Kruegel / Pascucci benchmark SEDs,
+ * whose data are not available here.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).  -ffp-contract=off
+ * matters: every product/sum below is rounded separately, exactly as written.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* CODATA 2018 / SI-2019 exact constants in cgs (reading Q15). */
+static const double ORC_H = 6.62607015e-27;  /* erg s   */
+static const double ORC_K = 1.380649e-16;    /* erg / K */
+static const double ORC_C = 2.99792458e10;   /* cm / s  */
+static const double ORC_TWO_PI = 6.283185307179586476925286766559;
+static const double ORC_FOUR_PI = 12.566370614359172953850573533118;
+
+/* ------------------------------------------------------------------------------------------------
+ * O2  Random numbers.  Philox-4x32-10 (Salmon, Moraes, Dror & Shaw 2011): 10 rounds, multipliers
+ * 0xD2511F53 / 0xCD9E8D57, Weyl key increments 0x9E3779B9 / 0xBB67AE85.  Replaces the paper's
+ * per-thread Mersenne Twister streams (Sect. 3.4) -- north_star item (1).
+ * ---------------------------------------------------------------------------------------------- */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * (uint64_t)c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * (uint64_t)c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* One block -> two uniforms strictly inside (0,1) (reading Q3): u52 = top 52 bits of (w_a*2^32+w_b),
+ * zeta = (2*u52 + 1) * 2^-53.  key = (seed lo, seed hi); counter = (pid lo, pid hi, draw index, pass). */
+void orc_uniforms(uint64_t seed, uint64_t pid, uint32_t draw, uint32_t pass, double out[2])
+{
+    uint32_t ctr[4] = { (uint32_t)pid, (uint32_t)(pid >> 32), draw, pass };
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t w[4];
+    orc_philox4x32_10(ctr, key, w);
+    uint64_t a = (((uint64_t)w[0] << 32) | (uint64_t)w[1]) >> 12;
+    uint64_t b = (((uint64_t)w[2] << 32) | (uint64_t)w[3]) >> 12;
+    out[0] = (double)(2 * a + 1) * 0x1.0p-53;
+    out[1] = (double)(2 * b + 1) * 0x1.0p-53;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O1  Tables.
+ * ---------------------------------------------------------------------------------------------- */
+/* Planck function B_nu(T), erg s^-1 cm^-2 Hz^-1 sr^-1 (Eq. 4). */
+double orc_planck(double nu, double T)
+{
+    double x = ORC_H * nu / (ORC_K * T);
+    return 2.0 * ORC_H * nu * nu * nu / (ORC_C * ORC_C) / expm1(x);
+}
+
+/* dB_nu/dT (Eq. 10): 2 h^2 nu^4 / (c^2 k T^2) * e^-x / (1 - e^-x)^2, x = h nu / k T. */
+double orc_dplanck_dT(double nu, double T)
+{
+    double x = ORC_H * nu / (ORC_K * T);
+    double em = exp(-x);
+    double om = -expm1(-x);
+    return 2.0 * ORC_H * ORC_H * nu * nu * nu * nu / (ORC_C * ORC_C * ORC_K * T * T) * em / (om * om);
+}
+
+/* Bin widths: bin j spans the geometric means of nu_j with its neighbours; the two end bins are
+ * extrapolated with the neighbouring ratio (reading Q15; the paper only says a bin lies between
+ * nu_j and nu_j+1). */
+void orc_bin_widths(int nf, const double *nu, double *dnu)
+{
+    for (int j = 0; j < nf; ++j) {
+        double lo = (j == 0) ? nu[0] * sqrt(nu[0] / nu[1]) : sqrt(nu[j - 1] * nu[j]);
+        double hi = (j == nf - 1) ? nu[nf - 1] * sqrt(nu[nf - 1] / nu[nf - 2]) : sqrt(nu[j] * nu[j + 1]);
+        dnu[j] = hi - lo;
+    }
+}
+
+/* Running sum from the lowest frequency divided by the total; last entry forced to exactly 1.
+ * Returns the total.  A row with zero total becomes (0,...,0,1). */
+static double cumulative(int n, const double *w, double *cdf)
+{
+    double tot = 0.0;
+    for (int j = 0; j < n; ++j) tot += w[j];
+    double run = 0.0;
+    for (int j = 0; j < n; ++j) {
+        run += w[j];
+        cdf[j] = (tot > 0.0) ? run / tot : 0.0;
+    }
+    cdf[n - 1] = 1.0;
+    return tot;
+}
+
+/* Smallest index j with cdf[j] >= z ("the shortest frequency nu' for which the cumulative reaches
+ * zeta", Eq. 5, 116-118 Eq. 10; reading Q17). */
+int orc_lower_bound(const double *cdf, int n, double z)
+{
+    int lo = 0, hi = n - 1;
+    while (lo < hi) {
+        int mid = (lo + hi) / 2;
+        if (cdf[mid] >= z) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+typedef struct {
+    int nx, ny, nz, ns, nf, nT, ndir;
+    double h;              /* cell size, cm */
+    float *rho;            /* [nz][ny][nx] */
+    uint8_t *sp;           /* [nz][ny][nx] */
+    double *nu, *dnu;      /* [nf] */
+    double *kabs, *ksca, *g; /* [ns][nf] */
+    double *Tg;            /* [nT] */
+    double *mu_edges;      /* [ndir+1] */
+    double L;              /* erg/s */
+    double pos[3];         /* source position in cell units */
+    /* tables (O1) */
+    double *kext_h;        /* (kabs+ksca)*h : optical depth per unit density per cell length */
+    double *kabs_h;        /* kabs*h */
+    double *albedo;        /* ksca/(ksca+kabs) */
+    double *J;             /* [ns][nT]  sum_j kabs B_j(T) dnu_j, left side of Eq. 4 */
+    double *cdfB;          /* [ns][nT][nf], Eq. 5 */
+    double *cdfdB;         /* [ns][nT][nf], Eq. 10 */
+    double *srccdf;        /* [nf] */
+} orc_ctx;
+
+orc_ctx *orc_create(int nx, int ny, int nz, double h, const float *rho, const uint8_t *sp, int ns,
+                    int nf, const double *nu, const double *kabs, const double *ksca, const double *g,
+                    int nT, const double *Tg, double L, double Tstar, const double *Lnu_w,
+                    const double pos_cm[3], int ndir, const double *mu_edges)
+{
+    orc_ctx *C = (orc_ctx *)calloc(1, sizeof(orc_ctx));
+    size_t nc = (size_t)nx * ny * nz;
+    C->nx = nx; C->ny = ny; C->nz = nz; C->ns = ns; C->nf = nf; C->nT = nT; C->ndir = ndir; C->h = h; C->L = L;
+    C->rho = (float *)malloc(nc * sizeof(float));       memcpy(C->rho, rho, nc * sizeof(float));
+    C->sp = (uint8_t *)malloc(nc);                      memcpy(C->sp, sp, nc);
+    C->nu = (double *)malloc(nf * sizeof(double));      memcpy(C->nu, nu, nf * sizeof(double));
+    C->dnu = (double *)malloc(nf * sizeof(double));
+    size_t nsf = (size_t)ns * nf;
+    C->kabs = (double *)malloc(nsf * sizeof(double));   memcpy(C->kabs, kabs, nsf * sizeof(double));
+    C->ksca = (double *)malloc(nsf * sizeof(double));   memcpy(C->ksca, ksca, nsf * sizeof(double));
+    C->g = (double *)malloc(nsf * sizeof(double));      memcpy(C->g, g, nsf * sizeof(double));
+    C->Tg = (double *)malloc(nT * sizeof(double));      memcpy(C->Tg, Tg, nT * sizeof(double));
+    C->mu_edges = (double *)malloc((ndir + 1) * sizeof(double));
+    memcpy(C->mu_edges, mu_edges, (ndir + 1) * sizeof(double));
+    for (int a = 0; a < 3; ++a) C->pos[a] = pos_cm[a] / h;
+
+    orc_bin_widths(nf, nu, C->dnu);
+    C->kext_h = (double *)malloc(nsf * sizeof(double));
+    C->kabs_h = (double *)malloc(nsf * sizeof(double));
+    C->albedo = (double *)malloc(nsf * sizeof(double));
+    for (size_t i = 0; i < nsf; ++i) {
+        double kext = kabs[i] + ksca[i];
+        C->kext_h[i] = kext * h;
+        C->kabs_h[i] = kabs[i] * h;
+        C->albedo[i] = (kext > 0.0) ? ksca[i] / kext : 0.0;
+    }
+    C->J = (double *)malloc((size_t)ns * nT * sizeof(double));
+    C->cdfB = (double *)malloc((size_t)ns * nT * nf * sizeof(double));
+    C->cdfdB = (double *)malloc((size_t)ns * nT * nf * sizeof(double));
+    double *w = (double *)malloc(nf * sizeof(double));
+    for (int s = 0; s < ns; ++s)
+        for (int m = 0; m < nT; ++m) {
+            size_t row = ((size_t)s * nT + m) * nf;
+            for (int j = 0; j < nf; ++j) w[j] = kabs[s * nf + j] * orc_planck(nu[j], Tg[m]) * C->dnu[j];
+            C->J[(size_t)s * nT + m] = cumulative(nf, w, C->cdfB + row);
+            for (int j = 0; j < nf; ++j) w[j] = kabs[s * nf + j] * orc_dplanck_dT(nu[j], Tg[m]) * C->dnu[j];
+            cumulative(nf, w, C->cdfdB + row);
+        }
+    /* source: equal-energy packets drawn through the cumulative source spectrum (PAPER.md:39-45,
+     * Eq. 1; reading Q1/Q2: one draw through the CDF on the shared grid). */
+    C->srccdf = (double *)malloc(nf * sizeof(double));
+    for (int j = 0; j < nf; ++j)
+        w[j] = ((Tstar > 0.0) ? orc_planck(nu[j], Tstar) : Lnu_w[j]) * C->dnu[j];
+    cumulative(nf, w, C->srccdf);
+    free(w);
+    return C;
+}
+
+void orc_destroy(orc_ctx *C)
+{
+    if (!C) return;
+    free(C->rho); free(C->sp); free(C->nu); free(C->dnu); free(C->kabs); free(C->ksca); free(C->g);
+    free(C->Tg); free(C->mu_edges); free(C->kext_h); free(C->kabs_h); free(C->albedo); free(C->J);
+    free(C->cdfB); free(C->cdfdB); free(C->srccdf); free(C);
+}
+
+/* table accessors for the pins */
+void orc_get_tables(const orc_ctx *C, double *dnu, double *J, double *cdfB, double *cdfdB, double *albedo,
+                    double *srccdf)
+{
+    if (dnu) memcpy(dnu, C->dnu, C->nf * sizeof(double));
+    if (J) memcpy(J, C->J, (size_t)C->ns * C->nT * sizeof(double));
+    if (cdfB) memcpy(cdfB, C->cdfB, (size_t)C->ns * C->nT * C->nf * sizeof(double));
+    if (cdfdB) memcpy(cdfdB, C->cdfdB, (size_t)C->ns * C->nT * C->nf * sizeof(double));
+    if (albedo) memcpy(albedo, C->albedo, (size_t)C->ns * C->nf * sizeof(double));
+    if (srccdf) memcpy(srccdf, C->srccdf, C->nf * sizeof(double));
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Directions.
+ * ---------------------------------------------------------------------------------------------- */
+/* phi = 2 pi zeta_1, cos(theta) = 1 - 2 zeta_2.  (Here zeta0 -> cos theta, zeta1 -> phi.) */
+void orc_isotropic(double z0, double z1, double u[3])
+{
+    double mu = 1.0 - 2.0 * z0;
+    double phi = ORC_TWO_PI * z1;
+    double st = sqrt(1.0 - mu * mu);
+    u[0] = st * cos(phi);
+    u[1] = st * sin(phi);
+    u[2] = mu;
+}
+
+/* O7 Henyey-Greenstein scattering (phase function Eq. 15).  The paper
+ * gives only P_HG; the sampling is its analytic inversion (reading Q12), isotropic below |g| = 1e-6,
+ * and the new direction is (theta, phi) about the old one (reading Q13). */
+void orc_hg_scatter(double gg, double z0, double z1, const double u[3], double un[3])
+{
+    double mu;
+    if (fabs(gg) <= 1e-6) {
+        mu = 1.0 - 2.0 * z0;
+    } else {
+        double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
+        mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
+        if (mu > 1.0) mu = 1.0;
+        if (mu < -1.0) mu = -1.0;
+    }
+    double phi = ORC_TWO_PI * z1;
+    double sp = sin(phi), cp = cos(phi);
+    double st = sqrt(1.0 - mu * mu);
+    double a0, a1, a2;
+    if (fabs(u[2]) > 0.99999) {
+        a0 = st * cp;
+        a1 = st * sp;
+        a2 = (u[2] > 0.0) ? mu : -mu;
+    } else {
+        double w = sqrt(1.0 - u[2] * u[2]);
+        double iw = 1.0 / w;
+        double t0 = u[0] * u[2] * cp - u[1] * sp;
+        double t1 = u[1] * u[2] * cp + u[0] * sp;
+        a0 = st * t0 * iw + u[0] * mu;
+        a1 = st * t1 * iw + u[1] * mu;
+        a2 = u[2] * mu - st * cp * w;
+    }
+    double inorm = 1.0 / sqrt(a0 * a0 + a1 * a1 + a2 * a2);
+    un[0] = a0 * inorm;
+    un[1] = a1 * inorm;
+    un[2] = a2 * inorm;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * O4  Cell walk.  The paper says only that a packet "enters a neighboring cell according to its
+ * direction of travel"; the walk is the Amanatides-Woo voxel traversal (reading Q8):
+ * per axis the parameter t of the next face, measured from the flight origin in cell units;
+ * the axis with the smallest one is crossed next (ties x before y before z).
+ * ---------------------------------------------------------------------------------------------- */
+typedef struct {
+    double tmax[3], tdel[3];
+    int step[3];
+} orc_dda;
+
+static void dda_setup(orc_dda *D, const double p[3], const double u[3], const int c[3])
+{
+    for (int a = 0; a < 3; ++a) {
+        if (u[a] > 0.0) {
+            double inv = 1.0 / u[a];
+            D->step[a] = 1;
+            D->tmax[a] = ((double)(c[a] + 1) - p[a]) * inv;
+            D->tdel[a] = inv;
+        } else if (u[a] < 0.0) {
+            double inv = 1.0 / u[a];
+            D->step[a] = -1;
+            D->tmax[a] = ((double)c[a] - p[a]) * inv;
+            D->tdel[a] = -inv;
+        } else {
+            D->step[a] = 0;
+            D->tmax[a] = INFINITY;
+            D->tdel[a] = INFINITY;
+        }
+    }
+}
+
+static inline int dda_axis(const orc_dda *D)
+{
+    if (D->tmax[0] <= D->tmax[1] && D->tmax[0] <= D->tmax[2]) return 0;
+    if (D->tmax[1] <= D->tmax[2]) return 1;
+    return 2;
+}
+
+/* start cell of a point (O3; reading Q9): floor(p) unless p sits on a face, then by direction sign */
+static void start_cell(const double p[3], const double u[3], int c[3])
+{
+    for (int a = 0; a < 3; ++a) {
+        double fl = floor(p[a]);
+        if (p[a] != fl) c[a] = (int)fl;
+        else c[a] = (u[a] >= 0.0) ? (int)fl : (int)fl - 1;
+    }
+}
+
+/* Pin helper: list (cell, segment length) of a ray from p along u until it leaves the grid. */
+int orc_dda_trace(int nx, int ny, int nz, const double p[3], const double u[3], int max_n,
+                  int64_t *cells, double *ds_out)
+{
+    int c[3];
+    int n[3] = { nx, ny, nz };
+    start_cell(p, u, c);
+    orc_dda D;
+    dda_setup(&D, p, u, c);
+    double t = 0.0;
+    int cnt = 0;
+    for (;;) {
+        if (c[0] < 0 || c[0] >= n[0] || c[1] < 0 || c[1] >= n[1] || c[2] < 0 || c[2] >= n[2]) break;
+        int a = dda_axis(&D);
+        double tn = D.tmax[a];
+        if (cnt < max_n) {
+            cells[cnt] = ((int64_t)c[2] * ny + c[1]) * nx + c[0];
+            ds_out[cnt] = tn - t;
+        }
+        ++cnt;
+        t = tn;
+        c[a] += D.step[a];
+        D.tmax[a] += D.tdel[a];
+    }
+    return cnt;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * Run state and the packet routine.
+ * ---------------------------------------------------------------------------------------------- */
+enum { ORC_MODE_BW_EPOCH = 0, ORC_MODE_FROZEN_SWEEP = 1 };
+enum { ORC_EV_EMIT = 0, ORC_EV_SCATTER = 1, ORC_EV_ABSORB = 2, ORC_EV_ESCAPE = 3 };
+
+typedef struct {
+    uint64_t hash;
+    uint32_t crossings, scatterings, absorptions, escape_bin;
+} orc_digest;
+
+typedef struct {
+    uint64_t packets, crossings, dusty_crossings, flights, scatterings, absorptions, escapes,
+        direct_escapes, epochs, lucy_adds;
+    int32_t fx_bits, overflow;
+} orc_stats;
+
+typedef struct {
+    int32_t mode;            /* ORC_MODE_* */
+    uint64_t B0, Bmax;       /* epoch schedule; 0 = defaults of O11 */
+    int32_t n_sweeps;        /* frozen-T sweeps (mode 1) */
+    int32_t sweep_T_from_lucy; /* 1: sweeps take T from the Lucy tally, 0: from counts */
+    int32_t n_threads;       /* 1 = serial */
+    int32_t absorb_and_stop; /* pin P10: an absorbed packet ends */
+    int32_t per_cell_redraw; /* pin P11: new zeta on every cell entry, the paper's literal form */
+    int32_t keep_fp64_lucy;  /* pin P14: also keep a compensated fp64 Lucy sum (serial only) */
+    int32_t reset;           /* zero tallies first */
+    uint32_t pass0;          /* RNG pass word of the B&W run */
+} orc_opts;
+
+typedef struct {
+    const orc_ctx *C;
+    uint64_t *k, *kprev;     /* absorption counts */
+    int64_t *Lfx;            /* Lucy path-length tally, fixed point (O9) */
+    double *Lsum, *Lcmp;     /* compensated fp64 copy */
+    uint16_t *tidx;          /* temperature index per cell (O11) */
+    uint64_t *sed, *sed_direct; /* [ndir][nf] */
+    orc_digest *dig;         /* [n_packets] or NULL */
+    double *kabs_fx;         /* kabs_h * 2^FX */
+    const double *cdf;       /* cdfdB (B&W) or cdfB (sweeps) */
+    uint64_t seed;
+    uint32_t pass;
+    int fx;
+    uint64_t pid0_digest;
+    const orc_opts *o;
+} orc_run_t;
+
+static inline void hash_mix(uint64_t *h, uint64_t w)
+{
+    *h = (*h ^ w) * 0x100000001B3ull;
+}
+
+static inline uint64_t event_word(int type, int j, uint64_t cell)
+{
+    return (uint64_t)type | ((uint64_t)j << 8) | (cell << 24);
+}
+
+/* O9 Lucy path-length tally: every traversed dusty cell receives kappa_abs*rho*h*ds (in units of the
+ * packet energy), the linear form of PAPER.md:105 Eq. 9 (reading Q21), kept as a 64-bit fixed-point
+ * integer so that the sum does not depend on the order of additions (integer atomics). */
+static inline void lucy_add(orc_run_t *R, size_t ci, int sj, double rho_c, double ds, orc_stats *st)
+{
+    if (rho_c > 0.0) {
+        double x = R->kabs_fx[sj] * rho_c * ds;
+        int64_t q = (int64_t)llrint(x);
+        __atomic_fetch_add(&R->Lfx[ci], q, __ATOMIC_RELAXED);
+        st->lucy_adds++;
+        if (R->Lsum) { /* Kahan */
+            double y = R->C->kabs_h[sj] * rho_c * ds - R->Lcmp[ci];
+            double tt = R->Lsum[ci] + y;
+            R->Lcmp[ci] = (tt - R->Lsum[ci]) - y;
+            R->Lsum[ci] = tt;
+        }
+    }
+}
+
+static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
+{
+    const orc_ctx *C = R->C;
+    const int nf = C->nf;
+    const int n[3] = { C->nx, C->ny, C->nz };
+    uint32_t d = 0;
+    double z[2];
+    double p[3], u[3];
+    int c[3];
+    uint32_t ncross = 0, nsca = 0, nabs = 0;
+    uint64_t hash = 0xCBF29CE484222325ull;
+
+    /* O3 emit: frequency through the source CDF, isotropic direction */
+    orc_uniforms(R->seed, pid, d++, R->pass, z);
+    int j = orc_lower_bound(C->srccdf, nf, z[0]);
+    orc_uniforms(R->seed, pid, d++, R->pass, z);
+    orc_isotropic(z[0], z[1], u);
+    p[0] = C->pos[0]; p[1] = C->pos[1]; p[2] = C->pos[2];
+    start_cell(p, u, c);
+    hash_mix(&hash, event_word(ORC_EV_EMIT, j, ((uint64_t)c[2] * n[1] + c[1]) * n[0] + c[0]));
+    st->packets++;
+
+    for (;;) { /* one flight per iteration */
+        /* O4 / S3: optical depth to the next interaction, tau = -ln zeta (Eq. 3;
+         * one draw per flight, the form of footnote 1; readings Q4-Q6) */
+        orc_uniforms(R->seed, pid, d++, R->pass, z);
+        double tau = -log(z[0]);
+        double ztype = z[1];
+        st->flights++;
+        orc_dda D;
+        dda_setup(&D, p, u, c);
+        double t = 0.0;
+        size_t ci;
+        int s, sj;
+        double rho_c, kk;
+        int first_cell = 1;
+        for (;;) {
+            int a = dda_axis(&D);
+            double tn = D.tmax[a];
+            double ds = tn - t;
+            ci = ((size_t)c[2] * n[1] + c[1]) * n[0] + c[0];
+            rho_c = (double)C->rho[ci];
+            s = C->sp[ci];
+            sj = s * nf + j;
+            if (R->o->per_cell_redraw && !first_cell) { /* new random number on cell entry */
+                orc_uniforms(R->seed, pid, d++, R->pass, z);
+                tau = -log(z[0]);
+            }
+            first_cell = 0;
+            kk = C->kext_h[sj] * rho_c;   /* Eq. 2 per unit path: (kabs+ksca) * h * rho */
+            double dtau = kk * ds;        /* tau_i, Eq. 2 */
+            if (dtau > tau) break;        /* interact inside this cell (reading Q5: equality leaves) */
+            tau -= dtau;
+            lucy_add(R, ci, sj, rho_c, ds, st);
+            t = tn;
+            c[a] += D.step[a];
+            D.tmax[a] += D.tdel[a];
+            ncross++;
+            st->crossings++;
+            if (rho_c > 0.0) st->dusty_crossings++;
+            if (c[a] < 0 || c[a] >= n[a]) goto escaped;
+        }
+        /* O5 interaction point: l' = tau / (rho (kabs+ksca)) (Eq. 3) */
+        {
+            double sint = tau / kk;
+            lucy_add(R, ci, sj, rho_c, sint, st);
+            double tint = t + sint;
+            for (int a = 0; a < 3; ++a) {
+                double q = p[a] + u[a] * tint;
+                double lo = (double)c[a], hi = (double)(c[a] + 1);
+                if (q < lo) q = lo;
+                if (q > hi) q = hi;
+                p[a] = q;
+            }
+        }
+        /* O6 scatter with probability albedo */
+        if (ztype < C->albedo[sj]) {
+            orc_uniforms(R->seed, pid, d++, R->pass, z);
+            double un[3];
+            orc_hg_scatter(C->g[sj], z[0], z[1], u, un);
+            u[0] = un[0]; u[1] = un[1]; u[2] = un[2];
+            nsca++;
+            st->scatterings++;
+            hash_mix(&hash, event_word(ORC_EV_SCATTER, j, ci));
+        } else {
+            /* O8 absorption: count it, re-emit at once from the same position with a new
+             * frequency and an isotropic direction (readings Q18, Q20) */
+            __atomic_fetch_add(&R->k[ci], (uint64_t)1, __ATOMIC_RELAXED);
+            nabs++;
+            st->absorptions++;
+            if (R->o->absorb_and_stop) {
+                hash_mix(&hash, event_word(ORC_EV_ABSORB, j, ci));
+                goto done;
+            }
+            int m = R->tidx[ci];
+            orc_uniforms(R->seed, pid, d++, R->pass, z);
+            j = orc_lower_bound(R->cdf + ((size_t)s * C->nT + m) * nf, nf, z[0]); /* Eq. 10 / Eq. 5 */
+            orc_uniforms(R->seed, pid, d++, R->pass, z);
+            orc_isotropic(z[0], z[1], u);
+            hash_mix(&hash, event_word(ORC_EV_ABSORB, j, ci));
+        }
+    }
+escaped:
+    {
+        /* O10 escape tally: frequency x |cos i| bin */
+        double amu = fabs(u[2]);
+        int bin = 0;
+        for (int b = 1; b < C->ndir; ++b) if (C->mu_edges[b] <= amu) bin = b;
+        __atomic_fetch_add(&R->sed[(size_t)bin * nf + j], (uint64_t)1, __ATOMIC_RELAXED);
+        st->escapes++;
+        if (nsca + nabs == 0) {
+            __atomic_fetch_add(&R->sed_direct[(size_t)bin * nf + j], (uint64_t)1, __ATOMIC_RELAXED);
+            st->direct_escapes++;
+        }
+        hash_mix(&hash, event_word(ORC_EV_ESCAPE, j, (uint64_t)bin));
+        if (R->dig) R->dig[pid - R->pid0_digest].escape_bin = (uint32_t)bin;
+    }
+done:
+    hash_mix(&hash, (uint64_t)ncross);
+    hash_mix(&hash, (uint64_t)nsca | ((uint64_t)nabs << 32));
+    if (R->dig) {
+        orc_digest *g = &R->dig[pid - R->pid0_digest];
+        g->hash = hash; g->crossings = ncross; g->scatterings = nsca; g->absorptions = nabs;
+    }
+}
+
+static void run_range(orc_run_t *R, uint64_t pid0, uint64_t count, orc_stats *total)
+{
+    int nth = R->o->n_threads > 1 ? R->o->n_threads : 1;
+    if (R->Lsum) nth = 1;
+#ifdef _OPENMP
+    if (nth > 1) {
+        /* packets are independent inside an epoch; integer tallies make the result
+         * independent of the thread count */
+#pragma omp parallel num_threads(nth)
+        {
+            orc_stats st;
+            memset(&st, 0, sizeof st);
+#pragma omp for schedule(dynamic, 64)
+            for (int64_t i = 0; i < (int64_t)count; ++i) run_packet(R, pid0 + (uint64_t)i, &st);
+#pragma omp critical
+            {
+                total->packets += st.packets; total->crossings += st.crossings;
+                total->dusty_crossings += st.dusty_crossings; total->flights += st.flights;
+                total->scatterings += st.scatterings; total->absorptions += st.absorptions;
+                total->escapes += st.escapes; total->direct_escapes += st.direct_escapes;
+                total->lucy_adds += st.lucy_adds;
+            }
+        }
+        return;
+    }
+#endif
+    for (uint64_t i = 0; i < count; ++i) run_packet(R, pid0 + i, total);
+}
+
+/* number of J[s][.] entries strictly below x, clamped to [0, nT-1] */
+static inline int t_index(const orc_ctx *C, int s, double x)
+{
+    const double *J = C->J + (size_t)s * C->nT;
+    int lo = 0, hi = C->nT; /* first index with J >= x */
+    while (lo < hi) {
+        int mid = (lo + hi) / 2;
+        if (J[mid] < x) lo = mid + 1; else hi = mid;
+    }
+    if (lo > C->nT - 1) lo = C->nT - 1;
+    return lo;
+}
+
+typedef struct {
+    const orc_ctx *C;
+    size_t nc;
+    uint64_t *k, *kprev;
+    int64_t *Lfx;
+    double *Lsum, *Lcmp;
+    uint16_t *tidx;
+    uint64_t *sed, *sed_direct;
+    int fx;
+    double xi;               /* packet energy L/N of the last run */
+} orc_state;
+
+orc_state *orc_state_create(const orc_ctx *C)
+{
+    orc_state *S = (orc_state *)calloc(1, sizeof(orc_state));
+    S->C = C;
+    S->nc = (size_t)C->nx * C->ny * C->nz;
+    S->k = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
+    S->kprev = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
+    S->Lfx = (int64_t *)calloc(S->nc, sizeof(int64_t));
+    S->tidx = (uint16_t *)calloc(S->nc, sizeof(uint16_t));
+    S->sed = (uint64_t *)calloc((size_t)C->ndir * C->nf, sizeof(uint64_t));
+    S->sed_direct = (uint64_t *)calloc((size_t)C->ndir * C->nf, sizeof(uint64_t));
+    return S;
+}
+
+void orc_state_destroy(orc_state *S)
+{
+    if (!S) return;
+    free(S->k); free(S->kprev); free(S->Lfx); free(S->Lsum); free(S->Lcmp); free(S->tidx);
+    free(S->sed); free(S->sed_direct); free(S);
+}
+
+static void zero_tallies(orc_state *S)
+{
+    memset(S->k, 0, S->nc * sizeof(uint64_t));
+    memset(S->kprev, 0, S->nc * sizeof(uint64_t));
+    memset(S->Lfx, 0, S->nc * sizeof(int64_t));
+    if (S->Lsum) { memset(S->Lsum, 0, S->nc * sizeof(double)); memset(S->Lcmp, 0, S->nc * sizeof(double)); }
+    memset(S->sed, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
+    memset(S->sed_direct, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
+}
+
+/* fixed-point fraction bits (O9): FX = min(40, 58 - ceil(log2 N)) */
+int orc_fx_bits(uint64_t n_packets)
+{
+    int cl = 0;
+    while (((uint64_t)1 << cl) < n_packets && cl < 63) ++cl;
+    int fx = 58 - cl;
+    if (fx > 40) fx = 40;
+    if (fx < 0) fx = 0;
+    return fx;
+}
+
+/* default epoch schedule (O11): B0 = max(256, largest power of two <= N/256), Bmax = 2^20 */
+void orc_default_schedule(uint64_t n_packets, uint64_t *B0, uint64_t *Bmax)
+{
+    uint64_t q = n_packets / 256, b = 256;
+    while (b * 2 <= q) b *= 2;
+    *B0 = b;
+    *Bmax = (uint64_t)1 << 20;
+}
+
+/* O11 epoch rule.  Bjorkman & Wood adjust the temperature after every absorption;
+ * under parallel execution the order of absorptions is undefined, so packets are
+ * processed in epochs in pid order and the temperature index of every cell is frozen inside an epoch
+ * at a midpoint prediction of its count (reading Q19/Q20):
+ *   k~ = k + max(1, 1/2 (k - k_prev) B_e / B_{e-1}),   x = k~ xi / (4 pi rho h^3)   (Eq. 4)
+ *   tidx = #{ J[s][.] < x } clamped. */
+static void epoch_update(orc_state *S, int first_epoch, double ratio, double cellfac)
+{
+    const orc_ctx *C = S->C;
+    for (size_t ci = 0; ci < S->nc; ++ci) {
+        double rho_c = (double)C->rho[ci];
+        uint64_t kk = S->k[ci];
+        if (rho_c > 0.0) {
+            double kt;
+            if (first_epoch) kt = (double)kk + 1.0;
+            else {
+                double pred = 0.5 * (double)(kk - S->kprev[ci]) * ratio;
+                kt = (double)kk + ((pred > 1.0) ? pred : 1.0);
+            }
+            double x = kt * cellfac / rho_c;
+            S->tidx[ci] = (uint16_t)t_index(C, C->sp[ci], x);
+        } else {
+            S->tidx[ci] = 0;
+        }
+        S->kprev[ci] = kk;
+    }
+}
+
+/* S12: temperature index for a frozen-T sweep from the previous pass's tallies */
+static void sweep_update(orc_state *S, int from_lucy, double cellfac)
+{
+    const orc_ctx *C = S->C;
+    double inv_fx = ldexp(1.0, -S->fx);
+    for (size_t ci = 0; ci < S->nc; ++ci) {
+        double rho_c = (double)C->rho[ci];
+        if (rho_c > 0.0) {
+            double e = from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+            double x = e * cellfac / rho_c;
+            S->tidx[ci] = (uint16_t)t_index(C, C->sp[ci], x);
+        } else {
+            S->tidx[ci] = 0;
+        }
+    }
+}
+
+/* O-run: the whole path for N packets.  Returns 0, or -5 on fixed-point overflow (|L| > 2^62). */
+int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, orc_stats *stats,
+            orc_digest *digests)
+{
+    const orc_ctx *C = S->C;
+    orc_stats st;
+    memset(&st, 0, sizeof st);
+    orc_run_t R;
+    memset(&R, 0, sizeof R);
+    if (o->keep_fp64_lucy && !S->Lsum) {
+        S->Lsum = (double *)calloc(S->nc, sizeof(double));
+        S->Lcmp = (double *)calloc(S->nc, sizeof(double));
+    }
+    if (o->reset) zero_tallies(S);
+    S->fx = orc_fx_bits(n_packets);
+    S->xi = C->L / (double)n_packets;                    /* xi = L/N */
+    double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h); /* xi / (4 pi V), Eq. 4 */
+    size_t nsf = (size_t)C->ns * C->nf;
+    R.C = C; R.k = S->k; R.kprev = S->kprev; R.Lfx = S->Lfx; R.tidx = S->tidx;
+    R.Lsum = o->keep_fp64_lucy ? S->Lsum : NULL; R.Lcmp = S->Lcmp;
+    R.sed = S->sed; R.sed_direct = S->sed_direct; R.dig = digests; R.seed = seed; R.fx = S->fx; R.o = o;
+    R.pid0_digest = 0;
+    R.kabs_fx = (double *)malloc(nsf * sizeof(double));
+    for (size_t i = 0; i < nsf; ++i) R.kabs_fx[i] = ldexp(C->kabs_h[i], S->fx);
+    st.fx_bits = S->fx;
+
+    if (o->mode == ORC_MODE_BW_EPOCH) {
+        uint64_t B0 = o->B0, Bmax = o->Bmax, d0, d1;
+        orc_default_schedule(n_packets, &d0, &d1);
+        if (B0 == 0) B0 = d0;
+        if (Bmax == 0) Bmax = d1;
+        if (Bmax < B0) Bmax = B0;
+        R.cdf = C->cdfdB;
+        R.pass = o->pass0;
+        uint64_t done = 0, Bnom = B0, Bprev = 0;
+        int e = 0;
+        while (done < n_packets) {
+            uint64_t Be = n_packets - done < Bnom ? n_packets - done : Bnom;
+            epoch_update(S, e == 0, e == 0 ? 1.0 : (double)Be / (double)Bprev, cellfac);
+            run_range(&R, done, Be, &st);
+            done += Be;
+            Bprev = Be;
+            Bnom = (Bnom * 2 > Bmax) ? Bmax : Bnom * 2;
+            ++e;
+            st.epochs++;
+        }
+    } else {
+        /* iterative scheme of PAPER.md:73: temperatures of the previous run, Eq. 5 for the frequency */
+        R.cdf = C->cdfB;
+        for (int sw = 1; sw <= o->n_sweeps; ++sw) {
+            sweep_update(S, o->sweep_T_from_lucy, cellfac);
+            zero_tallies(S);
+            R.pass = o->pass0 + (uint32_t)sw;
+            run_range(&R, 0, n_packets, &st);
+            st.epochs++;
+        }
+    }
+    free(R.kabs_fx);
+    for (size_t ci = 0; ci < S->nc; ++ci) {
+        int64_t v = S->Lfx[ci];
+        if (v > ((int64_t)1 << 62) || v < -((int64_t)1 << 62)) st.overflow = 1;
+    }
+    if (stats) *stats = st;
+    return st.overflow ? -5 : 0;
+}
+
+/* raw tallies for the parity tests */
+void orc_read_raw(const orc_state *S, uint64_t *k, int64_t *Lfx, uint64_t *sed, uint64_t *sed_direct,
+                  uint16_t *tidx, double *Lsum)
+{
+    if (k) memcpy(k, S->k, S->nc * sizeof(uint64_t));
+    if (Lfx) memcpy(Lfx, S->Lfx, S->nc * sizeof(int64_t));
+    if (sed) memcpy(sed, S->sed, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
+    if (sed_direct) memcpy(sed_direct, S->sed_direct, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
+    if (tidx) memcpy(tidx, S->tidx, S->nc * sizeof(uint16_t));
+    if (Lsum && S->Lsum) memcpy(Lsum, S->Lsum, S->nc * sizeof(double));
+}
+
+/* invert J[s](T) = x by log-log interpolation (O12; Eq. 4; clamp per reading Q16) */
+double orc_T_of_x(const orc_ctx *C, int s, double x)
+{
+    const double *J = C->J + (size_t)s * C->nT;
+    if (!(x > 0.0)) return 0.0;
+    if (x <= J[0]) return C->Tg[0];
+    if (x >= J[C->nT - 1]) return C->Tg[C->nT - 1];
+    int lo = 0, hi = C->nT - 1; /* J[lo] <= x < J[hi] */
+    while (hi - lo > 1) {
+        int mid = (lo + hi) / 2;
+        if (J[mid] <= x) lo = mid; else hi = mid;
+    }
+    double f = log(x / J[lo]) / log(J[hi] / J[lo]);
+    return C->Tg[lo] * exp(f * log(C->Tg[hi] / C->Tg[lo]));
+}
+
+/* O12 physical outputs: E_count = k xi, E_lucy = xi L / 2^FX (erg/s absorbed per cell), T from either,
+ * SED = counts xi / (dnu_j dOmega_bin), dOmega_bin = 4 pi d|mu| (both hemispheres; reading Q22). */
+void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int T_from_lucy, double *SED)
+{
+    const orc_ctx *C = S->C;
+    double inv_fx = ldexp(1.0, -S->fx);
+    double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h);
+    for (size_t ci = 0; ci < S->nc; ++ci) {
+        double ec = (double)S->k[ci] * S->xi;
+        double el = (double)S->Lfx[ci] * inv_fx * S->xi;
+        if (E_count) E_count[ci] = ec;
+        if (E_lucy) E_lucy[ci] = el;
+        if (T) {
+            double rho_c = (double)C->rho[ci];
+            if (rho_c > 0.0) {
+                double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+                T[ci] = (float)orc_T_of_x(C, C->sp[ci], e * cellfac / rho_c);
+            } else T[ci] = 0.0f;
+        }
+    }
+    if (SED)
+        for (int b = 0; b < C->ndir; ++b)
+            for (int j = 0; j < C->nf; ++j) {
+                double dom = ORC_FOUR_PI * (C->mu_edges[b + 1] - C->mu_edges[b]);
+                SED[(size_t)b * C->nf + j] = (double)S->sed[(size_t)b * C->nf + j] * S->xi / (C->dnu[j] * dom);
+            }
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

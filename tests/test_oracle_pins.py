@@ -1,0 +1,458 @@
+"""Pins for the CPU oracle (no GPU): the oracle is checked against what the paper and the mathematics
+fix -- known-answer vectors, closed forms, invariants, brute force -- never against itself.
+
+Pin numbers follow SURVEY.md section 8(c) / DESIGN.md "Pins".
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import special
+
+from paper_1203_2941_b200 import workloads as W
+
+H_PLANCK, K_BOLTZ, C_LIGHT, SIGMA_SB = 6.62607015e-27, 1.380649e-16, 2.99792458e10, 5.670374419e-5
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+NTH = min(8, os.cpu_count() or 1)
+
+
+# ------------------------------------------------------------------------------------------ P1 RNG
+def test_p1_philox_known_answers(orc):
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = orc.philox(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_p1_uniform_mapping(orc):
+    # zeta = (2*u52+1)/2^53 from the block's words; strictly inside (0,1); counter layout (pid lo, pid hi, d, pass)
+    for seed, pid, d, pas in [(1, 0, 0, 0), (2 ** 40 + 5, 2 ** 33 + 7, 11, 3), (0xFFFFFFFFFFFFFFFF, 12345, 2 ** 31, 1)]:
+        w = orc.philox([pid & 0xFFFFFFFF, pid >> 32, d, pas], [seed & 0xFFFFFFFF, seed >> 32])
+        z = orc.uniforms(seed, pid, d, pas)
+        for i in range(2):
+            u52 = ((int(w[2 * i]) << 32) | int(w[2 * i + 1])) >> 12
+            assert z[i] == (2 * u52 + 1) / 2.0 ** 53
+            assert 0.0 < z[i] < 1.0
+    zs = np.array([orc.uniforms(9, p, 0) for p in range(20000)])
+    assert abs(zs.mean() - 0.5) < 4 * math.sqrt(1 / 12 / zs.size)
+    assert abs(np.corrcoef(zs[:, 0], zs[:, 1])[0, 1]) < 0.03
+
+
+# ------------------------------------------------------------------------------------------ P2 DDA
+def _slab_segments(nx, ny, nz, p, u):
+    """Brute force: intersect the ray with every cell's box, keep positive-length overlaps."""
+    out = []
+    for iz in range(nz):
+        for iy in range(ny):
+            for ix in range(nx):
+                t0, t1 = 0.0, np.inf
+                for a, c in zip(range(3), (ix, iy, iz)):
+                    if u[a] == 0.0:  # ray parallel to the faces: a point on a face belongs to the upper cell (Q9)
+                        if not (c <= p[a] < c + 1):
+                            t0, t1 = 1.0, 0.0
+                        continue
+                    ta, tb = (c - p[a]) / u[a], (c + 1 - p[a]) / u[a]
+                    t0, t1 = max(t0, min(ta, tb)), min(t1, max(ta, tb))
+                if t1 - t0 > 1e-11:
+                    out.append((t0, (iz * ny + iy) * nx + ix, t1 - t0))
+    out.sort()
+    return out
+
+
+def test_p2_dda_vs_brute_force(orc):
+    rng = np.random.default_rng(42)
+    n_rays = 0
+    for _ in range(400):
+        nx, ny, nz = rng.integers(1, 6, 3)
+        p = rng.random(3) * np.array([nx, ny, nz])
+        if rng.random() < 0.2:  # start exactly on a face / edge / corner
+            for a in range(3):
+                if rng.random() < 0.5:
+                    p[a] = float(rng.integers(1, [nx, ny, nz][a] + 1) - (1 if [nx, ny, nz][a] > 1 else 0.5))
+            p = np.minimum(np.maximum(p, 1e-9), np.array([nx, ny, nz]) - 1e-9)
+        u = orc.isotropic(rng.random(), rng.random())
+        if rng.random() < 0.1:
+            u = np.zeros(3); u[rng.integers(0, 3)] = rng.choice([-1.0, 1.0])  # axis-parallel
+        cells, ds = orc.dda_trace(int(nx), int(ny), int(nz), p, u)
+        assert np.all(ds >= 0.0)
+        keep = ds > 1e-11
+        ref = _slab_segments(int(nx), int(ny), int(nz), p, u)
+        assert list(cells[keep]) == [r[1] for r in ref]
+        np.testing.assert_allclose(ds[keep], [r[2] for r in ref], rtol=0, atol=1e-12)
+        # chord length to the exit face
+        tex = min(((n if u[a] > 0 else 0.0) - p[a]) / u[a] for a, n in zip(range(3), (nx, ny, nz)) if u[a] != 0)
+        assert abs(ds.sum() - tex) < 1e-12
+        n_rays += 1
+    assert n_rays == 400
+
+
+def test_p2_start_cell_on_corner(orc):
+    # central source on an even grid sits on a corner of 8 cells: the start cell follows the direction signs (Q9)
+    for sx in (-1, 1):
+        for sy in (-1, 1):
+            for sz in (-1, 1):
+                u = np.array([sx, sy, sz]) / math.sqrt(3)
+                cells, ds = orc.dda_trace(4, 4, 4, [2.0, 2.0, 2.0], u)
+                ix, iy, iz = (2 if sx > 0 else 1), (2 if sy > 0 else 1), (2 if sz > 0 else 1)
+                assert cells[0] == (iz * 4 + iy) * 4 + ix
+                assert abs(ds.sum() - 2 * math.sqrt(3)) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------ helpers
+def _mean_over_directions(f, nmu=600, nphi=1200):
+    mu = (np.arange(nmu) + 0.5) / nmu * 2 - 1
+    phi = (np.arange(nphi) + 0.5) / nphi * 2 * np.pi
+    MU, PHI = np.meshgrid(mu, phi, indexing="ij")
+    st = np.sqrt(1 - MU ** 2)
+    return f(st * np.cos(PHI), st * np.sin(PHI), MU)
+
+
+# ------------------------------------------------------------------------------------------ P3 transmission
+def test_p3_pure_absorber_transmission(orc):
+    """Uniform pure-absorber cube, central source: the directly escaping fraction per frequency is the
+    direction average of exp(-kappa rho l(u)), l(u) = (n/2)/max|u_a| (exp(-tau) law)."""
+    n, N = 8, 400_000
+    w = W.uniform_cube(n, tau_edge_V=1.5, albedo=0.0, g_const=0.0, n_nu=12, slope=-1.0, T_star=3000.0)
+    o = orc.Oracle.from_workload(w)
+    r = o.run(N, seed=11, absorb_and_stop=True, n_threads=NTH)
+    raw = o.read_raw()
+    assert r["escapes"] + r["absorptions"] == N  # absorbed + escaped = emitted, exactly
+    assert np.array_equal(raw["sed"], raw["sed_direct"])
+    t = o.tables()
+    pj = np.diff(np.concatenate([[0.0], t["srccdf"]]))
+    kext = (w.kappa_abs + w.kappa_sca)[0]
+    rho0 = float(w.rho.flat[0])
+    for j in range(w.n_nu):
+        tau_half = kext[j] * rho0 * w.cell_size_cm * n / 2
+        f = _mean_over_directions(lambda x, y, z: np.exp(-tau_half / np.maximum(np.maximum(abs(x), abs(y)), abs(z)))).mean()
+        p = pj[j] * f
+        got = int(raw["sed_direct"][0, j])
+        sigma = math.sqrt(N * p * (1 - p))
+        assert abs(got - N * p) < 4 * sigma + 1, (j, got, N * p, sigma)
+
+
+# ------------------------------------------------------------------------------------------ P4 HG
+@pytest.mark.parametrize("g", [0.0, 0.3, -0.3, 0.5, 0.7, 0.95])
+def test_p4_henyey_greenstein_moments(orc, g):
+    """<mu> = g and <mu^2> = (1 + 2 g^2)/3 for the phase function of PAPER.md:203 Eq. 15."""
+    rng = np.random.default_rng(int(1000 * abs(g)) + (7 if g < 0 else 3))
+    n = 40000
+    mus = np.empty(n)
+    perp = np.empty((n, 2))
+    for i in range(n):
+        u = orc.isotropic(rng.random(), rng.random())
+        if i % 50 == 0:
+            u = np.array([0.0, 0.0, 1.0 if i % 100 == 0 else -1.0])  # exercise the polar branch
+        v = orc.hg_scatter(g, rng.random(), rng.random(), u)
+        assert abs(np.dot(v, v) - 1.0) < 1e-14
+        mus[i] = np.dot(u, v)
+        # azimuth about u must be uniform: project on a fixed perpendicular frame
+        e1 = np.cross(u, [0.3, -0.5, 0.8]); e1 /= np.linalg.norm(e1)
+        e2 = np.cross(u, e1)
+        perp[i] = (np.dot(v, e1), np.dot(v, e2))
+    var_mu = (1 + 2 * g * g) / 3 - g * g
+    assert abs(mus.mean() - g) < 4 * math.sqrt(var_mu / n) + 1e-12
+    assert abs((mus ** 2).mean() - (1 + 2 * g * g) / 3) < 4 * math.sqrt(0.2 / n)
+    assert np.all(np.abs(perp.mean(axis=0)) < 4 * math.sqrt(0.5 / n))
+
+
+def test_p4_hg_distribution_shape(orc):
+    """Binned cos(theta) follows the integral of P_HG (Eq. 15) between bin edges."""
+    g, n = 0.6, 60000
+    rng = np.random.default_rng(5)
+    u = np.array([0.6, 0.0, 0.8])
+    mus = np.array([np.dot(u, orc.hg_scatter(g, rng.random(), rng.random(), u)) for _ in range(n)])
+    edges = np.linspace(-1, 1, 21)
+    cum = lambda m: (1 - g * g) / (2 * g) * (1 / np.sqrt(1 + g * g - 2 * g * m) - 1 / (1 + g))  # CDF of Eq. 15 in mu
+    p = np.diff(cum(edges))
+    assert abs(p.sum() - 1) < 1e-12
+    cnt, _ = np.histogram(mus, edges)
+    chi2 = ((cnt - n * p) ** 2 / (n * p)).sum()
+    assert chi2 < 50  # 19 dof; 50 is ~1e-4 tail
+
+
+# ------------------------------------------------------------------------------------------ P5 isotropy
+def test_p5_isotropic_emission_and_empty_grid(orc):
+    zs = np.random.default_rng(3).random((50000, 2))
+    us = np.array([orc.isotropic(a, b) for a, b in zs])
+    np.testing.assert_allclose(np.linalg.norm(us, axis=1), 1.0, atol=1e-15)
+    assert np.all(np.abs(us.mean(axis=0)) < 4 * math.sqrt(1 / 3 / len(us)))
+    assert np.all(np.abs((us ** 2).mean(axis=0) - 1 / 3) < 4 * math.sqrt(4 / 45 / len(us)))
+    # empty grid: every packet escapes directly; counts are multinomial with p = w_j * d|mu|
+    w = W.uniform_cube(6, tau_edge_V=0.0, albedo=0.5, g_const=0.0, n_nu=10, n_dir=5, T_star=4000.0)
+    N = 200_000
+    o = orc.Oracle.from_workload(w)
+    r = o.run(N, seed=5, n_threads=NTH)
+    raw = o.read_raw()
+    assert r["direct_escapes"] == N and r["absorptions"] == 0 and r["scatterings"] == 0
+    assert np.array_equal(raw["sed"], raw["sed_direct"]) and raw["sed"].sum() == N
+    pj = np.diff(np.concatenate([[0.0], o.tables()["srccdf"]]))
+    p = np.outer(np.diff(w.abs_mu_edges), pj)
+    sel = p * N > 20
+    chi2 = (((raw["sed"] - N * p) ** 2)[sel] / (N * p)[sel]).sum()
+    assert chi2 < sel.sum() + 5 * math.sqrt(2 * sel.sum())
+    # the walk length of a central source in an n-cube: crossings >= n/2 per packet
+    assert r["crossings"] >= N * 3
+
+
+# ------------------------------------------------------------------------------------------ P6/P7/P13
+def test_p6_p7_p13_conservation_albedo_determinism(orc):
+    w = W.sphere32(tau_V=3.0)
+    N = 30000
+    o = orc.Oracle.from_workload(w)
+    r1 = o.run(N, seed=1, digests=True, n_threads=1)
+    raw1 = o.read_raw()
+    d1 = r1["digests"]
+    # P6 exact invariants
+    assert raw1["sed"].sum() == N == r1["escapes"]
+    assert raw1["k"].sum() == r1["absorptions"] == d1["absorptions"].sum()
+    assert r1["crossings"] == d1["crossings"].sum()
+    assert r1["scatterings"] == d1["scatterings"].sum()
+    assert raw1["sed_direct"].sum() == r1["direct_escapes"] == ((d1["absorptions"] + d1["scatterings"]) == 0).sum()
+    assert r1["flights"] == N + r1["scatterings"] + r1["absorptions"]
+    assert np.all(raw1["lucy_fx"] >= 0) and np.all(raw1["lucy_fx"][w.rho.reshape(-1) == 0] == 0)
+    # P7 constant albedo 0.5
+    n_int = r1["scatterings"] + r1["absorptions"]
+    assert abs(r1["scatterings"] / n_int - 0.5) < 4 * math.sqrt(0.25 / n_int)
+    # P13 thread count must not change anything
+    r8 = o.run(N, seed=1, digests=True, n_threads=NTH)
+    raw8 = o.read_raw()
+    for key in ("k", "lucy_fx", "sed", "sed_direct", "tidx"):
+        assert np.array_equal(raw1[key], raw8[key]), key
+    assert np.array_equal(d1, r8["digests"])
+    # a different seed gives a different realisation
+    r2 = o.run(N, seed=2, digests=True, n_threads=NTH)
+    assert not np.array_equal(d1["hash"], r2["digests"]["hash"])
+
+
+# ------------------------------------------------------------------------------------------ P9 tables
+def _wide(n_nu=400, lam_min=0.05, lam_max=2e5):
+    lam = W.wavelength_grid_um(n_nu, lam_min, lam_max)
+    return W.nu_from_lambda_um(lam)
+
+
+def test_p9_planck_closed_forms(orc):
+    nu = _wide()
+    dnu = orc.bin_widths(nu)
+    assert np.all(dnu > 0)
+    # bins tile the axis: sum of widths = outer edge - inner edge
+    assert abs(dnu.sum() - (nu[-1] * math.sqrt(nu[-1] / nu[-2]) - nu[0] * math.sqrt(nu[0] / nu[1]))) < 1e-9 * nu[-1]
+    for T in (30.0, 300.0, 1500.0):
+        B = np.array([orc.planck(v, T) for v in nu])
+        # Stefan-Boltzmann: integral B_nu dnu = sigma T^4 / pi
+        assert abs((B * dnu).sum() / (SIGMA_SB * T ** 4 / math.pi) - 1) < 2e-3
+        # Wien displacement in frequency: h nu_max / k T = 2.821439...
+        fine = np.linspace(2.0, 3.6, 4001) * K_BOLTZ * T / H_PLANCK
+        xm = H_PLANCK * fine[np.argmax([orc.planck(v, T) for v in fine])] / (K_BOLTZ * T)
+        assert abs(xm - 2.8214393721) < 1e-3
+        # dB/dT against a centred finite difference of B
+        for v in (nu[50], nu[200], nu[330]):
+            fd = (orc.planck(v, T * (1 + 1e-5)) - orc.planck(v, T * (1 - 1e-5))) / (2e-5 * T)
+            assert abs(orc.dplanck_dT(v, T) / fd - 1) < 1e-6 if fd > 1e-300 else True
+    # Rayleigh-Jeans limit 2 nu^2 k T / c^2
+    assert abs(orc.planck(1e9, 100.0) / (2 * 1e18 * K_BOLTZ * 100.0 / C_LIGHT ** 2) - 1) < 1e-3
+
+
+@pytest.mark.parametrize("beta", [0.0, 1.5])
+def test_p9_tables_power_law(orc, beta):
+    """For kappa ~ nu^beta: J ~ T^(4+beta); mean h nu/kT of the Eq. 5 CDF is (4+b) zeta(5+b)/zeta(4+b)
+    (3.8322 at b=0, 5.4292 at b=1.5) and of the Eq. 10 CDF (5+b) zeta(5+b)/zeta(4+b) (4.7903, 6.4163)."""
+    nu = _wide()
+    Tg = W.temperature_grid(200, 5.0, 1500.0)
+    kabs = (nu / nu[0]) ** beta
+    o = orc.Oracle(1, 1, 1, 1.0, np.zeros(1, np.float32), np.zeros(1, np.uint8), 1, nu, kabs[None], kabs[None] * 0,
+                   np.zeros((1, len(nu))), Tg, 1.0, 1000.0, None, [0.5, 0.5, 0.5], [0.0, 1.0])
+    t = o.tables()
+    J = t["J"][0]
+    slope = np.diff(np.log(J)) / np.diff(np.log(Tg))
+    np.testing.assert_allclose(slope, 4 + beta, atol=2e-3)
+    # closed form of the integral: 2 h/c^2 (kT/h)^(4+b) Gamma(4+b) zeta(4+b) / nu0^b
+    m = 120
+    closed = 2 * H_PLANCK / C_LIGHT ** 2 * (K_BOLTZ * Tg[m] / H_PLANCK) ** (4 + beta) * special.gamma(4 + beta) \
+        * special.zeta(4 + beta, 1) / nu[0] ** beta
+    assert abs(J[m] / closed - 1) < 2e-3
+    zB = (4 + beta) * special.zeta(5 + beta, 1) / special.zeta(4 + beta, 1)
+    zdB = (5 + beta) * special.zeta(5 + beta, 1) / special.zeta(4 + beta, 1)
+    assert abs(zB - (3.8322 if beta == 0 else 5.4292)) < 1e-3
+    assert abs(zdB - (4.7903 if beta == 0 else 6.4163)) < 1e-3
+    for m in (20, 100, 180):
+        x = H_PLANCK * nu / (K_BOLTZ * Tg[m])
+        for key, ref in (("cdfB", zB), ("cdfdB", zdB)):
+            cdf = t[key][0, m]
+            assert cdf[-1] == 1.0 and np.all(np.diff(cdf) >= 0) and cdf[0] >= 0
+            pj = np.diff(np.concatenate([[0.0], cdf]))
+            assert abs((pj * x).sum() / ref - 1) < 3e-3, (key, m)
+    # T(J(T_m)) round trip and monotone inversion in between
+    for m in (0, 17, 199):
+        assert abs(o.T_of_x(0, J[m]) / Tg[m] - 1) < 1e-12
+    xm = math.sqrt(J[40] * J[41])
+    assert Tg[40] < o.T_of_x(0, xm) < Tg[41]
+    assert abs(o.T_of_x(0, xm) / math.sqrt(Tg[40] * Tg[41]) - 1) < 1e-3
+    assert o.T_of_x(0, 0.0) == 0.0 and o.T_of_x(0, J[0] * 0.1) == Tg[0] and o.T_of_x(0, J[-1] * 10) == Tg[-1]
+    # albedo and lower_bound semantics
+    assert np.all(t["albedo"] == 0.0)
+    cdf = np.array([0.1, 0.1, 0.4, 1.0])
+    assert [orc.lower_bound(cdf, z) for z in (0.05, 0.1, 0.1000001, 0.4, 0.9, 1.0)] == [0, 0, 2, 2, 3, 3]
+
+
+# ------------------------------------------------------------------------------------------ P8 thin temperature
+def test_p8_optically_thin_temperature(orc):
+    """Optically thin sphere, kappa ~ nu^beta, blackbody source inside the T grid:
+    the Lucy-tally temperature follows T = T* (R*/2r)^(2/(4+beta))  (radiative balance, Eq. 4 with Eq. 9)."""
+    beta, Tstar, n, N = 1.0, 1500.0, 24, 600_000
+    lam = W.wavelength_grid_um(160, 0.2, 1e5)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = 100.0 * (nu / nu[-1]) ** beta
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    rho0 = 1e-3 / (kabs.max() * n / 2 * h)  # tau <= 1e-3 at every frequency
+    rho = np.where(r < n / 2, rho0, 0.0).astype(np.float32)
+    L = W.LSUN_ERG_S
+    c = n / 2 * h
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 1, nu, kabs[None], np.zeros((1, len(nu))),
+                   np.zeros((1, len(nu))), W.temperature_grid(1000, 2.0, 2000.0), L, Tstar, None, [c, c, c],
+                   [0.0, 1.0])
+    res = o.run(N, seed=8, n_threads=NTH)
+    assert res["absorptions"] < 0.01 * N
+    T = o.read(T_from_lucy=True)["T"].reshape(n, n, n).astype(np.float64)
+    Rstar = math.sqrt(L / (4 * math.pi * SIGMA_SB * Tstar ** 4))
+    for r_lo in (4.0, 7.0, 10.0):
+        sel = (r >= r_lo) & (r < r_lo + 1.0)
+        T_exp = Tstar * (Rstar / (2 * r[sel] * h)) ** (2 / (4 + beta))
+        ratio = (T[sel] / T_exp)
+        assert abs(ratio.mean() - 1) < 0.01, (r_lo, ratio.mean())
+    # the estimator itself, free of the T tables: x_cell r^2 16 pi^2 / L = sum_j kappa_j p_j
+    out = o.read()
+    pj = np.diff(np.concatenate([[0.0], o.tables()["srccdf"]]))
+    sel = (r >= 5.0) & (r < 9.0)
+    xcell = out["E_lucy"].reshape(n, n, n)[sel] / (4 * math.pi * rho0 * h ** 3)
+    got = (xcell * (r[sel] * h) ** 2).mean() * 16 * math.pi ** 2 / L
+    assert abs(got / (kabs * pj).sum() - 1) < 0.01
+
+
+# ------------------------------------------------------------------------------------------ P10 brute force 2x2x2
+def test_p10_brute_force_2x2x2(orc):
+    """2x2x2 grid of different densities, grey pure absorber, off-centre source, absorb-and-stop:
+    E[k_c] = N <exp(-tau_in) - exp(-tau_out)> by dense direction quadrature with slab intersections;
+    the Lucy tally has the same expectation."""
+    N = 400_000
+    w = W.uniform_cube(2, tau_edge_V=1.0, albedo=0.0, g_const=0.0, n_nu=4, slope=0.0,
+                       source_offset_cells=(0.3, -0.2, 0.1))
+    base = float(w.rho.flat[0])
+    w.rho[:] = (base * np.array([0.5, 1.0, 2.0, 0.0, 1.5, 3.0, 0.25, 0.8], np.float32)).reshape(2, 2, 2)
+    o = orc.Oracle.from_workload(w)
+    r = o.run(N, seed=21, absorb_and_stop=True, n_threads=NTH)
+    raw = o.read_raw()
+    kext = float((w.kappa_abs + w.kappa_sca)[0, 0])
+    assert np.allclose((w.kappa_abs + w.kappa_sca)[0], kext)
+    p = np.array(w.source_pos_cm) / w.cell_size_cm
+
+    def expect(ux, uy, uz):
+        u = np.stack([ux, uy, uz])
+        t_in = np.zeros((8,) + ux.shape)
+        t_out = np.zeros_like(t_in)
+        for c in range(8):
+            idx = (c & 1, (c >> 1) & 1, (c >> 2) & 1)
+            lo, hi = np.zeros_like(ux), np.full_like(ux, np.inf)
+            for a in range(3):
+                ta, tb = (idx[a] - p[a]) / u[a], (idx[a] + 1 - p[a]) / u[a]
+                lo, hi = np.maximum(lo, np.minimum(ta, tb)), np.minimum(hi, np.maximum(ta, tb))
+            t_in[c], t_out[c] = lo, np.maximum(hi, lo)
+        dtau = (t_out - t_in) * (kext * w.rho.reshape(-1).astype(np.float64) * w.cell_size_cm)[:, None, None]
+        tau_in = np.zeros_like(t_in)
+        for c in range(8):
+            for c2 in range(8):
+                tau_in[c] += np.where(t_in[c2] < t_in[c] - 1e-13, dtau[c2], 0.0)
+        return np.exp(-tau_in) - np.exp(-(tau_in + dtau))
+
+    prob = _mean_over_directions(expect, 500, 1000).mean(axis=(1, 2))
+    k = raw["k"].astype(np.float64)
+    lucy = raw["lucy_fx"] / 2.0 ** r["fx_bits"]
+    for c in range(8):
+        sig = math.sqrt(N * prob[c] * (1 - prob[c])) + 1
+        assert abs(k[c] - N * prob[c]) < 4 * sig, (c, k[c], N * prob[c])
+        assert abs(lucy[c] - N * prob[c]) < 5 * sig, (c, lucy[c], N * prob[c])
+    assert raw["k"][3] == 0 and raw["lucy_fx"][3] == 0
+    assert raw["k"].sum() + raw["sed"].sum() == N
+
+
+# ------------------------------------------------------------------------------------------ P11 redraw
+def test_p11_per_cell_redraw_equivalence(orc):
+    """PAPER.md:51 (new zeta on every cell entry) vs footnote 1, PAPER.md:61 (one zeta per flight)."""
+    w = W.sphere32(tau_V=2.0, n=16)
+    N = 150_000
+    o = orc.Oracle.from_workload(w)
+    ra = o.run(N, seed=31, n_threads=NTH)
+    a = o.read_raw()
+    rb = o.run(N, seed=32, per_cell_redraw=True, n_threads=NTH)
+    b = o.read_raw()
+    for key in ("absorptions", "scatterings", "crossings", "direct_escapes"):
+        va, vb = ra[key], rb[key]
+        # totals are sums over packets of over-dispersed counts: allow 5 sigma with dispersion factor 4
+        assert abs(va - vb) < 5 * math.sqrt(4 * (va + vb)), (key, va, vb)
+    x = (np.arange(16) + 0.5) - 8
+    rr = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2).reshape(-1)
+    for lo in range(0, 8, 2):
+        sel = (rr >= lo) & (rr < lo + 2)
+        ka, kb = a["k"][sel].sum(), b["k"][sel].sum()
+        assert abs(float(ka) - float(kb)) < 5 * math.sqrt(2.0 * (ka + kb)), (lo, ka, kb)
+        la, lb = a["lucy_fx"][sel].sum(), b["lucy_fx"][sel].sum()
+        assert abs(la / lb - 1) < 0.03
+    sa, sb = a["sed"].sum(axis=0).astype(float), b["sed"].sum(axis=0).astype(float)
+    sel = sa + sb > 200
+    assert (((sa - sb) ** 2)[sel] / (sa + sb)[sel]).sum() < sel.sum() + 5 * math.sqrt(2 * sel.sum())
+
+
+# ------------------------------------------------------------------------------------------ P12 epochs
+def test_p12_epoch_vs_serial_bjorkman_wood(orc):
+    """Epoch semantics (reading Q19) against serial Bjorkman & Wood (B0 = Bmax = 1, T updated after every
+    packet): temperatures from counts agree to 0.5 % shell by shell, emergent spectrum agrees band by band."""
+    w = W.sphere32(tau_V=5.0, n=10)
+    N = 60_000
+    o = orc.Oracle.from_workload(w)
+    re = o.run(N, seed=41, n_threads=NTH)
+    e_raw, e_out = o.read_raw(), o.read()
+    assert re["epochs"] > 5
+    rs = o.run(N, seed=41, B0=1, Bmax=1)
+    s_raw, s_out = o.read_raw(), o.read()
+    assert rs["epochs"] == N
+    x = (np.arange(10) + 0.5) - 5
+    rr = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2).reshape(-1)
+    for lo in range(0, 5):
+        sel = (rr >= lo) & (rr < lo + 1) & (w.rho.reshape(-1) > 0)
+        Te, Ts = e_out["T"][sel].astype(float).mean(), s_out["T"][sel].astype(float).mean()
+        assert abs(Te / Ts - 1) < 0.005, (lo, Te, Ts)
+    # count-T and Lucy-T are consistent where counts are large (both estimate the same energy)
+    big = e_raw["k"] > 400
+    assert big.sum() >= 8
+    Tl = o.read(T_from_lucy=True)["T"][big].astype(float)
+    assert np.all(np.abs(Tl / s_out["T"][big] - 1) < 0.03)
+    # emergent spectrum in 8 broad bands (same seeds, so noise is correlated and the bound is loose)
+    se, ss = e_raw["sed"].sum(axis=0).astype(float), s_raw["sed"].sum(axis=0).astype(float)
+    be, bs = se.reshape(8, 8).sum(axis=1), ss.reshape(8, 8).sum(axis=1)
+    sel = bs > 500
+    assert np.all(np.abs(be[sel] / bs[sel] - 1) < 0.03 + 3 / np.sqrt(bs[sel]))
+
+
+# ------------------------------------------------------------------------------------------ P14 fixed point
+def test_p14_fixed_point_vs_compensated_fp64(orc):
+    w = W.sphere32(tau_V=1.0)
+    o = orc.Oracle.from_workload(w)
+    r = o.run(50_000, seed=1, keep_fp64_lucy=True)
+    raw = o.read_raw(fp64_lucy=True)
+    fx = r["fx_bits"]
+    assert fx == 40 == orc.fx_bits(50_000)
+    assert orc.fx_bits(10 ** 9) == 28 and orc.fx_bits(10 ** 8) == 31 and orc.fx_bits(2 ** 20) == 38
+    L = raw["lucy_fx"] / 2.0 ** fx
+    sel = raw["lucy_fp64"] > 0
+    assert sel.sum() > 10000
+    rel = np.abs(L[sel] / raw["lucy_fp64"][sel] - 1)
+    assert rel.max() < 1e-6
+    # quantisation bound: each add is off by <= 2^-(fx+1)
+    assert np.all(np.abs(L - raw["lucy_fp64"]) <= r["lucy_adds"] * 2.0 ** -(fx + 1))
+    assert orc.default_schedule(10 ** 8) == (2 ** 18, 2 ** 20) and orc.default_schedule(10 ** 5) == (256, 2 ** 20)
+    assert orc.default_schedule(1000) == (256, 2 ** 20)
