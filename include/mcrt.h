@@ -1,0 +1,184 @@
+/*
+ * mcrt.h -- C ABI of the B200-native photon-packet transport library (libmcrt_b200.so).
+ *
+ * The library implements the hot path of the 3-D Monte Carlo dust radiative-transfer method of
+ * Heymann & Siebenmorgen (arxiv 1203.2941; citations are lines of /root/reference/PAPER.md):
+ * packets emitted by a point source walk cell by cell through a Cartesian dust grid (PAPER.md:45-53,
+ * Eq. 2-3), scatter with Henyey-Greenstein sampling (Eq. 15 at PAPER.md:203) or are
+ * absorbed and immediately re-emitted Bjorkman & Wood style (Eq. 4, 5, 10),
+ * while absorption counts, Lucy path-length tallies (Eq. 9) and the escape SED
+ * are accumulated.  Every step runs in hand-written CUDA kernels for sm_100a.
+ *
+ * Conventions
+ *  - Every call returns an int: MCRT_OK (0) or a negative MCRT_E* code.  No exception or abort crosses
+ *    the ABI; mcrt_last_error() returns the message of the last failure of that context.
+ *  - Pointers are HOST pointers unless the call takes an `mcrt_mem where` argument, in which case the
+ *    array arguments marked [where] live in host memory (MCRT_HOST) or in device memory of the
+ *    context's device (MCRT_DEVICE).  The caller owns every array it passes and may free or reuse it
+ *    as soon as the call returns (the library copies what it keeps).  Outputs go to caller-allocated
+ *    buffers; a NULL output pointer skips that output.
+ *  - Grid arrays are [nz][ny][nx] with x the fastest index; the grid spans [0,nx*h]x[0,ny*h]x[0,nz*h].
+ *  - Frequency tables are [n_species][n_nu] on an ascending frequency grid.
+ *  - All work is issued on the context's stream (default: the legacy default stream; see
+ *    mcrt_set_stream).  Calls that return data to the host synchronise that stream.
+ *  - One context = one device (the current device at mcrt_grid_create) = one stream.  A context is
+ *    not thread safe.
+ *  - Call order: mcrt_grid_create -> mcrt_dust_tables -> mcrt_source -> [mcrt_escape_bins] ->
+ *    mcrt_run (any number of times) -> mcrt_read / mcrt_read_raw -> mcrt_destroy.  Out-of-order calls
+ *    return MCRT_ESTATE.
+ */
+#ifndef MCRT_H_
+#define MCRT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mcrt_ctx mcrt_ctx; /* opaque */
+
+typedef enum { MCRT_HOST = 0, MCRT_DEVICE = 1 } mcrt_mem;
+
+enum {
+    MCRT_OK = 0,
+    MCRT_EINVAL = -1,   /* bad argument (message says which) */
+    MCRT_ESTATE = -2,   /* call out of order */
+    MCRT_ENOMEM = -3,   /* workspace too small / allocation failed */
+    MCRT_ECUDA = -4,    /* CUDA runtime error */
+    MCRT_EOVERFLOW = -5 /* a fixed-point Lucy tally exceeded 2^62 */
+};
+
+typedef enum {
+    MCRT_MODE_BW_EPOCH = 0,      /* Bjorkman & Wood immediate re-emission, Eq. 10, deterministic epochs */
+    MCRT_MODE_FROZEN_T_SWEEP = 1 /* iterative scheme of PAPER.md:73: T frozen per sweep, Eq. 5 */
+} mcrt_mode;
+
+/* Options of mcrt_run.  Fill with mcrt_default_opts() first. */
+typedef struct {
+    int32_t mode;              /* mcrt_mode */
+    uint64_t epoch_B0;         /* first epoch size; 0 = max(256, largest power of two <= N/256) */
+    uint64_t epoch_Bmax;       /* largest epoch size; 0 = 2^20.  Epoch e has min(B0*2^e, Bmax) packets */
+    int32_t n_sweeps;          /* MCRT_MODE_FROZEN_T_SWEEP: number of sweeps (each emits N packets) */
+    int32_t sweep_T_from_lucy; /* sweeps take T from the Lucy tally (1) or from absorption counts (0) */
+    int32_t record_digests;    /* keep a per-packet event digest (needs digest capacity in the workspace) */
+    int32_t reset_tallies;     /* zero all tallies before the run (default 1) */
+    uint32_t rng_pass;         /* 4th Philox counter word of the B&W run; sweep s uses rng_pass + s */
+    int32_t grid_blocks;       /* launch tuning, 0 = auto.  Results never depend on it. */
+    int32_t block_threads;     /* launch tuning, 0 = auto (multiple of 32, <= 256) */
+    int32_t time_kernels;      /* bracket every kernel with CUDA events on the context's stream; the
+                                  summed durations are returned in mcrt_run_stats (transport_ms, update_ms) */
+} mcrt_run_opts;
+
+/* Counters of the runs since the last reset (all exact integers). */
+typedef struct {
+    uint64_t packets;          /* packets emitted */
+    uint64_t crossings;        /* cell faces crossed, including the final exit */
+    uint64_t dusty_crossings;  /* of those, traversed cells with rho > 0 */
+    uint64_t flights;          /* optical-depth draws: packets + scatterings + absorptions */
+    uint64_t scatterings;
+    uint64_t absorptions;
+    uint64_t escapes;
+    uint64_t direct_escapes;   /* escaped without any interaction */
+    uint64_t epochs;           /* transport-kernel launches */
+    uint64_t lucy_adds;        /* fixed-point tally additions */
+    uint64_t gpu_launches;     /* all kernels launched by mcrt_run */
+    int32_t fx_bits;           /* fraction bits of the Lucy fixed point, min(40, 58 - ceil(log2 N)) */
+    int32_t overflow;          /* 1 if some |tally| exceeded 2^62 */
+    double transport_ms;       /* summed device time of the transport kernel launches (time_kernels = 1) */
+    double update_ms;          /* summed device time of the per-epoch update / range-check kernels */
+} mcrt_run_stats;
+
+/* Per-packet digest used by the parity tests: 64-bit FNV-1a style hash over the packet's events
+ * (EMIT, SCATTER, ABSORB, ESCAPE; each with cell index and frequency bin) and its counts. */
+typedef struct {
+    uint64_t hash;
+    uint32_t crossings, scatterings, absorptions, escape_bin;
+} mcrt_digest;
+
+/* Bytes of device workspace a context of these sizes needs (pure function).  n_digests = capacity of
+ * the per-packet digest buffer (0 if digests are never recorded). */
+int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_T, int n_dir,
+                         uint64_t n_digests, size_t *bytes_out);
+
+/* Create a context for an nx*ny*nz grid of cubic cells of edge cell_size_cm.
+ *  rho      [where] float  [nz][ny][nx], dust mass density in g cm^-3, finite and >= 0 (0 = vacuum)
+ *  species  [where] uint8  [nz][ny][nx], dust species of the cell, < n_species (1 <= n_species <= 255)
+ *  workspace  device pointer to workspace_bytes bytes owned by the caller (e.g. a torch tensor) that
+ *             must stay valid until mcrt_destroy, or NULL to let the library cudaMalloc its memory.
+ *             256-byte alignment required.  The library sub-allocates from it in call order (grid
+ *             here, tables in mcrt_dust_tables, histograms and digests at the first mcrt_run that
+ *             needs them) and returns MCRT_ENOMEM when it runs out; size it with mcrt_workspace_bytes.
+ * The grid is re-laid out on the device into 4x4x4 bricks of packed 8-byte cell words. */
+int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm, const float *rho,
+                     const uint8_t *species, int n_species, mcrt_mem where, void *workspace,
+                     size_t workspace_bytes);
+
+/* Dust cross sections per species on the frequency grid and the temperature
+ * grid of the T(E) and re-emission tables (Eq. 4, 5, 10).  Host pointers.
+ *  nu_hz [n_nu] strictly ascending; kappa_abs, kappa_sca [n_species][n_nu] in cm^2 g^-1, >= 0 with
+ *  kappa_abs + kappa_sca > 0; g [n_species][n_nu] with |g| < 1; T_grid [n_T] strictly ascending, K.
+ *  2 <= n_nu <= 65535, 2 <= n_T <= 65535.  May be called once per context. */
+int mcrt_dust_tables(mcrt_ctx *ctx, int n_nu, const double *nu_hz, const double *kappa_abs,
+                     const double *kappa_sca, const double *g, int n_T, const double *T_grid);
+
+/* Point source: luminosity L_erg_s split into equal-energy packets xi = L/N.
+ *  T_star_K > 0: blackbody spectrum; otherwise L_nu_weights [n_nu] gives the spectral shape L_nu at the
+ *  grid frequencies (any normalisation, >= 0, not all zero).  pos_cm strictly inside the grid. */
+int mcrt_source(mcrt_ctx *ctx, double L_erg_s, double T_star_K, const double *L_nu_weights,
+                const double pos_cm[3]);
+
+/* Escape histogram bins in |cos i|: abs_mu_edges [n_dir+1] ascending from 0 to 1.
+ * Default (if never called): one bin. */
+int mcrt_escape_bins(mcrt_ctx *ctx, int n_dir, const double *abs_mu_edges);
+
+void mcrt_default_opts(mcrt_run_opts *opts);
+
+/* Transport n_packets packets with ids 0..n_packets-1 ("follow all N photon packets ...
+ * until they ... escape").  opts NULL = defaults.  If stats_out is NULL the call only enqueues work on
+ * the stream and returns without synchronising; otherwise it synchronises and fills stats_out. */
+int mcrt_run(mcrt_ctx *ctx, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts,
+             mcrt_run_stats *stats_out);
+
+/* Synchronise and return the counters accumulated since the last reset. */
+int mcrt_get_stats(mcrt_ctx *ctx, mcrt_run_stats *stats_out);
+
+/* Physical outputs, [where] arrays of the grid shape [nz][ny][nx] unless noted:
+ *  E_abs_count  double, k * xi: absorbed luminosity per cell from absorption counts, erg s^-1 (Eq. 4)
+ *  E_abs_lucy   double, path-length estimate of the same quantity (Eq. 9, linear form)
+ *  T_count, T_lucy  float, dust temperature from either estimate by inverting Eq. 4 (0 where rho = 0
+ *               or nothing was absorbed; clamped to the T grid)
+ *  SED          double [n_dir][n_nu], escaping L_nu per solid angle, erg s^-1 Hz^-1 sr^-1 */
+int mcrt_read(mcrt_ctx *ctx, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy,
+              double *SED, mcrt_mem where);
+
+/* Raw integer tallies (parity tests), [where]: k_abs uint64 [cells]; lucy_fx int64 [cells];
+ * sed_counts, sed_direct uint64 [n_dir][n_nu]; tidx uint16 [cells] (temperature index of the last
+ * epoch); digests [n_packets of the last run] (only if recorded). */
+int mcrt_read_raw(mcrt_ctx *ctx, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_counts,
+                  uint64_t *sed_direct, uint16_t *tidx, mcrt_digest *digests, mcrt_mem where);
+
+/* Host copies of the derived tables (tests): dnu [n_nu], J [n_species][n_T], cdf_B and cdf_dB
+ * [n_species][n_T][n_nu], albedo [n_species][n_nu], src_cdf [n_nu]. */
+int mcrt_read_tables(mcrt_ctx *ctx, double *dnu, double *J, double *cdf_B, double *cdf_dB, double *albedo,
+                     double *src_cdf);
+
+/* Raw Philox-4x32-10 blocks computed ON THE DEVICE for n (counter, key) pairs given on the host
+ * (ctr [n][4], key [n][2], out [n][4]); lets the tests pin the device generator. */
+int mcrt_philox_device(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
+
+/* Use this CUDA stream (a cudaStream_t passed as void*) for all later work of the context. */
+int mcrt_set_stream(mcrt_ctx *ctx, void *cuda_stream);
+
+/* Launch configuration the transport kernel will use on this device (blocks, threads, dynamic smem). */
+int mcrt_launch_config(mcrt_ctx *ctx, int *grid_blocks, int *block_threads, size_t *smem_bytes);
+
+const char *mcrt_last_error(const mcrt_ctx *ctx); /* ctx may be NULL: error of the last failed create */
+const char *mcrt_version(void);
+void mcrt_destroy(mcrt_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCRT_H_ */

@@ -692,10 +692,10 @@ static void epoch_update(orc_state *S, int first_epoch, double ratio, double cel
 }
 
 /* S12: temperature index for a frozen-T sweep from the previous pass's tallies */
-static void sweep_update(orc_state *S, int from_lucy, double cellfac)
+static void sweep_update(orc_state *S, int from_lucy, double cellfac, int fx_of_tallies)
 {
     const orc_ctx *C = S->C;
-    double inv_fx = ldexp(1.0, -S->fx);
+    double inv_fx = ldexp(1.0, -fx_of_tallies);
     for (size_t ci = 0; ci < S->nc; ++ci) {
         double rho_c = (double)C->rho[ci];
         if (rho_c > 0.0) {
@@ -721,7 +721,9 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
         S->Lsum = (double *)calloc(S->nc, sizeof(double));
         S->Lcmp = (double *)calloc(S->nc, sizeof(double));
     }
-    if (o->reset) zero_tallies(S);
+    /* sweeps (S12) take their temperatures from the previous pass's tallies, so only a B&W run resets first */
+    if (o->reset && o->mode == ORC_MODE_BW_EPOCH) zero_tallies(S);
+    const int prev_fx = S->fx;
     S->fx = orc_fx_bits(n_packets);
     S->xi = C->L / (double)n_packets;                    /* xi = L/N */
     double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h); /* xi / (4 pi V), Eq. 4 */
@@ -758,7 +760,7 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
         /* iterative scheme of PAPER.md:73: temperatures of the previous run, Eq. 5 for the frequency */
         R.cdf = C->cdfB;
         for (int sw = 1; sw <= o->n_sweeps; ++sw) {
-            sweep_update(S, o->sweep_T_from_lucy, cellfac);
+            sweep_update(S, o->sweep_T_from_lucy, cellfac, sw == 1 ? prev_fx : S->fx);
             zero_tallies(S);
             R.pass = o->pass0 + (uint32_t)sw;
             run_range(&R, 0, n_packets, &st);

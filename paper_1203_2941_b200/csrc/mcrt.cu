@@ -1,0 +1,1297 @@
+// mcrt.cu -- B200-native (sm_100a) photon-packet transport: C-ABI host layer + CUDA kernels.
+//
+// Implements include/mcrt.h.  Citations are lines of the paper text of Heymann &
+// Siebenmorgen, arxiv 1203.2941.  Design notes, data layout and rooflines: DESIGN.md.
+//
+// Compile with -fmad=false: the fp64 trajectory arithmetic is written so that every product and sum is
+// rounded separately (the parity contract with the CPU oracle).
+//
+// There is NO CPU fallback in this file: every step of the path (S0-S12 of DESIGN.md) runs in the
+// kernels below; host code only builds the small lookup tables once and marshals arguments.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <math_constants.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "mcrt.h"
+
+#define MCRT_VERSION_STRING "mcrt-b200 0.1 (sm_100a)"
+
+// ------------------------------------------------------------------------------------------------
+// constants
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr double kPlanckH = 6.62607015e-27;   // erg s
+constexpr double kBoltzK = 1.380649e-16;      // erg K^-1
+constexpr double kLightC = 2.99792458e10;     // cm s^-1
+constexpr double kTwoPi = 6.283185307179586476925286766559;
+constexpr double kFourPi = 12.566370614359172953850573533118;
+
+constexpr int kBrickCells = 64;     // 4x4x4 cells per brick; 64 cells * 8 B = 512 B = 4 cache lines
+constexpr unsigned kFull = 0xffffffffu;
+
+enum : int { ST_IDLE = 0, ST_EMIT = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4 };
+enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
+
+// device counters (unsigned long long each)
+enum : int { CNT_PACKETS = 0, CNT_CROSS, CNT_DUSTY, CNT_SCA, CNT_ABS, CNT_DIRECT, CNT_OVERFLOW, CNT_NEXT, CNT_N };
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// context
+// ------------------------------------------------------------------------------------------------
+struct mcrt_ctx {
+    int device = 0;
+    cudaStream_t stream = 0;
+    std::string err;
+    // grid
+    int nx = 0, ny = 0, nz = 0, ns = 0;
+    int nbx = 0, nby = 0, nbz = 0;   // bricks per axis
+    size_t nc = 0, ncp = 0;          // cells, padded (bricked) cells
+    double h = 0.0;
+    // workspace (bump allocator)
+    char *ws = nullptr;
+    size_t ws_bytes = 0, ws_used = 0;
+    bool ws_owned_by_caller = false;
+    std::vector<void *> owned;       // cudaMalloc'ed blocks when no workspace was given
+    // device arrays
+    uint2 *cellw = nullptr;               // [ncp] {rho bits, species | tidx<<16}
+    long long *lfx = nullptr;             // [ncp] Lucy fixed-point tally
+    unsigned long long *kabs_cnt = nullptr, *kprev = nullptr;  // [ncp]
+    void *scratch = nullptr;              // [nc*8 bytes]
+    unsigned long long *counters = nullptr;  // [CNT_N]
+    unsigned long long *sed = nullptr, *sed_direct = nullptr;  // [ndir*nf]
+    double *d_kext_h = nullptr, *d_kabs_fx = nullptr, *d_albedo = nullptr, *d_g = nullptr;  // [ns*nf]
+    double *d_srccdf = nullptr, *d_dnu = nullptr, *d_J = nullptr, *d_Tg = nullptr, *d_cdfB = nullptr, *d_cdfdB = nullptr;
+    double *d_mu = nullptr;
+    mcrt_digest *dig = nullptr;
+    uint64_t dig_cap = 0, dig_n = 0;
+    // host tables
+    int nf = 0, nT = 0, ndir = 1, ndir_alloc = 0;
+    std::vector<double> nu, dnu, kabs, ksca, g, Tg, kext_h, kabs_h, albedo, J, cdfB, cdfdB, srccdf, mu_edges;
+    double L = 0.0, pos[3] = {0, 0, 0};
+    bool have_tables = false, have_source = false, mu_dirty = true;
+    // run state
+    uint64_t last_n = 0;
+    int fx = 40;
+    double xi = 0.0;
+    uint64_t epochs = 0, launches = 0;
+    int occ_blocks = 0;
+    // optional per-kernel timing: events e[3i], e[3i+1], e[3i+2] bracket update and transport of launch pair i
+    std::vector<cudaEvent_t> ev_pool;
+    size_t ev_used = 0;
+    double transport_ms = 0.0, update_ms = 0.0;
+};
+
+namespace {
+
+int fail(mcrt_ctx *c, int code, const std::string &msg)
+{
+    if (c) c->err = msg; else g_create_error = msg;
+    return code;
+}
+
+#define CUDA_TRY(c, expr)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (expr);                                                                  \
+        if (e__ != cudaSuccess)                                                                    \
+            return fail((c), MCRT_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e__));     \
+    } while (0)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// record the next timing event on the context's stream (no-op unless timing is on)
+void mark(mcrt_ctx *c, bool on)
+{
+    if (!on) return;
+    if (c->ev_used == c->ev_pool.size()) {
+        cudaEvent_t e;
+        if (cudaEventCreate(&e) != cudaSuccess) return;
+        c->ev_pool.push_back(e);
+    }
+    cudaEventRecord(c->ev_pool[c->ev_used++], c->stream);
+}
+
+// fold the recorded (start, after-update, after-transport) triples into the running sums
+void fold_timing(mcrt_ctx *c)
+{
+    for (size_t i = 0; i + 2 < c->ev_used; i += 3) {
+        float a = 0.f, b = 0.f;
+        if (cudaEventElapsedTime(&a, c->ev_pool[i], c->ev_pool[i + 1]) == cudaSuccess) c->update_ms += a;
+        if (cudaEventElapsedTime(&b, c->ev_pool[i + 1], c->ev_pool[i + 2]) == cudaSuccess) c->transport_ms += b;
+    }
+    c->ev_used = 0;
+}
+
+int ws_alloc(mcrt_ctx *c, void **out, size_t bytes)
+{
+    bytes = align_up(bytes ? bytes : 1, 256);
+    if (c->ws) {
+        if (c->ws_used + bytes > c->ws_bytes)
+            return fail(c, MCRT_ENOMEM, "workspace too small: need " + std::to_string(c->ws_used + bytes) +
+                                            " bytes, have " + std::to_string(c->ws_bytes));
+        *out = c->ws + c->ws_used;
+        c->ws_used += bytes;
+        return MCRT_OK;
+    }
+    void *p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) return fail(c, MCRT_ENOMEM, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    c->owned.push_back(p);
+    *out = p;
+    return MCRT_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------------
+
+// S1  Philox-4x32-10 (Salmon et al. 2011): counter-based, so a packet's stream depends only on
+// (seed, packet id, draw index, pass) and never on scheduling.  Replaces the per-thread Mersenne
+// Twister streams of PAPER.md:126.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t &o0, uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0;
+        const uint32_t n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
+// one block -> two uniforms strictly inside (0,1): zeta = (2*u52+1) * 2^-53
+__device__ __forceinline__ void draw2(uint32_t seed_lo, uint32_t seed_hi, unsigned long long pid, uint32_t d,
+                                      uint32_t pass, double &z0, double &z1)
+{
+    uint32_t w0, w1, w2, w3;
+    philox4x32_10((uint32_t)pid, (uint32_t)(pid >> 32), d, pass, seed_lo, seed_hi, w0, w1, w2, w3);
+    const unsigned long long a = (((unsigned long long)w0 << 32) | w1) >> 12;
+    const unsigned long long b = (((unsigned long long)w2 << 32) | w3) >> 12;
+    z0 = __ull2double_rn(2ull * a + 1ull) * 0x1.0p-53;
+    z1 = __ull2double_rn(2ull * b + 1ull) * 0x1.0p-53;
+}
+
+// smallest j with cdf[j] >= z (Eq. 5 / Eq. 10: "the shortest frequency nu' for which ...")
+__device__ __forceinline__ int lower_bound_cdf(const double *cdf, int n, double z)
+{
+    int lo = 0, hi = n - 1;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (cdf[mid] >= z) hi = mid; else lo = mid + 1;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ void hash_mix(unsigned long long &h, unsigned long long w)
+{
+    h = (h ^ w) * 0x100000001B3ull;
+}
+
+__device__ __forceinline__ unsigned long long event_word(int type, int j, unsigned long long cell)
+{
+    return (unsigned long long)type | ((unsigned long long)j << 8) | (cell << 24);
+}
+
+// brick-major cell index: the grid is stored as 4x4x4 bricks so that a packet's next cell is usually
+// in the same 128-byte line (x or y step) or in the same 512-byte brick (z step).
+__device__ __forceinline__ uint32_t bx_part(int i) { return ((uint32_t)(i >> 2) << 6) | (uint32_t)(i & 3); }
+__device__ __forceinline__ uint32_t by_part(int i, uint32_t sby) { return (uint32_t)(i >> 2) * sby + ((uint32_t)(i & 3) << 2); }
+__device__ __forceinline__ uint32_t bz_part(int i, uint32_t sbz) { return (uint32_t)(i >> 2) * sbz + ((uint32_t)(i & 3) << 4); }
+
+struct TransportParams {
+    const uint2 *__restrict__ cellw;
+    long long *__restrict__ lfx;
+    unsigned long long *__restrict__ kcnt;
+    const double *__restrict__ kext_h, *__restrict__ kabs_fx, *__restrict__ albedo, *__restrict__ g;
+    const double *__restrict__ srccdf, *__restrict__ cdf, *__restrict__ mu_edges;
+    unsigned long long *__restrict__ sed, *__restrict__ sed_direct, *__restrict__ counters;
+    mcrt_digest *__restrict__ dig;
+    int nx, ny, nz, ns, nf, nT, ndir;
+    uint32_t sby, sbz;  // brick strides: nbx*64, nbx*nby*64
+    double px, py, pz;  // source position, cell units
+    unsigned long long pid0, count;
+    uint32_t seed_lo, seed_hi, pass;
+};
+
+// ------------------------------------------------------------------------------------------------
+// S0-S10  the transport kernel: persistent threads, one packet per lane, warp-level refill.
+//
+// Every lane is a small state machine (EMIT / FLY / INTERACT / IDLE).  A warp alternates between
+//  (a) refill: idle lanes take the next packet ids with ONE warp-aggregated atomic on the epoch counter,
+//  (b) events: all lanes that need an emission, a scattering or an absorption + re-emission do it together
+//      (they share the Philox / sincos / DDA-setup code), and
+//  (c) the cell walk: flying lanes step cell by cell; the walk loop keeps going until fewer than
+//      WALK_MIN lanes are still flying while others wait for an event, so both phases run with most
+//      lanes active whatever the mix of optical depths (the paper parks long-lived packets instead,
+//      PAPER.md:128).
+// ------------------------------------------------------------------------------------------------
+#ifndef MCRT_WALK_MIN
+#define MCRT_WALK_MIN 20
+#endif
+
+template <bool RECORD>
+__global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
+{
+    extern __shared__ double smem_d[];
+    const int nsf = P.ns * P.nf;
+    double *s_kext = smem_d;
+    double *s_kabsfx = s_kext + nsf;
+    double *s_alb = s_kabsfx + nsf;
+    double *s_g = s_alb + nsf;
+    double *s_src = s_g + nsf;
+    double *s_mu = s_src + P.nf;
+    unsigned long long *s_cnt = reinterpret_cast<unsigned long long *>(s_mu + P.ndir + 1);
+    unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
+    const int nhist = 2 * P.ndir * P.nf;
+
+    for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
+        s_kext[i] = P.kext_h[i];
+        s_kabsfx[i] = P.kabs_fx[i];
+        s_alb[i] = P.albedo[i];
+        s_g[i] = P.g[i];
+    }
+    for (int i = threadIdx.x; i < P.nf; i += blockDim.x) s_src[i] = P.srccdf[i];
+    for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
+    for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
+    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0ull;
+    __syncthreads();
+
+    const unsigned lane = threadIdx.x & 31u;
+    const unsigned lane_lt = (1u << lane) - 1u;
+    const int nf = P.nf;
+
+    int state = ST_IDLE;
+    bool exhausted = false;
+    unsigned long long pid = 0ull, hash = 0ull;
+    uint32_t d = 0u, ncross = 0u, ndusty = 0u, nsca = 0u, nabs = 0u;
+    double px = 0.0, py = 0.0, pz = 0.0, ux = 0.0, uy = 0.0, uz = 1.0;
+    double tmx = 0.0, tmy = 0.0, tmz = 0.0, tdx = 0.0, tdy = 0.0, tdz = 0.0, t = 0.0, tau = 0.0, ztype = 0.0;
+    int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0, j = 0;
+    uint32_t cpx = 0u, cpy = 0u, cpz = 0u;  // brick-index parts of (ix, iy, iz)
+    double rho_c = 0.0, kk = 0.0;
+    int sj = 0;
+    uint32_t cwy = 0u;
+
+    for (;;) {
+        // ---------------------------------------------------------------- (a) S0 refill
+        const unsigned need = __ballot_sync(kFull, state == ST_IDLE && !exhausted);
+        if (need) {
+            const int leader = __ffs(need) - 1;
+            unsigned long long base = 0ull;
+            if ((int)lane == leader) base = atomicAdd(&P.counters[CNT_NEXT], (unsigned long long)__popc(need));
+            base = __shfl_sync(kFull, base, leader);
+            if (state == ST_IDLE && !exhausted) {
+                const unsigned long long idx = base + (unsigned long long)__popc(need & lane_lt);
+                if (idx < P.count) { pid = P.pid0 + idx; state = ST_EMIT; }
+                else exhausted = true;
+            }
+            if (__any_sync(kFull, exhausted)) exhausted = true;  // the counter only grows
+        }
+        if (exhausted && state == ST_IDLE) state = ST_DONE;
+        const unsigned ev = __ballot_sync(kFull, state == ST_EMIT || state == ST_INTERACT);
+        const unsigned fl = __ballot_sync(kFull, state == ST_FLY);
+        if ((ev | fl) == 0u) break;
+
+        // ---------------------------------------------------------------- (b) events
+        if (state == ST_EMIT || state == ST_INTERACT) {
+            double z0, z1;
+            bool scatter = false;
+            if (state == ST_EMIT) {
+                // S2 emit: frequency through the source CDF (Eq. 1)
+                d = 0u; ncross = 0u; ndusty = 0u; nsca = 0u; nabs = 0u;
+                hash = 0xCBF29CE484222325ull;
+                draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                j = lower_bound_cdf(s_src, nf, z0);
+                px = P.px; py = P.py; pz = P.pz;
+            } else {
+                // S5 partial segment up to the interaction point l' = tau/(rho kappa_ext) (Eq. 3)
+                const double sint = tau / kk;
+                {
+                    const double x = s_kabsfx[sj] * rho_c * sint;
+                    atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + (cpx + cpy + cpz)),
+                              (unsigned long long)__double2ll_rn(x));
+                }
+                const double tint = t + sint;
+                double q;
+                q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
+                q = py + uy * tint; q = fmax(q, (double)iy); q = fmin(q, (double)(iy + 1)); py = q;
+                q = pz + uz * tint; q = fmax(q, (double)iz); q = fmin(q, (double)(iz + 1)); pz = q;
+                const unsigned long long cell = ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
+                // S6 scatter with probability albedo
+                if (ztype < s_alb[sj]) {
+                    scatter = true;
+                    nsca++;
+                    if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
+                } else {
+                    // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
+                    // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
+                    atomicAdd(&P.kcnt[cpx + cpy + cpz], 1ull);
+                    nabs++;
+                    const int s = (int)(cwy & 0xffu);
+                    const int m = (int)(cwy >> 16);
+                    draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                    j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
+                    if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
+                }
+            }
+            // new direction: isotropic or Henyey-Greenstein about the old one (S7)
+            draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+            double mu = 1.0 - 2.0 * z0;
+            if (scatter) {
+                const double gg = s_g[sj];
+                if (fabs(gg) > 1e-6) {
+                    const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
+                    mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
+                    mu = fmin(mu, 1.0);
+                    mu = fmax(mu, -1.0);
+                }
+            }
+            const double phi = kTwoPi * z1;
+            double sp, cp;
+            sincos(phi, &sp, &cp);
+            const double st = sqrt(1.0 - mu * mu);
+            if (scatter) {
+                double a0, a1, a2;
+                if (fabs(uz) > 0.99999) {
+                    a0 = st * cp;
+                    a1 = st * sp;
+                    a2 = (uz > 0.0) ? mu : -mu;
+                } else {
+                    const double w = sqrt(1.0 - uz * uz);
+                    const double iw = 1.0 / w;
+                    const double t0 = ux * uz * cp - uy * sp;
+                    const double t1 = uy * uz * cp + ux * sp;
+                    a0 = st * t0 * iw + ux * mu;
+                    a1 = st * t1 * iw + uy * mu;
+                    a2 = uz * mu - st * cp * w;
+                }
+                const double inorm = 1.0 / sqrt(a0 * a0 + a1 * a1 + a2 * a2);
+                ux = a0 * inorm; uy = a1 * inorm; uz = a2 * inorm;
+            } else {
+                ux = st * cp; uy = st * sp; uz = mu;
+            }
+            if (state == ST_EMIT) {
+                // start cell: floor(p), or by direction sign when p sits on a face (reading Q9)
+                double f;
+                f = floor(px); ix = (px != f) ? (int)f : ((ux >= 0.0) ? (int)f : (int)f - 1);
+                f = floor(py); iy = (py != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1);
+                f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
+                if (RECORD)
+                    hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
+            }
+            // S3 optical depth of the flight: tau = -ln zeta, zeta_1 kept for S6
+            draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+            tau = -log(z0);
+            ztype = z1;
+            // S4 set up the walk (Amanatides-Woo): parameter of the next face per axis
+            if (ux > 0.0) { const double inv = 1.0 / ux; stx = 1; tmx = ((double)(ix + 1) - px) * inv; tdx = inv; }
+            else if (ux < 0.0) { const double inv = 1.0 / ux; stx = -1; tmx = ((double)ix - px) * inv; tdx = -inv; }
+            else { stx = 0; tmx = CUDART_INF; tdx = CUDART_INF; }
+            if (uy > 0.0) { const double inv = 1.0 / uy; sty = 1; tmy = ((double)(iy + 1) - py) * inv; tdy = inv; }
+            else if (uy < 0.0) { const double inv = 1.0 / uy; sty = -1; tmy = ((double)iy - py) * inv; tdy = -inv; }
+            else { sty = 0; tmy = CUDART_INF; tdy = CUDART_INF; }
+            if (uz > 0.0) { const double inv = 1.0 / uz; stz = 1; tmz = ((double)(iz + 1) - pz) * inv; tdz = inv; }
+            else if (uz < 0.0) { const double inv = 1.0 / uz; stz = -1; tmz = ((double)iz - pz) * inv; tdz = -inv; }
+            else { stz = 0; tmz = CUDART_INF; tdz = CUDART_INF; }
+            t = 0.0;
+            cpx = bx_part(ix); cpy = by_part(iy, P.sby); cpz = bz_part(iz, P.sbz);
+            state = ST_FLY;
+        }
+
+        // ---------------------------------------------------------------- (c) S4/S5 cell walk
+        for (;;) {
+            const unsigned flying = __ballot_sync(kFull, state == ST_FLY);
+            if (flying == 0u) break;
+            if (__popc(flying) < MCRT_WALK_MIN &&
+                __any_sync(kFull, state == ST_INTERACT || (state == ST_IDLE && !exhausted))) break;
+            if (state == ST_FLY) {
+                const bool selx = (tmx <= tmy) && (tmx <= tmz);
+                const bool sely = !selx && (tmy <= tmz);
+                const double tn = selx ? tmx : (sely ? tmy : tmz);
+                const double ds = tn - t;
+                const uint32_t cidx = cpx + cpy + cpz;
+                const uint2 cw = __ldg(P.cellw + cidx);
+                rho_c = (double)__uint_as_float(cw.x);
+                cwy = cw.y;
+                sj = (int)(cw.y & 0xffu) * nf + j;
+                kk = s_kext[sj] * rho_c;          // (kabs+ksca) h rho  (Eq. 2 per unit path)
+                const double dtau = kk * ds;      // tau_i of PAPER.md:49
+                if (dtau > tau) {
+                    state = ST_INTERACT;          // interaction inside this cell (equality leaves, Q5)
+                } else {
+                    tau -= dtau;
+                    if (rho_c > 0.0) {
+                        // S5 Lucy path-length tally, 64-bit fixed point (Eq. 9, linear form)
+                        const double x = s_kabsfx[sj] * rho_c * ds;
+                        atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx),
+                                  (unsigned long long)__double2ll_rn(x));
+                        ndusty++;
+                    }
+                    t = tn;
+                    ncross++;
+                    bool out;
+                    if (selx) { ix += stx; tmx += tdx; cpx = bx_part(ix); out = (unsigned)ix >= (unsigned)P.nx; }
+                    else if (sely) { iy += sty; tmy += tdy; cpy = by_part(iy, P.sby); out = (unsigned)iy >= (unsigned)P.ny; }
+                    else { iz += stz; tmz += tdz; cpz = bz_part(iz, P.sbz); out = (unsigned)iz >= (unsigned)P.nz; }
+                    if (out) {
+                        // S10 escape tally: frequency x |cos i| bin, block-private histogram
+                        const double amu = fabs(uz);
+                        int bin = 0;
+                        for (int b = 1; b < P.ndir; ++b) if (s_mu[b] <= amu) bin = b;
+                        atomicAdd(&s_hist[bin * nf + j], 1u);
+                        const bool direct = (nsca + nabs) == 0u;
+                        if (direct) atomicAdd(&s_hist[P.ndir * nf + bin * nf + j], 1u);
+                        atomicAdd(&s_cnt[CNT_PACKETS], 1ull);
+                        atomicAdd(&s_cnt[CNT_CROSS], (unsigned long long)ncross);
+                        atomicAdd(&s_cnt[CNT_DUSTY], (unsigned long long)ndusty);
+                        atomicAdd(&s_cnt[CNT_SCA], (unsigned long long)nsca);
+                        atomicAdd(&s_cnt[CNT_ABS], (unsigned long long)nabs);
+                        if (direct) atomicAdd(&s_cnt[CNT_DIRECT], 1ull);
+                        if (RECORD) {
+                            hash_mix(hash, event_word(EV_ESCAPE, j, (unsigned long long)bin));
+                            hash_mix(hash, (unsigned long long)ncross);
+                            hash_mix(hash, (unsigned long long)nsca | ((unsigned long long)nabs << 32));
+                            mcrt_digest dg;
+                            dg.hash = hash; dg.crossings = ncross; dg.scatterings = nsca; dg.absorptions = nabs;
+                            dg.escape_bin = (uint32_t)bin;
+                            P.dig[pid] = dg;  // packet ids of a run start at 0
+                        }
+                        state = ST_IDLE;
+                    }
+                }
+            }
+        }
+    }
+
+    // flush the block-private histogram and counters
+    __syncthreads();
+    const int half = P.ndir * nf;
+    for (int i = threadIdx.x; i < nhist; i += blockDim.x) {
+        const unsigned int v = s_hist[i];
+        if (v) atomicAdd(i < half ? &P.sed[i] : &P.sed_direct[i - half], (unsigned long long)v);
+    }
+    if (threadIdx.x < CNT_NEXT && threadIdx.x != CNT_OVERFLOW) {
+        const unsigned long long v = s_cnt[threadIdx.x];
+        if (v) atomicAdd(&P.counters[threadIdx.x], v);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// S11 epoch temperature-index update (streaming over cells, between transport launches).
+//   k~ = k + max(1, 1/2 (k - k_prev) B_e/B_{e-1});  x = k~ xi / (4 pi rho h^3) (Eq. 4);
+//   tidx = #{ J[s][.] < x } clamped to [0, nT-1];  k_prev = k.   Also checks the fixed-point range.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int t_index(const double *J, int nT, double x)
+{
+    int lo = 0, hi = nT;
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (J[mid] < x) lo = mid + 1; else hi = mid;
+    }
+    return lo > nT - 1 ? nT - 1 : lo;
+}
+
+__global__ void __launch_bounds__(256) k_epoch_update(uint2 *__restrict__ cellw, const unsigned long long *__restrict__ kcnt,
+                                                      unsigned long long *__restrict__ kprev,
+                                                      const long long *__restrict__ lfx, const double *__restrict__ J,
+                                                      int nT, int ns, size_t ncp, int first_epoch, double ratio,
+                                                      double cellfac, unsigned long long *__restrict__ counters)
+{
+    extern __shared__ double s_J[];
+    for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
+    bool ovf = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
+        uint2 cw = cellw[i];
+        const double rho_c = (double)__uint_as_float(cw.x);
+        const unsigned long long kc = kcnt[i];
+        uint32_t m = 0u;
+        if (rho_c > 0.0) {
+            double kt;
+            if (first_epoch) kt = (double)kc + 1.0;
+            else {
+                const double pred = 0.5 * (double)(kc - kprev[i]) * ratio;
+                kt = (double)kc + ((pred > 1.0) ? pred : 1.0);
+            }
+            const double x = kt * cellfac / rho_c;
+            m = (uint32_t)t_index(s_J + (cw.y & 0xffu) * nT, nT, x);
+            const long long v = lfx[i];
+            ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
+        }
+        kprev[i] = kc;
+        const uint32_t ny_ = (cw.y & 0xffffu) | (m << 16);
+        if (ny_ != cw.y) cellw[i].y = ny_;
+    }
+    if (ovf) counters[CNT_OVERFLOW] = 1ull;
+}
+
+// S12 temperature index for a frozen-T sweep from the previous pass's tallies; zeroes them.
+__global__ void __launch_bounds__(256) k_sweep_update(uint2 *__restrict__ cellw, unsigned long long *__restrict__ kcnt,
+                                                      unsigned long long *__restrict__ kprev, long long *__restrict__ lfx,
+                                                      const double *__restrict__ J, int nT, int ns, size_t ncp,
+                                                      int from_lucy, double inv_fx, double cellfac,
+                                                      unsigned long long *__restrict__ counters)
+{
+    extern __shared__ double s_J[];
+    for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
+        uint2 cw = cellw[i];
+        const double rho_c = (double)__uint_as_float(cw.x);
+        uint32_t m = 0u;
+        if (rho_c > 0.0) {
+            const double e = from_lucy ? (double)lfx[i] * inv_fx : (double)kcnt[i];
+            const double x = e * cellfac / rho_c;
+            m = (uint32_t)t_index(s_J + (cw.y & 0xffu) * nT, nT, x);
+        }
+        cellw[i].y = (cw.y & 0xffffu) | (m << 16);
+        kcnt[i] = 0ull;
+        kprev[i] = 0ull;
+        lfx[i] = 0ll;
+    }
+}
+
+// range check of the fixed-point tallies after the last epoch (|L| <= 2^62, O9)
+__global__ void __launch_bounds__(256) k_range_check(const long long *__restrict__ lfx, size_t ncp,
+                                                     unsigned long long *__restrict__ counters)
+{
+    bool ovf = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
+        const long long v = lfx[i];
+        ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
+    }
+    if (ovf) counters[CNT_OVERFLOW] = 1ull;
+}
+
+// ------------------------------------------------------------------------------------------------
+// layout kernels: canonical [nz][ny][nx] <-> brick-major
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ size_t brick_index(int ix, int iy, int iz, int nbx, int nby)
+{
+    return ((size_t)((iz >> 2) * nby + (iy >> 2)) * nbx + (ix >> 2)) * kBrickCells + ((iz & 3) << 4) + ((iy & 3) << 2) + (ix & 3);
+}
+
+__global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__restrict__ sp, uint2 *__restrict__ cellw,
+                            int nx, int ny, int nz, int nbx, int nby, int nbz, int ns, unsigned long long *__restrict__ bad)
+{
+    const size_t ncp = (size_t)nbx * nby * nbz * kBrickCells;
+    for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < ncp; b += (size_t)gridDim.x * blockDim.x) {
+        const size_t brick = b >> 6;
+        const int l = (int)(b & 63);
+        const int bxi = (int)(brick % nbx), byi = (int)((brick / nbx) % nby), bzi = (int)(brick / ((size_t)nbx * nby));
+        const int ix = bxi * 4 + (l & 3), iy = byi * 4 + ((l >> 2) & 3), iz = bzi * 4 + (l >> 4);
+        uint2 cw = make_uint2(0u, 0u);
+        if (ix < nx && iy < ny && iz < nz) {
+            const size_t i = ((size_t)iz * ny + iy) * nx + ix;
+            const float r = rho[i];
+            const uint32_t s = sp[i];
+            if (!(r >= 0.0f) || isinf(r)) atomicAdd(&bad[0], 1ull);
+            if (s >= (uint32_t)ns) atomicAdd(&bad[1], 1ull);
+            cw.x = __float_as_uint(r);
+            cw.y = s;
+        }
+        cellw[b] = cw;
+    }
+}
+
+enum : int { G_K = 0, G_LFX = 1, G_TIDX = 2, G_ECOUNT = 3, G_ELUCY = 4, G_TCOUNT = 5, G_TLUCY = 6 };
+
+__device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int nT, double x)
+{
+    if (!(x > 0.0)) return 0.0;
+    if (x <= J[0]) return Tg[0];
+    if (x >= J[nT - 1]) return Tg[nT - 1];
+    int lo = 0, hi = nT - 1;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (J[mid] <= x) lo = mid; else hi = mid;
+    }
+    const double f = log(x / J[lo]) / log(J[hi] / J[lo]);
+    return Tg[lo] * exp(f * log(Tg[hi] / Tg[lo]));
+}
+
+// gathers one output array in canonical order (O12: E_count = k xi, E_lucy = xi L / 2^FX, T by inverting Eq. 4)
+__global__ void k_gather(int what, void *__restrict__ out, const uint2 *__restrict__ cellw,
+                         const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
+                         const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
+                         int nbx, int nby, double xi, double inv_fx, double cellfac)
+{
+    const size_t nc = (size_t)nx * ny * nz;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
+        const size_t b = brick_index(ix, iy, iz, nbx, nby);
+        switch (what) {
+        case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
+        case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[b]; break;
+        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)(cellw[b].y >> 16); break;
+        case G_ECOUNT: reinterpret_cast<double *>(out)[i] = (double)kcnt[b] * xi; break;
+        case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[b] * inv_fx * xi; break;
+        default: {
+            const uint2 cw = cellw[b];
+            const double rho_c = (double)__uint_as_float(cw.x);
+            float T = 0.0f;
+            if (rho_c > 0.0) {
+                const double e = (what == G_TLUCY) ? (double)lfx[b] * inv_fx : (double)kcnt[b];
+                T = (float)T_of_x(J + (cw.y & 0xffu) * nT, Tg, nT, e * cellfac / rho_c);
+            }
+            reinterpret_cast<float *>(out)[i] = T;
+        }
+        }
+    }
+}
+
+// SED = counts xi / (dnu_j dOmega_bin), dOmega = 4 pi d|mu| (reading Q22)
+__global__ void k_sed(double *__restrict__ out, const unsigned long long *__restrict__ sed, const double *__restrict__ dnu,
+                      const double *__restrict__ mu, int ndir, int nf, double xi)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < ndir * nf) {
+        const int b = i / nf, j = i % nf;
+        const double dom = kFourPi * (mu[b + 1] - mu[b]);
+        out[i] = (double)sed[i] * xi / (dnu[j] * dom);
+    }
+}
+
+__global__ void k_philox_test(const uint32_t *__restrict__ ctr, const uint32_t *__restrict__ key, uint32_t *__restrict__ out,
+                              unsigned long long n)
+{
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        uint32_t o0, o1, o2, o3;
+        philox4x32_10(ctr[4 * i], ctr[4 * i + 1], ctr[4 * i + 2], ctr[4 * i + 3], key[2 * i], key[2 * i + 1], o0, o1, o2, o3);
+        out[4 * i] = o0; out[4 * i + 1] = o1; out[4 * i + 2] = o2; out[4 * i + 3] = o3;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// host-side tables (O1) -- small, built once per context
+// ------------------------------------------------------------------------------------------------
+double planck_nu(double nu, double T)
+{
+    const double x = kPlanckH * nu / (kBoltzK * T);
+    return 2.0 * kPlanckH * nu * nu * nu / (kLightC * kLightC) / expm1(x);
+}
+
+double dplanck_nu_dT(double nu, double T)
+{
+    const double x = kPlanckH * nu / (kBoltzK * T);
+    const double em = exp(-x);
+    const double om = -expm1(-x);
+    return 2.0 * kPlanckH * kPlanckH * nu * nu * nu * nu / (kLightC * kLightC * kBoltzK * T * T) * em / (om * om);
+}
+
+double make_cdf(const std::vector<double> &w, double *cdf)
+{
+    const size_t n = w.size();
+    double tot = 0.0;
+    for (size_t i = 0; i < n; ++i) tot += w[i];
+    double acc = 0.0;
+    for (size_t i = 0; i < n; ++i) {
+        acc += w[i];
+        cdf[i] = tot > 0.0 ? acc / tot : 0.0;
+    }
+    cdf[n - 1] = 1.0;
+    return tot;
+}
+
+int fx_bits_for(uint64_t n)
+{
+    int cl = 0;
+    while (((uint64_t)1 << cl) < n && cl < 63) ++cl;
+    int fx = 58 - cl;
+    if (fx > 40) fx = 40;
+    if (fx < 0) fx = 0;
+    return fx;
+}
+
+size_t transport_smem_bytes(int ns, int nf, int ndir)
+{
+    return (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) + 8 * sizeof(unsigned long long) +
+           (size_t)2 * ndir * nf * sizeof(unsigned int);
+}
+
+int stream_grid(size_t n)
+{
+    size_t b = (n + 255) / 256;
+    if (b > 148 * 16) b = 148 * 16;
+    if (b < 1) b = 1;
+    return (int)b;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------
+// C ABI
+// ------------------------------------------------------------------------------------------------
+extern "C" {
+
+const char *mcrt_version(void) { return MCRT_VERSION_STRING; }
+
+const char *mcrt_last_error(const mcrt_ctx *ctx) { return ctx ? ctx->err.c_str() : g_create_error.c_str(); }
+
+void mcrt_default_opts(mcrt_run_opts *o)
+{
+    if (!o) return;
+    memset(o, 0, sizeof(*o));
+    o->mode = MCRT_MODE_BW_EPOCH;
+    o->sweep_T_from_lucy = 1;
+    o->reset_tallies = 1;
+}
+
+int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_T, int n_dir, uint64_t n_digests,
+                         size_t *bytes_out)
+{
+    if (!bytes_out || nx < 1 || ny < 1 || nz < 1 || n_species < 1 || n_nu < 2 || n_T < 2 || n_dir < 1) return MCRT_EINVAL;
+    const size_t nc = (size_t)nx * ny * nz;
+    const size_t ncp = (size_t)((nx + 3) / 4) * ((ny + 3) / 4) * ((nz + 3) / 4) * kBrickCells;
+    size_t b = 0;
+    auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
+    add(ncp * sizeof(uint2));            // cell words
+    add(ncp * sizeof(long long));        // Lucy tally
+    add(ncp * sizeof(long long));        // k
+    add(ncp * sizeof(long long));        // k_prev
+    add(nc * 8);                         // scratch (staging of inputs / outputs)
+    add(CNT_N * 8 + 64);                 // counters (+ validation flags)
+    const size_t nsf = (size_t)n_species * n_nu;
+    for (int i = 0; i < 4; ++i) add(nsf * 8);
+    add((size_t)n_nu * 8); add((size_t)n_nu * 8);            // srccdf, dnu
+    add((size_t)n_species * n_T * 8); add((size_t)n_T * 8);  // J, Tg
+    add(nsf * n_T * 8); add(nsf * n_T * 8);                  // cdf_B, cdf_dB
+    add((size_t)(n_dir + 1) * 8);
+    add((size_t)n_dir * n_nu * 8); add((size_t)n_dir * n_nu * 8);
+    add((size_t)n_dir * n_nu * 8);                           // SED staging
+    if (n_digests) add(n_digests * sizeof(mcrt_digest));
+    *bytes_out = b + 4096;
+    return MCRT_OK;
+}
+
+int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm, const float *rho, const uint8_t *species,
+                     int n_species, mcrt_mem where, void *workspace, size_t workspace_bytes)
+{
+    if (!out) return fail(nullptr, MCRT_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be >= 1");
+    if ((size_t)nx * ny * nz > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
+    if (!(cell_size_cm > 0.0) || !isfinite(cell_size_cm)) return fail(nullptr, MCRT_EINVAL, "cell_size_cm must be > 0");
+    if (!rho || !species) return fail(nullptr, MCRT_EINVAL, "rho / species is NULL");
+    if (n_species < 1 || n_species > 255) return fail(nullptr, MCRT_EINVAL, "n_species must be in 1..255");
+    if (workspace && ((uintptr_t)workspace & 255u)) return fail(nullptr, MCRT_EINVAL, "workspace must be 256-byte aligned");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+        return fail(nullptr, MCRT_ECUDA, "no CUDA device: this library has no CPU fallback");
+    mcrt_ctx *c = new mcrt_ctx();
+    cudaGetDevice(&c->device);
+    c->nx = nx; c->ny = ny; c->nz = nz; c->ns = n_species; c->h = cell_size_cm;
+    c->nbx = (nx + 3) / 4; c->nby = (ny + 3) / 4; c->nbz = (nz + 3) / 4;
+    c->nc = (size_t)nx * ny * nz;
+    c->ncp = (size_t)c->nbx * c->nby * c->nbz * kBrickCells;
+    c->ws = (char *)workspace; c->ws_bytes = workspace_bytes; c->ws_owned_by_caller = workspace != nullptr;
+    int rc;
+#define GC_TRY(expr)                                                       \
+    do {                                                                   \
+        rc = (expr);                                                       \
+        if (rc != MCRT_OK) { g_create_error = c->err; mcrt_destroy(c); return rc; } \
+    } while (0)
+#define GC_CUDA(expr)                                                                                  \
+    do {                                                                                               \
+        cudaError_t e__ = (expr);                                                                      \
+        if (e__ != cudaSuccess) {                                                                      \
+            g_create_error = std::string(#expr) + ": " + cudaGetErrorString(e__);                      \
+            mcrt_destroy(c);                                                                           \
+            return MCRT_ECUDA;                                                                         \
+        }                                                                                              \
+    } while (0)
+    GC_TRY(ws_alloc(c, (void **)&c->cellw, c->ncp * sizeof(uint2)));
+    GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
+    GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
+    GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
+    GC_TRY(ws_alloc(c, (void **)&c->scratch, c->nc * 8));
+    GC_TRY(ws_alloc(c, (void **)&c->counters, CNT_N * 8 + 64));
+    GC_CUDA(cudaMemsetAsync(c->counters, 0, CNT_N * 8 + 64, c->stream));
+    const float *d_rho = rho;
+    const uint8_t *d_sp = species;
+    if (where == MCRT_HOST) {
+        float *sr = (float *)c->scratch;
+        uint8_t *ss = (uint8_t *)c->scratch + c->nc * 4;
+        GC_CUDA(cudaMemcpyAsync(sr, rho, c->nc * 4, cudaMemcpyHostToDevice, c->stream));
+        GC_CUDA(cudaMemcpyAsync(ss, species, c->nc, cudaMemcpyHostToDevice, c->stream));
+        d_rho = sr; d_sp = ss;
+    }
+    unsigned long long *bad = c->counters + CNT_N;
+    k_pack_grid<<<stream_grid(c->ncp), 256, 0, c->stream>>>(d_rho, d_sp, c->cellw, nx, ny, nz, c->nbx, c->nby, c->nbz,
+                                                           n_species, bad);
+    GC_CUDA(cudaGetLastError());
+    GC_CUDA(cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
+    GC_CUDA(cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
+    GC_CUDA(cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
+    unsigned long long hbad[2] = {0, 0};
+    GC_CUDA(cudaMemcpyAsync(hbad, bad, 16, cudaMemcpyDeviceToHost, c->stream));
+    GC_CUDA(cudaStreamSynchronize(c->stream));
+    if (hbad[0] || hbad[1]) {
+        g_create_error = hbad[0] ? "rho holds negative, NaN or infinite values" : "species index >= n_species";
+        mcrt_destroy(c);
+        return MCRT_EINVAL;
+    }
+#undef GC_TRY
+#undef GC_CUDA
+    *out = c;
+    return MCRT_OK;
+}
+
+int mcrt_set_stream(mcrt_ctx *c, void *cuda_stream)
+{
+    if (!c) return MCRT_EINVAL;
+    c->stream = (cudaStream_t)cuda_stream;
+    return MCRT_OK;
+}
+
+int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *kappa_abs, const double *kappa_sca,
+                     const double *g, int n_T, const double *T_grid)
+{
+    if (!c) return MCRT_EINVAL;
+    if (c->have_tables) return fail(c, MCRT_ESTATE, "mcrt_dust_tables may be called once per context");
+    if (!nu_hz || !kappa_abs || !kappa_sca || !g || !T_grid) return fail(c, MCRT_EINVAL, "NULL table pointer");
+    if (n_nu < 2 || n_nu > 65535 || n_T < 2 || n_T > 65535) return fail(c, MCRT_EINVAL, "n_nu and n_T must be in 2..65535");
+    for (int j = 0; j < n_nu; ++j) {
+        if (!(nu_hz[j] > 0.0) || !isfinite(nu_hz[j]) || (j && !(nu_hz[j] > nu_hz[j - 1])))
+            return fail(c, MCRT_EINVAL, "nu_hz must be positive and strictly ascending");
+    }
+    for (int m = 0; m < n_T; ++m)
+        if (!(T_grid[m] > 0.0) || !isfinite(T_grid[m]) || (m && !(T_grid[m] > T_grid[m - 1])))
+            return fail(c, MCRT_EINVAL, "T_grid must be positive and strictly ascending");
+    const int ns = c->ns;
+    const size_t nsf = (size_t)ns * n_nu;
+    for (size_t i = 0; i < nsf; ++i) {
+        if (!(kappa_abs[i] >= 0.0) || !(kappa_sca[i] >= 0.0) || !isfinite(kappa_abs[i]) || !isfinite(kappa_sca[i]))
+            return fail(c, MCRT_EINVAL, "kappa must be finite and >= 0");
+        if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
+        if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
+    }
+    if (transport_smem_bytes(ns, n_nu, 16) > 200 * 1024)
+        return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
+    c->nf = n_nu; c->nT = n_T;
+    c->nu.assign(nu_hz, nu_hz + n_nu);
+    c->kabs.assign(kappa_abs, kappa_abs + nsf);
+    c->ksca.assign(kappa_sca, kappa_sca + nsf);
+    c->g.assign(g, g + nsf);
+    c->Tg.assign(T_grid, T_grid + n_T);
+    // bin widths: edges at the geometric means of neighbours, end bins extrapolated with the neighbouring ratio
+    c->dnu.resize(n_nu);
+    {
+        std::vector<double> edge(n_nu + 1);
+        for (int j = 1; j < n_nu; ++j) edge[j] = sqrt(c->nu[j - 1] * c->nu[j]);
+        edge[0] = c->nu[0] * sqrt(c->nu[0] / c->nu[1]);
+        edge[n_nu] = c->nu[n_nu - 1] * sqrt(c->nu[n_nu - 1] / c->nu[n_nu - 2]);
+        for (int j = 0; j < n_nu; ++j) c->dnu[j] = edge[j + 1] - edge[j];
+    }
+    c->kext_h.resize(nsf); c->kabs_h.resize(nsf); c->albedo.resize(nsf);
+    for (size_t i = 0; i < nsf; ++i) {
+        const double kext = c->kabs[i] + c->ksca[i];
+        c->kext_h[i] = kext * c->h;        // optical depth per unit density per cell length (Eq. 2)
+        c->kabs_h[i] = c->kabs[i] * c->h;
+        c->albedo[i] = c->ksca[i] / kext;
+    }
+    c->J.resize((size_t)ns * n_T);
+    c->cdfB.resize(nsf * n_T);
+    c->cdfdB.resize(nsf * n_T);
+    std::vector<double> w(n_nu);
+    for (int s = 0; s < ns; ++s)
+        for (int m = 0; m < n_T; ++m) {
+            const size_t row = ((size_t)s * n_T + m) * n_nu;
+            for (int j = 0; j < n_nu; ++j) w[j] = c->kabs[(size_t)s * n_nu + j] * planck_nu(c->nu[j], c->Tg[m]) * c->dnu[j];
+            c->J[(size_t)s * n_T + m] = make_cdf(w, &c->cdfB[row]);      // Eq. 4 left side, Eq. 5
+            for (int j = 0; j < n_nu; ++j) w[j] = c->kabs[(size_t)s * n_nu + j] * dplanck_nu_dT(c->nu[j], c->Tg[m]) * c->dnu[j];
+            make_cdf(w, &c->cdfdB[row]);                                  // Eq. 10
+        }
+    int rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_kext_h, nsf * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_kabs_fx, nsf * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_albedo, nsf * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_g, nsf * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_srccdf, (size_t)n_nu * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_dnu, (size_t)n_nu * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_J, (size_t)ns * n_T * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_Tg, (size_t)n_T * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_cdfB, nsf * n_T * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_cdfdB, nsf * n_T * 8))) return rc;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_kext_h, c->kext_h.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_albedo, c->albedo.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_g, c->g.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_dnu, c->dnu.data(), (size_t)n_nu * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_J, c->J.data(), (size_t)ns * n_T * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_Tg, c->Tg.data(), (size_t)n_T * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_cdfB, c->cdfB.data(), nsf * n_T * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_cdfdB, c->cdfdB.data(), nsf * n_T * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_tables = true;
+    return MCRT_OK;
+}
+
+int mcrt_source(mcrt_ctx *c, double L_erg_s, double T_star_K, const double *L_nu_weights, const double pos_cm[3])
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->have_tables) return fail(c, MCRT_ESTATE, "call mcrt_dust_tables before mcrt_source");
+    if (!(L_erg_s > 0.0) || !isfinite(L_erg_s)) return fail(c, MCRT_EINVAL, "L_erg_s must be > 0");
+    if (!pos_cm) return fail(c, MCRT_EINVAL, "pos_cm is NULL");
+    const int n[3] = {c->nx, c->ny, c->nz};
+    for (int a = 0; a < 3; ++a) {
+        const double p = pos_cm[a] / c->h;
+        if (!(p > 0.0) || !(p < (double)n[a])) return fail(c, MCRT_EINVAL, "source position must be strictly inside the grid");
+        c->pos[a] = p;
+    }
+    std::vector<double> w(c->nf);
+    if (T_star_K > 0.0) {
+        for (int j = 0; j < c->nf; ++j) w[j] = planck_nu(c->nu[j], T_star_K) * c->dnu[j];
+    } else {
+        if (!L_nu_weights) return fail(c, MCRT_EINVAL, "T_star_K <= 0 needs L_nu_weights");
+        double tot = 0.0;
+        for (int j = 0; j < c->nf; ++j) {
+            if (!(L_nu_weights[j] >= 0.0) || !isfinite(L_nu_weights[j])) return fail(c, MCRT_EINVAL, "L_nu_weights must be finite and >= 0");
+            w[j] = L_nu_weights[j] * c->dnu[j];
+            tot += w[j];
+        }
+        if (!(tot > 0.0)) return fail(c, MCRT_EINVAL, "L_nu_weights are all zero");
+    }
+    c->srccdf.resize(c->nf);
+    make_cdf(w, c->srccdf.data());
+    c->L = L_erg_s;
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_srccdf, c->srccdf.data(), (size_t)c->nf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    c->have_source = true;
+    return MCRT_OK;
+}
+
+int mcrt_escape_bins(mcrt_ctx *c, int n_dir, const double *abs_mu_edges)
+{
+    if (!c) return MCRT_EINVAL;
+    if (n_dir < 1 || n_dir > 4096 || !abs_mu_edges) return fail(c, MCRT_EINVAL, "n_dir must be in 1..4096");
+    if (abs_mu_edges[0] != 0.0 || abs_mu_edges[n_dir] != 1.0) return fail(c, MCRT_EINVAL, "abs_mu_edges must run from 0 to 1");
+    for (int b = 0; b < n_dir; ++b)
+        if (!(abs_mu_edges[b + 1] > abs_mu_edges[b])) return fail(c, MCRT_EINVAL, "abs_mu_edges must be strictly ascending");
+    c->ndir = n_dir;
+    c->mu_edges.assign(abs_mu_edges, abs_mu_edges + n_dir + 1);
+    c->mu_dirty = true;
+    return MCRT_OK;
+}
+
+static int ensure_histograms(mcrt_ctx *c)
+{
+    if (c->mu_edges.empty()) { c->mu_edges = {0.0, 1.0}; c->ndir = 1; c->mu_dirty = true; }
+    if (!c->mu_dirty) return MCRT_OK;
+    int rc;
+    if (c->ndir > c->ndir_alloc) {
+        if ((rc = ws_alloc(c, (void **)&c->d_mu, (size_t)(c->ndir + 1) * 8))) return rc;
+        if ((rc = ws_alloc(c, (void **)&c->sed, (size_t)c->ndir * c->nf * 8))) return rc;
+        if ((rc = ws_alloc(c, (void **)&c->sed_direct, (size_t)c->ndir * c->nf * 8))) return rc;
+        c->ndir_alloc = c->ndir;
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_mu, c->mu_edges.data(), (size_t)(c->ndir + 1) * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, (size_t)c->ndir * c->nf * 8, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, (size_t)c->ndir * c->nf * 8, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));  // mu_edges.data() must outlive the copy
+    c->mu_dirty = false;
+    return MCRT_OK;
+}
+
+static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem)
+{
+    *threads = (o && o->block_threads > 0) ? o->block_threads : 256;
+    if (*threads % 32 || *threads > 256 || *threads < 32) return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32..256");
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir);
+    if (*smem > 48 * 1024) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_transport<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
+        CUDA_TRY(c, cudaFuncSetAttribute(k_transport<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
+    }
+    int nsm = 148, occ = 1;
+    CUDA_TRY(c, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device));
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport<false>, *threads, *smem));
+    if (occ < 1) return fail(c, MCRT_EINVAL, "transport kernel does not fit on an SM with these table sizes");
+    c->occ_blocks = occ;
+    *blocks = (o && o->grid_blocks > 0) ? o->grid_blocks : nsm * occ;  // persistent: every CTA resident
+    return MCRT_OK;
+}
+
+int mcrt_launch_config(mcrt_ctx *c, int *grid_blocks, int *block_threads, size_t *smem_bytes)
+{
+    if (!c || !c->have_tables) return c ? fail(c, MCRT_ESTATE, "tables not set") : MCRT_EINVAL;
+    int rc = ensure_histograms(c);
+    if (rc) return rc;
+    int b, t; size_t s;
+    if ((rc = transport_config(c, nullptr, &b, &t, &s))) return rc;
+    if (grid_blocks) *grid_blocks = b;
+    if (block_threads) *block_threads = t;
+    if (smem_bytes) *smem_bytes = s;
+    return MCRT_OK;
+}
+
+static int fill_stats(mcrt_ctx *c, mcrt_run_stats *st)
+{
+    unsigned long long h[CNT_N];
+    CUDA_TRY(c, cudaMemcpyAsync(h, c->counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    fold_timing(c);
+    memset(st, 0, sizeof(*st));
+    st->transport_ms = c->transport_ms; st->update_ms = c->update_ms;
+    st->packets = h[CNT_PACKETS]; st->crossings = h[CNT_CROSS]; st->dusty_crossings = h[CNT_DUSTY];
+    st->scatterings = h[CNT_SCA]; st->absorptions = h[CNT_ABS]; st->direct_escapes = h[CNT_DIRECT];
+    st->escapes = h[CNT_PACKETS];
+    st->flights = h[CNT_PACKETS] + h[CNT_SCA] + h[CNT_ABS];
+    st->lucy_adds = h[CNT_DUSTY] + h[CNT_SCA] + h[CNT_ABS];
+    st->epochs = c->epochs; st->gpu_launches = c->launches;
+    st->fx_bits = c->fx; st->overflow = h[CNT_OVERFLOW] ? 1 : 0;
+    return MCRT_OK;
+}
+
+int mcrt_get_stats(mcrt_ctx *c, mcrt_run_stats *st)
+{
+    if (!c || !st) return MCRT_EINVAL;
+    int rc = fill_stats(c, st);
+    if (rc) return rc;
+    return st->overflow ? fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62") : MCRT_OK;
+}
+
+int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts, mcrt_run_stats *stats_out)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->have_tables || !c->have_source) return fail(c, MCRT_ESTATE, "call mcrt_dust_tables and mcrt_source before mcrt_run");
+    if (n_packets < 1) return fail(c, MCRT_EINVAL, "n_packets must be >= 1");
+    mcrt_run_opts o;
+    if (opts) o = *opts; else mcrt_default_opts(&o);
+    if (o.mode != MCRT_MODE_BW_EPOCH && o.mode != MCRT_MODE_FROZEN_T_SWEEP) return fail(c, MCRT_EINVAL, "unknown mode");
+    if (o.mode == MCRT_MODE_FROZEN_T_SWEEP && o.n_sweeps < 1) return fail(c, MCRT_EINVAL, "n_sweeps must be >= 1");
+    int rc = ensure_histograms(c);
+    if (rc) return rc;
+    int blocks, threads; size_t smem;
+    if ((rc = transport_config(c, &o, &blocks, &threads, &smem))) return rc;
+    const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
+
+    if (o.record_digests) {
+        if (c->dig_cap < n_packets) {
+            if ((rc = ws_alloc(c, (void **)&c->dig, n_packets * sizeof(mcrt_digest)))) return rc;
+            c->dig_cap = n_packets;
+        }
+        c->dig_n = n_packets;
+    } else c->dig_n = 0;
+
+    if (o.reset_tallies && o.mode == MCRT_MODE_BW_EPOCH) {
+        CUDA_TRY(c, cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_N * 8, c->stream));
+        c->epochs = 0; c->launches = 0;
+        if (c->ev_used) { cudaStreamSynchronize(c->stream); fold_timing(c); }
+        c->transport_ms = 0.0; c->update_ms = 0.0;
+    }
+    const bool timing = o.time_kernels != 0;
+    const int prev_fx = c->fx;
+    c->fx = fx_bits_for(n_packets);
+    c->xi = c->L / (double)n_packets;                            // xi = L/N
+    const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);  // xi / (4 pi V) of Eq. 4
+    c->last_n = n_packets;
+    {
+        const size_t nsf = (size_t)c->ns * c->nf;
+        std::vector<double> kfx(nsf);
+        for (size_t i = 0; i < nsf; ++i) kfx[i] = ldexp(c->kabs_h[i], c->fx);
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_kabs_fx, kfx.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+
+    TransportParams P;
+    memset(&P, 0, sizeof(P));
+    P.cellw = c->cellw; P.lfx = c->lfx; P.kcnt = c->kabs_cnt;
+    P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
+    P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
+    P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
+    P.dig = o.record_digests ? c->dig : nullptr;
+    P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
+    P.sby = (uint32_t)c->nbx * kBrickCells; P.sbz = (uint32_t)c->nbx * c->nby * kBrickCells;
+    P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
+    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
+    const size_t j_smem = (size_t)c->ns * c->nT * 8;
+    if (j_smem > 48 * 1024) {
+        CUDA_TRY(c, cudaFuncSetAttribute(k_epoch_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
+        CUDA_TRY(c, cudaFuncSetAttribute(k_sweep_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
+    }
+    const int ugrid = stream_grid(c->ncp);
+
+    if (o.mode == MCRT_MODE_BW_EPOCH) {
+        uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
+        if (B0 == 0) { B0 = 256; while (B0 * 2 <= n_packets / 256) B0 *= 2; }
+        if (Bmax == 0) Bmax = (uint64_t)1 << 20;
+        if (Bmax < B0) Bmax = B0;
+        P.cdf = c->d_cdfdB;
+        P.pass = o.rng_pass;
+        uint64_t done = 0, Bnom = B0, Bprev = 0;
+        int e = 0;
+        while (done < n_packets) {
+            const uint64_t Be = (n_packets - done < Bnom) ? n_packets - done : Bnom;
+            mark(c, timing);
+            k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns,
+                                                             c->ncp, e == 0, e == 0 ? 1.0 : (double)Be / (double)Bprev,
+                                                             cellfac, c->counters);
+            P.pid0 = done; P.count = Be;
+            mark(c, timing);
+            if (o.record_digests) k_transport<true><<<blocks, threads, smem, c->stream>>>(P);
+            else k_transport<false><<<blocks, threads, smem, c->stream>>>(P);
+            mark(c, timing);
+            c->launches += 2;
+            c->epochs++;
+            done += Be; Bprev = Be;
+            Bnom = (Bnom * 2 > Bmax) ? Bmax : Bnom * 2;
+            ++e;
+        }
+    } else {
+        P.cdf = c->d_cdfB;
+        for (int sw = 1; sw <= o.n_sweeps; ++sw) {
+            // temperatures of the previous pass (its own fixed-point scale), then zero and re-run all N packets
+            mark(c, timing);
+            k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns,
+                                                             c->ncp, o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? prev_fx : c->fx)),
+                                                             cellfac, c->counters);
+            CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
+            P.pass = o.rng_pass + (uint32_t)sw;
+            P.pid0 = 0; P.count = n_packets;
+            mark(c, timing);
+            if (o.record_digests) k_transport<true><<<blocks, threads, smem, c->stream>>>(P);
+            else k_transport<false><<<blocks, threads, smem, c->stream>>>(P);
+            mark(c, timing);
+            c->launches += 2;
+            c->epochs++;
+        }
+    }
+    k_range_check<<<ugrid, 256, 0, c->stream>>>(c->lfx, c->ncp, c->counters);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    if (stats_out) {
+        if ((rc = fill_stats(c, stats_out))) return rc;
+        if (stats_out->overflow) return fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62");
+    }
+    return MCRT_OK;
+}
+
+static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem where)
+{
+    if (!dst) return MCRT_OK;
+    void *dev = (where == MCRT_DEVICE) ? dst : c->scratch;
+    const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
+    k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, c->nT, c->nx,
+                                                       c->ny, c->nz, c->nbx, c->nby, c->xi, ldexp(1.0, -c->fx), cellfac);
+    CUDA_TRY(c, cudaGetLastError());
+    if (where == MCRT_HOST) {
+        CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    return MCRT_OK;
+}
+
+int mcrt_read(mcrt_ctx *c, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy, double *SED, mcrt_mem where)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read before mcrt_run");
+    int rc;
+    if ((rc = gather_out(c, G_ECOUNT, E_abs_count, 8, where))) return rc;
+    if ((rc = gather_out(c, G_ELUCY, E_abs_lucy, 8, where))) return rc;
+    if ((rc = gather_out(c, G_TCOUNT, T_count, 4, where))) return rc;
+    if ((rc = gather_out(c, G_TLUCY, T_lucy, 4, where))) return rc;
+    if (SED) {
+        const int n = c->ndir * c->nf;
+        double *dev = (where == MCRT_DEVICE) ? SED : (double *)c->scratch;
+        k_sed<<<(n + 255) / 256, 256, 0, c->stream>>>(dev, c->sed, c->d_dnu, c->d_mu, c->ndir, c->nf, c->xi);
+        CUDA_TRY(c, cudaGetLastError());
+        if (where == MCRT_HOST) {
+            CUDA_TRY(c, cudaMemcpyAsync(SED, dev, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream));
+        }
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
+int mcrt_read_raw(mcrt_ctx *c, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_counts, uint64_t *sed_direct, uint16_t *tidx,
+                  mcrt_digest *digests, mcrt_mem where)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read_raw before mcrt_run");
+    int rc;
+    if ((rc = gather_out(c, G_K, k_abs, 8, where))) return rc;
+    if ((rc = gather_out(c, G_LFX, lucy_fx, 8, where))) return rc;
+    if ((rc = gather_out(c, G_TIDX, tidx, 2, where))) return rc;
+    const cudaMemcpyKind kind = (where == MCRT_HOST) ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+    const size_t hb = (size_t)c->ndir * c->nf * 8;
+    if (sed_counts) CUDA_TRY(c, cudaMemcpyAsync(sed_counts, c->sed, hb, kind, c->stream));
+    if (sed_direct) CUDA_TRY(c, cudaMemcpyAsync(sed_direct, c->sed_direct, hb, kind, c->stream));
+    if (digests) {
+        if (!c->dig_n) return fail(c, MCRT_ESTATE, "digests were not recorded by the last run");
+        CUDA_TRY(c, cudaMemcpyAsync(digests, c->dig, c->dig_n * sizeof(mcrt_digest), kind, c->stream));
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
+int mcrt_read_tables(mcrt_ctx *c, double *dnu, double *J, double *cdf_B, double *cdf_dB, double *albedo, double *src_cdf)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->have_tables) return fail(c, MCRT_ESTATE, "tables not set");
+    const size_t nsf = (size_t)c->ns * c->nf;
+    // read back from the DEVICE copies: these are the values the kernels use
+    if (dnu) CUDA_TRY(c, cudaMemcpyAsync(dnu, c->d_dnu, (size_t)c->nf * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (J) CUDA_TRY(c, cudaMemcpyAsync(J, c->d_J, (size_t)c->ns * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (cdf_B) CUDA_TRY(c, cudaMemcpyAsync(cdf_B, c->d_cdfB, nsf * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (cdf_dB) CUDA_TRY(c, cudaMemcpyAsync(cdf_dB, c->d_cdfdB, nsf * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (albedo) CUDA_TRY(c, cudaMemcpyAsync(albedo, c->d_albedo, nsf * 8, cudaMemcpyDeviceToHost, c->stream));
+    if (src_cdf) {
+        if (!c->have_source) return fail(c, MCRT_ESTATE, "source not set");
+        CUDA_TRY(c, cudaMemcpyAsync(src_cdf, c->d_srccdf, (size_t)c->nf * 8, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
+int mcrt_philox_device(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n)
+{
+    if (!ctr || !key || !out || n == 0) return MCRT_EINVAL;
+    uint32_t *d = nullptr;
+    if (cudaMalloc(&d, n * 10 * 4) != cudaSuccess) return fail(nullptr, MCRT_ENOMEM, "cudaMalloc failed");
+    uint32_t *dc = d, *dk = d + 4 * n, *dout = d + 6 * n;
+    cudaError_t e = cudaMemcpy(dc, ctr, n * 16, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(dk, key, n * 8, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_philox_test<<<(unsigned)((n + 255) / 256), 256>>>(dc, dk, dout, n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
+    return MCRT_OK;
+}
+
+void mcrt_destroy(mcrt_ctx *c)
+{
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
+    for (void *p : c->owned) cudaFree(p);
+    delete c;
+}
+
+}  // extern "C"

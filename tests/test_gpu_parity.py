@@ -1,0 +1,273 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars:
+  * per-packet event digests equal for >= 99.9 % of packets;
+  * if all digests are equal: absorption counts k, escape histograms, temperature indices BIT-EXACT;
+    otherwise sum|dk| bounded by the absorptions of the differing packets (exact integer bound);
+  * Lucy fixed-point tallies within 1e-6 relative (and a few units of 2^-FX absolute: log/sincos of the two
+    math libraries differ in the last ulp, which moves a rounding boundary now and then);
+  * temperatures within 0.5 %, SED within 1e-6 relative.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1203_2941_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+NTH = min(8, os.cpu_count() or 1)
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1203_2941_b200 import binding
+
+    binding.load_library()  # fails loudly if the extension is missing
+    return binding
+
+
+def _run_both(orc, B, w, N, seed, mode=0, n_sweeps=0, from_lucy=1, B0=0, Bmax=0, grid_blocks=0, block_threads=0):
+    o = orc.Oracle.from_workload(w)
+    c = B.Context(w, n_digests=N)
+    if mode == 1:  # sweeps start from the temperatures of a B&W pass
+        o.run(N, seed, n_threads=NTH)
+        c.run(N, seed)
+    ro = o.run(N, seed, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, B0=B0, Bmax=Bmax, digests=True,
+               n_threads=NTH)
+    rg = c.run(N, seed, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, epoch_B0=B0, epoch_Bmax=Bmax,
+               record_digests=1, grid_blocks=grid_blocks, block_threads=block_threads)
+    return o, c, ro, rg
+
+
+def _assert_parity(o, c, ro, rg, w, N):
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    do, dg = ro["digests"], raw_g["digests"]
+    same = do["hash"] == dg["hash"]
+    frac = same.mean()
+    assert frac >= 0.999, f"only {frac:.6f} of packets have identical event sequences"
+    assert rg["packets"] == N == rg["escapes"] == int(raw_g["sed"].sum())
+    if same.all():
+        assert np.array_equal(do, dg)
+        for key in ("packets", "crossings", "dusty_crossings", "flights", "scatterings", "absorptions", "escapes",
+                    "direct_escapes", "epochs", "lucy_adds", "fx_bits"):
+            assert ro[key] == rg[key], key
+        for key in ("k", "sed", "sed_direct", "tidx"):
+            assert np.array_equal(raw_o[key], raw_g[key]), key
+        lucy_abs_tol = 16
+    else:
+        budget = int(do["absorptions"][~same].sum()) + int(dg["absorptions"][~same].sum())
+        assert int(np.abs(raw_o["k"].astype(np.int64) - raw_g["k"].astype(np.int64)).sum()) <= budget
+        nd = int((~same).sum())
+        assert int(np.abs(raw_o["sed"].astype(np.int64) - raw_g["sed"].astype(np.int64)).sum()) <= 2 * nd
+        lucy_abs_tol = None
+    Lo, Lg = raw_o["lucy_fx"], raw_g["lucy_fx"]
+    assert np.all(Lg[w.rho.reshape(-1) == 0] == 0)
+    if lucy_abs_tol is not None:
+        d = np.abs(Lo - Lg)
+        assert d.max() <= lucy_abs_tol, f"Lucy tallies differ by {d.max()} fixed-point units"
+        assert np.all(d <= 1e-6 * np.abs(Lo) + lucy_abs_tol)
+    assert abs(int(Lo.sum()) - int(Lg.sum())) <= 1e-9 * abs(int(Lo.sum())) + 1000
+    # physical outputs
+    out_g = c.read()
+    out_o, out_ol = o.read(), o.read(T_from_lucy=True)
+    if same.all():
+        np.testing.assert_allclose(out_g["E_count"], out_o["E_count"], rtol=1e-12, atol=0)
+        np.testing.assert_allclose(out_g["E_lucy"], out_o["E_lucy"], rtol=1e-6, atol=out_o["E_lucy"].max() * 1e-12)
+        np.testing.assert_allclose(out_g["SED"], out_o["SED"], rtol=1e-6, atol=0)
+        np.testing.assert_allclose(out_g["T_count"], out_o["T"], rtol=5e-3, atol=0)
+        np.testing.assert_allclose(out_g["T_lucy"], out_ol["T"], rtol=5e-3, atol=0)
+        # far tighter in practice: same integers in, fp64 interpolation on both sides
+        np.testing.assert_allclose(out_g["T_count"], out_o["T"], rtol=1e-6, atol=0)
+    return frac
+
+
+def test_device_philox_known_answers(B):
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "philox4x32_10_kat.txt"))
+            if l.strip() and l[0] != "#"]
+    v = np.array([[int(x, 16) for x in r] for r in rows], dtype=np.uint64).astype(np.uint32)
+    out = B.mcrt_philox_device(v[:, 0:4], v[:, 4:6])
+    assert np.array_equal(out, v[:, 6:10])
+
+
+def test_device_philox_matches_oracle_bulk(B, orc):
+    rng = np.random.default_rng(0)
+    ctr = rng.integers(0, 2 ** 32, (4096, 4), dtype=np.uint64).astype(np.uint32)
+    key = rng.integers(0, 2 ** 32, (4096, 2), dtype=np.uint64).astype(np.uint32)
+    out = B.mcrt_philox_device(ctr, key)
+    for i in range(0, 4096, 64):
+        assert np.array_equal(out[i], orc.philox(ctr[i], key[i]))
+
+
+def test_tables_match_oracle(B, orc):
+    w = W.torus256(n_clumps=50, n=16)
+    o = orc.Oracle.from_workload(w)
+    c = B.Context(w)
+    tg, to = c.tables(), o.tables()
+    for key in tg:
+        np.testing.assert_allclose(tg[key], to[key], rtol=1e-13, atol=1e-300, err_msg=key)
+    c.close()
+
+
+def test_parity_config1_sphere32_full(B, orc):
+    """BASELINE config 1 at its full size: 32^3 sphere, 1e5 packets, seed 1."""
+    w = W.sphere32()
+    o, c, ro, rg = _run_both(orc, B, w, w.n_packets, w.seed)
+    assert _assert_parity(o, c, ro, rg, w, w.n_packets) == 1.0
+    c.close()
+
+
+def test_parity_ragged_grid_offcentre_source_bins(B, orc):
+    """Grid sizes that are not multiples of the 4-cell brick, off-centre source, 4 direction bins."""
+    w = W.uniform_cube(8, 2.0, 0.6, 0.3, n_nu=16, n_dir=4, nxyz=(13, 7, 10), source_offset_cells=(0.3, -0.2, 0.1))
+    o, c, ro, rg = _run_both(orc, B, w, 60000, 3)
+    _assert_parity(o, c, ro, rg, w, 60000)
+    c.close()
+
+
+def test_parity_single_cell_and_thin_slab(B, orc):
+    for nxyz, src in (((1, 1, 1), (0.1, 0.2, -0.3)), ((1, 5, 2), (0.25, 0.0, 0.0)), ((2, 2, 2), (0.0, 0.0, 0.0))):
+        w = W.uniform_cube(2, 1.0, 0.3, -0.4, n_nu=8, n_dir=2, nxyz=nxyz, source_offset_cells=src)
+        o, c, ro, rg = _run_both(orc, B, w, 20000, 9)
+        _assert_parity(o, c, ro, rg, w, 20000)
+        c.close()
+
+
+def test_parity_empty_grid(B, orc):
+    w = W.uniform_cube(6, 0.0, 0.5, 0.0, n_nu=10, n_dir=5, T_star=4000.0)
+    o, c, ro, rg = _run_both(orc, B, w, 50000, 5)
+    _assert_parity(o, c, ro, rg, w, 50000)
+    assert rg["direct_escapes"] == 50000 and rg["absorptions"] == 0
+    c.close()
+
+
+def test_parity_optically_thick_cube(B, orc):
+    """tau = 30 from centre to face: hundreds of interactions per packet, B&W re-emission dominates."""
+    w = W.uniform_cube(12, 30.0, 0.5, 0.6, n_nu=32, slope=-1.0, T_star=3000.0)
+    o, c, ro, rg = _run_both(orc, B, w, 20000, 17)
+    _assert_parity(o, c, ro, rg, w, 20000)
+    assert rg["absorptions"] > 2 * 20000 and rg["scatterings"] > 2 * 20000
+    c.close()
+
+
+@pytest.mark.parametrize("tau_V", [1.0, 100.0])
+def test_parity_config2_shell(B, orc, tau_V):
+    w = W.shell128(tau_V=tau_V, n=64)
+    N = 300_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+def test_parity_config3_disk_two_species(B, orc):
+    w = W.disk256(tau_V=10.0, n=64)
+    N = 300_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+def test_parity_config4_torus_three_species(B, orc):
+    w = W.torus256(n_clumps=400, n=64)
+    N = 300_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+def test_parity_config5_torus_lognormal_then_sweeps(B, orc):
+    """Config 5 shape (lognormal clump tau, 200 wavelengths) at reduced size, then 2 frozen-T sweeps (S12)."""
+    w = W.torus512(n_clumps=300, n=48)
+    N = 100_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed, mode=1, n_sweeps=2, from_lucy=1)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed, mode=1, n_sweeps=1, from_lucy=0)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+def test_parity_custom_epoch_schedule(B, orc):
+    w = W.sphere32(tau_V=4.0, n=16)
+    o, c, ro, rg = _run_both(orc, B, w, 30000, 23, B0=100, Bmax=3000)
+    _assert_parity(o, c, ro, rg, w, 30000)
+    assert rg["epochs"] == ro["epochs"] > 10
+    c.close()
+
+
+def test_determinism_across_launch_configurations(B):
+    """P13: results do not depend on scheduling -- different grid / block sizes, bit-identical tallies and digests."""
+    w = W.torus256(n_clumps=200, n=48)
+    N = 100_000
+    ref = None
+    for blocks, threads in ((0, 0), (7, 64), (148, 128), (1000, 32)):
+        c = B.Context(w, n_digests=N)
+        c.run(N, 11, record_digests=1, grid_blocks=blocks, block_threads=threads)
+        raw = c.read_raw(digests=True)
+        c.close()
+        if ref is None:
+            ref = raw
+        else:
+            for key in ("k", "lucy_fx", "sed", "sed_direct", "tidx", "digests"):
+                assert np.array_equal(ref[key], raw[key]), (key, blocks, threads)
+
+
+def test_device_resident_inputs_and_outputs(B):
+    """MCRT_DEVICE path: inputs read from device tensors, outputs written to device tensors."""
+    import torch
+
+    w = W.sphere32(n=16)
+    c_h = B.Context(w)
+    c_h.run(20000, 2)
+    ref = c_h.read()
+    c_d = B.Context(w, inputs_on_device=True)
+    c_d.run(20000, 2)
+    Ec = torch.zeros(c_d.nc, dtype=torch.float64, device="cuda")
+    Tl = torch.zeros(c_d.nc, dtype=torch.float32, device="cuda")
+    sed = torch.zeros(c_d.ndir * c_d.nf, dtype=torch.float64, device="cuda")
+    B.mcrt_read(c_d.ctx, E_abs_count=Ec, T_lucy=Tl, SED=sed, where=B.MCRT_DEVICE)
+    torch.cuda.synchronize()
+    assert np.array_equal(Ec.cpu().numpy(), ref["E_count"])
+    assert np.array_equal(Tl.cpu().numpy(), ref["T_lucy"])
+    assert np.array_equal(sed.cpu().numpy().reshape(ref["SED"].shape), ref["SED"])
+    c_h.close(); c_d.close()
+
+
+def test_error_paths(B):
+    w = W.sphere32(n=8)
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_grid_create(0, 8, 8, 1.0, np.zeros(1, np.float32), np.zeros(1, np.uint8), 1)
+    assert e.value.code == B.MCRT_EINVAL
+    bad = w.rho.copy(); bad[0, 0, 0] = -1.0
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_grid_create(8, 8, 8, 1.0, bad, w.species, 1)
+    assert e.value.code == B.MCRT_EINVAL
+    sp = w.species.copy(); sp[1, 2, 3] = 4
+    with pytest.raises(B.McrtError):
+        B.mcrt_grid_create(8, 8, 8, 1.0, w.rho, sp, 1)
+    ctx = B.mcrt_grid_create(8, 8, 8, w.cell_size_cm, w.rho, w.species, 1)
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_run(ctx, 10, 1)
+    assert e.value.code == B.MCRT_ESTATE
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_dust_tables(ctx, w.nu_hz[::-1], w.kappa_abs, w.kappa_sca, w.g, w.T_grid)
+    assert e.value.code == B.MCRT_EINVAL
+    B.mcrt_dust_tables(ctx, w.nu_hz, w.kappa_abs, w.kappa_sca, w.g, w.T_grid)
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_source(ctx, 1.0, 5000.0, None, (0.0, 1.0, 1.0))
+    assert e.value.code == B.MCRT_EINVAL
+    B.mcrt_source(ctx, w.L_erg_s, w.T_star_K, None, w.source_pos_cm)
+    with pytest.raises(B.McrtError):
+        B.mcrt_escape_bins(ctx, [0.0, 0.5, 0.4, 1.0])
+    st = B.mcrt_run(ctx, 1000, 1)
+    assert st["packets"] == 1000
+    # too small a caller workspace -> MCRT_ENOMEM
+    import torch
+
+    ws = torch.empty(4096, dtype=torch.uint8, device="cuda")
+    with pytest.raises(B.McrtError) as e:
+        B.mcrt_grid_create(8, 8, 8, 1.0, w.rho, w.species, 1, B.MCRT_HOST, ws, 4096)
+    assert e.value.code == B.MCRT_ENOMEM
+    B.mcrt_destroy(ctx)
