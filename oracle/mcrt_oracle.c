@@ -760,6 +760,11 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
         /* iterative scheme of PAPER.md:73: temperatures of the previous run, Eq. 5 for the frequency */
         R.cdf = C->cdfB;
         for (int sw = 1; sw <= o->n_sweeps; ++sw) {
+            /* counters describe the tallies they go with: each sweep starts both from zero */
+            uint64_t ep = st.epochs;
+            memset(&st, 0, sizeof st);
+            st.epochs = ep;
+            st.fx_bits = S->fx;
             sweep_update(S, o->sweep_T_from_lucy, cellfac, sw == 1 ? prev_fx : S->fx);
             zero_tallies(S);
             R.pass = o->pass0 + (uint32_t)sw;

@@ -14,7 +14,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "lib", "libmcrt_b200.so")
+LIB_PATH = os.environ.get("MCRT_B200_LIB") or os.path.join(_HERE, "lib", "libmcrt_b200.so")
 
 MCRT_HOST, MCRT_DEVICE = 0, 1
 MCRT_OK, MCRT_EINVAL, MCRT_ESTATE, MCRT_ENOMEM, MCRT_ECUDA, MCRT_EOVERFLOW = 0, -1, -2, -3, -4, -5

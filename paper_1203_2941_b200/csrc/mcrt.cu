@@ -207,12 +207,8 @@ __device__ __forceinline__ unsigned long long event_word(int type, int j, unsign
     return (unsigned long long)type | ((unsigned long long)j << 8) | (cell << 24);
 }
 
-// brick-major cell index: the grid is stored as 4x4x4 bricks so that a packet's next cell is usually
-// in the same 128-byte line (x or y step) or in the same 512-byte brick (z step).
-__device__ __forceinline__ uint32_t bx_part(int i) { return ((uint32_t)(i >> 2) << 6) | (uint32_t)(i & 3); }
-__device__ __forceinline__ uint32_t by_part(int i, uint32_t sby) { return (uint32_t)(i >> 2) * sby + ((uint32_t)(i & 3) << 2); }
-__device__ __forceinline__ uint32_t bz_part(int i, uint32_t sbz) { return (uint32_t)(i >> 2) * sbz + ((uint32_t)(i & 3) << 4); }
-
+// The grid is stored brick-major (4x4x4 bricks) so that a packet's next cell is usually in the same 128-byte
+// line (x or y step) or in the same 512-byte brick (z step); see brick_cell() below.
 struct TransportParams {
     const uint2 *__restrict__ cellw;
     long long *__restrict__ lfx;
@@ -222,7 +218,7 @@ struct TransportParams {
     unsigned long long *__restrict__ sed, *__restrict__ sed_direct, *__restrict__ counters;
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
-    uint32_t sby, sbz;  // brick strides: nbx*64, nbx*nby*64
+    int nbx, nby;       // bricks per axis
     double px, py, pz;  // source position, cell units
     unsigned long long pid0, count;
     uint32_t seed_lo, seed_hi, pass;
@@ -243,27 +239,33 @@ struct TransportParams {
 #ifndef MCRT_WALK_MIN
 #define MCRT_WALK_MIN 20
 #endif
+#ifndef MCRT_MIN_BLOCKS
+#define MCRT_MIN_BLOCKS 4
+#endif
+
+// full brick-major index of cell (ix, iy, iz); nbx, nby = bricks per axis
+__device__ __forceinline__ uint32_t brick_cell(int ix, int iy, int iz, int nbx, int nby)
+{
+    const uint32_t brick = (uint32_t)((iz >> 2) * nby + (iy >> 2)) * (uint32_t)nbx + (uint32_t)(ix >> 2);
+    return (brick << 6) | (uint32_t)(((iz & 3) << 4) | ((iy & 3) << 2) | (ix & 3));
+}
 
 template <bool RECORD>
-__global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
+__global__ void __launch_bounds__(256, MCRT_MIN_BLOCKS) k_transport(const TransportParams P)
 {
-    extern __shared__ double smem_d[];
+    extern __shared__ double2 smem_d2[];
     const int nsf = P.ns * P.nf;
-    double *s_kext = smem_d;
-    double *s_kabsfx = s_kext + nsf;
-    double *s_alb = s_kabsfx + nsf;
-    double *s_g = s_alb + nsf;
-    double *s_src = s_g + nsf;
+    double2 *s_kk = smem_d2;                 // {kext_h, kabs_fx} per (species, frequency): one LDS.128 per crossing
+    double2 *s_ag = s_kk + nsf;              // {albedo, g}
+    double *s_src = reinterpret_cast<double *>(s_ag + nsf);
     double *s_mu = s_src + P.nf;
     unsigned long long *s_cnt = reinterpret_cast<unsigned long long *>(s_mu + P.ndir + 1);
     unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
     const int nhist = 2 * P.ndir * P.nf;
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
-        s_kext[i] = P.kext_h[i];
-        s_kabsfx[i] = P.kabs_fx[i];
-        s_alb[i] = P.albedo[i];
-        s_g[i] = P.g[i];
+        s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
+        s_ag[i] = make_double2(P.albedo[i], P.g[i]);
     }
     for (int i = threadIdx.x; i < P.nf; i += blockDim.x) s_src[i] = P.srccdf[i];
     for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
@@ -282,10 +284,8 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
     double px = 0.0, py = 0.0, pz = 0.0, ux = 0.0, uy = 0.0, uz = 1.0;
     double tmx = 0.0, tmy = 0.0, tmz = 0.0, tdx = 0.0, tdy = 0.0, tdz = 0.0, t = 0.0, tau = 0.0, ztype = 0.0;
     int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-    uint32_t cpx = 0u, cpy = 0u, cpz = 0u;  // brick-index parts of (ix, iy, iz)
-    double rho_c = 0.0, kk = 0.0;
-    int sj = 0;
-    uint32_t cwy = 0u;
+    uint32_t cidx = 0u;                 // brick-major index of the current cell
+    uint2 cw = make_uint2(0u, 0u);      // its packed word {rho bits, species | tidx << 16}
 
     for (;;) {
         // ---------------------------------------------------------------- (a) S0 refill
@@ -303,14 +303,13 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
             if (__any_sync(kFull, exhausted)) exhausted = true;  // the counter only grows
         }
         if (exhausted && state == ST_IDLE) state = ST_DONE;
-        const unsigned ev = __ballot_sync(kFull, state == ST_EMIT || state == ST_INTERACT);
-        const unsigned fl = __ballot_sync(kFull, state == ST_FLY);
-        if ((ev | fl) == 0u) break;
+        if (!__any_sync(kFull, state != ST_DONE)) break;
 
         // ---------------------------------------------------------------- (b) events
         if (state == ST_EMIT || state == ST_INTERACT) {
             double z0, z1;
             bool scatter = false;
+            int sj = 0;
             if (state == ST_EMIT) {
                 // S2 emit: frequency through the source CDF (Eq. 1)
                 d = 0u; ncross = 0u; ndusty = 0u; nsca = 0u; nabs = 0u;
@@ -320,11 +319,14 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
                 px = P.px; py = P.py; pz = P.pz;
             } else {
                 // S5 partial segment up to the interaction point l' = tau/(rho kappa_ext) (Eq. 3)
+                const double rho_c = (double)__uint_as_float(cw.x);
+                sj = (int)(cw.y & 0xffu) * nf + j;
+                const double2 kq = s_kk[sj];
+                const double kk = kq.x * rho_c;
                 const double sint = tau / kk;
                 {
-                    const double x = s_kabsfx[sj] * rho_c * sint;
-                    atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + (cpx + cpy + cpz)),
-                              (unsigned long long)__double2ll_rn(x));
+                    const double x = kq.y * rho_c * sint;
+                    atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx), (unsigned long long)__double2ll_rn(x));
                 }
                 const double tint = t + sint;
                 double q;
@@ -333,17 +335,17 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
                 q = pz + uz * tint; q = fmax(q, (double)iz); q = fmin(q, (double)(iz + 1)); pz = q;
                 const unsigned long long cell = ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
                 // S6 scatter with probability albedo
-                if (ztype < s_alb[sj]) {
+                if (ztype < s_ag[sj].x) {
                     scatter = true;
                     nsca++;
                     if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
                 } else {
                     // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                     // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                    atomicAdd(&P.kcnt[cpx + cpy + cpz], 1ull);
+                    atomicAdd(&P.kcnt[cidx], 1ull);
                     nabs++;
-                    const int s = (int)(cwy & 0xffu);
-                    const int m = (int)(cwy >> 16);
+                    const int s = (int)(cw.y & 0xffu);
+                    const int m = (int)(cw.y >> 16);
                     draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                     j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
                     if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
@@ -353,7 +355,7 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
             draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
             double mu = 1.0 - 2.0 * z0;
             if (scatter) {
-                const double gg = s_g[sj];
+                const double gg = s_ag[sj].y;
                 if (fabs(gg) > 1e-6) {
                     const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
                     mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
@@ -391,6 +393,8 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
                 f = floor(px); ix = (px != f) ? (int)f : ((ux >= 0.0) ? (int)f : (int)f - 1);
                 f = floor(py); iy = (py != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1);
                 f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
+                cidx = brick_cell(ix, iy, iz, P.nbx, P.nby);
+                cw = __ldg(P.cellw + cidx);
                 if (RECORD)
                     hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
             }
@@ -409,11 +413,12 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
             else if (uz < 0.0) { const double inv = 1.0 / uz; stz = -1; tmz = ((double)iz - pz) * inv; tdz = -inv; }
             else { stz = 0; tmz = CUDART_INF; tdz = CUDART_INF; }
             t = 0.0;
-            cpx = bx_part(ix); cpy = by_part(iy, P.sby); cpz = bz_part(iz, P.sbz);
             state = ST_FLY;
         }
 
         // ---------------------------------------------------------------- (c) S4/S5 cell walk
+        // Branch-free step: the axis choice, the next cell and its prefetch do not depend on the current
+        // cell's data, so the load of cell n+1 is in flight while cell n is tallied.
         for (;;) {
             const unsigned flying = __ballot_sync(kFull, state == ST_FLY);
             if (flying == 0u) break;
@@ -422,32 +427,38 @@ __global__ void __launch_bounds__(256, 2) k_transport(const TransportParams P)
             if (state == ST_FLY) {
                 const bool selx = (tmx <= tmy) && (tmx <= tmz);
                 const bool sely = !selx && (tmy <= tmz);
+                const bool selz = !selx && !sely;
                 const double tn = selx ? tmx : (sely ? tmy : tmz);
+                const int nix = ix + (selx ? stx : 0);
+                const int niy = iy + (sely ? sty : 0);
+                const int niz = iz + (selz ? stz : 0);
+                const bool out = ((unsigned)nix >= (unsigned)P.nx) | ((unsigned)niy >= (unsigned)P.ny) |
+                                 ((unsigned)niz >= (unsigned)P.nz);
+                const uint32_t ncidx = out ? cidx : brick_cell(nix, niy, niz, P.nbx, P.nby);
+                const uint2 cwn = __ldg(P.cellw + ncidx);  // prefetch of the next cell's word
                 const double ds = tn - t;
-                const uint32_t cidx = cpx + cpy + cpz;
-                const uint2 cw = __ldg(P.cellw + cidx);
-                rho_c = (double)__uint_as_float(cw.x);
-                cwy = cw.y;
-                sj = (int)(cw.y & 0xffu) * nf + j;
-                kk = s_kext[sj] * rho_c;          // (kabs+ksca) h rho  (Eq. 2 per unit path)
-                const double dtau = kk * ds;      // tau_i of PAPER.md:49
+                const double rho_c = (double)__uint_as_float(cw.x);
+                const double2 kq = s_kk[(int)(cw.y & 0xffu) * nf + j];
+                const double dtau = kq.x * rho_c * ds;  // tau_i = (kabs+ksca) h rho ds (Eq. 2)
                 if (dtau > tau) {
-                    state = ST_INTERACT;          // interaction inside this cell (equality leaves, Q5)
+                    state = ST_INTERACT;               // interaction inside this cell (equality leaves, Q5)
                 } else {
                     tau -= dtau;
                     if (rho_c > 0.0) {
                         // S5 Lucy path-length tally, 64-bit fixed point (Eq. 9, linear form)
-                        const double x = s_kabsfx[sj] * rho_c * ds;
-                        atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx),
-                                  (unsigned long long)__double2ll_rn(x));
+                        const double x = kq.y * rho_c * ds;
+                        atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx), (unsigned long long)__double2ll_rn(x));
                         ndusty++;
                     }
                     t = tn;
                     ncross++;
-                    bool out;
-                    if (selx) { ix += stx; tmx += tdx; cpx = bx_part(ix); out = (unsigned)ix >= (unsigned)P.nx; }
-                    else if (sely) { iy += sty; tmy += tdy; cpy = by_part(iy, P.sby); out = (unsigned)iy >= (unsigned)P.ny; }
-                    else { iz += stz; tmz += tdz; cpz = bz_part(iz, P.sbz); out = (unsigned)iz >= (unsigned)P.nz; }
+                    const double tnew = tn + (selx ? tdx : (sely ? tdy : tdz));
+                    tmx = selx ? tnew : tmx;
+                    tmy = sely ? tnew : tmy;
+                    tmz = selz ? tnew : tmz;
+                    ix = nix; iy = niy; iz = niz;
+                    cidx = ncidx;
+                    cw = cwn;
                     if (out) {
                         // S10 escape tally: frequency x |cos i| bin, block-private histogram
                         const double amu = fabs(uz);
@@ -1123,7 +1134,7 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
     P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
     P.dig = o.record_digests ? c->dig : nullptr;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
-    P.sby = (uint32_t)c->nbx * kBrickCells; P.sbz = (uint32_t)c->nbx * c->nby * kBrickCells;
+    P.nbx = c->nbx; P.nby = c->nby;
     P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     const size_t j_smem = (size_t)c->ns * c->nT * 8;

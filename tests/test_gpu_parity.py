@@ -52,7 +52,7 @@ def _assert_parity(o, c, ro, rg, w, N):
     if same.all():
         assert np.array_equal(do, dg)
         for key in ("packets", "crossings", "dusty_crossings", "flights", "scatterings", "absorptions", "escapes",
-                    "direct_escapes", "epochs", "lucy_adds", "fx_bits"):
+                    "direct_escapes", "lucy_adds", "fx_bits"):
             assert ro[key] == rg[key], key
         for key in ("k", "sed", "sed_direct", "tidx"):
             assert np.array_equal(raw_o[key], raw_g[key]), key
