@@ -284,32 +284,38 @@ void orc_hg_scatter(double gg, double z0, double z1, const double u[3], double u
  * O4  Cell walk.  The paper says only that a packet "enters a neighboring cell according to its
  * direction of travel"; the walk is the Amanatides-Woo voxel traversal (reading Q8):
  * per axis the parameter t of the next face, measured from the flight origin in cell units;
- * the axis with the smallest one is crossed next (ties x before y before z).
+ * the axis with the smallest one is crossed next (ties x before y before z).  The parameter of a
+ * face is always computed from the face coordinate itself, t = (f - p_a) * (1/u_a) (reading Q8,
+ * DESIGN.md section 2): it is a function of the face alone, so the walk is the three-way merge of the
+ * per-axis face sequences ordered by (t, axis) and carries no accumulated rounding.
  * ---------------------------------------------------------------------------------------------- */
 typedef struct {
-    double tmax[3], tdel[3];
+    double tmax[3], inv[3], p[3];
     int step[3];
 } orc_dda;
+
+/* parameter of the face the packet leaves cell c_a through, along axis a */
+static inline double dda_face_t(const orc_dda *D, int a, int c_a)
+{
+    if (D->step[a] == 0) return INFINITY;
+    return ((double)(c_a + (D->step[a] > 0 ? 1 : 0)) - D->p[a]) * D->inv[a];
+}
 
 static void dda_setup(orc_dda *D, const double p[3], const double u[3], const int c[3])
 {
     for (int a = 0; a < 3; ++a) {
-        if (u[a] > 0.0) {
-            double inv = 1.0 / u[a];
-            D->step[a] = 1;
-            D->tmax[a] = ((double)(c[a] + 1) - p[a]) * inv;
-            D->tdel[a] = inv;
-        } else if (u[a] < 0.0) {
-            double inv = 1.0 / u[a];
-            D->step[a] = -1;
-            D->tmax[a] = ((double)c[a] - p[a]) * inv;
-            D->tdel[a] = -inv;
-        } else {
-            D->step[a] = 0;
-            D->tmax[a] = INFINITY;
-            D->tdel[a] = INFINITY;
-        }
+        D->p[a] = p[a];
+        D->step[a] = (u[a] > 0.0) ? 1 : ((u[a] < 0.0) ? -1 : 0);
+        D->inv[a] = (D->step[a] != 0) ? 1.0 / u[a] : INFINITY;
+        D->tmax[a] = dda_face_t(D, a, c[a]);
     }
+}
+
+/* cross the face of axis a: next cell, and the parameter of the face it will be left through */
+static inline void dda_advance(orc_dda *D, int a, int c[3])
+{
+    c[a] += D->step[a];
+    D->tmax[a] = dda_face_t(D, a, c[a]);
 }
 
 static inline int dda_axis(const orc_dda *D)
@@ -350,8 +356,7 @@ int orc_dda_trace(int nx, int ny, int nz, const double p[3], const double u[3], 
         }
         ++cnt;
         t = tn;
-        c[a] += D.step[a];
-        D.tmax[a] += D.tdel[a];
+        dda_advance(&D, a, c);
     }
     return cnt;
 }
@@ -487,8 +492,7 @@ static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
             tau -= dtau;
             lucy_add(R, ci, sj, rho_c, ds, st);
             t = tn;
-            c[a] += D.step[a];
-            D.tmax[a] += D.tdel[a];
+            dda_advance(&D, a, c);
             ncross++;
             st->crossings++;
             if (rho_c > 0.0) st->dusty_crossings++;
