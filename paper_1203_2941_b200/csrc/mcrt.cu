@@ -19,6 +19,7 @@
 #include <vector>
 
 #include "mcrt.h"
+#include "dda.h"
 
 #define MCRT_VERSION_STRING "mcrt-b200 0.1 (sm_100a)"
 
@@ -33,7 +34,6 @@ constexpr double kLightC = 2.99792458e10;     // cm s^-1
 constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
-constexpr int kBrickCells = 64;     // 4x4x4 cells per brick; 64 cells * 8 B = 512 B = 4 cache lines
 constexpr unsigned kFull = 0xffffffffu;
 
 enum : int { ST_IDLE = 0, ST_EMIT = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4 };
@@ -64,7 +64,9 @@ struct mcrt_ctx {
     bool ws_owned_by_caller = false;
     std::vector<void *> owned;       // cudaMalloc'ed blocks when no workspace was given
     // device arrays
-    uint2 *cellw = nullptr;               // [ncp] {rho bits, species | tidx<<16}
+    unsigned long long *cellw = nullptr;  // [ncp] packed cell words (see "Packed cell word")
+    uint32_t *vmask = nullptr;            // vacuum masks, three levels back to back
+    int msh = 2, mbx[3] = {0, 0, 0}, mby[3] = {0, 0, 0}, mbz[3] = {0, 0, 0}, moff[3] = {0, 0, 0}, mwords = 0;
     long long *lfx = nullptr;             // [ncp] Lucy fixed-point tally
     unsigned long long *kabs_cnt = nullptr, *kprev = nullptr;  // [ncp]
     void *scratch = nullptr;              // [nc*8 bytes]
@@ -207,61 +209,131 @@ __device__ __forceinline__ unsigned long long event_word(int type, int j, unsign
     return (unsigned long long)type | ((unsigned long long)j << 8) | (cell << 24);
 }
 
-// The grid is stored brick-major (4x4x4 bricks) so that a packet's next cell is usually in the same 128-byte
-// line (x or y step) or in the same 512-byte brick (z step); see brick_cell() below.
+// ------------------------------------------------------------------------------------------------
+// Packed cell word (8 bytes, one per cell, brick-major order):
+//   the fp64 bit pattern of the cell's fp32 density -- exact, its low 29 mantissa bits are always zero --
+//   with the dust species in bits 0-7 and the frozen-epoch temperature index in bits 8-23.
+// One 8-byte load per crossing serves S4, S5, S6 and S9, and the density needs no fp32->fp64 conversion.
+// ------------------------------------------------------------------------------------------------
+constexpr unsigned long long kRhoMask = 0xFFFFFFFFE0000000ull;
+
+__device__ __forceinline__ double cw_rho(unsigned long long cw) { return __longlong_as_double((long long)(cw & kRhoMask)); }
+__device__ __forceinline__ int cw_species(unsigned long long cw) { return (int)((unsigned)cw & 0xffu); }
+__device__ __forceinline__ int cw_tidx(unsigned long long cw) { return (int)(((unsigned)cw >> 8) & 0xffffu); }
+__device__ __forceinline__ bool cw_vacuum(unsigned long long cw) { return (unsigned)(cw >> 32) == 0u; }  // rho == +0
+
+// The grid is stored brick-major: bricks of E^3 cells, E = 1 << bsh (4 for grids up to 256^3, 8 up to 512^3),
+// so that a packet's next cell is usually in the same 128-byte line or at least in the same brick.
+//
+// Vacuum masks: three bit arrays, level l = 0,1,2, one bit per aligned box of (E << 2l)^3 cells, set when
+// every cell of the box (clipped to the grid) has rho == 0.  A level-0 box IS a brick, so the brick number
+// of a cell indexes both its mask bit and its storage.  Level 0 lives in shared memory: cells of an empty
+// brick are never loaded.
 struct TransportParams {
-    const uint2 *__restrict__ cellw;
+    const unsigned long long *__restrict__ cellw;
     long long *__restrict__ lfx;
     unsigned long long *__restrict__ kcnt;
     const double *__restrict__ kext_h, *__restrict__ kabs_fx, *__restrict__ albedo, *__restrict__ g;
     const double *__restrict__ srccdf, *__restrict__ cdf, *__restrict__ mu_edges;
+    const uint32_t *__restrict__ vmask;   // the three levels, back to back
     unsigned long long *__restrict__ sed, *__restrict__ sed_direct, *__restrict__ counters;
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
     int nbx, nby;       // bricks per axis
+    int bsh;            // log2 of the brick edge
+    int m0words;        // 32-bit words of the level-0 mask
     double px, py, pz;  // source position, cell units
     unsigned long long pid0, count;
     uint32_t seed_lo, seed_hi, pass;
 };
 
+// full brick-major index of cell (ix, iy, iz)
+__device__ __forceinline__ uint32_t brick_of(int ix, int iy, int iz, int nbx, int nby, int bsh)
+{
+    return (uint32_t)((iz >> bsh) * nby + (iy >> bsh)) * (uint32_t)nbx + (uint32_t)(ix >> bsh);
+}
+__device__ __forceinline__ uint32_t cell_in_brick(uint32_t brick, int ix, int iy, int iz, int bsh)
+{
+    const int m = (1 << bsh) - 1;
+    return (((brick << bsh) | (uint32_t)(iz & m)) << (2 * bsh)) | (uint32_t)(((iy & m) << bsh) | (ix & m));
+}
+__device__ __forceinline__ bool brick_empty(const uint32_t *m0, uint32_t brick) { return (m0[brick >> 5] >> (brick & 31u)) & 1u; }
+
+// S5 Lucy path-length tally: L[c] += rint(x), x = kabs h rho ds 2^FX >= 0 (Eq. 9, linear form;
+// PAPER.md:142 integer atomics).  rint by the 1.5 * 2^52 trick: round to nearest even, exact below 2^51, and
+// x < 37 * 2^40 always, because a packet never spends more than its tau = -ln zeta <= 36.8 in one cell.
+__device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
+{
+    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
+    atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
+}
+
 // ------------------------------------------------------------------------------------------------
-// S0-S10  the transport kernel: persistent threads, one packet per lane, warp-level refill.
+// S0-S10  the transport kernel: persistent CTAs; every warp owns a POOL of kSlots packets in shared memory.
 //
-// Every lane is a small state machine (EMIT / FLY / INTERACT / IDLE).  A warp alternates between
-//  (a) refill: idle lanes take the next packet ids with ONE warp-aggregated atomic on the epoch counter,
-//  (b) events: all lanes that need an emission, a scattering or an absorption + re-emission do it together
-//      (they share the Philox / sincos / DDA-setup code), and
-//  (c) the cell walk: flying lanes step cell by cell; the walk loop keeps going until fewer than
-//      WALK_MIN lanes are still flying while others wait for an event, so both phases run with most
-//      lanes active whatever the mix of optical depths (the paper parks long-lived packets instead,
-//      PAPER.md:128).
+// A packet is either FLYING (walking cell by cell towards its next interaction) or waiting for an EVENT
+// (emission of the slot's next packet, an interaction, the escape tally).  The two kinds of work share no
+// code, so a warp never mixes them: it alternates between
+//   S phase: the 32 lanes check 32 flying packets out of the pool into registers and step them cell by cell
+//            (S4/S5) until kSwap of them have reached an event; then all are parked again;
+//   E phase: entered when fewer than 32 packets can fly; the lanes take up to 32 waiting packets and each
+//            performs that packet's event (S1-S3, S6-S10, S0 refill with one warp-aggregated atomic).
+// With 64 packets per warp both phases run with (nearly) all lanes active whatever the mix of optical
+// depths -- the scheduling-independent replacement of the paper's pause/resume balancer.
+// Results never depend on which lane or warp carries a packet: all random numbers are Philox blocks keyed
+// by (seed, packet id, draw index, pass) and all tallies are integer atomics.
 // ------------------------------------------------------------------------------------------------
-#ifndef MCRT_WALK_MIN
-#define MCRT_WALK_MIN 20
-#endif
-#ifndef MCRT_MIN_BLOCKS
-#define MCRT_MIN_BLOCKS 4
+constexpr int kSlots = 64;          // packets per warp
+constexpr int kSlotF64 = 15;        // 8-byte fields per slot
+constexpr int kSlotU32 = 6;         // 4-byte fields per slot
+constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
+#ifndef MCRT_SWAP_MIN
+#define MCRT_SWAP_MIN 8             // an S phase ends when this many of its packets wait for an event
 #endif
 
-// full brick-major index of cell (ix, iy, iz); nbx, nby = bricks per axis
-__device__ __forceinline__ uint32_t brick_cell(int ix, int iy, int iz, int nbx, int nby)
+enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_IVX, F_IVY, F_IVZ, F_T, F_TAU, F_ZTYPE, F_CW, F_HASH, F_PID };
+enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
+enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
+
+// position of the n-th set bit (n = 0, 1, ...) of a 64-bit mask; n < popc(m)
+__device__ __forceinline__ int nth_set64(unsigned long long m, int n)
 {
-    const uint32_t brick = (uint32_t)((iz >> 2) * nby + (iy >> 2)) * (uint32_t)nbx + (uint32_t)(ix >> 2);
-    return (brick << 6) | (uint32_t)(((iz & 3) << 4) | ((iy & 3) << 2) | (ix & 3));
+    const uint32_t lo = (uint32_t)m, hi = (uint32_t)(m >> 32);
+    const int clo = __popc(lo);
+    const bool up = n >= clo;
+    const uint32_t w = up ? hi : lo;
+    n = up ? n - clo : n;
+    int pos = 0;
+#pragma unroll
+    for (int sft = 16; sft; sft >>= 1) {
+        const int c = __popc((w >> pos) & ((1u << sft) - 1u));
+        if (n >= c) { n -= c; pos += sft; }
+    }
+    return pos + (up ? 32 : 0);
+}
+
+// warp-wide OR of one 64-bit word per lane
+__device__ __forceinline__ unsigned long long warp_or64(unsigned long long v)
+{
+    const uint32_t lo = __reduce_or_sync(kFull, (uint32_t)v), hi = __reduce_or_sync(kFull, (uint32_t)(v >> 32));
+    return ((unsigned long long)hi << 32) | lo;
 }
 
 template <bool RECORD>
-__global__ void __launch_bounds__(256, MCRT_MIN_BLOCKS) k_transport(const TransportParams P)
+__global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
 {
     extern __shared__ double2 smem_d2[];
     const int nsf = P.ns * P.nf;
-    double2 *s_kk = smem_d2;                 // {kext_h, kabs_fx} per (species, frequency): one LDS.128 per crossing
-    double2 *s_ag = s_kk + nsf;              // {albedo, g}
+    const int nwarps = blockDim.x >> 5;
+    double *s_pool = reinterpret_cast<double *>(smem_d2);                // [nwarps][kPoolBytesPerWarp]
+    double2 *s_kk = reinterpret_cast<double2 *>(s_pool + (size_t)nwarps * (kPoolBytesPerWarp / 8));
+    double2 *s_ag = s_kk + nsf;              // {albedo, g};  s_kk = {kext_h, kabs_fx}: one LDS.128 per crossing
     double *s_src = reinterpret_cast<double *>(s_ag + nsf);
     double *s_mu = s_src + P.nf;
     unsigned long long *s_cnt = reinterpret_cast<unsigned long long *>(s_mu + P.ndir + 1);
     unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
     const int nhist = 2 * P.ndir * P.nf;
+    uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -270,224 +342,302 @@ __global__ void __launch_bounds__(256, MCRT_MIN_BLOCKS) k_transport(const Transp
     for (int i = threadIdx.x; i < P.nf; i += blockDim.x) s_src[i] = P.srccdf[i];
     for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
+    for (int i = threadIdx.x; i < P.m0words; i += blockDim.x) s_m0[i] = P.vmask[i];
     if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0ull;
     __syncthreads();
 
-    const unsigned lane = threadIdx.x & 31u;
-    const unsigned lane_lt = (1u << lane) - 1u;
-    const int nf = P.nf;
+    const int lane = (int)(threadIdx.x & 31u);
+    const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby;
+    double *wf = s_pool + (size_t)(threadIdx.x >> 5) * (kPoolBytesPerWarp / 8);   // this warp's pool, f64 fields
+    uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kSlotF64 * kSlots);          // its u32 fields
+#define SF(f, s) wf[(f) * kSlots + (s)]
+#define SU(f, s) wu[(f) * kSlots + (s)]
 
-    int state = ST_IDLE;
-    bool exhausted = false;
-    unsigned long long pid = 0ull, hash = 0ull;
-    uint32_t d = 0u, ncross = 0u, ndusty = 0u, nsca = 0u, nabs = 0u;
-    double px = 0.0, py = 0.0, pz = 0.0, ux = 0.0, uy = 0.0, uz = 1.0;
-    double tmx = 0.0, tmy = 0.0, tmz = 0.0, tdx = 0.0, tdy = 0.0, tdz = 0.0, t = 0.0, tau = 0.0, ztype = 0.0;
-    int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-    uint32_t cidx = 0u;                 // brick-major index of the current cell
-    uint2 cw = make_uint2(0u, 0u);      // its packed word {rho bits, species | tidx << 16}
+    // every slot starts as "emit the next packet"
+    for (int s = lane; s < kSlots; s += 32) SU(U_DK, s) = K_EMIT << 30;
+    __syncwarp();
+    unsigned long long mFly = 0ull, mEv = ~0ull;   // warp-uniform: parked flying packets / packets waiting for an event
+    bool exhausted = false;                        // the epoch counter has run out (warp-uniform)
+    unsigned long long ndusty_acc = 0ull;          // dusty crossings stepped by this lane
 
     for (;;) {
-        // ---------------------------------------------------------------- (a) S0 refill
-        const unsigned need = __ballot_sync(kFull, state == ST_IDLE && !exhausted);
-        if (need) {
-            const int leader = __ffs(need) - 1;
-            unsigned long long base = 0ull;
-            if ((int)lane == leader) base = atomicAdd(&P.counters[CNT_NEXT], (unsigned long long)__popc(need));
-            base = __shfl_sync(kFull, base, leader);
-            if (state == ST_IDLE && !exhausted) {
-                const unsigned long long idx = base + (unsigned long long)__popc(need & lane_lt);
-                if (idx < P.count) { pid = P.pid0 + idx; state = ST_EMIT; }
-                else exhausted = true;
+        const int nfly = __popcll(mFly);
+        if (nfly >= 32 || (nfly > 0 && mEv == 0ull)) {
+            // =========================================================== S phase: S4/S5 cell walk
+            const int nact = min(nfly, 32);
+            const bool act = lane < nact;
+            int slot = 0, state = ST_IDLE;
+            double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
+            double t = 0.0, tau = 0.0;
+            int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0, j = 0;
+            uint32_t cidx = 0u, ncross = 0u;
+            unsigned long long cw = 0ull;
+            if (act) {
+                slot = nth_set64(mFly, lane);
+                px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
+                ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+                t = SF(F_T, slot); tau = SF(F_TAU, slot);
+                cw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
+                ncross = SU(U_NCROSS, slot);
+                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
+                // the stored 1/u is +inf for a zero direction component: that axis never moves
+                stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
+                sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
+                stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
+                tmx = mcrt::face_t(ix, stx, px, ivx);
+                tmy = mcrt::face_t(iy, sty, py, ivy);
+                tmz = mcrt::face_t(iz, stz, pz, ivz);
+                cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                state = ST_FLY;
             }
-            if (__any_sync(kFull, exhausted)) exhausted = true;  // the counter only grows
-        }
-        if (exhausted && state == ST_IDLE) state = ST_DONE;
-        if (!__any_sync(kFull, state != ST_DONE)) break;
-
-        // ---------------------------------------------------------------- (b) events
-        if (state == ST_EMIT || state == ST_INTERACT) {
-            double z0, z1;
-            bool scatter = false;
-            int sj = 0;
-            if (state == ST_EMIT) {
-                // S2 emit: frequency through the source CDF (Eq. 1)
-                d = 0u; ncross = 0u; ndusty = 0u; nsca = 0u; nabs = 0u;
-                hash = 0xCBF29CE484222325ull;
-                draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
-                j = lower_bound_cdf(s_src, nf, z0);
-                px = P.px; py = P.py; pz = P.pz;
-            } else {
-                // S5 partial segment up to the interaction point l' = tau/(rho kappa_ext) (Eq. 3)
-                const double rho_c = (double)__uint_as_float(cw.x);
-                sj = (int)(cw.y & 0xffu) * nf + j;
-                const double2 kq = s_kk[sj];
-                const double kk = kq.x * rho_c;
-                const double sint = tau / kk;
-                {
-                    const double x = kq.y * rho_c * sint;
-                    atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx), (unsigned long long)__double2ll_rn(x));
-                }
-                const double tint = t + sint;
-                double q;
-                q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
-                q = py + uy * tint; q = fmax(q, (double)iy); q = fmin(q, (double)(iy + 1)); py = q;
-                q = pz + uz * tint; q = fmax(q, (double)iz); q = fmin(q, (double)(iz + 1)); pz = q;
-                const unsigned long long cell = ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
-                // S6 scatter with probability albedo
-                if (ztype < s_ag[sj].x) {
-                    scatter = true;
-                    nsca++;
-                    if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
-                } else {
-                    // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
-                    // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                    atomicAdd(&P.kcnt[cidx], 1ull);
-                    nabs++;
-                    const int s = (int)(cw.y & 0xffu);
-                    const int m = (int)(cw.y >> 16);
-                    draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
-                    j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
-                    if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
-                }
-            }
-            // new direction: isotropic or Henyey-Greenstein about the old one (S7)
-            draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
-            double mu = 1.0 - 2.0 * z0;
-            if (scatter) {
-                const double gg = s_ag[sj].y;
-                if (fabs(gg) > 1e-6) {
-                    const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
-                    mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
-                    mu = fmin(mu, 1.0);
-                    mu = fmax(mu, -1.0);
-                }
-            }
-            const double phi = kTwoPi * z1;
-            double sp, cp;
-            sincos(phi, &sp, &cp);
-            const double st = sqrt(1.0 - mu * mu);
-            if (scatter) {
-                double a0, a1, a2;
-                if (fabs(uz) > 0.99999) {
-                    a0 = st * cp;
-                    a1 = st * sp;
-                    a2 = (uz > 0.0) ? mu : -mu;
-                } else {
-                    const double w = sqrt(1.0 - uz * uz);
-                    const double iw = 1.0 / w;
-                    const double t0 = ux * uz * cp - uy * sp;
-                    const double t1 = uy * uz * cp + ux * sp;
-                    a0 = st * t0 * iw + ux * mu;
-                    a1 = st * t1 * iw + uy * mu;
-                    a2 = uz * mu - st * cp * w;
-                }
-                const double inorm = 1.0 / sqrt(a0 * a0 + a1 * a1 + a2 * a2);
-                ux = a0 * inorm; uy = a1 * inorm; uz = a2 * inorm;
-            } else {
-                ux = st * cp; uy = st * sp; uz = mu;
-            }
-            if (state == ST_EMIT) {
-                // start cell: floor(p), or by direction sign when p sits on a face (reading Q9)
-                double f;
-                f = floor(px); ix = (px != f) ? (int)f : ((ux >= 0.0) ? (int)f : (int)f - 1);
-                f = floor(py); iy = (py != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1);
-                f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
-                cidx = brick_cell(ix, iy, iz, P.nbx, P.nby);
-                cw = __ldg(P.cellw + cidx);
-                if (RECORD)
-                    hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
-            }
-            // S3 optical depth of the flight: tau = -ln zeta, zeta_1 kept for S6
-            draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
-            tau = -log(z0);
-            ztype = z1;
-            // S4 set up the walk (Amanatides-Woo): parameter of the next face per axis
-            if (ux > 0.0) { const double inv = 1.0 / ux; stx = 1; tmx = ((double)(ix + 1) - px) * inv; tdx = inv; }
-            else if (ux < 0.0) { const double inv = 1.0 / ux; stx = -1; tmx = ((double)ix - px) * inv; tdx = -inv; }
-            else { stx = 0; tmx = CUDART_INF; tdx = CUDART_INF; }
-            if (uy > 0.0) { const double inv = 1.0 / uy; sty = 1; tmy = ((double)(iy + 1) - py) * inv; tdy = inv; }
-            else if (uy < 0.0) { const double inv = 1.0 / uy; sty = -1; tmy = ((double)iy - py) * inv; tdy = -inv; }
-            else { sty = 0; tmy = CUDART_INF; tdy = CUDART_INF; }
-            if (uz > 0.0) { const double inv = 1.0 / uz; stz = 1; tmz = ((double)(iz + 1) - pz) * inv; tdz = inv; }
-            else if (uz < 0.0) { const double inv = 1.0 / uz; stz = -1; tmz = ((double)iz - pz) * inv; tdz = -inv; }
-            else { stz = 0; tmz = CUDART_INF; tdz = CUDART_INF; }
-            t = 0.0;
-            state = ST_FLY;
-        }
-
-        // ---------------------------------------------------------------- (c) S4/S5 cell walk
-        // Branch-free step: the axis choice, the next cell and its prefetch do not depend on the current
-        // cell's data, so the load of cell n+1 is in flight while cell n is tallied.
-        for (;;) {
-            const unsigned flying = __ballot_sync(kFull, state == ST_FLY);
-            if (flying == 0u) break;
-            if (__popc(flying) < MCRT_WALK_MIN &&
-                __any_sync(kFull, state == ST_INTERACT || (state == ST_IDLE && !exhausted))) break;
-            if (state == ST_FLY) {
-                const bool selx = (tmx <= tmy) && (tmx <= tmz);
-                const bool sely = !selx && (tmy <= tmz);
-                const bool selz = !selx && !sely;
-                const double tn = selx ? tmx : (sely ? tmy : tmz);
-                const int nix = ix + (selx ? stx : 0);
-                const int niy = iy + (sely ? sty : 0);
-                const int niz = iz + (selz ? stz : 0);
-                const bool out = ((unsigned)nix >= (unsigned)P.nx) | ((unsigned)niy >= (unsigned)P.ny) |
-                                 ((unsigned)niz >= (unsigned)P.nz);
-                const uint32_t ncidx = out ? cidx : brick_cell(nix, niy, niz, P.nbx, P.nby);
-                const uint2 cwn = __ldg(P.cellw + ncidx);  // prefetch of the next cell's word
-                const double ds = tn - t;
-                const double rho_c = (double)__uint_as_float(cw.x);
-                const double2 kq = s_kk[(int)(cw.y & 0xffu) * nf + j];
-                const double dtau = kq.x * rho_c * ds;  // tau_i = (kabs+ksca) h rho ds (Eq. 2)
-                if (dtau > tau) {
-                    state = ST_INTERACT;               // interaction inside this cell (equality leaves, Q5)
-                } else {
-                    tau -= dtau;
-                    if (rho_c > 0.0) {
-                        // S5 Lucy path-length tally, 64-bit fixed point (Eq. 9, linear form)
-                        const double x = kq.y * rho_c * ds;
-                        atomicAdd(reinterpret_cast<unsigned long long *>(P.lfx + cidx), (unsigned long long)__double2ll_rn(x));
-                        ndusty++;
+            mFly &= ~warp_or64(act ? (1ull << slot) : 0ull);
+            const int stop_at = max(nact - MCRT_SWAP_MIN, 0);
+            // Branch-free step: the axis choice, the next cell and its prefetch do not depend on the current
+            // cell's data, so the load of cell n+1 is in flight while cell n is tallied.
+            for (;;) {
+                if (state == ST_FLY) {
+                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
+                    const bool sely = !selx && (tmy <= tmz);
+                    const bool selz = !selx && !sely;
+                    const double tn = selx ? tmx : (sely ? tmy : tmz);
+                    const int nix = ix + (selx ? stx : 0);
+                    const int niy = iy + (sely ? sty : 0);
+                    const int niz = iz + (selz ? stz : 0);
+                    const bool out = ((unsigned)nix >= (unsigned)P.nx) | ((unsigned)niy >= (unsigned)P.ny) |
+                                     ((unsigned)niz >= (unsigned)P.nz);
+                    // parameter of the face through which the next cell will be left (reading Q8)
+                    if (selx) tmx = (mcrt::int_to_double(nix + ((stx + 1) >> 1)) - px) * ivx;
+                    if (sely) tmy = (mcrt::int_to_double(niy + ((sty + 1) >> 1)) - py) * ivy;
+                    if (selz) tmz = (mcrt::int_to_double(niz + ((stz + 1) >> 1)) - pz) * ivz;
+                    unsigned long long cwn = 0ull;
+                    uint32_t ncidx = cidx;
+                    if (!out) {
+                        const uint32_t brick = brick_of(nix, niy, niz, nbx, nby, bsh);
+                        ncidx = cell_in_brick(brick, nix, niy, niz, bsh);
+                        if (!brick_empty(s_m0, brick)) cwn = __ldg(P.cellw + ncidx);   // prefetch
                     }
-                    t = tn;
-                    ncross++;
-                    const double tnew = tn + (selx ? tdx : (sely ? tdy : tdz));
-                    tmx = selx ? tnew : tmx;
-                    tmy = sely ? tnew : tmy;
-                    tmz = selz ? tnew : tmz;
-                    ix = nix; iy = niy; iz = niz;
-                    cidx = ncidx;
-                    cw = cwn;
-                    if (out) {
-                        // S10 escape tally: frequency x |cos i| bin, block-private histogram
-                        const double amu = fabs(uz);
-                        int bin = 0;
-                        for (int b = 1; b < P.ndir; ++b) if (s_mu[b] <= amu) bin = b;
-                        atomicAdd(&s_hist[bin * nf + j], 1u);
-                        const bool direct = (nsca + nabs) == 0u;
-                        if (direct) atomicAdd(&s_hist[P.ndir * nf + bin * nf + j], 1u);
-                        atomicAdd(&s_cnt[CNT_PACKETS], 1ull);
-                        atomicAdd(&s_cnt[CNT_CROSS], (unsigned long long)ncross);
-                        atomicAdd(&s_cnt[CNT_DUSTY], (unsigned long long)ndusty);
-                        atomicAdd(&s_cnt[CNT_SCA], (unsigned long long)nsca);
-                        atomicAdd(&s_cnt[CNT_ABS], (unsigned long long)nabs);
-                        if (direct) atomicAdd(&s_cnt[CNT_DIRECT], 1ull);
-                        if (RECORD) {
-                            hash_mix(hash, event_word(EV_ESCAPE, j, (unsigned long long)bin));
-                            hash_mix(hash, (unsigned long long)ncross);
-                            hash_mix(hash, (unsigned long long)nsca | ((unsigned long long)nabs << 32));
-                            mcrt_digest dg;
-                            dg.hash = hash; dg.crossings = ncross; dg.scatterings = nsca; dg.absorptions = nabs;
-                            dg.escape_bin = (uint32_t)bin;
-                            P.dig[pid] = dg;  // packet ids of a run start at 0
+                    const double ds = tn - t;
+                    const double rho_c = cw_rho(cw);
+                    const double2 kq = s_kk[cw_species(cw) * nf + j];
+                    const double dtau = kq.x * rho_c * ds;  // tau_i = (kabs+ksca) h rho ds (Eq. 2)
+                    if (dtau > tau) {
+                        state = ST_INTERACT;               // interaction inside this cell (equality leaves, Q5)
+                    } else {
+                        tau -= dtau;
+                        if (!cw_vacuum(cw)) {
+                            lucy_add(P.lfx, cidx, kq.y * rho_c * ds);
+                            ndusty_acc++;
                         }
-                        state = ST_IDLE;
+                        t = tn;
+                        ncross++;
+                        ix = nix; iy = niy; iz = niz;
+                        cidx = ncidx;
+                        cw = cwn;
+                        if (out) state = ST_DONE;          // left the grid: escape tally in the E phase
                     }
                 }
+                if (__popc(__ballot_sync(kFull, state == ST_FLY)) <= stop_at) break;
             }
+            // park: only what the walk changes (p, u, 1/u stay as the event left them)
+            if (act) {
+                SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
+                SF(F_CW, slot) = __longlong_as_double((long long)cw);
+                SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
+                SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | ((uint32_t)j << 16);
+                SU(U_NCROSS, slot) = ncross;
+                if (state != ST_FLY)
+                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
+            }
+            mFly |= warp_or64((act && state == ST_FLY) ? (1ull << slot) : 0ull);
+            mEv |= warp_or64((act && state != ST_FLY) ? (1ull << slot) : 0ull);
+            __syncwarp();
+        } else if (mEv != 0ull) {
+            // =========================================================== E phase: one event per lane
+            const int nev = min(__popcll(mEv), 32);
+            const bool act = lane < nev;
+            const int slot = act ? nth_set64(mEv, lane) : 0;
+            uint32_t kind = act ? (SU(U_DK, slot) >> 30) : 3u;
+            uint32_t d = SU(U_DK, slot) & 0x3fffffffu;
+            unsigned long long pid = 0ull, hash = 0ull;
+            uint32_t ncross = 0u, nsca = 0u, nabs = 0u;
+            int ix = 0, iy = 0, iz = 0, j = 0;
+            double ux = 0.0, uy = 0.0, uz = 1.0;
+            if (act && kind != K_EMIT) {
+                pid = (unsigned long long)__double_as_longlong(SF(F_PID, slot));
+                if (RECORD) hash = (unsigned long long)__double_as_longlong(SF(F_HASH, slot));
+                ncross = SU(U_NCROSS, slot); nsca = SU(U_NSCA, slot); nabs = SU(U_NABS, slot);
+                const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
+                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
+                ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+            }
+            if (kind == K_ESCAPED) {
+                // S10 escape tally: frequency x |cos i| bin, block-private histogram + counters
+                const double amu = fabs(uz);
+                int bin = 0;
+                for (int b = 1; b < P.ndir; ++b) if (s_mu[b] <= amu) bin = b;
+                atomicAdd(&s_hist[bin * nf + j], 1u);
+                const bool direct = (nsca + nabs) == 0u;
+                if (direct) atomicAdd(&s_hist[P.ndir * nf + bin * nf + j], 1u);
+                atomicAdd(&s_cnt[CNT_PACKETS], 1ull);
+                atomicAdd(&s_cnt[CNT_CROSS], (unsigned long long)ncross);
+                atomicAdd(&s_cnt[CNT_SCA], (unsigned long long)nsca);
+                atomicAdd(&s_cnt[CNT_ABS], (unsigned long long)nabs);
+                if (direct) atomicAdd(&s_cnt[CNT_DIRECT], 1ull);
+                if (RECORD) {
+                    hash_mix(hash, event_word(EV_ESCAPE, j, (unsigned long long)bin));
+                    hash_mix(hash, (unsigned long long)ncross);
+                    hash_mix(hash, (unsigned long long)nsca | ((unsigned long long)nabs << 32));
+                    mcrt_digest dg;
+                    dg.hash = hash; dg.crossings = ncross; dg.scatterings = nsca; dg.absorptions = nabs;
+                    dg.escape_bin = (uint32_t)bin;
+                    P.dig[pid] = dg;  // packet ids of a run start at 0
+                }
+                kind = K_EMIT;        // the slot takes the next packet of the epoch
+            }
+            // S0 refill: the slots that need a new packet take the next ids with ONE atomic per warp
+            const unsigned need = __ballot_sync(kFull, kind == K_EMIT);
+            bool dead = false;
+            if (need) {
+                unsigned long long base = P.count;
+                if (!exhausted) {
+                    const int leader = __ffs(need) - 1;
+                    if (lane == leader) base = atomicAdd(&P.counters[CNT_NEXT], (unsigned long long)__popc(need));
+                    base = __shfl_sync(kFull, base, leader);
+                }
+                if (kind == K_EMIT) {
+                    const unsigned long long idx = base + (unsigned long long)__popc(need & ((1u << lane) - 1u));
+                    if (idx < P.count) pid = P.pid0 + idx; else dead = true;
+                }
+                if (__any_sync(kFull, dead)) exhausted = true;   // the counter only grows
+            }
+            if (act && !dead) {
+                double px, py, pz, z0, z1;
+                bool scatter = false;
+                int sj = 0;
+                unsigned long long cw;
+                uint32_t cidx;
+                if (kind == K_EMIT) {
+                    // S2 emit: frequency through the source CDF (Eq. 1)
+                    d = 0u; ncross = 0u; nsca = 0u; nabs = 0u;
+                    hash = 0xCBF29CE484222325ull;
+                    draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                    j = lower_bound_cdf(s_src, nf, z0);
+                    px = P.px; py = P.py; pz = P.pz;
+                    cw = 0ull; cidx = 0u;
+                } else {
+                    // S5 partial segment up to the interaction point l' = tau/(rho kappa_ext) (Eq. 3)
+                    px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
+                    const double t = SF(F_T, slot), tau = SF(F_TAU, slot), ztype = SF(F_ZTYPE, slot);
+                    cw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                    cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                    const double rho_c = cw_rho(cw);
+                    sj = cw_species(cw) * nf + j;
+                    const double2 kq = s_kk[sj];
+                    const double kk = kq.x * rho_c;
+                    const double sint = tau / kk;
+                    lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
+                    const double tint = t + sint;
+                    double q;
+                    q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
+                    q = py + uy * tint; q = fmax(q, (double)iy); q = fmin(q, (double)(iy + 1)); py = q;
+                    q = pz + uz * tint; q = fmax(q, (double)iz); q = fmin(q, (double)(iz + 1)); pz = q;
+                    const unsigned long long cell = ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
+                    // S6 scatter with probability albedo
+                    if (ztype < s_ag[sj].x) {
+                        scatter = true;
+                        nsca++;
+                        if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
+                    } else {
+                        // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
+                        // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
+                        atomicAdd(&P.kcnt[cidx], 1ull);
+                        nabs++;
+                        const int s = cw_species(cw);
+                        const int m = cw_tidx(cw);
+                        draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                        j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
+                        if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
+                    }
+                }
+                // new direction: isotropic or Henyey-Greenstein about the old one (S7)
+                draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                double mu = 1.0 - 2.0 * z0;
+                if (scatter) {
+                    const double gg = s_ag[sj].y;
+                    if (fabs(gg) > 1e-6) {
+                        const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
+                        mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
+                        mu = fmin(mu, 1.0);
+                        mu = fmax(mu, -1.0);
+                    }
+                }
+                const double phi = kTwoPi * z1;
+                double sp, cp;
+                sincos(phi, &sp, &cp);
+                const double st = sqrt(1.0 - mu * mu);
+                if (scatter) {
+                    double a0, a1, a2;
+                    if (fabs(uz) > 0.99999) {
+                        a0 = st * cp;
+                        a1 = st * sp;
+                        a2 = (uz > 0.0) ? mu : -mu;
+                    } else {
+                        const double w = sqrt(1.0 - uz * uz);
+                        const double iw = 1.0 / w;
+                        const double t0 = ux * uz * cp - uy * sp;
+                        const double t1 = uy * uz * cp + ux * sp;
+                        a0 = st * t0 * iw + ux * mu;
+                        a1 = st * t1 * iw + uy * mu;
+                        a2 = uz * mu - st * cp * w;
+                    }
+                    const double inorm = 1.0 / sqrt(a0 * a0 + a1 * a1 + a2 * a2);
+                    ux = a0 * inorm; uy = a1 * inorm; uz = a2 * inorm;
+                } else {
+                    ux = st * cp; uy = st * sp; uz = mu;
+                }
+                if (kind == K_EMIT) {
+                    // start cell: floor(p), or by direction sign when p sits on a face (reading Q9)
+                    double f;
+                    f = floor(px); ix = (px != f) ? (int)f : ((ux >= 0.0) ? (int)f : (int)f - 1);
+                    f = floor(py); iy = (py != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1);
+                    f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
+                    const uint32_t brick = brick_of(ix, iy, iz, nbx, nby, bsh);
+                    cidx = cell_in_brick(brick, ix, iy, iz, bsh);
+                    cw = brick_empty(s_m0, brick) ? 0ull : __ldg(P.cellw + cidx);
+                    if (RECORD)
+                        hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
+                }
+                // S3 optical depth of the flight: tau = -ln zeta, zeta_1 kept for S6
+                draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                // park the new flight (reading Q8: the walk needs p, 1/u, the cell; t = 0)
+                SF(F_PX, slot) = px; SF(F_PY, slot) = py; SF(F_PZ, slot) = pz;
+                SF(F_UX, slot) = ux; SF(F_UY, slot) = uy; SF(F_UZ, slot) = uz;
+                SF(F_IVX, slot) = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
+                SF(F_IVY, slot) = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
+                SF(F_IVZ, slot) = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+                SF(F_T, slot) = 0.0;
+                SF(F_TAU, slot) = -log(z0);
+                SF(F_ZTYPE, slot) = z1;
+                SF(F_CW, slot) = __longlong_as_double((long long)cw);
+                SF(F_PID, slot) = __longlong_as_double((long long)pid);
+                if (RECORD) SF(F_HASH, slot) = __longlong_as_double((long long)hash);
+                SU(U_DK, slot) = d;    // kind is set when the walk stops
+                SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
+                SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
+                SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | ((uint32_t)j << 16);
+            }
+            const unsigned long long mine = act ? (1ull << slot) : 0ull;
+            mEv &= ~warp_or64(mine);                       // taken: now flying, or dead (no packets left)
+            mFly |= warp_or64(dead ? 0ull : mine);
+            __syncwarp();
+        } else {
+            break;
         }
     }
+#undef SF
+#undef SU
+    if (ndusty_acc) atomicAdd(&s_cnt[CNT_DUSTY], ndusty_acc);
 
     // flush the block-private histogram and counters
     __syncthreads();
@@ -517,7 +667,7 @@ __device__ __forceinline__ int t_index(const double *J, int nT, double x)
     return lo > nT - 1 ? nT - 1 : lo;
 }
 
-__global__ void __launch_bounds__(256) k_epoch_update(uint2 *__restrict__ cellw, const unsigned long long *__restrict__ kcnt,
+__global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__restrict__ cellw, const unsigned long long *__restrict__ kcnt,
                                                       unsigned long long *__restrict__ kprev,
                                                       const long long *__restrict__ lfx, const double *__restrict__ J,
                                                       int nT, int ns, size_t ncp, int first_epoch, double ratio,
@@ -529,8 +679,8 @@ __global__ void __launch_bounds__(256) k_epoch_update(uint2 *__restrict__ cellw,
     if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
     bool ovf = false;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
-        uint2 cw = cellw[i];
-        const double rho_c = (double)__uint_as_float(cw.x);
+        const unsigned long long cw = cellw[i];
+        const double rho_c = cw_rho(cw);
         const unsigned long long kc = kcnt[i];
         uint32_t m = 0u;
         if (rho_c > 0.0) {
@@ -541,19 +691,19 @@ __global__ void __launch_bounds__(256) k_epoch_update(uint2 *__restrict__ cellw,
                 kt = (double)kc + ((pred > 1.0) ? pred : 1.0);
             }
             const double x = kt * cellfac / rho_c;
-            m = (uint32_t)t_index(s_J + (cw.y & 0xffu) * nT, nT, x);
+            m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, x);
             const long long v = lfx[i];
             ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
         }
         kprev[i] = kc;
-        const uint32_t ny_ = (cw.y & 0xffffu) | (m << 16);
-        if (ny_ != cw.y) cellw[i].y = ny_;
+        const uint32_t lo = (uint32_t)cw, nlo = (lo & 0xFF0000FFu) | (m << 8);
+        if (nlo != lo) reinterpret_cast<uint32_t *>(cellw + i)[0] = nlo;  // low word: species | tidx << 8 | rho bits 29-31
     }
     if (ovf) counters[CNT_OVERFLOW] = 1ull;
 }
 
 // S12 temperature index for a frozen-T sweep from the previous pass's tallies; zeroes them.
-__global__ void __launch_bounds__(256) k_sweep_update(uint2 *__restrict__ cellw, unsigned long long *__restrict__ kcnt,
+__global__ void __launch_bounds__(256) k_sweep_update(unsigned long long *__restrict__ cellw, unsigned long long *__restrict__ kcnt,
                                                       unsigned long long *__restrict__ kprev, long long *__restrict__ lfx,
                                                       const double *__restrict__ J, int nT, int ns, size_t ncp,
                                                       int from_lucy, double inv_fx, double cellfac,
@@ -564,15 +714,15 @@ __global__ void __launch_bounds__(256) k_sweep_update(uint2 *__restrict__ cellw,
     __syncthreads();
     if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
-        uint2 cw = cellw[i];
-        const double rho_c = (double)__uint_as_float(cw.x);
+        const unsigned long long cw = cellw[i];
+        const double rho_c = cw_rho(cw);
         uint32_t m = 0u;
         if (rho_c > 0.0) {
             const double e = from_lucy ? (double)lfx[i] * inv_fx : (double)kcnt[i];
             const double x = e * cellfac / rho_c;
-            m = (uint32_t)t_index(s_J + (cw.y & 0xffu) * nT, nT, x);
+            m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, x);
         }
-        cellw[i].y = (cw.y & 0xffffu) | (m << 16);
+        reinterpret_cast<uint32_t *>(cellw + i)[0] = ((uint32_t)cw & 0xFF0000FFu) | (m << 8);
         kcnt[i] = 0ull;
         kprev[i] = 0ull;
         lfx[i] = 0ll;
@@ -594,31 +744,69 @@ __global__ void __launch_bounds__(256) k_range_check(const long long *__restrict
 // ------------------------------------------------------------------------------------------------
 // layout kernels: canonical [nz][ny][nx] <-> brick-major
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ size_t brick_index(int ix, int iy, int iz, int nbx, int nby)
+__device__ __forceinline__ size_t brick_index(int ix, int iy, int iz, int nbx, int nby, int bsh)
 {
-    return ((size_t)((iz >> 2) * nby + (iy >> 2)) * nbx + (ix >> 2)) * kBrickCells + ((iz & 3) << 4) + ((iy & 3) << 2) + (ix & 3);
+    return cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
 }
 
-__global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__restrict__ sp, uint2 *__restrict__ cellw,
-                            int nx, int ny, int nz, int nbx, int nby, int nbz, int ns, unsigned long long *__restrict__ bad)
+__global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__restrict__ sp, unsigned long long *__restrict__ cellw,
+                            int nx, int ny, int nz, int nbx, int nby, int nbz, int bsh, int ns, unsigned long long *__restrict__ bad)
 {
-    const size_t ncp = (size_t)nbx * nby * nbz * kBrickCells;
+    const size_t ncp = ((size_t)nbx * nby * nbz) << (3 * bsh);
+    const int m = (1 << bsh) - 1;
     for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < ncp; b += (size_t)gridDim.x * blockDim.x) {
-        const size_t brick = b >> 6;
-        const int l = (int)(b & 63);
+        const size_t brick = b >> (3 * bsh);
+        const int l = (int)(b & (((size_t)1 << (3 * bsh)) - 1));
         const int bxi = (int)(brick % nbx), byi = (int)((brick / nbx) % nby), bzi = (int)(brick / ((size_t)nbx * nby));
-        const int ix = bxi * 4 + (l & 3), iy = byi * 4 + ((l >> 2) & 3), iz = bzi * 4 + (l >> 4);
-        uint2 cw = make_uint2(0u, 0u);
+        const int ix = (bxi << bsh) + (l & m), iy = (byi << bsh) + ((l >> bsh) & m), iz = (bzi << bsh) + (l >> (2 * bsh));
+        unsigned long long cw = 0ull;
         if (ix < nx && iy < ny && iz < nz) {
             const size_t i = ((size_t)iz * ny + iy) * nx + ix;
             const float r = rho[i];
             const uint32_t s = sp[i];
             if (!(r >= 0.0f) || isinf(r)) atomicAdd(&bad[0], 1ull);
             if (s >= (uint32_t)ns) atomicAdd(&bad[1], 1ull);
-            cw.x = __float_as_uint(r);
-            cw.y = s;
+            // fp32 -> fp64 is exact and leaves the low 29 mantissa bits zero; -0 is stored as +0
+            const double rd = (r > 0.0f) ? (double)r : 0.0;
+            cw = ((unsigned long long)__double_as_longlong(rd) & kRhoMask) | (unsigned long long)(s & 0xffu);
         }
         cellw[b] = cw;
+    }
+}
+
+// Vacuum mask of one level: bit of box (bx, by, bz) is set when all its in-grid cells have rho == 0.
+// Level 0 is built from the packed cells, level l > 0 from level l - 1 (4x4x4 children per box).
+__global__ void k_build_mask0(const unsigned long long *__restrict__ cellw, uint32_t *__restrict__ m, int nx, int ny, int nz,
+                              int nbx, int nby, int sh, int mbx, int mby, int mbz)
+{
+    const int nb = mbx * mby * mbz;
+    for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
+        const int bx = b % mbx, by = (b / mbx) % mby, bz = b / (mbx * mby);
+        const int x0 = bx << sh, y0 = by << sh, z0 = bz << sh;
+        const int x1 = min(x0 + (1 << sh), nx), y1 = min(y0 + (1 << sh), ny), z1 = min(z0 + (1 << sh), nz);
+        bool empty = true;
+        for (int z = z0; z < z1 && empty; ++z)
+            for (int y = y0; y < y1 && empty; ++y)
+                for (int x = x0; x < x1; ++x)
+                    if (!cw_vacuum(cellw[brick_index(x, y, z, nbx, nby, sh)])) { empty = false; break; }
+        if (empty) atomicOr(&m[b >> 5], 1u << (b & 31));
+    }
+}
+
+__global__ void k_build_mask_up(const uint32_t *__restrict__ lower, uint32_t *__restrict__ m, int lbx, int lby, int lbz,
+                                int mbx, int mby, int mbz)
+{
+    const int nb = mbx * mby * mbz;
+    for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
+        const int bx = b % mbx, by = (b / mbx) % mby, bz = b / (mbx * mby);
+        bool empty = true;
+        for (int z = bz * 4; z < min(bz * 4 + 4, lbz) && empty; ++z)
+            for (int y = by * 4; y < min(by * 4 + 4, lby) && empty; ++y)
+                for (int x = bx * 4; x < min(bx * 4 + 4, lbx); ++x) {
+                    const int c = (z * lby + y) * lbx + x;
+                    if (!((lower[c >> 5] >> (c & 31)) & 1u)) { empty = false; break; }
+                }
+        if (empty) atomicOr(&m[b >> 5], 1u << (b & 31));
     }
 }
 
@@ -639,28 +827,28 @@ __device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int 
 }
 
 // gathers one output array in canonical order (O12: E_count = k xi, E_lucy = xi L / 2^FX, T by inverting Eq. 4)
-__global__ void k_gather(int what, void *__restrict__ out, const uint2 *__restrict__ cellw,
+__global__ void k_gather(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
                          const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
                          const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
-                         int nbx, int nby, double xi, double inv_fx, double cellfac)
+                         int nbx, int nby, int bsh, double xi, double inv_fx, double cellfac)
 {
     const size_t nc = (size_t)nx * ny * nz;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
         const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
-        const size_t b = brick_index(ix, iy, iz, nbx, nby);
+        const size_t b = brick_index(ix, iy, iz, nbx, nby, bsh);
         switch (what) {
         case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
         case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[b]; break;
-        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)(cellw[b].y >> 16); break;
+        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)cw_tidx(cellw[b]); break;
         case G_ECOUNT: reinterpret_cast<double *>(out)[i] = (double)kcnt[b] * xi; break;
         case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[b] * inv_fx * xi; break;
         default: {
-            const uint2 cw = cellw[b];
-            const double rho_c = (double)__uint_as_float(cw.x);
+            const unsigned long long cw = cellw[b];
+            const double rho_c = cw_rho(cw);
             float T = 0.0f;
             if (rho_c > 0.0) {
                 const double e = (what == G_TLUCY) ? (double)lfx[b] * inv_fx : (double)kcnt[b];
-                T = (float)T_of_x(J + (cw.y & 0xffu) * nT, Tg, nT, e * cellfac / rho_c);
+                T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
             }
             reinterpret_cast<float *>(out)[i] = T;
         }
@@ -732,10 +920,38 @@ int fx_bits_for(uint64_t n)
     return fx;
 }
 
-size_t transport_smem_bytes(int ns, int nf, int ndir)
+size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads)
 {
-    return (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) + 8 * sizeof(unsigned long long) +
-           (size_t)2 * ndir * nf * sizeof(unsigned int);
+    return (size_t)(threads / 32) * kPoolBytesPerWarp + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
+           8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
+           (size_t)mask0_words * sizeof(uint32_t);
+}
+
+// Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
+// which level 0 fits 32 KB of shared memory; each further level is 4x coarser per axis.
+struct MaskGeom {
+    int msh, mbx[3], mby[3], mbz[3], moff[3], mwords;
+};
+
+MaskGeom mask_geom(int nx, int ny, int nz)
+{
+    MaskGeom g;
+    g.msh = 2;
+    for (;;) {
+        const size_t e = (size_t)1 << g.msh;
+        const size_t bits = ((nx + e - 1) / e) * ((ny + e - 1) / e) * ((nz + e - 1) / e);
+        if (bits <= ((size_t)1 << 18)) break;
+        ++g.msh;
+    }
+    int off = 0;
+    for (int l = 0; l < 3; ++l) {
+        const int e = 1 << (g.msh + 2 * l);
+        g.mbx[l] = (nx + e - 1) / e; g.mby[l] = (ny + e - 1) / e; g.mbz[l] = (nz + e - 1) / e;
+        g.moff[l] = off;
+        off += (g.mbx[l] * g.mby[l] * g.mbz[l] + 31) / 32;
+    }
+    g.mwords = off;
+    return g;
 }
 
 int stream_grid(size_t n)
@@ -771,10 +987,12 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
 {
     if (!bytes_out || nx < 1 || ny < 1 || nz < 1 || n_species < 1 || n_nu < 2 || n_T < 2 || n_dir < 1) return MCRT_EINVAL;
     const size_t nc = (size_t)nx * ny * nz;
-    const size_t ncp = (size_t)((nx + 3) / 4) * ((ny + 3) / 4) * ((nz + 3) / 4) * kBrickCells;
+    const MaskGeom mg = mask_geom(nx, ny, nz);
+    const size_t ncp = ((size_t)mg.mbx[0] * mg.mby[0] * mg.mbz[0]) << (3 * mg.msh);
     size_t b = 0;
     auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
     add(ncp * sizeof(uint2));            // cell words
+    add((size_t)mg.mwords * 4);          // vacuum masks
     add(ncp * sizeof(long long));        // Lucy tally
     add(ncp * sizeof(long long));        // k
     add(ncp * sizeof(long long));        // k_prev
@@ -799,6 +1017,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     if (!out) return fail(nullptr, MCRT_EINVAL, "out is NULL");
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be >= 1");
+    if (nx > 65535 || ny > 65535 || nz > 65535) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be <= 65535");
     if ((size_t)nx * ny * nz > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
     if (!(cell_size_cm > 0.0) || !isfinite(cell_size_cm)) return fail(nullptr, MCRT_EINVAL, "cell_size_cm must be > 0");
     if (!rho || !species) return fail(nullptr, MCRT_EINVAL, "rho / species is NULL");
@@ -810,9 +1029,14 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     mcrt_ctx *c = new mcrt_ctx();
     cudaGetDevice(&c->device);
     c->nx = nx; c->ny = ny; c->nz = nz; c->ns = n_species; c->h = cell_size_cm;
-    c->nbx = (nx + 3) / 4; c->nby = (ny + 3) / 4; c->nbz = (nz + 3) / 4;
+    {
+        const MaskGeom g = mask_geom(nx, ny, nz);   // a brick is a level-0 mask box
+        c->msh = g.msh; c->mwords = g.mwords;
+        for (int l = 0; l < 3; ++l) { c->mbx[l] = g.mbx[l]; c->mby[l] = g.mby[l]; c->mbz[l] = g.mbz[l]; c->moff[l] = g.moff[l]; }
+    }
+    c->nbx = c->mbx[0]; c->nby = c->mby[0]; c->nbz = c->mbz[0];
     c->nc = (size_t)nx * ny * nz;
-    c->ncp = (size_t)c->nbx * c->nby * c->nbz * kBrickCells;
+    c->ncp = ((size_t)c->nbx * c->nby * c->nbz) << (3 * c->msh);
     c->ws = (char *)workspace; c->ws_bytes = workspace_bytes; c->ws_owned_by_caller = workspace != nullptr;
     int rc;
 #define GC_TRY(expr)                                                       \
@@ -830,6 +1054,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         }                                                                                              \
     } while (0)
     GC_TRY(ws_alloc(c, (void **)&c->cellw, c->ncp * sizeof(uint2)));
+    GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
     GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
@@ -847,7 +1072,15 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     }
     unsigned long long *bad = c->counters + CNT_N;
     k_pack_grid<<<stream_grid(c->ncp), 256, 0, c->stream>>>(d_rho, d_sp, c->cellw, nx, ny, nz, c->nbx, c->nby, c->nbz,
-                                                           n_species, bad);
+                                                           c->msh, n_species, bad);
+    GC_CUDA(cudaGetLastError());
+    GC_CUDA(cudaMemsetAsync(c->vmask, 0, (size_t)c->mwords * 4, c->stream));
+    k_build_mask0<<<stream_grid((size_t)c->mbx[0] * c->mby[0] * c->mbz[0]), 256, 0, c->stream>>>(
+        c->cellw, c->vmask + c->moff[0], nx, ny, nz, c->nbx, c->nby, c->msh, c->mbx[0], c->mby[0], c->mbz[0]);
+    for (int l = 1; l < 3; ++l)
+        k_build_mask_up<<<stream_grid((size_t)c->mbx[l] * c->mby[l] * c->mbz[l]), 256, 0, c->stream>>>(
+            c->vmask + c->moff[l - 1], c->vmask + c->moff[l], c->mbx[l - 1], c->mby[l - 1], c->mbz[l - 1], c->mbx[l],
+            c->mby[l], c->mbz[l]);
     GC_CUDA(cudaGetLastError());
     GC_CUDA(cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
     GC_CUDA(cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
@@ -895,7 +1128,7 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
         if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
         if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
     }
-    if (transport_smem_bytes(ns, n_nu, 16) > 200 * 1024)
+    if (transport_smem_bytes(ns, n_nu, 16, c->moff[1], 256) > 220 * 1024)
         return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
     c->nf = n_nu; c->nT = n_T;
     c->nu.assign(nu_hz, nu_hz + n_nu);
@@ -1023,9 +1256,11 @@ static int ensure_histograms(mcrt_ctx *c)
 
 static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem)
 {
-    *threads = (o && o->block_threads > 0) ? o->block_threads : 256;
-    if (*threads % 32 || *threads > 256 || *threads < 32) return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32..256");
-    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir);
+    *threads = (o && o->block_threads > 0) ? o->block_threads : 512;
+    if (*threads % 32 || *threads > 512 || *threads < 32) return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32..512");
+    // as many warps (each with its packet pool) as fit beside the tables in 227 KB of shared memory
+    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->moff[1], *threads) > 227 * 1024) *threads -= 32;
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->moff[1], *threads);
     if (*smem > 48 * 1024) {
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
@@ -1135,6 +1370,7 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
     P.dig = o.record_digests ? c->dig : nullptr;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
     P.nbx = c->nbx; P.nby = c->nby;
+    P.vmask = c->vmask; P.bsh = c->msh; P.m0words = c->moff[1];
     P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     const size_t j_smem = (size_t)c->ns * c->nT * 8;
@@ -1207,7 +1443,7 @@ static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem wh
     void *dev = (where == MCRT_DEVICE) ? dst : c->scratch;
     const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
     k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, c->nT, c->nx,
-                                                       c->ny, c->nz, c->nbx, c->nby, c->xi, ldexp(1.0, -c->fx), cellfac);
+                                                       c->ny, c->nz, c->nbx, c->nby, c->msh, c->xi, ldexp(1.0, -c->fx), cellfac);
     CUDA_TRY(c, cudaGetLastError());
     if (where == MCRT_HOST) {
         CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
