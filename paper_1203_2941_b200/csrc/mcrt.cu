@@ -319,6 +319,18 @@ __device__ __forceinline__ unsigned long long warp_or64(unsigned long long v)
     return ((unsigned long long)hi << 32) | lo;
 }
 
+// 8-byte asynchronous copy global -> shared (LDGSTS), per-thread groups
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+constexpr int kRing = 4;            // cell-word ring slots per thread (cells n .. n+3)
+
 template <bool RECORD>
 __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
 {
@@ -334,6 +346,10 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
     const int nhist = 2 * P.ndir * P.nf;
     uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
+    // cell-word ring: slot k of thread i at s_ring[k * blockDim.x + i]
+    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.m0words + 1) & ~1));
+    volatile unsigned long long *ring = s_ring + threadIdx.x;
+    const int ring_stride = blockDim.x;
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -364,60 +380,84 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
         const int nfly = __popcll(mFly);
         if (nfly >= 32 || (nfly > 0 && mEv == 0ull)) {
             // =========================================================== S phase: S4/S5 cell walk
+            // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
+            // (G: axis choice, next cell, exit parameter) runs kAhead = 2 cells ahead of the physics and the
+            // cell words travel global -> shared memory with cp.async into a small per-thread ring: the latency
+            // of a cell's word is covered by two walk iterations of every resident warp.
             const int nact = min(nfly, 32);
             const bool act = lane < nact;
             int slot = 0, state = ST_IDLE;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
-            double t = 0.0, tau = 0.0;
-            int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-            uint32_t cidx = 0u, ncross = 0u;
-            unsigned long long cw = 0ull;
+            double t = 0.0, tau = 0.0, tn0 = 0.0, tn1 = 0.0;
+            int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
+            uint32_t xy0 = 0u, xy1 = 0u, z0 = 0u, z1 = 0u;      // packed coordinates of cells n, n+1
+            uint32_t cidx0 = 0u, cidx1 = 0u, gcidx = 0u, ncross = 0u;
+            bool o1 = true, o2 = true;                          // cell n+1 / n+2 lies outside the grid
+            int r = 0;                                          // ring slot of cell n
+
+            // advance G by one cell: returns the exit parameter of the cell it leaves, requests the word of
+            // the cell it enters (ring slot rs) unless that cell is outside the grid or in an empty brick
+            auto advance = [&](double &tn_left, bool &entered_out, int rs) {
+                const bool selx = (tmx <= tmy) && (tmx <= tmz);
+                const bool sely = !selx && (tmy <= tmz);
+                const bool selz = !selx && !sely;
+                tn_left = selx ? tmx : (sely ? tmy : tmz);
+                gx += selx ? stx : 0;
+                gy += sely ? sty : 0;
+                gz += selz ? stz : 0;
+                // parameter of the face through which the entered cell will be left (reading Q8)
+                if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;
+                if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;
+                if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;
+                entered_out = ((unsigned)gx >= (unsigned)P.nx) | ((unsigned)gy >= (unsigned)P.ny) |
+                              ((unsigned)gz >= (unsigned)P.nz);
+                if (!entered_out) {
+                    const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);
+                    gcidx = cell_in_brick(brick, gx, gy, gz, bsh);
+                    if (!brick_empty(s_m0, brick)) cp_async8(const_cast<unsigned long long *>(ring) + rs * ring_stride, P.cellw + gcidx);
+                    else ring[rs * ring_stride] = 0ull;
+                }
+            };
+
             if (act) {
                 slot = nth_set64(mFly, lane);
                 px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                 ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
                 t = SF(F_T, slot); tau = SF(F_TAU, slot);
-                cw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                ring[0] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                 const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
                 ncross = SU(U_NCROSS, slot);
-                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
+                gx = (int)(w0 & 0xffffu); gy = (int)(w0 >> 16); gz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
                 // the stored 1/u is +inf for a zero direction component: that axis never moves
                 stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
                 sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
                 stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
-                tmx = mcrt::face_t(ix, stx, px, ivx);
-                tmy = mcrt::face_t(iy, sty, py, ivy);
-                tmz = mcrt::face_t(iz, stz, pz, ivz);
-                cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                tmx = mcrt::face_t(gx, stx, px, ivx);
+                tmy = mcrt::face_t(gy, sty, py, ivy);
+                tmz = mcrt::face_t(gz, stz, pz, ivz);
+                xy0 = w0; z0 = w1 & 0xffffu;
+                cidx0 = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
+                advance(tn0, o1, 1);                              // G: cell n -> n+1
+                cp_async_commit();
+                xy1 = (uint32_t)(gx & 0xffff) | ((uint32_t)gy << 16); z1 = (uint32_t)gz; cidx1 = gcidx;
+                if (!o1) advance(tn1, o2, 2);                     // G: cell n+1 -> n+2
+                cp_async_commit();
                 state = ST_FLY;
             }
             mFly &= ~warp_or64(act ? (1ull << slot) : 0ull);
             const int stop_at = max(nact - MCRT_SWAP_MIN, 0);
-            // Branch-free step: the axis choice, the next cell and its prefetch do not depend on the current
-            // cell's data, so the load of cell n+1 is in flight while cell n is tallied.
             for (;;) {
                 if (state == ST_FLY) {
-                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
-                    const bool sely = !selx && (tmy <= tmz);
-                    const bool selz = !selx && !sely;
-                    const double tn = selx ? tmx : (sely ? tmy : tmz);
-                    const int nix = ix + (selx ? stx : 0);
-                    const int niy = iy + (sely ? sty : 0);
-                    const int niz = iz + (selz ? stz : 0);
-                    const bool out = ((unsigned)nix >= (unsigned)P.nx) | ((unsigned)niy >= (unsigned)P.ny) |
-                                     ((unsigned)niz >= (unsigned)P.nz);
-                    // parameter of the face through which the next cell will be left (reading Q8)
-                    if (selx) tmx = (mcrt::int_to_double(nix + ((stx + 1) >> 1)) - px) * ivx;
-                    if (sely) tmy = (mcrt::int_to_double(niy + ((sty + 1) >> 1)) - py) * ivy;
-                    if (selz) tmz = (mcrt::int_to_double(niz + ((stz + 1) >> 1)) - pz) * ivz;
-                    unsigned long long cwn = 0ull;
-                    uint32_t ncidx = cidx;
-                    if (!out) {
-                        const uint32_t brick = brick_of(nix, niy, niz, nbx, nby, bsh);
-                        ncidx = cell_in_brick(brick, nix, niy, niz, bsh);
-                        if (!brick_empty(s_m0, brick)) cwn = __ldg(P.cellw + ncidx);   // prefetch
-                    }
-                    const double ds = tn - t;
+                    cp_async_wait<2>();                           // the word of cell n has landed
+                    const unsigned long long cw = ring[r * ring_stride];
+                    // G: cell n+2 -> n+3 (keeps two requests in flight)
+                    const uint32_t xy2 = (uint32_t)(gx & 0xffff) | ((uint32_t)gy << 16), z2 = (uint32_t)gz, cidx2 = gcidx;
+                    double tn2 = 0.0;
+                    bool o3 = true;
+                    if (!o2) advance(tn2, o3, (r + 3) & 3);
+                    cp_async_commit();
+                    // physics of cell n
+                    const double ds = tn0 - t;
                     const double rho_c = cw_rho(cw);
                     const double2 kq = s_kk[cw_species(cw) * nf + j];
                     const double dtau = kq.x * rho_c * ds;  // tau_i = (kabs+ksca) h rho ds (Eq. 2)
@@ -426,25 +466,30 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                     } else {
                         tau -= dtau;
                         if (!cw_vacuum(cw)) {
-                            lucy_add(P.lfx, cidx, kq.y * rho_c * ds);
+                            lucy_add(P.lfx, cidx0, kq.y * rho_c * ds);
                             ndusty_acc++;
                         }
-                        t = tn;
+                        t = tn0;
                         ncross++;
-                        ix = nix; iy = niy; iz = niz;
-                        cidx = ncidx;
-                        cw = cwn;
-                        if (out) state = ST_DONE;          // left the grid: escape tally in the E phase
+                        if (o1) {
+                            state = ST_DONE;               // left the grid: escape tally in the E phase
+                        } else {
+                            xy0 = xy1; z0 = z1; cidx0 = cidx1; tn0 = tn1;
+                            xy1 = xy2; z1 = z2; cidx1 = cidx2; tn1 = tn2;
+                            o1 = o2; o2 = o3;
+                            r = (r + 1) & 3;
+                        }
                     }
                 }
                 if (__popc(__ballot_sync(kFull, state == ST_FLY)) <= stop_at) break;
             }
+            cp_async_wait<0>();
             // park: only what the walk changes (p, u, 1/u stay as the event left them)
             if (act) {
                 SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
-                SF(F_CW, slot) = __longlong_as_double((long long)cw);
-                SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
-                SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | ((uint32_t)j << 16);
+                SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
+                SU(U_W0, slot) = xy0;
+                SU(U_W1, slot) = z0 | ((uint32_t)j << 16);
                 SU(U_NCROSS, slot) = ncross;
                 if (state != ST_FLY)
                     SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
@@ -924,7 +969,7 @@ size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threa
 {
     return (size_t)(threads / 32) * kPoolBytesPerWarp + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
            8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
-           (size_t)mask0_words * sizeof(uint32_t);
+           (size_t)((mask0_words + 1) & ~1) * sizeof(uint32_t) + (size_t)kRing * threads * sizeof(unsigned long long);
 }
 
 // Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
