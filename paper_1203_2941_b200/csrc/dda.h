@@ -90,21 +90,26 @@ MCRT_HD unsigned box_jump(int &ix, int &iy, int &iz, double &tmx, double &tmy, d
     const bool ey = !ex && (Ty <= Tz);
     const bool ez = !ex && !ey;
     const double Te = ex ? Tx : (ey ? Ty : Tz);
-    int nxf, nyf, nzf;
-    if (ex) nxf = (stx > 0) ? (hix - ix) : (ix - lox + 1);
-    else nxf = faces_before(ix, stx, px, ivx, ux, (stx > 0) ? (hix - 1 - ix) : (ix - lox), Te, true);
-    if (ey) nyf = (sty > 0) ? (hiy - iy) : (iy - loy + 1);
-    else nyf = faces_before(iy, sty, py, ivy, uy, (sty > 0) ? (hiy - 1 - iy) : (iy - loy), Te, ez);
-    if (ez) nzf = (stz > 0) ? (hiz - iz) : (iz - loz + 1);
-    else nzf = faces_before(iz, stz, pz, ivz, uz, (stz > 0) ? (hiz - 1 - iz) : (iz - loz), Te, false);
-    ix += stx * nxf;
-    iy += sty * nyf;
-    iz += stz * nzf;
+    // faces crossed on the exit axis, its box face included
+    const int ce = ex ? ix : (ey ? iy : iz), ste = ex ? stx : (ey ? sty : stz);
+    const int loe = ex ? lox : (ey ? loy : loz), hie = ex ? hix : (ey ? hiy : hiz);
+    const int ne = (ste > 0) ? (hie - ce) : (ce - loe + 1);
+    // the two other axes, in axis order: a1 = (x unless x exits, then y), a2 = (z unless z exits, then y).
+    // A face of a1 / a2 that ties with the exit face comes first when its axis comes first.
+    const int c1 = ex ? iy : ix, st1 = ex ? sty : stx, lo1 = ex ? loy : lox, hi1 = ex ? hiy : hix;
+    const double p1 = ex ? py : px, iv1 = ex ? ivy : ivx, u1 = ex ? uy : ux;
+    const int c2 = ez ? iy : iz, st2 = ez ? sty : stz, lo2 = ez ? loy : loz, hi2 = ez ? hiy : hiz;
+    const double p2 = ez ? py : pz, iv2 = ez ? ivy : ivz, u2 = ez ? uy : uz;
+    const int n1 = faces_before(c1, st1, p1, iv1, u1, (st1 > 0) ? (hi1 - 1 - c1) : (c1 - lo1), Te, !ex);
+    const int n2 = faces_before(c2, st2, p2, iv2, u2, (st2 > 0) ? (hi2 - 1 - c2) : (c2 - lo2), Te, ez);
+    ix += stx * (ex ? ne : n1);
+    iy += sty * (ey ? ne : (ex ? n1 : n2));
+    iz += stz * (ez ? ne : n2);
     tmx = face_t(ix, stx, px, ivx);
     tmy = face_t(iy, sty, py, ivy);
     tmz = face_t(iz, stz, pz, ivz);
     t = Te;
-    return (unsigned)(nxf + nyf + nzf);
+    return (unsigned)(ne + n1 + n2);
 }
 
 }  // namespace mcrt

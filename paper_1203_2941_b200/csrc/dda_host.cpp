@@ -68,7 +68,30 @@ int mcrt_dda_host_trace(int nx, int ny, int nz, const uint8_t *dusty, int msh, c
     for (;;) {
         if ((unsigned)ix >= (unsigned)nx || (unsigned)iy >= (unsigned)ny || (unsigned)iz >= (unsigned)nz) break;
         const bool d = dusty[((size_t)iz * ny + iy) * nx + ix] != 0;
-        if (use_jumps && !d && M.empty(0, ix, iy, iz)) {
+        if (use_jumps == 2 && !d && M.empty(0, ix, iy, iz)) {
+            // the kernel's box: cube of bricks closer (max norm) than the nearest brick with dust
+            const int bx = ix >> msh, by = iy >> msh, bz = iz >> msh;
+            int dd = 255;
+            for (int z = 0; z < M.mb[0][2]; ++z)
+                for (int y = 0; y < M.mb[0][1]; ++y)
+                    for (int x = 0; x < M.mb[0][0]; ++x)
+                        if (!M.m[0][((size_t)z * M.mb[0][1] + y) * M.mb[0][0] + x]) {
+                            const int ax = x > bx ? x - bx : bx - x, ay = y > by ? y - by : by - y, az = z > bz ? z - bz : bz - z;
+                            const int m = ax > ay ? (ax > az ? ax : az) : (ay > az ? ay : az);
+                            if (m < dd) dd = m;
+                        }
+            dd -= 1;
+            const int lox = ((bx - dd) << msh) > 0 ? ((bx - dd) << msh) : 0, loy = ((by - dd) << msh) > 0 ? ((by - dd) << msh) : 0,
+                      loz = ((bz - dd) << msh) > 0 ? ((bz - dd) << msh) : 0;
+            const int hix = ((bx + dd + 1) << msh) < nx ? ((bx + dd + 1) << msh) : nx,
+                      hiy = ((by + dd + 1) << msh) < ny ? ((by + dd + 1) << msh) : ny,
+                      hiz = ((bz + dd + 1) << msh) < nz ? ((bz + dd + 1) << msh) : nz;
+            nf += mcrt::box_jump(ix, iy, iz, tmx, tmy, tmz, t, p[0], p[1], p[2], ivx, ivy, ivz, u[0], u[1], u[2], stx,
+                                 sty, stz, lox, loy, loz, hix, hiy, hiz);
+            ++nj;
+            continue;
+        }
+        if (use_jumps == 1 && !d && M.empty(0, ix, iy, iz)) {
             int sh = msh;
             if (M.empty(2, ix, iy, iz)) sh = msh + 4;
             else if (M.empty(1, ix, iy, iz)) sh = msh + 2;

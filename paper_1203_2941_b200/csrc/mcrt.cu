@@ -36,7 +36,7 @@ constexpr double kFourPi = 12.566370614359172953850573533118;
 
 constexpr unsigned kFull = 0xffffffffu;
 
-enum : int { ST_IDLE = 0, ST_EMIT = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4 };
+enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4 };
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
 
 // device counters (unsigned long long each)
@@ -65,8 +65,10 @@ struct mcrt_ctx {
     std::vector<void *> owned;       // cudaMalloc'ed blocks when no workspace was given
     // device arrays
     unsigned long long *cellw = nullptr;  // [ncp] packed cell words (see "Packed cell word")
-    uint32_t *vmask = nullptr;            // vacuum masks, three levels back to back
-    int msh = 2, mbx[3] = {0, 0, 0}, mby[3] = {0, 0, 0}, mbz[3] = {0, 0, 0}, moff[3] = {0, 0, 0}, mwords = 0;
+    uint32_t *vmask = nullptr;            // vacuum mask: one bit per brick
+    uint4 *vbox = nullptr;                // [bricks] a large box of empty bricks around every empty brick
+    int *vsat = nullptr;                  // scratch: summed-area table of dusty bricks
+    int msh = 2, mwords = 0;              // log2 brick edge; 32-bit words of the mask
     long long *lfx = nullptr;             // [ncp] Lucy fixed-point tally
     unsigned long long *kabs_cnt = nullptr, *kprev = nullptr;  // [ncp]
     void *scratch = nullptr;              // [nc*8 bytes]
@@ -235,13 +237,14 @@ struct TransportParams {
     unsigned long long *__restrict__ kcnt;
     const double *__restrict__ kext_h, *__restrict__ kabs_fx, *__restrict__ albedo, *__restrict__ g;
     const double *__restrict__ srccdf, *__restrict__ cdf, *__restrict__ mu_edges;
-    const uint32_t *__restrict__ vmask;   // the three levels, back to back
+    const uint32_t *__restrict__ vmask;   // one bit per brick: every cell of the brick has rho == 0
+    const uint4 *__restrict__ vbox;       // per empty brick: box of empty bricks {lox|loy<<16, loz|hix<<16, hiy|hiz<<16, -}
     unsigned long long *__restrict__ sed, *__restrict__ sed_direct, *__restrict__ counters;
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
     int nbx, nby;       // bricks per axis
     int bsh;            // log2 of the brick edge
-    int m0words;        // 32-bit words of the level-0 mask
+    int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
     unsigned long long pid0, count;
     uint32_t seed_lo, seed_hi, pass;
@@ -258,6 +261,7 @@ __device__ __forceinline__ uint32_t cell_in_brick(uint32_t brick, int ix, int iy
     return (((brick << bsh) | (uint32_t)(iz & m)) << (2 * bsh)) | (uint32_t)(((iy & m) << bsh) | (ix & m));
 }
 __device__ __forceinline__ bool brick_empty(const uint32_t *m0, uint32_t brick) { return (m0[brick >> 5] >> (brick & 31u)) & 1u; }
+
 
 // S5 Lucy path-length tally: L[c] += rint(x), x = kabs h rho ds 2^FX >= 0 (Eq. 9, linear form;
 // PAPER.md:142 integer atomics).  rint by the 1.5 * 2^52 trick: round to nearest even, exact below 2^51, and
@@ -294,6 +298,8 @@ constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_IVX, F_IVY, F_IVZ, F_T, F_TAU, F_ZTYPE, F_CW, F_HASH, F_PID };
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
+// ring word that stands for "this cell lies in an empty brick": no real cell word has bit 28 set with rho = 0
+constexpr unsigned long long kJumpWord = 0x10000000ull;
 
 // position of the n-th set bit (n = 0, 1, ...) of a 64-bit mask; n < popc(m)
 __device__ __forceinline__ int nth_set64(unsigned long long m, int n)
@@ -347,7 +353,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     const int nhist = 2 * P.ndir * P.nf;
     uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
     // cell-word ring: slot k of thread i at s_ring[k * blockDim.x + i]
-    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.m0words + 1) & ~1));
+    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.mwords + 1) & ~1));
+
     volatile unsigned long long *ring = s_ring + threadIdx.x;
     const int ring_stride = blockDim.x;
 
@@ -358,7 +365,7 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     for (int i = threadIdx.x; i < P.nf; i += blockDim.x) s_src[i] = P.srccdf[i];
     for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
-    for (int i = threadIdx.x; i < P.m0words; i += blockDim.x) s_m0[i] = P.vmask[i];
+    for (int i = threadIdx.x; i < P.mwords; i += blockDim.x) s_m0[i] = P.vmask[i];
     if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0ull;
     __syncthreads();
 
@@ -372,13 +379,14 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     // every slot starts as "emit the next packet"
     for (int s = lane; s < kSlots; s += 32) SU(U_DK, s) = K_EMIT << 30;
     __syncwarp();
-    unsigned long long mFly = 0ull, mEv = ~0ull;   // warp-uniform: parked flying packets / packets waiting for an event
+    // warp-uniform slot sets: parked flying packets / packets inside a run of empty bricks / packets waiting for an event
+    unsigned long long mFly = 0ull, mJ = 0ull, mEv = ~0ull;
     bool exhausted = false;                        // the epoch counter has run out (warp-uniform)
     unsigned long long ndusty_acc = 0ull;          // dusty crossings stepped by this lane
 
     for (;;) {
-        const int nfly = __popcll(mFly);
-        if (nfly >= 32 || (nfly > 0 && mEv == 0ull)) {
+        const int nfly = __popcll(mFly), njmp = __popcll(mJ), nevt = __popcll(mEv);
+        if (nfly >= 32 || (nfly > 0 && njmp == 0 && nevt == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
             // (G: axis choice, next cell, exit parameter) runs kAhead = 2 cells ahead of the physics and the
@@ -415,7 +423,7 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                     const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);
                     gcidx = cell_in_brick(brick, gx, gy, gz, bsh);
                     if (!brick_empty(s_m0, brick)) cp_async8(const_cast<unsigned long long *>(ring) + rs * ring_stride, P.cellw + gcidx);
-                    else ring[rs * ring_stride] = 0ull;
+                    else ring[rs * ring_stride] = kJumpWord;
                 }
             };
 
@@ -457,6 +465,9 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                     if (!o2) advance(tn2, o3, (r + 3) & 3);
                     cp_async_commit();
                     // physics of cell n
+                    if (cw == kJumpWord) {
+                        state = ST_JUMP;                   // cell n starts a run of empty bricks: J phase
+                    } else {
                     const double ds = tn0 - t;
                     const double rho_c = cw_rho(cw);
                     const double2 kq = s_kk[cw_species(cw) * nf + j];
@@ -480,6 +491,7 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                             r = (r + 1) & 3;
                         }
                     }
+                    }
                 }
                 if (__popc(__ballot_sync(kFull, state == ST_FLY)) <= stop_at) break;
             }
@@ -491,11 +503,73 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 SU(U_W0, slot) = xy0;
                 SU(U_W1, slot) = z0 | ((uint32_t)j << 16);
                 SU(U_NCROSS, slot) = ncross;
-                if (state != ST_FLY)
+                if (state == ST_DONE || state == ST_INTERACT)
                     SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
             }
             mFly |= warp_or64((act && state == ST_FLY) ? (1ull << slot) : 0ull);
-            mEv |= warp_or64((act && state != ST_FLY) ? (1ull << slot) : 0ull);
+            mJ |= warp_or64((act && state == ST_JUMP) ? (1ull << slot) : 0ull);
+            mEv |= warp_or64((act && (state == ST_DONE || state == ST_INTERACT)) ? (1ull << slot) : 0ull);
+            __syncwarp();
+        } else if (njmp > 0 && njmp >= nevt) {
+            // =========================================================== J phase: runs of empty bricks
+            // Each lane takes one packet whose current cell lies in an empty brick and crosses, one box per
+            // step, the largest aligned empty box around it (mcrt::box_jump, identical to the cell-by-cell
+            // walk: same faces, same count, same exit parameter) until it reaches a brick that holds dust or
+            // leaves the grid.  No global memory is touched on the way.
+            const int nj = min(njmp, 32);
+            const bool act = lane < nj;
+            const int slot = act ? nth_set64(mJ, lane) : 0;
+            bool busy = act, escaped = false;
+            double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, ux = 0.0, uy = 0.0, uz = 0.0;
+            double tmx = 0.0, tmy = 0.0, tmz = 0.0, t = 0.0;
+            int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0;
+            uint32_t ncross = 0u, w1 = 0u;
+            if (act) {
+                px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
+                ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+                ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+                t = SF(F_T, slot);
+                const uint32_t w0 = SU(U_W0, slot);
+                w1 = SU(U_W1, slot);
+                ncross = SU(U_NCROSS, slot);
+                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu);
+                stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
+                sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
+                stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
+                tmx = mcrt::face_t(ix, stx, px, ivx);
+                tmy = mcrt::face_t(iy, sty, py, ivy);
+                tmz = mcrt::face_t(iz, stz, pz, ivz);
+            }
+            while (__any_sync(kFull, busy)) {
+                if (busy) {
+                    // the precomputed box of empty bricks around this brick, in cells, clipped to the grid
+                    const uint4 bb = __ldg(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
+                    const int lox = (int)(bb.x & 0xffffu) << bsh, loy = (int)(bb.x >> 16) << bsh, loz = (int)(bb.y & 0xffffu) << bsh;
+                    const int hix = min((int)(bb.y >> 16) << bsh, P.nx), hiy = min((int)(bb.z & 0xffffu) << bsh, P.ny),
+                              hiz = min((int)(bb.z >> 16) << bsh, P.nz);
+                    ncross += mcrt::box_jump(ix, iy, iz, tmx, tmy, tmz, t, px, py, pz, ivx, ivy, ivz, ux, uy, uz,
+                                             stx, sty, stz, lox, loy, loz, hix, hiy, hiz);
+                    escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) |
+                              ((unsigned)iz >= (unsigned)P.nz);
+                    busy = !escaped && brick_empty(s_m0, brick_of(ix, iy, iz, nbx, nby, bsh));
+                }
+            }
+            if (act) {
+                SF(F_T, slot) = t;
+                SU(U_NCROSS, slot) = ncross;
+                if (escaped) {
+                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                } else {
+                    SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
+                    SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | (w1 & 0xffff0000u);
+                    const uint32_t cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                    SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + cidx));
+                }
+            }
+            const unsigned long long mine = act ? (1ull << slot) : 0ull;
+            mJ &= ~warp_or64(mine);
+            mEv |= warp_or64(escaped ? mine : 0ull);
+            mFly |= warp_or64((act && !escaped) ? mine : 0ull);
             __syncwarp();
         } else if (mEv != 0ull) {
             // =========================================================== E phase: one event per lane
@@ -556,6 +630,7 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 }
                 if (__any_sync(kFull, dead)) exhausted = true;   // the counter only grows
             }
+            bool to_jump = false;                       // the new flight starts in an empty brick
             if (act && !dead) {
                 double px, py, pz, z0, z1;
                 bool scatter = false;
@@ -649,7 +724,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                     f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
                     const uint32_t brick = brick_of(ix, iy, iz, nbx, nby, bsh);
                     cidx = cell_in_brick(brick, ix, iy, iz, bsh);
-                    cw = brick_empty(s_m0, brick) ? 0ull : __ldg(P.cellw + cidx);
+                    to_jump = brick_empty(s_m0, brick);
+                    cw = to_jump ? 0ull : __ldg(P.cellw + cidx);
                     if (RECORD)
                         hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
                 }
@@ -674,7 +750,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             }
             const unsigned long long mine = act ? (1ull << slot) : 0ull;
             mEv &= ~warp_or64(mine);                       // taken: now flying, or dead (no packets left)
-            mFly |= warp_or64(dead ? 0ull : mine);
+            mFly |= warp_or64((dead || to_jump) ? 0ull : mine);
+            mJ |= warp_or64((!dead && to_jump) ? mine : 0ull);
             __syncwarp();
         } else {
             break;
@@ -838,20 +915,66 @@ __global__ void k_build_mask0(const unsigned long long *__restrict__ cellw, uint
     }
 }
 
-__global__ void k_build_mask_up(const uint32_t *__restrict__ lower, uint32_t *__restrict__ m, int lbx, int lby, int lbz,
-                                int mbx, int mby, int mbz)
+// Empty boxes for the J phase.  sat[z][y][x] (dims nb+1) = number of dusty bricks in [0,x) x [0,y) x [0,z): built
+// by three prefix passes; k_grow_boxes then grows, for every empty brick, a box of empty bricks around it: the
+// six faces are pushed out one layer at a time, round robin, as long as the added layer holds no dust (one
+// summed-area query each), so the box first grows like a cube and then keeps extending where space is left.
+__global__ void k_sat_pass(const uint32_t *__restrict__ mask, int *__restrict__ sat, int nbx, int nby, int nbz, int axis)
 {
-    const int nb = mbx * mby * mbz;
+    const int sx = nbx + 1, sy = nby + 1;
+    const int n1 = axis == 0 ? nby : nbx, n2 = axis == 2 ? nby : nbz;   // the two axes a thread does not scan
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n1 * n2; i += gridDim.x * blockDim.x) {
+        const int a = i % n1, b = i / n1;
+        int run = 0;
+        if (axis == 0) {
+            for (int x = 0; x < nbx; ++x) {
+                const int o = (b * nby + a) * nbx + x;
+                run += ((mask[o >> 5] >> (o & 31)) & 1u) ? 0 : 1;
+                sat[((size_t)(b + 1) * sy + (a + 1)) * sx + (x + 1)] = run;
+            }
+        } else if (axis == 1) {
+            for (int y = 0; y < nby; ++y) {
+                int *q = sat + ((size_t)(b + 1) * sy + (y + 1)) * sx + (a + 1);
+                run += *q; *q = run;
+            }
+        } else {
+            for (int z = 0; z < nbz; ++z) {
+                int *q = sat + ((size_t)(z + 1) * sy + (b + 1)) * sx + (a + 1);
+                run += *q; *q = run;
+            }
+        }
+    }
+}
+
+__device__ __forceinline__ int sat_count(const int *__restrict__ sat, int sx, int sy, int x0, int y0, int z0, int x1, int y1, int z1)
+{
+#define SAT_(x, y, z) sat[((size_t)(z) * sy + (y)) * sx + (x)]
+    return SAT_(x1, y1, z1) - SAT_(x0, y1, z1) - SAT_(x1, y0, z1) - SAT_(x1, y1, z0) + SAT_(x0, y0, z1) + SAT_(x0, y1, z0) +
+           SAT_(x1, y0, z0) - SAT_(x0, y0, z0);
+#undef SAT_
+}
+
+__global__ void k_grow_boxes(const uint32_t *__restrict__ mask, const int *__restrict__ sat, uint4 *__restrict__ box, int nbx,
+                             int nby, int nbz)
+{
+    const int nb = nbx * nby * nbz, sx = nbx + 1, sy = nby + 1;
     for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
-        const int bx = b % mbx, by = (b / mbx) % mby, bz = b / (mbx * mby);
-        bool empty = true;
-        for (int z = bz * 4; z < min(bz * 4 + 4, lbz) && empty; ++z)
-            for (int y = by * 4; y < min(by * 4 + 4, lby) && empty; ++y)
-                for (int x = bx * 4; x < min(bx * 4 + 4, lbx); ++x) {
-                    const int c = (z * lby + y) * lbx + x;
-                    if (!((lower[c >> 5] >> (c & 31)) & 1u)) { empty = false; break; }
-                }
-        if (empty) atomicOr(&m[b >> 5], 1u << (b & 31));
+        int x0 = b % nbx, y0 = (b / nbx) % nby, z0 = b / (nbx * nby);
+        int x1 = x0 + 1, y1 = y0 + 1, z1 = z0 + 1;
+        if ((mask[b >> 5] >> (b & 31)) & 1u) {
+            bool grew = true;
+            while (grew) {
+                grew = false;
+                if (x0 > 0 && sat_count(sat, sx, sy, x0 - 1, y0, z0, x0, y1, z1) == 0) { --x0; grew = true; }
+                if (x1 < nbx && sat_count(sat, sx, sy, x1, y0, z0, x1 + 1, y1, z1) == 0) { ++x1; grew = true; }
+                if (y0 > 0 && sat_count(sat, sx, sy, x0, y0 - 1, z0, x1, y0, z1) == 0) { --y0; grew = true; }
+                if (y1 < nby && sat_count(sat, sx, sy, x0, y1, z0, x1, y1 + 1, z1) == 0) { ++y1; grew = true; }
+                if (z0 > 0 && sat_count(sat, sx, sy, x0, y0, z0 - 1, x1, y1, z0) == 0) { --z0; grew = true; }
+                if (z1 < nbz && sat_count(sat, sx, sy, x0, y0, z1, x1, y1, z1 + 1) == 0) { ++z1; grew = true; }
+            }
+        }
+        box[b] = make_uint4((uint32_t)x0 | ((uint32_t)y0 << 16), (uint32_t)z0 | ((uint32_t)x1 << 16),
+                            (uint32_t)y1 | ((uint32_t)z1 << 16), 0u);
     }
 }
 
@@ -975,7 +1098,7 @@ size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threa
 // Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
 // which level 0 fits 32 KB of shared memory; each further level is 4x coarser per axis.
 struct MaskGeom {
-    int msh, mbx[3], mby[3], mbz[3], moff[3], mwords;
+    int msh, nbx, nby, nbz, mwords;
 };
 
 MaskGeom mask_geom(int nx, int ny, int nz)
@@ -988,14 +1111,9 @@ MaskGeom mask_geom(int nx, int ny, int nz)
         if (bits <= ((size_t)1 << 18)) break;
         ++g.msh;
     }
-    int off = 0;
-    for (int l = 0; l < 3; ++l) {
-        const int e = 1 << (g.msh + 2 * l);
-        g.mbx[l] = (nx + e - 1) / e; g.mby[l] = (ny + e - 1) / e; g.mbz[l] = (nz + e - 1) / e;
-        g.moff[l] = off;
-        off += (g.mbx[l] * g.mby[l] * g.mbz[l] + 31) / 32;
-    }
-    g.mwords = off;
+    const int e = 1 << g.msh;
+    g.nbx = (nx + e - 1) / e; g.nby = (ny + e - 1) / e; g.nbz = (nz + e - 1) / e;
+    g.mwords = (g.nbx * g.nby * g.nbz + 31) / 32;
     return g;
 }
 
@@ -1033,11 +1151,14 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     if (!bytes_out || nx < 1 || ny < 1 || nz < 1 || n_species < 1 || n_nu < 2 || n_T < 2 || n_dir < 1) return MCRT_EINVAL;
     const size_t nc = (size_t)nx * ny * nz;
     const MaskGeom mg = mask_geom(nx, ny, nz);
-    const size_t ncp = ((size_t)mg.mbx[0] * mg.mby[0] * mg.mbz[0]) << (3 * mg.msh);
+    const size_t nbricks = (size_t)mg.nbx * mg.nby * mg.nbz;
+    const size_t ncp = nbricks << (3 * mg.msh);
     size_t b = 0;
     auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
     add(ncp * sizeof(uint2));            // cell words
-    add((size_t)mg.mwords * 4);          // vacuum masks
+    add((size_t)mg.mwords * 4);          // vacuum mask
+    add(nbricks * sizeof(uint4));        // empty boxes of the J phase
+    add((size_t)(mg.nbx + 1) * (mg.nby + 1) * (mg.nbz + 1) * sizeof(int));   // summed-area scratch
     add(ncp * sizeof(long long));        // Lucy tally
     add(ncp * sizeof(long long));        // k
     add(ncp * sizeof(long long));        // k_prev
@@ -1075,11 +1196,10 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     cudaGetDevice(&c->device);
     c->nx = nx; c->ny = ny; c->nz = nz; c->ns = n_species; c->h = cell_size_cm;
     {
-        const MaskGeom g = mask_geom(nx, ny, nz);   // a brick is a level-0 mask box
+        const MaskGeom g = mask_geom(nx, ny, nz);
         c->msh = g.msh; c->mwords = g.mwords;
-        for (int l = 0; l < 3; ++l) { c->mbx[l] = g.mbx[l]; c->mby[l] = g.mby[l]; c->mbz[l] = g.mbz[l]; c->moff[l] = g.moff[l]; }
+        c->nbx = g.nbx; c->nby = g.nby; c->nbz = g.nbz;
     }
-    c->nbx = c->mbx[0]; c->nby = c->mby[0]; c->nbz = c->mbz[0];
     c->nc = (size_t)nx * ny * nz;
     c->ncp = ((size_t)c->nbx * c->nby * c->nbz) << (3 * c->msh);
     c->ws = (char *)workspace; c->ws_bytes = workspace_bytes; c->ws_owned_by_caller = workspace != nullptr;
@@ -1100,6 +1220,8 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     } while (0)
     GC_TRY(ws_alloc(c, (void **)&c->cellw, c->ncp * sizeof(uint2)));
     GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
+    GC_TRY(ws_alloc(c, (void **)&c->vbox, (size_t)c->nbx * c->nby * c->nbz * sizeof(uint4)));
+    GC_TRY(ws_alloc(c, (void **)&c->vsat, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int)));
     GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
@@ -1120,12 +1242,16 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
                                                            c->msh, n_species, bad);
     GC_CUDA(cudaGetLastError());
     GC_CUDA(cudaMemsetAsync(c->vmask, 0, (size_t)c->mwords * 4, c->stream));
-    k_build_mask0<<<stream_grid((size_t)c->mbx[0] * c->mby[0] * c->mbz[0]), 256, 0, c->stream>>>(
-        c->cellw, c->vmask + c->moff[0], nx, ny, nz, c->nbx, c->nby, c->msh, c->mbx[0], c->mby[0], c->mbz[0]);
-    for (int l = 1; l < 3; ++l)
-        k_build_mask_up<<<stream_grid((size_t)c->mbx[l] * c->mby[l] * c->mbz[l]), 256, 0, c->stream>>>(
-            c->vmask + c->moff[l - 1], c->vmask + c->moff[l], c->mbx[l - 1], c->mby[l - 1], c->mbz[l - 1], c->mbx[l],
-            c->mby[l], c->mbz[l]);
+    {
+        const size_t nbr = (size_t)c->nbx * c->nby * c->nbz;
+        k_build_mask0<<<stream_grid(nbr), 256, 0, c->stream>>>(c->cellw, c->vmask, nx, ny, nz, c->nbx, c->nby, c->msh, c->nbx,
+                                                             c->nby, c->nbz);
+        GC_CUDA(cudaMemsetAsync(c->vsat, 0, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int), c->stream));
+        k_sat_pass<<<stream_grid((size_t)c->nby * c->nbz), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 0);
+        k_sat_pass<<<stream_grid((size_t)c->nbx * c->nbz), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 1);
+        k_sat_pass<<<stream_grid((size_t)c->nbx * c->nby), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 2);
+        k_grow_boxes<<<stream_grid(nbr), 256, 0, c->stream>>>(c->vmask, c->vsat, c->vbox, c->nbx, c->nby, c->nbz);
+    }
     GC_CUDA(cudaGetLastError());
     GC_CUDA(cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
     GC_CUDA(cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
@@ -1173,7 +1299,7 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
         if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
         if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
     }
-    if (transport_smem_bytes(ns, n_nu, 16, c->moff[1], 256) > 220 * 1024)
+    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256) > 220 * 1024)
         return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
     c->nf = n_nu; c->nT = n_T;
     c->nu.assign(nu_hz, nu_hz + n_nu);
@@ -1304,8 +1430,8 @@ static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, in
     *threads = (o && o->block_threads > 0) ? o->block_threads : 512;
     if (*threads % 32 || *threads > 512 || *threads < 32) return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32..512");
     // as many warps (each with its packet pool) as fit beside the tables in 227 KB of shared memory
-    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->moff[1], *threads) > 227 * 1024) *threads -= 32;
-    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->moff[1], *threads);
+    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads) > 227 * 1024) *threads -= 32;
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads);
     if (*smem > 48 * 1024) {
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
@@ -1415,7 +1541,7 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
     P.dig = o.record_digests ? c->dig : nullptr;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
     P.nbx = c->nbx; P.nby = c->nby;
-    P.vmask = c->vmask; P.bsh = c->msh; P.m0words = c->moff[1];
+    P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords;
     P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     const size_t j_smem = (size_t)c->ns * c->nT * 8;

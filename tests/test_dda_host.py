@@ -49,7 +49,7 @@ def _start_cell(p, u):
 def test_jump_walk_equals_cell_walk_random(orc, dda):
     rng = np.random.default_rng(7)
     total_jumps = 0
-    for case in range(400):
+    for case in range(300):
         n = rng.integers(1, 41, 3)
         msh = int(rng.integers(2, 4))
         fill = rng.choice([0.0, 0.002, 0.02, 0.3])
@@ -87,6 +87,10 @@ def test_jump_walk_equals_cell_walk_random(orc, dda):
             keep = dusty.reshape(-1)[cells_o] != 0
             cells_j, ds_j, faces, te, nj = dda(n, dusty, msh, p, u, c0)
             cells_s, ds_s, faces_s, te_s, nj_s = dda(n, dusty, msh, p, u, c0, use_jumps=0)
+            cells_c, ds_c, faces_c, te_c, nj_c = dda(n, dusty, msh, p, u, c0, use_jumps=2)   # distance-map cubes
+            assert faces_c == faces and np.array_equal(cells_c, cells_j), (case, p, u)
+            assert np.array_equal(ds_c.view(np.uint64), ds_j.view(np.uint64)), (case, p, u)
+            assert np.float64(te_c).view(np.uint64) == np.float64(te_s).view(np.uint64), (case, p, u)
             assert nj_s == 0 and faces_s == len(cells_o) == faces, (case, p, u)
             assert np.array_equal(cells_j, cells_o[keep]), (case, p, u)
             assert np.array_equal(ds_j.view(np.uint64), ds_o[keep].view(np.uint64)), (case, p, u)
