@@ -292,12 +292,27 @@ constexpr int kSlotF64 = 15;        // 8-byte fields per slot
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
 #ifndef MCRT_SWAP_MIN
-#define MCRT_SWAP_MIN 8             // an S phase ends when this many of its packets wait for an event
+#define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
+#endif
+#ifndef MCRT_S_ENTER
+#define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
+#endif
+#ifndef MCRT_S_LEAVE
+#define MCRT_S_LEAVE 8              // ... and ends when this many lanes are idle and nothing is left to refill them
+#endif
+#ifndef MCRT_J_MIN
+#define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
 #endif
 
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_IVX, F_IVY, F_IVZ, F_T, F_TAU, F_ZTYPE, F_CW, F_HASH, F_PID };
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
+constexpr uint32_t kOutCell = 0xffffffffu;   // storage index of "outside the grid"
+// cell coordinates packed in 32 bits: x, y < 2048, z < 1024
+__device__ __forceinline__ uint32_t pack_xyz(int x, int y, int z) { return (uint32_t)x | ((uint32_t)y << 11) | ((uint32_t)z << 22); }
+__device__ __forceinline__ int unpack_x(uint32_t w) { return (int)(w & 0x7ffu); }
+__device__ __forceinline__ int unpack_y(uint32_t w) { return (int)((w >> 11) & 0x7ffu); }
+__device__ __forceinline__ int unpack_z(uint32_t w) { return (int)(w >> 22); }
 // ring word that stands for "this cell lies in an empty brick": no real cell word has bit 28 set with rho = 0
 constexpr unsigned long long kJumpWord = 0x10000000ull;
 
@@ -382,133 +397,155 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     // warp-uniform slot sets: parked flying packets / packets inside a run of empty bricks / packets waiting for an event
     unsigned long long mFly = 0ull, mJ = 0ull, mEv = ~0ull;
     bool exhausted = false;                        // the epoch counter has run out (warp-uniform)
-    unsigned long long ndusty_acc = 0ull;          // dusty crossings stepped by this lane
+    uint32_t ndusty_acc = 0u;                      // dusty crossings stepped by this lane
 
     for (;;) {
         const int nfly = __popcll(mFly), njmp = __popcll(mJ), nevt = __popcll(mEv);
-        if (nfly >= 32 || (nfly > 0 && njmp == 0 && nevt == 0)) {
+        if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
-            // (G: axis choice, next cell, exit parameter) runs kAhead = 2 cells ahead of the physics and the
-            // cell words travel global -> shared memory with cp.async into a small per-thread ring: the latency
-            // of a cell's word is covered by two walk iterations of every resident warp.
-            const int nact = min(nfly, 32);
-            const bool act = lane < nact;
+            // (G: axis choice, next cell, exit parameter) runs two cells ahead of the physics and the cell words
+            // travel global -> shared memory with cp.async into a small per-thread ring: the latency of a
+            // cell's word is covered by two walk iterations of every resident warp.  The queue between G and
+            // the physics (exit parameter, storage index, packed coordinates of cells n and n+1) rotates through
+            // three register sets A, B, C, so the loop body is three steps and nothing is moved.
+            // Lanes whose packet reaches an event or an empty brick park it and take another flying packet
+            // from the pool without leaving the loop; a new packet enters the pipeline behind two no-op cells
+            // (zero length, vacuum), which the physics passes without effect.  The phase ends when the pool has
+            // no flying packet left for MCRT_S_LEAVE idle lanes.
             int slot = 0, state = ST_IDLE;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
-            double t = 0.0, tau = 0.0, tn0 = 0.0, tn1 = 0.0;
+            double t = 0.0, tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;
             int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-            uint32_t xy0 = 0u, xy1 = 0u, z0 = 0u, z1 = 0u;      // packed coordinates of cells n, n+1
-            uint32_t cidx0 = 0u, cidx1 = 0u, gcidx = 0u, ncross = 0u;
-            bool o1 = true, o2 = true;                          // cell n+1 / n+2 lies outside the grid
+            uint32_t ciA = 0u, ciB = 0u, ciC = 0u, xzA = 0u, xzB = 0u, xzC = 0u;   // storage index, packed coordinates
+            uint32_t gcidx = 0u, ncross = 0u, pk_xyz = 0u;
+            unsigned long long pk_cw = 0ull;
             int r = 0;                                          // ring slot of cell n
+            int nidle = 32;
+            bool first = true;
 
-            // advance G by one cell: returns the exit parameter of the cell it leaves, requests the word of
-            // the cell it enters (ring slot rs) unless that cell is outside the grid or in an empty brick
-            auto advance = [&](double &tn_left, bool &entered_out, int rs) {
-                const bool selx = (tmx <= tmy) && (tmx <= tmz);
-                const bool sely = !selx && (tmy <= tmz);
-                const bool selz = !selx && !sely;
-                tn_left = selx ? tmx : (sely ? tmy : tmz);
-                gx += selx ? stx : 0;
-                gy += sely ? sty : 0;
-                gz += selz ? stz : 0;
-                // parameter of the face through which the entered cell will be left (reading Q8)
-                if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;
-                if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;
-                if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;
-                entered_out = ((unsigned)gx >= (unsigned)P.nx) | ((unsigned)gy >= (unsigned)P.ny) |
-                              ((unsigned)gz >= (unsigned)P.nz);
-                if (!entered_out) {
-                    const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);
-                    gcidx = cell_in_brick(brick, gx, gy, gz, bsh);
-                    if (!brick_empty(s_m0, brick)) cp_async8(const_cast<unsigned long long *>(ring) + rs * ring_stride, P.cellw + gcidx);
-                    else ring[rs * ring_stride] = kJumpWord;
+            // one step: G advances one cell (queue entry 2 receives the cell G leaves), the physics handles cell n
+            // (queue entry 0; entry 1 only tells whether cell n+1 is outside the grid)
+            auto step = [&](const double tn0, const uint32_t ci0, const uint32_t xz0, const uint32_t ci1, double &tn2,
+                            uint32_t &ci2, uint32_t &xz2) {
+                cp_async_wait<2>();                               // the word of cell n has landed
+                const unsigned long long cw = ring[r * ring_stride];
+                ci2 = gcidx;
+                xz2 = pack_xyz(gx, gy, gz);
+                if (gcidx != kOutCell) {
+                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
+                    const bool sely = !selx && (tmy <= tmz);
+                    const bool selz = !selx && !sely;
+                    tn2 = selx ? tmx : (sely ? tmy : tmz);
+                    gx += selx ? stx : 0;
+                    gy += sely ? sty : 0;
+                    gz += selz ? stz : 0;
+                    // parameter of the face through which the entered cell will be left (reading Q8)
+                    if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;
+                    if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;
+                    if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;
+                    gcidx = kOutCell;
+                    if (((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) & ((unsigned)gz < (unsigned)P.nz)) {
+                        const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);
+                        gcidx = cell_in_brick(brick, gx, gy, gz, bsh);
+                        unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;
+                        if (!brick_empty(s_m0, brick)) cp_async8(dst, P.cellw + gcidx);
+                        else *reinterpret_cast<volatile unsigned long long *>(dst) = kJumpWord;
+                    }
                 }
-            };
-
-            if (act) {
-                slot = nth_set64(mFly, lane);
-                px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
-                ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
-                t = SF(F_T, slot); tau = SF(F_TAU, slot);
-                ring[0] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
-                ncross = SU(U_NCROSS, slot);
-                gx = (int)(w0 & 0xffffu); gy = (int)(w0 >> 16); gz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
-                // the stored 1/u is +inf for a zero direction component: that axis never moves
-                stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
-                sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
-                stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
-                tmx = mcrt::face_t(gx, stx, px, ivx);
-                tmy = mcrt::face_t(gy, sty, py, ivy);
-                tmz = mcrt::face_t(gz, stz, pz, ivz);
-                xy0 = w0; z0 = w1 & 0xffffu;
-                cidx0 = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
-                advance(tn0, o1, 1);                              // G: cell n -> n+1
                 cp_async_commit();
-                xy1 = (uint32_t)(gx & 0xffff) | ((uint32_t)gy << 16); z1 = (uint32_t)gz; cidx1 = gcidx;
-                if (!o1) advance(tn1, o2, 2);                     // G: cell n+1 -> n+2
-                cp_async_commit();
-                state = ST_FLY;
-            }
-            mFly &= ~warp_or64(act ? (1ull << slot) : 0ull);
-            const int stop_at = max(nact - MCRT_SWAP_MIN, 0);
-            for (;;) {
-                if (state == ST_FLY) {
-                    cp_async_wait<2>();                           // the word of cell n has landed
-                    const unsigned long long cw = ring[r * ring_stride];
-                    // G: cell n+2 -> n+3 (keeps two requests in flight)
-                    const uint32_t xy2 = (uint32_t)(gx & 0xffff) | ((uint32_t)gy << 16), z2 = (uint32_t)gz, cidx2 = gcidx;
-                    double tn2 = 0.0;
-                    bool o3 = true;
-                    if (!o2) advance(tn2, o3, (r + 3) & 3);
-                    cp_async_commit();
-                    // physics of cell n
-                    if (cw == kJumpWord) {
-                        state = ST_JUMP;                   // cell n starts a run of empty bricks: J phase
-                    } else {
+                // physics of cell n
+                if (cw == kJumpWord) {
+                    state = ST_JUMP;                           // cell n starts a run of empty bricks: J phase
+                    pk_xyz = xz0;
+                } else {
                     const double ds = tn0 - t;
                     const double rho_c = cw_rho(cw);
                     const double2 kq = s_kk[cw_species(cw) * nf + j];
-                    const double dtau = kq.x * rho_c * ds;  // tau_i = (kabs+ksca) h rho ds (Eq. 2)
+                    const double dtau = kq.x * rho_c * ds;      // tau_i = (kabs+ksca) h rho ds (Eq. 2)
                     if (dtau > tau) {
-                        state = ST_INTERACT;               // interaction inside this cell (equality leaves, Q5)
+                        state = ST_INTERACT;                   // interaction inside this cell (equality leaves, Q5)
+                        pk_xyz = xz0; pk_cw = cw;
                     } else {
                         tau -= dtau;
                         if (!cw_vacuum(cw)) {
-                            lucy_add(P.lfx, cidx0, kq.y * rho_c * ds);
+                            lucy_add(P.lfx, ci0, kq.y * rho_c * ds);
                             ndusty_acc++;
                         }
                         t = tn0;
                         ncross++;
-                        if (o1) {
-                            state = ST_DONE;               // left the grid: escape tally in the E phase
-                        } else {
-                            xy0 = xy1; z0 = z1; cidx0 = cidx1; tn0 = tn1;
-                            xy1 = xy2; z1 = z2; cidx1 = cidx2; tn1 = tn2;
-                            o1 = o2; o2 = o3;
-                            r = (r + 1) & 3;
-                        }
-                    }
+                        r = (r + 1) & 3;
+                        if (ci1 == kOutCell) state = ST_DONE;  // left the grid: escape tally in the E phase
                     }
                 }
-                if (__popc(__ballot_sync(kFull, state == ST_FLY)) <= stop_at) break;
+            };
+
+            for (;;) {
+                // ---- park packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
+                const int nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
+                if (first || nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) {
+                    first = false;
+                    const bool stopped = state != ST_FLY && state != ST_IDLE;
+                    if (stopped) {
+                        SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
+                        SF(F_CW, slot) = __longlong_as_double((long long)pk_cw);
+                        SU(U_W0, slot) = pk_xyz;
+                        SU(U_NCROSS, slot) = ncross;
+                        if (state != ST_JUMP)
+                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
+                    }
+                    mJ |= warp_or64(state == ST_JUMP ? (1ull << slot) : 0ull);
+                    mEv |= warp_or64((state == ST_DONE || state == ST_INTERACT) ? (1ull << slot) : 0ull);
+                    if (stopped) state = ST_IDLE;
+                    const unsigned idle = __ballot_sync(kFull, state == ST_IDLE);
+                    const int nfl = 32 - __popc(idle);
+                    // nothing left to refill with and many lanes idle: let the other phases make flying packets
+                    if (mFly == 0ull && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && (mJ | mEv) != 0ull))) {
+                        if (state == ST_FLY) {
+                            cp_async_wait<0>();
+                            SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
+                            SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
+                            SU(U_W0, slot) = xzA;
+                            SU(U_NCROSS, slot) = ncross;
+                        }
+                        mFly |= warp_or64(state == ST_FLY ? (1ull << slot) : 0ull);
+                        break;
+                    }
+                    const int k = __popc(idle & ((1u << lane) - 1u));
+                    const bool take = state == ST_IDLE && k < __popcll(mFly);
+                    if (take) {
+                        slot = nth_set64(mFly, k);
+                        cp_async_wait<0>();                       // no stale request may land in the ring later
+                        px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
+                        ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+                        t = SF(F_T, slot); tau = SF(F_TAU, slot);
+                        const uint32_t w0 = SU(U_W0, slot);
+                        j = (int)SU(U_W1, slot);
+                        ncross = SU(U_NCROSS, slot) - 2u;         // the two no-op cells below count themselves
+                        gx = unpack_x(w0); gy = unpack_y(w0); gz = unpack_z(w0);
+                        // the stored 1/u is +inf for a zero direction component: that axis never moves
+                        stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
+                        sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
+                        stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
+                        tmx = mcrt::face_t(gx, stx, px, ivx);
+                        tmy = mcrt::face_t(gy, sty, py, ivy);
+                        tmz = mcrt::face_t(gz, stz, pz, ivz);
+                        gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
+                        // pipeline: two no-op cells (zero length, vacuum word), then the packet's cell
+                        r = 0;
+                        ring[0] = 0ull; ring[ring_stride] = 0ull;
+                        ring[2 * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        tnA = t; tnB = t; ciA = 0u; ciB = 0u; xzA = w0; xzB = w0;
+                        state = ST_FLY;
+                    }
+                    mFly &= ~warp_or64(take ? (1ull << slot) : 0ull);
+                    nidle = __popc(__ballot_sync(kFull, state == ST_IDLE));
+                }
+                // ---- three steps
+                if (state == ST_FLY) step(tnA, ciA, xzA, ciB, tnC, ciC, xzC);
+                if (state == ST_FLY) step(tnB, ciB, xzB, ciC, tnA, ciA, xzA);
+                if (state == ST_FLY) step(tnC, ciC, xzC, ciA, tnB, ciB, xzB);
             }
-            cp_async_wait<0>();
-            // park: only what the walk changes (p, u, 1/u stay as the event left them)
-            if (act) {
-                SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
-                SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
-                SU(U_W0, slot) = xy0;
-                SU(U_W1, slot) = z0 | ((uint32_t)j << 16);
-                SU(U_NCROSS, slot) = ncross;
-                if (state == ST_DONE || state == ST_INTERACT)
-                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
-            }
-            mFly |= warp_or64((act && state == ST_FLY) ? (1ull << slot) : 0ull);
-            mJ |= warp_or64((act && state == ST_JUMP) ? (1ull << slot) : 0ull);
-            mEv |= warp_or64((act && (state == ST_DONE || state == ST_INTERACT)) ? (1ull << slot) : 0ull);
             __syncwarp();
         } else if (njmp > 0 && njmp >= nevt) {
             // =========================================================== J phase: runs of empty bricks
@@ -523,16 +560,15 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, ux = 0.0, uy = 0.0, uz = 0.0;
             double tmx = 0.0, tmy = 0.0, tmz = 0.0, t = 0.0;
             int ix = 0, iy = 0, iz = 0, stx = 0, sty = 0, stz = 0;
-            uint32_t ncross = 0u, w1 = 0u;
+            uint32_t ncross = 0u;
             if (act) {
                 px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                 ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
                 t = SF(F_T, slot);
                 const uint32_t w0 = SU(U_W0, slot);
-                w1 = SU(U_W1, slot);
                 ncross = SU(U_NCROSS, slot);
-                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu);
+                ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0);
                 stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
                 sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
                 stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
@@ -540,7 +576,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 tmy = mcrt::face_t(iy, sty, py, ivy);
                 tmz = mcrt::face_t(iz, stz, pz, ivz);
             }
-            while (__any_sync(kFull, busy)) {
+            const int jmin = min(nj, MCRT_J_MIN);
+            do {
                 if (busy) {
                     // the precomputed box of empty bricks around this brick, in cells, clipped to the grid
                     const uint4 bb = __ldg(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
@@ -553,23 +590,24 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                               ((unsigned)iz >= (unsigned)P.nz);
                     busy = !escaped && brick_empty(s_m0, brick_of(ix, iy, iz, nbx, nby, bsh));
                 }
-            }
+            } while (__popc(__ballot_sync(kFull, busy)) >= max(jmin, 1));
             if (act) {
                 SF(F_T, slot) = t;
                 SU(U_NCROSS, slot) = ncross;
                 if (escaped) {
                     SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
                 } else {
-                    SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
-                    SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | (w1 & 0xffff0000u);
-                    const uint32_t cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
-                    SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + cidx));
+                    SU(U_W0, slot) = pack_xyz(ix, iy, iz);
+                    if (!busy) {
+                        const uint32_t cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                        SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + cidx));
+                    }
                 }
             }
-            const unsigned long long mine = act ? (1ull << slot) : 0ull;
+            const unsigned long long mine = (act && !busy) ? (1ull << slot) : 0ull;   // still jumping: stays in mJ
             mJ &= ~warp_or64(mine);
             mEv |= warp_or64(escaped ? mine : 0ull);
-            mFly |= warp_or64((act && !escaped) ? mine : 0ull);
+            mFly |= warp_or64(!escaped ? mine : 0ull);
             __syncwarp();
         } else if (mEv != 0ull) {
             // =========================================================== E phase: one event per lane
@@ -586,8 +624,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 pid = (unsigned long long)__double_as_longlong(SF(F_PID, slot));
                 if (RECORD) hash = (unsigned long long)__double_as_longlong(SF(F_HASH, slot));
                 ncross = SU(U_NCROSS, slot); nsca = SU(U_NSCA, slot); nabs = SU(U_NABS, slot);
-                const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
-                ix = (int)(w0 & 0xffffu); iy = (int)(w0 >> 16); iz = (int)(w1 & 0xffffu); j = (int)(w1 >> 16);
+                const uint32_t w0 = SU(U_W0, slot);
+                ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0); j = (int)SU(U_W1, slot);
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
             }
             if (kind == K_ESCAPED) {
@@ -745,8 +783,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 if (RECORD) SF(F_HASH, slot) = __longlong_as_double((long long)hash);
                 SU(U_DK, slot) = d;    // kind is set when the walk stops
                 SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
-                SU(U_W0, slot) = (uint32_t)(ix & 0xffff) | ((uint32_t)iy << 16);
-                SU(U_W1, slot) = (uint32_t)(iz & 0xffff) | ((uint32_t)j << 16);
+                SU(U_W0, slot) = pack_xyz(ix, iy, iz);
+                SU(U_W1, slot) = (uint32_t)j;
             }
             const unsigned long long mine = act ? (1ull << slot) : 0ull;
             mEv &= ~warp_or64(mine);                       // taken: now flying, or dead (no packets left)
@@ -759,7 +797,7 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
     }
 #undef SF
 #undef SU
-    if (ndusty_acc) atomicAdd(&s_cnt[CNT_DUSTY], ndusty_acc);
+    if (ndusty_acc) atomicAdd(&s_cnt[CNT_DUSTY], (unsigned long long)ndusty_acc);
 
     // flush the block-private histogram and counters
     __syncthreads();
@@ -1183,7 +1221,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     if (!out) return fail(nullptr, MCRT_EINVAL, "out is NULL");
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be >= 1");
-    if (nx > 65535 || ny > 65535 || nz > 65535) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be <= 65535");
+    if (nx > 2048 || ny > 2048 || nz > 1024) return fail(nullptr, MCRT_EINVAL, "grid too large: nx, ny <= 2048 and nz <= 1024");
     if ((size_t)nx * ny * nz > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
     if (!(cell_size_cm > 0.0) || !isfinite(cell_size_cm)) return fail(nullptr, MCRT_EINVAL, "cell_size_cm must be > 0");
     if (!rho || !species) return fail(nullptr, MCRT_EINVAL, "rho / species is NULL");
