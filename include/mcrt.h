@@ -59,7 +59,7 @@ typedef enum {
 typedef struct {
     int32_t mode;              /* mcrt_mode */
     uint64_t epoch_B0;         /* first epoch size; 0 = max(256, largest power of two <= N/256) */
-    uint64_t epoch_Bmax;       /* largest epoch size; 0 = 2^20.  Epoch e has min(B0*2^e, Bmax) packets */
+    uint64_t epoch_Bmax;       /* largest epoch size; 0 = 2^22.  Epoch e has min(B0*2^e, Bmax) packets */
     int32_t n_sweeps;          /* MCRT_MODE_FROZEN_T_SWEEP: number of sweeps (each emits N packets) */
     int32_t sweep_T_from_lucy; /* sweeps take T from the Lucy tally (1) or from absorption counts (0) */
     int32_t record_digests;    /* keep a per-packet event digest (needs digest capacity in the workspace) */

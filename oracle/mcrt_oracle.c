@@ -658,13 +658,13 @@ int orc_fx_bits(uint64_t n_packets)
     return fx;
 }
 
-/* default epoch schedule (O11): B0 = max(256, largest power of two <= N/256), Bmax = 2^20 */
+/* default epoch schedule (O11, reading Q19): B0 = max(256, largest power of two <= N/256), Bmax = 2^22 */
 void orc_default_schedule(uint64_t n_packets, uint64_t *B0, uint64_t *Bmax)
 {
     uint64_t q = n_packets / 256, b = 256;
     while (b * 2 <= q) b *= 2;
     *B0 = b;
-    *Bmax = (uint64_t)1 << 20;
+    *Bmax = (uint64_t)1 << 22;
 }
 
 /* O11 epoch rule.  Bjorkman & Wood adjust the temperature after every absorption;

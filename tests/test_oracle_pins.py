@@ -454,5 +454,5 @@ def test_p14_fixed_point_vs_compensated_fp64(orc):
     assert rel.max() < 1e-6
     # quantisation bound: each add is off by <= 2^-(fx+1)
     assert np.all(np.abs(L - raw["lucy_fp64"]) <= r["lucy_adds"] * 2.0 ** -(fx + 1))
-    assert orc.default_schedule(10 ** 8) == (2 ** 18, 2 ** 20) and orc.default_schedule(10 ** 5) == (256, 2 ** 20)
-    assert orc.default_schedule(1000) == (256, 2 ** 20)
+    assert orc.default_schedule(10 ** 8) == (2 ** 18, 2 ** 22) and orc.default_schedule(10 ** 5) == (256, 2 ** 22)
+    assert orc.default_schedule(1000) == (256, 2 ** 22)
