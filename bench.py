@@ -44,6 +44,7 @@ def parse():
     ap.add_argument("--packets", type=int, default=0, help="packets per step (0 = the configuration's full count)")
     ap.add_argument("--clumps", type=int, default=5000)
     ap.add_argument("--ref-packets", type=int, default=1_000_000, help="oracle sample size per step")
+    ap.add_argument("--bmax", type=int, default=0, help="experiment: epoch_Bmax override (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -194,7 +195,7 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     for i in range(args.warmup):
-        ctx.run(n_packets, seed, want_stats=False)
+        ctx.run(n_packets, seed, want_stats=False, epoch_Bmax=args.bmax)
     barrier()
     stats0 = None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -204,7 +205,7 @@ def run_ours(args):
         barrier()
         ev0.record()
         for i in range(args.steps):
-            ctx.run(n_packets, seed + i, want_stats=False, time_kernels=1)
+            ctx.run(n_packets, seed + i, want_stats=False, time_kernels=1, epoch_Bmax=args.bmax)
             if i < args.steps - 1:
                 # counters are reset by the next run: read them (tiny D2H, inside the timed region, honest)
                 st = ctx.stats()

@@ -292,13 +292,13 @@ constexpr int kSlotF64 = 15;        // 8-byte fields per slot
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
 #ifndef MCRT_SWAP_MIN
-#define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
+#define MCRT_SWAP_MIN 10            // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
 #ifndef MCRT_S_ENTER
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
 #endif
 #ifndef MCRT_S_LEAVE
-#define MCRT_S_LEAVE 8              // ... and ends when this many lanes are idle and nothing is left to refill them
+#define MCRT_S_LEAVE 14             // ... and ends when this many lanes are idle and nothing is left to refill them
 #endif
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
@@ -415,95 +415,99 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             // no flying packet left for MCRT_S_LEAVE idle lanes.
             int slot = 0, state = ST_IDLE;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
-            double t = 0.0, tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;
+            double tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;  // tn: parameter at which the cell of the entry is left
             int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
             uint32_t ciA = 0u, ciB = 0u, ciC = 0u, xzA = 0u, xzB = 0u, xzC = 0u;   // storage index, packed coordinates
-            uint32_t gcidx = 0u, ncross = 0u, pk_xyz = 0u;
-            unsigned long long pk_cw = 0ull;
+            uint32_t gcidx = 0u, ncross = 0u;
+            double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
+            int kq_sp = -1;
             int r = 0;                                          // ring slot of cell n
             int nidle = 32;
             bool first = true;
 
-            // one step: G advances one cell (queue entry 2 receives the cell G leaves), the physics handles cell n
-            // (queue entry 0; entry 1 only tells whether cell n+1 is outside the grid)
-            auto step = [&](const double tn0, const uint32_t ci0, const uint32_t xz0, const uint32_t ci1, double &tn2,
-                            uint32_t &ci2, uint32_t &xz2) {
-                cp_async_wait<2>();                               // the word of cell n has landed
-                const unsigned long long cw = ring[r * ring_stride];
-                ci2 = gcidx;
-                xz2 = pack_xyz(gx, gy, gz);
-                if (gcidx != kOutCell) {
-                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
-                    const bool sely = !selx && (tmy <= tmz);
-                    const bool selz = !selx && !sely;
-                    tn2 = selx ? tmx : (sely ? tmy : tmz);
-                    gx += selx ? stx : 0;
-                    gy += sely ? sty : 0;
-                    gz += selz ? stz : 0;
-                    // parameter of the face through which the entered cell will be left (reading Q8)
-                    if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;
-                    if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;
-                    if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;
-                    gcidx = kOutCell;
-                    if (((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) & ((unsigned)gz < (unsigned)P.nz)) {
-                        const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);
-                        gcidx = cell_in_brick(brick, gx, gy, gz, bsh);
-                        unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;
-                        if (!brick_empty(s_m0, brick)) cp_async8(dst, P.cellw + gcidx);
-                        else *reinterpret_cast<volatile unsigned long long *>(dst) = kJumpWord;
-                    }
-                }
-                cp_async_commit();
-                // physics of cell n
-                if (cw == kJumpWord) {
-                    state = ST_JUMP;                           // cell n starts a run of empty bricks: J phase
-                    pk_xyz = xz0;
-                } else {
-                    const double ds = tn0 - t;
-                    const double rho_c = cw_rho(cw);
-                    const double2 kq = s_kk[cw_species(cw) * nf + j];
-                    const double dtau = kq.x * rho_c * ds;      // tau_i = (kabs+ksca) h rho ds (Eq. 2)
-                    if (dtau > tau) {
-                        state = ST_INTERACT;                   // interaction inside this cell (equality leaves, Q5)
-                        pk_xyz = xz0; pk_cw = cw;
-                    } else {
-                        tau -= dtau;
-                        if (!cw_vacuum(cw)) {
-                            lucy_add(P.lfx, ci0, kq.y * rho_c * ds);
-                            ndusty_acc++;
-                        }
-                        t = tn0;
-                        ncross++;
-                        r = (r + 1) & 3;
-                        if (ci1 == kOutCell) state = ST_DONE;  // left the grid: escape tally in the E phase
-                    }
-                }
-            };
+// One step.  G advances one cell: queue entry 2 (whose exit parameter is the parameter at which cell n was
+// entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0; entry 1 only tells
+// whether cell n+1 is outside the grid.  A packet that stops writes what the next phase needs into its slot and
+// leaves the loop body.
+#define S_STEP(TN0, CI0, XZ0, CI1, TN2, CI2, XZ2)                                                                     \
+    {                                                                                                                  \
+        cp_async_wait<2>(); /* the word of cell n has landed */                                                        \
+        const unsigned long long cw = ring[r * ring_stride];                                                           \
+        const double t_in = TN2;                                                                                       \
+        CI2 = gcidx;                                                                                                   \
+        XZ2 = pack_xyz(gx, gy, gz);                                                                                    \
+        if (gcidx != kOutCell) {                                                                                       \
+            const bool selx = (tmx <= tmy) && (tmx <= tmz);                                                            \
+            const bool sely = !selx && (tmy <= tmz);                                                                   \
+            const bool selz = !selx && !sely;                                                                          \
+            TN2 = selx ? tmx : (sely ? tmy : tmz);                                                                     \
+            gx += selx ? stx : 0;                                                                                      \
+            gy += sely ? sty : 0;                                                                                      \
+            gz += selz ? stz : 0;                                                                                      \
+            /* parameter of the face through which the entered cell will be left (reading Q8) */                       \
+            if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;                                   \
+            if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;                                   \
+            if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;                                   \
+            gcidx = kOutCell;                                                                                          \
+            if (((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) & ((unsigned)gz < (unsigned)P.nz)) { \
+                const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);                                            \
+                gcidx = cell_in_brick(brick, gx, gy, gz, bsh);                                                         \
+                unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;        \
+                if (!brick_empty(s_m0, brick)) cp_async8(dst, P.cellw + gcidx);                                        \
+                else *reinterpret_cast<volatile unsigned long long *>(dst) = kJumpWord;                                \
+            }                                                                                                          \
+        }                                                                                                              \
+        cp_async_commit();                                                                                             \
+        /* physics of cell n */                                                                                        \
+        if (cw == kJumpWord) { /* cell n starts a run of empty bricks: J phase */                                      \
+            SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0; SU(U_NCROSS, slot) = ncross;            \
+            state = ST_JUMP;                                                                                           \
+            continue;                                                                                                  \
+        }                                                                                                              \
+        const double ds = TN0 - t_in;                                                                                  \
+        const double rho_c = cw_rho(cw);                                                                               \
+        if (cw_species(cw) != kq_sp) { /* opacities of this species at the packet's frequency: kept in registers */   \
+            kq_sp = cw_species(cw);                                                                                    \
+            kq = s_kk[kq_sp * nf + j];                                                                                 \
+        }                                                                                                              \
+        const double dtau = kq.x * rho_c * ds; /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */                 \
+        if (dtau > tau) { /* interaction inside this cell (equality leaves, Q5) */                                     \
+            SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0; SU(U_NCROSS, slot) = ncross;            \
+            SF(F_CW, slot) = __longlong_as_double((long long)cw);                                                      \
+            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);                                      \
+            state = ST_INTERACT;                                                                                       \
+            continue;                                                                                                  \
+        }                                                                                                              \
+        tau -= dtau;                                                                                                   \
+        if (!cw_vacuum(cw)) {                                                                                          \
+            lucy_add(P.lfx, CI0, kq.y * rho_c * ds);                                                                   \
+            ndusty_acc++;                                                                                              \
+        }                                                                                                              \
+        ncross++;                                                                                                      \
+        r = (r + 1) & 3;                                                                                               \
+        if (CI1 == kOutCell) { /* left the grid: escape tally in the E phase */                                        \
+            SU(U_NCROSS, slot) = ncross;                                                                               \
+            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);                                       \
+            state = ST_DONE;                                                                                           \
+            continue;                                                                                                  \
+        }                                                                                                              \
+    }
 
             for (;;) {
-                // ---- park packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
+                // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
                 const int nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
                 if (first || nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) {
                     first = false;
-                    const bool stopped = state != ST_FLY && state != ST_IDLE;
-                    if (stopped) {
-                        SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
-                        SF(F_CW, slot) = __longlong_as_double((long long)pk_cw);
-                        SU(U_W0, slot) = pk_xyz;
-                        SU(U_NCROSS, slot) = ncross;
-                        if (state != ST_JUMP)
-                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | ((state == ST_DONE ? K_ESCAPED : K_INTERACT) << 30);
-                    }
                     mJ |= warp_or64(state == ST_JUMP ? (1ull << slot) : 0ull);
                     mEv |= warp_or64((state == ST_DONE || state == ST_INTERACT) ? (1ull << slot) : 0ull);
-                    if (stopped) state = ST_IDLE;
+                    if (state != ST_FLY) state = ST_IDLE;
                     const unsigned idle = __ballot_sync(kFull, state == ST_IDLE);
                     const int nfl = 32 - __popc(idle);
                     // nothing left to refill with and many lanes idle: let the other phases make flying packets
                     if (mFly == 0ull && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && (mJ | mEv) != 0ull))) {
-                        if (state == ST_FLY) {
+                        if (state == ST_FLY) {   // park mid-flight: cell n is entry A, entered at tnC
                             cp_async_wait<0>();
-                            SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
+                            SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
                             SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
                             SU(U_W0, slot) = xzA;
                             SU(U_NCROSS, slot) = ncross;
@@ -518,7 +522,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                         cp_async_wait<0>();                       // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
-                        t = SF(F_T, slot); tau = SF(F_TAU, slot);
+                        const double t = SF(F_T, slot);
+                        tau = SF(F_TAU, slot);
                         const uint32_t w0 = SU(U_W0, slot);
                         j = (int)SU(U_W1, slot);
                         ncross = SU(U_NCROSS, slot) - 2u;         // the two no-op cells below count themselves
@@ -535,17 +540,21 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                         r = 0;
                         ring[0] = 0ull; ring[ring_stride] = 0ull;
                         ring[2 * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        tnA = t; tnB = t; ciA = 0u; ciB = 0u; xzA = w0; xzB = w0;
+                        tnA = t; tnB = t; tnC = t; ciA = 0u; ciB = 0u; xzA = w0; xzB = w0;
+                        kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
                     mFly &= ~warp_or64(take ? (1ull << slot) : 0ull);
                     nidle = __popc(__ballot_sync(kFull, state == ST_IDLE));
                 }
                 // ---- three steps
-                if (state == ST_FLY) step(tnA, ciA, xzA, ciB, tnC, ciC, xzC);
-                if (state == ST_FLY) step(tnB, ciB, xzB, ciC, tnA, ciA, xzA);
-                if (state == ST_FLY) step(tnC, ciC, xzC, ciA, tnB, ciB, xzB);
+                if (state == ST_FLY) {
+                    S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
+                    S_STEP(tnB, ciB, xzB, ciC, tnA, ciA, xzA)
+                    S_STEP(tnC, ciC, xzC, ciA, tnB, ciB, xzB)
+                }
             }
+#undef S_STEP
             __syncwarp();
         } else if (njmp > 0 && njmp >= nevt) {
             // =========================================================== J phase: runs of empty bricks
@@ -1592,7 +1601,7 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
     if (o.mode == MCRT_MODE_BW_EPOCH) {
         uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
         if (B0 == 0) { B0 = 256; while (B0 * 2 <= n_packets / 256) B0 *= 2; }
-        if (Bmax == 0) Bmax = (uint64_t)1 << 20;
+        if (Bmax == 0) Bmax = (uint64_t)1 << 22;
         if (Bmax < B0) Bmax = B0;
         P.cdf = c->d_cdfdB;
         P.pass = o.rng_pass;
