@@ -416,6 +416,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             int slot = 0, state = ST_IDLE;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
             double tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;  // tn: parameter at which the cell of the entry is left
+            double fdx = 0.0, fdy = 0.0, fdz = 0.0;             // coordinate of the face through which G's cell is left
+            double sdx = 0.0, sdy = 0.0, sdz = 0.0;             // step per axis as a double (+1, -1 or 0)
             int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
             uint32_t ciA = 0u, ciB = 0u, ciC = 0u, xzA = 0u, xzB = 0u, xzC = 0u;   // storage index, packed coordinates
             uint32_t gcidx = 0u, ncross = 0u;
@@ -444,10 +446,11 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             gx += selx ? stx : 0;                                                                                      \
             gy += sely ? sty : 0;                                                                                      \
             gz += selz ? stz : 0;                                                                                      \
-            /* parameter of the face through which the entered cell will be left (reading Q8) */                       \
-            if (selx) tmx = (mcrt::int_to_double(gx + ((stx + 1) >> 1)) - px) * ivx;                                   \
-            if (sely) tmy = (mcrt::int_to_double(gy + ((sty + 1) >> 1)) - py) * ivy;                                   \
-            if (selz) tmz = (mcrt::int_to_double(gz + ((stz + 1) >> 1)) - pz) * ivz;                                   \
+            /* parameter of the face through which the entered cell will be left (reading Q8): the face        */   \
+            /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u)                       */   \
+            if (selx) { fdx += sdx; tmx = (fdx - px) * ivx; }                                                          \
+            if (sely) { fdy += sdy; tmy = (fdy - py) * ivy; }                                                          \
+            if (selz) { fdz += sdz; tmz = (fdz - pz) * ivz; }                                                          \
             gcidx = kOutCell;                                                                                          \
             if (((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) & ((unsigned)gz < (unsigned)P.nz)) { \
                 const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);                                            \
@@ -535,6 +538,9 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                         tmx = mcrt::face_t(gx, stx, px, ivx);
                         tmy = mcrt::face_t(gy, sty, py, ivy);
                         tmz = mcrt::face_t(gz, stz, pz, ivz);
+                        fdx = (double)(gx + ((stx + 1) >> 1)); sdx = (double)stx;
+                        fdy = (double)(gy + ((sty + 1) >> 1)); sdy = (double)sty;
+                        fdz = (double)(gz + ((stz + 1) >> 1)); sdz = (double)stz;
                         gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
                         // pipeline: two no-op cells (zero length, vacuum word), then the packet's cell
                         r = 0;
