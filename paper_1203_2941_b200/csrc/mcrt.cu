@@ -288,9 +288,12 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
 // by (seed, packet id, draw index, pass) and all tallies are integer atomics.
 // ------------------------------------------------------------------------------------------------
 constexpr int kSlots = 64;          // packets per warp
-constexpr int kSlotF64 = 15;        // 8-byte fields per slot
+constexpr int kSlotF64 = 11;        // 8-byte fields per slot (+1, the digest hash, in the recording kernel)
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
-constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
+__host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlots * ((kSlotF64 + (record ? 1 : 0)) * 8 + kSlotU32 * 4); }
+#ifndef MCRT_MAX_THREADS
+#define MCRT_MAX_THREADS 640        // 20 warps per SM: at most 102 registers per thread
+#endif
 #ifndef MCRT_SWAP_MIN
 #define MCRT_SWAP_MIN 10            // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
@@ -304,7 +307,7 @@ constexpr int kPoolBytesPerWarp = kSlots * (kSlotF64 * 8 + kSlotU32 * 4);
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
 #endif
 
-enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_IVX, F_IVY, F_IVZ, F_T, F_TAU, F_ZTYPE, F_CW, F_HASH, F_PID };
+enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_HASH };
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
 constexpr uint32_t kOutCell = 0xffffffffu;   // storage index of "outside the grid"
@@ -353,13 +356,15 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 constexpr int kRing = 4;            // cell-word ring slots per thread (cells n .. n+3)
 
 template <bool RECORD>
-__global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
+__global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const TransportParams P)
 {
     extern __shared__ double2 smem_d2[];
     const int nsf = P.ns * P.nf;
     const int nwarps = blockDim.x >> 5;
-    double *s_pool = reinterpret_cast<double *>(smem_d2);                // [nwarps][kPoolBytesPerWarp]
-    double2 *s_kk = reinterpret_cast<double2 *>(s_pool + (size_t)nwarps * (kPoolBytesPerWarp / 8));
+    constexpr int kPoolF64 = pool_bytes_per_warp(RECORD) / 8;
+    constexpr int kNF64 = kSlotF64 + (RECORD ? 1 : 0);
+    double *s_pool = reinterpret_cast<double *>(smem_d2);                // [nwarps][pool_bytes_per_warp]
+    double2 *s_kk = reinterpret_cast<double2 *>(s_pool + (size_t)nwarps * kPoolF64);
     double2 *s_ag = s_kk + nsf;              // {albedo, g};  s_kk = {kext_h, kabs_fx}: one LDS.128 per crossing
     double *s_src = reinterpret_cast<double *>(s_ag + nsf);
     double *s_mu = s_src + P.nf;
@@ -386,8 +391,8 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
 
     const int lane = (int)(threadIdx.x & 31u);
     const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby;
-    double *wf = s_pool + (size_t)(threadIdx.x >> 5) * (kPoolBytesPerWarp / 8);   // this warp's pool, f64 fields
-    uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kSlotF64 * kSlots);          // its u32 fields
+    double *wf = s_pool + (size_t)(threadIdx.x >> 5) * kPoolF64;                  // this warp's pool, f64 fields
+    uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kNF64 * kSlots);             // its u32 fields
 #define SF(f, s) wf[(f) * kSlots + (s)]
 #define SU(f, s) wu[(f) * kSlots + (s)]
 
@@ -524,7 +529,12 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                         slot = nth_set64(mFly, k);
                         cp_async_wait<0>();                       // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
-                        ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+                        {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
+                            const double ux = SF(F_UX, slot), uy = SF(F_UY, slot), uz = SF(F_UZ, slot);
+                            ivx = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
+                            ivy = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
+                            ivz = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+                        }
                         const double t = SF(F_T, slot);
                         tau = SF(F_TAU, slot);
                         const uint32_t w0 = SU(U_W0, slot);
@@ -578,8 +588,10 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
             uint32_t ncross = 0u;
             if (act) {
                 px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
-                ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+                ivx = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
+                ivy = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
+                ivz = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
                 t = SF(F_T, slot);
                 const uint32_t w0 = SU(U_W0, slot);
                 ncross = SU(U_NCROSS, slot);
@@ -787,9 +799,6 @@ __global__ void __launch_bounds__(512, 1) k_transport(const TransportParams P)
                 // park the new flight (reading Q8: the walk needs p, 1/u, the cell; t = 0)
                 SF(F_PX, slot) = px; SF(F_PY, slot) = py; SF(F_PZ, slot) = pz;
                 SF(F_UX, slot) = ux; SF(F_UY, slot) = uy; SF(F_UZ, slot) = uz;
-                SF(F_IVX, slot) = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
-                SF(F_IVY, slot) = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
-                SF(F_IVZ, slot) = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
                 SF(F_T, slot) = 0.0;
                 SF(F_TAU, slot) = -log(z0);
                 SF(F_ZTYPE, slot) = z1;
@@ -1141,9 +1150,9 @@ int fx_bits_for(uint64_t n)
     return fx;
 }
 
-size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads)
+size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record)
 {
-    return (size_t)(threads / 32) * kPoolBytesPerWarp + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
+    return (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
            8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
            (size_t)((mask0_words + 1) & ~1) * sizeof(uint32_t) + (size_t)kRing * threads * sizeof(unsigned long long);
 }
@@ -1352,7 +1361,7 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
         if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
         if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
     }
-    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256) > 220 * 1024)
+    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256, true) > 220 * 1024)
         return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
     c->nf = n_nu; c->nT = n_T;
     c->nu.assign(nu_hz, nu_hz + n_nu);
@@ -1480,11 +1489,13 @@ static int ensure_histograms(mcrt_ctx *c)
 
 static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem)
 {
-    *threads = (o && o->block_threads > 0) ? o->block_threads : 512;
-    if (*threads % 32 || *threads > 512 || *threads < 32) return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32..512");
+    const bool record = o && o->record_digests;
+    *threads = (o && o->block_threads > 0) ? o->block_threads : MCRT_MAX_THREADS;
+    if (*threads % 32 || *threads > MCRT_MAX_THREADS || *threads < 32)
+        return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32.." + std::to_string(MCRT_MAX_THREADS));
     // as many warps (each with its packet pool) as fit beside the tables in 227 KB of shared memory
-    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads) > 227 * 1024) *threads -= 32;
-    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads);
+    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record) > 227 * 1024) *threads -= 32;
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record);
     if (*smem > 48 * 1024) {
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_transport<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
