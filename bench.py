@@ -5,8 +5,8 @@
                     [--workload torus256] [--packets P] [--clumps C]
 
 One "step" is one pass of the whole hot path (S0-S12: tally reset, per-epoch temperature-index
-update, persistent transport kernel, range check) over one batch of `--packets` synthetic packets of the
-named workload.  Prints ONE JSON line (rank 0).  `value` = cell crossings per second with the inputs resident
+update, persistent transport kernel with its S / J / E phases, range check) over one batch of `--packets`
+synthetic packets of the named workload (default: BASELINE config 4, torus256, 5000 clumps, 1e8 packets).  Prints ONE JSON line (rank 0).  `value` = cell crossings per second with the inputs resident
 in HBM; `e2e` = the same metric through the C ABI with HOST buffers (grid/tables host->device and
 E_abs/T/SED device->host inside the timed region).
 
@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--workload", default="torus256")
     ap.add_argument("--packets", type=int, default=0, help="packets per step (0 = the configuration's full count)")
     ap.add_argument("--clumps", type=int, default=5000)
-    ap.add_argument("--ref-packets", type=int, default=1_000_000, help="oracle sample size per step")
+    ap.add_argument("--ref-packets", type=int, default=10_000_000, help="oracle sample size per step (about 15 s on 16 cores)")
     ap.add_argument("--bmax", type=int, default=0, help="experiment: epoch_Bmax override (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")

@@ -66,7 +66,7 @@ typedef struct {
     int32_t reset_tallies;     /* zero all tallies before the run (default 1) */
     uint32_t rng_pass;         /* 4th Philox counter word of the B&W run; sweep s uses rng_pass + s */
     int32_t grid_blocks;       /* launch tuning, 0 = auto.  Results never depend on it. */
-    int32_t block_threads;     /* launch tuning, 0 = auto (multiple of 32, <= 256) */
+    int32_t block_threads;     /* launch tuning, 0 = auto (multiple of 32, <= 512) */
     int32_t time_kernels;      /* bracket every kernel with CUDA events on the context's stream; the
                                   summed durations are returned in mcrt_run_stats (transport_ms, update_ms) */
 } mcrt_run_opts;
@@ -110,7 +110,10 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
  *             256-byte alignment required.  The library sub-allocates from it in call order (grid
  *             here, tables in mcrt_dust_tables, histograms and digests at the first mcrt_run that
  *             needs them) and returns MCRT_ENOMEM when it runs out; size it with mcrt_workspace_bytes.
- * The grid is re-laid out on the device into 4x4x4 bricks of packed 8-byte cell words. */
+ *  nx, ny <= 2048 and nz <= 1024 (cell coordinates are carried packed in 32 bits).
+ * The grid is re-laid out on the device into bricks of packed 8-byte cell words (4x4x4 cells up to 256^3,
+ * 8x8x8 up to 512^3, ...); a bit mask of the bricks without dust and, for each of them, a large box of empty
+ * bricks around it are built here as well (they let packets cross vacuum without touching memory). */
 int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm, const float *rho,
                      const uint8_t *species, int n_species, mcrt_mem where, void *workspace,
                      size_t workspace_bytes);

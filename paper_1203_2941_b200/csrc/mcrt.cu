@@ -292,7 +292,7 @@ constexpr int kSlotF64 = 11;        // 8-byte fields per slot (+1, the digest ha
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlots * ((kSlotF64 + (record ? 1 : 0)) * 8 + kSlotU32 * 4); }
 #ifndef MCRT_MAX_THREADS
-#define MCRT_MAX_THREADS 640        // 20 warps per SM: at most 102 registers per thread
+#define MCRT_MAX_THREADS 512        // 16 warps per SM, up to 128 registers per thread (640 = 20 warps measured no faster)
 #endif
 #ifndef MCRT_SWAP_MIN
 #define MCRT_SWAP_MIN 10            // S phase: stopped packets are parked / replaced this many lanes at a time
