@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--workload", default="torus256")
     ap.add_argument("--packets", type=int, default=0, help="packets per step (0 = the configuration's full count)")
     ap.add_argument("--clumps", type=int, default=5000)
-    ap.add_argument("--ref-packets", type=int, default=10_000_000, help="oracle sample size per step (about 15 s on 16 cores)")
+    ap.add_argument("--ref-packets", type=int, default=30_000_000, help="oracle sample size per step (about 15 s on 16 cores)")
     ap.add_argument("--bmax", type=int, default=0, help="experiment: epoch_Bmax override (0 = library default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -240,10 +240,17 @@ def run_ours(args):
         "bytes_per_crossing": algo_bytes / max(1, tot["crossings"]),
         "traffic": None,
     }
-    prof = os.path.join(ROOT, "profiles", "traffic.json")
+    # DRAM traffic of one k_transport launch from the committed ncu capture (profiles/traffic.csv), scaled from the
+    # captured launch (2^22 packets) to this run's average launch by packets
+    prof = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(prof):
         try:
-            roofline["traffic"] = json.load(open(prof)).get(w.name)
+            import csv
+            for row in csv.DictReader(open(prof)):
+                if row["workload"] == w.name:
+                    per_packet = float(row["dram_bytes_per_launch"]) / float(row["launch_packets"])
+                    roofline["traffic"] = per_packet * tot["packets"] / n_launch
+                    roofline["traffic_source"] = "profiles/" + row["source"]
         except Exception:
             pass
     ctx.close()
@@ -317,8 +324,10 @@ def run_ours(args):
             "config": {"workload": w.name, "grid": [w.nx, w.ny, w.nz], "n_clumps": w.meta.get("n_clumps"),
                        "n_nu": w.n_nu, "n_species": w.n_species, "packets_per_step": n_packets,
                        "mode": "bw_epoch", "launch": {"blocks": blocks, "threads": threads, "smem": smem},
-                       "l2": "working set (cell words + tallies, %.0f MB) larger than the 126 MB L2; tallies reset every step"
-                             % (w.n_cells * 32 / 1e6),
+                       "l2": "inputs larger than L2: cell words + tallies %.0f MB (dusty part %.0f MB) vs 126 MB; tallies reset and "
+                             "the per-epoch update streams all cells between transport launches"
+                             % (w.n_cells * 32 / 1e6, float((w.rho > 0).sum()) * 32 / 1e6),
+                       "epoch_Bmax": args.bmax if args.bmax else "default 2^22",
                        "parallelism": "replicas" if world > 1 else "single"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": int(tot["gpu_launches"]),

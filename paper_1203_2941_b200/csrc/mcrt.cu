@@ -272,6 +272,26 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
     atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
 }
 
+// Warp-aggregated tallies ("local copies reduce interference").  The lanes of the calling group
+// that address the same cell are found with __match_any_sync; their integer contributions are summed with
+// __reduce_add_sync in three 16-bit limbs (x < 2^46, so 32 lanes cannot overflow a limb sum) and the lowest
+// lane of each group issues one atomic.  Integer sums: the result is the same as with one atomic per lane.
+__device__ __forceinline__ void lucy_add_aggregated(long long *__restrict__ lfx, uint32_t cidx, double x)
+{
+    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
+    const unsigned grp = __match_any_sync(__activemask(), cidx);
+    const unsigned long long s0 = __reduce_add_sync(grp, (unsigned)(q & 0xffffull));
+    const unsigned long long s1 = __reduce_add_sync(grp, (unsigned)((q >> 16) & 0xffffull));
+    const unsigned long long s2 = __reduce_add_sync(grp, (unsigned)(q >> 32));
+    if ((threadIdx.x & 31u) == (unsigned)(__ffs(grp) - 1))
+        atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), s0 + (s1 << 16) + (s2 << 32));
+}
+__device__ __forceinline__ void count_add_aggregated(unsigned long long *__restrict__ kcnt, uint32_t cidx)
+{
+    const unsigned grp = __match_any_sync(__activemask(), cidx);
+    if ((threadIdx.x & 31u) == (unsigned)(__ffs(grp) - 1)) atomicAdd(&kcnt[cidx], (unsigned long long)__popc(grp));
+}
+
 // ------------------------------------------------------------------------------------------------
 // S0-S10  the transport kernel: persistent CTAs; every warp owns a POOL of kSlots packets in shared memory.
 //
@@ -302,6 +322,9 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #endif
 #ifndef MCRT_S_LEAVE
 #define MCRT_S_LEAVE 14             // ... and ends when this many lanes are idle and nothing is left to refill them
+#endif
+#ifndef MCRT_S_MATCH
+#define MCRT_S_MATCH 0              // 1: the per-crossing Lucy adds of the S phase are warp-aggregated as well
 #endif
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
@@ -432,6 +455,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             int nidle = 32;
             bool first = true;
 
+#if MCRT_S_MATCH
+#define S_LUCY_ADD lucy_add_aggregated
+#else
+#define S_LUCY_ADD lucy_add
+#endif
 // One step.  G advances one cell: queue entry 2 (whose exit parameter is the parameter at which cell n was
 // entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0; entry 1 only tells
 // whether cell n+1 is outside the grid.  A packet that stops writes what the next phase needs into its slot and
@@ -488,7 +516,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         }                                                                                                              \
         tau -= dtau;                                                                                                   \
         if (!cw_vacuum(cw)) {                                                                                          \
-            lucy_add(P.lfx, CI0, kq.y * rho_c * ds);                                                                   \
+            S_LUCY_ADD(P.lfx, CI0, kq.y * rho_c * ds);                                                                 \
             ndusty_acc++;                                                                                              \
         }                                                                                                              \
         ncross++;                                                                                                      \
@@ -721,7 +749,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double2 kq = s_kk[sj];
                     const double kk = kq.x * rho_c;
                     const double sint = tau / kk;
-                    lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
+                    lucy_add_aggregated(P.lfx, cidx, kq.y * rho_c * sint);
                     const double tint = t + sint;
                     double q;
                     q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
@@ -736,7 +764,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                        atomicAdd(&P.kcnt[cidx], 1ull);
+                        count_add_aggregated(P.kcnt, cidx);
                         nabs++;
                         const int s = cw_species(cw);
                         const int m = cw_tidx(cw);
