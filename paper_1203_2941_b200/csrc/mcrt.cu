@@ -307,7 +307,10 @@ __device__ __forceinline__ void count_add_aggregated(unsigned long long *__restr
 // Results never depend on which lane or warp carries a packet: all random numbers are Philox blocks keyed
 // by (seed, packet id, draw index, pass) and all tallies are integer atomics.
 // ------------------------------------------------------------------------------------------------
-constexpr int kSlots = 64;          // packets per warp
+#ifndef MCRT_SLOTS
+#define MCRT_SLOTS 64
+#endif
+constexpr int kSlots = MCRT_SLOTS;  // packets per warp (<= 128: the slot sets are one or two 64-bit masks)
 constexpr int kSlotF64 = 11;        // 8-byte fields per slot (+1, the digest hash, in the recording kernel)
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlots * ((kSlotF64 + (record ? 1 : 0)) * 8 + kSlotU32 * 4); }
@@ -366,6 +369,50 @@ __device__ __forceinline__ unsigned long long warp_or64(unsigned long long v)
     return ((unsigned long long)hi << 32) | lo;
 }
 
+// A set of pool slots, warp-uniform (every lane holds the same value): one or two 64-bit masks.
+constexpr int kSetWords = (kSlots + 63) / 64;
+struct SlotSet {
+    unsigned long long w[kSetWords];
+    __device__ __forceinline__ void clear() {
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) w[i] = 0ull;
+    }
+    __device__ __forceinline__ void fill() {   // slots 0 .. kSlots-1
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) {
+            const int n = kSlots - 64 * i;
+            w[i] = n >= 64 ? ~0ull : ((1ull << (n & 63)) - 1ull);
+        }
+    }
+    __device__ __forceinline__ int count() const {
+        int c = 0;
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) c += __popcll(w[i]);
+        return c;
+    }
+    __device__ __forceinline__ bool empty() const {
+        unsigned long long a = 0ull;
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) a |= w[i];
+        return a == 0ull;
+    }
+    // slot number of the n-th member (n = 0, 1, ...; n < count())
+    __device__ __forceinline__ int nth(int n) const {
+        if (kSetWords == 1) return nth_set64(w[0], n);
+        const int c0 = __popcll(w[0]);
+        return n < c0 ? nth_set64(w[0], n) : 64 + nth_set64(w[kSetWords - 1], n - c0);
+    }
+    // every lane with on == true contributes its slot: add them to / remove them from the set (warp-wide)
+    __device__ __forceinline__ void add(bool on, int slot) {
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) w[i] |= warp_or64((on && (slot >> 6) == i) ? (1ull << (slot & 63)) : 0ull);
+    }
+    __device__ __forceinline__ void remove(bool on, int slot) {
+#pragma unroll
+        for (int i = 0; i < kSetWords; ++i) w[i] &= ~warp_or64((on && (slot >> 6) == i) ? (1ull << (slot & 63)) : 0ull);
+    }
+};
+
 // 8-byte asynchronous copy global -> shared (LDGSTS), per-thread groups
 __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
 {
@@ -423,12 +470,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int s = lane; s < kSlots; s += 32) SU(U_DK, s) = K_EMIT << 30;
     __syncwarp();
     // warp-uniform slot sets: parked flying packets / packets inside a run of empty bricks / packets waiting for an event
-    unsigned long long mFly = 0ull, mJ = 0ull, mEv = ~0ull;
+    SlotSet mFly, mJ, mEv;
+    mFly.clear(); mJ.clear(); mEv.fill();
     bool exhausted = false;                        // the epoch counter has run out (warp-uniform)
     uint32_t ndusty_acc = 0u;                      // dusty crossings stepped by this lane
 
     for (;;) {
-        const int nfly = __popcll(mFly), njmp = __popcll(mJ), nevt = __popcll(mEv);
+        const int nfly = mFly.count(), njmp = mJ.count(), nevt = mEv.count();
         if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
@@ -534,13 +582,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 const int nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
                 if (first || nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) {
                     first = false;
-                    mJ |= warp_or64(state == ST_JUMP ? (1ull << slot) : 0ull);
-                    mEv |= warp_or64((state == ST_DONE || state == ST_INTERACT) ? (1ull << slot) : 0ull);
+                    mJ.add(state == ST_JUMP, slot);
+                    mEv.add(state == ST_DONE || state == ST_INTERACT, slot);
                     if (state != ST_FLY) state = ST_IDLE;
                     const unsigned idle = __ballot_sync(kFull, state == ST_IDLE);
                     const int nfl = 32 - __popc(idle);
                     // nothing left to refill with and many lanes idle: let the other phases make flying packets
-                    if (mFly == 0ull && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && (mJ | mEv) != 0ull))) {
+                    if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty())))) {
                         if (state == ST_FLY) {   // park mid-flight: cell n is entry A, entered at tnC
                             cp_async_wait<0>();
                             SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
@@ -548,13 +596,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             SU(U_W0, slot) = xzA;
                             SU(U_NCROSS, slot) = ncross;
                         }
-                        mFly |= warp_or64(state == ST_FLY ? (1ull << slot) : 0ull);
+                        mFly.add(state == ST_FLY, slot);
                         break;
                     }
                     const int k = __popc(idle & ((1u << lane) - 1u));
-                    const bool take = state == ST_IDLE && k < __popcll(mFly);
+                    const bool take = state == ST_IDLE && k < mFly.count();
                     if (take) {
-                        slot = nth_set64(mFly, k);
+                        slot = mFly.nth(k);
                         cp_async_wait<0>();                       // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
@@ -588,7 +636,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
-                    mFly &= ~warp_or64(take ? (1ull << slot) : 0ull);
+                    mFly.remove(take, slot);
                     nidle = __popc(__ballot_sync(kFull, state == ST_IDLE));
                 }
                 // ---- three steps
@@ -608,7 +656,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             // leaves the grid.  No global memory is touched on the way.
             const int nj = min(njmp, 32);
             const bool act = lane < nj;
-            const int slot = act ? nth_set64(mJ, lane) : 0;
+            const int slot = act ? mJ.nth(lane) : 0;
             bool busy = act, escaped = false;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, ux = 0.0, uy = 0.0, uz = 0.0;
             double tmx = 0.0, tmy = 0.0, tmz = 0.0, t = 0.0;
@@ -659,16 +707,16 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }
                 }
             }
-            const unsigned long long mine = (act && !busy) ? (1ull << slot) : 0ull;   // still jumping: stays in mJ
-            mJ &= ~warp_or64(mine);
-            mEv |= warp_or64(escaped ? mine : 0ull);
-            mFly |= warp_or64(!escaped ? mine : 0ull);
+            const bool mine = act && !busy;   // still jumping: stays in mJ
+            mJ.remove(mine, slot);
+            mEv.add(mine && escaped, slot);
+            mFly.add(mine && !escaped, slot);
             __syncwarp();
-        } else if (mEv != 0ull) {
+        } else if (nevt > 0) {
             // =========================================================== E phase: one event per lane
-            const int nev = min(__popcll(mEv), 32);
+            const int nev = min(nevt, 32);
             const bool act = lane < nev;
-            const int slot = act ? nth_set64(mEv, lane) : 0;
+            const int slot = act ? mEv.nth(lane) : 0;
             uint32_t kind = act ? (SU(U_DK, slot) >> 30) : 3u;
             uint32_t d = SU(U_DK, slot) & 0x3fffffffu;
             unsigned long long pid = 0ull, hash = 0ull;
@@ -838,10 +886,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 SU(U_W0, slot) = pack_xyz(ix, iy, iz);
                 SU(U_W1, slot) = (uint32_t)j;
             }
-            const unsigned long long mine = act ? (1ull << slot) : 0ull;
-            mEv &= ~warp_or64(mine);                       // taken: now flying, or dead (no packets left)
-            mFly |= warp_or64((dead || to_jump) ? 0ull : mine);
-            mJ |= warp_or64((!dead && to_jump) ? mine : 0ull);
+            mEv.remove(act, slot);                         // taken: now flying, jumping, or dead (no packets left)
+            mFly.add(act && !dead && !to_jump, slot);
+            mJ.add(act && !dead && to_jump, slot);
             __syncwarp();
         } else {
             break;
