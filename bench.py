@@ -164,6 +164,25 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def reduce_over_ranks(elapsed, counts, device, world):
+    """Whole-job figures of N independent replicas: the elapsed time is the MAX over
+    ranks, the unit counts are SUMMED.  Uses the default process group (NCCL on GPUs, gloo in the CPU test)."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([elapsed], dtype=torch.float64, device=device)
+    c = torch.tensor([float(x) for x in counts], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return float(t.item()), [float(x) for x in c.tolist()]
+
+
+def replica_seed(base_seed, rank):
+    """Seed of rank's replica: same problem, disjoint Philox keys."""
+    return base_seed + 1000 * rank
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -183,7 +202,7 @@ def run_ours(args):
     B.load_library()
 
     w, n_packets = make_workload(args)
-    seed = w.seed + 1000 * rank  # N > 1: independent replicas of the same problem
+    seed = replica_seed(w.seed, rank)  # N > 1: independent replicas of the same problem
 
     # ------------------------------------------------------------------ resident-input arm
     ctx = B.Context(w, device=str(dev), inputs_on_device=True)
@@ -217,13 +236,8 @@ def run_ours(args):
     for k in tot:
         tot[k] += st[k]
     ms = ev0.elapsed_time(ev1)
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    cnt = torch.tensor([tot["crossings"], tot["packets"], tot["dusty_crossings"]], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
-    ms_all = float(t.item())
-    crossings_all, packets_all, dusty_all = (float(x) for x in cnt.tolist())
+    ms_all, (crossings_all, packets_all, dusty_all) = reduce_over_ranks(
+        ms, [tot["crossings"], tot["packets"], tot["dusty_crossings"]], dev, world)
     value = crossings_all / (ms_all * 1e-3)
 
     # roofline of the dominant kernel (k_transport), this rank: algorithmic bytes / its own launch time
@@ -288,17 +302,13 @@ def run_ours(args):
             c_e2e += e2e_step(seed + i)["crossings"]
         barrier()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device=dev)
-        cc = torch.tensor([float(c_e2e)], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            dist.all_reduce(cc, op=dist.ReduceOp.SUM)
+        dt_all, (c_all,) = reduce_over_ranks(dt, [float(c_e2e)], dev, world)
         nsf = w.n_species * w.n_nu
         h2d = nc * 5 + 8 * (4 * nsf + 2 * w.n_nu + w.n_species * len(w.T_grid) + len(w.T_grid)
                             + 2 * nsf * len(w.T_grid) + w.n_dir + 1)
         d2h = nc * 12 + 8 * w.n_dir * w.n_nu
-        e2e = {"value": float(cc.item()) / float(tt.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": 1e3 * float(tt.item()) / e2e_steps,
+        e2e = {"value": c_all / dt_all, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": e2e_steps, "ms_per_step": 1e3 * dt_all / e2e_steps,
                "includes": "grid_create+dust_tables+source+run+read(E_lucy,T_lucy,SED)+destroy with pinned host buffers"}
 
     # ------------------------------------------------------------------ CPU baseline (rank 0, N = 1 only)
