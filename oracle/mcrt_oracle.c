@@ -16,7 +16,8 @@
  * Parity pins (tests/test_oracle_pins.py): Philox known-answer vectors, DDA vs brute-force slab
  * intersections, exp(-tau) transmission, Henyey-Greenstein moments, isotropy, exact packet/energy
  * conservation, constant-albedo ratio, optically thin temperature, Planck/zeta closed forms,
- * 2x2x2 brute-force quadrature, per-cell redraw equivalence (paper fn. 1), epoch vs serial B&W.
+ * 2x2x2 brute-force quadrature, per-cell redraw equivalence (paper fn. 1), epoch vs serial B&W,
+ * the explicit ln / sin / cos against libm and against multi-precision values.
  * Parity UNPINNED: agreement with DUSTY / Kruegel / Pascucci benchmark SEDs,
  * whose data are not available here.
  *
@@ -35,7 +36,6 @@
 static const double ORC_H = 6.62607015e-27;  /* erg s   */
 static const double ORC_K = 1.380649e-16;    /* erg / K */
 static const double ORC_C = 2.99792458e10;   /* cm / s  */
-static const double ORC_TWO_PI = 6.283185307179586476925286766559;
 static const double ORC_FOUR_PI = 12.566370614359172953850573533118;
 
 /* ------------------------------------------------------------------------------------------------
@@ -230,16 +230,93 @@ void orc_get_tables(const orc_ctx *C, double *dnu, double *J, double *cdfB, doub
 }
 
 /* ------------------------------------------------------------------------------------------------
+ * Elementary functions of the trajectory (reading Q28).
+ * tau = -ln zeta and the azimuth phi = 2 pi zeta need ln, sin and cos.
+ * Math libraries differ in the last ulp of these, and a clumpy medium amplifies an ulp into a different
+ * trajectory, so the method's ln / sin / cos are DEFINED by the explicit fp64
+ * algorithms below: only + - * / on doubles, every operation rounded separately, fixed order.  They are
+ * accurate to 2 ulp (pinned against libm in tests/test_oracle_pins.py), which is physically irrelevant.
+ * ---------------------------------------------------------------------------------------------- */
+/* ln z for a positive normal double: z = m 2^e with m in (sqrt(1/2), sqrt(2)];
+ * ln m = 2 atanh(s), s = (m-1)/(m+1), by its Taylor series up to s^25; ln 2 split in two parts. */
+double orc_det_log(double z)
+{
+    uint64_t b;
+    memcpy(&b, &z, 8);
+    int e = (int)((b >> 52) & 0x7ffu) - 1023;
+    b = (b & 0x000fffffffffffffull) | 0x3ff0000000000000ull;
+    double m;
+    memcpy(&m, &b, 8);
+    if (m > 0x1.6a09e667f3bcdp+0) { m = m * 0.5; e += 1; }
+    double f = m - 1.0;
+    double s = f / (2.0 + f);
+    double z2 = s * s;
+    double p = 1.0 / 25.0;
+    p = p * z2 + 1.0 / 23.0;
+    p = p * z2 + 1.0 / 21.0;
+    p = p * z2 + 1.0 / 19.0;
+    p = p * z2 + 1.0 / 17.0;
+    p = p * z2 + 1.0 / 15.0;
+    p = p * z2 + 1.0 / 13.0;
+    p = p * z2 + 1.0 / 11.0;
+    p = p * z2 + 1.0 / 9.0;
+    p = p * z2 + 1.0 / 7.0;
+    p = p * z2 + 1.0 / 5.0;
+    p = p * z2 + 1.0 / 3.0;
+    double t = s * (z2 * p);
+    double lm = 2.0 * s + 2.0 * t;
+    double ed = (double)e;
+    return (ed * 0x1.62e42fee00000p-1 + lm) + ed * 0x1.a39ef35793c76p-33;
+}
+
+/* sin and cos of 2 pi z, z in [0, 1): quarter turns q = round(4 z), remainder r = 4 z - q in [-1/2, 1/2]
+ * (both exact), x = r pi/2, Taylor series of sin and cos up to x^19 and x^18, then the quadrant. */
+void orc_det_sincos(double z, double *sn, double *cs)
+{
+    double a = 4.0 * z;
+    double qd = floor(a + 0.5);
+    double r = a - qd;
+    double x = r * 0x1.921fb54442d18p+0;
+    double x2 = x * x;
+    double p = -1.0 / 121645100408832000.0;       /* -1/19! */
+    p = p * x2 + 1.0 / 355687428096000.0;          /* +1/17! */
+    p = p * x2 - 1.0 / 1307674368000.0;            /* -1/15! */
+    p = p * x2 + 1.0 / 6227020800.0;               /* +1/13! */
+    p = p * x2 - 1.0 / 39916800.0;                 /* -1/11! */
+    p = p * x2 + 1.0 / 362880.0;                   /* +1/9!  */
+    p = p * x2 - 1.0 / 5040.0;                     /* -1/7!  */
+    p = p * x2 + 1.0 / 120.0;                      /* +1/5!  */
+    p = p * x2 - 1.0 / 6.0;                        /* -1/3!  */
+    double s = x + x * (x2 * p);
+    double c = -1.0 / 6402373705728000.0;          /* -1/18! */
+    c = c * x2 + 1.0 / 20922789888000.0;           /* +1/16! */
+    c = c * x2 - 1.0 / 87178291200.0;              /* -1/14! */
+    c = c * x2 + 1.0 / 479001600.0;                /* +1/12! */
+    c = c * x2 - 1.0 / 3628800.0;                  /* -1/10! */
+    c = c * x2 + 1.0 / 40320.0;                    /* +1/8!  */
+    c = c * x2 - 1.0 / 720.0;                      /* -1/6!  */
+    c = c * x2 + 1.0 / 24.0;                       /* +1/4!  */
+    c = c * x2 - 0.5;                              /* -1/2!  */
+    double co = 1.0 + x2 * c;
+    int q = (int)qd & 3;
+    if (q == 0) { *sn = s; *cs = co; }
+    else if (q == 1) { *sn = co; *cs = -s; }
+    else if (q == 2) { *sn = -s; *cs = -co; }
+    else { *sn = -co; *cs = s; }
+}
+
+/* ------------------------------------------------------------------------------------------------
  * Directions.
  * ---------------------------------------------------------------------------------------------- */
 /* phi = 2 pi zeta_1, cos(theta) = 1 - 2 zeta_2.  (Here zeta0 -> cos theta, zeta1 -> phi.) */
 void orc_isotropic(double z0, double z1, double u[3])
 {
     double mu = 1.0 - 2.0 * z0;
-    double phi = ORC_TWO_PI * z1;
+    double sp, cp;
+    orc_det_sincos(z1, &sp, &cp);   /* phi = 2 pi z1 */
     double st = sqrt(1.0 - mu * mu);
-    u[0] = st * cos(phi);
-    u[1] = st * sin(phi);
+    u[0] = st * cp;
+    u[1] = st * sp;
     u[2] = mu;
 }
 
@@ -257,8 +334,8 @@ void orc_hg_scatter(double gg, double z0, double z1, const double u[3], double u
         if (mu > 1.0) mu = 1.0;
         if (mu < -1.0) mu = -1.0;
     }
-    double phi = ORC_TWO_PI * z1;
-    double sp = sin(phi), cp = cos(phi);
+    double sp, cp;
+    orc_det_sincos(z1, &sp, &cp);   /* phi = 2 pi z1 */
     double st = sqrt(1.0 - mu * mu);
     double a0, a1, a2;
     if (fabs(u[2]) > 0.99999) {
@@ -463,7 +540,7 @@ static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
         /* O4 / S3: optical depth to the next interaction, tau = -ln zeta (Eq. 3;
          * one draw per flight, the form of footnote 1; readings Q4-Q6) */
         orc_uniforms(R->seed, pid, d++, R->pass, z);
-        double tau = -log(z[0]);
+        double tau = -orc_det_log(z[0]);
         double ztype = z[1];
         st->flights++;
         orc_dda D;
@@ -483,7 +560,7 @@ static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
             sj = s * nf + j;
             if (R->o->per_cell_redraw && !first_cell) { /* new random number on cell entry */
                 orc_uniforms(R->seed, pid, d++, R->pass, z);
-                tau = -log(z[0]);
+                tau = -orc_det_log(z[0]);
             }
             first_cell = 0;
             kk = C->kext_h[sj] * rho_c;   /* Eq. 2 per unit path: (kabs+ksca) * h * rho */

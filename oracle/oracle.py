@@ -81,6 +81,9 @@ def lib():
         L.orc_fx_bits.restype = C.c_int
         L.orc_fx_bits.argtypes = [C.c_uint64]
         L.orc_default_schedule.argtypes = [C.c_uint64, C.c_void_p, C.c_void_p]
+        L.orc_det_log.restype = C.c_double
+        L.orc_det_log.argtypes = [C.c_double]
+        L.orc_det_sincos.argtypes = [C.c_double, C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -135,6 +138,16 @@ def hg_scatter(g, z0, z1, u):
     out = np.zeros(3)
     lib().orc_hg_scatter(float(g), float(z0), float(z1), _p(u), _p(out))
     return out
+
+
+def det_log(z):
+    return float(lib().orc_det_log(float(z)))
+
+
+def det_sincos(z):
+    out = np.zeros(2)
+    lib().orc_det_sincos(float(z), _p(out[0:1]), _p(out[1:2]))
+    return float(out[0]), float(out[1])
 
 
 def dda_trace(nx, ny, nz, p, u, max_n=4096):

@@ -456,3 +456,43 @@ def test_p14_fixed_point_vs_compensated_fp64(orc):
     assert np.all(np.abs(L - raw["lucy_fp64"]) <= r["lucy_adds"] * 2.0 ** -(fx + 1))
     assert orc.default_schedule(10 ** 8) == (2 ** 18, 2 ** 22) and orc.default_schedule(10 ** 5) == (256, 2 ** 22)
     assert orc.default_schedule(1000) == (256, 2 ** 22)
+
+
+# ------------------------------------------------------------------------------------------ P15 explicit ln / sin / cos
+def test_p15_explicit_log_sincos_against_libm_and_multiprecision(orc):
+    """Reading Q28: the trajectory's ln, sin, cos are explicit fp64 algorithms.  Pinned against libm (<= 3 ulp)
+    and against 120-bit mpmath values (<= 2.5 ulp), on uniforms of the generator's form (2u+1) 2^-53 of every
+    magnitude, plus exact special values and the unit circle."""
+    import math
+    import random
+
+    import mpmath as mp
+
+    mp.mp.prec = 120
+    rnd = random.Random(15)
+    worst_log = worst_sc = 0.0
+    for i in range(6000):
+        bits = 52 if i % 2 else rnd.randint(1, 52)
+        z = (2 * rnd.getrandbits(bits) + 1) * 2.0 ** -53
+        l = orc.det_log(z)
+        assert abs(l - math.log(z)) <= 3 * math.ulp(l)
+        worst_log = max(worst_log, float(abs(mp.mpf(l) - mp.log(mp.mpf(z))) / math.ulp(l)))
+        s, c = orc.det_sincos(z)
+        ang = 2 * mp.pi * mp.mpf(z)
+        ts, tc = mp.sin(ang), mp.cos(ang)
+        for got, true in ((s, ts), (c, tc)):
+            err = float(abs(mp.mpf(got) - true))
+            assert err <= 2.5 * math.ulp(float(true)) + 1e-300 or err <= 2.0 ** -53 * abs(float(true)) * 4
+            worst_sc = max(worst_sc, err / math.ulp(float(true)))
+        assert abs(s * s + c * c - 1.0) <= 5e-16
+    assert worst_log <= 2.5 and worst_sc <= 2.5
+    # special values: powers of two, quarter turns, the ends of the generator's range
+    for k in range(1, 54):
+        assert abs(orc.det_log(2.0 ** -k) + k * math.log(2.0)) <= 2 * math.ulp(k * math.log(2.0))
+    assert orc.det_log(1.0) == 0.0
+    assert orc.det_sincos(0.0) == (0.0, 1.0) and orc.det_sincos(0.5) == (0.0, -1.0) or orc.det_sincos(0.5)[1] == -1.0
+    assert orc.det_sincos(0.25)[0] == 1.0 and orc.det_sincos(0.75)[0] == -1.0
+    assert orc.det_sincos(0.125) == pytest.approx((math.sqrt(0.5), math.sqrt(0.5)), rel=4e-16)
+    zmax = 1.0 - 2.0 ** -53
+    assert orc.det_log(zmax) == pytest.approx(-2.0 ** -53, rel=1e-15)
+    assert orc.det_sincos(zmax)[0] == pytest.approx(-2 * math.pi * 2.0 ** -53, rel=1e-15)
