@@ -171,6 +171,11 @@ int mcrt_read_tables(mcrt_ctx *ctx, double *dnu, double *J, double *cdf_B, doubl
  * (ctr [n][4], key [n][2], out [n][4]); lets the tests pin the device generator. */
 int mcrt_philox_device(const uint32_t *ctr, const uint32_t *key, uint32_t *out, uint64_t n);
 
+/* The trajectory's elementary functions computed ON THE DEVICE for n host values z in (0,1): ln z (used as
+ * tau = -ln zeta) and sin / cos of 2 pi z (azimuth).  They are explicit fp64
+ * algorithms (reading Q28), so the tests can demand bit-equality with the oracle's. */
+int mcrt_traj_math_device(const double *z, double *ln_z, double *sin_2piz, double *cos_2piz, uint64_t n);
+
 /* Use this CUDA stream (a cudaStream_t passed as void*) for all later work of the context. */
 int mcrt_set_stream(mcrt_ctx *ctx, void *cuda_stream);
 

@@ -23,7 +23,7 @@ MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP = 0, 1
 EXPORTS = [
     "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
     "mcrt_default_opts", "mcrt_run", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
-    "mcrt_philox_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
+    "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
 
@@ -82,6 +82,7 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_tables.argtypes = [vp] + [vp] * 6
     L.mcrt_philox_device.argtypes = [vp, vp, vp, u64]
+    L.mcrt_traj_math_device.argtypes = [vp, vp, vp, vp, u64]
     L.mcrt_set_stream.argtypes = [vp, vp]
     L.mcrt_launch_config.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(C.c_size_t)]
     L.mcrt_last_error.argtypes = [vp]
@@ -193,6 +194,13 @@ def mcrt_philox_device(ctr, key):
     out = np.zeros_like(c)
     _check(load_library().mcrt_philox_device(_ptr(c), _ptr(k), _ptr(out), len(c)))
     return out
+
+
+def mcrt_traj_math_device(z):
+    z = np.ascontiguousarray(z, np.float64).reshape(-1)
+    ln, s, c = np.zeros_like(z), np.zeros_like(z), np.zeros_like(z)
+    _check(load_library().mcrt_traj_math_device(_ptr(z), _ptr(ln), _ptr(s), _ptr(c), len(z)))
+    return ln, s, c
 
 
 def mcrt_set_stream(ctx, cuda_stream: int):

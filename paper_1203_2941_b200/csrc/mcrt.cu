@@ -31,7 +31,6 @@ namespace {
 constexpr double kPlanckH = 6.62607015e-27;   // erg s
 constexpr double kBoltzK = 1.380649e-16;      // erg K^-1
 constexpr double kLightC = 2.99792458e10;     // cm s^-1
-constexpr double kTwoPi = 6.283185307179586476925286766559;
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
 constexpr unsigned kFull = 0xffffffffu;
@@ -188,6 +187,75 @@ __device__ __forceinline__ void draw2(uint32_t seed_lo, uint32_t seed_hi, unsign
     const unsigned long long b = (((unsigned long long)w2 << 32) | w3) >> 12;
     z0 = __ull2double_rn(2ull * a + 1ull) * 0x1.0p-53;
     z1 = __ull2double_rn(2ull * b + 1ull) * 0x1.0p-53;
+}
+
+// Elementary functions of the trajectory (reading Q28).  tau = -ln zeta and the azimuth
+// 2 pi zeta are evaluated by explicit fp64 algorithms -- only + - * / on doubles, each rounded
+// separately (this file is compiled with -fmad=false), fixed order -- so that the result does not depend on a
+// math library's last ulp.  Coefficients are the correctly rounded doubles of 1/(2k+1) and of 1/n!.
+//
+// ln z, z a positive normal double: z = m 2^e, m in (sqrt(1/2), sqrt(2)]; ln m = 2 atanh(s), s = (m-1)/(m+1),
+// Taylor series up to s^25 (Horner in s^2); ln 2 = hi + lo with e * hi exact.
+__device__ __forceinline__ double traj_log(double z)
+{
+    int hi = __double2hiint(z);
+    const int lo = __double2loint(z);
+    int e = ((hi >> 20) & 0x7ff) - 1023;
+    double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
+    if (m > 0x1.6a09e667f3bcdp+0) { m = m * 0.5; e += 1; }
+    const double f = m - 1.0;
+    const double s = f / (2.0 + f);
+    const double w = s * s;
+    double p = 0x1.47ae147ae147bp-5;       // 1/25
+    p = p * w + 0x1.642c8590b2164p-5;      // 1/23
+    p = p * w + 0x1.8618618618618p-5;      // 1/21
+    p = p * w + 0x1.af286bca1af28p-5;      // 1/19
+    p = p * w + 0x1.e1e1e1e1e1e1ep-5;      // 1/17
+    p = p * w + 0x1.1111111111111p-4;      // 1/15
+    p = p * w + 0x1.3b13b13b13b14p-4;      // 1/13
+    p = p * w + 0x1.745d1745d1746p-4;      // 1/11
+    p = p * w + 0x1.c71c71c71c71cp-4;      // 1/9
+    p = p * w + 0x1.2492492492492p-3;      // 1/7
+    p = p * w + 0x1.999999999999ap-3;      // 1/5
+    p = p * w + 0x1.5555555555555p-2;      // 1/3
+    const double t = s * (w * p);
+    const double lm = 2.0 * s + 2.0 * t;
+    const double ed = (double)e;
+    return (ed * 0x1.62e42fee00000p-1 + lm) + ed * 0x1.a39ef35793c76p-33;
+}
+
+// sin and cos of 2 pi z, z in [0, 1): q = round(4 z) quarter turns, r = 4 z - q in [-1/2, 1/2] (both exact),
+// x = r pi/2, Taylor series to x^19 / x^18 (Horner in x^2), then the quadrant q mod 4.
+__device__ __forceinline__ void traj_sincos_turns(double z, double &sn, double &cs)
+{
+    const double a = 4.0 * z;
+    const double qd = floor(a + 0.5);
+    const double r = a - qd;
+    const double x = r * 0x1.921fb54442d18p+0;
+    const double w = x * x;
+    double p = -0x1.2f49b46814157p-57;     // -1/19!
+    p = p * w + 0x1.952c77030ad4ap-49;     // +1/17!
+    p = p * w - 0x1.ae7f3e733b81fp-41;     // -1/15!
+    p = p * w + 0x1.6124613a86d09p-33;     // +1/13!
+    p = p * w - 0x1.ae64567f544e4p-26;     // -1/11!
+    p = p * w + 0x1.71de3a556c734p-19;     // +1/9!
+    p = p * w - 0x1.a01a01a01a01ap-13;     // -1/7!
+    p = p * w + 0x1.1111111111111p-7;      // +1/5!
+    p = p * w - 0x1.5555555555555p-3;      // -1/3!
+    const double s = x + x * (w * p);
+    double c = -0x1.6827863b97d97p-53;     // -1/18!
+    c = c * w + 0x1.ae7f3e733b81fp-45;     // +1/16!
+    c = c * w - 0x1.93974a8c07c9dp-37;     // -1/14!
+    c = c * w + 0x1.1eed8eff8d898p-29;     // +1/12!
+    c = c * w - 0x1.27e4fb7789f5cp-22;     // -1/10!
+    c = c * w + 0x1.a01a01a01a01ap-16;     // +1/8!
+    c = c * w - 0x1.6c16c16c16c17p-10;     // -1/6!
+    c = c * w + 0x1.5555555555555p-5;      // +1/4!
+    c = c * w - 0.5;                       // -1/2!
+    const double co = 1.0 + w * c;
+    const int q = (int)qd & 3;
+    sn = (q == 0) ? s : (q == 1) ? co : (q == 2) ? -s : -co;
+    cs = (q == 0) ? co : (q == 1) ? -s : (q == 2) ? -co : s;
 }
 
 // smallest j with cdf[j] >= z (Eq. 5 / Eq. 10: "the shortest frequency nu' for which ...")
@@ -833,9 +901,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         mu = fmax(mu, -1.0);
                     }
                 }
-                const double phi = kTwoPi * z1;
                 double sp, cp;
-                sincos(phi, &sp, &cp);
+                traj_sincos_turns(z1, sp, cp);   // phi = 2 pi z1
                 const double st = sqrt(1.0 - mu * mu);
                 if (scatter) {
                     double a0, a1, a2;
@@ -876,7 +943,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 SF(F_PX, slot) = px; SF(F_PY, slot) = py; SF(F_PZ, slot) = pz;
                 SF(F_UX, slot) = ux; SF(F_UY, slot) = uy; SF(F_UZ, slot) = uz;
                 SF(F_T, slot) = 0.0;
-                SF(F_TAU, slot) = -log(z0);
+                SF(F_TAU, slot) = -traj_log(z0);
                 SF(F_ZTYPE, slot) = z1;
                 SF(F_CW, slot) = __longlong_as_double((long long)cw);
                 SF(F_PID, slot) = __longlong_as_double((long long)pid);
@@ -1170,6 +1237,16 @@ __global__ void k_sed(double *__restrict__ out, const unsigned long long *__rest
         const int b = i / nf, j = i % nf;
         const double dom = kFourPi * (mu[b + 1] - mu[b]);
         out[i] = (double)sed[i] * xi / (dnu[j] * dom);
+    }
+}
+
+__global__ void k_traj_math_test(const double *__restrict__ z, double *__restrict__ out, unsigned long long n)
+{
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        double s, c;
+        traj_sincos_turns(z[i], s, c);
+        out[3 * i] = traj_log(z[i]); out[3 * i + 1] = s; out[3 * i + 2] = c;
     }
 }
 
@@ -1839,6 +1916,24 @@ int mcrt_philox_device(const uint32_t *ctr, const uint32_t *key, uint32_t *out, 
     if (e == cudaSuccess) e = cudaMemcpy(out, dout, n * 16, cudaMemcpyDeviceToHost);
     cudaFree(d);
     if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
+    return MCRT_OK;
+}
+
+int mcrt_traj_math_device(const double *z, double *ln_z, double *sin_2piz, double *cos_2piz, uint64_t n)
+{
+    if (!z || !ln_z || !sin_2piz || !cos_2piz || n == 0) return MCRT_EINVAL;
+    double *d = nullptr;
+    if (cudaMalloc(&d, n * 4 * sizeof(double)) != cudaSuccess) return fail(nullptr, MCRT_ENOMEM, "cudaMalloc failed");
+    std::vector<double> h(3 * n);
+    cudaError_t e = cudaMemcpy(d, z, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_traj_math_test<<<(unsigned)((n + 255) / 256), 256>>>(d, d + n, n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(h.data(), d + n, 3 * n * sizeof(double), cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
+    for (uint64_t i = 0; i < n; ++i) { ln_z[i] = h[3 * i]; sin_2piz[i] = h[3 * i + 1]; cos_2piz[i] = h[3 * i + 2]; }
     return MCRT_OK;
 }
 
