@@ -311,6 +311,7 @@ struct TransportParams {
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
     int nbx, nby;       // bricks per axis
+    uint32_t ncp;       // padded cell count: cellw[ncp] holds the marker word kJumpWord
     int bsh;            // log2 of the brick edge
     int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
@@ -338,6 +339,14 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
 {
     const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
     atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
+}
+
+// the same, issued only where on != 0 (a predicated RED instead of a branch around it)
+__device__ __forceinline__ void lucy_add_if(long long *__restrict__ lfx, uint32_t cidx, double x, uint32_t on)
+{
+    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}" ::"l"(lfx + cidx), "l"(q), "r"(on)
+                 : "memory");
 }
 
 // Warp-aggregated tallies ("local copies reduce interference").  The lanes of the calling group
@@ -393,9 +402,6 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #endif
 #ifndef MCRT_S_LEAVE
 #define MCRT_S_LEAVE 14             // ... and ends when this many lanes are idle and nothing is left to refill them
-#endif
-#ifndef MCRT_S_MATCH
-#define MCRT_S_MATCH 0              // 1: the per-crossing Lucy adds of the S phase are warp-aggregated as well
 #endif
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
@@ -571,10 +577,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             int nidle = 32;
             bool first = true;
 
+#ifndef MCRT_S_MATCH
+#define MCRT_S_MATCH 0              // 1 (experiment): warp-aggregate the per-crossing Lucy adds too; 2.5-5x slower
+#endif
 #if MCRT_S_MATCH
-#define S_LUCY_ADD lucy_add_aggregated
+#define S_LUCY_ADD(L, C, X, ON) do { if (ON) lucy_add_aggregated(L, C, X); } while (0)
 #else
-#define S_LUCY_ADD lucy_add
+#define S_LUCY_ADD(L, C, X, ON) lucy_add_if(L, C, X, ON)
 #endif
 // One step.  G advances one cell: queue entry 2 (whose exit parameter is the parameter at which cell n was
 // entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0; entry 1 only tells
@@ -605,8 +614,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);                                            \
                 gcidx = cell_in_brick(brick, gx, gy, gz, bsh);                                                         \
                 unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;        \
-                if (!brick_empty(s_m0, brick)) cp_async8(dst, P.cellw + gcidx);                                        \
-                else *reinterpret_cast<volatile unsigned long long *>(dst) = kJumpWord;                                \
+                /* cells of an empty brick are not read: their request goes to the marker word behind the grid */     \
+                cp_async8(dst, P.cellw + (brick_empty(s_m0, brick) ? P.ncp : gcidx));                                  \
             }                                                                                                          \
         }                                                                                                              \
         cp_async_commit();                                                                                             \
@@ -631,9 +640,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             continue;                                                                                                  \
         }                                                                                                              \
         tau -= dtau;                                                                                                   \
-        if (!cw_vacuum(cw)) {                                                                                          \
-            S_LUCY_ADD(P.lfx, CI0, kq.y * rho_c * ds);                                                                 \
-            ndusty_acc++;                                                                                              \
+        { /* S5: predicated, no branch: a vacuum cell (rho = 0) would add 0 */                                         \
+            const uint32_t dusty = cw_vacuum(cw) ? 0u : 1u;                                                            \
+            S_LUCY_ADD(P.lfx, CI0, kq.y * rho_c * ds, dusty);                                                          \
+            ndusty_acc += dusty;                                                                                       \
         }                                                                                                              \
         ncross++;                                                                                                      \
         r = (r + 1) & 3;                                                                                               \
@@ -1098,6 +1108,7 @@ __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__rest
         }
         cellw[b] = cw;
     }
+    if (blockIdx.x == 0 && threadIdx.x == 0) cellw[ncp] = kJumpWord;   // marker word behind the grid
 }
 
 // Vacuum mask of one level: bit of box (bx, by, bz) is set when all its in-grid cells have rho == 0.
@@ -1369,7 +1380,7 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     const size_t ncp = nbricks << (3 * mg.msh);
     size_t b = 0;
     auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
-    add(ncp * sizeof(uint2));            // cell words
+    add((ncp + 1) * sizeof(uint2));      // cell words + marker word
     add((size_t)mg.mwords * 4);          // vacuum mask
     add(nbricks * sizeof(uint4));        // empty boxes of the J phase
     add((size_t)(mg.nbx + 1) * (mg.nby + 1) * (mg.nbz + 1) * sizeof(int));   // summed-area scratch
@@ -1432,7 +1443,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
             return MCRT_ECUDA;                                                                         \
         }                                                                                              \
     } while (0)
-    GC_TRY(ws_alloc(c, (void **)&c->cellw, c->ncp * sizeof(uint2)));
+    GC_TRY(ws_alloc(c, (void **)&c->cellw, (c->ncp + 1) * sizeof(uint2)));   // + the marker word
     GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
     GC_TRY(ws_alloc(c, (void **)&c->vbox, (size_t)c->nbx * c->nby * c->nbz * sizeof(uint4)));
     GC_TRY(ws_alloc(c, (void **)&c->vsat, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int)));
@@ -1757,7 +1768,7 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
     P.dig = o.record_digests ? c->dig : nullptr;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
     P.nbx = c->nbx; P.nby = c->nby;
-    P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords;
+    P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords; P.ncp = (uint32_t)c->ncp;
     P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
     P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     const size_t j_smem = (size_t)c->ns * c->nT * 8;
