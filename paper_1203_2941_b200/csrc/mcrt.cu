@@ -596,7 +596,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         const double t_in = TN2;                                                                                       \
         CI2 = gcidx;                                                                                                   \
         XZ2 = pack_xyz(gx, gy, gz);                                                                                    \
-        if (gcidx != kOutCell) {                                                                                       \
+        { /* branch-free: a G that has left the grid keeps stepping outwards and requests the marker word */         \
+            const bool gin = gcidx != kOutCell;                                                                        \
             const bool selx = (tmx <= tmy) && (tmx <= tmz);                                                            \
             const bool sely = !selx && (tmy <= tmz);                                                                   \
             const bool selz = !selx && !sely;                                                                          \
@@ -609,18 +610,18 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             if (selx) { fdx += sdx; tmx = (fdx - px) * ivx; }                                                          \
             if (sely) { fdy += sdy; tmy = (fdy - py) * ivy; }                                                          \
             if (selz) { fdz += sdz; tmz = (fdz - pz) * ivz; }                                                          \
-            gcidx = kOutCell;                                                                                          \
-            if (((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) & ((unsigned)gz < (unsigned)P.nz)) { \
-                const uint32_t brick = brick_of(gx, gy, gz, nbx, nby, bsh);                                            \
-                gcidx = cell_in_brick(brick, gx, gy, gz, bsh);                                                         \
-                unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;        \
-                /* cells of an empty brick are not read: their request goes to the marker word behind the grid */     \
-                cp_async8(dst, P.cellw + (brick_empty(s_m0, brick) ? P.ncp : gcidx));                                  \
-            }                                                                                                          \
+            const bool inside = gin & ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &              \
+                                ((unsigned)gz < (unsigned)P.nz);                                                       \
+            const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;                                  \
+            const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);                                               \
+            gcidx = inside ? cell : kOutCell;                                                                          \
+            unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;            \
+            /* cells of an empty brick are not read: their request goes to the marker word behind the grid */         \
+            cp_async8(dst, P.cellw + ((inside && !brick_empty(s_m0, brick)) ? cell : P.ncp));                          \
         }                                                                                                              \
         cp_async_commit();                                                                                             \
         /* physics of cell n */                                                                                        \
-        if (cw == kJumpWord) { /* cell n starts a run of empty bricks: J phase */                                      \
+        if ((uint32_t)cw & (uint32_t)kJumpWord) { /* bit 28: cell n starts a run of empty bricks: J phase */            \
             SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0; SU(U_NCROSS, slot) = ncross;            \
             state = ST_JUMP;                                                                                           \
             continue;                                                                                                  \
