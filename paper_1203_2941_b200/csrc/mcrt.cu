@@ -395,13 +395,13 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #define MCRT_MAX_THREADS 512        // 16 warps per SM, up to 128 registers per thread (640 = 20 warps measured no faster)
 #endif
 #ifndef MCRT_SWAP_MIN
-#define MCRT_SWAP_MIN 10            // S phase: stopped packets are parked / replaced this many lanes at a time
+#define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
 #ifndef MCRT_S_ENTER
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
 #endif
 #ifndef MCRT_S_LEAVE
-#define MCRT_S_LEAVE 14             // ... and ends when this many lanes are idle and nothing is left to refill them
+#define MCRT_S_LEAVE 10             // ... and ends when this many lanes are idle and nothing is left to refill them
 #endif
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
