@@ -397,6 +397,9 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #ifndef MCRT_SWAP_MIN
 #define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
+#ifndef MCRT_S_UNROLL
+#define MCRT_S_UNROLL 1             // cells per S-loop body: 1 (queue rotated by moves; the loop fits the instruction cache) or 3
+#endif
 #ifndef MCRT_S_ENTER
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
 #endif
@@ -574,7 +577,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
             int kq_sp = -1;
             int r = 0;                                          // ring slot of cell n
-            int nidle = 32;
+            int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
             bool first = true;
 
 #ifndef MCRT_S_MATCH
@@ -668,7 +671,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const int nfl = 32 - __popc(idle);
                     // nothing left to refill with and many lanes idle: let the other phases make flying packets
                     if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty())))) {
-                        if (state == ST_FLY) {   // park mid-flight: cell n is entry A, entered at tnC
+                        // park mid-flight: cell n is entry A, entered at tnC.  A packet still behind its no-op cells has
+                        // not started: its slot is as the refill found it
+                        if (state == ST_FLY && prime == 0) {
                             cp_async_wait<0>();
                             SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
                             SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
@@ -712,6 +717,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         ring[0] = 0ull; ring[ring_stride] = 0ull;
                         ring[2 * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                         tnA = t; tnB = t; tnC = t; ciA = 0u; ciB = 0u; xzA = w0; xzB = w0;
+                        prime = 2;
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
@@ -720,9 +726,21 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 }
                 // ---- three steps
                 if (state == ST_FLY) {
+#if MCRT_S_UNROLL == 3
                     S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
                     S_STEP(tnB, ciB, xzB, ciC, tnA, ciA, xzA)
                     S_STEP(tnC, ciC, xzC, ciA, tnB, ciB, xzB)
+                    prime = 0;
+#else
+                    // one step per iteration: the loop fits the instruction cache next to the scheduler; the queue
+                    // is rotated by moves, (A, B, C) <- (B, C, A)
+                    S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
+                    const double tt = tnA; const uint32_t tc = ciA, tx = xzA;
+                    tnA = tnB; ciA = ciB; xzA = xzB;
+                    tnB = tnC; ciB = ciC; xzB = xzC;
+                    tnC = tt; ciC = tc; xzC = tx;
+                    prime = max(prime - 1, 0);
+#endif
                 }
             }
 #undef S_STEP
