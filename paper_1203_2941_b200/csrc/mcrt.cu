@@ -404,7 +404,7 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
 #endif
 #ifndef MCRT_S_LEAVE
-#define MCRT_S_LEAVE 10             // ... and ends when this many lanes are idle and nothing is left to refill them
+#define MCRT_S_LEAVE 8              // ... and ends when this many lanes are idle and nothing is left to refill them
 #endif
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
@@ -578,7 +578,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             int kq_sp = -1;
             int r = 0;                                          // ring slot of cell n
             int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
-            bool first = true;
 
 #ifndef MCRT_S_MATCH
 #define MCRT_S_MATCH 0              // 1 (experiment): warp-aggregate the per-crossing Lucy adds too; 2.5-5x slower
@@ -661,9 +660,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
-                const int nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
-                if (first || nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) {
-                    first = false;
+                {
                     mJ.add(state == ST_JUMP, slot);
                     mEv.add(state == ST_DONE || state == ST_INTERACT, slot);
                     if (state != ST_FLY) state = ST_IDLE;
@@ -724,7 +721,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     mFly.remove(take, slot);
                     nidle = __popc(__ballot_sync(kFull, state == ST_IDLE));
                 }
-                // ---- three steps
+                // ---- the walk: a tight inner loop (nothing but the step, so that it stays in the instruction cache)
+                // until MCRT_SWAP_MIN more lanes have stopped
+                int nnot;
+                do {
                 if (state == ST_FLY) {
 #if MCRT_S_UNROLL == 3
                     S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
@@ -742,6 +742,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     prime = max(prime - 1, 0);
 #endif
                 }
+                } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
             }
 #undef S_STEP
             __syncwarp();
