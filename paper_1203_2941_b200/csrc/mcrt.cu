@@ -397,9 +397,6 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #ifndef MCRT_SWAP_MIN
 #define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
-#ifndef MCRT_S_UNROLL
-#define MCRT_S_UNROLL 1             // cells per S-loop body: 1 (queue rotated by moves; the loop fits the instruction cache) or 3
-#endif
 #ifndef MCRT_S_ENTER
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
 #endif
@@ -519,11 +516,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
     const int nhist = 2 * P.ndir * P.nf;
     uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
-    // cell-word ring: slot k of thread i at s_ring[k * blockDim.x + i]
+    // cell-word ring: slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
     unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.mwords + 1) & ~1));
 
-    volatile unsigned long long *ring = s_ring + threadIdx.x;
-    const int ring_stride = blockDim.x;
+    volatile unsigned long long *ring = s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u);
+    constexpr int ring_stride = 32;
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -560,8 +557,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             // (G: axis choice, next cell, exit parameter) runs two cells ahead of the physics and the cell words
             // travel global -> shared memory with cp.async into a small per-thread ring: the latency of a
             // cell's word is covered by two walk iterations of every resident warp.  The queue between G and
-            // the physics (exit parameter, storage index, packed coordinates of cells n and n+1) rotates through
-            // three register sets A, B, C, so the loop body is three steps and nothing is moved.
+            // the physics (exit parameter, storage index, packed coordinates of cells n, n+1, n+2) is three
+            // register sets A, B, C, rotated by moves after every step.  The ring slot of cell n is the same in
+            // every lane, so the ring addresses are warp-uniform arithmetic.
             // Lanes whose packet reaches an event or an empty brick park it and take another flying packet
             // from the pool without leaving the loop; a new packet enters the pipeline behind two no-op cells
             // (zero length, vacuum), which the physics passes without effect.  The phase ends when the pool has
@@ -576,25 +574,31 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             uint32_t gcidx = 0u, ncross = 0u;
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
             int kq_sp = -1;
-            int r = 0;                                          // ring slot of cell n
+            int r = 0;                                          // ring slot of cell n: the same in every lane (warp-uniform)
             int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
 
+#ifndef MCRT_S_RED_ALWAYS
+#define MCRT_S_RED_ALWAYS 1             // S phase: every stepped cell issues its RED (a vacuum cell adds 0): no branch around it
+#endif
 #ifndef MCRT_S_MATCH
 #define MCRT_S_MATCH 0              // 1 (experiment): warp-aggregate the per-crossing Lucy adds too; 2.5-5x slower
 #endif
 #if MCRT_S_MATCH
 #define S_LUCY_ADD(L, C, X, ON) do { if (ON) lucy_add_aggregated(L, C, X); } while (0)
 #else
+#if MCRT_S_RED_ALWAYS
+#define S_LUCY_ADD(L, C, X, ON) lucy_add(L, C, X)   /* a vacuum cell adds 0 */
+#else
 #define S_LUCY_ADD(L, C, X, ON) lucy_add_if(L, C, X, ON)
 #endif
+#endif
 // One step.  G advances one cell: queue entry 2 (whose exit parameter is the parameter at which cell n was
-// entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0; entry 1 only tells
-// whether cell n+1 is outside the grid.  A packet that stops writes what the next phase needs into its slot and
-// leaves the loop body.
-#define S_STEP(TN0, CI0, XZ0, CI1, TN2, CI2, XZ2)                                                                     \
+// entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0.  A packet that
+// stops writes what the next phase needs into its slot and leaves the loop body.
+#define S_STEP(TN0, CI0, XZ0, TN2, CI2, XZ2)                                                                          \
     {                                                                                                                  \
         cp_async_wait<2>(); /* the word of cell n has landed */                                                        \
-        const unsigned long long cw = ring[r * ring_stride];                                                           \
+        const unsigned long long cw = ring[rc * ring_stride];                                                          \
         const double t_in = TN2;                                                                                       \
         CI2 = gcidx;                                                                                                   \
         XZ2 = pack_xyz(gx, gy, gz);                                                                                    \
@@ -617,17 +621,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;                                  \
             const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);                                               \
             gcidx = inside ? cell : kOutCell;                                                                          \
-            unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((r + 3) & 3) * ring_stride;            \
+            unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((rc + 3) & 3) * ring_stride;           \
             /* cells of an empty brick are not read: their request goes to the marker word behind the grid */         \
-            cp_async8(dst, P.cellw + ((inside && !brick_empty(s_m0, brick)) ? cell : P.ncp));                          \
+            cp_async8(dst, P.cellw + ((inside & !brick_empty(s_m0, brick)) ? cell : P.ncp));                           \
         }                                                                                                              \
         cp_async_commit();                                                                                             \
-        /* physics of cell n */                                                                                        \
-        if ((uint32_t)cw & (uint32_t)kJumpWord) { /* bit 28: cell n starts a run of empty bricks: J phase */            \
-            SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0; SU(U_NCROSS, slot) = ncross;            \
-            state = ST_JUMP;                                                                                           \
-            continue;                                                                                                  \
-        }                                                                                                              \
+        /* physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick and the   */   \
+        /* word requested for a cell outside the grid are both the marker word (bit 28; rho = 0, so dtau = 0) */   \
         const double ds = TN0 - t_in;                                                                                  \
         const double rho_c = cw_rho(cw);                                                                               \
         if (cw_species(cw) != kq_sp) { /* opacities of this species at the packet's frequency: kept in registers */   \
@@ -635,27 +635,31 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             kq = s_kk[kq_sp * nf + j];                                                                                 \
         }                                                                                                              \
         const double dtau = kq.x * rho_c * ds; /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */                 \
-        if (dtau > tau) { /* interaction inside this cell (equality leaves, Q5) */                                     \
-            SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0; SU(U_NCROSS, slot) = ncross;            \
-            SF(F_CW, slot) = __longlong_as_double((long long)cw);                                                      \
-            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);                                      \
-            state = ST_INTERACT;                                                                                       \
+        const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;                                                \
+        if (__builtin_expect(marker || dtau > tau, 0)) { /* interaction inside this cell: equality leaves (Q5) */     \
+            SU(U_NCROSS, slot) = ncross;                                                                               \
+            if (CI0 == kOutCell) { /* cell n lies outside: the packet has left the grid, escape tally in the E phase */ \
+                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);                                   \
+                state = ST_DONE;                                                                                       \
+            } else {                                                                                                   \
+                SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0;                                     \
+                if (marker) { /* cell n starts a run of empty bricks: J phase */                                       \
+                    state = ST_JUMP;                                                                                   \
+                } else {                                                                                               \
+                    SF(F_CW, slot) = __longlong_as_double((long long)cw);                                              \
+                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);                              \
+                    state = ST_INTERACT;                                                                               \
+                }                                                                                                      \
+            }                                                                                                          \
             continue;                                                                                                  \
         }                                                                                                              \
         tau -= dtau;                                                                                                   \
-        { /* S5: predicated, no branch: a vacuum cell (rho = 0) would add 0 */                                         \
+        { /* S5: no branch: a vacuum cell (rho = 0) adds 0 */                                                          \
             const uint32_t dusty = cw_vacuum(cw) ? 0u : 1u;                                                            \
             S_LUCY_ADD(P.lfx, CI0, kq.y * rho_c * ds, dusty);                                                          \
             ndusty_acc += dusty;                                                                                       \
         }                                                                                                              \
         ncross++;                                                                                                      \
-        r = (r + 1) & 3;                                                                                               \
-        if (CI1 == kOutCell) { /* left the grid: escape tally in the E phase */                                        \
-            SU(U_NCROSS, slot) = ncross;                                                                               \
-            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);                                       \
-            state = ST_DONE;                                                                                           \
-            continue;                                                                                                  \
-        }                                                                                                              \
     }
 
             for (;;) {
@@ -672,12 +676,18 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // not started: its slot is as the refill found it
                         if (state == ST_FLY && prime == 0) {
                             cp_async_wait<0>();
-                            SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
-                            SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
-                            SU(U_W0, slot) = xzA;
                             SU(U_NCROSS, slot) = ncross;
+                            if (ciA == kOutCell) {     // cell n lies outside the grid: the packet has escaped
+                                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                                state = ST_DONE;
+                            } else {
+                                SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
+                                SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
+                                SU(U_W0, slot) = xzA;
+                            }
                         }
                         mFly.add(state == ST_FLY, slot);
+                        mEv.add(state == ST_DONE, slot);
                         break;
                     }
                     const int k = __popc(idle & ((1u << lane) - 1u));
@@ -710,10 +720,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         fdz = (double)(gz + ((stz + 1) >> 1)); sdz = (double)stz;
                         gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
                         // pipeline: two no-op cells (zero length, vacuum word), then the packet's cell
-                        r = 0;
-                        ring[0] = 0ull; ring[ring_stride] = 0ull;
-                        ring[2 * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        tnA = t; tnB = t; tnC = t; ciA = 0u; ciB = 0u; xzA = w0; xzB = w0;
+                        ring[r * ring_stride] = 0ull; ring[((r + 1) & 3) * ring_stride] = 0ull;
+                        ring[((r + 2) & 3) * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        tnA = t; tnB = t; tnC = t; ciA = gcidx; ciB = gcidx; xzA = w0; xzB = w0;
                         prime = 2;
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
@@ -725,22 +734,18 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // until MCRT_SWAP_MIN more lanes have stopped
                 int nnot;
                 do {
+                const int rc = r;               // ring slot of cell n in this step
+                r = (r + 1) & 3;
                 if (state == ST_FLY) {
-#if MCRT_S_UNROLL == 3
-                    S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
-                    S_STEP(tnB, ciB, xzB, ciC, tnA, ciA, xzA)
-                    S_STEP(tnC, ciC, xzC, ciA, tnB, ciB, xzB)
-                    prime = 0;
-#else
-                    // one step per iteration: the loop fits the instruction cache next to the scheduler; the queue
-                    // is rotated by moves, (A, B, C) <- (B, C, A)
-                    S_STEP(tnA, ciA, xzA, ciB, tnC, ciC, xzC)
+                    // one step per iteration: the loop (3 KB) fits the instruction cache next to the scheduler; the
+                    // queue is rotated by moves, (A, B, C) <- (B, C, A).  Three steps per iteration without the moves
+                    // measured 7 % slower (10 KB).
+                    S_STEP(tnA, ciA, xzA, tnC, ciC, xzC)
                     const double tt = tnA; const uint32_t tc = ciA, tx = xzA;
                     tnA = tnB; ciA = ciB; xzA = xzB;
                     tnB = tnC; ciB = ciC; xzB = xzC;
                     tnC = tt; ciC = tc; xzC = tx;
                     prime = max(prime - 1, 0);
-#endif
                 }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
             }
