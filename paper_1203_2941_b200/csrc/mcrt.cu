@@ -519,8 +519,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     // cell-word ring: slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
     unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.mwords + 1) & ~1));
 
-    volatile unsigned long long *ring = s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u);
-    constexpr int ring_stride = 32;
+    char *ring = reinterpret_cast<char *>(s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u));
+    constexpr int kRingStep = 32 * 8, kRingMask = (kRing - 1) * kRingStep;   // ring slots as byte offsets 0, 256, 512, 768
+#define RING(off) (*reinterpret_cast<volatile unsigned long long *>(ring + (off)))
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -568,13 +569,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
             double tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;  // tn: parameter at which the cell of the entry is left
             double fdx = 0.0, fdy = 0.0, fdz = 0.0;             // coordinate of the face through which G's cell is left
-            double sdx = 0.0, sdy = 0.0, sdz = 0.0;             // step per axis as a double (+1, -1 or 0)
+            int shx = 0, shy = 0, shz = 0;                      // high word of the step per axis as a double (+1, -1 or 0)
             int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
             uint32_t ciA = 0u, ciB = 0u, ciC = 0u, xzA = 0u, xzB = 0u, xzC = 0u;   // storage index, packed coordinates
             uint32_t gcidx = 0u, ncross = 0u;
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
             int kq_sp = -1;
-            int r = 0;                                          // ring slot of cell n: the same in every lane (warp-uniform)
+            int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
             int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
 
 #ifndef MCRT_S_RED_ALWAYS
@@ -598,7 +599,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 #define S_STEP(TN0, CI0, XZ0, TN2, CI2, XZ2)                                                                          \
     {                                                                                                                  \
         cp_async_wait<2>(); /* the word of cell n has landed */                                                        \
-        const unsigned long long cw = ring[rc * ring_stride];                                                          \
+        const unsigned long long cw = RING(rc);                                                                        \
         const double t_in = TN2;                                                                                       \
         CI2 = gcidx;                                                                                                   \
         XZ2 = pack_xyz(gx, gy, gz);                                                                                    \
@@ -612,16 +613,21 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             gy += sely ? sty : 0;                                                                                      \
             gz += selz ? stz : 0;                                                                                      \
             /* parameter of the face through which the entered cell will be left (reading Q8): the face        */   \
-            /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u)                       */   \
-            if (selx) { fdx += sdx; tmx = (fdx - px) * ivx; }                                                          \
-            if (sely) { fdy += sdy; tmy = (fdy - py) * ivy; }                                                          \
-            if (selz) { fdz += sdz; tmz = (fdz - pz) * ivz; }                                                          \
+            /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'  */   \
+            /* f moves by its step, the others by 0, and all three t are recomputed: the same value for an      */   \
+            /* axis that did not move, so nothing has to be selected afterwards                                 */   \
+            fdx += __hiloint2double(selx ? shx : 0, 0);                                                                \
+            fdy += __hiloint2double(sely ? shy : 0, 0);                                                                \
+            fdz += __hiloint2double(selz ? shz : 0, 0);                                                                \
+            tmx = (fdx - px) * ivx;                                                                                    \
+            tmy = (fdy - py) * ivy;                                                                                    \
+            tmz = (fdz - pz) * ivz;                                                                                    \
             const bool inside = gin & ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &              \
                                 ((unsigned)gz < (unsigned)P.nz);                                                       \
             const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;                                  \
             const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);                                               \
             gcidx = inside ? cell : kOutCell;                                                                          \
-            unsigned long long *dst = const_cast<unsigned long long *>(ring) + ((rc + 3) & 3) * ring_stride;           \
+            void *dst = ring + ((rc + 3 * kRingStep) & kRingMask);                                                     \
             /* cells of an empty brick are not read: their request goes to the marker word behind the grid */         \
             cp_async8(dst, P.cellw + ((inside & !brick_empty(s_m0, brick)) ? cell : P.ncp));                           \
         }                                                                                                              \
@@ -682,7 +688,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                                 state = ST_DONE;
                             } else {
                                 SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
-                                SF(F_CW, slot) = __longlong_as_double((long long)ring[r * ring_stride]);
+                                SF(F_CW, slot) = __longlong_as_double((long long)RING(r));
                                 SU(U_W0, slot) = xzA;
                             }
                         }
@@ -715,13 +721,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         tmx = mcrt::face_t(gx, stx, px, ivx);
                         tmy = mcrt::face_t(gy, sty, py, ivy);
                         tmz = mcrt::face_t(gz, stz, pz, ivz);
-                        fdx = (double)(gx + ((stx + 1) >> 1)); sdx = (double)stx;
-                        fdy = (double)(gy + ((sty + 1) >> 1)); sdy = (double)sty;
-                        fdz = (double)(gz + ((stz + 1) >> 1)); sdz = (double)stz;
+                        // an axis that never moves: f = +inf, so that (f - p) * (1/u) = inf * inf stays +inf
+                        fdx = stx ? (double)(gx + ((stx + 1) >> 1)) : CUDART_INF; shx = __double2hiint((double)stx);
+                        fdy = sty ? (double)(gy + ((sty + 1) >> 1)) : CUDART_INF; shy = __double2hiint((double)sty);
+                        fdz = stz ? (double)(gz + ((stz + 1) >> 1)) : CUDART_INF; shz = __double2hiint((double)stz);
                         gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
                         // pipeline: two no-op cells (zero length, vacuum word), then the packet's cell
-                        ring[r * ring_stride] = 0ull; ring[((r + 1) & 3) * ring_stride] = 0ull;
-                        ring[((r + 2) & 3) * ring_stride] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        RING(r) = 0ull; RING((r + kRingStep) & kRingMask) = 0ull;
+                        RING((r + 2 * kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                         tnA = t; tnB = t; tnC = t; ciA = gcidx; ciB = gcidx; xzA = w0; xzB = w0;
                         prime = 2;
                         kq_sp = 0; kq = s_kk[j];
@@ -735,7 +742,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 int nnot;
                 do {
                 const int rc = r;               // ring slot of cell n in this step
-                r = (r + 1) & 3;
+                r = (r + kRingStep) & kRingMask;
                 if (state == ST_FLY) {
                     // one step per iteration: the loop (3 KB) fits the instruction cache next to the scheduler; the
                     // queue is rotated by moves, (A, B, C) <- (B, C, A).  Three steps per iteration without the moves
@@ -997,6 +1004,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         }
     }
 #undef SF
+#undef RING
 #undef SU
     if (ndusty_acc) atomicAdd(&s_cnt[CNT_DUSTY], (unsigned long long)ndusty_acc);
 
