@@ -341,14 +341,6 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
     atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
 }
 
-// the same, issued only where on != 0 (a predicated RED instead of a branch around it)
-__device__ __forceinline__ void lucy_add_if(long long *__restrict__ lfx, uint32_t cidx, double x, uint32_t on)
-{
-    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}" ::"l"(lfx + cidx), "l"(q), "r"(on)
-                 : "memory");
-}
-
 // Warp-aggregated tallies ("local copies reduce interference").  The lanes of the calling group
 // that address the same cell are found with __match_any_sync; their integer contributions are summed with
 // __reduce_add_sync in three 16-bit limbs (x < 2^46, so 32 lanes cannot overflow a limb sum) and the lowest
@@ -555,118 +547,28 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
-            // (G: axis choice, next cell, exit parameter) runs two cells ahead of the physics and the cell words
-            // travel global -> shared memory with cp.async into a small per-thread ring: the latency of a
-            // cell's word is covered by two walk iterations of every resident warp.  The queue between G and
-            // the physics (exit parameter, storage index, packed coordinates of cells n, n+1, n+2) is three
-            // register sets A, B, C, rotated by moves after every step.  The ring slot of cell n is the same in
-            // every lane, so the ring addresses are warp-uniform arithmetic.
+            // (G: axis choice, next cell, exit parameter) runs ahead of the physics and the cell words travel
+            // global -> shared memory with cp.async into a small per-thread ring: the word of cell n+2 is
+            // requested in the step that handles cell n, so its latency is covered by two walk iterations of
+            // every resident warp.  Between G and the physics sits one queue entry (exit parameter, storage
+            // index, packed coordinates of cell n).  The ring slot of cell n is the same in every lane.
             // Lanes whose packet reaches an event or an empty brick park it and take another flying packet
-            // from the pool without leaving the loop; a new packet enters the pipeline behind two no-op cells
+            // from the pool without leaving the loop; a new packet enters the pipeline behind one no-op cell
             // (zero length, vacuum), which the physics passes without effect.  The phase ends when the pool has
             // no flying packet left for MCRT_S_LEAVE idle lanes.
             int slot = 0, state = ST_IDLE;
             double px = 0.0, py = 0.0, pz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0, tmx = 0.0, tmy = 0.0, tmz = 0.0;
-            double tau = 0.0, tnA = 0.0, tnB = 0.0, tnC = 0.0;  // tn: parameter at which the cell of the entry is left
+            double tau = 0.0;
+            double tprev = 0.0, tnA = 0.0;                      // parameters at which cell n is entered and left
             double fdx = 0.0, fdy = 0.0, fdz = 0.0;             // coordinate of the face through which G's cell is left
             int shx = 0, shy = 0, shz = 0;                      // high word of the step per axis as a double (+1, -1 or 0)
             int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-            uint32_t ciA = 0u, ciB = 0u, ciC = 0u, xzA = 0u, xzB = 0u, xzC = 0u;   // storage index, packed coordinates
+            uint32_t ciA = 0u, xzA = 0u;                        // storage index and packed coordinates of cell n
             uint32_t gcidx = 0u, ncross = 0u;
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
             int kq_sp = -1;
             int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
             int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
-
-#ifndef MCRT_S_RED_ALWAYS
-#define MCRT_S_RED_ALWAYS 1             // S phase: every stepped cell issues its RED (a vacuum cell adds 0): no branch around it
-#endif
-#ifndef MCRT_S_MATCH
-#define MCRT_S_MATCH 0              // 1 (experiment): warp-aggregate the per-crossing Lucy adds too; 2.5-5x slower
-#endif
-#if MCRT_S_MATCH
-#define S_LUCY_ADD(L, C, X, ON) do { if (ON) lucy_add_aggregated(L, C, X); } while (0)
-#else
-#if MCRT_S_RED_ALWAYS
-#define S_LUCY_ADD(L, C, X, ON) lucy_add(L, C, X)   /* a vacuum cell adds 0 */
-#else
-#define S_LUCY_ADD(L, C, X, ON) lucy_add_if(L, C, X, ON)
-#endif
-#endif
-// One step.  G advances one cell: queue entry 2 (whose exit parameter is the parameter at which cell n was
-// entered, read first) receives the cell G leaves.  The physics handles cell n = queue entry 0.  A packet that
-// stops writes what the next phase needs into its slot and leaves the loop body.
-#define S_STEP(TN0, CI0, XZ0, TN2, CI2, XZ2)                                                                          \
-    {                                                                                                                  \
-        cp_async_wait<2>(); /* the word of cell n has landed */                                                        \
-        const unsigned long long cw = RING(rc);                                                                        \
-        const double t_in = TN2;                                                                                       \
-        CI2 = gcidx;                                                                                                   \
-        XZ2 = pack_xyz(gx, gy, gz);                                                                                    \
-        { /* branch-free: a G that has left the grid keeps stepping outwards and requests the marker word */         \
-            const bool gin = gcidx != kOutCell;                                                                        \
-            const bool selx = (tmx <= tmy) && (tmx <= tmz);                                                            \
-            const bool sely = !selx && (tmy <= tmz);                                                                   \
-            const bool selz = !selx && !sely;                                                                          \
-            TN2 = selx ? tmx : (sely ? tmy : tmz);                                                                     \
-            gx += selx ? stx : 0;                                                                                      \
-            gy += sely ? sty : 0;                                                                                      \
-            gz += selz ? stz : 0;                                                                                      \
-            /* parameter of the face through which the entered cell will be left (reading Q8): the face        */   \
-            /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'  */   \
-            /* f moves by its step, the others by 0, and all three t are recomputed: the same value for an      */   \
-            /* axis that did not move, so nothing has to be selected afterwards                                 */   \
-            fdx += __hiloint2double(selx ? shx : 0, 0);                                                                \
-            fdy += __hiloint2double(sely ? shy : 0, 0);                                                                \
-            fdz += __hiloint2double(selz ? shz : 0, 0);                                                                \
-            tmx = (fdx - px) * ivx;                                                                                    \
-            tmy = (fdy - py) * ivy;                                                                                    \
-            tmz = (fdz - pz) * ivz;                                                                                    \
-            const bool inside = gin & ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &              \
-                                ((unsigned)gz < (unsigned)P.nz);                                                       \
-            const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;                                  \
-            const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);                                               \
-            gcidx = inside ? cell : kOutCell;                                                                          \
-            void *dst = ring + ((rc + 3 * kRingStep) & kRingMask);                                                     \
-            /* cells of an empty brick are not read: their request goes to the marker word behind the grid */         \
-            cp_async8(dst, P.cellw + ((inside & !brick_empty(s_m0, brick)) ? cell : P.ncp));                           \
-        }                                                                                                              \
-        cp_async_commit();                                                                                             \
-        /* physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick and the   */   \
-        /* word requested for a cell outside the grid are both the marker word (bit 28; rho = 0, so dtau = 0) */   \
-        const double ds = TN0 - t_in;                                                                                  \
-        const double rho_c = cw_rho(cw);                                                                               \
-        if (cw_species(cw) != kq_sp) { /* opacities of this species at the packet's frequency: kept in registers */   \
-            kq_sp = cw_species(cw);                                                                                    \
-            kq = s_kk[kq_sp * nf + j];                                                                                 \
-        }                                                                                                              \
-        const double dtau = kq.x * rho_c * ds; /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */                 \
-        const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;                                                \
-        if (__builtin_expect(marker || dtau > tau, 0)) { /* interaction inside this cell: equality leaves (Q5) */     \
-            SU(U_NCROSS, slot) = ncross;                                                                               \
-            if (CI0 == kOutCell) { /* cell n lies outside: the packet has left the grid, escape tally in the E phase */ \
-                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);                                   \
-                state = ST_DONE;                                                                                       \
-            } else {                                                                                                   \
-                SF(F_T, slot) = t_in; SF(F_TAU, slot) = tau; SU(U_W0, slot) = XZ0;                                     \
-                if (marker) { /* cell n starts a run of empty bricks: J phase */                                       \
-                    state = ST_JUMP;                                                                                   \
-                } else {                                                                                               \
-                    SF(F_CW, slot) = __longlong_as_double((long long)cw);                                              \
-                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);                              \
-                    state = ST_INTERACT;                                                                               \
-                }                                                                                                      \
-            }                                                                                                          \
-            continue;                                                                                                  \
-        }                                                                                                              \
-        tau -= dtau;                                                                                                   \
-        { /* S5: no branch: a vacuum cell (rho = 0) adds 0 */                                                          \
-            const uint32_t dusty = cw_vacuum(cw) ? 0u : 1u;                                                            \
-            S_LUCY_ADD(P.lfx, CI0, kq.y * rho_c * ds, dusty);                                                          \
-            ndusty_acc += dusty;                                                                                       \
-        }                                                                                                              \
-        ncross++;                                                                                                      \
-    }
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
@@ -678,8 +580,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const int nfl = 32 - __popc(idle);
                     // nothing left to refill with and many lanes idle: let the other phases make flying packets
                     if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty())))) {
-                        // park mid-flight: cell n is entry A, entered at tnC.  A packet still behind its no-op cells has
-                        // not started: its slot is as the refill found it
+                        // park mid-flight: cell n, entered at tprev.  A packet still behind its no-op cell has not
+                        // started: its slot is as the refill found it
                         if (state == ST_FLY && prime == 0) {
                             cp_async_wait<0>();
                             SU(U_NCROSS, slot) = ncross;
@@ -687,7 +589,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                                 SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
                                 state = ST_DONE;
                             } else {
-                                SF(F_T, slot) = tnC; SF(F_TAU, slot) = tau;
+                                SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau;
                                 SF(F_CW, slot) = __longlong_as_double((long long)RING(r));
                                 SU(U_W0, slot) = xzA;
                             }
@@ -712,7 +614,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         tau = SF(F_TAU, slot);
                         const uint32_t w0 = SU(U_W0, slot);
                         j = (int)SU(U_W1, slot);
-                        ncross = SU(U_NCROSS, slot) - 2u;         // the two no-op cells below count themselves
+                        ncross = SU(U_NCROSS, slot) - 1u;         // the no-op cell below counts itself
                         gx = unpack_x(w0); gy = unpack_y(w0); gz = unpack_z(w0);
                         // the stored 1/u is +inf for a zero direction component: that axis never moves
                         stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
@@ -726,11 +628,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         fdy = sty ? (double)(gy + ((sty + 1) >> 1)) : CUDART_INF; shy = __double2hiint((double)sty);
                         fdz = stz ? (double)(gz + ((stz + 1) >> 1)) : CUDART_INF; shz = __double2hiint((double)stz);
                         gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
-                        // pipeline: two no-op cells (zero length, vacuum word), then the packet's cell
-                        RING(r) = 0ull; RING((r + kRingStep) & kRingMask) = 0ull;
-                        RING((r + 2 * kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        tnA = t; tnB = t; tnC = t; ciA = gcidx; ciB = gcidx; xzA = w0; xzB = w0;
-                        prime = 2;
+                        // pipeline: one no-op cell (zero length, vacuum word; its zero tally goes to the packet's own
+                        // cell), then the packet's cell
+                        RING(r) = 0ull;
+                        RING((r + kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        tprev = t; tnA = t; ciA = gcidx; xzA = w0;
+                        prime = 1;
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
@@ -744,19 +647,80 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 const int rc = r;               // ring slot of cell n in this step
                 r = (r + kRingStep) & kRingMask;
                 if (state == ST_FLY) {
-                    // one step per iteration: the loop (3 KB) fits the instruction cache next to the scheduler; the
-                    // queue is rotated by moves, (A, B, C) <- (B, C, A).  Three steps per iteration without the moves
-                    // measured 7 % slower (10 KB).
-                    S_STEP(tnA, ciA, xzA, tnC, ciC, xzC)
-                    const double tt = tnA; const uint32_t tc = ciA, tx = xzA;
-                    tnA = tnB; ciA = ciB; xzA = xzB;
-                    tnB = tnC; ciB = ciC; xzB = xzC;
-                    tnC = tt; ciC = tc; xzC = tx;
+                    // One step per iteration: the loop (2.5 KB) fits the instruction cache next to the scheduler
+                    // (three steps per iteration measured 7 % slower).
+                    cp_async_wait<1>();                               // the word of cell n has landed
+                    const unsigned long long cw = RING(rc);
+                    // ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and requests
+                    // its word.  Branch-free: a G that has left the grid keeps stepping outwards (a straight line
+                    // does not come back) and requests the marker word.
+                    const uint32_t ciN = gcidx, xzN = pack_xyz(gx, gy, gz);
+                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
+                    const bool sely = !selx && (tmy <= tmz);
+                    const bool selz = !selx && !sely;
+                    const double tnN = selx ? tmx : (sely ? tmy : tmz);
+                    gx += selx ? stx : 0;
+                    gy += sely ? sty : 0;
+                    gz += selz ? stz : 0;
+                    // parameter of the face through which the entered cell will be left (reading Q8): the face
+                    // coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'
+                    // f moves by its step, the others by 0, and all three t are recomputed: the same value for an
+                    // axis that did not move, so nothing has to be selected afterwards
+                    fdx += __hiloint2double(selx ? shx : 0, 0);
+                    fdy += __hiloint2double(sely ? shy : 0, 0);
+                    fdz += __hiloint2double(selz ? shz : 0, 0);
+                    tmx = (fdx - px) * ivx;
+                    tmy = (fdy - py) * ivy;
+                    tmz = (fdz - pz) * ivz;
+                    {
+                        const bool inside = ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &
+                                            ((unsigned)gz < (unsigned)P.nz);
+                        const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;
+                        const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);
+                        gcidx = inside ? cell : kOutCell;
+                        // cells of an empty brick are not read: their request goes to the marker word behind the grid
+                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask),
+                                  P.cellw + ((inside & !brick_empty(s_m0, brick)) ? cell : P.ncp));
+                    }
+                    cp_async_commit();
+                    // ---- physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick
+                    // and the word requested for a cell outside the grid are both the marker word (bit 28; rho = 0,
+                    // so dtau = 0)
+                    const double ds = tnA - tprev;
+                    const double rho_c = cw_rho(cw);
+                    if (cw_species(cw) != kq_sp) {   // opacities of this species at the packet's frequency: kept in registers
+                        kq_sp = cw_species(cw);
+                        kq = s_kk[kq_sp * nf + j];
+                    }
+                    const double dtau = kq.x * rho_c * ds;            // tau_i = (kabs+ksca) h rho ds (Eq. 2)
+                    const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;
+                    if (__builtin_expect(marker || dtau > tau, 0)) {  // interaction inside this cell: equality leaves (Q5)
+                        SU(U_NCROSS, slot) = ncross;
+                        if (ciA == kOutCell) {   // cell n lies outside: the packet has left the grid, escape tally in the E phase
+                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                            state = ST_DONE;
+                        } else {
+                            SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SU(U_W0, slot) = xzA;
+                            if (marker) {        // cell n starts a run of empty bricks: J phase
+                                state = ST_JUMP;
+                            } else {
+                                SF(F_CW, slot) = __longlong_as_double((long long)cw);
+                                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
+                                state = ST_INTERACT;
+                            }
+                        }
+                        continue;
+                    }
+                    tau -= dtau;
+                    // S5: no branch around the RED: a vacuum cell (rho = 0) adds 0
+                    lucy_add(P.lfx, ciA, kq.y * rho_c * ds);
+                    ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
+                    ncross++;
+                    tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
                     prime = max(prime - 1, 0);
                 }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
             }
-#undef S_STEP
             __syncwarp();
         } else if (njmp > 0 && njmp >= nevt) {
             // =========================================================== J phase: runs of empty bricks
