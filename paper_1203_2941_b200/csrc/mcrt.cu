@@ -568,11 +568,25 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
             int kq_sp = -1;
             int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
-            int nidle = 32, prime = 0;                          // prime: no-op cells still ahead of the packet's cell
+            int nidle = 32;
+            unsigned long long cw = 0ull;                       // word of cell n
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
                 {
+                    if (state == ST_JUMP || state == ST_INTERACT || state == ST_DONE) {
+                        // stopped in the walk below: write what the next phase needs into the slot
+                        SU(U_NCROSS, slot) = ncross;
+                        if (state == ST_DONE) {
+                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                        } else {
+                            SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SU(U_W0, slot) = xzA;
+                            if (state == ST_INTERACT) {
+                                SF(F_CW, slot) = __longlong_as_double((long long)cw);
+                                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
+                            }
+                        }
+                    }
                     mJ.add(state == ST_JUMP, slot);
                     mEv.add(state == ST_DONE || state == ST_INTERACT, slot);
                     if (state != ST_FLY) state = ST_IDLE;
@@ -582,7 +596,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty())))) {
                         // park mid-flight: cell n, entered at tprev.  A packet still behind its no-op cell has not
                         // started: its slot is as the refill found it
-                        if (state == ST_FLY && prime == 0) {
+                        // (its crossing count is still below the slot's)
+                        if (state == ST_FLY && (int)(ncross - SU(U_NCROSS, slot)) >= 0) {
                             cp_async_wait<0>();
                             SU(U_NCROSS, slot) = ncross;
                             if (ciA == kOutCell) {     // cell n lies outside the grid: the packet has escaped
@@ -633,7 +648,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         RING(r) = 0ull;
                         RING((r + kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                         tprev = t; tnA = t; ciA = gcidx; xzA = w0;
-                        prime = 1;
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
@@ -650,7 +664,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     // One step per iteration: the loop (2.5 KB) fits the instruction cache next to the scheduler
                     // (three steps per iteration measured 7 % slower).
                     cp_async_wait<1>();                               // the word of cell n has landed
-                    const unsigned long long cw = RING(rc);
+                    cw = RING(rc);
                     // ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and requests
                     // its word.  Branch-free: a G that has left the grid keeps stepping outwards (a straight line
                     // does not come back) and requests the marker word.
@@ -694,21 +708,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }
                     const double dtau = kq.x * rho_c * ds;            // tau_i = (kabs+ksca) h rho ds (Eq. 2)
                     const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;
-                    if (__builtin_expect(marker || dtau > tau, 0)) {  // interaction inside this cell: equality leaves (Q5)
-                        SU(U_NCROSS, slot) = ncross;
-                        if (ciA == kOutCell) {   // cell n lies outside: the packet has left the grid, escape tally in the E phase
-                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
-                            state = ST_DONE;
-                        } else {
-                            SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SU(U_W0, slot) = xzA;
-                            if (marker) {        // cell n starts a run of empty bricks: J phase
-                                state = ST_JUMP;
-                            } else {
-                                SF(F_CW, slot) = __longlong_as_double((long long)cw);
-                                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
-                                state = ST_INTERACT;
-                            }
-                        }
+                    if (marker || dtau > tau) {   // interaction inside this cell: equality leaves (Q5)
+                        // Some lane of the warp stops in nearly every iteration, so this is all that happens here:
+                        // the packet's registers stay as they are until the block above writes them to its slot.
+                        // Marker word: cell n lies outside the grid (escape tally in the E phase) or starts a run of
+                        // empty bricks (J phase)
+                        state = marker ? (ciA == kOutCell ? ST_DONE : ST_JUMP) : ST_INTERACT;
                         continue;
                     }
                     tau -= dtau;
@@ -717,7 +722,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
                     ncross++;
                     tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
-                    prime = max(prime - 1, 0);
                 }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
             }
