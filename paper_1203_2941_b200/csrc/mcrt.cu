@@ -341,25 +341,9 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
     atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
 }
 
-// Warp-aggregated tallies ("local copies reduce interference").  The lanes of the calling group
-// that address the same cell are found with __match_any_sync; their integer contributions are summed with
-// __reduce_add_sync in three 16-bit limbs (x < 2^46, so 32 lanes cannot overflow a limb sum) and the lowest
-// lane of each group issues one atomic.  Integer sums: the result is the same as with one atomic per lane.
-__device__ __forceinline__ void lucy_add_aggregated(long long *__restrict__ lfx, uint32_t cidx, double x)
-{
-    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
-    const unsigned grp = __match_any_sync(__activemask(), cidx);
-    const unsigned long long s0 = __reduce_add_sync(grp, (unsigned)(q & 0xffffull));
-    const unsigned long long s1 = __reduce_add_sync(grp, (unsigned)((q >> 16) & 0xffffull));
-    const unsigned long long s2 = __reduce_add_sync(grp, (unsigned)(q >> 32));
-    if ((threadIdx.x & 31u) == (unsigned)(__ffs(grp) - 1))
-        atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), s0 + (s1 << 16) + (s2 << 32));
-}
-__device__ __forceinline__ void count_add_aggregated(unsigned long long *__restrict__ kcnt, uint32_t cidx)
-{
-    const unsigned grp = __match_any_sync(__activemask(), cidx);
-    if ((threadIdx.x & 31u) == (unsigned)(__ffs(grp) - 1)) atomicAdd(&kcnt[cidx], (unsigned long long)__popc(grp));
-}
+// Warp aggregation of these adds (__match_any_sync + __reduce_add_sync per group) was measured slower everywhere:
+// 2.5-5x in the cell walk, and in the event phase the groups are almost always single lanes, whose reductions
+// then run one after the other (7 % of the kernel's stall samples).  Plain RED atomics: L2 does the sums.
 
 // ------------------------------------------------------------------------------------------------
 // S0-S10  the transport kernel: persistent CTAs; every warp owns a POOL of kSlots packets in shared memory.
@@ -505,7 +489,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     double *s_src = reinterpret_cast<double *>(s_ag + nsf);
     double *s_mu = s_src + P.nf;
     unsigned long long *s_cnt = reinterpret_cast<unsigned long long *>(s_mu + P.ndir + 1);
-    unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8);
+    unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8 * nwarps);
     const int nhist = 2 * P.ndir * P.nf;
     uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
     // cell-word ring: slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
@@ -523,7 +507,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
     for (int i = threadIdx.x; i < P.mwords; i += blockDim.x) s_m0[i] = P.vmask[i];
-    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0ull;
+    for (int i = threadIdx.x; i < 8 * nwarps; i += blockDim.x) s_cnt[i] = 0ull;   // eight counters per warp
     __syncthreads();
 
     const int lane = (int)(threadIdx.x & 31u);
@@ -809,19 +793,34 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0); j = (int)SU(U_W1, slot);
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
             }
+            {   // run counters of the packets that escape in this phase: summed over the warp, then added to the warp's
+                // own counters in shared memory by one lane (no atomics)
+                const bool esc = kind == K_ESCAPED;
+                const unsigned em = __ballot_sync(kFull, esc);
+                if (em) {
+                    const uint32_t c_lo = __reduce_add_sync(kFull, esc ? (ncross & 0xffffu) : 0u);
+                    const uint32_t c_hi = __reduce_add_sync(kFull, esc ? (ncross >> 16) : 0u);
+                    const uint32_t n_sc = __reduce_add_sync(kFull, esc ? nsca : 0u);
+                    const uint32_t n_ab = __reduce_add_sync(kFull, esc ? nabs : 0u);
+                    const unsigned dm = __ballot_sync(kFull, esc && (nsca + nabs) == 0u);
+                    if (lane == 0) {
+                        volatile unsigned long long *wc = s_cnt + 8 * (threadIdx.x >> 5);
+                        wc[CNT_PACKETS] += (unsigned long long)__popc(em);
+                        wc[CNT_CROSS] += (unsigned long long)c_lo + ((unsigned long long)c_hi << 16);
+                        wc[CNT_SCA] += (unsigned long long)n_sc;
+                        wc[CNT_ABS] += (unsigned long long)n_ab;
+                        wc[CNT_DIRECT] += (unsigned long long)__popc(dm);
+                    }
+                }
+            }
             if (kind == K_ESCAPED) {
-                // S10 escape tally: frequency x |cos i| bin, block-private histogram + counters
+                // S10 escape tally: frequency x |cos i| bin, block-private histogram
                 const double amu = fabs(uz);
                 int bin = 0;
                 for (int b = 1; b < P.ndir; ++b) if (s_mu[b] <= amu) bin = b;
                 atomicAdd(&s_hist[bin * nf + j], 1u);
                 const bool direct = (nsca + nabs) == 0u;
                 if (direct) atomicAdd(&s_hist[P.ndir * nf + bin * nf + j], 1u);
-                atomicAdd(&s_cnt[CNT_PACKETS], 1ull);
-                atomicAdd(&s_cnt[CNT_CROSS], (unsigned long long)ncross);
-                atomicAdd(&s_cnt[CNT_SCA], (unsigned long long)nsca);
-                atomicAdd(&s_cnt[CNT_ABS], (unsigned long long)nabs);
-                if (direct) atomicAdd(&s_cnt[CNT_DIRECT], 1ull);
                 if (RECORD) {
                     hash_mix(hash, event_word(EV_ESCAPE, j, (unsigned long long)bin));
                     hash_mix(hash, (unsigned long long)ncross);
@@ -875,7 +874,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double2 kq = s_kk[sj];
                     const double kk = kq.x * rho_c;
                     const double sint = tau / kk;
-                    lucy_add_aggregated(P.lfx, cidx, kq.y * rho_c * sint);
+                    lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
                     const double tint = t + sint;
                     double q;
                     q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
@@ -890,7 +889,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                        count_add_aggregated(P.kcnt, cidx);
+                        atomicAdd(&P.kcnt[cidx], 1ull);
                         nabs++;
                         const int s = cw_species(cw);
                         const int m = cw_tidx(cw);
@@ -974,7 +973,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 #undef SF
 #undef RING
 #undef SU
-    if (ndusty_acc) atomicAdd(&s_cnt[CNT_DUSTY], (unsigned long long)ndusty_acc);
+    {   // dusty crossings stepped by this warp
+        const uint32_t nd = __reduce_add_sync(kFull, ndusty_acc & 0xffffu), ndh = __reduce_add_sync(kFull, ndusty_acc >> 16);
+        if (lane == 0) s_cnt[8 * (threadIdx.x >> 5) + CNT_DUSTY] += (unsigned long long)nd + ((unsigned long long)ndh << 16);
+    }
 
     // flush the block-private histogram and counters
     __syncthreads();
@@ -984,7 +986,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         if (v) atomicAdd(i < half ? &P.sed[i] : &P.sed_direct[i - half], (unsigned long long)v);
     }
     if (threadIdx.x < CNT_NEXT && threadIdx.x != CNT_OVERFLOW) {
-        const unsigned long long v = s_cnt[threadIdx.x];
+        unsigned long long v = 0ull;
+        for (int w = 0; w < nwarps; ++w) v += s_cnt[8 * w + threadIdx.x];
         if (v) atomicAdd(&P.counters[threadIdx.x], v);
     }
 }
@@ -1317,7 +1320,7 @@ int fx_bits_for(uint64_t n)
 size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record)
 {
     return (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
-           8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
+           (size_t)(threads / 32) * 8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
            (size_t)((mask0_words + 1) & ~1) * sizeof(uint32_t) + (size_t)kRing * threads * sizeof(unsigned long long);
 }
 
