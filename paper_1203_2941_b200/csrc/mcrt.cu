@@ -676,9 +676,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;
                         const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);
                         gcidx = inside ? cell : kOutCell;
-                        // cells of an empty brick are not read: their request goes to the marker word behind the grid
-                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask),
-                                  P.cellw + ((inside & !brick_empty(s_m0, brick)) ? cell : P.ncp));
+                        // a cell outside the grid requests the marker word behind the grid
+                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), P.cellw + (inside ? cell : P.ncp));
                     }
                     cp_async_commit();
                     // ---- physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick
@@ -1117,7 +1116,7 @@ __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__rest
 
 // Vacuum mask of one level: bit of box (bx, by, bz) is set when all its in-grid cells have rho == 0.
 // Level 0 is built from the packed cells, level l > 0 from level l - 1 (4x4x4 children per box).
-__global__ void k_build_mask0(const unsigned long long *__restrict__ cellw, uint32_t *__restrict__ m, int nx, int ny, int nz,
+__global__ void k_build_mask0(unsigned long long *__restrict__ cellw, uint32_t *__restrict__ m, int nx, int ny, int nz,
                               int nbx, int nby, int sh, int mbx, int mby, int mbz)
 {
     const int nb = mbx * mby * mbz;
@@ -1130,7 +1129,14 @@ __global__ void k_build_mask0(const unsigned long long *__restrict__ cellw, uint
             for (int y = y0; y < y1 && empty; ++y)
                 for (int x = x0; x < x1; ++x)
                     if (!cw_vacuum(cellw[brick_index(x, y, z, nbx, nby, sh)])) { empty = false; break; }
-        if (empty) atomicOr(&m[b >> 5], 1u << (b & 31));
+        if (empty) {
+            atomicOr(&m[b >> 5], 1u << (b & 31));
+            // every cell word of an empty brick carries the marker bit: the cell walk sees it in the word it reads
+            // anyway and needs no mask lookup
+            for (int z = z0; z < z1; ++z)
+                for (int y = y0; y < y1; ++y)
+                    for (int x = x0; x < x1; ++x) cellw[brick_index(x, y, z, nbx, nby, sh)] |= kJumpWord;
+        }
     }
 }
 
