@@ -337,7 +337,9 @@ __device__ __forceinline__ bool brick_empty(const uint32_t *m0, uint32_t brick) 
 // x < 37 * 2^40 always, because a packet never spends more than its tau = -ln zeta <= 36.8 in one cell.
 __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
 {
-    const unsigned long long q = (unsigned long long)__double_as_longlong(x + 6755399441055744.0) - 0x4338000000000000ull;
+    // round to nearest even by adding 1.5 * 2^52: the integer sits in the mantissa, the bias in the high word only
+    const double y = x + 6755399441055744.0;
+    const unsigned long long q = ((unsigned long long)(uint32_t)(__double2hiint(y) - 0x43380000) << 32) | (uint32_t)__double2loint(y);
     atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
 }
 
@@ -394,6 +396,8 @@ __device__ __forceinline__ int unpack_y(uint32_t w) { return (int)((w >> 11) & 0
 __device__ __forceinline__ int unpack_z(uint32_t w) { return (int)(w >> 22); }
 // ring word that stands for "this cell lies in an empty brick": no real cell word has bit 28 set with rho = 0
 constexpr unsigned long long kJumpWord = 0x10000000ull;
+// words behind the Lucy tally that take the (zero) adds of lanes that do not step a packet: one per thread of the grid
+constexpr size_t kLucyScratch = 131072;
 
 // position of the n-th set bit (n = 0, 1, ...) of a 64-bit mask; n < popc(m)
 __device__ __forceinline__ int nth_set64(unsigned long long m, int n)
@@ -511,7 +515,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     __syncthreads();
 
     const int lane = (int)(threadIdx.x & 31u);
-    const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby;
+    const int nf = P.nf, bsh = P.bsh;
+    // kept in registers (opaque to the compiler, which would otherwise reload them from the constant bank inside
+    // the walk loop and wait for them there)
+    int nbx, nby;
+    uint32_t ncp_r;
+    asm volatile("mov.u32 %0, %1;" : "=r"(nbx) : "r"(P.nbx));
+    asm volatile("mov.u32 %0, %1;" : "=r"(nby) : "r"(P.nby));
+    asm volatile("mov.u32 %0, %1;" : "=r"(ncp_r) : "r"(P.ncp));
     double *wf = s_pool + (size_t)(threadIdx.x >> 5) * kPoolF64;                  // this warp's pool, f64 fields
     uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kNF64 * kSlots);             // its u32 fields
 #define SF(f, s) wf[(f) * kSlots + (s)]
@@ -554,6 +565,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
             int nidle = 32;
             unsigned long long cw = 0ull;                       // word of cell n
+            const uint32_t scratch = ncp_r + 1u + ((blockIdx.x * blockDim.x + threadIdx.x) & (uint32_t)(kLucyScratch - 2));
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
@@ -644,14 +656,22 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 do {
                 const int rc = r;               // ring slot of cell n in this step
                 r = (r + kRingStep) & kRingMask;
-                if (state == ST_FLY) {
-                    // One step per iteration: the loop (2.5 KB) fits the instruction cache next to the scheduler
-                    // (three steps per iteration measured 7 % slower).
+                {
+                    // One step per iteration: the loop (2 KB) fits the instruction cache next to the scheduler
+                    // (three steps per iteration measured 7 % slower).  No branch: a divergent branch costs more
+                    // here (branch resolution, reconvergence) than the work it skips, so every lane runs the whole
+                    // step and a lane that holds no flying packet leaves no trace: its G walks on stale
+                    // coordinates, it requests the marker word, adds 0 to its scratch word and keeps its packet's
+                    // registers (they are written to the slot by the block above).
+                    const bool fly = state == ST_FLY;
                     cp_async_wait<1>();                               // the word of cell n has landed
-                    cw = RING(rc);
+                    {
+                        const unsigned long long w = RING(rc);
+                        cw = fly ? w : cw;
+                    }
                     // ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and requests
-                    // its word.  Branch-free: a G that has left the grid keeps stepping outwards (a straight line
-                    // does not come back) and requests the marker word.
+                    // its word.  A G that has left the grid keeps stepping outwards (a straight line does not come
+                    // back) and requests the marker word.
                     const uint32_t ciN = gcidx, xzN = pack_xyz(gx, gy, gz);
                     const bool selx = (tmx <= tmy) && (tmx <= tmz);
                     const bool sely = !selx && (tmy <= tmz);
@@ -671,13 +691,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     tmy = (fdy - py) * ivy;
                     tmz = (fdz - pz) * ivz;
                     {
-                        const bool inside = ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &
+                        const bool inside = fly & ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &
                                             ((unsigned)gz < (unsigned)P.nz);
-                        const uint32_t brick = inside ? brick_of(gx, gy, gz, nbx, nby, bsh) : 0u;
-                        const uint32_t cell = cell_in_brick(brick, gx, gy, gz, bsh);
+                        // (an index computed from coordinates outside the grid is not used)
+                        const uint32_t cell = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
                         gcidx = inside ? cell : kOutCell;
                         // a cell outside the grid requests the marker word behind the grid
-                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), P.cellw + (inside ? cell : P.ncp));
+                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), P.cellw + (inside ? cell : ncp_r));
                     }
                     cp_async_commit();
                     // ---- physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick
@@ -691,20 +711,20 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }
                     const double dtau = kq.x * rho_c * ds;            // tau_i = (kabs+ksca) h rho ds (Eq. 2)
                     const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;
-                    if (marker || dtau > tau) {   // interaction inside this cell: equality leaves (Q5)
-                        // Some lane of the warp stops in nearly every iteration, so this is all that happens here:
-                        // the packet's registers stay as they are until the block above writes them to its slot.
-                        // Marker word: cell n lies outside the grid (escape tally in the E phase) or starts a run of
-                        // empty bricks (J phase)
-                        state = marker ? (ciA == kOutCell ? ST_DONE : ST_JUMP) : ST_INTERACT;
-                        continue;
+                    const bool stop = marker || dtau > tau;           // interaction inside this cell: equality leaves (Q5)
+                    const bool go = fly && !stop;
+                    // Marker word: cell n lies outside the grid (escape tally in the E phase) or starts a run of empty
+                    // bricks (J phase)
+                    if (fly && stop) state = marker ? (ciA == kOutCell ? ST_DONE : ST_JUMP) : ST_INTERACT;
+                    // S5: no branch around the RED: a vacuum cell (rho = 0) adds 0 to its tally, a lane that does not
+                    // step adds 0 to its scratch word
+                    lucy_add(P.lfx, go ? ciA : scratch, go ? kq.y * rho_c * ds : 0.0);
+                    if (go) {
+                        tau -= dtau;
+                        ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
+                        ncross++;
+                        tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
                     }
-                    tau -= dtau;
-                    // S5: no branch around the RED: a vacuum cell (rho = 0) adds 0
-                    lucy_add(P.lfx, ciA, kq.y * rho_c * ds);
-                    ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
-                    ncross++;
-                    tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
                 }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
             }
@@ -1394,7 +1414,7 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     add((size_t)mg.mwords * 4);          // vacuum mask
     add(nbricks * sizeof(uint4));        // empty boxes of the J phase
     add((size_t)(mg.nbx + 1) * (mg.nby + 1) * (mg.nbz + 1) * sizeof(int));   // summed-area scratch
-    add(ncp * sizeof(long long));        // Lucy tally
+    add((ncp + kLucyScratch) * sizeof(long long));   // Lucy tally + scratch words (adds of lanes that do not step)
     add(ncp * sizeof(long long));        // k
     add(ncp * sizeof(long long));        // k_prev
     add(nc * 8);                         // scratch (staging of inputs / outputs)
@@ -1457,7 +1477,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
     GC_TRY(ws_alloc(c, (void **)&c->vbox, (size_t)c->nbx * c->nby * c->nbz * sizeof(uint4)));
     GC_TRY(ws_alloc(c, (void **)&c->vsat, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int)));
-    GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
+    GC_TRY(ws_alloc(c, (void **)&c->lfx, (c->ncp + kLucyScratch) * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->scratch, c->nc * 8));
