@@ -382,7 +382,7 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #define MCRT_S_LEAVE 8              // ... and ends when this many lanes are idle and nothing is left to refill them
 #endif
 #ifndef MCRT_J_MIN
-#define MCRT_J_MIN 6                // a J phase ends when fewer lanes than this still jump
+#define MCRT_J_MIN 10               // a J phase ends when fewer lanes than this still jump
 #endif
 
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_HASH };
