@@ -639,11 +639,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         fdy = sty ? (double)(gy + ((sty + 1) >> 1)) : CUDART_INF; shy = __double2hiint((double)sty);
                         fdz = stz ? (double)(gz + ((stz + 1) >> 1)) : CUDART_INF; shz = __double2hiint((double)stz);
                         gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
-                        // pipeline: one no-op cell (zero length, vacuum word; its zero tally goes to the packet's own
-                        // cell), then the packet's cell
+                        // pipeline: one no-op cell (zero length, vacuum word; its zero tally goes to the lane's scratch
+                        // word, not to the packet's cell: the cells where packets start are the most contended ones),
+                        // then the packet's cell
                         RING(r) = 0ull;
                         RING((r + kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        tprev = t; tnA = t; ciA = gcidx; xzA = w0;
+                        tprev = t; tnA = t; ciA = scratch; xzA = w0;
                         kq_sp = 0; kq = s_kk[j];
                         state = ST_FLY;
                     }
