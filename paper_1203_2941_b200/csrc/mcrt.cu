@@ -340,7 +340,8 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
     // round to nearest even by adding 1.5 * 2^52: the integer sits in the mantissa, the bias in the high word only
     const double y = x + 6755399441055744.0;
     const unsigned long long q = ((unsigned long long)(uint32_t)(__double2hiint(y) - 0x43380000) << 32) | (uint32_t)__double2loint(y);
-    atomicAdd(reinterpret_cast<unsigned long long *>(lfx + cidx), q);
+    // (explicitly global: a pointer that went through shared memory has lost its address space)
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + cidx), "l"(q) : "memory");
 }
 
 // Warp aggregation of these adds (__match_any_sync + __reduce_add_sync per group) was measured slower everywhere:
@@ -374,6 +375,9 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #endif
 #ifndef MCRT_SWAP_MIN
 #define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
+#endif
+#ifndef MCRT_PIN
+#define MCRT_PIN 3                  // how many of the walk loop's kernel parameters are pinned in registers (1..3)
 #endif
 #ifndef MCRT_S_ENTER
 #define MCRT_S_ENTER 32             // an S phase starts when the pool holds this many flying packets
@@ -512,17 +516,21 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
     for (int i = threadIdx.x; i < P.mwords; i += blockDim.x) s_m0[i] = P.vmask[i];
     for (int i = threadIdx.x; i < 8 * nwarps; i += blockDim.x) s_cnt[i] = 0ull;   // eight counters per warp
+    // Kernel parameters the walk loop uses, parked in shared memory: the S phase reads them into registers through
+    // a volatile pointer, so that they stay there (left to itself the compiler reloads a dozen of them from the
+    // constant bank in every iteration of the loop and waits for them)
+    __shared__ unsigned long long s_parp[2];
+    __shared__ uint32_t s_pari[8];
+    if (threadIdx.x == 0) {
+        s_parp[0] = reinterpret_cast<unsigned long long>(P.cellw);
+        s_parp[1] = reinterpret_cast<unsigned long long>(P.lfx);
+        s_pari[0] = P.ncp; s_pari[1] = (uint32_t)P.nbx; s_pari[2] = (uint32_t)P.nby; s_pari[3] = (uint32_t)P.nx;
+        s_pari[4] = (uint32_t)P.ny; s_pari[5] = (uint32_t)P.nz; s_pari[6] = (uint32_t)P.bsh; s_pari[7] = (uint32_t)P.nf;
+    }
     __syncthreads();
 
     const int lane = (int)(threadIdx.x & 31u);
-    const int nf = P.nf, bsh = P.bsh;
-    // kept in registers (opaque to the compiler, which would otherwise reload them from the constant bank inside
-    // the walk loop and wait for them there)
-    int nbx, nby;
-    uint32_t ncp_r;
-    asm volatile("mov.u32 %0, %1;" : "=r"(nbx) : "r"(P.nbx));
-    asm volatile("mov.u32 %0, %1;" : "=r"(nby) : "r"(P.nby));
-    asm volatile("mov.u32 %0, %1;" : "=r"(ncp_r) : "r"(P.ncp));
+    const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby;
     double *wf = s_pool + (size_t)(threadIdx.x >> 5) * kPoolF64;                  // this warp's pool, f64 fields
     uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kNF64 * kSlots);             // its u32 fields
 #define SF(f, s) wf[(f) * kSlots + (s)]
@@ -565,6 +573,23 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
             int nidle = 32;
             unsigned long long cw = 0ull;                       // word of cell n
+            const volatile unsigned long long *vpp = s_parp;
+            const volatile uint32_t *vpi = s_pari;
+            const unsigned long long *const cellw_r = reinterpret_cast<const unsigned long long *>(vpp[0]);
+            long long *const lfx_r = reinterpret_cast<long long *>(vpp[1]);
+            const uint32_t ncp_r = vpi[0];
+#if MCRT_PIN >= 2
+            const int nbx_r = (int)vpi[1], nby_r = (int)vpi[2];
+#else
+            const int nbx_r = nbx, nby_r = nby;
+#endif
+#if MCRT_PIN >= 3
+            const uint32_t nx_r = vpi[3], ny_r = vpi[4], nz_r = vpi[5];
+            const int bsh_r = (int)vpi[6];
+#else
+            const uint32_t nx_r = (uint32_t)P.nx, ny_r = (uint32_t)P.ny, nz_r = (uint32_t)P.nz;
+            const int bsh_r = bsh;
+#endif
             const uint32_t scratch = ncp_r + 1u + ((blockIdx.x * blockDim.x + threadIdx.x) & (uint32_t)(kLucyScratch - 2));
 
             for (;;) {
@@ -692,13 +717,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     tmy = (fdy - py) * ivy;
                     tmz = (fdz - pz) * ivz;
                     {
-                        const bool inside = fly & ((unsigned)gx < (unsigned)P.nx) & ((unsigned)gy < (unsigned)P.ny) &
-                                            ((unsigned)gz < (unsigned)P.nz);
+                        const bool inside = fly & ((unsigned)gx < nx_r) & ((unsigned)gy < ny_r) & ((unsigned)gz < nz_r);
                         // (an index computed from coordinates outside the grid is not used)
-                        const uint32_t cell = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
+                        const uint32_t cell = cell_in_brick(brick_of(gx, gy, gz, nbx_r, nby_r, bsh_r), gx, gy, gz, bsh_r);
                         gcidx = inside ? cell : kOutCell;
                         // a cell outside the grid requests the marker word behind the grid
-                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), P.cellw + (inside ? cell : ncp_r));
+                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), cellw_r + (inside ? cell : ncp_r));
                     }
                     cp_async_commit();
                     // ---- physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick
@@ -719,7 +743,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     if (fly && stop) state = marker ? (ciA == kOutCell ? ST_DONE : ST_JUMP) : ST_INTERACT;
                     // S5: no branch around the RED: a vacuum cell (rho = 0) adds 0 to its tally, a lane that does not
                     // step adds 0 to its scratch word
-                    lucy_add(P.lfx, go ? ciA : scratch, go ? kq.y * rho_c * ds : 0.0);
+                    lucy_add(lfx_r, go ? ciA : scratch, go ? kq.y * rho_c * ds : 0.0);
                     if (go) {
                         tau -= dtau;
                         ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
