@@ -590,7 +590,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const uint32_t nx_r = (uint32_t)P.nx, ny_r = (uint32_t)P.ny, nz_r = (uint32_t)P.nz;
             const int bsh_r = bsh;
 #endif
-            const uint32_t scratch = ncp_r + 1u + ((blockIdx.x * blockDim.x + threadIdx.x) & (uint32_t)(kLucyScratch - 2));
+            const uint32_t scratch = ncp_r + ((blockIdx.x * blockDim.x + threadIdx.x) & (uint32_t)(kLucyScratch - 1));   // this thread's word
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
