@@ -351,13 +351,15 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
 // ------------------------------------------------------------------------------------------------
 // S0-S10  the transport kernel: persistent CTAs; every warp owns a POOL of kSlots packets in shared memory.
 //
-// A packet is either FLYING (walking cell by cell towards its next interaction) or waiting for an EVENT
-// (emission of the slot's next packet, an interaction, the escape tally).  The two kinds of work share no
-// code, so a warp never mixes them: it alternates between
-//   S phase: the 32 lanes check 32 flying packets out of the pool into registers and step them cell by cell
-//            (S4/S5) until kSwap of them have reached an event; then all are parked again;
+// A packet is either FLYING (walking cell by cell towards its next interaction), JUMPING (inside a run of empty
+// bricks) or waiting for an EVENT (emission of the slot's next packet, an interaction, the escape tally).  The
+// three kinds of work share no code, so a warp never mixes them: it alternates between
+//   S phase: the 32 lanes check flying packets out of the pool into registers and step them cell by cell (S4/S5);
+//            lanes whose packet stopped are refilled from the pool MCRT_SWAP_MIN at a time, and the rest is parked
+//            again when the pool has nothing left for MCRT_S_LEAVE idle lanes;
+//   J phase: up to 32 jumping packets cross their runs of empty bricks box by box (mcrt::box_jump, dda.h);
 //   E phase: entered when fewer than 32 packets can fly; the lanes take up to 32 waiting packets and each
-//            performs that packet's event (S1-S3, S6-S10, S0 refill with one warp-aggregated atomic).
+//            performs that packet's event (S1-S3, S6-S10; S0 refill: one atomic per warp for the new packet ids).
 // With 64 packets per warp both phases run with (nearly) all lanes active whatever the mix of optical
 // depths -- the scheduling-independent replacement of the paper's pause/resume balancer.
 // Results never depend on which lane or warp carries a packet: all random numbers are Philox blocks keyed
