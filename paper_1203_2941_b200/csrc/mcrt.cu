@@ -748,7 +748,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     lucy_add(lfx_r, go ? ciA : scratch, go ? kq.y * rho_c * ds : 0.0);
                     if (go) {
                         tau -= dtau;
-                        ndusty_acc += cw_vacuum(cw) ? 0u : 1u;
+                        ndusty_acc += (__double2hiint(rho_c) != 0) ? 1u : 0u;   // rho > 0: its high word is not 0
                         ncross++;
                         tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
                     }
