@@ -369,7 +369,10 @@ __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t c
 #define MCRT_SLOTS 64
 #endif
 constexpr int kSlots = MCRT_SLOTS;  // packets per warp (<= 128: the slot sets are one or two 64-bit masks)
-constexpr int kSlotF64 = 11;        // 8-byte fields per slot (+1, the digest hash, in the recording kernel)
+#ifndef MCRT_SLOT_IV
+#define MCRT_SLOT_IV 0              // 1: the slot also holds 1/u per axis (computed once per direction, not per refill)
+#endif
+constexpr int kSlotF64 = 11 + 3 * MCRT_SLOT_IV;   // 8-byte fields per slot (+1, the digest hash, in the recording kernel)
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlots * ((kSlotF64 + (record ? 1 : 0)) * 8 + kSlotU32 * 4); }
 #ifndef MCRT_MAX_THREADS
@@ -391,7 +394,11 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #define MCRT_J_MIN 10               // a J phase ends when fewer lanes than this still jump
 #endif
 
+#if MCRT_SLOT_IV
+enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_IVX, F_IVY, F_IVZ, F_HASH };
+#else
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_HASH };
+#endif
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
 constexpr uint32_t kOutCell = 0xffffffffu;   // storage index of "outside the grid"
@@ -643,10 +650,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         cp_async_wait<0>();                       // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
+#if MCRT_SLOT_IV
+                            ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+#else
                             const double ux = SF(F_UX, slot), uy = SF(F_UY, slot), uz = SF(F_UZ, slot);
                             ivx = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
                             ivy = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
                             ivz = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+#endif
                         }
                         const double t = SF(F_T, slot);
                         tau = SF(F_TAU, slot);
@@ -773,9 +784,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             if (act) {
                 px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+#if MCRT_SLOT_IV
+                ivx = SF(F_IVX, slot); ivy = SF(F_IVY, slot); ivz = SF(F_IVZ, slot);
+#else
                 ivx = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
                 ivy = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
                 ivz = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+#endif
                 t = SF(F_T, slot);
                 const uint32_t w0 = SU(U_W0, slot);
                 ncross = SU(U_NCROSS, slot);
@@ -997,6 +1012,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // park the new flight (reading Q8: the walk needs p, 1/u, the cell; t = 0)
                 SF(F_PX, slot) = px; SF(F_PY, slot) = py; SF(F_PZ, slot) = pz;
                 SF(F_UX, slot) = ux; SF(F_UY, slot) = uy; SF(F_UZ, slot) = uz;
+#if MCRT_SLOT_IV
+                SF(F_IVX, slot) = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
+                SF(F_IVY, slot) = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
+                SF(F_IVZ, slot) = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+#endif
                 SF(F_T, slot) = 0.0;
                 SF(F_TAU, slot) = -traj_log(z0);
                 SF(F_ZTYPE, slot) = z1;
