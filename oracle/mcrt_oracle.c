@@ -16,8 +16,11 @@
  * Parity pins (tests/test_oracle_pins.py): Philox known-answer vectors, DDA vs brute-force slab
  * intersections, exp(-tau) transmission, Henyey-Greenstein moments, isotropy, exact packet/energy
  * conservation, constant-albedo ratio, optically thin temperature, Planck/zeta closed forms,
- * 2x2x2 brute-force quadrature, per-cell redraw equivalence (paper fn. 1), epoch vs serial B&W,
- * the explicit ln / sin / cos against libm and against multi-precision values.
+ * 2x2x2 brute-force quadrature, per-cell redraw equivalence (paper fn. 1), epoch vs serial B&W (also at the
+ * plateau-epoch shape of the default schedule, P12b), the explicit ln / sin / cos against libm and against
+ * multi-precision values, the frozen-T sweep against the closed-form T(r) and the Eq. 5 mean photon energy
+ * (P16), the SED flux conversion and E = k xi against L and the blackbody shape (P17), the position after
+ * interactions against the random-flight second moment 2 l^2 / [(1-a)(1-a g)] (P18).
  * Parity UNPINNED: agreement with DUSTY / Kruegel / Pascucci benchmark SEDs,
  * whose data are not available here.
  *
@@ -466,6 +469,8 @@ typedef struct {
     int32_t keep_fp64_lucy;  /* pin P14: also keep a compensated fp64 Lucy sum (serial only) */
     int32_t reset;           /* zero tallies first */
     uint32_t pass0;          /* RNG pass word of the B&W run */
+    uint64_t pid0;           /* id of the first packet of this run (continuing a run with further packets) */
+    uint64_t n_total;        /* the luminosity is split into this many packets, xi = L / n_total; 0 = n_packets */
 } orc_opts;
 
 typedef struct {
@@ -690,7 +695,7 @@ typedef struct {
     uint16_t *tidx;
     uint64_t *sed, *sed_direct;
     int fx;
-    double xi;               /* packet energy L/N of the last run */
+    double xi;               /* packet energy L/N of the run that produced the stored tallies */
 } orc_state;
 
 orc_state *orc_state_create(const orc_ctx *C)
@@ -789,7 +794,8 @@ static void sweep_update(orc_state *S, int from_lucy, double cellfac, int fx_of_
     }
 }
 
-/* O-run: the whole path for N packets.  Returns 0, or -5 on fixed-point overflow (|L| > 2^62). */
+/* O-run: the whole path for N packets.  Returns 0, -5 on fixed-point overflow (|L| > 2^62), -2 when a run
+ * without reset would mix tallies of different packet energies. */
 int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, orc_stats *stats,
             orc_digest *digests)
 {
@@ -804,15 +810,22 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
     }
     /* sweeps (S12) take their temperatures from the previous pass's tallies, so only a B&W run resets first */
     if (o->reset && o->mode == ORC_MODE_BW_EPOCH) zero_tallies(S);
+    const uint64_t n_xi = o->n_total ? o->n_total : n_packets;
+    /* the stored tallies are in units of the packet energy and fixed-point scale of the run that made them */
     const int prev_fx = S->fx;
-    S->fx = orc_fx_bits(n_packets);
-    S->xi = C->L / (double)n_packets;                    /* xi = L/N */
+    const double prev_xi = S->xi;
+    S->fx = orc_fx_bits(n_xi);
+    S->xi = C->L / (double)n_xi;                         /* xi = L/N */
+    if (!o->reset && o->mode == ORC_MODE_BW_EPOCH && prev_xi != 0.0 && (prev_xi != S->xi || prev_fx != S->fx))
+        return -2;                                       /* tallies of another packet energy cannot be continued */
     double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h); /* xi / (4 pi V), Eq. 4 */
+    /* Eq. 4 for the first sweep: k and L were counted in packets of the PREVIOUS run's energy */
+    double prev_cellfac = prev_xi / (ORC_FOUR_PI * C->h * C->h * C->h);
     size_t nsf = (size_t)C->ns * C->nf;
     R.C = C; R.k = S->k; R.kprev = S->kprev; R.Lfx = S->Lfx; R.tidx = S->tidx;
     R.Lsum = o->keep_fp64_lucy ? S->Lsum : NULL; R.Lcmp = S->Lcmp;
     R.sed = S->sed; R.sed_direct = S->sed_direct; R.dig = digests; R.seed = seed; R.fx = S->fx; R.o = o;
-    R.pid0_digest = 0;
+    R.pid0_digest = o->pid0;
     R.kabs_fx = (double *)malloc(nsf * sizeof(double));
     for (size_t i = 0; i < nsf; ++i) R.kabs_fx[i] = ldexp(C->kabs_h[i], S->fx);
     st.fx_bits = S->fx;
@@ -830,7 +843,7 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
         while (done < n_packets) {
             uint64_t Be = n_packets - done < Bnom ? n_packets - done : Bnom;
             epoch_update(S, e == 0, e == 0 ? 1.0 : (double)Be / (double)Bprev, cellfac);
-            run_range(&R, done, Be, &st);
+            run_range(&R, o->pid0 + done, Be, &st);
             done += Be;
             Bprev = Be;
             Bnom = (Bnom * 2 > Bmax) ? Bmax : Bnom * 2;
@@ -846,10 +859,10 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
             memset(&st, 0, sizeof st);
             st.epochs = ep;
             st.fx_bits = S->fx;
-            sweep_update(S, o->sweep_T_from_lucy, cellfac, sw == 1 ? prev_fx : S->fx);
+            sweep_update(S, o->sweep_T_from_lucy, sw == 1 ? prev_cellfac : cellfac, sw == 1 ? prev_fx : S->fx);
             zero_tallies(S);
             R.pass = o->pass0 + (uint32_t)sw;
-            run_range(&R, 0, n_packets, &st);
+            run_range(&R, o->pid0, n_packets, &st);
             st.epochs++;
         }
     }

@@ -496,3 +496,185 @@ def test_p15_explicit_log_sincos_against_libm_and_multiprecision(orc):
     zmax = 1.0 - 2.0 ** -53
     assert orc.det_log(zmax) == pytest.approx(-2.0 ** -53, rel=1e-15)
     assert orc.det_sincos(zmax)[0] == pytest.approx(-2 * math.pi * 2.0 ** -53, rel=1e-15)
+
+
+# ------------------------------------------------------------------------------------------ P12b plateau epochs
+def test_p12b_plateau_epochs_of_the_default_schedule(orc):
+    """Reading Q19 at the shipped default.  The default schedule for N = 1e8 is B0 = 2^18 = N/381 doubling up to
+    Bmax = 2^22 = N/23.8, i.e. 4 doubling epochs and then ~23 plateau epochs of 4.2 % of N each, during which the
+    temperature index stays frozen at the midpoint prediction.  The same shape scaled to what a serial run can
+    check: N = 1e5, B0 = 256 = N/391, Bmax = 4096 = N/24.4 (4 doubling + 24 plateau epochs, growth ratio 1),
+    against serial Bjorkman & Wood (B = 1): T within 0.5 % shell by shell, spectrum within 3 %."""
+    w = W.sphere32(tau_V=5.0, n=12)
+    N = 100_000
+    o = orc.Oracle.from_workload(w)
+    re = o.run(N, seed=43, B0=256, Bmax=4096, n_threads=NTH)
+    e_raw, e_out = o.read_raw(), o.read()
+    assert re["epochs"] == 4 + 24  # 256 + 512 + 1024 + 2048 = 3840, then 23 x 4096 + 1952
+    rs = o.run(N, seed=43, B0=1, Bmax=1)
+    s_raw, s_out = o.read_raw(), o.read()
+    assert rs["epochs"] == N
+    x = (np.arange(12) + 0.5) - 6
+    rr = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2).reshape(-1)
+    for lo in range(0, 6):
+        sel = (rr >= lo) & (rr < lo + 1) & (w.rho.reshape(-1) > 0)
+        Te, Ts = e_out["T"][sel].astype(float).mean(), s_out["T"][sel].astype(float).mean()
+        assert abs(Te / Ts - 1) < 0.005, (lo, Te, Ts)
+    # total absorbed energy and the emergent spectrum in 8 broad bands
+    assert abs(e_raw["k"].sum() / s_raw["k"].sum() - 1) < 0.005
+    se, ss = e_raw["sed"].sum(axis=0).astype(float), s_raw["sed"].sum(axis=0).astype(float)
+    be, bs = se.reshape(8, 8).sum(axis=1), ss.reshape(8, 8).sum(axis=1)
+    sel = bs > 500
+    assert sel.sum() >= 4
+    assert np.all(np.abs(be[sel] / bs[sel] - 1) < 0.03 + 3 / np.sqrt(bs[sel]))
+
+
+# ------------------------------------------------------------------------------------------ P16 frozen-T sweep
+def _thin_grey_sphere(orc, n=24, Tstar=1500.0, n_nu=160):
+    lam = W.wavelength_grid_um(n_nu, 0.2, 1e5)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = np.full(len(nu), 100.0)
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    rho0 = np.float32(1e-3 / (100.0 * n / 2 * h))   # radial tau = 1e-3 at every frequency (grey)
+    rho = np.where(r < n / 2, rho0, 0.0).astype(np.float32)
+    Tg = W.temperature_grid(1000, 2.0, 2000.0)
+    c = n / 2 * h
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 1, nu, kabs[None], np.zeros((1, len(nu))),
+                   np.zeros((1, len(nu))), Tg, W.LSUN_ERG_S, Tstar, None, [c, c, c], [0.0, 1.0])
+    return o, nu, Tg, rho, r, h, float(rho0)
+
+
+@pytest.mark.parametrize("from_lucy", [1, 0])
+def test_p16_frozen_temperature_sweep(orc, from_lucy):
+    """S12 / O-run mode 1 (Eq. 5): a sweep takes its temperatures from the PREVIOUS pass's tallies
+    (in that pass's packet energy and fixed-point scale), starts its own tallies from zero, and re-emits from the
+    Eq. 5 table kappa B_nu(T), not from the Eq. 10 table of the B&W pass.  Grey optically thin sphere, so that
+    T(r) = T* sqrt(R*/2r) is known in closed form (radiative balance, Eq. 4)."""
+    o, nu, Tg, rho, r, h, rho0 = _thin_grey_sphere(orc)
+    n = rho.shape[0]
+    N1, N2 = 2_000_000, 6_000_000            # different N: xi and the fixed-point scale differ between the passes
+    r1 = o.run(N1, seed=16, n_threads=NTH)
+    raw1 = o.read_raw()
+    r2 = o.run(N2, seed=16, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, sweep_T_from_lucy=from_lucy, n_threads=NTH)
+    raw2 = o.read_raw()
+    assert r1["fx_bits"] == 37 and r2["fx_bits"] == 35
+    L, Tstar = W.LSUN_ERG_S, 1500.0
+    dusty = rho.reshape(-1) > 0
+    tidx = raw2["tidx"].astype(np.int64)
+    J = o.tables()["J"][0]
+    xi1 = L / N1
+    # (a) the index is the Eq. 4 inversion of the previous pass's tallies at ITS xi and fixed-point scale
+    e1 = raw1["lucy_fx"] / 2.0 ** r1["fx_bits"] if from_lucy else raw1["k"].astype(np.float64)
+    x1 = e1 * (xi1 / (4 * math.pi * h ** 3)) / np.where(dusty, rho.reshape(-1), 1.0)
+    want = np.minimum(np.searchsorted(J, x1, side="left"), len(Tg) - 1)
+    assert (tidx[dusty] == want[dusty]).mean() > 0.9995       # (a cell whose x sits within rounding of a J entry may differ)
+    assert np.all(tidx[~dusty] == 0)
+    if from_lucy:
+        # (b) ... and that is the closed form T(r) = T* sqrt(R*/2r): position in the log T grid within +-1
+        Rstar = math.sqrt(L / (4 * math.pi * SIGMA_SB * Tstar ** 4))
+        dlnT = math.log(Tg[1] / Tg[0])
+        for r_lo in (4.0, 7.0, 10.0):
+            sel = ((r >= r_lo) & (r < r_lo + 1.0)).reshape(-1)
+            m_star = np.log(Tstar * np.sqrt(Rstar / (2 * r.reshape(-1)[sel] * h)) / Tg[0]) / dlnT
+            assert abs((tidx[sel] - m_star).mean() - 0.5) < 1.0, (r_lo, (tidx[sel] - m_star).mean())
+    else:
+        assert np.all(tidx[dusty & (raw1["k"] == 0)] == 0)
+    # (c) the sweep's tallies are its own: they start from zero
+    assert int(raw2["k"].sum()) == r2["absorptions"] and int(raw2["sed"].sum()) == N2 == r2["escapes"]
+    assert abs(r2["absorptions"] / N2 / (r1["absorptions"] / N1) - 1) < 5 / math.sqrt(r1["absorptions"])
+    l1, l2 = raw1["lucy_fx"].sum() / 2.0 ** 37 / N1, raw2["lucy_fx"].sum() / 2.0 ** 35 / N2
+    assert abs(l2 / l1 - 1) < 0.01 and abs(l2 / 1e-3 - 1) < 0.05   # sum of kappa rho ds per packet = radial tau
+    # (d) Eq. 5: the re-emitted packets (every interaction is an absorption here) carry <h nu> = zB k T_cell with
+    # zB = 4 zeta(5)/zeta(4) = 3.8322, not the 4.7903 of Eq. 10
+    re_em = (raw2["sed"] - raw2["sed_direct"]).sum(axis=0).astype(np.float64)
+    assert re_em.sum() > 3000
+    e_obs = (re_em * H_PLANCK * nu).sum() / re_em.sum()
+    k2 = raw2["k"].astype(np.float64)
+    kT = K_BOLTZ * (k2 * Tg[tidx]).sum() / k2.sum()
+    zB = 4 * special.zeta(5, 1) / special.zeta(4, 1)
+    ratio = e_obs / kT
+    assert abs(ratio / zB - 1) < 0.06, ratio
+    assert abs(ratio / (5 * special.zeta(5, 1) / special.zeta(4, 1)) - 1) > 0.12
+
+
+# ------------------------------------------------------------------------------------------ P17 outputs
+def test_p17_sed_flux_conversion_and_energy_outputs(orc):
+    """O12 outputs (PAPER.md:180 photon counting; PAPER.md:63 E = k xi).  Empty grid: every packet escapes, so
+    sum SED dnu dOmega = L exactly and SED_j = L_nu / 4 pi with L_nu the blackbody shape; dusty absorb-and-stop
+    run: E_count = k xi exactly and absorbed + escaped luminosity = L."""
+    Tstar, N = 4000.0, 400_000
+    w = W.uniform_cube(6, tau_edge_V=0.0, albedo=0.5, g_const=0.0, n_nu=24, n_dir=5, T_star=Tstar)
+    o = orc.Oracle.from_workload(w)
+    o.run(N, seed=17, n_threads=NTH)
+    sed, raw = o.read()["SED"], o.read_raw()
+    nu = w.nu_hz
+    # bin widths and blackbody weights written out independently (reading Q15)
+    edges = np.concatenate([[nu[0] * math.sqrt(nu[0] / nu[1])], np.sqrt(nu[:-1] * nu[1:]),
+                            [nu[-1] * math.sqrt(nu[-1] / nu[-2])]])
+    dnu = np.diff(edges)
+    Bnu = 2 * H_PLANCK * nu ** 3 / C_LIGHT ** 2 / np.expm1(H_PLANCK * nu / (K_BOLTZ * Tstar))
+    wj = Bnu * dnu / (Bnu * dnu).sum()
+    dom = 4 * math.pi * np.diff(w.abs_mu_edges)          # both hemispheres (reading Q22)
+    assert abs((sed * dnu[None, :] * dom[:, None]).sum() / w.L_erg_s - 1) < 1e-12
+    expect = w.L_erg_s * wj / (dnu * 4 * math.pi)          # erg s^-1 Hz^-1 sr^-1, the same in every direction bin
+    cnt_exp = N * np.outer(np.diff(w.abs_mu_edges), wj)
+    sel = cnt_exp > 30
+    assert sel.sum() >= 50
+    assert np.all(np.abs(sed / expect[None, :] - 1)[sel] < 4 / np.sqrt(cnt_exp[sel]))
+    np.testing.assert_allclose(sed, raw["sed"] * (w.L_erg_s / N) / (dnu[None, :] * dom[:, None]), rtol=1e-14)
+    # dusty: E_count = k xi and E_lucy = xi L / 2^FX exactly; absorbed + escaped = emitted
+    w2 = W.uniform_cube(8, tau_edge_V=1.0, albedo=0.0, g_const=0.0, n_nu=12, n_dir=3, T_star=Tstar)
+    o2 = orc.Oracle.from_workload(w2)
+    N2 = 50_000
+    r2 = o2.run(N2, seed=18, absorb_and_stop=True, n_threads=NTH)
+    out, raw2 = o2.read(), o2.read_raw()
+    xi = w2.L_erg_s / N2
+    assert np.array_equal(out["E_count"], raw2["k"].astype(np.float64) * xi)
+    assert np.array_equal(out["E_lucy"], raw2["lucy_fx"].astype(np.float64) * 2.0 ** -r2["fx_bits"] * xi)
+    nu2 = w2.nu_hz
+    e2 = np.concatenate([[nu2[0] * math.sqrt(nu2[0] / nu2[1])], np.sqrt(nu2[:-1] * nu2[1:]),
+                         [nu2[-1] * math.sqrt(nu2[-1] / nu2[-2])]])
+    esc = (out["SED"] * np.diff(e2)[None, :] * (4 * math.pi * np.diff(w2.abs_mu_edges))[:, None]).sum()
+    assert abs((out["E_count"].sum() + esc) / w2.L_erg_s - 1) < 1e-12
+    assert 0.2 < out["E_count"].sum() / w2.L_erg_s < 0.8
+    # the path-length estimate of the absorbed luminosity agrees with the counted one (PAPER.md:101)
+    assert abs(out["E_lucy"].sum() / out["E_count"].sum() - 1) < 4 / math.sqrt(raw2["k"].sum())
+
+
+# ------------------------------------------------------------------------------------------ P18 random flight
+@pytest.mark.parametrize("a,g", [(0.5, 0.0), (0.5, 0.6), (0.9, 0.0), (0.9, 0.6)])
+def test_p18_multiple_scattering_displacement(orc, a, g):
+    """O5 + O7 (Eq. 3; HG of Eq. 15): in an effectively infinite uniform grey medium a packet that
+    scatters with probability a (mean cosine g) and is absorbed otherwise ends at R = sum s_i u_i with exponential
+    flight lengths of mean l = 1/(kappa_ext rho), so <R^2> = 2 l^2 / [(1 - a)(1 - a g)], isotropic.  The tally
+    gives the absorption CELL: Sheppard's correction adds 1/12 cell^2 per axis.  This is the pin that fails when
+    the interaction point p += u t_int, its clamp or the rotation about the old direction is wrong."""
+    n, N = 160, 200_000
+    w = W.uniform_cube(n, tau_edge_V=40.0, albedo=a, g_const=g, n_nu=4, slope=0.0)
+    o = orc.Oracle.from_workload(w)
+    r = o.run(N, seed=1800 + int(100 * a + 10 * g), absorb_and_stop=True, B0=N, Bmax=N, n_threads=NTH)
+    assert r["escapes"] <= 2e-4 * N and r["absorptions"] + r["escapes"] == N
+    k = o.read_raw()["k"].reshape(n, n, n).astype(np.float64)
+    kext = float((w.kappa_abs + w.kappa_sca)[0, 0])
+    ell = 1.0 / (kext * float(w.rho.flat[0]) * w.cell_size_cm)          # mean free path in cells
+    assert abs(ell - 2.0) < 1e-6
+    assert abs(r["scatterings"] / (r["scatterings"] + r["absorptions"]) - a) < 4 * math.sqrt(a * (1 - a) / r["flights"])
+    d = (np.arange(n) + 0.5) - n / 2                                      # cell centre minus source, per axis
+    K = k.sum()
+    r2_true = 2 * ell ** 2 / ((1 - a) * (1 - a * g))
+    m2 = []
+    for axis, kk in enumerate((k.sum(axis=(0, 1)), k.sum(axis=(0, 2)), k.sum(axis=(1, 2)))):   # x, y, z marginals
+        m1 = (kk * d).sum() / K
+        v = (kk * d ** 2).sum() / K
+        s4 = (kk * d ** 4).sum() / K
+        assert abs(m1) < 4 * math.sqrt(v / K), (axis, m1)
+        assert abs(v - (r2_true / 3 + 1 / 12)) < 4 * math.sqrt((s4 - v * v) / K), (axis, v, r2_true / 3 + 1 / 12)
+        m2.append(v)
+    X, Y, Z = np.meshgrid(d, d, d, indexing="ij")
+    rr2 = (Z ** 2 + Y ** 2 + X ** 2)   # k is [z][y][x]; the sum of squares is symmetric
+    tot = (k * rr2).sum() / K
+    sig = math.sqrt(((k * rr2 ** 2).sum() / K - tot ** 2) / K)
+    assert abs(tot - (r2_true + 0.25)) < 4 * sig, (tot, r2_true + 0.25, sig)
+    assert sig / tot < 0.006            # the bound is sharp: 0.6 % (the voxel term alone is 0.3-1.5 %)
