@@ -47,7 +47,8 @@ enum {
     MCRT_ESTATE = -2,   /* call out of order */
     MCRT_ENOMEM = -3,   /* workspace too small / allocation failed */
     MCRT_ECUDA = -4,    /* CUDA runtime error */
-    MCRT_EOVERFLOW = -5 /* a fixed-point Lucy tally exceeded 2^62 */
+    MCRT_EOVERFLOW = -5 /* a fixed-point Lucy tally exceeded 2^62 (also returned by the read calls: the tallies
+                           they would hand back have wrapped) */
 };
 
 typedef enum {
@@ -69,6 +70,14 @@ typedef struct {
     int32_t block_threads;     /* launch tuning, 0 = auto (multiple of 32, <= 512) */
     int32_t time_kernels;      /* bracket every kernel with CUDA events on the context's stream; the
                                   summed durations are returned in mcrt_run_stats (transport_ms, update_ms) */
+    uint64_t first_packet_id;  /* the run's packets have ids first_packet_id .. first_packet_id + n_packets - 1
+                                  (a packet's random stream is keyed by its id, north_star item 1) */
+    uint64_t n_total;          /* the luminosity is split into this many packets, xi = L / n_total;
+                                  0 = n_packets.  Lets several runs (reset_tallies = 0, disjoint id ranges) add up
+                                  to one run of n_total packets */
+    double epoch_growth;       /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2.0; must be >= 1 */
+    int32_t part_index;        /* partitioned run (packets are independent): this context transports */
+    int32_t part_count;        /* slice part_index of part_count of EVERY epoch's id range; 0 or 1 = the whole run */
 } mcrt_run_opts;
 
 /* Counters of the runs since the last reset (all exact integers). */
@@ -138,11 +147,52 @@ int mcrt_escape_bins(mcrt_ctx *ctx, int n_dir, const double *abs_mu_edges);
 
 void mcrt_default_opts(mcrt_run_opts *opts);
 
-/* Transport n_packets packets with ids 0..n_packets-1 ("follow all N photon packets ...
- * until they ... escape").  opts NULL = defaults.  If stats_out is NULL the call only enqueues work on
- * the stream and returns without synchronising; otherwise it synchronises and fills stats_out. */
+/* Transport n_packets packets with ids opts.first_packet_id .. + n_packets - 1 ("follow all N
+ * photon packets ... until they ... escape").  opts NULL = defaults.  If stats_out is NULL the call only
+ * enqueues work on the stream and returns without synchronising (a fixed-point overflow is then reported by the
+ * next mcrt_get_stats / mcrt_read / mcrt_read_raw as MCRT_EOVERFLOW); otherwise it synchronises and fills
+ * stats_out.  With reset_tallies = 0 the run adds to the stored tallies; that is refused (MCRT_ESTATE) when their
+ * packet energy xi or fixed-point scale differs from this run's (use n_total). */
 int mcrt_run(mcrt_ctx *ctx, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts,
              mcrt_run_stats *stats_out);
+
+/* The same run one step at a time: mcrt_run(...) == mcrt_run_begin; while (!done) mcrt_run_step; mcrt_run_end.
+ * A step is one epoch (per-cell temperature-index update + transport of that epoch's packets) in
+ * MCRT_MODE_BW_EPOCH and one whole sweep in MCRT_MODE_FROZEN_T_SWEEP.  Only enqueues work on the stream.
+ * In a PARTITIONED run (opts.part_count > 1) every part calls the same sequence with the same
+ * n_packets / seed / opts except part_index, and after EVERY step the parts' tallies must be summed:
+ *   mcrt_exchange_begin (each part) -> element-wise 64-bit integer sum over the parts of every listed array,
+ *   written back to every part (ncclAllReduce(ncclSum, ncclInt64) in place, or mcrt_exchange_peer_sum) ->
+ *   mcrt_exchange_end (each part).
+ * The next mcrt_run_step / mcrt_run_end of a partitioned run returns MCRT_ESTATE until that has happened.  All
+ * tallies are integers, so the result is bit-identical to the unpartitioned run. */
+int mcrt_run_begin(mcrt_ctx *ctx, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts);
+int mcrt_run_step(mcrt_ctx *ctx, int *done_out);
+int mcrt_run_end(mcrt_ctx *ctx, mcrt_run_stats *stats_out /* NULL: do not synchronise */);
+
+/* Arrays of 64-bit integers (DEVICE pointers into the context's memory) to be summed over the parts now. */
+typedef struct {
+    int32_t n;            /* number of arrays (<= 8) */
+    void *ptr[8];
+    uint64_t words[8];    /* length of each array in 64-bit words (the same on every part) */
+} mcrt_exchange;
+
+/* After a step of a partitioned run.  Between two epochs of a B&W run only the absorption counts are listed
+ * (as this epoch's own increments; the temperature update is all that needs them); after the last epoch, and
+ * after every sweep, also the Lucy tallies, both escape histograms and the run counters. */
+int mcrt_exchange_begin(mcrt_ctx *ctx, mcrt_exchange *out);
+int mcrt_exchange_end(mcrt_ctx *ctx);
+
+/* The sum itself over peer-visible device memory (parts on one device, or on NVLink peers whose memory has been
+ * mapped into this process with CUDA IPC / peer access): views[p] is part p's mcrt_exchange.
+ *  phase 0 (reduce-scatter): this part sums slice part_index of every array over all parts into its own copy;
+ *  phase 1 (all-gather): this part copies every other slice from the part that owns it.
+ * All parts must have finished phase 0 before any starts phase 1 (stream order on one device, a barrier across
+ * processes).  Runs on ctx's stream; n_parts <= 16. */
+int mcrt_exchange_peer_sum(mcrt_ctx *ctx, int part_index, int n_parts, const mcrt_exchange *views, int phase);
+
+/* Convenience for parts that live in ONE process on ONE device (tests): begin + both phases + end for all. */
+int mcrt_exchange_local(mcrt_ctx *const *parts, int n_parts);
 
 /* Synchronise and return the counters accumulated since the last reset. */
 int mcrt_get_stats(mcrt_ctx *ctx, mcrt_run_stats *stats_out);

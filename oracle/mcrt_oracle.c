@@ -471,6 +471,7 @@ typedef struct {
     uint32_t pass0;          /* RNG pass word of the B&W run */
     uint64_t pid0;           /* id of the first packet of this run (continuing a run with further packets) */
     uint64_t n_total;        /* the luminosity is split into this many packets, xi = L / n_total; 0 = n_packets */
+    double growth;           /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2 (O11) */
 } orc_opts;
 
 typedef struct {
@@ -846,7 +847,12 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
             run_range(&R, o->pid0 + done, Be, &st);
             done += Be;
             Bprev = Be;
-            Bnom = (Bnom * 2 > Bmax) ? Bmax : Bnom * 2;
+            {
+                double nb = floor((double)Bnom * (o->growth > 0.0 ? o->growth : 2.0));
+                uint64_t nn = nb >= 1.8e19 ? Bmax : (uint64_t)nb;
+                if (nn < Bnom) nn = Bnom;
+                Bnom = nn > Bmax ? Bmax : nn;
+            }
             ++e;
             st.epochs++;
         }

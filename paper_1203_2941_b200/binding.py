@@ -22,7 +22,8 @@ MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP = 0, 1
 
 EXPORTS = [
     "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
-    "mcrt_default_opts", "mcrt_run", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
+    "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
+    "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
     "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
@@ -38,7 +39,13 @@ class RunOpts(C.Structure):
     _fields_ = [("mode", C.c_int32), ("epoch_B0", C.c_uint64), ("epoch_Bmax", C.c_uint64),
                 ("n_sweeps", C.c_int32), ("sweep_T_from_lucy", C.c_int32), ("record_digests", C.c_int32),
                 ("reset_tallies", C.c_int32), ("rng_pass", C.c_uint32), ("grid_blocks", C.c_int32),
-                ("block_threads", C.c_int32), ("time_kernels", C.c_int32)]
+                ("block_threads", C.c_int32), ("time_kernels", C.c_int32), ("first_packet_id", C.c_uint64),
+                ("n_total", C.c_uint64), ("epoch_growth", C.c_double), ("part_index", C.c_int32),
+                ("part_count", C.c_int32)]
+
+
+class Exchange(C.Structure):
+    _fields_ = [("n", C.c_int32), ("ptr", C.c_void_p * 8), ("words", C.c_uint64 * 8)]
 
 
 class RunStats(C.Structure):
@@ -77,6 +84,13 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_default_opts.argtypes = [C.POINTER(RunOpts)]
     L.mcrt_default_opts.restype = None
     L.mcrt_run.argtypes = [vp, u64, u64, C.POINTER(RunOpts), C.POINTER(RunStats)]
+    L.mcrt_run_begin.argtypes = [vp, u64, u64, C.POINTER(RunOpts)]
+    L.mcrt_run_step.argtypes = [vp, C.POINTER(i)]
+    L.mcrt_run_end.argtypes = [vp, C.POINTER(RunStats)]
+    L.mcrt_exchange_begin.argtypes = [vp, C.POINTER(Exchange)]
+    L.mcrt_exchange_end.argtypes = [vp]
+    L.mcrt_exchange_peer_sum.argtypes = [vp, i, i, C.POINTER(Exchange), i]
+    L.mcrt_exchange_local.argtypes = [C.POINTER(vp), i]
     L.mcrt_get_stats.argtypes = [vp, C.POINTER(RunStats)]
     L.mcrt_read.argtypes = [vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
@@ -164,6 +178,43 @@ def mcrt_run(ctx, n_packets, seed, opts: RunOpts | None = None, want_stats=True)
     _check(load_library().mcrt_run(ctx, int(n_packets), int(seed), C.byref(opts) if opts is not None else None,
                                    C.byref(st) if want_stats else None), ctx)
     return st.as_dict() if want_stats else None
+
+
+def mcrt_run_begin(ctx, n_packets, seed, opts: RunOpts | None = None):
+    _check(load_library().mcrt_run_begin(ctx, int(n_packets), int(seed), C.byref(opts) if opts is not None else None), ctx)
+
+
+def mcrt_run_step(ctx) -> bool:
+    """One epoch / sweep; returns True when it was the last one."""
+    done = C.c_int(0)
+    _check(load_library().mcrt_run_step(ctx, C.byref(done)), ctx)
+    return bool(done.value)
+
+
+def mcrt_run_end(ctx, want_stats=True):
+    st = RunStats()
+    _check(load_library().mcrt_run_end(ctx, C.byref(st) if want_stats else None), ctx)
+    return st.as_dict() if want_stats else None
+
+
+def mcrt_exchange_begin(ctx) -> Exchange:
+    ex = Exchange()
+    _check(load_library().mcrt_exchange_begin(ctx, C.byref(ex)), ctx)
+    return ex
+
+
+def mcrt_exchange_end(ctx):
+    _check(load_library().mcrt_exchange_end(ctx), ctx)
+
+
+def mcrt_exchange_peer_sum(ctx, part_index, views, phase):
+    arr = (Exchange * len(views))(*views)
+    _check(load_library().mcrt_exchange_peer_sum(ctx, int(part_index), len(views), arr, int(phase)), ctx)
+
+
+def mcrt_exchange_local(ctxs):
+    arr = (C.c_void_p * len(ctxs))(*[c.value if isinstance(c, C.c_void_p) else c for c in ctxs])
+    _check(load_library().mcrt_exchange_local(arr, len(ctxs)), ctxs[0])
 
 
 def mcrt_get_stats(ctx):
@@ -269,6 +320,24 @@ class Context:
         self._recorded = bool(o.record_digests)
         return mcrt_run(self.ctx, n_packets, seed, o, want_stats)
 
+    def _opts(self, n_packets, kw):
+        o = mcrt_default_opts()
+        for k, v in kw.items():
+            if not hasattr(o, k):
+                raise TypeError(f"unknown run option {k}")
+            setattr(o, k, v)
+        self.last_n = int(n_packets)
+        return o
+
+    def run_begin(self, n_packets, seed, **kw):
+        mcrt_run_begin(self.ctx, n_packets, seed, self._opts(n_packets, kw))
+
+    def run_step(self):
+        return mcrt_run_step(self.ctx)
+
+    def run_end(self, want_stats=True):
+        return mcrt_run_end(self.ctx, want_stats)
+
     def stats(self):
         return mcrt_get_stats(self.ctx)
 
@@ -313,3 +382,19 @@ class Context:
             self.close()
         except Exception:
             pass
+
+
+def run_parts_local(parts, n_packets, seed, **kw):
+    """A partitioned run whose parts are Contexts of ONE process on ONE device: every part
+    transports its slice of every epoch, then the tallies are summed with mcrt_exchange_local.  Returns the
+    (global) statistics.  Argument marshalling only."""
+    n = len(parts)
+    for r, c in enumerate(parts):
+        c.run_begin(n_packets, seed, part_index=r, part_count=n, **kw)
+    done = False
+    while not done:
+        flags = [c.run_step() for c in parts]
+        done = flags[0]
+        assert all(f == done for f in flags)
+        mcrt_exchange_local([c.ctx for c in parts])
+    return [c.run_end() for c in parts][0]

@@ -29,7 +29,8 @@ def nvcc_path() -> str:
 
 def build(force: bool = False, extra_flags=(), verbose: bool = False) -> str:
     os.makedirs(LIBDIR, exist_ok=True)
-    newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR), os.path.getmtime(__file__))
+    deps = [SRC, HDR, __file__] + [os.path.join(HERE, "csrc", f) for f in os.listdir(os.path.join(HERE, "csrc"))]
+    newest = max(os.path.getmtime(f) for f in deps)
     if (not force) and os.path.exists(OUT) and os.path.getmtime(OUT) >= newest:
         return OUT
     cmd = [nvcc_path(), *NVCC_FLAGS, *extra_flags, "-I", os.path.join(ROOT, "include"), "-o", OUT, SRC]

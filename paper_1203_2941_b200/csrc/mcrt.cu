@@ -83,11 +83,26 @@ struct mcrt_ctx {
     std::vector<double> nu, dnu, kabs, ksca, g, Tg, kext_h, kabs_h, albedo, J, cdfB, cdfdB, srccdf, mu_edges;
     double L = 0.0, pos[3] = {0, 0, 0};
     bool have_tables = false, have_source = false, mu_dirty = true;
-    // run state
+    double *sed_stage = nullptr;          // [ndir*nf] staging of the SED for host reads
+    // run state: fx / xi are the fixed-point scale and packet energy of the STORED tallies
     uint64_t last_n = 0;
     int fx = 40;
     double xi = 0.0;
     uint64_t epochs = 0, launches = 0;
+    uint64_t dig_base = 0;                // packet id of digest slot 0
+    // run in progress (mcrt_run_begin .. mcrt_run_end)
+    struct Run {
+        bool active = false;
+        mcrt_run_opts o;
+        uint64_t n = 0, seed = 0, done = 0, Bnom = 0, Bprev = 0, Bmax = 0;
+        int e = 0, sweep = 0, blocks = 0, threads = 0, prev_fx = 40;
+        size_t smem = 0;
+        double cellfac = 0.0, prev_cellfac = 0.0, growth = 2.0;
+        bool finished = false;            // every step has been issued
+    } run;
+    bool need_exchange = false;           // partitioned run: a step's tallies are still per-part
+    bool exchange_open = false, exchange_full = false;
+    bool globalised = false;              // the stored tallies are sums over the parts of a partitioned run
     int occ_blocks = 0;
     // optional per-kernel timing: events e[3i], e[3i+1], e[3i+2] bracket update and transport of launch pair i
     std::vector<cudaEvent_t> ev_pool;
@@ -315,7 +330,7 @@ struct TransportParams {
     int bsh;            // log2 of the brick edge
     int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
-    unsigned long long pid0, count;
+    unsigned long long pid0, count, dig_base;
     uint32_t seed_lo, seed_hi, pass;
 };
 
@@ -889,7 +904,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     mcrt_digest dg;
                     dg.hash = hash; dg.crossings = ncross; dg.scatterings = nsca; dg.absorptions = nabs;
                     dg.escape_bin = (uint32_t)bin;
-                    P.dig[pid] = dg;  // packet ids of a run start at 0
+                    P.dig[pid - P.dig_base] = dg;
                 }
                 kind = K_EMIT;        // the slot takes the next packet of the epoch
             }
@@ -1132,6 +1147,37 @@ __global__ void __launch_bounds__(256) k_sweep_update(unsigned long long *__rest
         kcnt[i] = 0ull;
         kprev[i] = 0ull;
         lfx[i] = 0ll;
+    }
+}
+
+// Partitioned runs: between epochs a part's absorption counts are exchanged as this epoch's own
+// increments, k - k_prev (k_prev = the global counts at the start of the epoch), and restored afterwards.
+__global__ void __launch_bounds__(256) k_count_delta(unsigned long long *__restrict__ kcnt, const unsigned long long *__restrict__ kprev,
+                                                     size_t n, int restore)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+        kcnt[i] = restore ? kcnt[i] + kprev[i] : kcnt[i] - kprev[i];
+}
+
+// Sum of the parts' tallies over peer-visible memory, reduce-scatter / all-gather (mcrt_exchange_peer_sum):
+// phase 0: own[i] = sum_p part_p[i] for i in this part's slice; phase 1: own[i] = owner(i)[i] for the other slices.
+constexpr int kMaxParts = 16;
+struct PeerPtrs { unsigned long long *p[kMaxParts]; };
+__global__ void __launch_bounds__(256) k_peer_sum(PeerPtrs pp, int me, int n_parts, size_t words, int phase)
+{
+    const size_t per = (words + (size_t)n_parts - 1) / (size_t)n_parts;
+    if (phase == 0) {
+        const size_t lo = per * (size_t)me, hi = lo + per < words ? lo + per : words;
+        for (size_t i = lo + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < hi; i += (size_t)gridDim.x * blockDim.x) {
+            unsigned long long v = 0ull;
+            for (int q = 0; q < n_parts; ++q) v += pp.p[q][i];
+            pp.p[me][i] = v;
+        }
+    } else {
+        for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < words; i += (size_t)gridDim.x * blockDim.x) {
+            const int owner = (int)(i / per);
+            if (owner != me) pp.p[me][i] = pp.p[owner][i];
+        }
     }
 }
 
@@ -1445,6 +1491,8 @@ void mcrt_default_opts(mcrt_run_opts *o)
     o->mode = MCRT_MODE_BW_EPOCH;
     o->sweep_T_from_lucy = 1;
     o->reset_tallies = 1;
+    o->epoch_growth = 2.0;
+    o->part_count = 1;
 }
 
 int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_T, int n_dir, uint64_t n_digests,
@@ -1717,6 +1765,7 @@ static int ensure_histograms(mcrt_ctx *c)
         if ((rc = ws_alloc(c, (void **)&c->d_mu, (size_t)(c->ndir + 1) * 8))) return rc;
         if ((rc = ws_alloc(c, (void **)&c->sed, (size_t)c->ndir * c->nf * 8))) return rc;
         if ((rc = ws_alloc(c, (void **)&c->sed_direct, (size_t)c->ndir * c->nf * 8))) return rc;
+        if ((rc = ws_alloc(c, (void **)&c->sed_stage, (size_t)c->ndir * c->nf * 8))) return rc;
         c->ndir_alloc = c->ndir;
     }
     CUDA_TRY(c, cudaMemcpyAsync(c->d_mu, c->mu_edges.data(), (size_t)(c->ndir + 1) * 8, cudaMemcpyHostToDevice, c->stream));
@@ -1788,20 +1837,61 @@ int mcrt_get_stats(mcrt_ctx *c, mcrt_run_stats *st)
     return st->overflow ? fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62") : MCRT_OK;
 }
 
-int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts, mcrt_run_stats *stats_out)
+static void fill_params(mcrt_ctx *c, TransportParams &P)
+{
+    memset(&P, 0, sizeof(P));
+    P.cellw = c->cellw; P.lfx = c->lfx; P.kcnt = c->kabs_cnt;
+    P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
+    P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
+    P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
+    P.dig = c->run.o.record_digests ? c->dig : nullptr;
+    P.dig_base = c->dig_base;
+    P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
+    P.nbx = c->nbx; P.nby = c->nby;
+    P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords; P.ncp = (uint32_t)c->ncp;
+    P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
+    P.seed_lo = (uint32_t)c->run.seed; P.seed_hi = (uint32_t)(c->run.seed >> 32);
+}
+
+// this part's slice [lo, hi) of an id range of `count` packets (every epoch is split the same way)
+static void part_slice(const mcrt_run_opts &o, uint64_t count, uint64_t *lo, uint64_t *hi)
+{
+    const uint64_t R = o.part_count > 1 ? (uint64_t)o.part_count : 1u, r = o.part_count > 1 ? (uint64_t)o.part_index : 0u;
+    *lo = (uint64_t)(((unsigned __int128)count * r) / R);
+    *hi = (uint64_t)(((unsigned __int128)count * (r + 1)) / R);
+}
+
+int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts)
 {
     if (!c) return MCRT_EINVAL;
+    if (c->run.active) return fail(c, MCRT_ESTATE, "a run is in progress: call mcrt_run_end first");
     if (!c->have_tables || !c->have_source) return fail(c, MCRT_ESTATE, "call mcrt_dust_tables and mcrt_source before mcrt_run");
     if (n_packets < 1) return fail(c, MCRT_EINVAL, "n_packets must be >= 1");
     mcrt_run_opts o;
     if (opts) o = *opts; else mcrt_default_opts(&o);
     if (o.mode != MCRT_MODE_BW_EPOCH && o.mode != MCRT_MODE_FROZEN_T_SWEEP) return fail(c, MCRT_EINVAL, "unknown mode");
     if (o.mode == MCRT_MODE_FROZEN_T_SWEEP && o.n_sweeps < 1) return fail(c, MCRT_EINVAL, "n_sweeps must be >= 1");
+    if (o.part_count < 0 || o.part_count > 65536 || (o.part_count > 1 && (o.part_index < 0 || o.part_index >= o.part_count)))
+        return fail(c, MCRT_EINVAL, "part_index must be in 0..part_count-1");
+    if (o.part_count <= 1) { o.part_count = 1; o.part_index = 0; }
+    if (o.epoch_growth == 0.0) o.epoch_growth = 2.0;
+    if (!(o.epoch_growth >= 1.0) || !isfinite(o.epoch_growth)) return fail(c, MCRT_EINVAL, "epoch_growth must be >= 1");
+    if (o.n_total && o.n_total < n_packets) return fail(c, MCRT_EINVAL, "n_total must be >= n_packets");
+    if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
     int rc = ensure_histograms(c);
     if (rc) return rc;
-    int blocks, threads; size_t smem;
-    if ((rc = transport_config(c, &o, &blocks, &threads, &smem))) return rc;
+    mcrt_ctx::Run &R = c->run;
+    if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem))) return rc;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
+
+    const uint64_t n_xi = o.n_total ? o.n_total : n_packets;
+    const int fx = fx_bits_for(n_xi);
+    const double xi = c->L / (double)n_xi;                          // xi = L/N
+    const bool continuing = o.mode == MCRT_MODE_BW_EPOCH && !o.reset_tallies && c->last_n != 0;
+    if (continuing && (xi != c->xi || fx != c->fx))
+        return fail(c, MCRT_ESTATE, "reset_tallies = 0: the stored tallies have another packet energy / fixed-point scale (set n_total)");
+    if (continuing && c->globalised)
+        return fail(c, MCRT_ESTATE, "reset_tallies = 0 after a partitioned run: the stored tallies are sums over the parts");
 
     if (o.record_digests) {
         if (c->dig_cap < n_packets) {
@@ -1809,7 +1899,9 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
             c->dig_cap = n_packets;
         }
         c->dig_n = n_packets;
+        if (o.part_count > 1) CUDA_TRY(c, cudaMemsetAsync(c->dig, 0, n_packets * sizeof(mcrt_digest), c->stream));
     } else c->dig_n = 0;
+    c->dig_base = o.first_packet_id;
 
     if (o.reset_tallies && o.mode == MCRT_MODE_BW_EPOCH) {
         CUDA_TRY(c, cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
@@ -1821,12 +1913,13 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
         c->epochs = 0; c->launches = 0;
         if (c->ev_used) { cudaStreamSynchronize(c->stream); fold_timing(c); }
         c->transport_ms = 0.0; c->update_ms = 0.0;
+        c->globalised = false;
     }
-    const bool timing = o.time_kernels != 0;
-    const int prev_fx = c->fx;
-    c->fx = fx_bits_for(n_packets);
-    c->xi = c->L / (double)n_packets;                            // xi = L/N
-    const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);  // xi / (4 pi V) of Eq. 4
+    // Eq. 4 for the first sweep: the stored k and L are in packets of the run that made them
+    R.prev_fx = c->fx;
+    R.prev_cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
+    c->fx = fx; c->xi = xi;
+    R.cellfac = xi / (kFourPi * c->h * c->h * c->h);             // xi / (4 pi V) of Eq. 4
     c->last_n = n_packets;
     {
         const size_t nsf = (size_t)c->ns * c->nf;
@@ -1835,80 +1928,207 @@ int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts
         CUDA_TRY(c, cudaMemcpyAsync(c->d_kabs_fx, kfx.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     }
-
-    TransportParams P;
-    memset(&P, 0, sizeof(P));
-    P.cellw = c->cellw; P.lfx = c->lfx; P.kcnt = c->kabs_cnt;
-    P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
-    P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
-    P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
-    P.dig = o.record_digests ? c->dig : nullptr;
-    P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
-    P.nbx = c->nbx; P.nby = c->nby;
-    P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords; P.ncp = (uint32_t)c->ncp;
-    P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
-    P.seed_lo = (uint32_t)seed; P.seed_hi = (uint32_t)(seed >> 32);
     const size_t j_smem = (size_t)c->ns * c->nT * 8;
     if (j_smem > 48 * 1024) {
         CUDA_TRY(c, cudaFuncSetAttribute(k_epoch_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_sweep_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
     }
-    const int ugrid = stream_grid(c->ncp);
+    R.o = o; R.n = n_packets; R.seed = seed; R.done = 0; R.Bprev = 0; R.e = 0; R.sweep = 0; R.finished = false;
+    R.growth = o.epoch_growth;
+    uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
+    if (B0 == 0) { B0 = 256; while (B0 * 2 <= n_packets / 256) B0 *= 2; }
+    if (Bmax == 0) Bmax = (uint64_t)1 << 22;
+    if (Bmax < B0) Bmax = B0;
+    R.Bnom = B0; R.Bmax = Bmax;
+    c->need_exchange = false; c->exchange_open = false;
+    R.active = true;
+    return MCRT_OK;
+}
 
+int mcrt_run_step(mcrt_ctx *c, int *done_out)
+{
+    if (!c) return MCRT_EINVAL;
+    mcrt_ctx::Run &R = c->run;
+    if (!R.active) return fail(c, MCRT_ESTATE, "mcrt_run_step without mcrt_run_begin");
+    if (c->need_exchange) return fail(c, MCRT_ESTATE, "partitioned run: the parts' tallies must be exchanged after every step");
+    if (R.finished) { if (done_out) *done_out = 1; return MCRT_OK; }
+    const mcrt_run_opts &o = R.o;
+    const bool timing = o.time_kernels != 0;
+    const size_t j_smem = (size_t)c->ns * c->nT * 8;
+    const int ugrid = stream_grid(c->ncp);
+    const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
+    TransportParams P;
+    fill_params(c, P);
+    uint64_t lo, hi;
     if (o.mode == MCRT_MODE_BW_EPOCH) {
-        uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
-        if (B0 == 0) { B0 = 256; while (B0 * 2 <= n_packets / 256) B0 *= 2; }
-        if (Bmax == 0) Bmax = (uint64_t)1 << 22;
-        if (Bmax < B0) Bmax = B0;
+        const uint64_t Be = (R.n - R.done < R.Bnom) ? R.n - R.done : R.Bnom;
         P.cdf = c->d_cdfdB;
         P.pass = o.rng_pass;
-        uint64_t done = 0, Bnom = B0, Bprev = 0;
-        int e = 0;
-        while (done < n_packets) {
-            const uint64_t Be = (n_packets - done < Bnom) ? n_packets - done : Bnom;
-            mark(c, timing);
-            k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns,
-                                                             c->ncp, e == 0, e == 0 ? 1.0 : (double)Be / (double)Bprev,
-                                                             cellfac, c->counters);
-            P.pid0 = done; P.count = Be;
-            mark(c, timing);
-            if (o.record_digests) k_transport<true><<<blocks, threads, smem, c->stream>>>(P);
-            else k_transport<false><<<blocks, threads, smem, c->stream>>>(P);
-            mark(c, timing);
-            c->launches += 2;
-            c->epochs++;
-            done += Be; Bprev = Be;
-            Bnom = (Bnom * 2 > Bmax) ? Bmax : Bnom * 2;
-            ++e;
+        mark(c, timing);
+        k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
+                                                         R.e == 0, R.e == 0 ? 1.0 : (double)Be / (double)R.Bprev,
+                                                         R.cellfac, c->counters);
+        part_slice(o, Be, &lo, &hi);
+        P.pid0 = o.first_packet_id + R.done + lo; P.count = hi - lo;
+        mark(c, timing);
+        if (P.count) {
+            if (o.record_digests) k_transport<true><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+            else k_transport<false><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
         }
+        mark(c, timing);
+        c->launches += P.count ? 2 : 1;
+        c->epochs++;
+        R.done += Be; R.Bprev = Be;
+        {   // B_{e+1} = min(floor(B_e * growth), Bmax), never shrinking
+            const double nb = floor((double)R.Bnom * R.growth);
+            uint64_t nn = nb >= 1.8e19 ? R.Bmax : (uint64_t)nb;
+            if (nn < R.Bnom) nn = R.Bnom;
+            R.Bnom = nn > R.Bmax ? R.Bmax : nn;
+        }
+        ++R.e;
+        R.finished = R.done >= R.n;
     } else {
+        const int sw = ++R.sweep;
         P.cdf = c->d_cdfB;
-        for (int sw = 1; sw <= o.n_sweeps; ++sw) {
-            // temperatures of the previous pass (its own fixed-point scale), then zero and re-run all N packets
-            mark(c, timing);
-            k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns,
-                                                             c->ncp, o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? prev_fx : c->fx)),
-                                                             cellfac, c->counters);
-            CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
-            CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
-            CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
-            P.pass = o.rng_pass + (uint32_t)sw;
-            P.pid0 = 0; P.count = n_packets;
-            mark(c, timing);
-            if (o.record_digests) k_transport<true><<<blocks, threads, smem, c->stream>>>(P);
-            else k_transport<false><<<blocks, threads, smem, c->stream>>>(P);
-            mark(c, timing);
-            c->launches += 2;
-            c->epochs++;
+        // temperatures of the previous pass (its own packet energy and fixed-point scale), then zero and re-run all N packets
+        mark(c, timing);
+        k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
+                                                         o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
+                                                         sw == 1 ? R.prev_cellfac : R.cellfac, c->counters);
+        CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
+        c->globalised = false;
+        if (o.part_count > 1 && o.record_digests) CUDA_TRY(c, cudaMemsetAsync(c->dig, 0, c->dig_n * sizeof(mcrt_digest), c->stream));
+        P.pass = o.rng_pass + (uint32_t)sw;
+        part_slice(o, R.n, &lo, &hi);
+        P.pid0 = o.first_packet_id + lo; P.count = hi - lo;
+        mark(c, timing);
+        if (P.count) {
+            if (o.record_digests) k_transport<true><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+            else k_transport<false><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
         }
+        mark(c, timing);
+        c->launches += P.count ? 2 : 1;
+        c->epochs++;
+        R.finished = sw >= o.n_sweeps;
     }
-    k_range_check<<<ugrid, 256, 0, c->stream>>>(c->lfx, c->ncp, c->counters);
+    CUDA_TRY(c, cudaGetLastError());
+    if (o.part_count > 1) {
+        c->need_exchange = true;
+        c->exchange_full = R.finished || o.mode == MCRT_MODE_FROZEN_T_SWEEP;
+    }
+    if (done_out) *done_out = R.finished ? 1 : 0;
+    return MCRT_OK;
+}
+
+int mcrt_run_end(mcrt_ctx *c, mcrt_run_stats *stats_out)
+{
+    if (!c) return MCRT_EINVAL;
+    mcrt_ctx::Run &R = c->run;
+    if (!R.active) return fail(c, MCRT_ESTATE, "mcrt_run_end without mcrt_run_begin");
+    if (!R.finished) return fail(c, MCRT_ESTATE, "mcrt_run_end before the last mcrt_run_step");
+    if (c->need_exchange) return fail(c, MCRT_ESTATE, "partitioned run: exchange the last step's tallies before mcrt_run_end");
+    k_range_check<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx, c->ncp, c->counters);
     c->launches += 1;
+    R.active = false;
     CUDA_TRY(c, cudaGetLastError());
     if (stats_out) {
+        int rc;
         if ((rc = fill_stats(c, stats_out))) return rc;
         if (stats_out->overflow) return fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62");
     }
+    return MCRT_OK;
+}
+
+int mcrt_run(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts, mcrt_run_stats *stats_out)
+{
+    if (!c) return MCRT_EINVAL;
+    if (opts && opts->part_count > 1)
+        return fail(c, MCRT_EINVAL, "a partitioned run needs an exchange after every step: use mcrt_run_begin / _step / _end");
+    int rc = mcrt_run_begin(c, n_packets, seed, opts);
+    if (rc) return rc;
+    int done = 0;
+    while (!done)
+        if ((rc = mcrt_run_step(c, &done))) { c->run.active = false; return rc; }
+    return mcrt_run_end(c, stats_out);
+}
+
+int mcrt_exchange_begin(mcrt_ctx *c, mcrt_exchange *out)
+{
+    if (!c || !out) return MCRT_EINVAL;
+    if (!c->need_exchange || c->exchange_open) return fail(c, MCRT_ESTATE, "mcrt_exchange_begin: no step of a partitioned run is waiting for its exchange");
+    memset(out, 0, sizeof(*out));
+    // this epoch's own increments k - k_prev (k_prev = the global counts the epoch started from)
+    k_count_delta<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->kabs_cnt, c->kprev, c->ncp, 0);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    int n = 0;
+    out->ptr[n] = c->kabs_cnt; out->words[n++] = c->ncp;
+    if (c->exchange_full) {
+        out->ptr[n] = c->lfx; out->words[n++] = c->ncp;
+        out->ptr[n] = c->sed; out->words[n++] = (uint64_t)c->ndir * c->nf;
+        out->ptr[n] = c->sed_direct; out->words[n++] = (uint64_t)c->ndir * c->nf;
+        out->ptr[n] = c->counters; out->words[n++] = CNT_NEXT;
+        if (c->dig_n) { out->ptr[n] = c->dig; out->words[n++] = c->dig_n * (sizeof(mcrt_digest) / 8); }  // zero except own packets
+    }
+    out->n = n;
+    c->exchange_open = true;
+    return MCRT_OK;
+}
+
+int mcrt_exchange_end(mcrt_ctx *c)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->exchange_open) return fail(c, MCRT_ESTATE, "mcrt_exchange_end without mcrt_exchange_begin");
+    k_count_delta<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->kabs_cnt, c->kprev, c->ncp, 1);
+    c->launches += 1;
+    CUDA_TRY(c, cudaGetLastError());
+    if (c->exchange_full) c->globalised = true;
+    c->exchange_open = false;
+    c->need_exchange = false;
+    return MCRT_OK;
+}
+
+int mcrt_exchange_peer_sum(mcrt_ctx *c, int part_index, int n_parts, const mcrt_exchange *views, int phase)
+{
+    if (!c || !views) return MCRT_EINVAL;
+    if (n_parts < 1 || n_parts > kMaxParts || part_index < 0 || part_index >= n_parts || (phase != 0 && phase != 1))
+        return fail(c, MCRT_EINVAL, "mcrt_exchange_peer_sum: 1 <= n_parts <= 16, 0 <= part_index < n_parts, phase 0 or 1");
+    for (int q = 1; q < n_parts; ++q) {
+        if (views[q].n != views[0].n) return fail(c, MCRT_EINVAL, "mcrt_exchange_peer_sum: the parts list different arrays");
+        for (int a = 0; a < views[0].n; ++a)
+            if (views[q].words[a] != views[0].words[a]) return fail(c, MCRT_EINVAL, "mcrt_exchange_peer_sum: array lengths differ between parts");
+    }
+    for (int a = 0; a < views[0].n; ++a) {
+        PeerPtrs pp;
+        for (int q = 0; q < kMaxParts; ++q) pp.p[q] = (unsigned long long *)views[q < n_parts ? q : 0].ptr[a];
+        const size_t words = views[0].words[a];
+        k_peer_sum<<<stream_grid(phase == 0 ? (words + n_parts - 1) / n_parts : words), 256, 0, c->stream>>>(pp, part_index, n_parts, words, phase);
+        c->launches += 1;
+    }
+    CUDA_TRY(c, cudaGetLastError());
+    return MCRT_OK;
+}
+
+int mcrt_exchange_local(mcrt_ctx *const *parts, int n_parts)
+{
+    if (!parts || n_parts < 1 || n_parts > kMaxParts) return MCRT_EINVAL;
+    std::vector<mcrt_exchange> v(n_parts);
+    int rc;
+    for (int q = 0; q < n_parts; ++q) {
+        if (!parts[q]) return MCRT_EINVAL;
+        if ((rc = mcrt_exchange_begin(parts[q], &v[q]))) return rc;
+    }
+    // one device, possibly several streams: every part's step must have finished before anyone reads its tallies
+    for (int phase = 0; phase < 2; ++phase) {
+        for (int q = 0; q < n_parts; ++q) CUDA_TRY(parts[q], cudaStreamSynchronize(parts[q]->stream));
+        for (int q = 0; q < n_parts; ++q)
+            if ((rc = mcrt_exchange_peer_sum(parts[q], q, n_parts, v.data(), phase))) return rc;
+    }
+    for (int q = 0; q < n_parts; ++q) CUDA_TRY(parts[q], cudaStreamSynchronize(parts[q]->stream));
+    for (int q = 0; q < n_parts; ++q)
+        if ((rc = mcrt_exchange_end(parts[q]))) return rc;
     return MCRT_OK;
 }
 
@@ -1927,18 +2147,29 @@ static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem wh
     return MCRT_OK;
 }
 
+// the read calls refuse to hand back wrapped tallies (the flag is set by the per-epoch update and the final range check)
+static int check_overflow(mcrt_ctx *c)
+{
+    unsigned long long flag = 0ull;
+    CUDA_TRY(c, cudaMemcpyAsync(&flag, c->counters + CNT_OVERFLOW, 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return flag ? fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62") : MCRT_OK;
+}
+
 int mcrt_read(mcrt_ctx *c, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy, double *SED, mcrt_mem where)
 {
     if (!c) return MCRT_EINVAL;
     if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read before mcrt_run");
+    if (c->run.active) return fail(c, MCRT_ESTATE, "mcrt_read inside mcrt_run_begin .. mcrt_run_end");
     int rc;
+    if ((rc = check_overflow(c))) return rc;
     if ((rc = gather_out(c, G_ECOUNT, E_abs_count, 8, where))) return rc;
     if ((rc = gather_out(c, G_ELUCY, E_abs_lucy, 8, where))) return rc;
     if ((rc = gather_out(c, G_TCOUNT, T_count, 4, where))) return rc;
     if ((rc = gather_out(c, G_TLUCY, T_lucy, 4, where))) return rc;
     if (SED) {
         const int n = c->ndir * c->nf;
-        double *dev = (where == MCRT_DEVICE) ? SED : (double *)c->scratch;
+        double *dev = (where == MCRT_DEVICE) ? SED : c->sed_stage;
         k_sed<<<(n + 255) / 256, 256, 0, c->stream>>>(dev, c->sed, c->d_dnu, c->d_mu, c->ndir, c->nf, c->xi);
         CUDA_TRY(c, cudaGetLastError());
         if (where == MCRT_HOST) {
@@ -1955,6 +2186,7 @@ int mcrt_read_raw(mcrt_ctx *c, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_
     if (!c) return MCRT_EINVAL;
     if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read_raw before mcrt_run");
     int rc;
+    if ((rc = check_overflow(c))) return rc;
     if ((rc = gather_out(c, G_K, k_abs, 8, where))) return rc;
     if ((rc = gather_out(c, G_LFX, lucy_fx, 8, where))) return rc;
     if ((rc = gather_out(c, G_TIDX, tidx, 2, where))) return rc;

@@ -15,7 +15,7 @@ import pytest
 from paper_1203_2941_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
-NTH = min(8, os.cpu_count() or 1)
+NTH = min(16, os.cpu_count() or 1)
 
 
 @pytest.fixture(scope="module")
@@ -29,16 +29,35 @@ def B():
     return binding
 
 
-def _run_both(orc, B, w, N, seed, mode=0, n_sweeps=0, from_lucy=1, B0=0, Bmax=0, grid_blocks=0, block_threads=0):
+COUNTERS = ("packets", "crossings", "dusty_crossings", "flights", "scatterings", "absorptions", "escapes",
+            "direct_escapes", "lucy_adds", "fx_bits")
+RAW_KEYS = ("k", "lucy_fx", "sed", "sed_direct", "tidx")
+
+
+def _run_both(orc, B, w, N, seed, mode=0, n_sweeps=0, from_lucy=1, B0=0, Bmax=0, grid_blocks=0, block_threads=0,
+              growth=0.0, N_first=None, plain=True):
+    """Oracle and CUDA path on the same inputs.  The CUDA path runs twice: recording per-packet digests
+    (k_transport<true>) and -- `plain` -- as bench.py runs it (k_transport<false>, another instantiation with
+    another pool slot layout); the second run's raw tallies and counters are kept in rg["plain"]."""
     o = orc.Oracle.from_workload(w)
     c = B.Context(w, n_digests=N)
-    if mode == 1:  # sweeps start from the temperatures of a B&W pass
-        o.run(N, seed, n_threads=NTH)
-        c.run(N, seed)
+    N1 = N if N_first is None else N_first
+    if mode == 1:  # sweeps start from the temperatures of a B&W pass (possibly of another N)
+        o.run(N1, seed, n_threads=NTH)
     ro = o.run(N, seed, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, B0=B0, Bmax=Bmax, digests=True,
-               n_threads=NTH)
-    rg = c.run(N, seed, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, epoch_B0=B0, epoch_Bmax=Bmax,
-               record_digests=1, grid_blocks=grid_blocks, block_threads=block_threads)
+               n_threads=NTH, growth=growth)
+    kw = dict(mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, epoch_B0=B0, epoch_Bmax=Bmax,
+              grid_blocks=grid_blocks, block_threads=block_threads, epoch_growth=growth)
+    plain_res = None
+    if plain:
+        if mode == 1:
+            c.run(N1, seed, grid_blocks=grid_blocks, block_threads=block_threads)
+        st = c.run(N, seed, record_digests=0, **kw)
+        plain_res = (st, c.read_raw())
+    if mode == 1:
+        c.run(N1, seed, grid_blocks=grid_blocks, block_threads=block_threads)
+    rg = c.run(N, seed, record_digests=1, **kw)
+    rg["plain"] = plain_res
     return o, c, ro, rg
 
 
@@ -51,12 +70,18 @@ def _assert_parity(o, c, ro, rg, w, N, min_frac=0.999):
     assert rg["packets"] == N == rg["escapes"] == int(raw_g["sed"].sum())
     if same.all():
         assert np.array_equal(do, dg)
-        for key in ("packets", "crossings", "dusty_crossings", "flights", "scatterings", "absorptions", "escapes",
-                    "direct_escapes", "lucy_adds", "fx_bits"):
+        for key in COUNTERS:
             assert ro[key] == rg[key], key
         for key in ("k", "sed", "sed_direct", "tidx"):
             assert np.array_equal(raw_o[key], raw_g[key]), key
         lucy_abs_tol = 16
+        if rg.get("plain") is not None:
+            # the instantiation bench.py times (no digests) against the oracle: every integer bit-exact
+            st_p, raw_p = rg["plain"]
+            for key in COUNTERS:
+                assert ro[key] == st_p[key], ("plain", key)
+            for key in RAW_KEYS:
+                assert np.array_equal(raw_o[key], raw_p[key]), ("plain", key)
     else:
         budget = int(do["absorptions"][~same].sum()) + int(dg["absorptions"][~same].sum())
         assert int(np.abs(raw_o["k"].astype(np.int64) - raw_g["k"].astype(np.int64)).sum()) <= budget
@@ -360,3 +385,160 @@ def test_error_paths(B):
     assert e.value.code == B.MCRT_ENOMEM
     B.mcrt_destroy(ctx)
 
+
+
+# ------------------------------------------------------------------------------------------ round 2
+@pytest.mark.parametrize("blocks,threads", [(2, 64), (1, 32)])
+@pytest.mark.parametrize("kind", ["torus", "thick_cube"])
+def test_parity_saturated_pools(B, orc, kind, blocks, threads):
+    """Every pool slot refilled hundreds of times: 1e5 packets on 2 x 2 x 64 (or 1 x 1 x 64) resident slots in one
+    32768-packet epoch after another, so the S-phase refill batches, mid-flight parking and pool exhaustion all
+    run with full warps -- compared with the oracle, in both kernel instantiations."""
+    w = W.torus256(n_clumps=400, n=64) if kind == "torus" else W.uniform_cube(12, 30.0, 0.5, 0.6, n_nu=32, slope=-1.0,
+                                                                               T_star=3000.0)
+    N = 100_000 if kind == "torus" else 20_000
+    o, c, ro, rg = _run_both(orc, B, w, N, 29, B0=32768, Bmax=32768, grid_blocks=blocks, block_threads=threads)
+    assert _assert_parity(o, c, ro, rg, w, N) == 1.0
+    c.close()
+
+
+def test_parity_config4_full_grid_1e7_packets_default_launch(B, orc):
+    """N_par = min(N, 1e7) on the full 256^3 torus in the launch configuration bench.py times.  The
+    schedule reaches full 2^22-packet epochs with every pool saturated.  Digests of 1e7 packets: 240 MB."""
+    w = W.torus256(n_clumps=5000)
+    N = 10_000_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    assert ro["epochs"] >= 9
+    assert _assert_parity(o, c, ro, rg, w, N) == 1.0
+    c.close()
+    o.close()
+
+
+@pytest.mark.parametrize("tau_V", [0.1, 100.0])
+def test_parity_config3_disk_optical_depths(B, orc, tau_V):
+    w = W.disk256(tau_V=tau_V, n=64)
+    N = 200_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+@pytest.mark.parametrize("n_clumps", [1000, 20000])
+def test_parity_config4_clump_numbers(B, orc, n_clumps):
+    w = W.torus256(n_clumps=n_clumps, n=64)
+    N = 200_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed)
+    _assert_parity(o, c, ro, rg, w, N)
+    c.close()
+
+
+def test_parity_config5_full_grid_three_sweeps(B, orc):
+    """BASELINE config 5 as specified: the full 512^3 grid (8-cell bricks), B&W pass, then 3 frozen-T sweeps
+    reusing the path-length tallies (S12), at the packet count the oracle finishes in seconds."""
+    w = W.torus512()
+    N = 100_000
+    o, c, ro, rg = _run_both(orc, B, w, N, w.seed, mode=1, n_sweeps=3, from_lucy=1)
+    assert _assert_parity(o, c, ro, rg, w, N) == 1.0
+    c.close()
+    o.close()
+
+
+def test_parity_sweep_after_pass_with_another_packet_count(B, orc):
+    """The first sweep inverts Eq. 4 with the packet energy and fixed-point scale of the pass whose tallies it
+    reads (oracle pin P16): B&W pass with 3e5 packets (FX 39), sweeps with 6e5 (FX 38)."""
+    w = W.torus512(n_clumps=300, n=48)
+    o, c, ro, rg = _run_both(orc, B, w, 600_000, w.seed, mode=1, n_sweeps=2, from_lucy=1, N_first=300_000)
+    assert ro["fx_bits"] == 38
+    _assert_parity(o, c, ro, rg, w, 600_000)
+    c.close()
+
+
+def test_parity_epoch_growth_option(B, orc):
+    w = W.sphere32(tau_V=4.0, n=16)
+    o, c, ro, rg = _run_both(orc, B, w, 30000, 23, B0=100, Bmax=5000, growth=1.25)
+    _assert_parity(o, c, ro, rg, w, 30000)
+    assert rg["epochs"] == ro["epochs"] > 12
+    c.close()
+
+
+def test_parity_run_continued_with_further_packet_ids(B, orc):
+    """first_packet_id / n_total: two runs over disjoint id ranges add up (reset_tallies = 0), xi = L / n_total."""
+    w = W.sphere32(tau_V=2.0, n=16)
+    N, Na = 60_000, 25_000
+    o = orc.Oracle.from_workload(w)
+    o.run(Na, 5, n_total=N, n_threads=NTH)
+    ro = o.run(N - Na, 5, n_total=N, pid0=Na, reset=False, n_threads=NTH, digests=True)
+    c = B.Context(w, n_digests=N)
+    c.run(Na, 5, n_total=N)
+    rg = c.run(N - Na, 5, n_total=N, first_packet_id=Na, reset_tallies=0, record_digests=1)
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    assert int(raw_g["sed"].sum()) == N
+    np.testing.assert_allclose(c.read()["E_count"], o.read()["E_count"], rtol=1e-12)
+    with pytest.raises(B.McrtError) as e:      # another packet energy cannot be added to these tallies
+        c.run(1000, 5, first_packet_id=N, reset_tallies=0)
+    assert e.value.code == B.MCRT_ESTATE
+    c.close()
+
+
+@pytest.mark.parametrize("n_parts", [2, 3])
+def test_partitioned_run_is_bit_identical(B, orc, n_parts):
+    """every epoch's packet ids split over the parts, integer tallies summed after every epoch
+    (mcrt_exchange_*: the peer-memory reduce-scatter / all-gather kernel) -- k, L, SED, tidx, digests and counters
+    bit-identical to the single-context run and to the oracle.  Parts = contexts on one device."""
+    w = W.torus256(n_clumps=400, n=64)
+    N = 150_001                                    # odd: uneven slices
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 77, n_threads=NTH, digests=True)
+    raw_o = o.read_raw()
+    single = B.Context(w, n_digests=N)
+    rs = single.run(N, 77, record_digests=1)
+    raw_s = single.read_raw(digests=True)
+    parts = [B.Context(w, n_digests=N) for _ in range(n_parts)]
+    rp = B.run_parts_local(parts, N, 77, record_digests=1)
+    for c in parts:
+        raw_p = c.read_raw(digests=True)
+        for key in RAW_KEYS + ("digests",):
+            assert np.array_equal(raw_s[key], raw_p[key]), key
+        for key in RAW_KEYS:
+            assert np.array_equal(raw_o[key], raw_p[key]), key
+        assert np.array_equal(ro["digests"], raw_p["digests"])
+    for key in COUNTERS:
+        assert rs[key] == rp[key] == ro[key], key
+    # then two frozen-T sweeps, partitioned the same way
+    ro2 = o.run(N, 77, mode=1, n_sweeps=2, n_threads=NTH)
+    raw_o2 = o.read_raw()
+    rp2 = B.run_parts_local(parts, N, 77, mode=1, n_sweeps=2)
+    for c in parts:
+        raw_p = c.read_raw()
+        for key in RAW_KEYS:
+            assert np.array_equal(raw_o2[key], raw_p[key]), key
+    for key in COUNTERS:
+        assert rp2[key] == ro2[key], key
+    # the protocol is enforced: a step without the exchange is refused
+    parts[0].run_begin(1000, 1, part_index=0, part_count=n_parts)
+    parts[0].run_step()
+    with pytest.raises(B.McrtError) as e:
+        parts[0].run_step()
+    assert e.value.code == B.MCRT_ESTATE
+    for c in parts + [single]:
+        c.close()
+
+
+def test_sed_read_to_host_on_a_tiny_grid(B, orc):
+    """n_dir * n_nu far larger than the cell count -- the SED staging buffer is its own allocation."""
+    w = W.uniform_cube(2, 1.0, 0.5, 0.3, n_nu=120, n_dir=9)
+    o = orc.Oracle.from_workload(w)
+    c = B.Context(w)
+    N = 50_000
+    ro = o.run(N, 3, n_threads=NTH)
+    rg = c.run(N, 3)
+    out = c.read()
+    np.testing.assert_allclose(out["SED"], o.read()["SED"], rtol=1e-12)
+    st = c.stats()
+    for key in COUNTERS:
+        assert st[key] == ro[key] == rg[key], key
+    assert st["overflow"] == 0
+    c.close()
