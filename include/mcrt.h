@@ -119,7 +119,7 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
  *             256-byte alignment required.  The library sub-allocates from it in call order (grid
  *             here, tables in mcrt_dust_tables, histograms and digests at the first mcrt_run that
  *             needs them) and returns MCRT_ENOMEM when it runs out; size it with mcrt_workspace_bytes.
- *  nx, ny <= 2048 and nz <= 1024 (cell coordinates are carried packed in 32 bits).
+ *  nx, ny <= 2040, nz <= 1016 and at most 2^31 cells with the guard shell (cell coordinates are carried packed in 32 bits).
  * The grid is re-laid out on the device into bricks of packed 8-byte cell words (4x4x4 cells up to 256^3,
  * 8x8x8 up to 512^3, ...); a bit mask of the bricks without dust and, for each of them, a large box of empty
  * bricks around it are built here as well (they let packets cross vacuum without touching memory). */

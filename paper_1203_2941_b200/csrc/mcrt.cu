@@ -35,7 +35,7 @@ constexpr double kFourPi = 12.566370614359172953850573533118;
 
 constexpr unsigned kFull = 0xffffffffu;
 
-enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4 };
+enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4, ST_STOP = 5 };
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
 
 // device counters (unsigned long long each)
@@ -55,7 +55,8 @@ struct mcrt_ctx {
     // grid
     int nx = 0, ny = 0, nz = 0, ns = 0;
     int nbx = 0, nby = 0, nbz = 0;   // bricks per axis
-    size_t nc = 0, ncp = 0;          // cells, padded (bricked) cells
+    size_t nc = 0, ncp = 0;          // cells, cells of the padded storage (guard shell included)
+    int px = 0, pxy = 0;             // row and plane pitch of the padded storage
     double h = 0.0;
     // workspace (bump allocator)
     char *ws = nullptr;
@@ -301,11 +302,18 @@ __device__ __forceinline__ unsigned long long event_word(int type, int j, unsign
 // One 8-byte load per crossing serves S4, S5, S6 and S9, and the density needs no fp32->fp64 conversion.
 // ------------------------------------------------------------------------------------------------
 constexpr unsigned long long kRhoMask = 0xFFFFFFFFE0000000ull;
+#ifndef MCRT_DEPTH
+#define MCRT_DEPTH 2                // cell words in flight per lane of the walk (the geometry runs this many cells ahead)
+#endif
+constexpr int kDepth = MCRT_DEPTH;
+constexpr int kGuard = kDepth + 1;  // guard cells around the grid in the padded storage (see "Storage order")
 
 __device__ __forceinline__ double cw_rho(unsigned long long cw) { return __longlong_as_double((long long)(cw & kRhoMask)); }
 __device__ __forceinline__ int cw_species(unsigned long long cw) { return (int)((unsigned)cw & 0xffu); }
 __device__ __forceinline__ int cw_tidx(unsigned long long cw) { return (int)(((unsigned)cw >> 8) & 0xffffu); }
 __device__ __forceinline__ bool cw_vacuum(unsigned long long cw) { return (unsigned)(cw >> 32) == 0u; }  // rho == +0
+// a cell that holds dust: 0 < rho < +inf (the cells of an empty brick carry the marker density +inf)
+__device__ __forceinline__ bool cw_dusty(unsigned long long cw) { return (unsigned)(cw >> 32) - 1u < 0x7FEFFFFFu; }
 
 // The grid is stored brick-major: bricks of E^3 cells, E = 1 << bsh (4 for grids up to 256^3, 8 up to 512^3),
 // so that a packet's next cell is usually in the same 128-byte line or at least in the same brick.
@@ -326,7 +334,9 @@ struct TransportParams {
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
     int nbx, nby;       // bricks per axis
-    uint32_t ncp;       // padded cell count: cellw[ncp] holds the marker word kJumpWord
+    uint32_t ncp;       // padded cell count
+    int lpx, lpxy;      // row and plane pitch of the padded storage
+    double inv_lpx, inv_lpxy;
     int bsh;            // log2 of the brick edge
     int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
@@ -339,22 +349,39 @@ __device__ __forceinline__ uint32_t brick_of(int ix, int iy, int iz, int nbx, in
 {
     return (uint32_t)((iz >> bsh) * nby + (iy >> bsh)) * (uint32_t)nbx + (uint32_t)(ix >> bsh);
 }
-__device__ __forceinline__ uint32_t cell_in_brick(uint32_t brick, int ix, int iy, int iz, int bsh)
+// storage index of cell (ix, iy, iz) (see "Storage order")
+__device__ __forceinline__ uint32_t lin_index(int ix, int iy, int iz, int px, int pxy)
 {
-    const int m = (1 << bsh) - 1;
-    return (((brick << bsh) | (uint32_t)(iz & m)) << (2 * bsh)) | (uint32_t)(((iy & m) << bsh) | (ix & m));
+    return (uint32_t)((iz + kGuard) * pxy + (iy + kGuard) * px + (ix + kGuard));
 }
-__device__ __forceinline__ bool brick_empty(const uint32_t *m0, uint32_t brick) { return (m0[brick >> 5] >> (brick & 31u)) & 1u; }
+// ... and back, for a cell inside the grid: packed coordinates (quotients by a reciprocal, corrected exactly)
+__device__ __forceinline__ uint32_t index_to_packed(uint32_t idx, uint32_t px, uint32_t pxy, double inv_px, double inv_pxy)
+{
+    uint32_t z = __double2uint_rz(__uint2double_rn(idx) * inv_pxy);
+    int r = (int)(idx - z * pxy);
+    if (r < 0) { --z; r += (int)pxy; }
+    if (r >= (int)pxy) { ++z; r -= (int)pxy; }
+    uint32_t y = __double2uint_rz(__uint2double_rn((uint32_t)r) * inv_px);
+    int x = r - (int)(y * px);
+    if (x < 0) { --y; x += (int)px; }
+    if (x >= (int)px) { ++y; x -= (int)px; }
+    return (uint32_t)(x - kGuard) | ((y - (uint32_t)kGuard) << 11) | ((z - (uint32_t)kGuard) << 22);
+}
+__device__ __forceinline__ bool brick_empty(const uint32_t *__restrict__ m0, uint32_t brick) { return (m0[brick >> 5] >> (brick & 31u)) & 1u; }
 
 
 // S5 Lucy path-length tally: L[c] += rint(x), x = kabs h rho ds 2^FX >= 0 (Eq. 9, linear form;
 // PAPER.md:142 integer atomics).  rint by the 1.5 * 2^52 trick: round to nearest even, exact below 2^51, and
 // x < 37 * 2^40 always, because a packet never spends more than its tau = -ln zeta <= 36.8 in one cell.
-__device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
+__device__ __forceinline__ unsigned long long lucy_round(double x)
 {
     // round to nearest even by adding 1.5 * 2^52: the integer sits in the mantissa, the bias in the high word only
     const double y = x + 6755399441055744.0;
-    const unsigned long long q = ((unsigned long long)(uint32_t)(__double2hiint(y) - 0x43380000) << 32) | (uint32_t)__double2loint(y);
+    return ((unsigned long long)(uint32_t)(__double2hiint(y) - 0x43380000) << 32) | (uint32_t)__double2loint(y);
+}
+__device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
+{
+    const unsigned long long q = lucy_round(x);
     // (explicitly global: a pointer that went through shared memory has lost its address space)
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + cidx), "l"(q) : "memory");
 }
@@ -391,10 +418,10 @@ constexpr int kSlotF64 = 11 + 3 * MCRT_SLOT_IV;   // 8-byte fields per slot (+1,
 constexpr int kSlotU32 = 6;         // 4-byte fields per slot
 __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlots * ((kSlotF64 + (record ? 1 : 0)) * 8 + kSlotU32 * 4); }
 #ifndef MCRT_MAX_THREADS
-#define MCRT_MAX_THREADS 512        // 16 warps per SM, up to 128 registers per thread (640 = 20 warps measured no faster)
+#define MCRT_MAX_THREADS 640        // 20 warps per SM at <= 96 registers per thread (512 threads / 128 registers: 1 % slower)
 #endif
 #ifndef MCRT_SWAP_MIN
-#define MCRT_SWAP_MIN 6             // S phase: stopped packets are parked / replaced this many lanes at a time
+#define MCRT_SWAP_MIN 8             // S phase: stopped packets are parked / replaced this many lanes at a time
 #endif
 #ifndef MCRT_PIN
 #define MCRT_PIN 3                  // how many of the walk loop's kernel parameters are pinned in registers (1..3)
@@ -408,6 +435,9 @@ __host__ __device__ constexpr int pool_bytes_per_warp(bool record) { return kSlo
 #ifndef MCRT_J_MIN
 #define MCRT_J_MIN 10               // a J phase ends when fewer lanes than this still jump
 #endif
+#ifndef MCRT_SMEM_MASK
+#define MCRT_SMEM_MASK 0            // 1: every CTA keeps a copy of the empty-brick mask in shared memory; 0: read through L1
+#endif
 
 #if MCRT_SLOT_IV
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_IVX, F_IVY, F_IVZ, F_HASH };
@@ -416,16 +446,22 @@ enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, 
 #endif
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
-constexpr uint32_t kOutCell = 0xffffffffu;   // storage index of "outside the grid"
 // cell coordinates packed in 32 bits: x, y < 2048, z < 1024
 __device__ __forceinline__ uint32_t pack_xyz(int x, int y, int z) { return (uint32_t)x | ((uint32_t)y << 11) | ((uint32_t)z << 22); }
 __device__ __forceinline__ int unpack_x(uint32_t w) { return (int)(w & 0x7ffu); }
 __device__ __forceinline__ int unpack_y(uint32_t w) { return (int)((w >> 11) & 0x7ffu); }
 __device__ __forceinline__ int unpack_z(uint32_t w) { return (int)(w >> 22); }
-// ring word that stands for "this cell lies in an empty brick": no real cell word has bit 28 set with rho = 0
-constexpr unsigned long long kJumpWord = 0x10000000ull;
-// words behind the Lucy tally that take the (zero) adds of lanes that do not step a packet: one per thread of the grid
-constexpr size_t kLucyScratch = 131072;
+// Marker words: density +inf.  The cell words of an empty brick carry it ("a run of empty bricks starts here"), and
+// so does the word stored behind the grid that stands for every cell outside it (with kOutFlag in the temperature
+// field).  The walk needs no test of its own for them: rho = +inf makes the optical depth of the cell infinite.
+constexpr unsigned long long kJumpWord = 0x7FF0000000000000ull;
+constexpr uint32_t kMarkHi = 0x7FF00000u, kOutFlag = 0x100u;
+constexpr unsigned long long kOutWord = kJumpWord | kOutFlag;
+// Storage order of the per-cell arrays (cell words, Lucy tally, absorption counts): linear, x fastest, with a shell
+// of kGuard cells around the grid that hold the "outside the grid" marker word:
+//     index(ix, iy, iz) = ((iz + kGuard) * PY + (iy + kGuard)) * PX + (ix + kGuard),  PX = nx + 2 kGuard, PY = ny + 2 kGuard.
+// A step of the walk along one axis is then one constant added to the index (+-1, +-PX, +-PX*PY), a cell outside
+// the grid needs no test (its word says so), and the geometry of the walk may run up to kGuard cells beyond the grid.
 
 // position of the n-th set bit (n = 0, 1, ...) of a 64-bit mask; n < popc(m)
 __device__ __forceinline__ int nth_set64(unsigned long long m, int n)
@@ -495,18 +531,6 @@ struct SlotSet {
     }
 };
 
-// 8-byte asynchronous copy global -> shared (LDGSTS), per-thread groups
-__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
-
-constexpr int kRing = 4;            // cell-word ring slots per thread (cells n .. n+3)
-
 template <bool RECORD>
 __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const TransportParams P)
 {
@@ -523,13 +547,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     unsigned long long *s_cnt = reinterpret_cast<unsigned long long *>(s_mu + P.ndir + 1);
     unsigned int *s_hist = reinterpret_cast<unsigned int *>(s_cnt + 8 * nwarps);
     const int nhist = 2 * P.ndir * P.nf;
-    uint32_t *s_m0 = s_hist + nhist;         // level-0 vacuum mask (one bit per brick)
-    // cell-word ring: slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
-    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0 + ((P.mwords + 1) & ~1));
-
-    char *ring = reinterpret_cast<char *>(s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u));
-    constexpr int kRingStep = 32 * 8, kRingMask = (kRing - 1) * kRingStep;   // ring slots as byte offsets 0, 256, 512, 768
-#define RING(off) (*reinterpret_cast<volatile unsigned long long *>(ring + (off)))
+    uint32_t *s_m0x = s_hist + nhist;        // level-0 vacuum mask (one bit per brick)
+    const int mw_smem = MCRT_SMEM_MASK ? P.mwords : 0;
+    const uint32_t *s_m0 = MCRT_SMEM_MASK ? s_m0x : P.vmask;
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -538,7 +558,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int i = threadIdx.x; i < P.nf; i += blockDim.x) s_src[i] = P.srccdf[i];
     for (int i = threadIdx.x; i <= P.ndir; i += blockDim.x) s_mu[i] = P.mu_edges[i];
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
-    for (int i = threadIdx.x; i < P.mwords; i += blockDim.x) s_m0[i] = P.vmask[i];
+    for (int i = threadIdx.x; i < mw_smem; i += blockDim.x) s_m0x[i] = P.vmask[i];
     for (int i = threadIdx.x; i < 8 * nwarps; i += blockDim.x) s_cnt[i] = 0ull;   // eight counters per warp
     // Kernel parameters the walk loop uses, parked in shared memory: the S phase reads them into registers through
     // a volatile pointer, so that they stay there (left to itself the compiler reloads a dozen of them from the
@@ -549,12 +569,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         s_parp[0] = reinterpret_cast<unsigned long long>(P.cellw);
         s_parp[1] = reinterpret_cast<unsigned long long>(P.lfx);
         s_pari[0] = P.ncp; s_pari[1] = (uint32_t)P.nbx; s_pari[2] = (uint32_t)P.nby; s_pari[3] = (uint32_t)P.nx;
-        s_pari[4] = (uint32_t)P.ny; s_pari[5] = (uint32_t)P.nz; s_pari[6] = (uint32_t)P.bsh; s_pari[7] = (uint32_t)P.nf;
+        s_pari[4] = (uint32_t)P.ny; s_pari[5] = (uint32_t)P.lpx; s_pari[6] = (uint32_t)P.lpxy; s_pari[7] = (uint32_t)P.nf;
     }
     __syncthreads();
 
     const int lane = (int)(threadIdx.x & 31u);
-    const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby;
+    const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby, lpx = P.lpx, lpxy = P.lpxy;
     double *wf = s_pool + (size_t)(threadIdx.x >> 5) * kPoolF64;                  // this warp's pool, f64 fields
     uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kNF64 * kSlots);             // its u32 fields
 #define SF(f, s) wf[(f) * kSlots + (s)]
@@ -574,11 +594,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
-            // (G: axis choice, next cell, exit parameter) runs ahead of the physics and the cell words travel
-            // global -> shared memory with cp.async into a small per-thread ring: the word of cell n+2 is
-            // requested in the step that handles cell n, so its latency is covered by two walk iterations of
-            // every resident warp.  Between G and the physics sits one queue entry (exit parameter, storage
-            // index, packed coordinates of cell n).  The ring slot of cell n is the same in every lane.
+            // (G: axis choice, next cell, exit parameter) runs ahead of the physics: in the step that handles cell n,
+            // G enters cell n+2 and issues the load of its word into a register (two words are in flight per lane,
+            // wA / wB, which alternate in the two steps of the loop body), so the latency of a cell word is covered
+            // by two walk steps of every resident warp.  Between G and the physics sits one queue entry (exit
+            // parameter and storage index of cell n+1).
             // Lanes whose packet reaches an event or an empty brick park it and take another flying packet
             // from the pool without leaving the loop; a new packet enters the pipeline behind one no-op cell
             // (zero length, vacuum), which the physics passes without effect.  The phase ends when the pool has
@@ -589,47 +609,44 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double tprev = 0.0, tnA = 0.0;                      // parameters at which cell n is entered and left
             double fdx = 0.0, fdy = 0.0, fdz = 0.0;             // coordinate of the face through which G's cell is left
             int shx = 0, shy = 0, shz = 0;                      // high word of the step per axis as a double (+1, -1 or 0)
-            int gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
-            uint32_t ciA = 0u, xzA = 0u;                        // storage index and packed coordinates of cell n
-            uint32_t gcidx = 0u, ncross = 0u;
-            double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at frequency j
-            int kq_sp = -1;
-            int r = 0;                                          // ring slot of cell n (byte offset): the same in every lane
+            uint32_t gi = 0u, ciA = 0u;                         // storage index of G's cell and of cell n
+            uint32_t dgx = 0u, dgy = 0u, dgz = 0u;              // the step per axis as an increment of the storage index
+            uint32_t ncross = 0u;
+            double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at the packet's frequency
+            uint32_t kq_sp = 0u;
+            const double2 *kq_row = s_kk;                       // s_kk + j
+            // Words of cells n .. n+kDepth-1, in registers.  (Measured against cp.async into a shared-memory ring with
+            // wait_group, which pipelines cleanly on one scoreboard: the ring costs 9 shared-memory wavefronts per step
+            // on a load/store data path that is the busiest unit of the SM here -- 5 % slower.)
+            unsigned long long cwr[kDepth];
+#pragma unroll
+            for (int i = 0; i < kDepth; ++i) cwr[i] = 0ull;
+            double tq[kDepth - 1];                              // queue between G and the physics: exit parameter and storage
+            uint32_t cq[kDepth - 1];                            // index of cells n+1 .. n+kDepth-2 (and of the cell G is in)
+#pragma unroll
+            for (int i = 0; i < kDepth - 1; ++i) { tq[i] = 0.0; cq[i] = 0u; }
             int nidle = 32;
-            unsigned long long cw = 0ull;                       // word of cell n
             const volatile unsigned long long *vpp = s_parp;
             const volatile uint32_t *vpi = s_pari;
             const unsigned long long *const cellw_r = reinterpret_cast<const unsigned long long *>(vpp[0]);
             long long *const lfx_r = reinterpret_cast<long long *>(vpp[1]);
-            const uint32_t ncp_r = vpi[0];
-#if MCRT_PIN >= 2
-            const int nbx_r = (int)vpi[1], nby_r = (int)vpi[2];
-#else
-            const int nbx_r = nbx, nby_r = nby;
-#endif
-#if MCRT_PIN >= 3
-            const uint32_t nx_r = vpi[3], ny_r = vpi[4], nz_r = vpi[5];
-            const int bsh_r = (int)vpi[6];
-#else
-            const uint32_t nx_r = (uint32_t)P.nx, ny_r = (uint32_t)P.ny, nz_r = (uint32_t)P.nz;
-            const int bsh_r = bsh;
-#endif
-            const uint32_t scratch = ncp_r + ((blockIdx.x * blockDim.x + threadIdx.x) & (uint32_t)(kLucyScratch - 1));   // this thread's word
+            const uint32_t px_r = vpi[5], pxy_r = vpi[6];
+            const uint32_t nf_r = vpi[7];
 
             for (;;) {
                 // ---- account for packets that stopped, refill idle lanes (batched: MCRT_SWAP_MIN lanes at a time)
                 {
-                    if (state == ST_JUMP || state == ST_INTERACT || state == ST_DONE) {
-                        // stopped in the walk below: write what the next phase needs into the slot
-                        SU(U_NCROSS, slot) = ncross;
-                        if (state == ST_DONE) {
-                            SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
-                        } else {
-                            SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SU(U_W0, slot) = xzA;
-                            if (state == ST_INTERACT) {
-                                SF(F_CW, slot) = __longlong_as_double((long long)cw);
-                                SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
-                            }
+                    if (state == ST_STOP) {
+                        // stopped in the walk below, which stored the flight's state in the slot; what kind of stop is
+                        // read off the cell word: a marker word (rho = +inf) is a cell outside the grid (bit 8) or the
+                        // first cell of a run of empty bricks, anything else an interaction in that cell
+                        const unsigned long long scw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        const bool mk = (uint32_t)(scw >> 32) == kMarkHi;
+                        state = mk ? (((uint32_t)scw & kOutFlag) ? ST_DONE : ST_JUMP) : ST_INTERACT;
+                        if (state == ST_DONE) SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                        else {
+                            SU(U_W0, slot) = index_to_packed(SU(U_W0, slot), px_r, pxy_r, P.inv_lpx, P.inv_lpxy);   // the walk stored the index
+                            if (state == ST_INTERACT) SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
                         }
                     }
                     mJ.add(state == ST_JUMP, slot);
@@ -643,15 +660,15 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // started: its slot is as the refill found it
                         // (its crossing count is still below the slot's)
                         if (state == ST_FLY && (int)(ncross - SU(U_NCROSS, slot)) >= 0) {
-                            cp_async_wait<0>();
+                            const unsigned long long wn = cwr[0];
                             SU(U_NCROSS, slot) = ncross;
-                            if (ciA == kOutCell) {     // cell n lies outside the grid: the packet has escaped
+                            if (wn == kOutWord) {      // cell n lies outside the grid: the packet has escaped
                                 SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
                                 state = ST_DONE;
                             } else {
                                 SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau;
-                                SF(F_CW, slot) = __longlong_as_double((long long)RING(r));
-                                SU(U_W0, slot) = xzA;
+                                SF(F_CW, slot) = __longlong_as_double((long long)wn);
+                                SU(U_W0, slot) = index_to_packed(ciA, px_r, pxy_r, P.inv_lpx, P.inv_lpxy);
                             }
                         }
                         mFly.add(state == ST_FLY, slot);
@@ -662,7 +679,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool take = state == ST_IDLE && k < mFly.count();
                     if (take) {
                         slot = mFly.nth(k);
-                        cp_async_wait<0>();                       // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
 #if MCRT_SLOT_IV
@@ -677,13 +693,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         const double t = SF(F_T, slot);
                         tau = SF(F_TAU, slot);
                         const uint32_t w0 = SU(U_W0, slot);
-                        j = (int)SU(U_W1, slot);
-                        ncross = SU(U_NCROSS, slot) - 1u;         // the no-op cell below counts itself
-                        gx = unpack_x(w0); gy = unpack_y(w0); gz = unpack_z(w0);
+                        const int j = (int)SU(U_W1, slot);
+                        ncross = SU(U_NCROSS, slot) - (uint32_t)(kDepth - 1);   // the no-op cells below count themselves
+                        const int gx = unpack_x(w0), gy = unpack_y(w0), gz = unpack_z(w0);
                         // the stored 1/u is +inf for a zero direction component: that axis never moves
-                        stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
-                        sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
-                        stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
+                        const int stx = isinf(ivx) ? 0 : (ivx > 0.0 ? 1 : -1);
+                        const int sty = isinf(ivy) ? 0 : (ivy > 0.0 ? 1 : -1);
+                        const int stz = isinf(ivz) ? 0 : (ivz > 0.0 ? 1 : -1);
                         tmx = mcrt::face_t(gx, stx, px, ivx);
                         tmy = mcrt::face_t(gy, sty, py, ivy);
                         tmz = mcrt::face_t(gz, stz, pz, ivz);
@@ -691,95 +707,101 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         fdx = stx ? (double)(gx + ((stx + 1) >> 1)) : CUDART_INF; shx = __double2hiint((double)stx);
                         fdy = sty ? (double)(gy + ((sty + 1) >> 1)) : CUDART_INF; shy = __double2hiint((double)sty);
                         fdz = stz ? (double)(gz + ((stz + 1) >> 1)) : CUDART_INF; shz = __double2hiint((double)stz);
-                        gcidx = cell_in_brick(brick_of(gx, gy, gz, nbx, nby, bsh), gx, gy, gz, bsh);
-                        // pipeline: one no-op cell (zero length, vacuum word; its zero tally goes to the lane's scratch
-                        // word, not to the packet's cell: the cells where packets start are the most contended ones),
-                        // then the packet's cell
-                        RING(r) = 0ull;
-                        RING((r + kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        tprev = t; tnA = t; ciA = scratch; xzA = w0;
-                        kq_sp = 0; kq = s_kk[j];
+                        gi = lin_index(gx, gy, gz, (int)px_r, (int)pxy_r);
+                        dgx = (uint32_t)stx; dgy = (uint32_t)(sty * (int)px_r); dgz = (uint32_t)(stz * (int)pxy_r);
+                        // pipeline: kDepth - 1 no-op cells (zero length, vacuum word: nothing is tallied), then the packet's
+                        // cell, in which G stands
+#pragma unroll
+                        for (int i = 0; i < kDepth - 1; ++i) cwr[i] = 0ull;
+                        cwr[kDepth - 1] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        tprev = t; tnA = t; ciA = 0u;
+#pragma unroll
+                        for (int i = 0; i < kDepth - 2; ++i) { tq[i] = t; cq[i] = 0u; }
+                        kq_row = s_kk + j;
+                        kq_sp = 0u; kq = kq_row[0];
                         state = ST_FLY;
                     }
                     mFly.remove(take, slot);
                     nidle = __popc(__ballot_sync(kFull, state == ST_IDLE));
                 }
                 // ---- the walk: a tight inner loop (nothing but the step, so that it stays in the instruction cache)
-                // until MCRT_SWAP_MIN more lanes have stopped
+                // until MCRT_SWAP_MIN more lanes have stopped.  kDepth cells per iteration, one per word in flight.
+                //
+                // No branch in a step: a divergent branch costs more here (branch resolution, reconvergence) than the
+                // work it skips, so every lane runs the whole step.  A lane that holds no flying packet leaves no
+                // trace: its G stands still and loads nothing, its physics works on whatever its registers
+                // hold and tallies nothing.  A lane whose packet stops stores the flight's state in its slot at once
+                // (predicated stores), so that nothing but `state` and `slot` has to survive until the next refill:
+                // every other update of the step is unconditional.
+                // Shared memory is touched only by the rare events of a step (stop, change of species): the step's
+                // two global accesses (cell word, tally) already keep the SM's load/store data path busy.
                 int nnot;
-                do {
-                const int rc = r;               // ring slot of cell n in this step
-                r = (r + kRingStep) & kRingMask;
-                {
-                    // One step per iteration: the loop (2 KB) fits the instruction cache next to the scheduler
-                    // (three steps per iteration measured 7 % slower).  No branch: a divergent branch costs more
-                    // here (branch resolution, reconvergence) than the work it skips, so every lane runs the whole
-                    // step and a lane that holds no flying packet leaves no trace: its G walks on stale
-                    // coordinates, it requests the marker word, adds 0 to its scratch word and keeps its packet's
-                    // registers (they are written to the slot by the block above).
-                    const bool fly = state == ST_FLY;
-                    cp_async_wait<1>();                               // the word of cell n has landed
-                    {
-                        const unsigned long long w = RING(rc);
-                        cw = fly ? w : cw;
-                    }
-                    // ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and requests
-                    // its word.  A G that has left the grid keeps stepping outwards (a straight line does not come
-                    // back) and requests the marker word.
-                    const uint32_t ciN = gcidx, xzN = pack_xyz(gx, gy, gz);
-                    const bool selx = (tmx <= tmy) && (tmx <= tmz);
-                    const bool sely = !selx && (tmy <= tmz);
-                    const bool selz = !selx && !sely;
-                    const double tnN = selx ? tmx : (sely ? tmy : tmz);
-                    gx += selx ? stx : 0;
-                    gy += sely ? sty : 0;
-                    gz += selz ? stz : 0;
-                    // parameter of the face through which the entered cell will be left (reading Q8): the face
-                    // coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'
-                    // f moves by its step, the others by 0, and all three t are recomputed: the same value for an
-                    // axis that did not move, so nothing has to be selected afterwards
-                    fdx += __hiloint2double(selx ? shx : 0, 0);
-                    fdy += __hiloint2double(sely ? shy : 0, 0);
-                    fdz += __hiloint2double(selz ? shz : 0, 0);
-                    tmx = (fdx - px) * ivx;
-                    tmy = (fdy - py) * ivy;
-                    tmz = (fdz - pz) * ivz;
-                    {
-                        const bool inside = fly & ((unsigned)gx < nx_r) & ((unsigned)gy < ny_r) & ((unsigned)gz < nz_r);
-                        // (an index computed from coordinates outside the grid is not used)
-                        const uint32_t cell = cell_in_brick(brick_of(gx, gy, gz, nbx_r, nby_r, bsh_r), gx, gy, gz, bsh_r);
-                        gcidx = inside ? cell : kOutCell;
-                        // a cell outside the grid requests the marker word behind the grid
-                        cp_async8(ring + ((rc + 2 * kRingStep) & kRingMask), cellw_r + (inside ? cell : ncp_r));
-                    }
-                    cp_async_commit();
-                    // ---- physics of cell n.  One exit for every kind of stop: the word of a cell in an empty brick
-                    // and the word requested for a cell outside the grid are both the marker word (bit 28; rho = 0,
-                    // so dtau = 0)
-                    const double ds = tnA - tprev;
-                    const double rho_c = cw_rho(cw);
-                    if (cw_species(cw) != kq_sp) {   // opacities of this species at the packet's frequency: kept in registers
-                        kq_sp = cw_species(cw);
-                        kq = s_kk[kq_sp * nf + j];
-                    }
-                    const double dtau = kq.x * rho_c * ds;            // tau_i = (kabs+ksca) h rho ds (Eq. 2)
-                    const bool marker = ((uint32_t)cw & (uint32_t)kJumpWord) != 0u;
-                    const bool stop = marker || dtau > tau;           // interaction inside this cell: equality leaves (Q5)
-                    const bool go = fly && !stop;
-                    // Marker word: cell n lies outside the grid (escape tally in the E phase) or starts a run of empty
-                    // bricks (J phase)
-                    if (fly && stop) state = marker ? (ciA == kOutCell ? ST_DONE : ST_JUMP) : ST_INTERACT;
-                    // S5: no branch around the RED: a vacuum cell (rho = 0) adds 0 to its tally, a lane that does not
-                    // step adds 0 to its scratch word
-                    lucy_add(lfx_r, go ? ciA : scratch, go ? kq.y * rho_c * ds : 0.0);
-                    if (go) {
-                        tau -= dtau;
-                        ndusty_acc += (__double2hiint(rho_c) != 0) ? 1u : 0u;   // rho > 0: its high word is not 0
-                        ncross++;
-                        tprev = tnA; tnA = tnN; ciA = ciN; xzA = xzN;
-                    }
+#define WALK_STEP(W)                                                                                                          \
+                {                                                                                                           \
+                    const bool fly = state == ST_FLY;                                                                       \
+                    const unsigned long long cw = W;                  /* the word of cell n (waits for its load) */        \
+                    /* ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and loads its  */ \
+                    /* word.  G stands still once its lane has stopped; until then it may run up to kGuard cells beyond  */ \
+                    /* the grid (the storage has that many guard cells on every side).                                   */ \
+                    const uint32_t ciN = gi;                                                                                \
+                    const bool selx = (tmx <= tmy) && (tmx <= tmz);                                                         \
+                    const bool sely = !selx && (tmy <= tmz);                                                                \
+                    const bool selz = !selx && !sely;                                                                       \
+                    const double tnN = selx ? tmx : (sely ? tmy : tmz);                                                     \
+                    gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                     \
+                    /* the load of cell n+kDepth replaces, in place, the word just read (lanes without a flying packet   */ \
+                    /* keep theirs): tied to W, so that no move has to wait for the load                                  */ \
+                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"         \
+                                 : "+l"(W) : "l"(cellw_r + gi), "r"((uint32_t)fly));                                       \
+                    /* parameter of the face through which the entered cell will be left (reading Q8): the face          */ \
+                    /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'   */ \
+                    /* f moves by its step, the others by 0, and all three t are recomputed: the same value for an axis  */ \
+                    /* that did not move, so nothing has to be selected afterwards                                       */ \
+                    fdx += __hiloint2double(selx ? shx : 0, 0);                                                             \
+                    fdy += __hiloint2double(sely ? shy : 0, 0);                                                             \
+                    fdz += __hiloint2double(selz ? shz : 0, 0);                                                             \
+                    tmx = (fdx - px) * ivx;                                                                                 \
+                    tmy = (fdy - py) * ivy;                                                                                 \
+                    tmz = (fdz - pz) * ivz;                                                                                 \
+                    /* ---- physics of cell n.  One test for every kind of stop: a marker word (cell in an empty brick,  */ \
+                    /* cell outside the grid) has rho = +inf, so dtau is +inf or (ds = 0) NaN                             */ \
+                    const double ds = tnA - tprev;                                                                          \
+                    const double rho_c = cw_rho(cw);                                                                        \
+                    if (cw_species(cw) != kq_sp) {   /* opacities of this species at the packet's frequency */              \
+                        kq_sp = cw_species(cw);                                                                             \
+                        kq = kq_row[kq_sp * nf_r];                                                                          \
+                    }                                                                                                       \
+                    const double dtau = kq.x * rho_c * ds;            /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */ \
+                    const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
+                    if (fly && stop) {                                                                                      \
+                        state = ST_STOP;                                                                                    \
+                        SU(U_NCROSS, slot) = ncross; SU(U_W0, slot) = ciA;                                                  \
+                        SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SF(F_CW, slot) = __longlong_as_double((long long)cw); \
+                    }                                                                                                       \
+                    /* S5: tally of a traversed dusty cell (a vacuum cell has nothing to add) */                           \
+                    {                                                                                                       \
+                        const unsigned long long q = lucy_round(kq.y * rho_c * ds);                                         \
+                        const bool go = fly && !stop;                                                                       \
+                        const uint32_t dusty = (go && __double2hiint(rho_c) != 0) ? 1u : 0u;                                \
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
+                                     ::"l"(lfx_r + ciA), "l"(q), "r"(dusty) : "memory");                                    \
+                        ndusty_acc += dusty;                                                                                \
+                    }                                                                                                       \
+                    tau -= dtau;                                                                                            \
+                    ncross++;                                                                                               \
+                    tprev = tnA;                                                                                            \
+                    if (kDepth == 2) { tnA = tnN; ciA = ciN; }                                                              \
+                    else {                                                                                                  \
+                        tnA = tq[0]; ciA = cq[0];                                                                           \
+                        _Pragma("unroll") for (int i = 0; i < kDepth - 3; ++i) { tq[i] = tq[i + 1]; cq[i] = cq[i + 1]; }    \
+                        tq[kDepth - 3 >= 0 ? kDepth - 3 : 0] = tnN; cq[kDepth - 3 >= 0 ? kDepth - 3 : 0] = ciN;             \
+                    }                                                                                                       \
                 }
+                do {
+#pragma unroll
+                    for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i])
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
+#undef WALK_STEP
             }
             __syncwarp();
         } else if (njmp > 0 && njmp >= nevt) {
@@ -840,7 +862,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 } else {
                     SU(U_W0, slot) = pack_xyz(ix, iy, iz);
                     if (!busy) {
-                        const uint32_t cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                        const uint32_t cidx = lin_index(ix, iy, iz, lpx, lpxy);
                         SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + cidx));
                     }
                 }
@@ -944,7 +966,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                     const double t = SF(F_T, slot), tau = SF(F_TAU, slot), ztype = SF(F_ZTYPE, slot);
                     cw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                    cidx = cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
+                    cidx = lin_index(ix, iy, iz, lpx, lpxy);
                     const double rho_c = cw_rho(cw);
                     sj = cw_species(cw) * nf + j;
                     const double2 kq = s_kk[sj];
@@ -1016,7 +1038,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     f = floor(py); iy = (py != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1);
                     f = floor(pz); iz = (pz != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1);
                     const uint32_t brick = brick_of(ix, iy, iz, nbx, nby, bsh);
-                    cidx = cell_in_brick(brick, ix, iy, iz, bsh);
+                    cidx = lin_index(ix, iy, iz, lpx, lpxy);
                     to_jump = brick_empty(s_m0, brick);
                     cw = to_jump ? 0ull : __ldg(P.cellw + cidx);
                     if (RECORD)
@@ -1052,7 +1074,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         }
     }
 #undef SF
-#undef RING
 #undef SU
     {   // dusty crossings stepped by this warp
         const uint32_t nd = __reduce_add_sync(kFull, ndusty_acc & 0xffffu), ndh = __reduce_add_sync(kFull, ndusty_acc >> 16);
@@ -1104,7 +1125,7 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
         const double rho_c = cw_rho(cw);
         const unsigned long long kc = kcnt[i];
         uint32_t m = 0u;
-        if (rho_c > 0.0) {
+        if (cw_dusty(cw)) {
             double kt;
             if (first_epoch) kt = (double)kc + 1.0;
             else {
@@ -1118,7 +1139,8 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
         }
         kprev[i] = kc;
         const uint32_t lo = (uint32_t)cw, nlo = (lo & 0xFF0000FFu) | (m << 8);
-        if (nlo != lo) reinterpret_cast<uint32_t *>(cellw + i)[0] = nlo;  // low word: species | tidx << 8 | rho bits 29-31
+        // low word: species | tidx << 8 | rho bits 29-31 (the words of vacuum and marker cells are never written)
+        if (nlo != lo && cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + i)[0] = nlo;
     }
     if (ovf) counters[CNT_OVERFLOW] = 1ull;
 }
@@ -1138,12 +1160,12 @@ __global__ void __launch_bounds__(256) k_sweep_update(unsigned long long *__rest
         const unsigned long long cw = cellw[i];
         const double rho_c = cw_rho(cw);
         uint32_t m = 0u;
-        if (rho_c > 0.0) {
+        if (cw_dusty(cw)) {
             const double e = from_lucy ? (double)lfx[i] * inv_fx : (double)kcnt[i];
             const double x = e * cellfac / rho_c;
             m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, x);
         }
-        reinterpret_cast<uint32_t *>(cellw + i)[0] = ((uint32_t)cw & 0xFF0000FFu) | (m << 8);
+        if (cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + i)[0] = ((uint32_t)cw & 0xFF0000FFu) | (m << 8);
         kcnt[i] = 0ull;
         kprev[i] = 0ull;
         lfx[i] = 0ll;
@@ -1196,41 +1218,32 @@ __global__ void __launch_bounds__(256) k_range_check(const long long *__restrict
 // ------------------------------------------------------------------------------------------------
 // layout kernels: canonical [nz][ny][nx] <-> brick-major
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ size_t brick_index(int ix, int iy, int iz, int nbx, int nby, int bsh)
-{
-    return cell_in_brick(brick_of(ix, iy, iz, nbx, nby, bsh), ix, iy, iz, bsh);
-}
-
 __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__restrict__ sp, unsigned long long *__restrict__ cellw,
-                            int nx, int ny, int nz, int nbx, int nby, int nbz, int bsh, int ns, unsigned long long *__restrict__ bad)
+                            int nx, int ny, int nz, int px, int pxy, size_t ncp, int ns, unsigned long long *__restrict__ bad)
 {
-    const size_t ncp = ((size_t)nbx * nby * nbz) << (3 * bsh);
-    const int m = (1 << bsh) - 1;
     for (size_t b = (size_t)blockIdx.x * blockDim.x + threadIdx.x; b < ncp; b += (size_t)gridDim.x * blockDim.x) {
-        const size_t brick = b >> (3 * bsh);
-        const int l = (int)(b & (((size_t)1 << (3 * bsh)) - 1));
-        const int bxi = (int)(brick % nbx), byi = (int)((brick / nbx) % nby), bzi = (int)(brick / ((size_t)nbx * nby));
-        const int ix = (bxi << bsh) + (l & m), iy = (byi << bsh) + ((l >> bsh) & m), iz = (bzi << bsh) + (l >> (2 * bsh));
-        unsigned long long cw = 0ull;
-        if (ix < nx && iy < ny && iz < nz) {
+        const int iz = (int)(b / (size_t)pxy) - kGuard;
+        const int rem = (int)(b % (size_t)pxy);
+        const int iy = rem / px - kGuard, ix = rem % px - kGuard;
+        unsigned long long cw = kOutWord;        // the guard shell: "outside the grid"
+        if ((unsigned)ix < (unsigned)nx && (unsigned)iy < (unsigned)ny && (unsigned)iz < (unsigned)nz) {
             const size_t i = ((size_t)iz * ny + iy) * nx + ix;
             const float r = rho[i];
             const uint32_t s = sp[i];
             if (!(r >= 0.0f) || isinf(r)) atomicAdd(&bad[0], 1ull);
             if (s >= (uint32_t)ns) atomicAdd(&bad[1], 1ull);
             // fp32 -> fp64 is exact and leaves the low 29 mantissa bits zero; -0 is stored as +0
-            const double rd = (r > 0.0f) ? (double)r : 0.0;
+            const double rd = (r > 0.0f && !isinf(r)) ? (double)r : 0.0;
             cw = ((unsigned long long)__double_as_longlong(rd) & kRhoMask) | (unsigned long long)(s & 0xffu);
         }
         cellw[b] = cw;
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) cellw[ncp] = kJumpWord;   // marker word behind the grid
 }
 
 // Vacuum mask of one level: bit of box (bx, by, bz) is set when all its in-grid cells have rho == 0.
 // Level 0 is built from the packed cells, level l > 0 from level l - 1 (4x4x4 children per box).
 __global__ void k_build_mask0(unsigned long long *__restrict__ cellw, uint32_t *__restrict__ m, int nx, int ny, int nz,
-                              int nbx, int nby, int sh, int mbx, int mby, int mbz)
+                              int px, int pxy, int sh, int mbx, int mby, int mbz)
 {
     const int nb = mbx * mby * mbz;
     for (int b = blockIdx.x * blockDim.x + threadIdx.x; b < nb; b += gridDim.x * blockDim.x) {
@@ -1241,14 +1254,14 @@ __global__ void k_build_mask0(unsigned long long *__restrict__ cellw, uint32_t *
         for (int z = z0; z < z1 && empty; ++z)
             for (int y = y0; y < y1 && empty; ++y)
                 for (int x = x0; x < x1; ++x)
-                    if (!cw_vacuum(cellw[brick_index(x, y, z, nbx, nby, sh)])) { empty = false; break; }
+                    if (!cw_vacuum(cellw[lin_index(x, y, z, px, pxy)])) { empty = false; break; }
         if (empty) {
             atomicOr(&m[b >> 5], 1u << (b & 31));
             // every cell word of an empty brick carries the marker bit: the cell walk sees it in the word it reads
             // anyway and needs no mask lookup
             for (int z = z0; z < z1; ++z)
                 for (int y = y0; y < y1; ++y)
-                    for (int x = x0; x < x1; ++x) cellw[brick_index(x, y, z, nbx, nby, sh)] |= kJumpWord;
+                    for (int x = x0; x < x1; ++x) cellw[lin_index(x, y, z, px, pxy)] |= kJumpWord;
         }
     }
 }
@@ -1336,12 +1349,12 @@ __device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int 
 __global__ void k_gather(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
                          const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
                          const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
-                         int nbx, int nby, int bsh, double xi, double inv_fx, double cellfac)
+                         int px, int pxy, double xi, double inv_fx, double cellfac)
 {
     const size_t nc = (size_t)nx * ny * nz;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
         const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
-        const size_t b = brick_index(ix, iy, iz, nbx, nby, bsh);
+        const size_t b = lin_index(ix, iy, iz, px, pxy);
         switch (what) {
         case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
         case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[b]; break;
@@ -1352,7 +1365,7 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
             const unsigned long long cw = cellw[b];
             const double rho_c = cw_rho(cw);
             float T = 0.0f;
-            if (rho_c > 0.0) {
+            if (cw_dusty(cw)) {
                 const double e = (what == G_TLUCY) ? (double)lfx[b] * inv_fx : (double)kcnt[b];
                 T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
             }
@@ -1440,7 +1453,7 @@ size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threa
 {
     return (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
            (size_t)(threads / 32) * 8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
-           (size_t)((mask0_words + 1) & ~1) * sizeof(uint32_t) + (size_t)kRing * threads * sizeof(unsigned long long);
+           (size_t)(MCRT_SMEM_MASK ? ((mask0_words + 1) & ~1) : 0) * sizeof(uint32_t);
 }
 
 // Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
@@ -1502,14 +1515,14 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     const size_t nc = (size_t)nx * ny * nz;
     const MaskGeom mg = mask_geom(nx, ny, nz);
     const size_t nbricks = (size_t)mg.nbx * mg.nby * mg.nbz;
-    const size_t ncp = nbricks << (3 * mg.msh);
+    const size_t ncp = (size_t)(nx + 2 * kGuard) * (ny + 2 * kGuard) * (nz + 2 * kGuard);
     size_t b = 0;
     auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
-    add((ncp + 1) * sizeof(uint2));      // cell words + marker word
+    add((ncp + 1) * sizeof(uint2));      // cell words
     add((size_t)mg.mwords * 4);          // vacuum mask
     add(nbricks * sizeof(uint4));        // empty boxes of the J phase
     add((size_t)(mg.nbx + 1) * (mg.nby + 1) * (mg.nbz + 1) * sizeof(int));   // summed-area scratch
-    add((ncp + kLucyScratch) * sizeof(long long));   // Lucy tally + scratch words (adds of lanes that do not step)
+    add(ncp * sizeof(long long));        // Lucy tally
     add(ncp * sizeof(long long));        // k
     add(ncp * sizeof(long long));        // k_prev
     add(nc * 8);                         // scratch (staging of inputs / outputs)
@@ -1533,8 +1546,8 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     if (!out) return fail(nullptr, MCRT_EINVAL, "out is NULL");
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be >= 1");
-    if (nx > 2048 || ny > 2048 || nz > 1024) return fail(nullptr, MCRT_EINVAL, "grid too large: nx, ny <= 2048 and nz <= 1024");
-    if ((size_t)nx * ny * nz > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
+    if (nx > 2040 || ny > 2040 || nz > 1016) return fail(nullptr, MCRT_EINVAL, "grid too large: nx, ny <= 2040 and nz <= 1016");
+    if ((size_t)(nx + 2 * kGuard) * (ny + 2 * kGuard) * (nz + 2 * kGuard) > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
     if (!(cell_size_cm > 0.0) || !isfinite(cell_size_cm)) return fail(nullptr, MCRT_EINVAL, "cell_size_cm must be > 0");
     if (!rho || !species) return fail(nullptr, MCRT_EINVAL, "rho / species is NULL");
     if (n_species < 1 || n_species > 255) return fail(nullptr, MCRT_EINVAL, "n_species must be in 1..255");
@@ -1551,7 +1564,8 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         c->nbx = g.nbx; c->nby = g.nby; c->nbz = g.nbz;
     }
     c->nc = (size_t)nx * ny * nz;
-    c->ncp = ((size_t)c->nbx * c->nby * c->nbz) << (3 * c->msh);
+    c->px = nx + 2 * kGuard; c->pxy = c->px * (ny + 2 * kGuard);
+    c->ncp = (size_t)c->pxy * (nz + 2 * kGuard);
     c->ws = (char *)workspace; c->ws_bytes = workspace_bytes; c->ws_owned_by_caller = workspace != nullptr;
     int rc;
 #define GC_TRY(expr)                                                       \
@@ -1568,11 +1582,11 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
             return MCRT_ECUDA;                                                                         \
         }                                                                                              \
     } while (0)
-    GC_TRY(ws_alloc(c, (void **)&c->cellw, (c->ncp + 1) * sizeof(uint2)));   // + the marker word
+    GC_TRY(ws_alloc(c, (void **)&c->cellw, (c->ncp + 1) * sizeof(uint2)));
     GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
     GC_TRY(ws_alloc(c, (void **)&c->vbox, (size_t)c->nbx * c->nby * c->nbz * sizeof(uint4)));
     GC_TRY(ws_alloc(c, (void **)&c->vsat, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int)));
-    GC_TRY(ws_alloc(c, (void **)&c->lfx, (c->ncp + kLucyScratch) * sizeof(long long)));
+    GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->scratch, c->nc * 8));
@@ -1588,13 +1602,12 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         d_rho = sr; d_sp = ss;
     }
     unsigned long long *bad = c->counters + CNT_N;
-    k_pack_grid<<<stream_grid(c->ncp), 256, 0, c->stream>>>(d_rho, d_sp, c->cellw, nx, ny, nz, c->nbx, c->nby, c->nbz,
-                                                           c->msh, n_species, bad);
+    k_pack_grid<<<stream_grid(c->ncp), 256, 0, c->stream>>>(d_rho, d_sp, c->cellw, nx, ny, nz, c->px, c->pxy, c->ncp, n_species, bad);
     GC_CUDA(cudaGetLastError());
     GC_CUDA(cudaMemsetAsync(c->vmask, 0, (size_t)c->mwords * 4, c->stream));
     {
         const size_t nbr = (size_t)c->nbx * c->nby * c->nbz;
-        k_build_mask0<<<stream_grid(nbr), 256, 0, c->stream>>>(c->cellw, c->vmask, nx, ny, nz, c->nbx, c->nby, c->msh, c->nbx,
+        k_build_mask0<<<stream_grid(nbr), 256, 0, c->stream>>>(c->cellw, c->vmask, nx, ny, nz, c->px, c->pxy, c->msh, c->nbx,
                                                              c->nby, c->nbz);
         GC_CUDA(cudaMemsetAsync(c->vsat, 0, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int), c->stream));
         k_sat_pass<<<stream_grid((size_t)c->nby * c->nbz), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 0);
@@ -1849,6 +1862,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
     P.nbx = c->nbx; P.nby = c->nby;
     P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords; P.ncp = (uint32_t)c->ncp;
+    P.lpx = c->px; P.lpxy = c->pxy; P.inv_lpx = 1.0 / (double)c->px; P.inv_lpxy = 1.0 / (double)c->pxy;
     P.px = c->pos[0]; P.py = c->pos[1]; P.pz = c->pos[2];
     P.seed_lo = (uint32_t)c->run.seed; P.seed_hi = (uint32_t)(c->run.seed >> 32);
 }
@@ -2138,7 +2152,7 @@ static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem wh
     void *dev = (where == MCRT_DEVICE) ? dst : c->scratch;
     const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
     k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, c->nT, c->nx,
-                                                       c->ny, c->nz, c->nbx, c->nby, c->msh, c->xi, ldexp(1.0, -c->fx), cellfac);
+                                                       c->ny, c->nz, c->px, c->pxy, c->xi, ldexp(1.0, -c->fx), cellfac);
     CUDA_TRY(c, cudaGetLastError());
     if (where == MCRT_HOST) {
         CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
