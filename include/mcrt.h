@@ -194,6 +194,20 @@ int mcrt_exchange_peer_sum(mcrt_ctx *ctx, int part_index, int n_parts, const mcr
 /* Convenience for parts that live in ONE process on ONE device (tests): begin + both phases + end for all. */
 int mcrt_exchange_local(mcrt_ctx *const *parts, int n_parts);
 
+/* Pure host helpers (no device needed), so that every part of a partitioned run derives the same schedule:
+ * mcrt_epoch_schedule writes the epoch sizes of a B&W run of n_packets (B0 / Bmax / growth as in mcrt_run_opts, 0 =
+ * default) to sizes_out[0 .. min(n, max_epochs) - 1] and the epoch count n to *n_epochs_out; mcrt_part_slice gives
+ * the slice [lo, hi) of an id range of `count` packets that part part_index of part_count transports
+ * (lo = floor(count * r / R), hi = floor(count * (r + 1) / R): the slices tile the range). */
+int mcrt_epoch_schedule(uint64_t n_packets, uint64_t epoch_B0, uint64_t epoch_Bmax, double epoch_growth,
+                        uint64_t *sizes_out, uint64_t max_epochs, uint64_t *n_epochs_out);
+int mcrt_part_slice(uint64_t count, int part_index, int part_count, uint64_t *lo_out, uint64_t *hi_out);
+
+/* Measurement aid (configurations whose arrays fit L2 are reported against a MEASURED L2 read
+ * bandwidth): streams a device buffer of `bytes` bytes `repeats` times with 16-byte loads from every SM and
+ * returns the best read rate in GB/s.  A buffer far below the L2 size measures L2, a far larger one HBM. */
+int mcrt_measure_read_bandwidth(size_t bytes, int repeats, double *gb_per_s_out);
+
 /* Synchronise and return the counters accumulated since the last reset. */
 int mcrt_get_stats(mcrt_ctx *ctx, mcrt_run_stats *stats_out);
 

@@ -23,7 +23,8 @@ MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP = 0, 1
 EXPORTS = [
     "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
     "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
-    "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
+    "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_epoch_schedule", "mcrt_part_slice",
+    "mcrt_measure_read_bandwidth", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
     "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
@@ -91,6 +92,9 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_exchange_end.argtypes = [vp]
     L.mcrt_exchange_peer_sum.argtypes = [vp, i, i, C.POINTER(Exchange), i]
     L.mcrt_exchange_local.argtypes = [C.POINTER(vp), i]
+    L.mcrt_epoch_schedule.argtypes = [u64, u64, u64, d, vp, u64, C.POINTER(u64)]
+    L.mcrt_part_slice.argtypes = [u64, i, i, C.POINTER(u64), C.POINTER(u64)]
+    L.mcrt_measure_read_bandwidth.argtypes = [C.c_size_t, i, C.POINTER(d)]
     L.mcrt_get_stats.argtypes = [vp, C.POINTER(RunStats)]
     L.mcrt_read.argtypes = [vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
@@ -215,6 +219,28 @@ def mcrt_exchange_peer_sum(ctx, part_index, views, phase):
 def mcrt_exchange_local(ctxs):
     arr = (C.c_void_p * len(ctxs))(*[c.value if isinstance(c, C.c_void_p) else c for c in ctxs])
     _check(load_library().mcrt_exchange_local(arr, len(ctxs)), ctxs[0])
+
+
+def mcrt_epoch_schedule(n_packets, epoch_B0=0, epoch_Bmax=0, epoch_growth=0.0):
+    n = C.c_uint64(0)
+    _check(load_library().mcrt_epoch_schedule(int(n_packets), int(epoch_B0), int(epoch_Bmax), float(epoch_growth), None, 0,
+                                              C.byref(n)))
+    sizes = np.zeros(n.value, np.uint64)
+    _check(load_library().mcrt_epoch_schedule(int(n_packets), int(epoch_B0), int(epoch_Bmax), float(epoch_growth), _ptr(sizes),
+                                              n.value, C.byref(n)))
+    return sizes
+
+
+def mcrt_part_slice(count, part_index, part_count):
+    lo, hi = C.c_uint64(0), C.c_uint64(0)
+    _check(load_library().mcrt_part_slice(int(count), int(part_index), int(part_count), C.byref(lo), C.byref(hi)))
+    return lo.value, hi.value
+
+
+def mcrt_measure_read_bandwidth(nbytes, repeats=10) -> float:
+    g = C.c_double(0.0)
+    _check(load_library().mcrt_measure_read_bandwidth(int(nbytes), int(repeats), C.byref(g)))
+    return g.value
 
 
 def mcrt_get_stats(ctx):

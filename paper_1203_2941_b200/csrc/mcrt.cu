@@ -1387,6 +1387,23 @@ __global__ void k_sed(double *__restrict__ out, const unsigned long long *__rest
     }
 }
 
+// read-bandwidth probe: every thread sums 16-byte words of a buffer with a grid stride, eight loads in flight
+__global__ void __launch_bounds__(512) k_read_probe(const uint4 *__restrict__ buf, size_t n16, unsigned long long *__restrict__ sink)
+{
+    unsigned long long acc = 0ull;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + 7 * stride < n16; i += 8 * stride) {
+        uint4 v[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k] = __ldcg(buf + i + k * stride);   // L2, not L1: what a resident grid's arrays see
+#pragma unroll
+        for (int k = 0; k < 8; ++k) acc += (unsigned long long)(v[k].x ^ v[k].y) + (unsigned long long)(v[k].z ^ v[k].w);
+    }
+    for (; i < n16; i += stride) { const uint4 v = __ldcg(buf + i); acc += (unsigned long long)(v.x ^ v.y) + (unsigned long long)(v.z ^ v.w); }
+    if (acc == 0x123456789abcdefull) sink[0] = acc;   // keeps the loads alive
+}
+
 __global__ void k_traj_math_test(const double *__restrict__ z, double *__restrict__ out, unsigned long long n)
 {
     const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -1875,6 +1892,80 @@ static void part_slice(const mcrt_run_opts &o, uint64_t count, uint64_t *lo, uin
     *hi = (uint64_t)(((unsigned __int128)count * (r + 1)) / R);
 }
 
+// epoch schedule (reading Q19): B0 doubling (or growing by `growth`) up to Bmax
+static void schedule_defaults(uint64_t n_packets, uint64_t *B0, uint64_t *Bmax, double *growth)
+{
+    if (*B0 == 0) { *B0 = 256; while (*B0 * 2 <= n_packets / 256) *B0 *= 2; }
+    if (*Bmax == 0) *Bmax = (uint64_t)1 << 22;
+    if (*Bmax < *B0) *Bmax = *B0;
+    if (*growth == 0.0) *growth = 2.0;
+}
+static uint64_t next_epoch_size(uint64_t Bnom, uint64_t Bmax, double growth)
+{
+    // B_{e+1} = min(floor(B_e * growth), Bmax), never shrinking
+    const double nb = floor((double)Bnom * growth);
+    uint64_t nn = nb >= 1.8e19 ? Bmax : (uint64_t)nb;
+    if (nn < Bnom) nn = Bnom;
+    return nn > Bmax ? Bmax : nn;
+}
+
+int mcrt_epoch_schedule(uint64_t n_packets, uint64_t epoch_B0, uint64_t epoch_Bmax, double epoch_growth, uint64_t *sizes_out,
+                        uint64_t max_epochs, uint64_t *n_epochs_out)
+{
+    if (n_packets < 1 || !n_epochs_out || (epoch_growth != 0.0 && !(epoch_growth >= 1.0))) return MCRT_EINVAL;
+    schedule_defaults(n_packets, &epoch_B0, &epoch_Bmax, &epoch_growth);
+    uint64_t done = 0, Bnom = epoch_B0, e = 0;
+    while (done < n_packets) {
+        const uint64_t Be = (n_packets - done < Bnom) ? n_packets - done : Bnom;
+        if (sizes_out && e < max_epochs) sizes_out[e] = Be;
+        done += Be; ++e;
+        Bnom = next_epoch_size(Bnom, epoch_Bmax, epoch_growth);
+    }
+    *n_epochs_out = e;
+    return MCRT_OK;
+}
+
+int mcrt_part_slice(uint64_t count, int part_index, int part_count, uint64_t *lo_out, uint64_t *hi_out)
+{
+    if (part_count < 1 || part_index < 0 || part_index >= part_count || !lo_out || !hi_out) return MCRT_EINVAL;
+    *lo_out = (uint64_t)(((unsigned __int128)count * (uint64_t)part_index) / (uint64_t)part_count);
+    *hi_out = (uint64_t)(((unsigned __int128)count * ((uint64_t)part_index + 1)) / (uint64_t)part_count);
+    return MCRT_OK;
+}
+
+int mcrt_measure_read_bandwidth(size_t bytes, int repeats, double *gb_per_s_out)
+{
+    if (!gb_per_s_out || bytes < 4096 || repeats < 1) return MCRT_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) return fail(nullptr, MCRT_ECUDA, "no CUDA device");
+    void *buf = nullptr; unsigned long long *sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    const size_t n16 = bytes / 16;
+    cudaError_t err = cudaMalloc(&buf, n16 * 16);
+    if (err == cudaSuccess) err = cudaMalloc((void **)&sink, 8);
+    if (err == cudaSuccess) err = cudaMemset(buf, 1, n16 * 16);
+    if (err == cudaSuccess) err = cudaEventCreate(&e0);
+    if (err == cudaSuccess) err = cudaEventCreate(&e1);
+    int nsm = 148;
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+    double best = 0.0;
+    for (int r = 0; err == cudaSuccess && r < repeats + 2; ++r) {     // two warm-up passes
+        cudaEventRecord(e0);
+        k_read_probe<<<nsm * 4, 512>>>((const uint4 *)buf, n16, sink);
+        cudaEventRecord(e1);
+        err = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (err == cudaSuccess && r >= 2 && ms > 0.f) { const double g = (double)(n16 * 16) / (ms * 1e-3) / 1e9; if (g > best) best = g; }
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    cudaFree(buf); cudaFree(sink);
+    if (err != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(err));
+    *gb_per_s_out = best;
+    return MCRT_OK;
+}
+
 int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_run_opts *opts)
 {
     if (!c) return MCRT_EINVAL;
@@ -1950,9 +2041,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     R.o = o; R.n = n_packets; R.seed = seed; R.done = 0; R.Bprev = 0; R.e = 0; R.sweep = 0; R.finished = false;
     R.growth = o.epoch_growth;
     uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
-    if (B0 == 0) { B0 = 256; while (B0 * 2 <= n_packets / 256) B0 *= 2; }
-    if (Bmax == 0) Bmax = (uint64_t)1 << 22;
-    if (Bmax < B0) Bmax = B0;
+    schedule_defaults(n_packets, &B0, &Bmax, &R.growth);
     R.Bnom = B0; R.Bmax = Bmax;
     c->need_exchange = false; c->exchange_open = false;
     R.active = true;
@@ -1993,12 +2082,7 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         c->launches += P.count ? 2 : 1;
         c->epochs++;
         R.done += Be; R.Bprev = Be;
-        {   // B_{e+1} = min(floor(B_e * growth), Bmax), never shrinking
-            const double nb = floor((double)R.Bnom * R.growth);
-            uint64_t nn = nb >= 1.8e19 ? R.Bmax : (uint64_t)nb;
-            if (nn < R.Bnom) nn = R.Bnom;
-            R.Bnom = nn > R.Bmax ? R.Bmax : nn;
-        }
+        R.Bnom = next_epoch_size(R.Bnom, R.Bmax, R.growth);
         ++R.e;
         R.finished = R.done >= R.n;
     } else {

@@ -542,3 +542,22 @@ def test_sed_read_to_host_on_a_tiny_grid(B, orc):
         assert st[key] == ro[key] == rg[key], key
     assert st["overflow"] == 0
     c.close()
+
+
+@pytest.mark.parametrize("mode", ["p2p", "allreduce"])
+def test_partitioned_run_across_processes(B, mode):
+    """Two processes (torch.distributed.run, gloo) sharing this GPU, one context each: the exchange over CUDA-IPC
+    mapped peer memory (mcrt_exchange_peer_sum) and the all_reduce path of paper_1203_2941_b200/multi.py both give
+    the unpartitioned run's integers (tests/mp_partition_worker.py)."""
+    import socket
+    import subprocess
+    import sys
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    worker = os.path.join(os.path.dirname(__file__), "mp_partition_worker.py")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", str(port), worker, mode],
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "PARTITION_OK" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])

@@ -1,5 +1,6 @@
-"""N > 1 path of bench.py on CPU: two gloo ranks, the whole-job reduction (time = max over ranks, units summed)
-and the per-rank replica seeds (independent replicas, no data-path collective)."""
+"""N > 1 path on CPU: two gloo ranks.  bench.py's whole-job reduction (time = max over ranks), and the partition
+arithmetic of a run shared by several GPUs: with the library's own host
+helpers every rank derives the same epoch schedule and the ranks' slices tile every epoch's packet ids."""
 import os
 import socket
 import subprocess
@@ -19,7 +20,23 @@ assert ms == 15.0, ms
 assert counts == [300.0, 14.0, 1.0], counts
 seeds = [None] * world
 dist.all_gather_object(seeds, bench.replica_seed(4, rank))
-assert seeds == [4, 1004] and len(set(seeds)) == world
+assert seeds == [4, 4]            # ONE run: every rank uses the same seed, packet ids tell the packets apart
+# partition arithmetic (pure host functions of the CUDA library): every epoch's ids are tiled by the ranks' slices
+from paper_1203_2941_b200 import binding as B
+for n, b0, bmax, growth in ((100001, 0, 0, 0.0), (10**8, 0, 0, 0.0), (5000, 100, 700, 1.5), (7, 0, 0, 0.0)):
+    sizes = B.mcrt_epoch_schedule(n, b0, bmax, growth)
+    assert int(sizes.sum()) == n and (growth or all(int(sizes[i + 1]) in (int(sizes[i]) * 2, int(sizes[i]), n - int(sizes[:i + 1].sum())) for i in range(len(sizes) - 1)))
+    mine = [B.mcrt_part_slice(int(be), rank, world) for be in sizes]
+    both = [None] * world
+    dist.all_gather_object(both, mine)
+    first = 0
+    for e, be in enumerate(sizes):
+        lo0, hi0 = both[0][e]; lo1, hi1 = both[1][e]
+        assert lo0 == 0 and hi0 == lo1 and hi1 == int(be), (e, both[0][e], both[1][e])   # the slices tile [0, B_e)
+        assert abs((hi0 - lo0) - (hi1 - lo1)) <= 1                                       # and are balanced
+        first += int(be)
+    assert first == n
+assert B.mcrt_epoch_schedule(10**8)[0] == 2**18 and int(B.mcrt_epoch_schedule(10**8).max()) == 2**22
 # the reference arm prints on rank 0 only
 dist.barrier()
 dist.destroy_process_group()
