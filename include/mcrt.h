@@ -78,6 +78,11 @@ typedef struct {
     double epoch_growth;       /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2.0; must be >= 1 */
     int32_t part_index;        /* partitioned run (packets are independent): this context transports */
     int32_t part_count;        /* slice part_index of part_count of EVERY epoch's id range; 0 or 1 = the whole run */
+    int32_t walk_words;        /* launch tuning (results never depend on it): how the cell walk keeps its cell words
+                                  in flight.  0 = auto (= 1), 1 = in registers, 2 = cp.async ring in shared memory
+                                  (never measured faster; kept for such measurements) */
+    int32_t no_hot_cells;      /* launch tuning: 1 = do not keep per-CTA copies of the tallies of the cells around the
+                                  source (default 0: kept; the sums are integers, so results do not depend on it) */
 } mcrt_run_opts;
 
 /* Counters of the runs since the last reset (all exact integers). */
@@ -119,7 +124,7 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
  *             256-byte alignment required.  The library sub-allocates from it in call order (grid
  *             here, tables in mcrt_dust_tables, histograms and digests at the first mcrt_run that
  *             needs them) and returns MCRT_ENOMEM when it runs out; size it with mcrt_workspace_bytes.
- *  nx, ny <= 2040, nz <= 1016 and at most 2^31 cells with the guard shell (cell coordinates are carried packed in 32 bits).
+ *  nx, ny <= 2040, nz <= 1016 and at most 2^30 cells with the guard shell (cell coordinates are carried packed in 32 bits).
  * The grid is re-laid out on the device into bricks of packed 8-byte cell words (4x4x4 cells up to 256^3,
  * 8x8x8 up to 512^3, ...); a bit mask of the bricks without dust and, for each of them, a large box of empty
  * bricks around it are built here as well (they let packets cross vacuum without touching memory). */

@@ -15,6 +15,7 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -34,6 +35,7 @@ constexpr double kLightC = 2.99792458e10;     // cm s^-1
 constexpr double kFourPi = 12.566370614359172953850573533118;
 
 constexpr unsigned kFull = 0xffffffffu;
+constexpr int kHot = 511;            // most hot cells around the source (see cw_hot)
 
 enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4, ST_STOP = 5 };
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
@@ -57,6 +59,12 @@ struct mcrt_ctx {
     int nbx = 0, nby = 0, nbz = 0;   // bricks per axis
     size_t nc = 0, ncp = 0;          // cells, cells of the padded storage (guard shell included)
     int px = 0, pxy = 0;             // row and plane pitch of the padded storage
+    unsigned long long n_dusty = 0;  // cells with rho > 0
+    uint32_t *d_hot_idx = nullptr;   // [kHot + 1] storage indices of the hot cells
+    int n_hot = 0, hot_max = 31;
+    uint32_t hot_shift = 24, hot_mask = 31, tidx_mask = 0xffffu;
+    std::vector<uint32_t> hot_idx;   // [n_hot + 1]
+    size_t l2_bytes = 126u << 20;
     double h = 0.0;
     // workspace (bump allocator)
     char *ws = nullptr;
@@ -100,6 +108,8 @@ struct mcrt_ctx {
         size_t smem = 0;
         double cellfac = 0.0, prev_cellfac = 0.0, growth = 2.0;
         bool finished = false;            // every step has been issued
+        bool ringw = false;               // walk variant of this run
+        bool hot = false;                 // hot cells tallied per CTA
     } run;
     bool need_exchange = false;           // partitioned run: a step's tallies are still per-part
     bool exchange_open = false, exchange_full = false;
@@ -302,15 +312,47 @@ __device__ __forceinline__ unsigned long long event_word(int type, int j, unsign
 // One 8-byte load per crossing serves S4, S5, S6 and S9, and the density needs no fp32->fp64 conversion.
 // ------------------------------------------------------------------------------------------------
 constexpr unsigned long long kRhoMask = 0xFFFFFFFFE0000000ull;
-#ifndef MCRT_DEPTH
-#define MCRT_DEPTH 2                // cell words in flight per lane of the walk (the geometry runs this many cells ahead)
+// kCS = stride of the cell-word array and of the Lucy-tally array in 8-byte words.  1: two separate arrays (default).
+// 2: one 16-byte record per cell, so that the walk's load of a cell and its tally add two steps later touch the same
+// 32-byte sector.  Measured (profiles/r02_experiments.md): disk256 +17 %, but torus256 -15 %, torus512 -18 %,
+// shell128 -61 % -- a RED into the sector a cell word lives in keeps evicting it from L1 and serialises with its
+// reads in L2, which costs far more where cells are revisited than the saved DRAM sector gains where they are not.
+#ifndef MCRT_PITCH_ALIGN
+#define MCRT_PITCH_ALIGN 1            // the row pitch of the padded storage is a multiple of this many cells
 #endif
-constexpr int kDepth = MCRT_DEPTH;
-constexpr int kGuard = kDepth + 1;  // guard cells around the grid in the padded storage (see "Storage order")
+#ifndef MCRT_CELL_STRIDE
+#define MCRT_CELL_STRIDE 1
+#endif
+constexpr int kCS = MCRT_CELL_STRIDE;
+// The walk keeps DEPTH cell words in flight per lane (its geometry runs that many cells ahead of the physics), in
+// one of two ways, chosen per grid at run time (mcrt_run_opts.walk_words):
+//   registers (kDepthReg = 2): fewest load/store wavefronts -- for grids whose dusty cells mostly hit L2;
+//   a cp.async ring in shared memory (kDepthRing, compile-time): the groups of a thread complete in order, so "all
+//   but the N newest have landed" is one wait on one scoreboard whatever N is (plain loads cannot be pipelined deeper
+//   than ptxas has scoreboards to spare: it gave both register loads the same one).  Measured at depth 2, 3 and 4 on
+//   all five workloads (profiles/r02_experiments.md): never faster than the registers, not even on the grids that
+//   wait for DRAM (disk256, torus512) -- their limit is the rate of scattered 32-byte DRAM sectors, not latency.
+//   Kept selectable for such measurements; auto = registers.
+#ifndef MCRT_DEPTH
+#define MCRT_DEPTH 2
+#endif
+#ifndef MCRT_RING_DEPTH
+#define MCRT_RING_DEPTH 2
+#endif
+constexpr int kDepthReg = MCRT_DEPTH, kDepthRing = MCRT_RING_DEPTH;
+constexpr int kGuard = (kDepthReg > kDepthRing ? kDepthReg : kDepthRing) + 1;  // guard cells around the grid (see "Storage order")
+constexpr int kRing = (kDepthRing + 1 <= 4) ? 4 : 8;   // ring slots per thread (cells n .. n+kDepthRing), a power of two
 
 __device__ __forceinline__ double cw_rho(unsigned long long cw) { return __longlong_as_double((long long)(cw & kRhoMask)); }
 __device__ __forceinline__ int cw_species(unsigned long long cw) { return (int)((unsigned)cw & 0xffu); }
-__device__ __forceinline__ int cw_tidx(unsigned long long cw) { return (int)(((unsigned)cw >> 8) & 0xffffu); }
+__device__ __forceinline__ int cw_tidx(unsigned long long cw, uint32_t tmask) { return (int)(((unsigned)cw >> 8) & tmask); }
+// Hot cells (north_star item 5; "local copies"): every packet starts in the few cells around the source,
+// so their tallies are same-address atomics from every SM at once, which one L2 slice serialises.  The dusty cells
+// nearest to the source are numbered 1, 2, ... in the bits of their cell word between the temperature index and the
+// density (mcrt_source: bits 20-28, 511 cells, when the temperature grid has at most 4096 points; else bits 24-28,
+// 31 cells) and tallied in a copy per CTA in shared memory, flushed with one atomic per CTA at the end of a launch.
+// Integer adds: the result is the same.
+__device__ __forceinline__ uint32_t cw_hot(unsigned long long cw, uint32_t shift, uint32_t mask) { return ((uint32_t)cw >> shift) & mask; }
 __device__ __forceinline__ bool cw_vacuum(unsigned long long cw) { return (unsigned)(cw >> 32) == 0u; }  // rho == +0
 // a cell that holds dust: 0 < rho < +inf (the cells of an empty brick carry the marker density +inf)
 __device__ __forceinline__ bool cw_dusty(unsigned long long cw) { return (unsigned)(cw >> 32) - 1u < 0x7FEFFFFFu; }
@@ -335,6 +377,9 @@ struct TransportParams {
     int nx, ny, nz, ns, nf, nT, ndir;
     int nbx, nby;       // bricks per axis
     uint32_t ncp;       // padded cell count
+    const uint32_t *__restrict__ hot_idx;   // [kHot + 1] storage index of hot cell number i (entry 0 unused)
+    uint32_t hot_shift, hot_mask, tidx_mask;   // fields of the cell word's low half: species 0-7 | T index | hot number | rho 29-31
+    int n_hot;
     int lpx, lpxy;      // row and plane pitch of the padded storage
     double inv_lpx, inv_lpxy;
     int bsh;            // log2 of the brick edge
@@ -379,11 +424,15 @@ __device__ __forceinline__ unsigned long long lucy_round(double x)
     const double y = x + 6755399441055744.0;
     return ((unsigned long long)(uint32_t)(__double2hiint(y) - 0x43380000) << 32) | (uint32_t)__double2loint(y);
 }
+__device__ __forceinline__ void lucy_add_raw(long long *__restrict__ lfx, uint32_t cidx, unsigned long long q)
+{
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + (size_t)kCS * cidx), "l"(q) : "memory");
+}
 __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
 {
     const unsigned long long q = lucy_round(x);
     // (explicitly global: a pointer that went through shared memory has lost its address space)
-    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + cidx), "l"(q) : "memory");
+    asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + (size_t)kCS * cidx), "l"(q) : "memory");
 }
 
 // Warp aggregation of these adds (__match_any_sync + __reduce_add_sync per group) was measured slower everywhere:
@@ -531,9 +580,32 @@ struct SlotSet {
     }
 };
 
-template <bool RECORD>
+// 8-byte asynchronous copy global -> shared (LDGSTS), per-thread groups
+__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
+{
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+// 64-bit add into a per-CTA hot-cell tally kept as two 32-bit limbs (native shared atomics; a 64-bit one is a CAS
+// loop): the carry out of the low limb goes into the high limb's add.  The limbs are put together at the flush.
+__device__ __forceinline__ void hot_add(unsigned int *lo, unsigned int *hi, uint32_t id, unsigned long long q)
+{
+    const unsigned int ql = (unsigned int)q, old = atomicAdd(&lo[id], ql);
+    const unsigned int carry = (old + ql < old) ? 1u : 0u;
+    const unsigned int qh = (unsigned int)(q >> 32) + carry;
+    if (qh) atomicAdd(&hi[id], qh);
+}
+
+template <bool RECORD, bool RINGW, bool HOT>
 __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const TransportParams P)
 {
+    __shared__ unsigned int s_hot_lo[HOT ? kHot + 1 : 1], s_hot_hi[HOT ? kHot + 1 : 1], s_hot_k[HOT ? kHot + 1 : 1];   // per-CTA tallies of the hot cells (64-bit as two limbs)
+    if (HOT) for (int i = threadIdx.x; i <= kHot; i += blockDim.x) { s_hot_lo[i] = 0u; s_hot_hi[i] = 0u; s_hot_k[i] = 0u; }
+    constexpr int kDepth = RINGW ? kDepthRing : kDepthReg;
     extern __shared__ double2 smem_d2[];
     const int nsf = P.ns * P.nf;
     const int nwarps = blockDim.x >> 5;
@@ -550,6 +622,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     uint32_t *s_m0x = s_hist + nhist;        // level-0 vacuum mask (one bit per brick)
     const int mw_smem = MCRT_SMEM_MASK ? P.mwords : 0;
     const uint32_t *s_m0 = MCRT_SMEM_MASK ? s_m0x : P.vmask;
+    // cell-word ring (RINGW): slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
+    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0x + ((mw_smem + 1) & ~1));
+    char *ring = reinterpret_cast<char *>(s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u));
+    constexpr int kRingStep = 32 * 8, kRingMask = (kRing - 1) * kRingStep;   // ring slots as byte offsets 0, 256, 512, ...
+#define RING(off) (*reinterpret_cast<volatile unsigned long long *>(ring + (off)))
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -560,6 +637,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
     for (int i = threadIdx.x; i < mw_smem; i += blockDim.x) s_m0x[i] = P.vmask[i];
     for (int i = threadIdx.x; i < 8 * nwarps; i += blockDim.x) s_cnt[i] = 0ull;   // eight counters per warp
+    if (RINGW) for (int i = threadIdx.x; i < kRing * (int)blockDim.x; i += blockDim.x) s_ring[i] = 0ull;   // every lane reads its ring in every step
     // Kernel parameters the walk loop uses, parked in shared memory: the S phase reads them into registers through
     // a volatile pointer, so that they stay there (left to itself the compiler reloads a dozen of them from the
     // constant bank in every iteration of the loop and waits for them)
@@ -615,12 +693,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at the packet's frequency
             uint32_t kq_sp = 0u;
             const double2 *kq_row = s_kk;                       // s_kk + j
-            // Words of cells n .. n+kDepth-1, in registers.  (Measured against cp.async into a shared-memory ring with
-            // wait_group, which pipelines cleanly on one scoreboard: the ring costs 9 shared-memory wavefronts per step
-            // on a load/store data path that is the busiest unit of the SM here -- 5 % slower.)
+            // words of cells n .. n+kDepth-1: in registers, or in the ring (slot r = cell n; the same r in every lane)
             unsigned long long cwr[kDepth];
 #pragma unroll
             for (int i = 0; i < kDepth; ++i) cwr[i] = 0ull;
+            int r = 0;
             double tq[kDepth - 1];                              // queue between G and the physics: exit parameter and storage
             uint32_t cq[kDepth - 1];                            // index of cells n+1 .. n+kDepth-2 (and of the cell G is in)
 #pragma unroll
@@ -660,7 +737,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // started: its slot is as the refill found it
                         // (its crossing count is still below the slot's)
                         if (state == ST_FLY && (int)(ncross - SU(U_NCROSS, slot)) >= 0) {
-                            const unsigned long long wn = cwr[0];
+                            if (RINGW) cp_async_wait<0>();
+                            const unsigned long long wn = RINGW ? RING(r) : cwr[0];
                             SU(U_NCROSS, slot) = ncross;
                             if (wn == kOutWord) {      // cell n lies outside the grid: the packet has escaped
                                 SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
@@ -679,6 +757,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool take = state == ST_IDLE && k < mFly.count();
                     if (take) {
                         slot = mFly.nth(k);
+                        if (RINGW) cp_async_wait<0>();            // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
 #if MCRT_SLOT_IV
@@ -712,8 +791,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // pipeline: kDepth - 1 no-op cells (zero length, vacuum word: nothing is tallied), then the packet's
                         // cell, in which G stands
 #pragma unroll
-                        for (int i = 0; i < kDepth - 1; ++i) cwr[i] = 0ull;
-                        cwr[kDepth - 1] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        for (int i = 0; i < kDepth - 1; ++i) {
+                            if (RINGW) RING((r + i * kRingStep) & kRingMask) = 0ull; else cwr[i] = 0ull;
+                        }
+                        if (RINGW) RING((r + (kDepth - 1) * kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        else cwr[kDepth - 1] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                         tprev = t; tnA = t; ciA = 0u;
 #pragma unroll
                         for (int i = 0; i < kDepth - 2; ++i) { tq[i] = t; cq[i] = 0u; }
@@ -736,10 +818,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // Shared memory is touched only by the rare events of a step (stop, change of species): the step's
                 // two global accesses (cell word, tally) already keep the SM's load/store data path busy.
                 int nnot;
-#define WALK_STEP(W)                                                                                                          \
+#define WALK_STEP(W, RC)                                                                                                      \
                 {                                                                                                           \
                     const bool fly = state == ST_FLY;                                                                       \
-                    const unsigned long long cw = W;                  /* the word of cell n (waits for its load) */        \
+                    if (RINGW) cp_async_wait<kDepth - 1>();           /* the word of cell n has landed */                   \
+                    const unsigned long long cw = RINGW ? RING(RC) : W;                                                     \
                     /* ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and loads its  */ \
                     /* word.  G stands still once its lane has stopped; until then it may run up to kGuard cells beyond  */ \
                     /* the grid (the storage has that many guard cells on every side).                                   */ \
@@ -751,8 +834,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                     \
                     /* the load of cell n+kDepth replaces, in place, the word just read (lanes without a flying packet   */ \
                     /* keep theirs): tied to W, so that no move has to wait for the load                                  */ \
-                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"         \
-                                 : "+l"(W) : "l"(cellw_r + gi), "r"((uint32_t)fly));                                       \
+                    if (RINGW) {                                                                                            \
+                        if (fly) cp_async8(ring + (((RC) + kDepth * kRingStep) & kRingMask), cellw_r + kCS * gi);               \
+                        cp_async_commit();                                                                                  \
+                    } else                                                                                                  \
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"     \
+                                     : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly));                             \
                     /* parameter of the face through which the entered cell will be left (reading Q8): the face          */ \
                     /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'   */ \
                     /* f moves by its step, the others by 0, and all three t are recomputed: the same value for an axis  */ \
@@ -783,8 +870,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         const unsigned long long q = lucy_round(kq.y * rho_c * ds);                                         \
                         const bool go = fly && !stop;                                                                       \
                         const uint32_t dusty = (go && __double2hiint(rho_c) != 0) ? 1u : 0u;                                \
+                        const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;   /* tallied in the CTA's own copy */ \
+                        const uint32_t cold = (dusty && hid == 0u) ? 1u : 0u;                                               \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
-                                     ::"l"(lfx_r + ciA), "l"(q), "r"(dusty) : "memory");                                    \
+                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"(HOT ? cold : dusty) : "memory");                 \
+                        if (HOT && __any_sync(kFull, dusty && hid != 0u)) {                                                 \
+                            if (dusty && hid != 0u) hot_add(s_hot_lo, s_hot_hi, hid, q);                                    \
+                        }                                                                                                   \
                         ndusty_acc += dusty;                                                                                \
                     }                                                                                                       \
                     tau -= dtau;                                                                                            \
@@ -798,8 +890,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }                                                                                                       \
                 }
                 do {
+                    if (RINGW) {
+                        WALK_STEP(cwr[0], r)
+                        WALK_STEP(cwr[0], (r + kRingStep) & kRingMask)
+                        r = (r + 2 * kRingStep) & kRingMask;
+                    } else {
 #pragma unroll
-                    for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i])
+                        for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i], 0)
+                    }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
 #undef WALK_STEP
             }
@@ -863,7 +961,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     SU(U_W0, slot) = pack_xyz(ix, iy, iz);
                     if (!busy) {
                         const uint32_t cidx = lin_index(ix, iy, iz, lpx, lpxy);
-                        SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + cidx));
+                        SF(F_CW, slot) = __longlong_as_double((long long)__ldg(P.cellw + (size_t)kCS * cidx));
                     }
                 }
             }
@@ -972,7 +1070,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double2 kq = s_kk[sj];
                     const double kk = kq.x * rho_c;
                     const double sint = tau / kk;
-                    lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
+                    const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;
+                    if (hid) hot_add(s_hot_lo, s_hot_hi, hid, lucy_round(kq.y * rho_c * sint));
+                    else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
                     const double tint = t + sint;
                     double q;
                     q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
@@ -987,10 +1087,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                        atomicAdd(&P.kcnt[cidx], 1ull);
+                        if (hid) atomicAdd(&s_hot_k[hid], 1u); else atomicAdd(&P.kcnt[cidx], 1ull);
                         nabs++;
                         const int s = cw_species(cw);
-                        const int m = cw_tidx(cw);
+                        const int m = cw_tidx(cw, P.tidx_mask);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                         j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
                         if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
@@ -1040,7 +1140,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const uint32_t brick = brick_of(ix, iy, iz, nbx, nby, bsh);
                     cidx = lin_index(ix, iy, iz, lpx, lpxy);
                     to_jump = brick_empty(s_m0, brick);
-                    cw = to_jump ? 0ull : __ldg(P.cellw + cidx);
+                    cw = to_jump ? 0ull : __ldg(P.cellw + (size_t)kCS * cidx);
                     if (RECORD)
                         hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
                 }
@@ -1074,6 +1174,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         }
     }
 #undef SF
+#undef RING
 #undef SU
     {   // dusty crossings stepped by this warp
         const uint32_t nd = __reduce_add_sync(kFull, ndusty_acc & 0xffffu), ndh = __reduce_add_sync(kFull, ndusty_acc >> 16);
@@ -1082,6 +1183,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 
     // flush the block-private histogram and counters
     __syncthreads();
+    if (HOT)
+        for (int i = 1 + (int)threadIdx.x; i <= P.n_hot; i += blockDim.x) {
+            const unsigned long long v = ((unsigned long long)s_hot_hi[i] << 32) + s_hot_lo[i];
+            const uint32_t ci = P.hot_idx[i];
+            if (v) lucy_add_raw(P.lfx, ci, v);
+            if (s_hot_k[i]) atomicAdd(&P.kcnt[ci], (unsigned long long)s_hot_k[i]);
+        }
     const int half = P.ndir * nf;
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) {
         const unsigned int v = s_hist[i];
@@ -1113,7 +1221,7 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
                                                       unsigned long long *__restrict__ kprev,
                                                       const long long *__restrict__ lfx, const double *__restrict__ J,
                                                       int nT, int ns, size_t ncp, int first_epoch, double ratio,
-                                                      double cellfac, unsigned long long *__restrict__ counters)
+                                                      double cellfac, unsigned long long *__restrict__ counters, uint32_t tmask)
 {
     extern __shared__ double s_J[];
     for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
@@ -1121,7 +1229,7 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
     if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
     bool ovf = false;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
-        const unsigned long long cw = cellw[i];
+        const unsigned long long cw = cellw[kCS * i];
         const double rho_c = cw_rho(cw);
         const unsigned long long kc = kcnt[i];
         uint32_t m = 0u;
@@ -1134,13 +1242,13 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
             }
             const double x = kt * cellfac / rho_c;
             m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, x);
-            const long long v = lfx[i];
+            const long long v = lfx[kCS * i];
             ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
         }
         kprev[i] = kc;
-        const uint32_t lo = (uint32_t)cw, nlo = (lo & 0xFF0000FFu) | (m << 8);
-        // low word: species | tidx << 8 | rho bits 29-31 (the words of vacuum and marker cells are never written)
-        if (nlo != lo && cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + i)[0] = nlo;
+        const uint32_t lo = (uint32_t)cw, nlo = (lo & ~(tmask << 8)) | (m << 8);
+        // low word: species | tidx << 8 | hot number | rho bits 29-31 (the words of vacuum and marker cells are never written)
+        if (nlo != lo && cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + kCS * i)[0] = nlo;
     }
     if (ovf) counters[CNT_OVERFLOW] = 1ull;
 }
@@ -1150,25 +1258,25 @@ __global__ void __launch_bounds__(256) k_sweep_update(unsigned long long *__rest
                                                       unsigned long long *__restrict__ kprev, long long *__restrict__ lfx,
                                                       const double *__restrict__ J, int nT, int ns, size_t ncp,
                                                       int from_lucy, double inv_fx, double cellfac,
-                                                      unsigned long long *__restrict__ counters)
+                                                      unsigned long long *__restrict__ counters, uint32_t tmask)
 {
     extern __shared__ double s_J[];
     for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
     __syncthreads();
     if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
-        const unsigned long long cw = cellw[i];
+        const unsigned long long cw = cellw[kCS * i];
         const double rho_c = cw_rho(cw);
         uint32_t m = 0u;
         if (cw_dusty(cw)) {
-            const double e = from_lucy ? (double)lfx[i] * inv_fx : (double)kcnt[i];
+            const double e = from_lucy ? (double)lfx[kCS * i] * inv_fx : (double)kcnt[i];
             const double x = e * cellfac / rho_c;
             m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, x);
         }
-        if (cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + i)[0] = ((uint32_t)cw & 0xFF0000FFu) | (m << 8);
+        if (cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + kCS * i)[0] = ((uint32_t)cw & ~(tmask << 8)) | (m << 8);
         kcnt[i] = 0ull;
         kprev[i] = 0ull;
-        lfx[i] = 0ll;
+        lfx[kCS * i] = 0ll;
     }
 }
 
@@ -1179,6 +1287,14 @@ __global__ void __launch_bounds__(256) k_count_delta(unsigned long long *__restr
 {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
         kcnt[i] = restore ? kcnt[i] + kprev[i] : kcnt[i] - kprev[i];
+}
+
+// gathers the Lucy tallies (stride kCS) into a contiguous buffer for the exchange, and back
+__global__ void __launch_bounds__(256) k_lucy_stage(long long *__restrict__ lfx, long long *__restrict__ stage, size_t n, int back)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        if (back) lfx[kCS * i] = stage[i]; else stage[i] = lfx[kCS * i];
+    }
 }
 
 // Sum of the parts' tallies over peer-visible memory, reduce-scatter / all-gather (mcrt_exchange_peer_sum):
@@ -1209,7 +1325,7 @@ __global__ void __launch_bounds__(256) k_range_check(const long long *__restrict
 {
     bool ovf = false;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
-        const long long v = lfx[i];
+        const long long v = lfx[kCS * i];
         ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
     }
     if (ovf) counters[CNT_OVERFLOW] = 1ull;
@@ -1234,9 +1350,10 @@ __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__rest
             if (s >= (uint32_t)ns) atomicAdd(&bad[1], 1ull);
             // fp32 -> fp64 is exact and leaves the low 29 mantissa bits zero; -0 is stored as +0
             const double rd = (r > 0.0f && !isinf(r)) ? (double)r : 0.0;
+            if (rd > 0.0) atomicAdd(&bad[2], 1ull);   // number of dusty cells (chooses the walk variant)
             cw = ((unsigned long long)__double_as_longlong(rd) & kRhoMask) | (unsigned long long)(s & 0xffu);
         }
-        cellw[b] = cw;
+        cellw[kCS * b] = cw;
     }
 }
 
@@ -1254,14 +1371,14 @@ __global__ void k_build_mask0(unsigned long long *__restrict__ cellw, uint32_t *
         for (int z = z0; z < z1 && empty; ++z)
             for (int y = y0; y < y1 && empty; ++y)
                 for (int x = x0; x < x1; ++x)
-                    if (!cw_vacuum(cellw[lin_index(x, y, z, px, pxy)])) { empty = false; break; }
+                    if (!cw_vacuum(cellw[(size_t)kCS * lin_index(x, y, z, px, pxy)])) { empty = false; break; }
         if (empty) {
             atomicOr(&m[b >> 5], 1u << (b & 31));
             // every cell word of an empty brick carries the marker bit: the cell walk sees it in the word it reads
             // anyway and needs no mask lookup
             for (int z = z0; z < z1; ++z)
                 for (int y = y0; y < y1; ++y)
-                    for (int x = x0; x < x1; ++x) cellw[lin_index(x, y, z, px, pxy)] |= kJumpWord;
+                    for (int x = x0; x < x1; ++x) cellw[(size_t)kCS * lin_index(x, y, z, px, pxy)] |= kJumpWord;
         }
     }
 }
@@ -1349,24 +1466,24 @@ __device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int 
 __global__ void k_gather(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
                          const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
                          const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
-                         int px, int pxy, double xi, double inv_fx, double cellfac)
+                         int px, int pxy, double xi, double inv_fx, double cellfac, uint32_t tmask)
 {
     const size_t nc = (size_t)nx * ny * nz;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
         const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
-        const size_t b = lin_index(ix, iy, iz, px, pxy);
+        const size_t b = lin_index(ix, iy, iz, px, pxy), bs = (size_t)kCS * b;
         switch (what) {
         case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
-        case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[b]; break;
-        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)cw_tidx(cellw[b]); break;
+        case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[bs]; break;
+        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)cw_tidx(cellw[bs], tmask); break;
         case G_ECOUNT: reinterpret_cast<double *>(out)[i] = (double)kcnt[b] * xi; break;
-        case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[b] * inv_fx * xi; break;
+        case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[bs] * inv_fx * xi; break;
         default: {
-            const unsigned long long cw = cellw[b];
+            const unsigned long long cw = cellw[bs];
             const double rho_c = cw_rho(cw);
             float T = 0.0f;
             if (cw_dusty(cw)) {
-                const double e = (what == G_TLUCY) ? (double)lfx[b] * inv_fx : (double)kcnt[b];
+                const double e = (what == G_TLUCY) ? (double)lfx[bs] * inv_fx : (double)kcnt[b];
                 T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
             }
             reinterpret_cast<float *>(out)[i] = T;
@@ -1385,6 +1502,24 @@ __global__ void k_sed(double *__restrict__ out, const unsigned long long *__rest
         const double dom = kFourPi * (mu[b + 1] - mu[b]);
         out[i] = (double)sed[i] * xi / (dnu[j] * dom);
     }
+}
+
+// numbers the hot cells in bits 24-28 of their cell words (id 0 clears)
+__global__ void k_set_hot(unsigned long long *__restrict__ cellw, const uint32_t *__restrict__ idx, const uint32_t *__restrict__ id, int n,
+                          uint32_t shift, uint32_t mask)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        uint32_t *lo = reinterpret_cast<uint32_t *>(cellw + (size_t)kCS * idx[i]);
+        *lo = (*lo & ~(mask << shift)) | (id[i] << shift);
+    }
+}
+
+// cell words of a list of cells (the candidates for hot cells)
+__global__ void k_fetch_words(const unsigned long long *__restrict__ cellw, const uint32_t *__restrict__ idx, unsigned long long *__restrict__ out, int n)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = cellw[(size_t)kCS * idx[i]];
 }
 
 // read-bandwidth probe: every thread sums 16-byte words of a buffer with a grid stride, eight loads in flight
@@ -1466,11 +1601,16 @@ int fx_bits_for(uint64_t n)
     return fx;
 }
 
-size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record)
+// Shared memory of a transport CTA is kept within the 196 KB carve-out: above it 28 KB of L1 remain for the walk's
+// scattered loads, which measured 2x slower.
+constexpr size_t kMaxTransportSmem = 195 * 1024;
+
+size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record, bool ringw)
 {
     return (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
            (size_t)(threads / 32) * 8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
-           (size_t)(MCRT_SMEM_MASK ? ((mask0_words + 1) & ~1) : 0) * sizeof(uint32_t);
+           (size_t)(MCRT_SMEM_MASK ? ((mask0_words + 1) & ~1) : 0) * sizeof(uint32_t) +
+           (ringw ? (size_t)kRing * threads * sizeof(unsigned long long) : 0);
 }
 
 // Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
@@ -1529,20 +1669,19 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
                          size_t *bytes_out)
 {
     if (!bytes_out || nx < 1 || ny < 1 || nz < 1 || n_species < 1 || n_nu < 2 || n_T < 2 || n_dir < 1) return MCRT_EINVAL;
-    const size_t nc = (size_t)nx * ny * nz;
     const MaskGeom mg = mask_geom(nx, ny, nz);
     const size_t nbricks = (size_t)mg.nbx * mg.nby * mg.nbz;
-    const size_t ncp = (size_t)(nx + 2 * kGuard) * (ny + 2 * kGuard) * (nz + 2 * kGuard);
+    const size_t ncp = (size_t)((nx + 2 * kGuard + MCRT_PITCH_ALIGN - 1) / MCRT_PITCH_ALIGN * MCRT_PITCH_ALIGN) * (ny + 2 * kGuard) * (nz + 2 * kGuard);
     size_t b = 0;
     auto add = [&b](size_t v) { b += align_up(v ? v : 1, 256); };
-    add((ncp + 1) * sizeof(uint2));      // cell words
+    add((ncp + 1) * sizeof(uint2) * kCS);   // cell words (kCS = 2: 16-byte records of cell word + Lucy tally)
     add((size_t)mg.mwords * 4);          // vacuum mask
     add(nbricks * sizeof(uint4));        // empty boxes of the J phase
     add((size_t)(mg.nbx + 1) * (mg.nby + 1) * (mg.nbz + 1) * sizeof(int));   // summed-area scratch
-    add(ncp * sizeof(long long));        // Lucy tally
+    if (kCS == 1) add(ncp * sizeof(long long));   // Lucy tally
     add(ncp * sizeof(long long));        // k
     add(ncp * sizeof(long long));        // k_prev
-    add(nc * 8);                         // scratch (staging of inputs / outputs)
+    add(ncp * 8);                        // scratch (staging of inputs / outputs / exchanged tallies)
     add(CNT_N * 8 + 64);                 // counters (+ validation flags)
     const size_t nsf = (size_t)n_species * n_nu;
     for (int i = 0; i < 4; ++i) add(nsf * 8);
@@ -1552,6 +1691,7 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     add((size_t)(n_dir + 1) * 8);
     add((size_t)n_dir * n_nu * 8); add((size_t)n_dir * n_nu * 8);
     add((size_t)n_dir * n_nu * 8);                           // SED staging
+    add((size_t)(5 * (kHot + 1) + 4 * 1400) * sizeof(uint32_t));   // hot-cell table and staging (mcrt_source)
     if (n_digests) add(n_digests * sizeof(mcrt_digest));
     *bytes_out = b + 4096;
     return MCRT_OK;
@@ -1564,7 +1704,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return fail(nullptr, MCRT_EINVAL, "nx, ny, nz must be >= 1");
     if (nx > 2040 || ny > 2040 || nz > 1016) return fail(nullptr, MCRT_EINVAL, "grid too large: nx, ny <= 2040 and nz <= 1016");
-    if ((size_t)(nx + 2 * kGuard) * (ny + 2 * kGuard) * (nz + 2 * kGuard) > ((size_t)1 << 31)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^31 cells");
+    if ((size_t)(nx + 2 * kGuard) * (ny + 2 * kGuard) * (nz + 2 * kGuard) > ((size_t)1 << 30)) return fail(nullptr, MCRT_EINVAL, "grid larger than 2^30 cells (guard shell included)");
     if (!(cell_size_cm > 0.0) || !isfinite(cell_size_cm)) return fail(nullptr, MCRT_EINVAL, "cell_size_cm must be > 0");
     if (!rho || !species) return fail(nullptr, MCRT_EINVAL, "rho / species is NULL");
     if (n_species < 1 || n_species > 255) return fail(nullptr, MCRT_EINVAL, "n_species must be in 1..255");
@@ -1581,7 +1721,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         c->nbx = g.nbx; c->nby = g.nby; c->nbz = g.nbz;
     }
     c->nc = (size_t)nx * ny * nz;
-    c->px = nx + 2 * kGuard; c->pxy = c->px * (ny + 2 * kGuard);
+    c->px = (nx + 2 * kGuard + MCRT_PITCH_ALIGN - 1) / MCRT_PITCH_ALIGN * MCRT_PITCH_ALIGN; c->pxy = c->px * (ny + 2 * kGuard);
     c->ncp = (size_t)c->pxy * (nz + 2 * kGuard);
     c->ws = (char *)workspace; c->ws_bytes = workspace_bytes; c->ws_owned_by_caller = workspace != nullptr;
     int rc;
@@ -1599,14 +1739,15 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
             return MCRT_ECUDA;                                                                         \
         }                                                                                              \
     } while (0)
-    GC_TRY(ws_alloc(c, (void **)&c->cellw, (c->ncp + 1) * sizeof(uint2)));
+    GC_TRY(ws_alloc(c, (void **)&c->cellw, (c->ncp + 1) * sizeof(uint2) * kCS));
     GC_TRY(ws_alloc(c, (void **)&c->vmask, (size_t)c->mwords * 4));
     GC_TRY(ws_alloc(c, (void **)&c->vbox, (size_t)c->nbx * c->nby * c->nbz * sizeof(uint4)));
     GC_TRY(ws_alloc(c, (void **)&c->vsat, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int)));
-    GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
+    if (kCS == 1) GC_TRY(ws_alloc(c, (void **)&c->lfx, c->ncp * sizeof(long long)));
+    else c->lfx = reinterpret_cast<long long *>(c->cellw + 1);   // second word of every 16-byte cell record
     GC_TRY(ws_alloc(c, (void **)&c->kabs_cnt, c->ncp * sizeof(long long)));
     GC_TRY(ws_alloc(c, (void **)&c->kprev, c->ncp * sizeof(long long)));
-    GC_TRY(ws_alloc(c, (void **)&c->scratch, c->nc * 8));
+    GC_TRY(ws_alloc(c, (void **)&c->scratch, c->ncp * 8));   // staging: inputs, outputs, the Lucy tallies of an exchange
     GC_TRY(ws_alloc(c, (void **)&c->counters, CNT_N * 8 + 64));
     GC_CUDA(cudaMemsetAsync(c->counters, 0, CNT_N * 8 + 64, c->stream));
     const float *d_rho = rho;
@@ -1633,16 +1774,21 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         k_grow_boxes<<<stream_grid(nbr), 256, 0, c->stream>>>(c->vmask, c->vsat, c->vbox, c->nbx, c->nby, c->nbz);
     }
     GC_CUDA(cudaGetLastError());
-    GC_CUDA(cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
+    GC_CUDA(cudaMemset2DAsync(c->lfx, 8 * kCS, 0, 8, c->ncp, c->stream));
     GC_CUDA(cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
     GC_CUDA(cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
-    unsigned long long hbad[2] = {0, 0};
-    GC_CUDA(cudaMemcpyAsync(hbad, bad, 16, cudaMemcpyDeviceToHost, c->stream));
+    unsigned long long hbad[3] = {0, 0, 0};
+    GC_CUDA(cudaMemcpyAsync(hbad, bad, 24, cudaMemcpyDeviceToHost, c->stream));
     GC_CUDA(cudaStreamSynchronize(c->stream));
     if (hbad[0] || hbad[1]) {
         g_create_error = hbad[0] ? "rho holds negative, NaN or infinite values" : "species index >= n_species";
         mcrt_destroy(c);
         return MCRT_EINVAL;
+    }
+    c->n_dusty = hbad[2];
+    {
+        int l2 = 0;
+        if (cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, c->device) == cudaSuccess && l2 > 0) c->l2_bytes = (size_t)l2;
     }
 #undef GC_TRY
 #undef GC_CUDA
@@ -1679,9 +1825,12 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
         if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
         if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
     }
-    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256, true) > 220 * 1024)
+    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256, true, true) > kMaxTransportSmem)
         return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
     c->nf = n_nu; c->nT = n_T;
+    // low half of the cell word: species 0-7 | temperature index (12 or 16 bits) | hot-cell number (9 or 5 bits) | rho 29-31
+    if (n_T <= 4096) { c->tidx_mask = 0xfffu; c->hot_shift = 20; c->hot_mask = 511u; c->hot_max = 511; }
+    else { c->tidx_mask = 0xffffu; c->hot_shift = 24; c->hot_mask = 31u; c->hot_max = 31; }
     c->nu.assign(nu_hz, nu_hz + n_nu);
     c->kabs.assign(kappa_abs, kappa_abs + nsf);
     c->ksca.assign(kappa_sca, kappa_sca + nsf);
@@ -1769,6 +1918,58 @@ int mcrt_source(mcrt_ctx *c, double L_erg_s, double T_star_K, const double *L_nu
     c->L = L_erg_s;
     CUDA_TRY(c, cudaMemcpyAsync(c->d_srccdf, c->srccdf.data(), (size_t)c->nf * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    {
+        // Hot cells: the (at most hot_max) dusty cells whose centres lie nearest to the source, within 5.5 cells.
+        int rc2;
+        const size_t stage_words = 4 * (size_t)(kHot + 1) + 2 * 1400;
+        if (!c->d_hot_idx && (rc2 = ws_alloc(c, (void **)&c->d_hot_idx, (kHot + 1 + stage_words + 2 * 1400) * sizeof(uint32_t)))) return rc2;
+        uint32_t *d_stage = c->d_hot_idx + (kHot + 1);
+        struct Cand { double d2; uint32_t idx; };
+        std::vector<Cand> cand;
+        const int sx = (int)floor(c->pos[0]), sy = (int)floor(c->pos[1]), sz = (int)floor(c->pos[2]);
+        for (int iz = sz - 5; iz <= sz + 5; ++iz)
+            for (int iy = sy - 5; iy <= sy + 5; ++iy)
+                for (int ix = sx - 5; ix <= sx + 5; ++ix) {
+                    if (ix < 0 || iy < 0 || iz < 0 || ix >= c->nx || iy >= c->ny || iz >= c->nz) continue;
+                    const double dx = ix + 0.5 - c->pos[0], dy = iy + 0.5 - c->pos[1], dz = iz + 0.5 - c->pos[2];
+                    const double d2 = dx * dx + dy * dy + dz * dz;
+                    if (d2 <= 30.25) cand.push_back({d2, (uint32_t)((iz + kGuard) * c->pxy + (iy + kGuard) * c->px + (ix + kGuard))});
+                }
+        const int nc_ = (int)cand.size();      // <= 11^3 = 1331
+        std::vector<unsigned long long> words(nc_);
+        if (nc_) {
+            std::vector<uint32_t> ci(nc_);
+            for (int i = 0; i < nc_; ++i) ci[i] = cand[i].idx;
+            unsigned long long *d_words = reinterpret_cast<unsigned long long *>(d_stage + 1400 + ((kHot + 1 + 1400) & 1));
+            CUDA_TRY(c, cudaMemcpyAsync(d_stage, ci.data(), nc_ * 4, cudaMemcpyHostToDevice, c->stream));
+            k_fetch_words<<<(nc_ + 127) / 128, 128, 0, c->stream>>>(c->cellw, d_stage, d_words, nc_);
+            CUDA_TRY(c, cudaGetLastError());
+            CUDA_TRY(c, cudaMemcpyAsync(words.data(), d_words, (size_t)nc_ * 8, cudaMemcpyDeviceToHost, c->stream));
+            CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        }
+        std::vector<Cand> dusty;
+        for (int i = 0; i < nc_; ++i) {
+            const uint32_t hi = (uint32_t)(words[i] >> 32);
+            if (hi - 1u < 0x7FEFFFFFu) dusty.push_back(cand[i]);
+        }
+        std::stable_sort(dusty.begin(), dusty.end(), [](const Cand &a, const Cand &b) { return a.d2 < b.d2 || (a.d2 == b.d2 && a.idx < b.idx); });
+        if ((int)dusty.size() > c->hot_max) dusty.resize(c->hot_max);
+        // clear the previous numbering, then number the new set
+        std::vector<uint32_t> h_idx, h_id;
+        for (int i = 1; i <= c->n_hot; ++i) { h_idx.push_back(c->hot_idx[i]); h_id.push_back(0u); }
+        c->n_hot = (int)dusty.size();
+        c->hot_idx.assign(kHot + 1, 0u);
+        for (int i = 1; i <= c->n_hot; ++i) { c->hot_idx[i] = dusty[i - 1].idx; h_idx.push_back(c->hot_idx[i]); h_id.push_back((uint32_t)i); }
+        const int n = (int)h_idx.size();       // <= 2 kHot
+        if (n) {
+            CUDA_TRY(c, cudaMemcpyAsync(d_stage, h_idx.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
+            CUDA_TRY(c, cudaMemcpyAsync(d_stage + 2 * (kHot + 1), h_id.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
+            k_set_hot<<<(n + 127) / 128, 128, 0, c->stream>>>(c->cellw, d_stage, d_stage + 2 * (kHot + 1), n, c->hot_shift, c->hot_mask);
+            CUDA_TRY(c, cudaGetLastError());
+        }
+        CUDA_TRY(c, cudaMemcpyAsync(c->d_hot_idx, c->hot_idx.data(), (kHot + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
     c->have_source = true;
     return MCRT_OK;
 }
@@ -1806,22 +2007,41 @@ static int ensure_histograms(mcrt_ctx *c)
     return MCRT_OK;
 }
 
+// the eight instantiations of the transport kernel
+typedef void (*transport_fn)(const TransportParams);
+static transport_fn transport_kernel(bool record, bool ringw, bool hot)
+{
+    static const transport_fn tab[8] = {k_transport<false, false, false>, k_transport<true, false, false>,
+                                        k_transport<false, true, false>,  k_transport<true, true, false>,
+                                        k_transport<false, false, true>,  k_transport<true, false, true>,
+                                        k_transport<false, true, true>,   k_transport<true, true, true>};
+    return tab[(record ? 1 : 0) | (ringw ? 2 : 0) | (hot ? 4 : 0)];
+}
+
+// which walk variant
+static bool use_ring(const mcrt_ctx *c, const mcrt_run_opts *o)
+{
+    (void)c;
+    return o && o->walk_words == 2;      // auto = registers: the ring was never faster (see kDepthRing)
+}
+
 static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem)
 {
     const bool record = o && o->record_digests;
+    const bool ringw = use_ring(c, o);
     *threads = (o && o->block_threads > 0) ? o->block_threads : MCRT_MAX_THREADS;
     if (*threads % 32 || *threads > MCRT_MAX_THREADS || *threads < 32)
         return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32.." + std::to_string(MCRT_MAX_THREADS));
     // as many warps (each with its packet pool) as fit beside the tables in 227 KB of shared memory
-    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record) > 227 * 1024) *threads -= 32;
-    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record);
+    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, ringw) > kMaxTransportSmem) *threads -= 32;
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, ringw);
     if (*smem > 48 * 1024) {
-        CUDA_TRY(c, cudaFuncSetAttribute(k_transport<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
-        CUDA_TRY(c, cudaFuncSetAttribute(k_transport<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
+        for (int v = 0; v < 8; ++v)
+            CUDA_TRY(c, cudaFuncSetAttribute(transport_kernel(v & 1, v & 2, v & 4), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
     }
     int nsm = 148, occ = 1;
     CUDA_TRY(c, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device));
-    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport<false>, *threads, *smem));
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, transport_kernel(false, true, true), *threads, *smem));
     if (occ < 1) return fail(c, MCRT_EINVAL, "transport kernel does not fit on an SM with these table sizes");
     c->occ_blocks = occ;
     *blocks = (o && o->grid_blocks > 0) ? o->grid_blocks : nsm * occ;  // persistent: every CTA resident
@@ -1867,6 +2087,12 @@ int mcrt_get_stats(mcrt_ctx *c, mcrt_run_stats *st)
     return st->overflow ? fail(c, MCRT_EOVERFLOW, "a Lucy fixed-point tally exceeded 2^62") : MCRT_OK;
 }
 
+static void launch_transport(mcrt_ctx *c, const TransportParams &P)
+{
+    const mcrt_ctx::Run &R = c->run;
+    transport_kernel(R.o.record_digests != 0, R.ringw, R.hot)<<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+}
+
 static void fill_params(mcrt_ctx *c, TransportParams &P)
 {
     memset(&P, 0, sizeof(P));
@@ -1874,6 +2100,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
     P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
     P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
+    P.hot_idx = c->d_hot_idx; P.hot_shift = c->hot_shift; P.hot_mask = c->hot_mask; P.tidx_mask = c->tidx_mask; P.n_hot = c->n_hot;
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
@@ -1980,6 +2207,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         return fail(c, MCRT_EINVAL, "part_index must be in 0..part_count-1");
     if (o.part_count <= 1) { o.part_count = 1; o.part_index = 0; }
     if (o.epoch_growth == 0.0) o.epoch_growth = 2.0;
+    if (o.walk_words < 0 || o.walk_words > 2) return fail(c, MCRT_EINVAL, "walk_words must be 0 (auto), 1 (registers) or 2 (ring)");
     if (!(o.epoch_growth >= 1.0) || !isfinite(o.epoch_growth)) return fail(c, MCRT_EINVAL, "epoch_growth must be >= 1");
     if (o.n_total && o.n_total < n_packets) return fail(c, MCRT_EINVAL, "n_total must be >= n_packets");
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
@@ -1987,6 +2215,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (rc) return rc;
     mcrt_ctx::Run &R = c->run;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem))) return rc;
+    R.ringw = use_ring(c, &o);
+    R.hot = c->n_hot > 0 && !o.no_hot_cells;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
     const uint64_t n_xi = o.n_total ? o.n_total : n_packets;
@@ -2009,7 +2239,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     c->dig_base = o.first_packet_id;
 
     if (o.reset_tallies && o.mode == MCRT_MODE_BW_EPOCH) {
-        CUDA_TRY(c, cudaMemsetAsync(c->lfx, 0, c->ncp * 8, c->stream));
+        CUDA_TRY(c, cudaMemset2DAsync(c->lfx, 8 * kCS, 0, 8, c->ncp, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
@@ -2070,13 +2300,12 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         mark(c, timing);
         k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          R.e == 0, R.e == 0 ? 1.0 : (double)Be / (double)R.Bprev,
-                                                         R.cellfac, c->counters);
+                                                         R.cellfac, c->counters, c->tidx_mask);
         part_slice(o, Be, &lo, &hi);
         P.pid0 = o.first_packet_id + R.done + lo; P.count = hi - lo;
         mark(c, timing);
         if (P.count) {
-            if (o.record_digests) k_transport<true><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
-            else k_transport<false><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+            launch_transport(c, P);
         }
         mark(c, timing);
         c->launches += P.count ? 2 : 1;
@@ -2092,7 +2321,7 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         mark(c, timing);
         k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
-                                                         sw == 1 ? R.prev_cellfac : R.cellfac, c->counters);
+                                                         sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
         CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
@@ -2103,8 +2332,7 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         P.pid0 = o.first_packet_id + lo; P.count = hi - lo;
         mark(c, timing);
         if (P.count) {
-            if (o.record_digests) k_transport<true><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
-            else k_transport<false><<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+            launch_transport(c, P);
         }
         mark(c, timing);
         c->launches += P.count ? 2 : 1;
@@ -2164,7 +2392,13 @@ int mcrt_exchange_begin(mcrt_ctx *c, mcrt_exchange *out)
     int n = 0;
     out->ptr[n] = c->kabs_cnt; out->words[n++] = c->ncp;
     if (c->exchange_full) {
-        out->ptr[n] = c->lfx; out->words[n++] = c->ncp;
+        if (kCS == 1) out->ptr[n] = c->lfx;
+        else {   // the tallies sit in the cell records: exchanged through a contiguous staging copy
+            k_lucy_stage<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx, (long long *)c->scratch, c->ncp, 0);
+            c->launches += 1;
+            out->ptr[n] = c->scratch;
+        }
+        out->words[n++] = c->ncp;
         out->ptr[n] = c->sed; out->words[n++] = (uint64_t)c->ndir * c->nf;
         out->ptr[n] = c->sed_direct; out->words[n++] = (uint64_t)c->ndir * c->nf;
         out->ptr[n] = c->counters; out->words[n++] = CNT_NEXT;
@@ -2181,6 +2415,10 @@ int mcrt_exchange_end(mcrt_ctx *c)
     if (!c->exchange_open) return fail(c, MCRT_ESTATE, "mcrt_exchange_end without mcrt_exchange_begin");
     k_count_delta<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->kabs_cnt, c->kprev, c->ncp, 1);
     c->launches += 1;
+    if (c->exchange_full && kCS != 1) {
+        k_lucy_stage<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx, (long long *)c->scratch, c->ncp, 1);
+        c->launches += 1;
+    }
     CUDA_TRY(c, cudaGetLastError());
     if (c->exchange_full) c->globalised = true;
     c->exchange_open = false;
@@ -2236,7 +2474,7 @@ static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem wh
     void *dev = (where == MCRT_DEVICE) ? dst : c->scratch;
     const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
     k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, c->nT, c->nx,
-                                                       c->ny, c->nz, c->px, c->pxy, c->xi, ldexp(1.0, -c->fx), cellfac);
+                                                       c->ny, c->nz, c->px, c->pxy, c->xi, ldexp(1.0, -c->fx), cellfac, c->tidx_mask);
     CUDA_TRY(c, cudaGetLastError());
     if (where == MCRT_HOST) {
         CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
