@@ -472,7 +472,22 @@ typedef struct {
     uint64_t pid0;           /* id of the first packet of this run (continuing a run with further packets) */
     uint64_t n_total;        /* the luminosity is split into this many packets, xi = L / n_total; 0 = n_packets */
     double growth;           /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2 (O11) */
+    uint32_t carry_K;        /* > 0: a packet is carried over to the next epoch after this many interactions in one epoch */
 } orc_opts;
+
+/* A packet carried over an epoch boundary: everything its continuation depends on.  The paper pauses packets with
+ * more than 100 interactions in one cell once 80 % of the threads have finished, stores position and frequency and
+ * resumes them at the end; which packets that hits depends on scheduling.  The deterministic
+ * restatement (reading Q23): a packet that has had carry_K interactions within ONE epoch stops after the
+ * carry_K-th (its new direction and frequency already drawn) and continues in the next epoch, from the same state
+ * and with its own random stream, at that epoch's temperatures.  After the last epoch the carried packets run in
+ * further epochs, with the budget doubled each time, until none is left. */
+typedef struct {
+    uint64_t pid, hash;
+    double p[3], u[3];
+    int32_t c[3], j;
+    uint32_t d, ncross, nsca, nabs;
+} orc_carry;
 
 typedef struct {
     const orc_ctx *C;
@@ -488,6 +503,7 @@ typedef struct {
     uint32_t pass;
     int fx;
     uint64_t pid0_digest;
+    uint32_t carry_K;        /* interaction budget of the current epoch (0 = none) */
     const orc_opts *o;
 } orc_run_t;
 
@@ -520,7 +536,9 @@ static inline void lucy_add(orc_run_t *R, size_t ci, int sj, double rho_c, doubl
     }
 }
 
-static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
+/* Follows one packet (a new one, or one carried over: `resume`) until it escapes -- returns 0 -- or until its
+ * interaction budget of this epoch is used up: its state is written to *park and 1 is returned. */
+static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry *resume, orc_carry *park)
 {
     const orc_ctx *C = R->C;
     const int nf = C->nf;
@@ -529,18 +547,25 @@ static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
     double z[2];
     double p[3], u[3];
     int c[3];
-    uint32_t ncross = 0, nsca = 0, nabs = 0;
+    uint32_t ncross = 0, nsca = 0, nabs = 0, nint = 0;
     uint64_t hash = 0xCBF29CE484222325ull;
+    int j;
 
-    /* O3 emit: frequency through the source CDF, isotropic direction */
-    orc_uniforms(R->seed, pid, d++, R->pass, z);
-    int j = orc_lower_bound(C->srccdf, nf, z[0]);
-    orc_uniforms(R->seed, pid, d++, R->pass, z);
-    orc_isotropic(z[0], z[1], u);
-    p[0] = C->pos[0]; p[1] = C->pos[1]; p[2] = C->pos[2];
-    start_cell(p, u, c);
-    hash_mix(&hash, event_word(ORC_EV_EMIT, j, ((uint64_t)c[2] * n[1] + c[1]) * n[0] + c[0]));
-    st->packets++;
+    if (resume) {
+        pid = resume->pid; hash = resume->hash; j = resume->j; d = resume->d;
+        ncross = resume->ncross; nsca = resume->nsca; nabs = resume->nabs;
+        for (int a = 0; a < 3; ++a) { p[a] = resume->p[a]; u[a] = resume->u[a]; c[a] = resume->c[a]; }
+    } else {
+        /* O3 emit: frequency through the source CDF, isotropic direction */
+        orc_uniforms(R->seed, pid, d++, R->pass, z);
+        j = orc_lower_bound(C->srccdf, nf, z[0]);
+        orc_uniforms(R->seed, pid, d++, R->pass, z);
+        orc_isotropic(z[0], z[1], u);
+        p[0] = C->pos[0]; p[1] = C->pos[1]; p[2] = C->pos[2];
+        start_cell(p, u, c);
+        hash_mix(&hash, event_word(ORC_EV_EMIT, j, ((uint64_t)c[2] * n[1] + c[1]) * n[0] + c[0]));
+        st->packets++;
+    }
 
     for (;;) { /* one flight per iteration */
         /* O4 / S3: optical depth to the next interaction, tau = -ln zeta (Eq. 3;
@@ -620,6 +645,13 @@ static void run_packet(orc_run_t *R, uint64_t pid, orc_stats *st)
             orc_isotropic(z[0], z[1], u);
             hash_mix(&hash, event_word(ORC_EV_ABSORB, j, ci));
         }
+        /* carry-over (see orc_carry): the budget of this epoch is used up */
+        if (R->carry_K && ++nint >= R->carry_K) {
+            park->pid = pid; park->hash = hash; park->j = j; park->d = d;
+            park->ncross = ncross; park->nsca = nsca; park->nabs = nabs;
+            for (int a = 0; a < 3; ++a) { park->p[a] = p[a]; park->u[a] = u[a]; park->c[a] = c[a]; }
+            return 1;
+        }
     }
 escaped:
     {
@@ -643,12 +675,45 @@ done:
         orc_digest *g = &R->dig[pid - R->pid0_digest];
         g->hash = hash; g->crossings = ncross; g->scatterings = nsca; g->absorptions = nabs;
     }
+    return 0;
 }
 
-static void run_range(orc_run_t *R, uint64_t pid0, uint64_t count, orc_stats *total)
+/* growing list of carried packets */
+typedef struct { orc_carry *v; size_t n, cap; } orc_carry_list;
+
+static void carry_push(orc_carry_list *L, const orc_carry *e)
+{
+    if (L->n == L->cap) {
+        L->cap = L->cap ? 2 * L->cap : 256;
+        L->v = (orc_carry *)realloc(L->v, L->cap * sizeof(orc_carry));
+    }
+    L->v[L->n++] = *e;
+}
+
+static int carry_cmp(const void *a, const void *b)
+{
+    const uint64_t x = ((const orc_carry *)a)->pid, y = ((const orc_carry *)b)->pid;
+    return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+static void add_stats(orc_stats *total, const orc_stats *st)
+{
+    total->packets += st->packets; total->crossings += st->crossings;
+    total->dusty_crossings += st->dusty_crossings; total->flights += st->flights;
+    total->scatterings += st->scatterings; total->absorptions += st->absorptions;
+    total->escapes += st->escapes; total->direct_escapes += st->direct_escapes;
+    total->lucy_adds += st->lucy_adds;
+}
+
+/* One epoch's packets: first the packets carried over from the previous epoch (`in`), then `count` new packets
+ * with ids from pid0.  Packets whose budget runs out are appended to `out` (sorted by id afterwards, so that the
+ * list does not depend on the thread count). */
+static void run_range(orc_run_t *R, uint64_t pid0, uint64_t count, orc_stats *total, const orc_carry_list *in,
+                      orc_carry_list *out)
 {
     int nth = R->o->n_threads > 1 ? R->o->n_threads : 1;
     if (R->Lsum) nth = 1;
+    const int64_t n_in = in ? (int64_t)in->n : 0, n_all = n_in + (int64_t)count;
 #ifdef _OPENMP
     if (nth > 1) {
         /* packets are independent inside an epoch; integer tallies make the result
@@ -657,21 +722,32 @@ static void run_range(orc_run_t *R, uint64_t pid0, uint64_t count, orc_stats *to
         {
             orc_stats st;
             memset(&st, 0, sizeof st);
+            orc_carry_list mine = { NULL, 0, 0 };
+            orc_carry e;
 #pragma omp for schedule(dynamic, 64)
-            for (int64_t i = 0; i < (int64_t)count; ++i) run_packet(R, pid0 + (uint64_t)i, &st);
+            for (int64_t i = 0; i < n_all; ++i) {
+                const int parked = (i < n_in) ? run_packet(R, 0, &st, &in->v[i], &e)
+                                              : run_packet(R, pid0 + (uint64_t)(i - n_in), &st, NULL, &e);
+                if (parked) carry_push(&mine, &e);
+            }
 #pragma omp critical
             {
-                total->packets += st.packets; total->crossings += st.crossings;
-                total->dusty_crossings += st.dusty_crossings; total->flights += st.flights;
-                total->scatterings += st.scatterings; total->absorptions += st.absorptions;
-                total->escapes += st.escapes; total->direct_escapes += st.direct_escapes;
-                total->lucy_adds += st.lucy_adds;
+                add_stats(total, &st);
+                for (size_t q = 0; q < mine.n; ++q) carry_push(out, &mine.v[q]);
             }
+            free(mine.v);
         }
+        if (out && out->n > 1) qsort(out->v, out->n, sizeof(orc_carry), carry_cmp);
         return;
     }
 #endif
-    for (uint64_t i = 0; i < count; ++i) run_packet(R, pid0 + i, total);
+    orc_carry e;
+    for (int64_t i = 0; i < n_all; ++i) {
+        const int parked = (i < n_in) ? run_packet(R, 0, total, &in->v[i], &e)
+                                      : run_packet(R, pid0 + (uint64_t)(i - n_in), total, NULL, &e);
+        if (parked) carry_push(out, &e);
+    }
+    if (out && out->n > 1) qsort(out->v, out->n, sizeof(orc_carry), carry_cmp);
 }
 
 /* number of J[s][.] entries strictly below x, clamped to [0, nT-1] */
@@ -841,10 +917,14 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
         R.pass = o->pass0;
         uint64_t done = 0, Bnom = B0, Bprev = 0;
         int e = 0;
+        orc_carry_list carried = { NULL, 0, 0 }, parked = { NULL, 0, 0 };
+        R.carry_K = o->absorb_and_stop ? 0u : o->carry_K;
         while (done < n_packets) {
             uint64_t Be = n_packets - done < Bnom ? n_packets - done : Bnom;
             epoch_update(S, e == 0, e == 0 ? 1.0 : (double)Be / (double)Bprev, cellfac);
-            run_range(&R, o->pid0 + done, Be, &st);
+            parked.n = 0;
+            run_range(&R, o->pid0 + done, Be, &st, &carried, &parked);
+            { orc_carry_list t = carried; carried = parked; parked = t; }
             done += Be;
             Bprev = Be;
             {
@@ -856,6 +936,17 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
             ++e;
             st.epochs++;
         }
+        /* the packets still carried run in further epochs (no new packets, same temperature rule with B_e / B_e-1
+         * = 1), the budget doubling each time, until all have escaped */
+        while (carried.n > 0) {
+            R.carry_K = R.carry_K > 0x40000000u ? 0x80000000u : 2u * R.carry_K;
+            epoch_update(S, 0, 1.0, cellfac);
+            parked.n = 0;
+            run_range(&R, 0, 0, &st, &carried, &parked);
+            { orc_carry_list t = carried; carried = parked; parked = t; }
+            st.epochs++;
+        }
+        free(carried.v); free(parked.v);
     } else {
         /* iterative scheme of PAPER.md:73: temperatures of the previous run, Eq. 5 for the frequency */
         R.cdf = C->cdfB;
@@ -868,7 +959,8 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
             sweep_update(S, o->sweep_T_from_lucy, sw == 1 ? prev_cellfac : cellfac, sw == 1 ? prev_fx : S->fx);
             zero_tallies(S);
             R.pass = o->pass0 + (uint32_t)sw;
-            run_range(&R, o->pid0, n_packets, &st);
+            R.carry_K = 0;
+            run_range(&R, o->pid0, n_packets, &st, NULL, NULL);
             st.epochs++;
         }
     }

@@ -678,3 +678,64 @@ def test_p18_multiple_scattering_displacement(orc, a, g):
     sig = math.sqrt(((k * rr2 ** 2).sum() / K - tot ** 2) / K)
     assert abs(tot - (r2_true + 0.25)) < 4 * sig, (tot, r2_true + 0.25, sig)
     assert sig / tot < 0.006            # the bound is sharp: 0.6 % (the voxel term alone is 0.3-1.5 %)
+
+
+# ------------------------------------------------------------------------------------------ P19 carry-over
+def test_p19_carry_over_of_long_lived_packets(orc):
+    """NEXT-1: the deterministic restatement of the paper's pause / resume of packets with more than 100
+    interactions (orc_carry in the oracle): a packet stops after carry_K interactions within one
+    epoch and continues in the next epoch from the same state and random stream, at that epoch's temperatures.
+      (a) grey dust: transport does not depend on frequency, so carrying cannot change a single path -- absorption
+          counts, Lucy tallies and every packet's crossing / scattering / absorption numbers are IDENTICAL to the
+          uncarried run (fails if the carried state loses position, direction, cell or draw counter);
+      (b) nothing is lost: every packet escapes exactly once, in whatever epoch;
+      (c) the result does not depend on the thread count (the carried list is ordered by packet id);
+      (d) a budget no packet reaches changes nothing at all;
+      (e) chromatic thick cube, 60 % of the packets carried at least once: temperatures within 0.5 % shell by
+          shell and the spectrum within 3 % band by band of the uncarried run (the paper's 100 interactions)."""
+    N = 20_000
+    grey = W.uniform_cube(10, 20.0, 0.6, 0.3, n_nu=32, slope=0.0, T_star=3000.0)
+    o = orc.Oracle.from_workload(grey)
+    r0 = o.run(N, 19, n_threads=NTH, digests=True)
+    raw0 = o.read_raw()
+    n_int = r0["digests"]["absorptions"].astype(np.int64) + r0["digests"]["scatterings"]
+    assert (n_int > 100).mean() > 0.5 and n_int.max() > 1000
+    r1 = o.run(N, 19, n_threads=NTH, digests=True, carry_K=100)
+    raw1 = o.read_raw()
+    assert r1["epochs"] > r0["epochs"]                                        # further epochs drained the carried packets
+    for key in ("k", "lucy_fx"):                                              # (a)
+        assert np.array_equal(raw0[key], raw1[key]), key
+    for key in ("crossings", "scatterings", "absorptions", "escape_bin"):
+        assert np.array_equal(r0["digests"][key], r1["digests"][key]), key
+    assert not np.array_equal(r0["digests"]["hash"], r1["digests"]["hash"])   # ... but re-emitted frequencies differ
+    assert int(raw1["sed"].sum()) == N == r1["escapes"] == r1["packets"]      # (b)
+    assert int(raw1["k"].sum()) == r1["absorptions"] and r1["flights"] == N + r1["scatterings"] + r1["absorptions"]
+    r2 = o.run(N, 19, n_threads=1, digests=True, carry_K=100)                 # (c)
+    raw2 = o.read_raw()
+    for key in raw1:
+        assert np.array_equal(raw1[key], raw2[key]), key
+    assert np.array_equal(r1["digests"], r2["digests"])
+    r3 = o.run(N, 19, n_threads=NTH, digests=True, carry_K=int(n_int.max()) + 1)   # (d)
+    raw3 = o.read_raw()
+    for key in raw0:
+        assert np.array_equal(raw0[key], raw3[key]), key
+    assert np.array_equal(r0["digests"], r3["digests"]) and r3["epochs"] == r0["epochs"]
+    # (e)
+    chrom = W.uniform_cube(10, 40.0, 0.6, 0.3, n_nu=32, slope=-0.3, T_star=3000.0)
+    oc = orc.Oracle.from_workload(chrom)
+    N2 = 40_000
+    ra = oc.run(N2, 17, n_threads=NTH, digests=True)
+    Ta, sa = oc.read()["T"].astype(float), oc.read_raw()["sed"].sum(axis=0).astype(float)
+    rb = oc.run(N2, 17, n_threads=NTH, digests=True, carry_K=100)
+    Tb, sb = oc.read()["T"].astype(float), oc.read_raw()["sed"].sum(axis=0).astype(float)
+    na = ra["digests"]["absorptions"].astype(np.int64) + ra["digests"]["scatterings"]
+    assert (na > 100).mean() > 0.5
+    assert (ra["digests"]["hash"] != rb["digests"]["hash"]).mean() > 0.5
+    x = (np.arange(10) + 0.5) - 5
+    rr = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2).reshape(-1)
+    for lo in range(5):
+        sel = (rr >= lo) & (rr < lo + 1)
+        assert abs(Tb[sel].mean() / Ta[sel].mean() - 1) < 0.005, lo
+    ba, bb = sa.reshape(8, 4).sum(axis=1), sb.reshape(8, 4).sum(axis=1)
+    sel = ba > 300
+    assert sel.sum() >= 3 and np.all(np.abs(bb[sel] / ba[sel] - 1) < 0.03 + 3 / np.sqrt(ba[sel]))
