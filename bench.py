@@ -56,6 +56,7 @@ def parse():
     ap.add_argument("--exchange", default="auto", choices=["auto", "p2p", "nccl"],
                     help="N > 1: how the ranks' tallies are summed (auto = peer memory, NCCL if that cannot be set up)")
     ap.add_argument("--walk-words", type=int, default=0, help="experiment: 1 = cell words in registers, 2 = cp.async ring (0 = library's choice)")
+    ap.add_argument("--carry", type=int, default=0, help="experiment: carry packets over epoch boundaries after this many interactions in one epoch (0 = off, the configuration's definition)")
     ap.add_argument("--no-hot", action="store_true", help="experiment: no per-CTA copies of the tallies of the cells around the source")
     ap.add_argument("--sweeps", type=int, default=-1, help="frozen-T sweeps after the B&W pass (-1 = the configuration's: 3 for torus512)")
     return ap.parse_args()
@@ -276,6 +277,8 @@ def run_ours(args, workload_name=None):
         kw = dict(epoch_Bmax=args.bmax, time_kernels=1 if timed else 0, walk_words=args.walk_words, no_hot_cells=1 if args.no_hot else 0)
         out = []
         sweep_kw = dict(mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=n_sweeps, **kw)
+        if args.carry and world == 1:
+            kw = dict(kw, carry_interactions=args.carry)
         if world > 1:
             multi.run_partitioned(ctx, n_packets, sd, peers=peers, want_stats=False, **kw)
             if timed:

@@ -81,6 +81,13 @@ typedef struct {
     int32_t walk_words;        /* launch tuning (results never depend on it): how the cell walk keeps its cell words
                                   in flight.  0 = auto (= 1), 1 = in registers, 2 = cp.async ring in shared memory
                                   (never measured faster; kept for such measurements) */
+    uint32_t carry_interactions; /* MCRT_MODE_BW_EPOCH: > 0 = a packet that has had this many interactions within one
+                                  epoch stops behind the last of them and continues in the next epoch, from the same
+                                  state and random stream, at that epoch's temperatures; packets still carried after
+                                  the last epoch run in further epochs, the budget doubling each time.  The
+                                  deterministic restatement of the pause / resume of PAPER.md:128-130 (paper: 100).
+                                  0 (default) = no limit.  <= 65535; not in partitioned runs.  The list of carried
+                                  packets is allocated with cudaMalloc (88 bytes per packet of an epoch). */
     int32_t no_hot_cells;      /* launch tuning: 1 = do not keep per-CTA copies of the tallies of the cells around the
                                   source (default 0: kept; the sums are integers, so results do not depend on it) */
 } mcrt_run_opts;

@@ -41,11 +41,20 @@ enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4,
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
 
 // device counters (unsigned long long each)
-enum : int { CNT_PACKETS = 0, CNT_CROSS, CNT_DUSTY, CNT_SCA, CNT_ABS, CNT_DIRECT, CNT_OVERFLOW, CNT_NEXT, CNT_N };
+enum : int { CNT_PACKETS = 0, CNT_CROSS, CNT_DUSTY, CNT_SCA, CNT_ABS, CNT_DIRECT, CNT_OVERFLOW, CNT_NEXT, CNT_CARRY, CNT_N };
 
 thread_local std::string g_create_error;
 
 }  // namespace
+
+// A packet carried over an epoch boundary (NEXT-1; PAPER.md:128-130 restated deterministically, reading Q23): after
+// carry_K interactions within one epoch a packet stops behind the carry_K-th (new direction and frequency drawn)
+// and continues in the next epoch from this state, with its own random stream, at that epoch's temperatures.
+struct CarryRec {
+    unsigned long long pid, hash;
+    double px, py, pz, ux, uy, uz;
+    uint32_t w0, j, d, ncross, nsca, nabs;
+};
 
 // ------------------------------------------------------------------------------------------------
 // context
@@ -99,6 +108,9 @@ struct mcrt_ctx {
     double xi = 0.0;
     uint64_t epochs = 0, launches = 0;
     uint64_t dig_base = 0;                // packet id of digest slot 0
+    CarryRec *carry_buf[2] = {nullptr, nullptr};   // carried packets: read by this epoch / written for the next (cudaMalloc)
+    size_t carry_cap[2] = {0, 0};
+    int carry_cur = 0;
     // run in progress (mcrt_run_begin .. mcrt_run_end)
     struct Run {
         bool active = false;
@@ -108,6 +120,8 @@ struct mcrt_ctx {
         size_t smem = 0;
         double cellfac = 0.0, prev_cellfac = 0.0, growth = 2.0;
         bool finished = false;            // every step has been issued
+        uint32_t carry_K = 0;             // interaction budget of the current epoch (0 = no carry-over)
+        uint64_t n_carry = 0;             // packets carried into the next epoch
         bool ringw = false;               // walk variant of this run
         bool hot = false;                 // hot cells tallied per CTA
     } run;
@@ -386,6 +400,9 @@ struct TransportParams {
     int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
     unsigned long long pid0, count, dig_base;
+    const CarryRec *__restrict__ carry_in;     // packets carried over from the previous epoch: taken before new ids
+    CarryRec *__restrict__ carry_out;          // packets whose budget runs out in this launch (counters[CNT_CARRY] of them)
+    uint32_t n_carry_in, carry_K;              // carry_K = 0: no budget
     uint32_t seed_lo, seed_hi, pass;
 };
 
@@ -772,7 +789,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         const double t = SF(F_T, slot);
                         tau = SF(F_TAU, slot);
                         const uint32_t w0 = SU(U_W0, slot);
-                        const int j = (int)SU(U_W1, slot);
+                        const int j = (int)(SU(U_W1, slot) & 0xffffu);   // (high half: interactions in this epoch)
                         ncross = SU(U_NCROSS, slot) - (uint32_t)(kDepth - 1);   // the no-op cells below count themselves
                         const int gx = unpack_x(w0), gy = unpack_y(w0), gz = unpack_z(w0);
                         // the stored 1/u is +inf for a zero direction component: that axis never moves
@@ -978,7 +995,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             uint32_t kind = act ? (SU(U_DK, slot) >> 30) : 3u;
             uint32_t d = SU(U_DK, slot) & 0x3fffffffu;
             unsigned long long pid = 0ull, hash = 0ull;
-            uint32_t ncross = 0u, nsca = 0u, nabs = 0u;
+            uint32_t ncross = 0u, nsca = 0u, nabs = 0u, nint = 0u;
             int ix = 0, iy = 0, iz = 0, j = 0;
             double ux = 0.0, uy = 0.0, uz = 1.0;
             if (act && kind != K_EMIT) {
@@ -986,7 +1003,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 if (RECORD) hash = (unsigned long long)__double_as_longlong(SF(F_HASH, slot));
                 ncross = SU(U_NCROSS, slot); nsca = SU(U_NSCA, slot); nabs = SU(U_NABS, slot);
                 const uint32_t w0 = SU(U_W0, slot);
-                ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0); j = (int)SU(U_W1, slot);
+                ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0);
+                j = (int)(SU(U_W1, slot) & 0xffffu); nint = SU(U_W1, slot) >> 16;
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
             }
             {   // run counters of the packets that escape in this phase: summed over the warp, then added to the warp's
@@ -1030,9 +1048,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             }
             // S0 refill: the slots that need a new packet take the next ids with ONE atomic per warp
             const unsigned need = __ballot_sync(kFull, kind == K_EMIT);
-            bool dead = false;
+            bool dead = false, resume = false;
+            const unsigned long long n_take = P.count + P.n_carry_in;   // carried packets first, then new ids
+            uint32_t resume_idx = 0u;
             if (need) {
-                unsigned long long base = P.count;
+                unsigned long long base = n_take;
                 if (!exhausted) {
                     const int leader = __ffs(need) - 1;
                     if (lane == leader) base = atomicAdd(&P.counters[CNT_NEXT], (unsigned long long)__popc(need));
@@ -1040,20 +1060,32 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 }
                 if (kind == K_EMIT) {
                     const unsigned long long idx = base + (unsigned long long)__popc(need & ((1u << lane) - 1u));
-                    if (idx < P.count) pid = P.pid0 + idx; else dead = true;
+                    if (idx < P.n_carry_in) { resume = true; resume_idx = (uint32_t)idx; }
+                    else if (idx < n_take) pid = P.pid0 + (idx - P.n_carry_in);
+                    else dead = true;
                 }
                 if (__any_sync(kFull, dead)) exhausted = true;   // the counter only grows
             }
             bool to_jump = false;                       // the new flight starts in an empty brick
+            bool carried = false;                       // the packet's budget of this epoch is used up: carried over
             if (act && !dead) {
                 double px, py, pz, z0, z1;
                 bool scatter = false;
                 int sj = 0;
                 unsigned long long cw;
                 uint32_t cidx;
-                if (kind == K_EMIT) {
+                if (resume) {
+                    // a packet carried over from the previous epoch: its state as it was left behind an interaction
+                    const CarryRec rc = P.carry_in[resume_idx];
+                    pid = rc.pid; hash = rc.hash; px = rc.px; py = rc.py; pz = rc.pz; ux = rc.ux; uy = rc.uy; uz = rc.uz;
+                    ix = unpack_x(rc.w0); iy = unpack_y(rc.w0); iz = unpack_z(rc.w0);
+                    j = (int)rc.j; d = rc.d; ncross = rc.ncross; nsca = rc.nsca; nabs = rc.nabs; nint = 0u;
+                    cidx = lin_index(ix, iy, iz, lpx, lpxy);
+                    to_jump = brick_empty(s_m0, brick_of(ix, iy, iz, nbx, nby, bsh));
+                    cw = to_jump ? 0ull : __ldg(P.cellw + (size_t)kCS * cidx);
+                } else if (kind == K_EMIT) {
                     // S2 emit: frequency through the source CDF (Eq. 1)
-                    d = 0u; ncross = 0u; nsca = 0u; nabs = 0u;
+                    d = 0u; ncross = 0u; nsca = 0u; nabs = 0u; nint = 0u;
                     hash = 0xCBF29CE484222325ull;
                     draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                     j = lower_bound_cdf(s_src, nf, z0);
@@ -1096,6 +1128,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
                     }
                 }
+                if (!resume) {
                 // new direction: isotropic or Henyey-Greenstein about the old one (S7)
                 draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                 double mu = 1.0 - 2.0 * z0;
@@ -1143,7 +1176,18 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     cw = to_jump ? 0ull : __ldg(P.cellw + (size_t)kCS * cidx);
                     if (RECORD)
                         hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
+                } else if (P.carry_K && ++nint >= P.carry_K) {
+                    // carry-over: the interaction budget of this epoch is used up.  The packet's state goes to the
+                    // list the next epoch starts with; the slot takes another packet.
+                    carried = true;
+                    CarryRec rc;
+                    rc.pid = pid; rc.hash = hash; rc.px = px; rc.py = py; rc.pz = pz; rc.ux = ux; rc.uy = uy; rc.uz = uz;
+                    rc.w0 = pack_xyz(ix, iy, iz); rc.j = (uint32_t)j; rc.d = d; rc.ncross = ncross; rc.nsca = nsca; rc.nabs = nabs;
+                    P.carry_out[atomicAdd(&P.counters[CNT_CARRY], 1ull)] = rc;
+                    SU(U_DK, slot) = K_EMIT << 30;
                 }
+                }   // !resume
+                if (!carried) {
                 // S3 optical depth of the flight: tau = -ln zeta, zeta_1 kept for S6
                 draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                 // park the new flight (reading Q8: the walk needs p, 1/u, the cell; t = 0)
@@ -1163,11 +1207,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 SU(U_DK, slot) = d;    // kind is set when the walk stops
                 SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
                 SU(U_W0, slot) = pack_xyz(ix, iy, iz);
-                SU(U_W1, slot) = (uint32_t)j;
+                SU(U_W1, slot) = (uint32_t)j | (nint << 16);
+                }   // !carried
             }
-            mEv.remove(act, slot);                         // taken: now flying, jumping, or dead (no packets left)
-            mFly.add(act && !dead && !to_jump, slot);
-            mJ.add(act && !dead && to_jump, slot);
+            mEv.remove(act && !carried, slot);             // taken: now flying, jumping, or dead (no packets left)
+            mFly.add(act && !dead && !to_jump && !carried, slot);
+            mJ.add(act && !dead && to_jump && !carried, slot);
             __syncwarp();
         } else {
             break;
@@ -1226,7 +1271,7 @@ __global__ void __launch_bounds__(256) k_epoch_update(unsigned long long *__rest
     extern __shared__ double s_J[];
     for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
     __syncthreads();
-    if (blockIdx.x == 0 && threadIdx.x == 0) counters[CNT_NEXT] = 0ull;
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters[CNT_NEXT] = 0ull; counters[CNT_CARRY] = 0ull; }
     bool ovf = false;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
         const unsigned long long cw = cellw[kCS * i];
@@ -2207,6 +2252,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         return fail(c, MCRT_EINVAL, "part_index must be in 0..part_count-1");
     if (o.part_count <= 1) { o.part_count = 1; o.part_index = 0; }
     if (o.epoch_growth == 0.0) o.epoch_growth = 2.0;
+    if (o.carry_interactions > 65535u) return fail(c, MCRT_EINVAL, "carry_interactions must be <= 65535");
+    if (o.carry_interactions && o.part_count > 1) return fail(c, MCRT_EINVAL, "carry_interactions is not available in a partitioned run");
     if (o.walk_words < 0 || o.walk_words > 2) return fail(c, MCRT_EINVAL, "walk_words must be 0 (auto), 1 (registers) or 2 (ring)");
     if (!(o.epoch_growth >= 1.0) || !isfinite(o.epoch_growth)) return fail(c, MCRT_EINVAL, "epoch_growth must be >= 1");
     if (o.n_total && o.n_total < n_packets) return fail(c, MCRT_EINVAL, "n_total must be >= n_packets");
@@ -2269,6 +2316,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         CUDA_TRY(c, cudaFuncSetAttribute(k_sweep_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
     }
     R.o = o; R.n = n_packets; R.seed = seed; R.done = 0; R.Bprev = 0; R.e = 0; R.sweep = 0; R.finished = false;
+    R.carry_K = (o.mode == MCRT_MODE_BW_EPOCH) ? o.carry_interactions : 0u; R.n_carry = 0;
     R.growth = o.epoch_growth;
     uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
     schedule_defaults(n_packets, &B0, &Bmax, &R.growth);
@@ -2294,26 +2342,54 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
     fill_params(c, P);
     uint64_t lo, hi;
     if (o.mode == MCRT_MODE_BW_EPOCH) {
-        const uint64_t Be = (R.n - R.done < R.Bnom) ? R.n - R.done : R.Bnom;
+        // an epoch of new packets, or -- all new packets done, some still carried -- an epoch of carried packets only,
+        // with the budget doubled (see CarryRec)
+        const bool drain = R.done >= R.n;
+        const uint64_t Be = drain ? 0 : ((R.n - R.done < R.Bnom) ? R.n - R.done : R.Bnom);
+        if (drain) R.carry_K = R.carry_K > 0x40000000u ? 0x80000000u : 2u * R.carry_K;
         P.cdf = c->d_cdfdB;
         P.pass = o.rng_pass;
+        if (R.carry_K) {
+            // room for every packet of this epoch in the list it may leave behind
+            const int out = c->carry_cur ^ 1;
+            const size_t need = (size_t)(R.n_carry + Be);
+            if (c->carry_cap[out] < need) {
+                if (c->carry_buf[out]) { CUDA_TRY(c, cudaStreamSynchronize(c->stream)); cudaFree(c->carry_buf[out]); c->carry_buf[out] = nullptr; c->carry_cap[out] = 0; }
+                const size_t cap = need + need / 4 + 1024;
+                if (cudaMalloc((void **)&c->carry_buf[out], cap * sizeof(CarryRec)) != cudaSuccess)
+                    return fail(c, MCRT_ENOMEM, "cudaMalloc of the carry-over list failed");
+                c->carry_cap[out] = cap;
+            }
+            P.carry_in = c->carry_buf[c->carry_cur]; P.carry_out = c->carry_buf[out];
+            P.n_carry_in = (uint32_t)R.n_carry; P.carry_K = R.carry_K;
+        }
         mark(c, timing);
         k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
-                                                         R.e == 0, R.e == 0 ? 1.0 : (double)Be / (double)R.Bprev,
+                                                         R.e == 0, (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev,
                                                          R.cellfac, c->counters, c->tidx_mask);
         part_slice(o, Be, &lo, &hi);
         P.pid0 = o.first_packet_id + R.done + lo; P.count = hi - lo;
         mark(c, timing);
-        if (P.count) {
+        if (P.count + P.n_carry_in) {
             launch_transport(c, P);
         }
         mark(c, timing);
-        c->launches += P.count ? 2 : 1;
+        c->launches += (P.count + P.n_carry_in) ? 2 : 1;
         c->epochs++;
-        R.done += Be; R.Bprev = Be;
-        R.Bnom = next_epoch_size(R.Bnom, R.Bmax, R.growth);
+        if (!drain) {
+            R.done += Be; R.Bprev = Be;
+            R.Bnom = next_epoch_size(R.Bnom, R.Bmax, R.growth);
+        }
         ++R.e;
-        R.finished = R.done >= R.n;
+        if (R.carry_K) {
+            // how many packets were carried over: needed to size the next launch (8-byte read, synchronises)
+            unsigned long long nc_ = 0ull;
+            CUDA_TRY(c, cudaMemcpyAsync(&nc_, c->counters + CNT_CARRY, 8, cudaMemcpyDeviceToHost, c->stream));
+            CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+            R.n_carry = nc_;
+            c->carry_cur ^= 1;
+        }
+        R.finished = R.done >= R.n && R.n_carry == 0;
     } else {
         const int sw = ++R.sweep;
         P.cdf = c->d_cdfB;
@@ -2599,6 +2675,7 @@ void mcrt_destroy(mcrt_ctx *c)
     cudaStreamSynchronize(c->stream);
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     for (void *p : c->owned) cudaFree(p);
+    for (int i = 0; i < 2; ++i) if (c->carry_buf[i]) cudaFree(c->carry_buf[i]);
     delete c;
 }
 

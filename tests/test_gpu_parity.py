@@ -35,7 +35,7 @@ RAW_KEYS = ("k", "lucy_fx", "sed", "sed_direct", "tidx")
 
 
 def _run_both(orc, B, w, N, seed, mode=0, n_sweeps=0, from_lucy=1, B0=0, Bmax=0, grid_blocks=0, block_threads=0,
-              growth=0.0, N_first=None, plain=True):
+              growth=0.0, N_first=None, plain=True, carry_K=0):
     """Oracle and CUDA path on the same inputs.  The CUDA path runs twice: recording per-packet digests
     (k_transport<true>) and -- `plain` -- as bench.py runs it (k_transport<false>, another instantiation with
     another pool slot layout); the second run's raw tallies and counters are kept in rg["plain"]."""
@@ -45,8 +45,8 @@ def _run_both(orc, B, w, N, seed, mode=0, n_sweeps=0, from_lucy=1, B0=0, Bmax=0,
     if mode == 1:  # sweeps start from the temperatures of a B&W pass (possibly of another N)
         o.run(N1, seed, n_threads=NTH)
     ro = o.run(N, seed, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, B0=B0, Bmax=Bmax, digests=True,
-               n_threads=NTH, growth=growth)
-    kw = dict(mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, epoch_B0=B0, epoch_Bmax=Bmax,
+               n_threads=NTH, growth=growth, carry_K=carry_K)
+    kw = dict(carry_interactions=carry_K, mode=mode, n_sweeps=n_sweeps, sweep_T_from_lucy=from_lucy, epoch_B0=B0, epoch_Bmax=Bmax,
               grid_blocks=grid_blocks, block_threads=block_threads, epoch_growth=growth)
     plain_res = None
     if plain:
@@ -525,6 +525,26 @@ def test_partitioned_run_is_bit_identical(B, orc, n_parts):
     assert e.value.code == B.MCRT_ESTATE
     for c in parts + [single]:
         c.close()
+
+
+@pytest.mark.parametrize("kind,K,blocks", [("grey", 100, 0), ("chromatic", 30, 0), ("chromatic", 7, 2), ("torus", 3, 0)])
+def test_parity_carry_over_of_long_lived_packets(B, orc, kind, K, blocks):
+    """NEXT-1 (deterministic restatement; oracle pin P19): packets are carried over epoch
+    boundaries after K interactions within one epoch and drained in further epochs -- event sequences, tallies,
+    temperature indices and the number of epochs bit-equal to the oracle's, in both kernel instantiations."""
+    if kind == "grey":
+        w, N = W.uniform_cube(10, 20.0, 0.6, 0.3, n_nu=32, slope=0.0, T_star=3000.0), 20_000
+    elif kind == "chromatic":
+        w, N = W.uniform_cube(10, 40.0, 0.6, 0.3, n_nu=32, slope=-0.3, T_star=3000.0), 30_000
+    else:
+        w, N = W.torus256(n_clumps=400, n=64), 150_000
+    o, c, ro, rg = _run_both(orc, B, w, N, 19, carry_K=K, grid_blocks=blocks, block_threads=64 if blocks else 0)
+    assert _assert_parity(o, c, ro, rg, w, N) == 1.0
+    assert rg["epochs"] == ro["epochs"]
+    ref = orc.Oracle.from_workload(w)
+    r0 = ref.run(N, 19, n_threads=NTH)
+    assert ro["epochs"] > r0["epochs"]          # packets were carried and drained in further epochs
+    c.close()
 
 
 @pytest.mark.parametrize("walk_words", [1, 2])
