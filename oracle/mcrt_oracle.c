@@ -475,6 +475,15 @@ typedef struct {
     uint32_t carry_K;        /* > 0: a packet is carried over to the next epoch after this many interactions in one epoch */
 } orc_opts;
 
+/* One stored scattering event ("The index of the cell, the frequency of the scattered photon and the
+ * incoming direction is stored"): cell in [nz][ny][nx] order, slot of the frequency bin among the recorded ones,
+ * incoming direction quantised to 16 bits per component, q_a = rint(32767 u_a). */
+typedef struct orc_sca_event_s {
+    uint32_t cell;
+    uint16_t slot;
+    int16_t q[3];
+} orc_sca_event;
+
 /* A packet carried over an epoch boundary: everything its continuation depends on.  The paper pauses packets with
  * more than 100 interactions in one cell once 80 % of the threads have finished, stores position and frequency and
  * resumes them at the end; which packets that hits depends on scheduling.  The deterministic
@@ -505,6 +514,10 @@ typedef struct {
     uint64_t pid0_digest;
     uint32_t carry_K;        /* interaction budget of the current epoch (0 = none) */
     const orc_opts *o;
+    /* scattering-event store: slot of each frequency bin (-1 = not recorded), list, fill count */
+    const int32_t *sca_slot;
+    struct orc_sca_event_s *sca_ev;
+    uint64_t sca_cap, *sca_n;
 } orc_run_t;
 
 static inline void hash_mix(uint64_t *h, uint64_t w)
@@ -624,6 +637,14 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
             orc_uniforms(R->seed, pid, d++, R->pass, z);
             double un[3];
             orc_hg_scatter(C->g[sj], z[0], z[1], u, un);
+            if (R->sca_slot && R->sca_slot[j] >= 0) {   /* store the event: cell, frequency, incoming direction */
+                uint64_t at = __atomic_fetch_add(R->sca_n, (uint64_t)1, __ATOMIC_RELAXED);
+                if (at < R->sca_cap) {
+                    orc_sca_event *ev = &R->sca_ev[at];
+                    ev->cell = (uint32_t)ci; ev->slot = (uint16_t)R->sca_slot[j];
+                    for (int a = 0; a < 3; ++a) ev->q[a] = (int16_t)llrint(32767.0 * u[a]);
+                }
+            }
             u[0] = un[0]; u[1] = un[1]; u[2] = un[2];
             nsca++;
             st->scatterings++;
@@ -773,6 +794,11 @@ typedef struct {
     uint64_t *sed, *sed_direct;
     int fx;
     double xi;               /* packet energy L/N of the run that produced the stored tallies */
+    int32_t *sca_slot;       /* [nf] slot of a recorded frequency bin, -1 otherwise; NULL = nothing is recorded */
+    int n_sca_bins;
+    int32_t sca_bins[16];
+    orc_sca_event *sca_ev;
+    uint64_t sca_cap, sca_n;
 } orc_state;
 
 orc_state *orc_state_create(const orc_ctx *C)
@@ -793,7 +819,7 @@ void orc_state_destroy(orc_state *S)
 {
     if (!S) return;
     free(S->k); free(S->kprev); free(S->Lfx); free(S->Lsum); free(S->Lcmp); free(S->tidx);
-    free(S->sed); free(S->sed_direct); free(S);
+    free(S->sed); free(S->sed_direct); free(S->sca_slot); free(S->sca_ev); free(S);
 }
 
 static void zero_tallies(orc_state *S)
@@ -804,6 +830,7 @@ static void zero_tallies(orc_state *S)
     if (S->Lsum) { memset(S->Lsum, 0, S->nc * sizeof(double)); memset(S->Lcmp, 0, S->nc * sizeof(double)); }
     memset(S->sed, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
     memset(S->sed_direct, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
+    S->sca_n = 0;
 }
 
 /* fixed-point fraction bits (O9): FX = min(40, 58 - ceil(log2 N)) */
@@ -903,6 +930,7 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
     R.Lsum = o->keep_fp64_lucy ? S->Lsum : NULL; R.Lcmp = S->Lcmp;
     R.sed = S->sed; R.sed_direct = S->sed_direct; R.dig = digests; R.seed = seed; R.fx = S->fx; R.o = o;
     R.pid0_digest = o->pid0;
+    R.sca_slot = S->sca_slot; R.sca_ev = S->sca_ev; R.sca_cap = S->sca_cap; R.sca_n = &S->sca_n;
     R.kabs_fx = (double *)malloc(nsf * sizeof(double));
     for (size_t i = 0; i < nsf; ++i) R.kabs_fx[i] = ldexp(C->kabs_h[i], S->fx);
     st.fx_bits = S->fx;
@@ -1027,6 +1055,144 @@ void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int
                 double dom = ORC_FOUR_PI * (C->mu_edges[b + 1] - C->mu_edges[b]);
                 SED[(size_t)b * C->nf + j] = (double)S->sed[(size_t)b * C->nf + j] * S->xi / (C->dnu[j] * dom);
             }
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * NEXT-2  Scattering-event store and ray tracer (Sect. 4, Eq. 11-17).
+ * ---------------------------------------------------------------------------------------------- */
+/* record the scattering events of later runs at these frequency bins (at most 16), up to `capacity` events */
+int orc_scatter_store(orc_state *S, int n_bins, const int32_t *bins, uint64_t capacity)
+{
+    if (n_bins < 1 || n_bins > 16) return -1;
+    free(S->sca_slot); free(S->sca_ev);
+    S->sca_slot = (int32_t *)malloc(S->C->nf * sizeof(int32_t));
+    for (int j = 0; j < S->C->nf; ++j) S->sca_slot[j] = -1;
+    for (int b = 0; b < n_bins; ++b) {
+        if (bins[b] < 0 || bins[b] >= S->C->nf) return -1;
+        S->sca_slot[bins[b]] = b; S->sca_bins[b] = bins[b];
+    }
+    S->n_sca_bins = n_bins;
+    S->sca_ev = (orc_sca_event *)malloc((capacity ? capacity : 1) * sizeof(orc_sca_event));
+    S->sca_cap = capacity; S->sca_n = 0;
+    return 0;
+}
+
+uint64_t orc_scatter_events(const orc_state *S, orc_sca_event *out, uint64_t max_n)
+{
+    uint64_t n = S->sca_n < S->sca_cap ? S->sca_n : S->sca_cap;
+    if (out) memcpy(out, S->sca_ev, (size_t)(n < max_n ? n : max_n) * sizeof(orc_sca_event));
+    return S->sca_n;
+}
+
+/* Henyey-Greenstein phase function, per steradian (Eq. 15) */
+double orc_phase_hg(double g, double cos_beta)
+{
+    double d = 1.0 + g * g - 2.0 * g * cos_beta;
+    return (1.0 - g * g) / (ORC_FOUR_PI * d * sqrt(d));
+}
+
+/* The image of Sect. 4 at frequency bin j for an observer in direction ez (unit vector from the object towards the
+ * observer) at distance D, parallel projection (Eq. 11): pixel (a, b) of nx x ny pixels of size pix looks along the
+ * line r = i0 + (a + 1/2 - nx/2) pix ex + (b + 1/2 - ny/2) pix ey + s ez, i0 = centre of the grid, ey = ez x ex.
+ * Along the line, from the observer's side inwards, every cell i adds (Eq. 12, 17)
+ *     A_pix / D^2 * (I_e + I_s) * exp(-tau),   tau = sum of the tau_cell of the cells between i and the observer,
+ *     tau_cell = kappa_abs rho l (Eq. 13: absorption cross section, as printed), l = length of the line inside the cell,
+ *     I_e = (1 - exp(-tau_cell)) B_nu(T_i)                                            (Eq. 14)
+ *     I_s = l / V * sum over the cell's stored events of P_HG(beta) xi / dnu           (Eq. 16)
+ * with beta the angle between ez and the event's incoming direction, V = h^3 (the events' scattered luminosity per
+ * steradian towards the observer, spread over the cell's volume -- reading Q30: Eq. 16 gives no normalisation).
+ * T_i inverts Eq. 4 from the counts (T_from_lucy = 0) or the Lucy tally (1).  Fe / Fs: [ny][nx], erg s^-1 cm^-2 Hz^-1. */
+int orc_ray_trace(const orc_state *S, const double ez_in[3], const double ex_in[3], int nx, int ny, double pix, double D,
+                  int j, int T_from_lucy, double *Fe, double *Fs)
+{
+    const orc_ctx *C = S->C;
+    if (j < 0 || j >= C->nf || nx < 1 || ny < 1 || !(pix > 0.0) || !(D > 0.0)) return -1;
+    const int n[3] = { C->nx, C->ny, C->nz };
+    double ez[3], ex[3], ey[3];
+    double nz_ = sqrt(ez_in[0] * ez_in[0] + ez_in[1] * ez_in[1] + ez_in[2] * ez_in[2]);
+    for (int a = 0; a < 3; ++a) ez[a] = ez_in[a] / nz_;
+    double dot = ex_in[0] * ez[0] + ex_in[1] * ez[1] + ex_in[2] * ez[2];
+    for (int a = 0; a < 3; ++a) ex[a] = ex_in[a] - dot * ez[a];
+    double nx_ = sqrt(ex[0] * ex[0] + ex[1] * ex[1] + ex[2] * ex[2]);
+    if (!(nx_ > 0.0)) return -1;
+    for (int a = 0; a < 3; ++a) ex[a] /= nx_;
+    ey[0] = ez[1] * ex[2] - ez[2] * ex[1]; ey[1] = ez[2] * ex[0] - ez[0] * ex[2]; ey[2] = ez[0] * ex[1] - ez[1] * ex[0];
+    /* per-cell sum of P_HG(beta) over the stored events of this frequency (the sum over beta of Eq. 16) */
+    size_t nc = S->nc;
+    double *src = (double *)calloc(nc, sizeof(double));
+    int slot = (S->sca_slot) ? S->sca_slot[j] : -1;
+    if (slot >= 0) {
+        uint64_t ne = S->sca_n < S->sca_cap ? S->sca_n : S->sca_cap;
+        for (uint64_t e = 0; e < ne; ++e) {
+            const orc_sca_event *ev = &S->sca_ev[e];
+            if (ev->slot != slot) continue;
+            double qx = ev->q[0], qy = ev->q[1], qz = ev->q[2];
+            double qn = sqrt(qx * qx + qy * qy + qz * qz);
+            double cb = (qx * ez[0] + qy * ez[1] + qz * ez[2]) / qn;
+            src[ev->cell] += orc_phase_hg(C->g[C->sp[ev->cell] * C->nf + j], cb);
+        }
+    }
+    const double inv_fx = ldexp(1.0, -S->fx);
+    const double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h);
+    const double apix_d2 = pix * pix / (D * D);
+    const double V = C->h * C->h * C->h;
+    const double u[3] = { -ez[0], -ez[1], -ez[2] };     /* the walk runs from the observer's side inwards */
+    for (int b = 0; b < ny; ++b)
+        for (int a = 0; a < nx; ++a) {
+            double fe = 0.0, fs = 0.0;
+            /* point of the line in cell units, then the slab parameters at which it is inside the grid */
+            double r0[3], smin = -INFINITY, smax = INFINITY;
+            double xa = ((double)a + 0.5 - 0.5 * nx) * pix / C->h, yb = ((double)b + 0.5 - 0.5 * ny) * pix / C->h;
+            for (int q = 0; q < 3; ++q) r0[q] = 0.5 * n[q] + xa * ex[q] + yb * ey[q];
+            int miss = 0;
+            for (int q = 0; q < 3; ++q) {
+                if (u[q] == 0.0) { if (!(r0[q] > 0.0 && r0[q] < (double)n[q])) miss = 1; continue; }
+                double s1 = (0.0 - r0[q]) / u[q], s2 = ((double)n[q] - r0[q]) / u[q];
+                double lo = s1 < s2 ? s1 : s2, hi = s1 < s2 ? s2 : s1;
+                if (lo > smin) smin = lo;
+                if (hi < smax) smax = hi;
+            }
+            if (!miss && smax > smin) {
+                double p[3];
+                int c[3];
+                for (int q = 0; q < 3; ++q) {
+                    p[q] = r0[q] + smin * u[q];
+                    if (p[q] < 0.0) p[q] = 0.0;
+                    if (p[q] > (double)n[q]) p[q] = (double)n[q];
+                }
+                start_cell(p, u, c);
+                int inside = 1;
+                for (int q = 0; q < 3; ++q) if (c[q] < 0 || c[q] >= n[q]) inside = 0;
+                if (inside) {
+                    orc_dda Dd;
+                    dda_setup(&Dd, p, u, c);
+                    double t = 0.0, tau = 0.0;
+                    for (;;) {
+                        int ax = dda_axis(&Dd);
+                        double tn = Dd.tmax[ax], l = (tn - t) * C->h;
+                        size_t ci = ((size_t)c[2] * n[1] + c[1]) * n[0] + c[0];
+                        double rho_c = (double)C->rho[ci];
+                        if (rho_c > 0.0) {
+                            int sp = C->sp[ci];
+                            double tc = C->kabs[sp * C->nf + j] * rho_c * l;
+                            double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+                            double T = orc_T_of_x(C, sp, e * cellfac / rho_c);
+                            double att = exp(-tau);
+                            if (T > 0.0) fe += -expm1(-tc) * orc_planck(C->nu[j], T) * att;
+                            fs += l / V * src[ci] * S->xi / C->dnu[j] * att;
+                            tau += tc;
+                        }
+                        t = tn;
+                        dda_advance(&Dd, ax, c);
+                        if (c[ax] < 0 || c[ax] >= n[ax]) break;
+                    }
+                }
+            }
+            Fe[(size_t)b * nx + a] = fe * apix_d2;
+            if (Fs) Fs[(size_t)b * nx + a] = fs * apix_d2;
+        }
+    free(src);
+    return 0;
 }
 
 int orc_max_threads(void)

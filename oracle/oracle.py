@@ -37,6 +37,8 @@ class Opts(C.Structure):
                 ("pass0", C.c_uint32), ("pid0", C.c_uint64), ("n_total", C.c_uint64), ("growth", C.c_double), ("carry_K", C.c_uint32)]
 
 
+SCA_EVENT_DTYPE = np.dtype([("cell", np.uint32), ("slot", np.uint16), ("q", np.int16, (3,))])
+
 DIGEST_DTYPE = np.dtype([("hash", np.uint64), ("crossings", np.uint32), ("scatterings", np.uint32),
                          ("absorptions", np.uint32), ("escape_bin", np.uint32)])
 
@@ -85,6 +87,15 @@ def lib():
         L.orc_det_log.argtypes = [C.c_double]
         L.orc_det_sincos.argtypes = [C.c_double, C.c_void_p, C.c_void_p]
         L.orc_max_threads.restype = C.c_int
+        L.orc_scatter_store.restype = C.c_int
+        L.orc_scatter_store.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_uint64]
+        L.orc_scatter_events.restype = C.c_uint64
+        L.orc_scatter_events.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64]
+        L.orc_phase_hg.restype = C.c_double
+        L.orc_phase_hg.argtypes = [C.c_double, C.c_double]
+        L.orc_ray_trace.restype = C.c_int
+        L.orc_ray_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_int,
+                                    C.c_int, C.c_void_p, C.c_void_p]
         _lib = L
     return _lib
 
@@ -167,6 +178,10 @@ def default_schedule(n):
     b = np.zeros(2, np.uint64)
     lib().orc_default_schedule(int(n), _p(b[0:1]), _p(b[1:2]))
     return int(b[0]), int(b[1])
+
+
+def phase_hg(g, cos_beta):
+    return lib().orc_phase_hg(float(g), float(cos_beta))
 
 
 def max_threads():
@@ -256,6 +271,26 @@ class Oracle:
         if fp64_lucy:
             out["lucy_fp64"] = Ls
         return out
+
+    def scatter_store(self, nu_bins, capacity):
+        b = np.ascontiguousarray(nu_bins, np.int32)
+        rc = lib().orc_scatter_store(self._state, len(b), _p(b), int(capacity))
+        assert rc == 0
+        self._sca_cap = int(capacity)
+
+    def scatter_events(self):
+        ev = np.zeros(self._sca_cap, SCA_EVENT_DTYPE)
+        n = lib().orc_scatter_events(self._state, _p(ev), self._sca_cap)
+        return ev[:min(n, self._sca_cap)], int(n)
+
+    def ray_trace(self, e_z, e_x, nx, ny, pixel_cm, distance_cm, nu_bin, T_from_lucy=False):
+        ez = np.ascontiguousarray(e_z, np.float64)
+        ex = np.ascontiguousarray(e_x, np.float64)
+        Fe, Fs = np.zeros((ny, nx)), np.zeros((ny, nx))
+        rc = lib().orc_ray_trace(self._state, _p(ez), _p(ex), int(nx), int(ny), float(pixel_cm), float(distance_cm),
+                                 int(nu_bin), int(T_from_lucy), _p(Fe), _p(Fs))
+        assert rc == 0
+        return Fe, Fs
 
     def read(self, T_from_lucy=False):
         Ec = np.zeros(self.nc)

@@ -739,3 +739,133 @@ def test_p19_carry_over_of_long_lived_packets(orc):
     ba, bb = sa.reshape(8, 4).sum(axis=1), sb.reshape(8, 4).sum(axis=1)
     sel = ba > 300
     assert sel.sum() >= 3 and np.all(np.abs(bb[sel] / ba[sel] - 1) < 0.03 + 3 / np.sqrt(ba[sel]))
+
+
+# ------------------------------------------------------------------------------------------ P20 scattering store + ray tracer
+def _bin_edges(nu):
+    return np.concatenate([[nu[0] * math.sqrt(nu[0] / nu[1])], np.sqrt(nu[:-1] * nu[1:]), [nu[-1] * math.sqrt(nu[-1] / nu[-2])]])
+
+
+def test_p20_phase_function_and_event_store(orc):
+    """NEXT-2 (Eq. 15-16).  P_HG is normalised over the sphere and 1/4pi for g = 0; with every frequency
+    bin recorded the store holds exactly one event per scattering, in dusty cells, with unit incoming directions."""
+    mu = (np.arange(4000) + 0.5) / 4000 * 2 - 1
+    for g in (0.0, 0.3, -0.5, 0.8):
+        p = np.array([orc.phase_hg(g, m) for m in mu])
+        assert abs(2 * math.pi * p.mean() * 2 - 1) < 1e-4
+    assert abs(orc.phase_hg(0.0, 0.3) - 1 / (4 * math.pi)) < 1e-16
+    assert abs(orc.phase_hg(0.6, 1.0) / orc.phase_hg(0.6, -1.0) - ((1 + 0.6) / (1 - 0.6)) ** 3) < 1e-9
+    w = W.uniform_cube(8, 2.0, 0.7, 0.4, n_nu=12, slope=-1.0)
+    o = orc.Oracle.from_workload(w)
+    o.scatter_store(list(range(12)), 400_000)
+    r = o.run(30_000, 20, n_threads=NTH)
+    ev, n = o.scatter_events()
+    assert n == r["scatterings"] == len(ev)
+    assert np.all(w.rho.reshape(-1)[ev["cell"]] > 0) and ev["slot"].max() < 12
+    qn = np.sqrt((ev["q"].astype(np.float64) ** 2).sum(axis=1))
+    assert np.all(np.abs(qn / 32767.0 - 1) < 1e-4)
+    # the next B&W run starts an empty store; a store with too little room counts what it could not keep
+    busiest = int(np.bincount(ev["slot"], minlength=12).argmax())
+    o.scatter_store([busiest], 10)
+    r = o.run(30_000, 20, n_threads=NTH)
+    ev, n = o.scatter_events()
+    assert len(ev) == 10 and 10 < n < r["scatterings"] and np.all(ev["slot"] == 0)
+
+
+def test_p20_ray_tracer_emission(orc):
+    """Eq. 12-14, 17.  (a) Optically thin dust in radiative equilibrium re-radiates what it absorbs: summed over
+    frequency and over the image, D^2 sum F_e dnu = sum_i E_i / 4 pi (Eq. 4 makes sum_j kappa_j B_j(T_i) dnu_j =
+    E_i / 4 pi rho V), whatever the direction of the observer.  (b) An opaque cube shows the Planck function
+    of the temperature of the cells on the OBSERVER's side (source off-centre, so the two sides differ)."""
+    n = 12
+    lam = W.wavelength_grid_um(24, 0.3, 3000.0)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = 50.0 * (nu / nu[-1]) ** 1.0
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    rho = np.where(r < n / 2, 2e-3 / (kabs.max() * n / 2 * h), 0.0).astype(np.float32)
+    c = n / 2 * h
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 1, nu, kabs[None], np.zeros((1, len(nu))),
+                   np.zeros((1, len(nu))), W.temperature_grid(1000, 2.0, 2000.0), W.LSUN_ERG_S, 3000.0, None, [c, c, c], [0.0, 1.0])
+    N = 400_000
+    o.run(N, 21, n_threads=NTH)
+    E_abs = o.read()["E_lucy"].sum()           # absorbed luminosity (path-length estimate: smooth in thin dust)
+    dnu = np.diff(_bin_edges(nu))
+    D, npx = 3.0e18, 88            # pixels of a quarter cell (the image covers the cube seen from any side)
+    for ez, ex in (((0.0, 0.0, 1.0), (1.0, 0.0, 0.0)), ((0.6, -0.48, 0.64), (0.0, 0.8, 0.6))):
+        tot = 0.0
+        for j in range(len(nu)):
+            Fe, Fs = o.ray_trace(ez, ex, npx, npx, h / 4, D, j, T_from_lucy=True)
+            assert np.all(Fs == 0.0) and np.all(Fe >= 0.0)
+            tot += Fe.sum() * dnu[j]
+        assert abs(tot * D * D / (E_abs / (4 * math.pi)) - 1) < 0.02, (ez, tot)
+    # (b) a cube that is opaque at the traced (shortest) wavelength and thin in the infrared, source off-centre along x
+    w = W.uniform_cube(6, 60.0, 0.0, 0.0, n_nu=16, slope=-1.5, T_star=4000.0, source_offset_cells=(1.5, 0.0, 0.0))
+    o2 = orc.Oracle.from_workload(w)
+    o2.run(100_000, 22, n_threads=NTH)
+    T = o2.read()["T"].reshape(6, 6, 6).astype(np.float64)
+    j = 15
+    assert w.kappa_abs[0, j] * float(w.rho.flat[0]) * w.cell_size_cm > 100.0
+    pix = w.cell_size_cm
+    for ez, face in (((1.0, 0.0, 0.0), T[:, :, 5]), ((-1.0, 0.0, 0.0), T[:, :, 0])):
+        Fe, _ = o2.ray_trace(ez, (0.0, 1.0, 0.0), 6, 6, pix, D, j)
+        # image axes: e_x' = +y, e_y' = e_z' x e_x' = +-z: pixel (a, b) looks at cell (y = a, z = b or 5 - b)
+        want = np.array([[orc.planck(w.nu_hz[j], face[b if ez[0] > 0 else 5 - b, a]) for a in range(6)] for b in range(6)])
+        np.testing.assert_allclose(Fe * D * D / pix ** 2, want, rtol=2e-3)     # (T is read back as fp32; h nu / k T is several hundred here)
+    assert abs(T[:, :, 5].mean() / T[:, :, 0].mean() - 1) > 0.02          # the two sides do differ
+
+
+def test_p20_ray_tracer_scattering(orc):
+    """Eq. 15-17.  (a) A pure scatterer neither absorbs nor attenuates (Eq. 13 has the absorption cross section), so
+    every stored event sends xi P_HG / dnu per steradian to the observer: for g = 0 the image sums to
+    N xi / (4 pi dnu D^2), N = number of stored events, for any direction.  (b) Two small clouds in front of and
+    behind the source as seen by the observer: per event, forward / backward scattering = ((1+g)/(1-g))^3."""
+    n, D = 10, 3.0e18
+    w = W.uniform_cube(n, 0.3, 1.0 - 1e-12, 0.0, n_nu=8, slope=0.0, T_star=5000.0)
+    o = orc.Oracle.from_workload(w)
+    j = 5                                  # 1.4 um: near the peak of the 5000 K source on this 8-point grid
+    o.scatter_store([j], 2_000_000)
+    N = 300_000
+    r = o.run(N, 23, n_threads=NTH)
+    ev, ne = o.scatter_events()
+    assert ne == len(ev) > 5000 and r["absorptions"] == 0
+    xi = w.L_erg_s / N
+    dnu = np.diff(_bin_edges(w.nu_hz))
+    npx = 72
+    for ez, ex in (((0.0, 0.0, 1.0), (1.0, 0.0, 0.0)), ((0.48, 0.6, -0.64), (0.8, 0.0, 0.6))):
+        Fe, Fs = o.ray_trace(ez, ex, npx, npx, w.cell_size_cm / 4, D, j)
+        assert np.all(Fe == 0.0)
+        assert abs(Fs.sum() / (ne * xi / (4 * math.pi * dnu[j] * D * D)) - 1) < 0.01
+    # (b)
+    g = 0.6
+    w2 = W.uniform_cube(15, 1.0, 1.0 - 1e-12, g, n_nu=8, slope=0.0, T_star=5000.0)
+    rho0 = w2.rho.max()
+    w2.rho[...] = 0.0
+    w2.rho[7, 7, 13] = rho0 * 0.5      # between the source (centre of cell 7,7,7) and an observer at +x
+    w2.rho[7, 7, 1] = rho0 * 0.5       # behind the source
+    o2 = orc.Oracle.from_workload(w2)
+    o2.scatter_store([j], 1_000_000)
+    o2.run(3_000_000, 24, n_threads=NTH)
+    ev, ne = o2.scatter_events()
+    cell_near, cell_far = (7 * 15 + 7) * 15 + 13, (7 * 15 + 7) * 15 + 1
+    n_near, n_far = int((ev["cell"] == cell_near).sum()), int((ev["cell"] == cell_far).sum())
+    assert n_near > 150 and n_far > 150 and n_near + n_far == ne
+    npx = 60
+    Fe, Fs = o2.ray_trace((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), npx, npx, 15 * w2.cell_size_cm / npx, D, j)
+    # parallel projection along x: both clouds fall on the same pixels, so separate them by tracing each alone
+    keep = w2.rho.copy()
+    per = {}
+    for name, cell in (("near", (7, 7, 13)), ("far", (7, 7, 1))):
+        w3 = W.uniform_cube(15, 1.0, 1.0 - 1e-12, g, n_nu=8, slope=0.0, T_star=5000.0)
+        w3.rho[...] = 0.0
+        w3.rho[cell] = rho0 * 0.5
+        o3 = orc.Oracle.from_workload(w3)
+        o3.scatter_store([j], 1_000_000)
+        o3.run(3_000_000, 24, n_threads=NTH)
+        ev3, ne3 = o3.scatter_events()
+        _, Fs3 = o3.ray_trace((1.0, 0.0, 0.0), (0.0, 1.0, 0.0), npx, npx, 15 * w3.cell_size_cm / npx, D, j)
+        per[name] = Fs3.sum() / ne3
+    ratio = per["near"] / per["far"]
+    assert abs(ratio / ((1 + g) / (1 - g)) ** 3 - 1) < 0.08, ratio
+    assert abs(Fs.sum() / (per["near"] * n_near + per["far"] * n_far) - 1) < 0.05
