@@ -238,6 +238,40 @@ int mcrt_read(mcrt_ctx *ctx, double *E_abs_count, double *E_abs_lucy, float *T_c
 int mcrt_read_raw(mcrt_ctx *ctx, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_counts,
                   uint64_t *sed_direct, uint16_t *tidx, mcrt_digest *digests, mcrt_mem where);
 
+/* ---- Scattering-event store and ray tracer (Sect. 4, Eq. 11-17) ----
+ * "The index of the cell, the frequency of the scattered photon and the incoming direction is stored":
+ * after mcrt_scatter_store every run appends one record per scattering at one of the listed frequency bins
+ * (n_bins <= 16 indices into the frequency grid) to a list of `capacity` records in device memory (cudaMalloc; 12
+ * bytes each).  A B&W run with reset_tallies and every frozen-T sweep start an empty list.  Events beyond the
+ * capacity are counted, not kept.  The order of the records depends on scheduling; the multiset does not. */
+typedef struct {
+    uint32_t cell;      /* [nz][ny][nx] index */
+    uint16_t slot;      /* position of the event's frequency bin in nu_bins */
+    int16_t q[3];       /* incoming direction, q_a = rint(32767 u_a) */
+} mcrt_scatter_event;
+int mcrt_scatter_store(mcrt_ctx *ctx, int n_bins, const int32_t *nu_bins, uint64_t capacity);
+/* *n_total_out = events counted; events [where], if not NULL, receives the first min(counted, capacity, max_events). */
+int mcrt_scatter_events(mcrt_ctx *ctx, uint64_t *n_total_out, mcrt_scatter_event *events, uint64_t max_events,
+                        mcrt_mem where);
+
+/* The image of Sect. 4 at frequency bin nu_bin for an observer at distance_cm in direction e_z (from the object
+ * towards the observer; need not be normalised), parallel projection (Eq. 11): pixel (a, b) of nx x ny square pixels
+ * of pixel_cm looks along r = i0 + (a + 1/2 - nx/2) pixel e_x + (b + 1/2 - ny/2) pixel e_y + s e_z, i0 the centre of
+ * the grid, e_x made orthogonal to e_z, e_y = e_z x e_x.  From the observer's side inwards every cell adds (Eq. 12, 17)
+ *     A_pix / D^2 (I_e + I_s) exp(-tau),  tau = absorption optical depth between the cell and the observer (Eq. 13),
+ *     I_e = (1 - exp(-tau_cell)) B_nu(T)  (Eq. 14; T from the counts, or from the Lucy tally if T_from_lucy),
+ *     I_s = l / V sum over the cell's stored events of P_HG(beta) xi / dnu  (Eq. 15, 16; beta between e_z and the
+ *           event's incoming direction; l = path length in the cell, V its volume).
+ * F_emission, F_scatter: [where] double [ny][nx], erg s^-1 cm^-2 Hz^-1 (F_scatter may be NULL; it is zero unless
+ * nu_bin is being stored).  Needs a finished run. */
+typedef struct {
+    double e_z[3], e_x[3];
+    int32_t nx, ny;
+    double pixel_cm, distance_cm;
+    int32_t nu_bin, T_from_lucy;
+} mcrt_image_opts;
+int mcrt_ray_trace(mcrt_ctx *ctx, const mcrt_image_opts *opts, double *F_emission, double *F_scatter, mcrt_mem where);
+
 /* Host copies of the derived tables (tests): dnu [n_nu], J [n_species][n_T], cdf_B and cdf_dB
  * [n_species][n_T][n_nu], albedo [n_species][n_nu], src_cdf [n_nu]. */
 int mcrt_read_tables(mcrt_ctx *ctx, double *dnu, double *J, double *cdf_B, double *cdf_dB, double *albedo,

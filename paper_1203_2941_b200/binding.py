@@ -24,7 +24,7 @@ EXPORTS = [
     "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
     "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
     "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_epoch_schedule", "mcrt_part_slice",
-    "mcrt_measure_read_bandwidth", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
+    "mcrt_measure_read_bandwidth", "mcrt_scatter_store", "mcrt_scatter_events", "mcrt_ray_trace", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
     "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
@@ -43,6 +43,14 @@ class RunOpts(C.Structure):
                 ("block_threads", C.c_int32), ("time_kernels", C.c_int32), ("first_packet_id", C.c_uint64),
                 ("n_total", C.c_uint64), ("epoch_growth", C.c_double), ("part_index", C.c_int32),
                 ("part_count", C.c_int32), ("walk_words", C.c_int32), ("carry_interactions", C.c_uint32), ("no_hot_cells", C.c_int32)]
+
+
+class ImageOpts(C.Structure):
+    _fields_ = [("e_z", C.c_double * 3), ("e_x", C.c_double * 3), ("nx", C.c_int32), ("ny", C.c_int32),
+                ("pixel_cm", C.c_double), ("distance_cm", C.c_double), ("nu_bin", C.c_int32), ("T_from_lucy", C.c_int32)]
+
+
+SCA_EVENT_DTYPE = np.dtype([("cell", np.uint32), ("slot", np.uint16), ("q", np.int16, (3,))])
 
 
 class Exchange(C.Structure):
@@ -95,6 +103,9 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_epoch_schedule.argtypes = [u64, u64, u64, d, vp, u64, C.POINTER(u64)]
     L.mcrt_part_slice.argtypes = [u64, i, i, C.POINTER(u64), C.POINTER(u64)]
     L.mcrt_measure_read_bandwidth.argtypes = [C.c_size_t, i, C.POINTER(d)]
+    L.mcrt_scatter_store.argtypes = [vp, i, vp, u64]
+    L.mcrt_scatter_events.argtypes = [vp, C.POINTER(u64), vp, u64, i]
+    L.mcrt_ray_trace.argtypes = [vp, C.POINTER(ImageOpts), vp, vp, i]
     L.mcrt_get_stats.argtypes = [vp, C.POINTER(RunStats)]
     L.mcrt_read.argtypes = [vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
@@ -241,6 +252,35 @@ def mcrt_measure_read_bandwidth(nbytes, repeats=10) -> float:
     g = C.c_double(0.0)
     _check(load_library().mcrt_measure_read_bandwidth(int(nbytes), int(repeats), C.byref(g)))
     return g.value
+
+
+_sca_capacity = {}   # context address -> capacity of its event list (to size the host buffer)
+
+
+def mcrt_scatter_store(ctx, nu_bins, capacity):
+    b = np.ascontiguousarray(nu_bins, np.int32)
+    _check(load_library().mcrt_scatter_store(ctx, len(b), _ptr(b), int(capacity)), ctx)
+    _sca_capacity[ctx.value] = int(capacity)
+
+
+def mcrt_scatter_events(ctx, max_events):
+    """(events kept, events counted)"""
+    n = C.c_uint64(0)
+    max_events = min(int(max_events), _sca_capacity.get(ctx.value, int(max_events)))
+    ev = np.zeros(max_events, SCA_EVENT_DTYPE)
+    _check(load_library().mcrt_scatter_events(ctx, C.byref(n), _ptr(ev), max_events, MCRT_HOST), ctx)
+    return ev[:min(int(n.value), max_events)], int(n.value)
+
+
+def mcrt_ray_trace(ctx, e_z, e_x, nx, ny, pixel_cm, distance_cm, nu_bin, T_from_lucy=False, scatter=True):
+    o = ImageOpts()
+    o.e_z[:] = [float(v) for v in e_z]
+    o.e_x[:] = [float(v) for v in e_x]
+    o.nx, o.ny, o.pixel_cm, o.distance_cm, o.nu_bin, o.T_from_lucy = int(nx), int(ny), float(pixel_cm), float(distance_cm), int(nu_bin), int(T_from_lucy)
+    Fe = np.zeros((ny, nx))
+    Fs = np.zeros((ny, nx)) if scatter else None
+    _check(load_library().mcrt_ray_trace(ctx, C.byref(o), _ptr(Fe), _ptr(Fs), MCRT_HOST), ctx)
+    return Fe, Fs
 
 
 def mcrt_get_stats(ctx):

@@ -41,7 +41,7 @@ enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4,
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
 
 // device counters (unsigned long long each)
-enum : int { CNT_PACKETS = 0, CNT_CROSS, CNT_DUSTY, CNT_SCA, CNT_ABS, CNT_DIRECT, CNT_OVERFLOW, CNT_NEXT, CNT_CARRY, CNT_N };
+enum : int { CNT_PACKETS = 0, CNT_CROSS, CNT_DUSTY, CNT_SCA, CNT_ABS, CNT_DIRECT, CNT_OVERFLOW, CNT_NEXT, CNT_CARRY, CNT_SCAEV, CNT_N };
 
 thread_local std::string g_create_error;
 
@@ -108,6 +108,11 @@ struct mcrt_ctx {
     double xi = 0.0;
     uint64_t epochs = 0, launches = 0;
     uint64_t dig_base = 0;                // packet id of digest slot 0
+    int8_t *d_sca_slot = nullptr;                  // scattering-event store (cudaMalloc)
+    mcrt_scatter_event *sca_ev = nullptr;
+    uint64_t sca_cap = 0;
+    std::vector<int> sca_bins;
+    double *img_buf = nullptr; size_t img_cap = 0; // ray tracer: images and per-species opacity staging (cudaMalloc)
     CarryRec *carry_buf[2] = {nullptr, nullptr};   // carried packets: read by this epoch / written for the next (cudaMalloc)
     size_t carry_cap[2] = {0, 0};
     int carry_cur = 0;
@@ -403,6 +408,9 @@ struct TransportParams {
     const CarryRec *__restrict__ carry_in;     // packets carried over from the previous epoch: taken before new ids
     CarryRec *__restrict__ carry_out;          // packets whose budget runs out in this launch (counters[CNT_CARRY] of them)
     uint32_t n_carry_in, carry_K;              // carry_K = 0: no budget
+    const int8_t *__restrict__ sca_slot;       // [nf] slot of a stored frequency bin (-1: not stored), or NULL
+    mcrt_scatter_event *__restrict__ sca_ev;   // the event list and its capacity; counters[CNT_SCAEV] counts
+    unsigned long long sca_cap;
     uint32_t seed_lo, seed_hi, pass;
 };
 
@@ -1115,6 +1123,17 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     if (ztype < s_ag[sj].x) {
                         scatter = true;
                         nsca++;
+                        if (P.sca_slot && P.sca_slot[j] >= 0) {   // store the event: cell, frequency, incoming direction
+                            const unsigned long long at = atomicAdd(&P.counters[CNT_SCAEV], 1ull);
+                            if (at < P.sca_cap) {
+                                mcrt_scatter_event ev;
+                                ev.cell = (uint32_t)cell; ev.slot = (uint16_t)P.sca_slot[j];
+                                ev.q[0] = (int16_t)__double2ll_rn(32767.0 * ux);
+                                ev.q[1] = (int16_t)__double2ll_rn(32767.0 * uy);
+                                ev.q[2] = (int16_t)__double2ll_rn(32767.0 * uz);
+                                P.sca_ev[at] = ev;
+                            }
+                        }
                         if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
@@ -1567,6 +1586,110 @@ __global__ void k_fetch_words(const unsigned long long *__restrict__ cellw, cons
     if (i < n) out[i] = cellw[(size_t)kCS * idx[i]];
 }
 
+// ------------------------------------------------------------------------------------------------
+// NEXT-2  ray tracer (Eq. 11-17)
+// ------------------------------------------------------------------------------------------------
+__host__ __device__ double planck_nu(double nu, double T);   // (defined with the host-side tables below)
+
+__device__ __forceinline__ double phase_hg(double g, double cb)
+{
+    const double d = 1.0 + g * g - 2.0 * g * cb;
+    return (1.0 - g * g) / (kFourPi * d * sqrt(d));        // Eq. 15, per steradian
+}
+
+// per-cell sum over the stored events of frequency slot `slot` of P_HG(beta) (the sum over beta of Eq. 16)
+__global__ void k_sca_source(const mcrt_scatter_event *__restrict__ ev, unsigned long long n, int slot, double ezx, double ezy, double ezz,
+                             const unsigned long long *__restrict__ cellw, const double *__restrict__ g, int nf, int j, int nx, int ny,
+                             int px, int pxy, double *__restrict__ src)
+{
+    for (unsigned long long e = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (unsigned long long)gridDim.x * blockDim.x) {
+        const mcrt_scatter_event v = ev[e];
+        if ((int)v.slot != slot) continue;
+        const double qx = v.q[0], qy = v.q[1], qz = v.q[2];
+        const double qn = sqrt(qx * qx + qy * qy + qz * qz);
+        const double cb = (qx * ezx + qy * ezy + qz * ezz) / qn;
+        const int ix = (int)(v.cell % (uint32_t)nx), iy = (int)((v.cell / (uint32_t)nx) % (uint32_t)ny), iz = (int)(v.cell / ((uint32_t)nx * (uint32_t)ny));
+        const unsigned long long cw = cellw[(size_t)kCS * lin_index(ix, iy, iz, px, pxy)];
+        atomicAdd(&src[v.cell], phase_hg(g[cw_species(cw) * nf + j], cb));
+    }
+}
+
+struct RayParams {
+    double ez[3], ex[3], ey[3];
+    int inx, iny;
+    double pix_cells, apix_d2, h, xi, inv_fx, cellfac, nu, inv_dnu;
+    int nx, ny, nz, px, pxy, nT, from_lucy, j, nf;
+};
+
+__global__ void __launch_bounds__(128) k_ray_trace(RayParams R, const unsigned long long *__restrict__ cellw, const unsigned long long *__restrict__ kcnt,
+                                                   const long long *__restrict__ lfx, const double *__restrict__ J, const double *__restrict__ Tg,
+                                                   const double *__restrict__ kabs_j /*[ns] at this frequency*/, const double *__restrict__ src,
+                                                   double *__restrict__ Fe, double *__restrict__ Fs)
+{
+    const int pixi = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pixi >= R.inx * R.iny) return;
+    const int a = pixi % R.inx, b = pixi / R.inx;
+    const int n[3] = {R.nx, R.ny, R.nz};
+    const double u[3] = {-R.ez[0], -R.ez[1], -R.ez[2]};     // the walk runs from the observer's side inwards
+    const double xa = ((double)a + 0.5 - 0.5 * R.inx) * R.pix_cells, yb = ((double)b + 0.5 - 0.5 * R.iny) * R.pix_cells;
+    double r0[3], smin = -CUDART_INF, smax = CUDART_INF;
+    bool miss = false;
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        r0[q] = 0.5 * n[q] + xa * R.ex[q] + yb * R.ey[q];
+        if (u[q] == 0.0) { if (!(r0[q] > 0.0 && r0[q] < (double)n[q])) miss = true; continue; }
+        const double s1 = (0.0 - r0[q]) / u[q], s2 = ((double)n[q] - r0[q]) / u[q];
+        smin = fmax(smin, fmin(s1, s2));
+        smax = fmin(smax, fmax(s1, s2));
+    }
+    double fe = 0.0, fs = 0.0;
+    if (!miss && smax > smin) {
+        double p[3];
+        int c[3], st[3];
+        double iv[3], tm[3];
+        bool inside = true;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            p[q] = fmin(fmax(r0[q] + smin * u[q], 0.0), (double)n[q]);
+            const double f = floor(p[q]);
+            c[q] = (p[q] != f) ? (int)f : ((u[q] >= 0.0) ? (int)f : (int)f - 1);   // start cell (reading Q9)
+            inside = inside && c[q] >= 0 && c[q] < n[q];
+            st[q] = (u[q] > 0.0) ? 1 : ((u[q] < 0.0) ? -1 : 0);
+            iv[q] = st[q] ? 1.0 / u[q] : CUDART_INF;
+        }
+        if (inside) {
+#pragma unroll
+            for (int q = 0; q < 3; ++q) tm[q] = mcrt::face_t(c[q], st[q], p[q], iv[q]);
+            const double V = R.h * R.h * R.h;
+            double t = 0.0, tau = 0.0;
+            for (;;) {
+                const int ax = (tm[0] <= tm[1] && tm[0] <= tm[2]) ? 0 : ((tm[1] <= tm[2]) ? 1 : 2);
+                const double tn = tm[ax], l = (tn - t) * R.h;
+                const unsigned long long cw = cellw[(size_t)kCS * lin_index(c[0], c[1], c[2], R.px, R.pxy)];
+                if (cw_dusty(cw)) {
+                    const size_t li = lin_index(c[0], c[1], c[2], R.px, R.pxy);
+                    const size_t ci = ((size_t)c[2] * R.ny + c[1]) * R.nx + c[0];
+                    const double rho_c = cw_rho(cw);
+                    const int sp = cw_species(cw);
+                    const double tc = kabs_j[sp] * rho_c * l;
+                    const double e = R.from_lucy ? (double)lfx[(size_t)kCS * li] * R.inv_fx : (double)kcnt[li];
+                    const double T = T_of_x(J + sp * R.nT, Tg, R.nT, e * R.cellfac / rho_c);
+                    const double att = exp(-tau);
+                    if (T > 0.0) fe += -expm1(-tc) * planck_nu(R.nu, T) * att;
+                    fs += l / V * src[ci] * R.xi * R.inv_dnu * att;
+                    tau += tc;
+                }
+                t = tn;
+                c[ax] += st[ax];
+                tm[ax] = mcrt::face_t(c[ax], st[ax], p[ax], iv[ax]);
+                if (c[ax] < 0 || c[ax] >= n[ax]) break;
+            }
+        }
+    }
+    Fe[pixi] = fe * R.apix_d2;
+    if (Fs) Fs[pixi] = fs * R.apix_d2;
+}
+
 // read-bandwidth probe: every thread sums 16-byte words of a buffer with a grid stride, eight loads in flight
 __global__ void __launch_bounds__(512) k_read_probe(const uint4 *__restrict__ buf, size_t n16, unsigned long long *__restrict__ sink)
 {
@@ -1608,7 +1731,7 @@ __global__ void k_philox_test(const uint32_t *__restrict__ ctr, const uint32_t *
 // ------------------------------------------------------------------------------------------------
 // host-side tables (O1) -- small, built once per context
 // ------------------------------------------------------------------------------------------------
-double planck_nu(double nu, double T)
+__host__ __device__ double planck_nu(double nu, double T)
 {
     const double x = kPlanckH * nu / (kBoltzK * T);
     return 2.0 * kPlanckH * nu * nu * nu / (kLightC * kLightC) / expm1(x);
@@ -2145,6 +2268,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
     P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
     P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
+    P.sca_slot = c->sca_ev ? c->d_sca_slot : nullptr; P.sca_ev = c->sca_ev; P.sca_cap = c->sca_cap;
     P.hot_idx = c->d_hot_idx; P.hot_shift = c->hot_shift; P.hot_mask = c->hot_mask; P.tidx_mask = c->tidx_mask; P.n_hot = c->n_hot;
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base;
@@ -2401,6 +2525,7 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
+        CUDA_TRY(c, cudaMemsetAsync(c->counters + CNT_SCAEV, 0, 8, c->stream));   // every sweep starts an empty event list
         c->globalised = false;
         if (o.part_count > 1 && o.record_digests) CUDA_TRY(c, cudaMemsetAsync(c->dig, 0, c->dig_n * sizeof(mcrt_digest), c->stream));
         P.pass = o.rng_pass + (uint32_t)sw;
@@ -2614,6 +2739,115 @@ int mcrt_read_raw(mcrt_ctx *c, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_
     return MCRT_OK;
 }
 
+int mcrt_scatter_store(mcrt_ctx *c, int n_bins, const int32_t *nu_bins, uint64_t capacity)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->have_tables) return fail(c, MCRT_ESTATE, "call mcrt_dust_tables before mcrt_scatter_store");
+    if (c->run.active) return fail(c, MCRT_ESTATE, "mcrt_scatter_store inside a run");
+    if (n_bins < 1 || n_bins > 16 || !nu_bins || capacity < 1) return fail(c, MCRT_EINVAL, "1 <= n_bins <= 16, capacity >= 1");
+    std::vector<int8_t> slot(c->nf, (int8_t)-1);
+    for (int b = 0; b < n_bins; ++b) {
+        if (nu_bins[b] < 0 || nu_bins[b] >= c->nf) return fail(c, MCRT_EINVAL, "nu_bins out of range");
+        slot[nu_bins[b]] = (int8_t)b;
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    if (c->sca_ev) { cudaFree(c->sca_ev); c->sca_ev = nullptr; c->sca_cap = 0; }
+    if (!c->d_sca_slot && cudaMalloc((void **)&c->d_sca_slot, c->nf) != cudaSuccess) return fail(c, MCRT_ENOMEM, "cudaMalloc failed");
+    if (cudaMalloc((void **)&c->sca_ev, capacity * sizeof(mcrt_scatter_event)) != cudaSuccess)
+        return fail(c, MCRT_ENOMEM, "cudaMalloc of the scattering-event list failed");
+    c->sca_cap = capacity;
+    c->sca_bins.assign(nu_bins, nu_bins + n_bins);
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_sca_slot, slot.data(), c->nf, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->counters + CNT_SCAEV, 0, 8, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
+int mcrt_scatter_events(mcrt_ctx *c, uint64_t *n_total_out, mcrt_scatter_event *events, uint64_t max_events, mcrt_mem where)
+{
+    if (!c || !n_total_out) return MCRT_EINVAL;
+    if (!c->sca_ev) return fail(c, MCRT_ESTATE, "no scattering-event store: call mcrt_scatter_store first");
+    unsigned long long n = 0ull;
+    CUDA_TRY(c, cudaMemcpyAsync(&n, c->counters + CNT_SCAEV, 8, cudaMemcpyDeviceToHost, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    *n_total_out = n;
+    if (events) {
+        uint64_t m = n < c->sca_cap ? n : c->sca_cap;
+        if (m > max_events) m = max_events;
+        CUDA_TRY(c, cudaMemcpyAsync(events, c->sca_ev, m * sizeof(mcrt_scatter_event),
+                                    where == MCRT_HOST ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    return MCRT_OK;
+}
+
+int mcrt_ray_trace(mcrt_ctx *c, const mcrt_image_opts *io, double *F_emission, double *F_scatter, mcrt_mem where)
+{
+    if (!c || !io || !F_emission) return MCRT_EINVAL;
+    if (!c->last_n || c->run.active) return fail(c, MCRT_ESTATE, "mcrt_ray_trace needs a finished run");
+    if (io->nx < 1 || io->ny < 1 || (size_t)io->nx * io->ny > ((size_t)1 << 28) || !(io->pixel_cm > 0.0) || !(io->distance_cm > 0.0) ||
+        io->nu_bin < 0 || io->nu_bin >= c->nf)
+        return fail(c, MCRT_EINVAL, "mcrt_ray_trace: bad image options");
+    int rc;
+    if ((rc = check_overflow(c))) return rc;
+    RayParams R;
+    {
+        const double *z = io->e_z, *x = io->e_x;
+        const double zn = sqrt(z[0] * z[0] + z[1] * z[1] + z[2] * z[2]);
+        if (!(zn > 0.0)) return fail(c, MCRT_EINVAL, "e_z is zero");
+        for (int a = 0; a < 3; ++a) R.ez[a] = z[a] / zn;
+        const double dot = x[0] * R.ez[0] + x[1] * R.ez[1] + x[2] * R.ez[2];
+        for (int a = 0; a < 3; ++a) R.ex[a] = x[a] - dot * R.ez[a];
+        const double xn = sqrt(R.ex[0] * R.ex[0] + R.ex[1] * R.ex[1] + R.ex[2] * R.ex[2]);
+        if (!(xn > 0.0)) return fail(c, MCRT_EINVAL, "e_x is parallel to e_z");
+        for (int a = 0; a < 3; ++a) R.ex[a] /= xn;
+        R.ey[0] = R.ez[1] * R.ex[2] - R.ez[2] * R.ex[1]; R.ey[1] = R.ez[2] * R.ex[0] - R.ez[0] * R.ex[2];
+        R.ey[2] = R.ez[0] * R.ex[1] - R.ez[1] * R.ex[0];
+    }
+    const int j = io->nu_bin;
+    R.inx = io->nx; R.iny = io->ny; R.pix_cells = io->pixel_cm / c->h;
+    R.apix_d2 = io->pixel_cm * io->pixel_cm / (io->distance_cm * io->distance_cm);
+    R.h = c->h; R.xi = c->xi; R.inv_fx = ldexp(1.0, -c->fx); R.cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
+    R.nu = c->nu[j]; R.inv_dnu = 1.0 / c->dnu[j];
+    R.nx = c->nx; R.ny = c->ny; R.nz = c->nz; R.px = c->px; R.pxy = c->pxy; R.nT = c->nT; R.from_lucy = io->T_from_lucy; R.j = j; R.nf = c->nf;
+    const size_t npix = (size_t)io->nx * io->ny;
+    const size_t need = 2 * npix + (size_t)c->ns + 8;
+    if (c->img_cap < need) {
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->img_buf) cudaFree(c->img_buf);
+        c->img_buf = nullptr; c->img_cap = 0;
+        if (cudaMalloc((void **)&c->img_buf, need * sizeof(double)) != cudaSuccess) return fail(c, MCRT_ENOMEM, "cudaMalloc of the image buffers failed");
+        c->img_cap = need;
+    }
+    double *d_fe = (where == MCRT_DEVICE) ? F_emission : c->img_buf;
+    double *d_fs = F_scatter ? ((where == MCRT_DEVICE) ? F_scatter : c->img_buf + npix) : nullptr;
+    double *d_kabs = c->img_buf + 2 * npix;
+    std::vector<double> kj(c->ns);
+    for (int s = 0; s < c->ns; ++s) kj[s] = c->kabs[(size_t)s * c->nf + j];
+    CUDA_TRY(c, cudaMemcpyAsync(d_kabs, kj.data(), c->ns * 8, cudaMemcpyHostToDevice, c->stream));
+    // the sum over the stored events (Eq. 16), per cell, in the scratch array
+    double *src = (double *)c->scratch;
+    CUDA_TRY(c, cudaMemsetAsync(src, 0, c->nc * 8, c->stream));
+    int slot = -1;
+    for (size_t b = 0; b < c->sca_bins.size(); ++b) if (c->sca_bins[b] == j) slot = (int)b;
+    if (c->sca_ev && slot >= 0 && F_scatter) {
+        unsigned long long n = 0ull;
+        CUDA_TRY(c, cudaMemcpyAsync(&n, c->counters + CNT_SCAEV, 8, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (n > c->sca_cap) n = c->sca_cap;
+        if (n) k_sca_source<<<stream_grid((size_t)n), 256, 0, c->stream>>>(c->sca_ev, n, slot, R.ez[0], R.ez[1], R.ez[2], c->cellw, c->d_g, c->nf, j,
+                                                                         c->nx, c->ny, c->px, c->pxy, src);
+    }
+    k_ray_trace<<<(unsigned)((npix + 127) / 128), 128, 0, c->stream>>>(R, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, d_kabs, src, d_fe, d_fs);
+    CUDA_TRY(c, cudaGetLastError());
+    if (where == MCRT_HOST) {
+        CUDA_TRY(c, cudaMemcpyAsync(F_emission, d_fe, npix * 8, cudaMemcpyDeviceToHost, c->stream));
+        if (F_scatter) CUDA_TRY(c, cudaMemcpyAsync(F_scatter, d_fs, npix * 8, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
 int mcrt_read_tables(mcrt_ctx *c, double *dnu, double *J, double *cdf_B, double *cdf_dB, double *albedo, double *src_cdf)
 {
     if (!c) return MCRT_EINVAL;
@@ -2676,6 +2910,9 @@ void mcrt_destroy(mcrt_ctx *c)
     for (cudaEvent_t e : c->ev_pool) cudaEventDestroy(e);
     for (void *p : c->owned) cudaFree(p);
     for (int i = 0; i < 2; ++i) if (c->carry_buf[i]) cudaFree(c->carry_buf[i]);
+    if (c->d_sca_slot) cudaFree(c->d_sca_slot);
+    if (c->sca_ev) cudaFree(c->sca_ev);
+    if (c->img_buf) cudaFree(c->img_buf);
     delete c;
 }
 

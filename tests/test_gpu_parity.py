@@ -547,6 +547,45 @@ def test_parity_carry_over_of_long_lived_packets(B, orc, kind, K, blocks):
     c.close()
 
 
+def test_parity_scattering_store_and_ray_tracer(B, orc):
+    """NEXT-2 (Sect. 4, Eq. 11-17; oracle pins P20): the stored scattering events are the oracle's as a
+    multiset (their order depends on scheduling), a store that is too small counts what it drops, and the emission
+    and scattering images for two observer orientations agree with the oracle's ray tracer to 1e-9."""
+    w = W.sphere32(tau_V=3.0, n=24)
+    N = 200_000
+    bins = [48, 52, 56]                       # 0.9, 0.5, 0.28 um on the 64-point grid: where the 5800 K source emits
+    o = orc.Oracle.from_workload(w)
+    o.scatter_store(bins, 4_000_000)
+    ro = o.run(N, 33, n_threads=NTH)
+    ev_o, n_o = o.scatter_events()
+    c = B.Context(w)
+    B.mcrt_scatter_store(c.ctx, bins, 4_000_000)
+    rg = c.run(N, 33)
+    ev_g, n_g = B.mcrt_scatter_events(c.ctx, 4_000_000)
+    assert n_g == n_o == len(ev_g) > 3_000 and rg["scatterings"] == ro["scatterings"]
+
+    def key(ev):
+        a = np.zeros((len(ev), 5), np.int64)
+        a[:, 0], a[:, 1], a[:, 2:] = ev["cell"], ev["slot"], ev["q"]
+        return a[np.lexsort(a.T[::-1])]
+    assert np.array_equal(key(ev_o), key(ev_g))
+    D = 3.0e20
+    for ez, ex, lucy in (((0.0, 0.0, 1.0), (1.0, 0.0, 0.0), False), ((0.5, -0.4, 0.3), (0.1, 0.9, 0.2), True)):
+        for j in (bins[0], bins[2], 20):       # 20: a frequency that is not stored (no scattered light; 54 um: dust emission)
+            Fe_o, Fs_o = o.ray_trace(ez, ex, 96, 80, w.cell_size_cm * 0.7, D, j, T_from_lucy=lucy)
+            Fe_g, Fs_g = B.mcrt_ray_trace(c.ctx, ez, ex, 96, 80, w.cell_size_cm * 0.7, D, j, T_from_lucy=lucy)
+            np.testing.assert_allclose(Fe_g, Fe_o, rtol=1e-9, atol=1e-12 * Fe_o.max())
+            np.testing.assert_allclose(Fs_g, Fs_o, rtol=1e-9, atol=1e-12 * max(Fs_o.max(), 1e-300))
+            assert (Fs_o.max() > 0) == (j in bins)
+        assert Fe_o.max() > 0
+    # a store that is too small keeps what fits and counts the rest; a new B&W run starts an empty list
+    B.mcrt_scatter_store(c.ctx, [bins[1]], 100)
+    c.run(N, 33)
+    ev_s, n_s = B.mcrt_scatter_events(c.ctx, 1000)
+    assert len(ev_s) == 100 and n_s == int((ev_o["slot"] == 1).sum()) and np.all(ev_s["slot"] == 0)
+    c.close()
+
+
 @pytest.mark.parametrize("walk_words", [1, 2])
 def test_parity_both_walk_variants(B, orc, walk_words):
     """The two ways the walk keeps its cell words in flight (registers, 2 cells ahead / cp.async ring, 4 cells
