@@ -53,7 +53,11 @@ enum {
 
 typedef enum {
     MCRT_MODE_BW_EPOCH = 0,      /* Bjorkman & Wood immediate re-emission, Eq. 10, deterministic epochs */
-    MCRT_MODE_FROZEN_T_SWEEP = 1 /* iterative scheme of PAPER.md:73: T frozen per sweep, Eq. 5 */
+    MCRT_MODE_FROZEN_T_SWEEP = 1,/* iterative scheme of PAPER.md:73: T frozen per sweep, Eq. 5 */
+    MCRT_MODE_LIVE_BW = 2        /* Bjorkman & Wood as printed: the temperature follows every single
+                                    absorption (atomic count with return, Eq. 4 inverted on the spot), all packets in one
+                                    launch.  The count a packet sees depends on the order of the atomics: results are
+                                    reproducible only statistically.  For comparison with the epochs. */
 } mcrt_mode;
 
 /* Options of mcrt_run.  Fill with mcrt_default_opts() first. */
@@ -81,6 +85,9 @@ typedef struct {
     int32_t walk_words;        /* launch tuning (results never depend on it): how the cell walk keeps its cell words
                                   in flight.  0 = auto (= 1), 1 = in registers, 2 = cp.async ring in shared memory
                                   (never measured faster; kept for such measurements) */
+    uint32_t source_strata;    /* > 0: stratified source frequencies (Eq. 1: equal-energy source bins with
+                                  equally many packets): packet id takes stratum id mod source_strata of the cumulative
+                                  source spectrum and a uniform position in it.  0 (default): plain sampling */
     uint32_t carry_interactions; /* MCRT_MODE_BW_EPOCH: > 0 = a packet that has had this many interactions within one
                                   epoch stops behind the last of them and continues in the next epoch, from the same
                                   state and random stream, at that epoch's temperatures; packets still carried after

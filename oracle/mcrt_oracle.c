@@ -473,6 +473,7 @@ typedef struct {
     uint64_t n_total;        /* the luminosity is split into this many packets, xi = L / n_total; 0 = n_packets */
     double growth;           /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2 (O11) */
     uint32_t carry_K;        /* > 0: a packet is carried over to the next epoch after this many interactions in one epoch */
+    uint32_t source_strata;  /* > 0: the source frequency is drawn stratified (Eq. 1): stratum = packet id mod source_strata */
 } orc_opts;
 
 /* One stored scattering event ("The index of the cell, the frequency of the scattered photon and the
@@ -571,6 +572,13 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
     } else {
         /* O3 emit: frequency through the source CDF, isotropic direction */
         orc_uniforms(R->seed, pid, d++, R->pass, z);
+        if (R->o->source_strata) {
+            /* Eq. 1: the source spectrum is split into equal-energy bins with the same number
+             * of packets each -- stratified sampling of the cumulative spectrum: packet pid takes stratum
+             * pid mod S and a uniform position inside it */
+            double S = (double)R->o->source_strata;
+            z[0] = ((double)(pid % R->o->source_strata) + z[0]) / S;
+        }
         j = orc_lower_bound(C->srccdf, nf, z[0]);
         orc_uniforms(R->seed, pid, d++, R->pass, z);
         orc_isotropic(z[0], z[1], u);

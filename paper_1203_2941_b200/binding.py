@@ -18,7 +18,7 @@ LIB_PATH = os.environ.get("MCRT_B200_LIB") or os.path.join(_HERE, "lib", "libmcr
 
 MCRT_HOST, MCRT_DEVICE = 0, 1
 MCRT_OK, MCRT_EINVAL, MCRT_ESTATE, MCRT_ENOMEM, MCRT_ECUDA, MCRT_EOVERFLOW = 0, -1, -2, -3, -4, -5
-MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP = 0, 1
+MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP, MCRT_MODE_LIVE_BW = 0, 1, 2
 
 EXPORTS = [
     "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
@@ -42,7 +42,7 @@ class RunOpts(C.Structure):
                 ("reset_tallies", C.c_int32), ("rng_pass", C.c_uint32), ("grid_blocks", C.c_int32),
                 ("block_threads", C.c_int32), ("time_kernels", C.c_int32), ("first_packet_id", C.c_uint64),
                 ("n_total", C.c_uint64), ("epoch_growth", C.c_double), ("part_index", C.c_int32),
-                ("part_count", C.c_int32), ("walk_words", C.c_int32), ("carry_interactions", C.c_uint32), ("no_hot_cells", C.c_int32)]
+                ("part_count", C.c_int32), ("walk_words", C.c_int32), ("source_strata", C.c_uint32), ("carry_interactions", C.c_uint32), ("no_hot_cells", C.c_int32)]
 
 
 class ImageOpts(C.Structure):

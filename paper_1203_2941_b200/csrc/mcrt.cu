@@ -408,6 +408,10 @@ struct TransportParams {
     const CarryRec *__restrict__ carry_in;     // packets carried over from the previous epoch: taken before new ids
     CarryRec *__restrict__ carry_out;          // packets whose budget runs out in this launch (counters[CNT_CARRY] of them)
     uint32_t n_carry_in, carry_K;              // carry_K = 0: no budget
+    uint32_t source_strata;                    // > 0: stratified source frequencies (Eq. 1)
+    int live_bw;                               // 1: the temperature index follows every absorption, not the epoch
+    const double *__restrict__ J;              // [ns][nT] left side of Eq. 4 (live_bw)
+    double cellfac;                            // xi / (4 pi V) (live_bw)
     const int8_t *__restrict__ sca_slot;       // [nf] slot of a stored frequency bin (-1: not stored), or NULL
     mcrt_scatter_event *__restrict__ sca_ev;   // the event list and its capacity; counters[CNT_SCAEV] counts
     unsigned long long sca_cap;
@@ -614,6 +618,8 @@ __device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+__device__ __forceinline__ int t_index(const double *J, int nT, double x);
 
 // 64-bit add into a per-CTA hot-cell tally kept as two 32-bit limbs (native shared atomics; a 64-bit one is a CAS
 // loop): the carry out of the low limb goes into the high limb's add.  The limbs are put together at the flush.
@@ -1096,6 +1102,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     d = 0u; ncross = 0u; nsca = 0u; nabs = 0u; nint = 0u;
                     hash = 0xCBF29CE484222325ull;
                     draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                    // Eq. 1: stratified over the cumulative source spectrum, stratum = pid mod S
+                    if (P.source_strata) z0 = ((double)(pid % P.source_strata) + z0) / (double)P.source_strata;
                     j = lower_bound_cdf(s_src, nf, z0);
                     px = P.px; py = P.py; pz = P.pz;
                     cw = 0ull; cidx = 0u;
@@ -1138,10 +1146,17 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
-                        if (hid) atomicAdd(&s_hot_k[hid], 1u); else atomicAdd(&P.kcnt[cidx], 1ull);
                         nabs++;
                         const int s = cw_species(cw);
-                        const int m = cw_tidx(cw, P.tidx_mask);
+                        int m = cw_tidx(cw, P.tidx_mask);
+                        if (P.live_bw) {
+                            // Bjorkman & Wood as printed: the temperature is adjusted after each
+                            // absorption -- T_{i,k} from the count including this one (Eq. 4).  The count a packet sees
+                            // depends on the order of the atomics: results are reproducible only statistically.
+                            const unsigned long long kn = atomicAdd(&P.kcnt[cidx], 1ull) + 1ull;
+                            m = t_index(P.J + s * P.nT, P.nT, (double)kn * P.cellfac / rho_c);
+                        } else if (hid) atomicAdd(&s_hot_k[hid], 1u);
+                        else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                         j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
                         if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
@@ -2268,6 +2283,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.kext_h = c->d_kext_h; P.kabs_fx = c->d_kabs_fx; P.albedo = c->d_albedo; P.g = c->d_g;
     P.srccdf = c->d_srccdf; P.mu_edges = c->d_mu;
     P.sed = c->sed; P.sed_direct = c->sed_direct; P.counters = c->counters;
+    P.source_strata = c->run.o.source_strata; P.live_bw = c->run.o.mode == MCRT_MODE_LIVE_BW; P.J = c->d_J; P.cellfac = c->run.cellfac;
     P.sca_slot = c->sca_ev ? c->d_sca_slot : nullptr; P.sca_ev = c->sca_ev; P.sca_cap = c->sca_cap;
     P.hot_idx = c->d_hot_idx; P.hot_shift = c->hot_shift; P.hot_mask = c->hot_mask; P.tidx_mask = c->tidx_mask; P.n_hot = c->n_hot;
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
@@ -2370,7 +2386,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (n_packets < 1) return fail(c, MCRT_EINVAL, "n_packets must be >= 1");
     mcrt_run_opts o;
     if (opts) o = *opts; else mcrt_default_opts(&o);
-    if (o.mode != MCRT_MODE_BW_EPOCH && o.mode != MCRT_MODE_FROZEN_T_SWEEP) return fail(c, MCRT_EINVAL, "unknown mode");
+    if (o.mode != MCRT_MODE_BW_EPOCH && o.mode != MCRT_MODE_FROZEN_T_SWEEP && o.mode != MCRT_MODE_LIVE_BW) return fail(c, MCRT_EINVAL, "unknown mode");
+    if (o.mode == MCRT_MODE_LIVE_BW && o.part_count > 1) return fail(c, MCRT_EINVAL, "MCRT_MODE_LIVE_BW is not available in a partitioned run");
     if (o.mode == MCRT_MODE_FROZEN_T_SWEEP && o.n_sweeps < 1) return fail(c, MCRT_EINVAL, "n_sweeps must be >= 1");
     if (o.part_count < 0 || o.part_count > 65536 || (o.part_count > 1 && (o.part_index < 0 || o.part_index >= o.part_count)))
         return fail(c, MCRT_EINVAL, "part_index must be in 0..part_count-1");
@@ -2387,13 +2404,13 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     mcrt_ctx::Run &R = c->run;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem))) return rc;
     R.ringw = use_ring(c, &o);
-    R.hot = c->n_hot > 0 && !o.no_hot_cells;
+    R.hot = c->n_hot > 0 && !o.no_hot_cells && o.mode != MCRT_MODE_LIVE_BW;   // (live B&W needs every count in global memory)
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
     const uint64_t n_xi = o.n_total ? o.n_total : n_packets;
     const int fx = fx_bits_for(n_xi);
     const double xi = c->L / (double)n_xi;                          // xi = L/N
-    const bool continuing = o.mode == MCRT_MODE_BW_EPOCH && !o.reset_tallies && c->last_n != 0;
+    const bool continuing = o.mode != MCRT_MODE_FROZEN_T_SWEEP && !o.reset_tallies && c->last_n != 0;
     if (continuing && (xi != c->xi || fx != c->fx))
         return fail(c, MCRT_ESTATE, "reset_tallies = 0: the stored tallies have another packet energy / fixed-point scale (set n_total)");
     if (continuing && c->globalised)
@@ -2409,7 +2426,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     } else c->dig_n = 0;
     c->dig_base = o.first_packet_id;
 
-    if (o.reset_tallies && o.mode == MCRT_MODE_BW_EPOCH) {
+    if (o.reset_tallies && o.mode != MCRT_MODE_FROZEN_T_SWEEP) {
         CUDA_TRY(c, cudaMemset2DAsync(c->lfx, 8 * kCS, 0, 8, c->ncp, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
@@ -2443,6 +2460,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     R.carry_K = (o.mode == MCRT_MODE_BW_EPOCH) ? o.carry_interactions : 0u; R.n_carry = 0;
     R.growth = o.epoch_growth;
     uint64_t B0 = o.epoch_B0, Bmax = o.epoch_Bmax;
+    if (o.mode == MCRT_MODE_LIVE_BW) B0 = Bmax = n_packets;      // one launch: nothing is frozen per epoch
     schedule_defaults(n_packets, &B0, &Bmax, &R.growth);
     R.Bnom = B0; R.Bmax = Bmax;
     c->need_exchange = false; c->exchange_open = false;
@@ -2465,7 +2483,7 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
     TransportParams P;
     fill_params(c, P);
     uint64_t lo, hi;
-    if (o.mode == MCRT_MODE_BW_EPOCH) {
+    if (o.mode != MCRT_MODE_FROZEN_T_SWEEP) {
         // an epoch of new packets, or -- all new packets done, some still carried -- an epoch of carried packets only,
         // with the budget doubled (see CarryRec)
         const bool drain = R.done >= R.n;

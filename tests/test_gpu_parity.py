@@ -547,6 +547,49 @@ def test_parity_carry_over_of_long_lived_packets(B, orc, kind, K, blocks):
     c.close()
 
 
+def test_parity_stratified_source(B, orc):
+    """NEXT-4, Eq. 1 (oracle pin P21): stratified source frequencies, bit-equal to the oracle."""
+    w = W.sphere32(tau_V=2.0, n=16)
+    N = 60_000
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 35, n_threads=NTH, digests=True, source_strata=1000)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 35, record_digests=1, source_strata=1000)
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    r0 = o.run(N, 35, n_threads=NTH, digests=True)
+    assert not np.array_equal(r0["digests"]["hash"], ro["digests"]["hash"])
+    c.close()
+
+
+def test_live_bjorkman_wood_statistical_parity(B, orc):
+    """NEXT-4: MCRT_MODE_LIVE_BW, Bjorkman & Wood as printed -- the temperature follows every
+    absorption through atomics, so a packet's path depends on scheduling and only statistics can be
+    compared: against the oracle's SERIAL B&W (one packet per epoch) temperatures agree within 0.5 % shell by shell
+    and the spectrum within 3 % band by band; counts are conserved exactly; two runs differ in detail."""
+    w = W.sphere32(tau_V=5.0, n=10)
+    N = 60_000
+    o = orc.Oracle.from_workload(w)
+    rs = o.run(N, 41, B0=1, Bmax=1)
+    To, so = o.read()["T"].astype(float), o.read_raw()["sed"].sum(axis=0).astype(float)
+    c = B.Context(w)
+    rg = c.run(N, 41, mode=B.MCRT_MODE_LIVE_BW)
+    raw = c.read_raw()
+    Tg, sg = c.read()["T_count"].astype(float), raw["sed"].sum(axis=0).astype(float)
+    assert rg["epochs"] == 1 and rg["packets"] == N == int(raw["sed"].sum()) and int(raw["k"].sum()) == rg["absorptions"]
+    x = (np.arange(10) + 0.5) - 5
+    rr = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2).reshape(-1)
+    for lo in range(5):
+        sel = (rr >= lo) & (rr < lo + 1) & (w.rho.reshape(-1) > 0)
+        assert abs(Tg[sel].mean() / To[sel].mean() - 1) < 0.005, lo
+    bo, bg = so.reshape(8, 8).sum(axis=1), sg.reshape(8, 8).sum(axis=1)
+    sel = bo > 500
+    assert sel.sum() >= 4 and np.all(np.abs(bg[sel] / bo[sel] - 1) < 0.03 + 3 / np.sqrt(bo[sel]))
+    c.close()
+
+
 def test_parity_scattering_store_and_ray_tracer(B, orc):
     """NEXT-2 (Sect. 4, Eq. 11-17; oracle pins P20): the stored scattering events are the oracle's as a
     multiset (their order depends on scheduling), a store that is too small counts what it drops, and the emission

@@ -869,3 +869,25 @@ def test_p20_ray_tracer_scattering(orc):
     ratio = per["near"] / per["far"]
     assert abs(ratio / ((1 + g) / (1 - g)) ** 3 - 1) < 0.08, ratio
     assert abs(Fs.sum() / (per["near"] * n_near + per["far"] * n_far) - 1) < 0.05
+
+
+# ------------------------------------------------------------------------------------------ P21 stratified source
+def test_p21_stratified_source_frequencies(orc):
+    """NEXT-4, Eq. 1 (1000 equal-energy bins x 1e5 packets at PAPER.md:232): with as many strata as
+    packets every packet takes its own quantile slice of the cumulative source spectrum, so the number of packets
+    emitted in frequency bin j is N p_j to within the two slices that straddle the bin's ends -- a deterministic
+    bound, where plain sampling scatters by sqrt(N p_j)."""
+    w = W.uniform_cube(4, 0.0, 0.5, 0.0, n_nu=24, T_star=5000.0)
+    o = orc.Oracle.from_workload(w)
+    N = 100_000
+    p = np.diff(np.concatenate([[0.0], o.tables()["srccdf"]]))
+    o.run(N, 21, n_threads=NTH, source_strata=N)
+    cnt = o.read_raw()["sed"].sum(axis=0).astype(np.int64)
+    assert cnt.sum() == N and np.all(np.abs(cnt - N * p) < 2.0)
+    o.run(N, 21, n_threads=NTH)                      # plain sampling: far outside that bound
+    cnt0 = o.read_raw()["sed"].sum(axis=0).astype(np.int64)
+    assert np.abs(cnt0 - N * p).max() > 20
+    o.run(N, 21, n_threads=NTH, source_strata=1000)  # 1000 strata x 100 packets, the paper's proportions
+    cnt1 = o.read_raw()["sed"].sum(axis=0).astype(np.int64)
+    big = N * p > 2000
+    assert np.all(np.abs(cnt1 - N * p)[big] < 0.35 * np.sqrt(N * p)[big] + 15)
