@@ -82,9 +82,6 @@ typedef struct {
     double epoch_growth;       /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2.0; must be >= 1 */
     int32_t part_index;        /* partitioned run (packets are independent): this context transports */
     int32_t part_count;        /* slice part_index of part_count of EVERY epoch's id range; 0 or 1 = the whole run */
-    int32_t walk_words;        /* launch tuning (results never depend on it): how the cell walk keeps its cell words
-                                  in flight.  0 = auto (= 1), 1 = in registers, 2 = cp.async ring in shared memory
-                                  (never measured faster; kept for such measurements) */
     uint32_t source_strata;    /* > 0: stratified source frequencies (Eq. 1: equal-energy source bins with
                                   equally many packets): packet id takes stratum id mod source_strata of the cumulative
                                   source spectrum and a uniform position in it.  0 (default): plain sampling */

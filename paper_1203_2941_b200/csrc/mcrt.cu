@@ -73,6 +73,7 @@ struct mcrt_ctx {
     int n_hot = 0, hot_max = 31;
     uint32_t hot_shift = 24, hot_mask = 31, tidx_mask = 0xffffu;
     std::vector<uint32_t> hot_idx;   // [n_hot + 1]
+    std::vector<uint32_t> hot_cand;  // storage indices of the dusty cells around the source, nearest first (<= hot_max)
     size_t l2_bytes = 126u << 20;
     double h = 0.0;
     // workspace (bump allocator)
@@ -99,6 +100,9 @@ struct mcrt_ctx {
     // host tables
     int nf = 0, nT = 0, ndir = 1, ndir_alloc = 0;
     std::vector<double> nu, dnu, kabs, ksca, g, Tg, kext_h, kabs_h, albedo, J, cdfB, cdfdB, srccdf, mu_edges;
+    std::vector<unsigned short> perm;     // Eytzinger position -> ascending position of a CDF row
+    unsigned short *d_perm = nullptr;
+    int nfs = 0;                          // row stride of the device CDF tables
     double L = 0.0, pos[3] = {0, 0, 0};
     bool have_tables = false, have_source = false, mu_dirty = true;
     double *sed_stage = nullptr;          // [ndir*nf] staging of the SED for host reads
@@ -127,7 +131,7 @@ struct mcrt_ctx {
         bool finished = false;            // every step has been issued
         uint32_t carry_K = 0;             // interaction budget of the current epoch (0 = no carry-over)
         uint64_t n_carry = 0;             // packets carried into the next epoch
-        bool ringw = false;               // walk variant of this run
+        bool xtra = false;                // carry-over / event store / stratified source / live B&W in use
         bool hot = false;                 // hot cells tallied per CTA
     } run;
     bool need_exchange = false;           // partitioned run: a step's tallies are still per-part
@@ -223,7 +227,15 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 // one block -> two uniforms strictly inside (0,1): zeta = (2*u52+1) * 2^-53
-__device__ __forceinline__ void draw2(uint32_t seed_lo, uint32_t seed_hi, unsigned long long pid, uint32_t d,
+#ifndef MCRT_PHILOX_INLINE
+#define MCRT_PHILOX_INLINE 1        // 0: one out-of-line copy of the generator (smaller code; measured 2 % slower on
+#endif                              //    torus256 than the inlined copies: the calls cost more than the cache misses)
+#if MCRT_PHILOX_INLINE
+__device__ __forceinline__
+#else
+__device__ __noinline__
+#endif
+void draw2(uint32_t seed_lo, uint32_t seed_hi, unsigned long long pid, uint32_t d,
                                       uint32_t pass, double &z0, double &z1)
 {
     uint32_t w0, w1, w2, w3;
@@ -314,6 +326,17 @@ __device__ __forceinline__ int lower_bound_cdf(const double *cdf, int n, double 
     return lo;
 }
 
+// The same lower bound on a row stored in Eytzinger (breadth-first) order, 1-based, the row 128-byte aligned: the
+// first four levels of the search (entries 1..15) share one cache line, so a search costs about four round trips to
+// L2 instead of seven or eight.  perm[k] = position of entry k in ascending order.
+__device__ __forceinline__ int lower_bound_eytzinger(const double *__restrict__ row, const unsigned short *__restrict__ perm, int n, double z)
+{
+    int k = 1;
+    while (k <= n) k = 2 * k + ((__ldg(row + k) < z) ? 1 : 0);
+    k >>= __ffs(~k);
+    return (int)perm[k];
+}
+
 __device__ __forceinline__ void hash_mix(unsigned long long &h, unsigned long long w)
 {
     h = (h ^ w) * 0x100000001B3ull;
@@ -343,24 +366,17 @@ constexpr unsigned long long kRhoMask = 0xFFFFFFFFE0000000ull;
 #define MCRT_CELL_STRIDE 1
 #endif
 constexpr int kCS = MCRT_CELL_STRIDE;
-// The walk keeps DEPTH cell words in flight per lane (its geometry runs that many cells ahead of the physics), in
-// one of two ways, chosen per grid at run time (mcrt_run_opts.walk_words):
-//   registers (kDepthReg = 2): fewest load/store wavefronts -- for grids whose dusty cells mostly hit L2;
-//   a cp.async ring in shared memory (kDepthRing, compile-time): the groups of a thread complete in order, so "all
-//   but the N newest have landed" is one wait on one scoreboard whatever N is (plain loads cannot be pipelined deeper
-//   than ptxas has scoreboards to spare: it gave both register loads the same one).  Measured at depth 2, 3 and 4 on
-//   all five workloads (profiles/r02_experiments.md): never faster than the registers, not even on the grids that
-//   wait for DRAM (disk256, torus512) -- their limit is the rate of scattered 32-byte DRAM sectors, not latency.
-//   Kept selectable for such measurements; auto = registers.
+// The walk keeps kDepthReg cell words in flight per lane, in registers (its geometry runs that many cells ahead of the
+// physics).  Round 1 kept them in a cp.async ring in shared memory: its groups complete in order, so any depth is
+// one wait on one scoreboard, whereas ptxas gives the two register loads the same scoreboard.  Both were measured
+// this round at depths 2-4 on all five workloads (profiles/r02_experiments.md, commits b3e3664..0e8480c carry the
+// ring as `walk_words = 2`): the ring was never faster, not even on the grids that wait for DRAM -- it costs 9
+// shared-memory wavefronts per step on the SM's busiest unit -- and was removed.
 #ifndef MCRT_DEPTH
 #define MCRT_DEPTH 2
 #endif
-#ifndef MCRT_RING_DEPTH
-#define MCRT_RING_DEPTH 2
-#endif
-constexpr int kDepthReg = MCRT_DEPTH, kDepthRing = MCRT_RING_DEPTH;
-constexpr int kGuard = (kDepthReg > kDepthRing ? kDepthReg : kDepthRing) + 1;  // guard cells around the grid (see "Storage order")
-constexpr int kRing = (kDepthRing + 1 <= 4) ? 4 : 8;   // ring slots per thread (cells n .. n+kDepthRing), a power of two
+constexpr int kDepthReg = MCRT_DEPTH;
+constexpr int kGuard = kDepthReg + 1;  // guard cells around the grid (see "Storage order")
 
 __device__ __forceinline__ double cw_rho(unsigned long long cw) { return __longlong_as_double((long long)(cw & kRhoMask)); }
 __device__ __forceinline__ int cw_species(unsigned long long cw) { return (int)((unsigned)cw & 0xffu); }
@@ -394,6 +410,8 @@ struct TransportParams {
     unsigned long long *__restrict__ sed, *__restrict__ sed_direct, *__restrict__ counters;
     mcrt_digest *__restrict__ dig;
     int nx, ny, nz, ns, nf, nT, ndir;
+    int nfs;            // stride of a re-emission CDF row (Eytzinger order, padded to 16 doubles)
+    const unsigned short *__restrict__ perm;   // [nf + 1] Eytzinger position -> ascending position
     int nbx, nby;       // bricks per axis
     uint32_t ncp;       // padded cell count
     const uint32_t *__restrict__ hot_idx;   // [kHot + 1] storage index of hot cell number i (entry 0 unused)
@@ -609,40 +627,37 @@ struct SlotSet {
     }
 };
 
-// 8-byte asynchronous copy global -> shared (LDGSTS), per-thread groups
-__device__ __forceinline__ void cp_async8(void *smem_dst, const void *gsrc)
-{
-    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gsrc) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N>
-__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
-
 __device__ __forceinline__ int t_index(const double *J, int nT, double x);
 
 // 64-bit add into a per-CTA hot-cell tally kept as two 32-bit limbs (native shared atomics; a 64-bit one is a CAS
 // loop): the carry out of the low limb goes into the high limb's add.  The limbs are put together at the flush.
-__device__ __forceinline__ void hot_add(unsigned int *lo, unsigned int *hi, uint32_t id, unsigned long long q)
+__device__ __forceinline__ void hot_add(unsigned int *hot, uint32_t id, unsigned long long q)
 {
-    const unsigned int ql = (unsigned int)q, old = atomicAdd(&lo[id], ql);
+    unsigned int *t = hot + 3u * id;
+    const unsigned int ql = (unsigned int)q, old = atomicAdd(t, ql);
     const unsigned int carry = (old + ql < old) ? 1u : 0u;
     const unsigned int qh = (unsigned int)(q >> 32) + carry;
-    if (qh) atomicAdd(&hi[id], qh);
+    if (qh) atomicAdd(t + 1, qh);
 }
+// shared-memory words of the hot-cell tallies (entry 0 unused), a whole number of 16-byte units
+__host__ __device__ constexpr int hot_smem_words(int n_hot) { return (3 * (n_hot + 1) + 3) & ~3; }
+constexpr int kPermSmem = 1024;
 
-template <bool RECORD, bool RINGW, bool HOT>
+template <bool RECORD, bool HOT, bool XTRA>
 __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const TransportParams P)
 {
-    __shared__ unsigned int s_hot_lo[HOT ? kHot + 1 : 1], s_hot_hi[HOT ? kHot + 1 : 1], s_hot_k[HOT ? kHot + 1 : 1];   // per-CTA tallies of the hot cells (64-bit as two limbs)
-    if (HOT) for (int i = threadIdx.x; i <= kHot; i += blockDim.x) { s_hot_lo[i] = 0u; s_hot_hi[i] = 0u; s_hot_k[i] = 0u; }
-    constexpr int kDepth = RINGW ? kDepthRing : kDepthReg;
+    constexpr int kDepth = kDepthReg;
     extern __shared__ double2 smem_d2[];
+    // Per-CTA tallies of the hot cells, at the START of the dynamic shared memory (compile-time addresses): three
+    // words per cell -- the two limbs of the 64-bit Lucy tally and the absorption count.
+    unsigned int *s_hot = reinterpret_cast<unsigned int *>(smem_d2);
+    const int hot_words = HOT ? hot_smem_words(P.n_hot) : 0;
+    if (HOT) for (int i = threadIdx.x; i < hot_words; i += blockDim.x) s_hot[i] = 0u;
     const int nsf = P.ns * P.nf;
     const int nwarps = blockDim.x >> 5;
     constexpr int kPoolF64 = pool_bytes_per_warp(RECORD) / 8;
     constexpr int kNF64 = kSlotF64 + (RECORD ? 1 : 0);
-    double *s_pool = reinterpret_cast<double *>(smem_d2);                // [nwarps][pool_bytes_per_warp]
+    double *s_pool = reinterpret_cast<double *>(s_hot + hot_words);      // [nwarps][pool_bytes_per_warp]
     double2 *s_kk = reinterpret_cast<double2 *>(s_pool + (size_t)nwarps * kPoolF64);
     double2 *s_ag = s_kk + nsf;              // {albedo, g};  s_kk = {kext_h, kabs_fx}: one LDS.128 per crossing
     double *s_src = reinterpret_cast<double *>(s_ag + nsf);
@@ -652,12 +667,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     const int nhist = 2 * P.ndir * P.nf;
     uint32_t *s_m0x = s_hist + nhist;        // level-0 vacuum mask (one bit per brick)
     const int mw_smem = MCRT_SMEM_MASK ? P.mwords : 0;
+    // Eytzinger permutation of the frequency grid (grids of kPermSmem points and more read P.perm instead)
+    unsigned short *s_perm = reinterpret_cast<unsigned short *>(s_m0x + ((mw_smem + 1) & ~1));
+    if (P.nf < kPermSmem) for (int i = threadIdx.x; i <= P.nf; i += blockDim.x) s_perm[i] = P.perm[i];
     const uint32_t *s_m0 = MCRT_SMEM_MASK ? s_m0x : P.vmask;
-    // cell-word ring (RINGW): slot k of lane l of warp w at s_ring[(w * kRing + k) * 32 + l]
-    unsigned long long *s_ring = reinterpret_cast<unsigned long long *>(s_m0x + ((mw_smem + 1) & ~1));
-    char *ring = reinterpret_cast<char *>(s_ring + (threadIdx.x >> 5) * (kRing * 32) + (threadIdx.x & 31u));
-    constexpr int kRingStep = 32 * 8, kRingMask = (kRing - 1) * kRingStep;   // ring slots as byte offsets 0, 256, 512, ...
-#define RING(off) (*reinterpret_cast<volatile unsigned long long *>(ring + (off)))
 
     for (int i = threadIdx.x; i < nsf; i += blockDim.x) {
         s_kk[i] = make_double2(P.kext_h[i], P.kabs_fx[i]);
@@ -668,7 +681,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) s_hist[i] = 0u;
     for (int i = threadIdx.x; i < mw_smem; i += blockDim.x) s_m0x[i] = P.vmask[i];
     for (int i = threadIdx.x; i < 8 * nwarps; i += blockDim.x) s_cnt[i] = 0ull;   // eight counters per warp
-    if (RINGW) for (int i = threadIdx.x; i < kRing * (int)blockDim.x; i += blockDim.x) s_ring[i] = 0ull;   // every lane reads its ring in every step
     // Kernel parameters the walk loop uses, parked in shared memory: the S phase reads them into registers through
     // a volatile pointer, so that they stay there (left to itself the compiler reloads a dozen of them from the
     // constant bank in every iteration of the loop and waits for them)
@@ -724,11 +736,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at the packet's frequency
             uint32_t kq_sp = 0u;
             const double2 *kq_row = s_kk;                       // s_kk + j
-            // words of cells n .. n+kDepth-1: in registers, or in the ring (slot r = cell n; the same r in every lane)
+            // words of cells n .. n+kDepth-1, in registers
             unsigned long long cwr[kDepth];
 #pragma unroll
             for (int i = 0; i < kDepth; ++i) cwr[i] = 0ull;
-            int r = 0;
             double tq[kDepth - 1];                              // queue between G and the physics: exit parameter and storage
             uint32_t cq[kDepth - 1];                            // index of cells n+1 .. n+kDepth-2 (and of the cell G is in)
 #pragma unroll
@@ -768,8 +779,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // started: its slot is as the refill found it
                         // (its crossing count is still below the slot's)
                         if (state == ST_FLY && (int)(ncross - SU(U_NCROSS, slot)) >= 0) {
-                            if (RINGW) cp_async_wait<0>();
-                            const unsigned long long wn = RINGW ? RING(r) : cwr[0];
+                            const unsigned long long wn = cwr[0];
                             SU(U_NCROSS, slot) = ncross;
                             if (wn == kOutWord) {      // cell n lies outside the grid: the packet has escaped
                                 SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
@@ -788,7 +798,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool take = state == ST_IDLE && k < mFly.count();
                     if (take) {
                         slot = mFly.nth(k);
-                        if (RINGW) cp_async_wait<0>();            // no stale request may land in the ring later
                         px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
                         {   // 1/u per axis (reading Q8); +inf for a zero direction component: that axis never moves
 #if MCRT_SLOT_IV
@@ -822,11 +831,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // pipeline: kDepth - 1 no-op cells (zero length, vacuum word: nothing is tallied), then the packet's
                         // cell, in which G stands
 #pragma unroll
-                        for (int i = 0; i < kDepth - 1; ++i) {
-                            if (RINGW) RING((r + i * kRingStep) & kRingMask) = 0ull; else cwr[i] = 0ull;
-                        }
-                        if (RINGW) RING((r + (kDepth - 1) * kRingStep) & kRingMask) = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
-                        else cwr[kDepth - 1] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+                        for (int i = 0; i < kDepth - 1; ++i) cwr[i] = 0ull;
+                        cwr[kDepth - 1] = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
                         tprev = t; tnA = t; ciA = 0u;
 #pragma unroll
                         for (int i = 0; i < kDepth - 2; ++i) { tq[i] = t; cq[i] = 0u; }
@@ -849,11 +855,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // Shared memory is touched only by the rare events of a step (stop, change of species): the step's
                 // two global accesses (cell word, tally) already keep the SM's load/store data path busy.
                 int nnot;
-#define WALK_STEP(W, RC)                                                                                                      \
+#define WALK_STEP(W)                                                                                                          \
                 {                                                                                                           \
                     const bool fly = state == ST_FLY;                                                                       \
-                    if (RINGW) cp_async_wait<kDepth - 1>();           /* the word of cell n has landed */                   \
-                    const unsigned long long cw = RINGW ? RING(RC) : W;                                                     \
+                    const unsigned long long cw = W;                  /* the word of cell n (waits for its load) */        \
                     /* ---- G: the queue entry of cell n+1 (the cell G is in), then G advances to cell n+2 and loads its  */ \
                     /* word.  G stands still once its lane has stopped; until then it may run up to kGuard cells beyond  */ \
                     /* the grid (the storage has that many guard cells on every side).                                   */ \
@@ -865,12 +870,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                     \
                     /* the load of cell n+kDepth replaces, in place, the word just read (lanes without a flying packet   */ \
                     /* keep theirs): tied to W, so that no move has to wait for the load                                  */ \
-                    if (RINGW) {                                                                                            \
-                        if (fly) cp_async8(ring + (((RC) + kDepth * kRingStep) & kRingMask), cellw_r + kCS * gi);               \
-                        cp_async_commit();                                                                                  \
-                    } else                                                                                                  \
-                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"     \
-                                     : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly));                             \
+                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"         \
+                                 : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly));                                 \
                     /* parameter of the face through which the entered cell will be left (reading Q8): the face          */ \
                     /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'   */ \
                     /* f moves by its step, the others by 0, and all three t are recomputed: the same value for an axis  */ \
@@ -906,7 +907,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
                                      ::"l"(lfx_r + kCS * ciA), "l"(q), "r"(HOT ? cold : dusty) : "memory");                 \
                         if (HOT && __any_sync(kFull, dusty && hid != 0u)) {                                                 \
-                            if (dusty && hid != 0u) hot_add(s_hot_lo, s_hot_hi, hid, q);                                    \
+                            if (dusty && hid != 0u) hot_add(s_hot, hid, q);                                    \
                         }                                                                                                   \
                         ndusty_acc += dusty;                                                                                \
                     }                                                                                                       \
@@ -921,14 +922,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }                                                                                                       \
                 }
                 do {
-                    if (RINGW) {
-                        WALK_STEP(cwr[0], r)
-                        WALK_STEP(cwr[0], (r + kRingStep) & kRingMask)
-                        r = (r + 2 * kRingStep) & kRingMask;
-                    } else {
 #pragma unroll
-                        for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i], 0)
-                    }
+                    for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i])
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
 #undef WALK_STEP
             }
@@ -1063,7 +1058,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             // S0 refill: the slots that need a new packet take the next ids with ONE atomic per warp
             const unsigned need = __ballot_sync(kFull, kind == K_EMIT);
             bool dead = false, resume = false;
-            const unsigned long long n_take = P.count + P.n_carry_in;   // carried packets first, then new ids
+            const unsigned long long n_take = P.count + (XTRA ? P.n_carry_in : 0u);   // carried packets first, then new ids
             uint32_t resume_idx = 0u;
             if (need) {
                 unsigned long long base = n_take;
@@ -1074,8 +1069,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 }
                 if (kind == K_EMIT) {
                     const unsigned long long idx = base + (unsigned long long)__popc(need & ((1u << lane) - 1u));
-                    if (idx < P.n_carry_in) { resume = true; resume_idx = (uint32_t)idx; }
-                    else if (idx < n_take) pid = P.pid0 + (idx - P.n_carry_in);
+                    if (XTRA && idx < P.n_carry_in) { resume = true; resume_idx = (uint32_t)idx; }
+                    else if (idx < n_take) pid = P.pid0 + (idx - (XTRA ? P.n_carry_in : 0u));
                     else dead = true;
                 }
                 if (__any_sync(kFull, dead)) exhausted = true;   // the counter only grows
@@ -1088,7 +1083,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 int sj = 0;
                 unsigned long long cw;
                 uint32_t cidx;
-                if (resume) {
+                if (XTRA && resume) {
                     // a packet carried over from the previous epoch: its state as it was left behind an interaction
                     const CarryRec rc = P.carry_in[resume_idx];
                     pid = rc.pid; hash = rc.hash; px = rc.px; py = rc.py; pz = rc.pz; ux = rc.ux; uy = rc.uy; uz = rc.uz;
@@ -1103,7 +1098,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     hash = 0xCBF29CE484222325ull;
                     draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                     // Eq. 1: stratified over the cumulative source spectrum, stratum = pid mod S
-                    if (P.source_strata) z0 = ((double)(pid % P.source_strata) + z0) / (double)P.source_strata;
+                    if (XTRA && P.source_strata) z0 = ((double)(pid % P.source_strata) + z0) / (double)P.source_strata;
                     j = lower_bound_cdf(s_src, nf, z0);
                     px = P.px; py = P.py; pz = P.pz;
                     cw = 0ull; cidx = 0u;
@@ -1119,7 +1114,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double kk = kq.x * rho_c;
                     const double sint = tau / kk;
                     const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;
-                    if (hid) hot_add(s_hot_lo, s_hot_hi, hid, lucy_round(kq.y * rho_c * sint));
+                    if (hid) hot_add(s_hot, hid, lucy_round(kq.y * rho_c * sint));
                     else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
                     const double tint = t + sint;
                     double q;
@@ -1131,7 +1126,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     if (ztype < s_ag[sj].x) {
                         scatter = true;
                         nsca++;
-                        if (P.sca_slot && P.sca_slot[j] >= 0) {   // store the event: cell, frequency, incoming direction
+                        if (XTRA && P.sca_slot && P.sca_slot[j] >= 0) {   // store the event: cell, frequency, incoming direction
                             const unsigned long long at = atomicAdd(&P.counters[CNT_SCAEV], 1ull);
                             if (at < P.sca_cap) {
                                 mcrt_scatter_event ev;
@@ -1149,20 +1144,20 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         nabs++;
                         const int s = cw_species(cw);
                         int m = cw_tidx(cw, P.tidx_mask);
-                        if (P.live_bw) {
+                        if (XTRA && P.live_bw) {
                             // Bjorkman & Wood as printed: the temperature is adjusted after each
                             // absorption -- T_{i,k} from the count including this one (Eq. 4).  The count a packet sees
                             // depends on the order of the atomics: results are reproducible only statistically.
                             const unsigned long long kn = atomicAdd(&P.kcnt[cidx], 1ull) + 1ull;
                             m = t_index(P.J + s * P.nT, P.nT, (double)kn * P.cellfac / rho_c);
-                        } else if (hid) atomicAdd(&s_hot_k[hid], 1u);
+                        } else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
                         else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
-                        j = lower_bound_cdf(P.cdf + ((size_t)s * P.nT + m) * nf, nf, z0);
+                        j = lower_bound_eytzinger(P.cdf + ((size_t)s * P.nT + m) * P.nfs, nf < kPermSmem ? s_perm : P.perm, nf, z0);
                         if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
                     }
                 }
-                if (!resume) {
+                if (!(XTRA && resume)) {
                 // new direction: isotropic or Henyey-Greenstein about the old one (S7)
                 draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                 double mu = 1.0 - 2.0 * z0;
@@ -1210,7 +1205,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     cw = to_jump ? 0ull : __ldg(P.cellw + (size_t)kCS * cidx);
                     if (RECORD)
                         hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
-                } else if (P.carry_K && ++nint >= P.carry_K) {
+                } else if (XTRA && P.carry_K && ++nint >= P.carry_K) {
                     // carry-over: the interaction budget of this epoch is used up.  The packet's state goes to the
                     // list the next epoch starts with; the slot takes another packet.
                     carried = true;
@@ -1253,7 +1248,6 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
         }
     }
 #undef SF
-#undef RING
 #undef SU
     {   // dusty crossings stepped by this warp
         const uint32_t nd = __reduce_add_sync(kFull, ndusty_acc & 0xffffu), ndh = __reduce_add_sync(kFull, ndusty_acc >> 16);
@@ -1264,10 +1258,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     __syncthreads();
     if (HOT)
         for (int i = 1 + (int)threadIdx.x; i <= P.n_hot; i += blockDim.x) {
-            const unsigned long long v = ((unsigned long long)s_hot_hi[i] << 32) + s_hot_lo[i];
+            const unsigned long long v = ((unsigned long long)s_hot[3 * i + 1] << 32) + s_hot[3 * i];
             const uint32_t ci = P.hot_idx[i];
             if (v) lucy_add_raw(P.lfx, ci, v);
-            if (s_hot_k[i]) atomicAdd(&P.kcnt[ci], (unsigned long long)s_hot_k[i]);
+            if (s_hot[3 * i + 2]) atomicAdd(&P.kcnt[ci], (unsigned long long)s_hot[3 * i + 2]);
         }
     const int half = P.ndir * nf;
     for (int i = threadIdx.x; i < nhist; i += blockDim.x) {
@@ -1786,14 +1780,28 @@ int fx_bits_for(uint64_t n)
 
 // Shared memory of a transport CTA is kept within the 196 KB carve-out: above it 28 KB of L1 remain for the walk's
 // scattered loads, which measured 2x slower.
-constexpr size_t kMaxTransportSmem = 195 * 1024;
 
-size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record, bool ringw)
+size_t transport_smem_bytes(int ns, int nf, int ndir, int mask0_words, int threads, bool record, int n_hot)
 {
-    return (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
+    return (size_t)(n_hot > 0 ? hot_smem_words(n_hot) : 0) * sizeof(unsigned int) +
+           (size_t)(threads / 32) * pool_bytes_per_warp(record) + (size_t)(4 * ns * nf + nf + ndir + 1) * sizeof(double) +
            (size_t)(threads / 32) * 8 * sizeof(unsigned long long) + (size_t)2 * ndir * nf * sizeof(unsigned int) +
            (size_t)(MCRT_SMEM_MASK ? ((mask0_words + 1) & ~1) : 0) * sizeof(uint32_t) +
-           (ringw ? (size_t)kRing * threads * sizeof(unsigned long long) : 0);
+           (size_t)(nf < kPermSmem ? ((nf + 1 + 7) & ~7) : 0) * sizeof(unsigned short);
+}
+
+// The SM splits 256 KB between shared memory and L1 in fixed steps; a CTA also pays for the kernel's static shared
+// memory and 1 KB the system reserves.  The walk's scattered loads live on what is left for L1: on torus256 the step
+// from 164 KB to 196 KB of shared memory (92 -> 60 KB of L1) costs 5-6 % of the throughput (profiles/
+// r02_experiments.md, section 5), so the hot-cell tallies only take what the carve-out the pools need leaves over.
+constexpr size_t kSmemOverhead = 1024 + 64;
+constexpr size_t kMaxTransportSmem = 196 * 1024 - kSmemOverhead;
+size_t smem_carveout(size_t dynamic_bytes)
+{
+    static const int kb[] = {8, 16, 32, 64, 100, 132, 164, 196, 228};
+    for (int k : kb)
+        if (dynamic_bytes + kSmemOverhead <= (size_t)k * 1024) return (size_t)k * 1024;
+    return (size_t)228 * 1024;
 }
 
 // Geometry of the three vacuum-mask levels: level-0 boxes of (1 << msh)^3 cells, msh >= 2 the smallest for
@@ -1870,7 +1878,8 @@ int mcrt_workspace_bytes(int nx, int ny, int nz, int n_species, int n_nu, int n_
     for (int i = 0; i < 4; ++i) add(nsf * 8);
     add((size_t)n_nu * 8); add((size_t)n_nu * 8);            // srccdf, dnu
     add((size_t)n_species * n_T * 8); add((size_t)n_T * 8);  // J, Tg
-    add(nsf * n_T * 8); add(nsf * n_T * 8);                  // cdf_B, cdf_dB
+    { const size_t nfs = (size_t)(n_nu + 1 + 15) / 16 * 16; add((size_t)n_species * n_T * nfs * 8); add((size_t)n_species * n_T * nfs * 8); }   // cdf_B, cdf_dB (Eytzinger rows)
+    add((size_t)(n_nu + 1) * 2);                             // their permutation
     add((size_t)(n_dir + 1) * 8);
     add((size_t)n_dir * n_nu * 8); add((size_t)n_dir * n_nu * 8);
     add((size_t)n_dir * n_nu * 8);                           // SED staging
@@ -2008,7 +2017,7 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
         if (!(kappa_abs[i] + kappa_sca[i] > 0.0)) return fail(c, MCRT_EINVAL, "kappa_abs + kappa_sca must be > 0");
         if (!(fabs(g[i]) < 1.0)) return fail(c, MCRT_EINVAL, "|g| must be < 1");
     }
-    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256, true, true) > kMaxTransportSmem)
+    if (transport_smem_bytes(ns, n_nu, 16, c->mwords, 256, true, 0) > kMaxTransportSmem)
         return fail(c, MCRT_EINVAL, "n_species * n_nu too large for the shared-memory tables");
     c->nf = n_nu; c->nT = n_T;
     // low half of the cell word: species 0-7 | temperature index (12 or 16 bits) | hot-cell number (9 or 5 bits) | rho 29-31
@@ -2056,18 +2065,65 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
     if ((rc = ws_alloc(c, (void **)&c->d_dnu, (size_t)n_nu * 8))) return rc;
     if ((rc = ws_alloc(c, (void **)&c->d_J, (size_t)ns * n_T * 8))) return rc;
     if ((rc = ws_alloc(c, (void **)&c->d_Tg, (size_t)n_T * 8))) return rc;
-    if ((rc = ws_alloc(c, (void **)&c->d_cdfB, nsf * n_T * 8))) return rc;
-    if ((rc = ws_alloc(c, (void **)&c->d_cdfdB, nsf * n_T * 8))) return rc;
+    // the re-emission rows go to the device in Eytzinger order (lower_bound_eytzinger), 1-based, rows padded to 16 doubles
+    c->nfs = (n_nu + 1 + 15) / 16 * 16;
+    c->perm.assign(n_nu + 1, 0);
+    {
+        int next = 0;
+        std::vector<int> stack;               // in-order walk of the implicit tree: node k gets the next ascending position
+        int k = 1;
+        while (!stack.empty() || k <= n_nu) {
+            while (k <= n_nu) { stack.push_back(k); k = 2 * k; }
+            k = stack.back(); stack.pop_back();
+            c->perm[k] = (unsigned short)next++;
+            k = 2 * k + 1;
+        }
+    }
+    const size_t rows = (size_t)ns * n_T;
+    std::vector<double> eyt(rows * c->nfs, 2.0);   // (padding above every CDF value: never taken)
+    if ((rc = ws_alloc(c, (void **)&c->d_cdfB, rows * c->nfs * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_cdfdB, rows * c->nfs * 8))) return rc;
+    if ((rc = ws_alloc(c, (void **)&c->d_perm, (size_t)(n_nu + 1) * 2))) return rc;
     CUDA_TRY(c, cudaMemcpyAsync(c->d_kext_h, c->kext_h.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_albedo, c->albedo.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_g, c->g.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_dnu, c->dnu.data(), (size_t)n_nu * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_J, c->J.data(), (size_t)ns * n_T * 8, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaMemcpyAsync(c->d_Tg, c->Tg.data(), (size_t)n_T * 8, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_cdfB, c->cdfB.data(), nsf * n_T * 8, cudaMemcpyHostToDevice, c->stream));
-    CUDA_TRY(c, cudaMemcpyAsync(c->d_cdfdB, c->cdfdB.data(), nsf * n_T * 8, cudaMemcpyHostToDevice, c->stream));
+    for (int pass = 0; pass < 2; ++pass) {
+        const std::vector<double> &src = pass ? c->cdfdB : c->cdfB;
+        for (size_t r = 0; r < rows; ++r)
+            for (int k = 1; k <= n_nu; ++k) eyt[r * c->nfs + k] = src[r * n_nu + c->perm[k]];
+        CUDA_TRY(c, cudaMemcpyAsync(pass ? c->d_cdfdB : c->d_cdfB, eyt.data(), rows * c->nfs * 8, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_perm, c->perm.data(), (size_t)(n_nu + 1) * 2, cudaMemcpyHostToDevice, c->stream));
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     c->have_tables = true;
+    return MCRT_OK;
+}
+
+// Number the first n_use candidates (nearest first) as hot cells 1..n_use in their cell words, after clearing the
+// numbering in force.
+static int apply_hot(mcrt_ctx *c, int n_use)
+{
+    if (n_use > (int)c->hot_cand.size()) n_use = (int)c->hot_cand.size();
+    if (n_use == c->n_hot) return MCRT_OK;
+    uint32_t *d_stage = c->d_hot_idx + (kHot + 1);
+    std::vector<uint32_t> h_idx, h_id;
+    for (int i = 1; i <= c->n_hot; ++i) { h_idx.push_back(c->hot_idx[i]); h_id.push_back(0u); }
+    c->n_hot = n_use;
+    c->hot_idx.assign(kHot + 1, 0u);
+    for (int i = 1; i <= c->n_hot; ++i) { c->hot_idx[i] = c->hot_cand[i - 1]; h_idx.push_back(c->hot_idx[i]); h_id.push_back((uint32_t)i); }
+    const int n = (int)h_idx.size();       // <= 2 kHot
+    if (n) {
+        CUDA_TRY(c, cudaMemcpyAsync(d_stage, h_idx.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
+        CUDA_TRY(c, cudaMemcpyAsync(d_stage + 2 * (kHot + 1), h_id.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
+        k_set_hot<<<(n + 127) / 128, 128, 0, c->stream>>>(c->cellw, d_stage, d_stage + 2 * (kHot + 1), n, c->hot_shift, c->hot_mask);
+        CUDA_TRY(c, cudaGetLastError());
+    }
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_hot_idx, c->hot_idx.data(), (kHot + 1) * 4, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MCRT_OK;
 }
 
@@ -2137,21 +2193,10 @@ int mcrt_source(mcrt_ctx *c, double L_erg_s, double T_star_K, const double *L_nu
         }
         std::stable_sort(dusty.begin(), dusty.end(), [](const Cand &a, const Cand &b) { return a.d2 < b.d2 || (a.d2 == b.d2 && a.idx < b.idx); });
         if ((int)dusty.size() > c->hot_max) dusty.resize(c->hot_max);
-        // clear the previous numbering, then number the new set
-        std::vector<uint32_t> h_idx, h_id;
-        for (int i = 1; i <= c->n_hot; ++i) { h_idx.push_back(c->hot_idx[i]); h_id.push_back(0u); }
-        c->n_hot = (int)dusty.size();
-        c->hot_idx.assign(kHot + 1, 0u);
-        for (int i = 1; i <= c->n_hot; ++i) { c->hot_idx[i] = dusty[i - 1].idx; h_idx.push_back(c->hot_idx[i]); h_id.push_back((uint32_t)i); }
-        const int n = (int)h_idx.size();       // <= 2 kHot
-        if (n) {
-            CUDA_TRY(c, cudaMemcpyAsync(d_stage, h_idx.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
-            CUDA_TRY(c, cudaMemcpyAsync(d_stage + 2 * (kHot + 1), h_id.data(), n * 4, cudaMemcpyHostToDevice, c->stream));
-            k_set_hot<<<(n + 127) / 128, 128, 0, c->stream>>>(c->cellw, d_stage, d_stage + 2 * (kHot + 1), n, c->hot_shift, c->hot_mask);
-            CUDA_TRY(c, cudaGetLastError());
-        }
-        CUDA_TRY(c, cudaMemcpyAsync(c->d_hot_idx, c->hot_idx.data(), (kHot + 1) * 4, cudaMemcpyHostToDevice, c->stream));
-        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        // the previous source's numbering goes; the new one is written when a run knows how many cells it can hold
+        if ((rc2 = apply_hot(c, 0))) return rc2;
+        c->hot_cand.clear();
+        for (const Cand &d : dusty) c->hot_cand.push_back(d.idx);
     }
     c->have_source = true;
     return MCRT_OK;
@@ -2192,32 +2237,39 @@ static int ensure_histograms(mcrt_ctx *c)
 
 // the eight instantiations of the transport kernel
 typedef void (*transport_fn)(const TransportParams);
-static transport_fn transport_kernel(bool record, bool ringw, bool hot)
+// (digests recorded, hot cells tallied per CTA, any of the rarely used extras: carry-over, scattering-event store,
+// stratified source, live B&W -- compiled out of the default kernels: the kernel's code has to fit the instruction
+// cache, and every feature inlined into the event phase cost 1-4 % of the default path's throughput)
+static transport_fn transport_kernel(bool record, bool hot, bool xtra)
 {
     static const transport_fn tab[8] = {k_transport<false, false, false>, k_transport<true, false, false>,
                                         k_transport<false, true, false>,  k_transport<true, true, false>,
                                         k_transport<false, false, true>,  k_transport<true, false, true>,
                                         k_transport<false, true, true>,   k_transport<true, true, true>};
-    return tab[(record ? 1 : 0) | (ringw ? 2 : 0) | (hot ? 4 : 0)];
+    return tab[(record ? 1 : 0) | (hot ? 2 : 0) | (xtra ? 4 : 0)];
 }
 
-// which walk variant
-static bool use_ring(const mcrt_ctx *c, const mcrt_run_opts *o)
-{
-    (void)c;
-    return o && o->walk_words == 2;      // auto = registers: the ring was never faster (see kDepthRing)
-}
-
-static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem)
+static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem, int *n_hot)
 {
     const bool record = o && o->record_digests;
-    const bool ringw = use_ring(c, o);
     *threads = (o && o->block_threads > 0) ? o->block_threads : MCRT_MAX_THREADS;
     if (*threads % 32 || *threads > MCRT_MAX_THREADS || *threads < 32)
         return fail(c, MCRT_EINVAL, "block_threads must be a multiple of 32 in 32.." + std::to_string(MCRT_MAX_THREADS));
-    // as many warps (each with its packet pool) as fit beside the tables in 227 KB of shared memory
-    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, ringw) > kMaxTransportSmem) *threads -= 32;
-    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, ringw);
+    // as many warps (each with its packet pool) as fit beside the tables in the 196 KB carve-out
+    while (*threads > 32 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0) > kMaxTransportSmem) *threads -= 32;
+    // up to two warps fewer if that gets from the 196 KB carve-out into the 164 KB one (torus512: 576 threads beside
+    // 92 KB of L1 are 4.5 % faster than 640 beside 60 KB; within one carve-out a warp less costs 1-2.5 %)
+    if (!(o && o->block_threads > 0) && smem_carveout(transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0)) > 164 * 1024)
+        for (int t = *threads - 32; t >= *threads - 64 && t >= 32; t -= 32)
+            if (smem_carveout(transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, t, record, 0)) <= 164 * 1024) { *threads = t; break; }
+    const size_t base = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0);
+    // ... and as many hot cells as the carve-out these need leaves room for (live B&W needs every count in global memory)
+    int nh = (o && (o->no_hot_cells || o->mode == MCRT_MODE_LIVE_BW)) ? 0 : (int)c->hot_cand.size();
+    const size_t cap = smem_carveout(base) - kSmemOverhead;
+    while (nh > 0 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh) > cap) --nh;
+    if (nh < 8) nh = 0;
+    *n_hot = nh;
+    *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh);
     if (*smem > 48 * 1024) {
         for (int v = 0; v < 8; ++v)
             CUDA_TRY(c, cudaFuncSetAttribute(transport_kernel(v & 1, v & 2, v & 4), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
@@ -2236,8 +2288,8 @@ int mcrt_launch_config(mcrt_ctx *c, int *grid_blocks, int *block_threads, size_t
     if (!c || !c->have_tables) return c ? fail(c, MCRT_ESTATE, "tables not set") : MCRT_EINVAL;
     int rc = ensure_histograms(c);
     if (rc) return rc;
-    int b, t; size_t s;
-    if ((rc = transport_config(c, nullptr, &b, &t, &s))) return rc;
+    int b, t, nh; size_t s;
+    if ((rc = transport_config(c, nullptr, &b, &t, &s, &nh))) return rc;
     if (grid_blocks) *grid_blocks = b;
     if (block_threads) *block_threads = t;
     if (smem_bytes) *smem_bytes = s;
@@ -2273,7 +2325,7 @@ int mcrt_get_stats(mcrt_ctx *c, mcrt_run_stats *st)
 static void launch_transport(mcrt_ctx *c, const TransportParams &P)
 {
     const mcrt_ctx::Run &R = c->run;
-    transport_kernel(R.o.record_digests != 0, R.ringw, R.hot)<<<R.blocks, R.threads, R.smem, c->stream>>>(P);
+    transport_kernel(R.o.record_digests != 0, R.hot, R.xtra)<<<R.blocks, R.threads, R.smem, c->stream>>>(P);
 }
 
 static void fill_params(mcrt_ctx *c, TransportParams &P)
@@ -2289,6 +2341,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
+    P.nfs = c->nfs; P.perm = c->d_perm;
     P.nbx = c->nbx; P.nby = c->nby;
     P.vmask = c->vmask; P.vbox = c->vbox; P.bsh = c->msh; P.mwords = c->mwords; P.ncp = (uint32_t)c->ncp;
     P.lpx = c->px; P.lpxy = c->pxy; P.inv_lpx = 1.0 / (double)c->px; P.inv_lpxy = 1.0 / (double)c->pxy;
@@ -2395,16 +2448,17 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (o.epoch_growth == 0.0) o.epoch_growth = 2.0;
     if (o.carry_interactions > 65535u) return fail(c, MCRT_EINVAL, "carry_interactions must be <= 65535");
     if (o.carry_interactions && o.part_count > 1) return fail(c, MCRT_EINVAL, "carry_interactions is not available in a partitioned run");
-    if (o.walk_words < 0 || o.walk_words > 2) return fail(c, MCRT_EINVAL, "walk_words must be 0 (auto), 1 (registers) or 2 (ring)");
     if (!(o.epoch_growth >= 1.0) || !isfinite(o.epoch_growth)) return fail(c, MCRT_EINVAL, "epoch_growth must be >= 1");
     if (o.n_total && o.n_total < n_packets) return fail(c, MCRT_EINVAL, "n_total must be >= n_packets");
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
     int rc = ensure_histograms(c);
     if (rc) return rc;
     mcrt_ctx::Run &R = c->run;
-    if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem))) return rc;
-    R.ringw = use_ring(c, &o);
-    R.hot = c->n_hot > 0 && !o.no_hot_cells && o.mode != MCRT_MODE_LIVE_BW;   // (live B&W needs every count in global memory)
+    int n_hot = 0;
+    if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
+    if ((rc = apply_hot(c, n_hot))) return rc;
+    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW;
+    R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
     const uint64_t n_xi = o.n_total ? o.n_total : n_packets;
@@ -2874,8 +2928,17 @@ int mcrt_read_tables(mcrt_ctx *c, double *dnu, double *J, double *cdf_B, double 
     // read back from the DEVICE copies: these are the values the kernels use
     if (dnu) CUDA_TRY(c, cudaMemcpyAsync(dnu, c->d_dnu, (size_t)c->nf * 8, cudaMemcpyDeviceToHost, c->stream));
     if (J) CUDA_TRY(c, cudaMemcpyAsync(J, c->d_J, (size_t)c->ns * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
-    if (cdf_B) CUDA_TRY(c, cudaMemcpyAsync(cdf_B, c->d_cdfB, nsf * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
-    if (cdf_dB) CUDA_TRY(c, cudaMemcpyAsync(cdf_dB, c->d_cdfdB, nsf * c->nT * 8, cudaMemcpyDeviceToHost, c->stream));
+    for (int pass = 0; pass < 2; ++pass) {
+        double *dst = pass ? cdf_dB : cdf_B;
+        if (!dst) continue;
+        // the device rows are in Eytzinger order: read them back and put them in ascending order again
+        const size_t rows = (size_t)c->ns * c->nT;
+        std::vector<double> eyt(rows * c->nfs);
+        CUDA_TRY(c, cudaMemcpyAsync(eyt.data(), pass ? c->d_cdfdB : c->d_cdfB, rows * c->nfs * 8, cudaMemcpyDeviceToHost, c->stream));
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        for (size_t r = 0; r < rows; ++r)
+            for (int k = 1; k <= c->nf; ++k) dst[r * c->nf + c->perm[k]] = eyt[r * c->nfs + k];
+    }
     if (albedo) CUDA_TRY(c, cudaMemcpyAsync(albedo, c->d_albedo, nsf * 8, cudaMemcpyDeviceToHost, c->stream));
     if (src_cdf) {
         if (!c->have_source) return fail(c, MCRT_ESTATE, "source not set");

@@ -629,28 +629,6 @@ def test_parity_scattering_store_and_ray_tracer(B, orc):
     c.close()
 
 
-@pytest.mark.parametrize("walk_words", [1, 2])
-def test_parity_both_walk_variants(B, orc, walk_words):
-    """The two ways the walk keeps its cell words in flight (registers, 2 cells ahead / cp.async ring, 4 cells
-    ahead; chosen per grid at run time) against the oracle, in both kernel instantiations, with saturated pools."""
-    w = W.torus256(n_clumps=400, n=64)
-    N = 150_000
-    o = orc.Oracle.from_workload(w)
-    ro = o.run(N, 31, n_threads=NTH, digests=True)
-    raw_o = o.read_raw()
-    c = B.Context(w, n_digests=N)
-    for rec, blocks in ((0, 0), (1, 3)):
-        st = c.run(N, 31, record_digests=rec, walk_words=walk_words, grid_blocks=blocks)
-        raw = c.read_raw(digests=bool(rec))
-        for key in RAW_KEYS:
-            assert np.array_equal(raw_o[key], raw[key]), (key, rec)
-        for key in COUNTERS:
-            assert st[key] == ro[key], (key, rec)
-        if rec:
-            assert np.array_equal(ro["digests"], raw["digests"])
-    c.close()
-
-
 def test_sed_read_to_host_on_a_tiny_grid(B, orc):
     """n_dir * n_nu far larger than the cell count -- the SED staging buffer is its own allocation."""
     w = W.uniform_cube(2, 1.0, 0.5, 0.3, n_nu=120, n_dir=9)
