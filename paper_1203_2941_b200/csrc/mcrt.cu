@@ -326,13 +326,43 @@ __device__ __forceinline__ int lower_bound_cdf(const double *cdf, int n, double 
     return lo;
 }
 
+// L1 policy of the walk's cell-word loads and of the event phase's table loads (CDF rows, empty boxes).  Measured
+// (profiles/r02_experiments.md, section 6): cell words kept longest +0.3-0.8 %; tables kept out of L1 -3 %.
+#ifndef MCRT_TABLE_POLICY
+#define MCRT_TABLE_POLICY ""
+#endif
+// Two walk-loop variants that lost (profiles/r02_experiments.md, section 6), kept selectable:
+//   MCRT_ROT4         four steps per iteration with the two words in flight rotating through four registers and
+//                     unpredicated loads (no copy and no wait for the loads at the end of an iteration): -6.5 %
+//   MCRT_STOP_RELOAD  a stopped packet's cell word is loaded again instead of being stored at the stop: -5 %
+#ifndef MCRT_ROT4
+#define MCRT_ROT4 0
+#endif
+#ifndef MCRT_STOP_RELOAD
+#define MCRT_STOP_RELOAD 0
+#endif
+#ifndef MCRT_CW_POLICY
+#define MCRT_CW_POLICY ".L1::evict_last"
+#endif
+__device__ __forceinline__ double ldg_table(const double *p)
+{
+    double v;
+    asm volatile("ld.global.nc" MCRT_TABLE_POLICY ".f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint4 ldg_table(const uint4 *p)
+{
+    uint4 v;
+    asm volatile("ld.global.nc" MCRT_TABLE_POLICY ".v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
 // The same lower bound on a row stored in Eytzinger (breadth-first) order, 1-based, the row 128-byte aligned: the
 // first four levels of the search (entries 1..15) share one cache line, so a search costs about four round trips to
 // L2 instead of seven or eight.  perm[k] = position of entry k in ascending order.
 __device__ __forceinline__ int lower_bound_eytzinger(const double *__restrict__ row, const unsigned short *__restrict__ perm, int n, double z)
 {
     int k = 1;
-    while (k <= n) k = 2 * k + ((__ldg(row + k) < z) ? 1 : 0);
+    while (k <= n) k = 2 * k + ((ldg_table(row + k) < z) ? 1 : 0);
     k >>= __ffs(~k);
     return (int)perm[k];
 }
@@ -738,6 +768,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const double2 *kq_row = s_kk;                       // s_kk + j
             // words of cells n .. n+kDepth-1, in registers
             unsigned long long cwr[kDepth];
+            unsigned long long wstop = 0ull;             // cell word of the cell this lane's packet stopped in (MCRT_STOP_RELOAD)
 #pragma unroll
             for (int i = 0; i < kDepth; ++i) cwr[i] = 0ull;
             double tq[kDepth - 1];                              // queue between G and the physics: exit parameter and storage
@@ -759,7 +790,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // stopped in the walk below, which stored the flight's state in the slot; what kind of stop is
                         // read off the cell word: a marker word (rho = +inf) is a cell outside the grid (bit 8) or the
                         // first cell of a run of empty bricks, anything else an interaction in that cell
+#if MCRT_STOP_RELOAD
+                        const unsigned long long scw = wstop;
+                        SF(F_CW, slot) = __longlong_as_double((long long)scw);
+#else
                         const unsigned long long scw = (unsigned long long)__double_as_longlong(SF(F_CW, slot));
+#endif
                         const bool mk = (uint32_t)(scw >> 32) == kMarkHi;
                         state = mk ? (((uint32_t)scw & kOutFlag) ? ST_DONE : ST_JUMP) : ST_INTERACT;
                         if (state == ST_DONE) SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
@@ -855,7 +891,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // Shared memory is touched only by the rare events of a step (stop, change of species): the step's
                 // two global accesses (cell word, tally) already keep the SM's load/store data path busy.
                 int nnot;
-#define WALK_STEP(W)                                                                                                          \
+#define WALK_STEP(W, WN)                                                                                                         \
                 {                                                                                                           \
                     const bool fly = state == ST_FLY;                                                                       \
                     const unsigned long long cw = W;                  /* the word of cell n (waits for its load) */        \
@@ -867,10 +903,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool sely = !selx && (tmy <= tmz);                                                                \
                     const bool selz = !selx && !sely;                                                                       \
                     const double tnN = selx ? tmx : (sely ? tmy : tmz);                                                     \
-                    gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                     \
+                    if (MCRT_ROT4) gi = fly ? gi + (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                  \
+                    else gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                \
                     /* the load of cell n+kDepth replaces, in place, the word just read (lanes without a flying packet   */ \
                     /* keep theirs): tied to W, so that no move has to wait for the load                                  */ \
-                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"         \
+                    if (MCRT_ROT4) asm("ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];" : "=l"(WN) : "l"(cellw_r + kCS * gi));     \
+                    else                                                                                                    \
+                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];\n\t}" \
                                  : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly));                                 \
                     /* parameter of the face through which the entered cell will be left (reading Q8): the face          */ \
                     /* coordinate f is kept as a double (integers are exact), t = (f - p) * (1/u).  The selected axis'   */ \
@@ -895,8 +934,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     if (fly && stop) {                                                                                      \
                         state = ST_STOP;                                                                                    \
                         SU(U_NCROSS, slot) = ncross; SU(U_W0, slot) = ciA;                                                  \
-                        SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau; SF(F_CW, slot) = __longlong_as_double((long long)cw); \
+                        SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau;                                                       \
+                        if (!MCRT_STOP_RELOAD) SF(F_CW, slot) = __longlong_as_double((long long)cw);                        \
                     }                                                                                                       \
+                    /* the stopped packet's cell word is read again (rare; an L1 hit) instead of being kept: its register */ \
+                    /* is then free for the load above, which otherwise needs a copy and a wait at the end of the loop  */ \
+                    if (MCRT_STOP_RELOAD)                                                                                   \
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc.u64 %0, [%1];\n\t}"      \
+                                     : "+l"(wstop) : "l"(cellw_r + kCS * ciA), "r"((uint32_t)(fly && stop)));               \
                     /* S5: tally of a traversed dusty cell (a vacuum cell has nothing to add) */                           \
                     {                                                                                                       \
                         const unsigned long long q = lucy_round(kq.y * rho_c * ds);                                         \
@@ -921,10 +966,27 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         tq[kDepth - 3 >= 0 ? kDepth - 3 : 0] = tnN; cq[kDepth - 3 >= 0 ? kDepth - 3 : 0] = ciN;             \
                     }                                                                                                       \
                 }
+#if MCRT_ROT4
+                static_assert(kDepth == 2, "the rotating walk loop is written for two words in flight");
+                unsigned long long cw2, cw3;
+                for (;;) {
+                    WALK_STEP(cwr[0], cw2)
+                    WALK_STEP(cwr[1], cw3)
+                    nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
+                    if (nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) { cwr[0] = cw2; cwr[1] = cw3; break; }
+                    WALK_STEP(cw2, cwr[0])
+                    WALK_STEP(cw3, cwr[1])
+                    nnot = __popc(__ballot_sync(kFull, state != ST_FLY));
+                    // (the empty statement gives this exit a block of its own: without it the copies that bring both
+                    // exits' words into the same registers are placed in the loop, behind a wait for the loads)
+                    if (nnot - nidle >= MCRT_SWAP_MIN || nnot == 32) { asm volatile(""); break; }
+                }
+#else
                 do {
 #pragma unroll
-                    for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i])
+                    for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i], cwr[i])
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
+#endif
 #undef WALK_STEP
             }
             __syncwarp();
@@ -967,7 +1029,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             do {
                 if (busy) {
                     // the precomputed box of empty bricks around this brick, in cells, clipped to the grid
-                    const uint4 bb = __ldg(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
+                    const uint4 bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
                     const int lox = (int)(bb.x & 0xffffu) << bsh, loy = (int)(bb.x >> 16) << bsh, loz = (int)(bb.y & 0xffffu) << bsh;
                     const int hix = min((int)(bb.y >> 16) << bsh, P.nx), hiy = min((int)(bb.z & 0xffffu) << bsh, P.ny),
                               hiz = min((int)(bb.z >> 16) << bsh, P.nz);
