@@ -352,10 +352,10 @@ def run_ours(args, workload_name=None):
     res_b = resident_bytes(w)
     if res_b < 0.8 * L2_BYTES:
         # the arrays fit L2 -- report against a MEASURED L2 read bandwidth
-        l2 = B.mcrt_measure_read_bandwidth(32 << 20, 10)
+        l2 = B.mcrt_measure_read_bandwidth(64 << 20, 10)
         roofline.update({"bound": "l2", "peak": l2, "frac": achieved / l2,
                          "frac_dusty_only": roofline["frac_dusty_only"] * peak / l2,
-                         "peak_source": "measured here: mcrt_measure_read_bandwidth, 32 MiB buffer resident in L2",
+                         "peak_source": "measured here: mcrt_measure_read_bandwidth, 64 MiB buffer resident in L2",
                          "frac_of_hbm_peak": achieved / peak, "hbm_peak": peak,
                          "resident_bytes": res_b})
     # DRAM traffic of one k_transport launch from the committed ncu capture (profiles/traffic.csv), scaled from the

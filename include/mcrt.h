@@ -220,8 +220,9 @@ int mcrt_epoch_schedule(uint64_t n_packets, uint64_t epoch_B0, uint64_t epoch_Bm
 int mcrt_part_slice(uint64_t count, int part_index, int part_count, uint64_t *lo_out, uint64_t *hi_out);
 
 /* Measurement aid (configurations whose arrays fit L2 are reported against a MEASURED L2 read
- * bandwidth): streams a device buffer of `bytes` bytes `repeats` times with 16-byte loads from every SM and
- * returns the best read rate in GB/s.  A buffer far below the L2 size measures L2, a far larger one HBM. */
+ * bandwidth): `repeats` timed launches (after two warm-up launches), each sweeping a device buffer of `bytes`
+ * bytes with 16-byte loads from every SM until about 4 GB have been read; returns the best read rate in GB/s.
+ * A buffer far below the L2 size measures L2, a far larger one HBM. */
 int mcrt_measure_read_bandwidth(size_t bytes, int repeats, double *gb_per_s_out);
 
 /* Synchronise and return the counters accumulated since the last reset. */

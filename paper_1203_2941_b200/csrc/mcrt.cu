@@ -326,6 +326,22 @@ __device__ __forceinline__ int lower_bound_cdf(const double *cdf, int n, double 
     return lo;
 }
 
+// -DMCRT_CHECK=1: a debug build in which every index the transport kernel computes is checked before it is used
+// (compute-sanitizer is not available on the pool this was developed on); a violation prints its site and traps.
+#ifndef MCRT_CHECK
+#define MCRT_CHECK 0
+#endif
+#if MCRT_CHECK
+#define MCRT_CHK(cond, what)                                                                                              \
+    do {                                                                                                                  \
+        if (!(cond)) {                                                                                                    \
+            printf("MCRT_CHECK failed: %s (line %d, block %d thread %d)\n", what, __LINE__, (int)blockIdx.x, (int)threadIdx.x); \
+            __trap();                                                                                                     \
+        }                                                                                                                 \
+    } while (0)
+#else
+#define MCRT_CHK(cond, what) do { } while (0)
+#endif
 // L1 policy of the walk's cell-word loads and of the event phase's table loads (CDF rows, empty boxes).  Measured
 // (profiles/r02_experiments.md, section 6): cell words kept longest +0.3-0.8 %; tables kept out of L1 -3 %.
 #ifndef MCRT_TABLE_POLICY
@@ -452,7 +468,7 @@ struct TransportParams {
     int bsh;            // log2 of the brick edge
     int mwords;         // 32-bit words of the mask
     double px, py, pz;  // source position, cell units
-    unsigned long long pid0, count, dig_base;
+    unsigned long long pid0, count, dig_base, dig_n;
     const CarryRec *__restrict__ carry_in;     // packets carried over from the previous epoch: taken before new ids
     CarryRec *__restrict__ carry_out;          // packets whose budget runs out in this launch (counters[CNT_CARRY] of them)
     uint32_t n_carry_in, carry_K;              // carry_K = 0: no budget
@@ -907,6 +923,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     else gi += fly ? (selx ? dgx : (sely ? dgy : dgz)) : 0u;                                                \
                     /* the load of cell n+kDepth replaces, in place, the word just read (lanes without a flying packet   */ \
                     /* keep theirs): tied to W, so that no move has to wait for the load                                  */ \
+                    MCRT_CHK(!fly || gi < P.ncp, "walk: storage index of the prefetched cell");                             \
                     if (MCRT_ROT4) asm("ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];" : "=l"(WN) : "l"(cellw_r + kCS * gi));     \
                     else                                                                                                    \
                     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];\n\t}" \
@@ -927,7 +944,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double rho_c = cw_rho(cw);                                                                        \
                     if (cw_species(cw) != kq_sp) {   /* opacities of this species at the packet's frequency */              \
                         kq_sp = cw_species(cw);                                                                             \
-                        kq = kq_row[kq_sp * nf_r];                                                                          \
+                        MCRT_CHK(!fly || kq_sp < (uint32_t)P.ns, "walk: species of the cell word");                         \
+                        kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
                     }                                                                                                       \
                     const double dtau = kq.x * rho_c * ds;            /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */ \
                     const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
@@ -949,6 +967,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         const uint32_t dusty = (go && __double2hiint(rho_c) != 0) ? 1u : 0u;                                \
                         const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;   /* tallied in the CTA's own copy */ \
                         const uint32_t cold = (dusty && hid == 0u) ? 1u : 0u;                                               \
+                        MCRT_CHK(!dusty || ciA < P.ncp, "walk: storage index of the tallied cell");                         \
+                        MCRT_CHK(hid <= (uint32_t)P.n_hot, "walk: hot-cell number");                                        \
+                        MCRT_CHK(!(fly && stop) || (uint32_t)slot < (uint32_t)kSlots, "walk: slot of the stopped packet");   \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
                                      ::"l"(lfx_r + kCS * ciA), "l"(q), "r"(HOT ? cold : dusty) : "memory");                 \
                         if (HOT && __any_sync(kFull, dusty && hid != 0u)) {                                                 \
@@ -1029,6 +1050,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             do {
                 if (busy) {
                     // the precomputed box of empty bricks around this brick, in cells, clipped to the grid
+                    MCRT_CHK(ix >= 0 && iy >= 0 && iz >= 0 && ix < P.nx && iy < P.ny && iz < P.nz, "jump: cell coordinates");
                     const uint4 bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
                     const int lox = (int)(bb.x & 0xffffu) << bsh, loy = (int)(bb.x >> 16) << bsh, loz = (int)(bb.y & 0xffffu) << bsh;
                     const int hix = min((int)(bb.y >> 16) << bsh, P.nx), hiy = min((int)(bb.z & 0xffffu) << bsh, P.ny),
@@ -1103,6 +1125,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 const double amu = fabs(uz);
                 int bin = 0;
                 for (int b = 1; b < P.ndir; ++b) if (s_mu[b] <= amu) bin = b;
+                MCRT_CHK(bin >= 0 && bin < P.ndir && j >= 0 && j < nf, "escape: histogram bin");
                 atomicAdd(&s_hist[bin * nf + j], 1u);
                 const bool direct = (nsca + nabs) == 0u;
                 if (direct) atomicAdd(&s_hist[P.ndir * nf + bin * nf + j], 1u);
@@ -1113,6 +1136,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     mcrt_digest dg;
                     dg.hash = hash; dg.crossings = ncross; dg.scatterings = nsca; dg.absorptions = nabs;
                     dg.escape_bin = (uint32_t)bin;
+                    MCRT_CHK(pid - P.dig_base < P.dig_n, "escape: digest index");
                     P.dig[pid - P.dig_base] = dg;
                 }
                 kind = K_EMIT;        // the slot takes the next packet of the epoch
@@ -1204,6 +1228,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
                         nabs++;
+                        MCRT_CHK(cidx < P.ncp, "absorption: storage index of the cell");
                         const int s = cw_species(cw);
                         int m = cw_tidx(cw, P.tidx_mask);
                         if (XTRA && P.live_bw) {
@@ -1215,6 +1240,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         } else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
                         else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
+                        MCRT_CHK(s >= 0 && s < P.ns && m >= 0 && m < P.nT, "absorption: CDF row");
                         j = lower_bound_eytzinger(P.cdf + ((size_t)s * P.nT + m) * P.nfs, nf < kPermSmem ? s_perm : P.perm, nf, z0);
                         if (RECORD) hash_mix(hash, event_word(EV_ABSORB, j, cell));
                     }
@@ -1761,20 +1787,23 @@ __global__ void __launch_bounds__(128) k_ray_trace(RayParams R, const unsigned l
     if (Fs) Fs[pixi] = fs * R.apix_d2;
 }
 
-// read-bandwidth probe: every thread sums 16-byte words of a buffer with a grid stride, eight loads in flight
-__global__ void __launch_bounds__(512) k_read_probe(const uint4 *__restrict__ buf, size_t n16, unsigned long long *__restrict__ sink)
+// read-bandwidth probe: `passes` sweeps over a buffer, every thread summing 16-byte words with a grid stride, eight
+// loads in flight
+__global__ void __launch_bounds__(512) k_read_probe(const uint4 *__restrict__ buf, size_t n16, int passes, unsigned long long *__restrict__ sink)
 {
     unsigned long long acc = 0ull;
     const size_t stride = (size_t)gridDim.x * blockDim.x;
-    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    for (; i + 7 * stride < n16; i += 8 * stride) {
-        uint4 v[8];
+    for (int pass = 0; pass < passes; ++pass) {
+        size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+        for (; i + 7 * stride < n16; i += 8 * stride) {
+            uint4 v[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) v[k] = __ldcg(buf + i + k * stride);   // L2, not L1: what a resident grid's arrays see
+            for (int k = 0; k < 8; ++k) v[k] = __ldcg(buf + i + k * stride);   // L2, not L1: what a resident grid's arrays see
 #pragma unroll
-        for (int k = 0; k < 8; ++k) acc += (unsigned long long)(v[k].x ^ v[k].y) + (unsigned long long)(v[k].z ^ v[k].w);
+            for (int k = 0; k < 8; ++k) acc += (unsigned long long)(v[k].x ^ v[k].y) + (unsigned long long)(v[k].z ^ v[k].w);
+        }
+        for (; i < n16; i += stride) { const uint4 v = __ldcg(buf + i); acc += (unsigned long long)(v.x ^ v.y) + (unsigned long long)(v.z ^ v.w); }
     }
-    for (; i < n16; i += stride) { const uint4 v = __ldcg(buf + i); acc += (unsigned long long)(v.x ^ v.y) + (unsigned long long)(v.z ^ v.w); }
     if (acc == 0x123456789abcdefull) sink[0] = acc;   // keeps the loads alive
 }
 
@@ -2401,7 +2430,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.sca_slot = c->sca_ev ? c->d_sca_slot : nullptr; P.sca_ev = c->sca_ev; P.sca_cap = c->sca_cap;
     P.hot_idx = c->d_hot_idx; P.hot_shift = c->hot_shift; P.hot_mask = c->hot_mask; P.tidx_mask = c->tidx_mask; P.n_hot = c->n_hot;
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
-    P.dig_base = c->dig_base;
+    P.dig_base = c->dig_base; P.dig_n = c->dig_n;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
     P.nfs = c->nfs; P.perm = c->d_perm;
     P.nbx = c->nbx; P.nby = c->nby;
@@ -2475,15 +2504,20 @@ int mcrt_measure_read_bandwidth(size_t bytes, int repeats, double *gb_per_s_out)
     if (err == cudaSuccess) err = cudaEventCreate(&e1);
     int nsm = 148;
     cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, 0);
+    // a launch long enough (about a millisecond) that its start and end do not count, and few enough threads that
+    // every one keeps eight loads in flight
+    int blocks = nsm * 4;
+    while (blocks > nsm && (size_t)blocks * 512 * 16 > n16) blocks -= nsm;
+    const int passes = (int)std::min<size_t>(4096, std::max<size_t>(1, ((size_t)4 << 30) / (n16 * 16)));
     double best = 0.0;
-    for (int r = 0; err == cudaSuccess && r < repeats + 2; ++r) {     // two warm-up passes
+    for (int r = 0; err == cudaSuccess && r < repeats + 2; ++r) {     // two warm-up launches
         cudaEventRecord(e0);
-        k_read_probe<<<nsm * 4, 512>>>((const uint4 *)buf, n16, sink);
+        k_read_probe<<<blocks, 512>>>((const uint4 *)buf, n16, passes, sink);
         cudaEventRecord(e1);
         err = cudaEventSynchronize(e1);
         float ms = 0.f;
         if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-        if (err == cudaSuccess && r >= 2 && ms > 0.f) { const double g = (double)(n16 * 16) / (ms * 1e-3) / 1e9; if (g > best) best = g; }
+        if (err == cudaSuccess && r >= 2 && ms > 0.f) { const double g = (double)passes * (double)(n16 * 16) / (ms * 1e-3) / 1e9; if (g > best) best = g; }
     }
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
