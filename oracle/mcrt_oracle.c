@@ -157,6 +157,14 @@ typedef struct {
     double *cdfB;          /* [ns][nT][nf], Eq. 5 */
     double *cdfdB;         /* [ns][nT][nf], Eq. 10 */
     double *srccdf;        /* [nf] */
+    /* NEXT-3 dust mixtures (orc_set_mixtures): with n_mix > 0 the species byte of a cell names a MIXTURE of one or
+     * two of the ns materials, and kext_h / kabs_h / albedo above have n_mix rows (ntab = rows of those tables) */
+    int ntab, n_mix;
+    int32_t *mx_ncomp;     /* [n_mix] 1 or 2 components */
+    int32_t *mx_mat;       /* [n_mix][2] material of each component */
+    double *mx_frac;       /* [n_mix][2] mass fraction of each component */
+    double *mx_S0, *mx_A0; /* [n_mix][nf] event thresholds (see orc_set_mixtures) */
+    double *mx_kabs1_h;    /* [n_mix][nf] f_1 kabs_1 h of the second component (0 without one) */
 } orc_ctx;
 
 orc_ctx *orc_create(int nx, int ny, int nz, double h, const float *rho, const uint8_t *sp, int ns,
@@ -167,6 +175,7 @@ orc_ctx *orc_create(int nx, int ny, int nz, double h, const float *rho, const ui
     orc_ctx *C = (orc_ctx *)calloc(1, sizeof(orc_ctx));
     size_t nc = (size_t)nx * ny * nz;
     C->nx = nx; C->ny = ny; C->nz = nz; C->ns = ns; C->nf = nf; C->nT = nT; C->ndir = ndir; C->h = h; C->L = L;
+    C->ntab = ns;
     C->rho = (float *)malloc(nc * sizeof(float));       memcpy(C->rho, rho, nc * sizeof(float));
     C->sp = (uint8_t *)malloc(nc);                      memcpy(C->sp, sp, nc);
     C->nu = (double *)malloc(nf * sizeof(double));      memcpy(C->nu, nu, nf * sizeof(double));
@@ -217,8 +226,84 @@ void orc_destroy(orc_ctx *C)
     if (!C) return;
     free(C->rho); free(C->sp); free(C->nu); free(C->dnu); free(C->kabs); free(C->ksca); free(C->g);
     free(C->Tg); free(C->mu_edges); free(C->kext_h); free(C->kabs_h); free(C->albedo); free(C->J);
-    free(C->cdfB); free(C->cdfdB); free(C->srccdf); free(C);
+    free(C->cdfB); free(C->cdfdB); free(C->srccdf);
+    free(C->mx_ncomp); free(C->mx_mat); free(C->mx_frac); free(C->mx_S0); free(C->mx_A0); free(C->mx_kabs1_h);
+    free(C);
 }
+
+/* NEXT-3: per-cell dust mixtures with per-material temperatures.  PAPER.md:17 "equilibrium
+ * temperatures of two populations of large grains", "different grain materials", "the total
+ * number of absorbed photon packets per particle and cell is used to calculate the temperature of each material".
+ * The paper gives no formulas for the mixture; readings Q34-Q36:
+ *   Q34  a cell of mixture x holds its components c = 0, 1 (materials m_c) with mass fractions f_c of the cell's
+ *        density; extinction adds up:  kext_x = (f_0 kabs_0 + f_0 ksca_0) + (f_1 kabs_1 + f_1 ksca_1)   (Eq. 2)
+ *   Q35  the ONE uniform number that decides scattering against absorption also decides which
+ *        component interacts, each in proportion to its share of kext_x:
+ *          z < S0           scattered by component 0   (its g in the HG function)   S0 = f_0 ksca_0 / kext_x
+ *          z < albedo       scattered by component 1                                albedo = (f_0 ksca_0 + f_1 ksca_1) / kext_x
+ *          z < A0           absorbed by component 0                                 A0 = ((f_0 ksca_0 + f_1 ksca_1) + f_0 kabs_0) / kext_x
+ *          else             absorbed by component 1
+ *   Q36  every component has its own absorption count, Lucy tally (f_c kabs_c rho ds per traversal) and
+ *        temperature: Eq. 4 with the component's material and its mass rho_i f_c V_i; an absorbed packet is
+ *        re-emitted from the absorbing component's Eq. 10 / Eq. 5 row at that component's temperature.
+ * Returns 0, -1 on bad arguments.  Call before orc_state_create. */
+int orc_set_mixtures(orc_ctx *C, int n_mix, const int32_t *ncomp, const int32_t *mat, const double *frac)
+{
+    if (n_mix < 1 || n_mix > 255) return -1;
+    for (int x = 0; x < n_mix; ++x) {
+        if (ncomp[x] < 1 || ncomp[x] > 2) return -1;
+        double tot = 0.0;
+        for (int c = 0; c < ncomp[x]; ++c) {
+            if (mat[2 * x + c] < 0 || mat[2 * x + c] >= C->ns || !(frac[2 * x + c] > 0.0)) return -1;
+            tot += frac[2 * x + c];
+        }
+        if (fabs(tot - 1.0) > 1e-12) return -1;
+    }
+    const int nf = C->nf;
+    const size_t n = (size_t)n_mix * nf;
+    C->n_mix = n_mix; C->ntab = n_mix;
+    C->mx_ncomp = (int32_t *)malloc(n_mix * sizeof(int32_t));
+    C->mx_mat = (int32_t *)calloc(2 * (size_t)n_mix, sizeof(int32_t));
+    C->mx_frac = (double *)calloc(2 * (size_t)n_mix, sizeof(double));
+    C->mx_S0 = (double *)calloc(n, sizeof(double));
+    C->mx_A0 = (double *)calloc(n, sizeof(double));
+    C->mx_kabs1_h = (double *)calloc(n, sizeof(double));
+    free(C->kext_h); free(C->kabs_h); free(C->albedo);
+    C->kext_h = (double *)malloc(n * sizeof(double));
+    C->kabs_h = (double *)malloc(n * sizeof(double));
+    C->albedo = (double *)malloc(n * sizeof(double));
+    for (int x = 0; x < n_mix; ++x) {
+        C->mx_ncomp[x] = ncomp[x];
+        for (int c = 0; c < ncomp[x]; ++c) { C->mx_mat[2 * x + c] = mat[2 * x + c]; C->mx_frac[2 * x + c] = frac[2 * x + c]; }
+        for (int j = 0; j < nf; ++j) {
+            const size_t i = (size_t)x * nf + j;
+            const int m0 = mat[2 * x];
+            if (ncomp[x] == 1) {      /* the material itself: the same arithmetic as without mixtures */
+                double kext = C->kabs[m0 * nf + j] + C->ksca[m0 * nf + j];
+                C->kext_h[i] = kext * C->h;
+                C->kabs_h[i] = C->kabs[m0 * nf + j] * C->h;
+                C->albedo[i] = (kext > 0.0) ? C->ksca[m0 * nf + j] / kext : 0.0;
+                C->mx_S0[i] = C->albedo[i]; C->mx_A0[i] = 1.0;
+            } else {
+                const int m1 = mat[2 * x + 1];
+                double ka0 = frac[2 * x] * C->kabs[m0 * nf + j], ks0 = frac[2 * x] * C->ksca[m0 * nf + j];
+                double ka1 = frac[2 * x + 1] * C->kabs[m1 * nf + j], ks1 = frac[2 * x + 1] * C->ksca[m1 * nf + j];
+                double kext = (ka0 + ks0) + (ka1 + ks1);
+                C->kext_h[i] = kext * C->h;
+                C->kabs_h[i] = ka0 * C->h;
+                C->mx_kabs1_h[i] = ka1 * C->h;
+                C->mx_S0[i] = (kext > 0.0) ? ks0 / kext : 0.0;
+                C->albedo[i] = (kext > 0.0) ? (ks0 + ks1) / kext : 0.0;
+                C->mx_A0[i] = (kext > 0.0) ? ((ks0 + ks1) + ka0) / kext : 1.0;
+            }
+        }
+    }
+    return 0;
+}
+
+/* material and mass fraction of component c of the cell species x (without mixtures: the material x itself) */
+static inline int comp_mat(const orc_ctx *C, int x, int c) { return C->n_mix ? C->mx_mat[2 * x + c] : x; }
+static inline int comp_count(const orc_ctx *C, int x) { return C->n_mix ? C->mx_ncomp[x] : 1; }
 
 /* table accessors for the pins */
 void orc_get_tables(const orc_ctx *C, double *dnu, double *J, double *cdfB, double *cdfdB, double *albedo,
@@ -505,6 +590,10 @@ typedef struct {
     int64_t *Lfx;            /* Lucy path-length tally, fixed point (O9) */
     double *Lsum, *Lcmp;     /* compensated fp64 copy */
     uint16_t *tidx;          /* temperature index per cell (O11) */
+    uint64_t *k1;            /* the same three for the second component of a mixture (NEXT-3), or NULL */
+    int64_t *Lfx1;
+    uint16_t *tidx1;
+    double *kabs1_fx;
     uint64_t *sed, *sed_direct; /* [ndir][nf] */
     orc_digest *dig;         /* [n_packets] or NULL */
     double *kabs_fx;         /* kabs_h * 2^FX */
@@ -541,6 +630,10 @@ static inline void lucy_add(orc_run_t *R, size_t ci, int sj, double rho_c, doubl
         int64_t q = (int64_t)llrint(x);
         __atomic_fetch_add(&R->Lfx[ci], q, __ATOMIC_RELAXED);
         st->lucy_adds++;
+        if (R->Lfx1 && R->C->mx_ncomp[sj / R->C->nf] == 2) {   /* second component of a mixture (reading Q36) */
+            int64_t q1 = (int64_t)llrint(R->kabs1_fx[sj] * rho_c * ds);
+            __atomic_fetch_add(&R->Lfx1[ci], q1, __ATOMIC_RELAXED);
+        }
         if (R->Lsum) { /* Kahan */
             double y = R->C->kabs_h[sj] * rho_c * ds - R->Lcmp[ci];
             double tt = R->Lsum[ci] + y;
@@ -644,7 +737,9 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
         if (ztype < C->albedo[sj]) {
             orc_uniforms(R->seed, pid, d++, R->pass, z);
             double un[3];
-            orc_hg_scatter(C->g[sj], z[0], z[1], u, un);
+            /* (a mixture: the component that scatters, reading Q35) */
+            const int cs = (comp_count(C, s) == 2 && !(ztype < C->mx_S0[sj])) ? 1 : 0;
+            orc_hg_scatter(C->g[comp_mat(C, s, cs) * nf + j], z[0], z[1], u, un);
             if (R->sca_slot && R->sca_slot[j] >= 0) {   /* store the event: cell, frequency, incoming direction */
                 uint64_t at = __atomic_fetch_add(R->sca_n, (uint64_t)1, __ATOMIC_RELAXED);
                 if (at < R->sca_cap) {
@@ -660,16 +755,18 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
         } else {
             /* O8 absorption: count it, re-emit at once from the same position with a new
              * frequency and an isotropic direction (readings Q18, Q20) */
-            __atomic_fetch_add(&R->k[ci], (uint64_t)1, __ATOMIC_RELAXED);
+            /* (a mixture: the component that absorbs, reading Q35; its count, temperature and emission row, Q36) */
+            const int ca = (comp_count(C, s) == 2 && !(ztype < C->mx_A0[sj])) ? 1 : 0;
+            __atomic_fetch_add(ca ? &R->k1[ci] : &R->k[ci], (uint64_t)1, __ATOMIC_RELAXED);
             nabs++;
             st->absorptions++;
             if (R->o->absorb_and_stop) {
                 hash_mix(&hash, event_word(ORC_EV_ABSORB, j, ci));
                 goto done;
             }
-            int m = R->tidx[ci];
+            int m = ca ? R->tidx1[ci] : R->tidx[ci];
             orc_uniforms(R->seed, pid, d++, R->pass, z);
-            j = orc_lower_bound(R->cdf + ((size_t)s * C->nT + m) * nf, nf, z[0]); /* Eq. 10 / Eq. 5 */
+            j = orc_lower_bound(R->cdf + ((size_t)comp_mat(C, s, ca) * C->nT + m) * nf, nf, z[0]); /* Eq. 10 / Eq. 5 */
             orc_uniforms(R->seed, pid, d++, R->pass, z);
             orc_isotropic(z[0], z[1], u);
             hash_mix(&hash, event_word(ORC_EV_ABSORB, j, ci));
@@ -799,6 +896,9 @@ typedef struct {
     int64_t *Lfx;
     double *Lsum, *Lcmp;
     uint16_t *tidx;
+    uint64_t *k1, *kprev1;   /* second component of a mixture (NEXT-3); NULL without mixtures */
+    int64_t *Lfx1;
+    uint16_t *tidx1;
     uint64_t *sed, *sed_direct;
     int fx;
     double xi;               /* packet energy L/N of the run that produced the stored tallies */
@@ -818,6 +918,12 @@ orc_state *orc_state_create(const orc_ctx *C)
     S->kprev = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
     S->Lfx = (int64_t *)calloc(S->nc, sizeof(int64_t));
     S->tidx = (uint16_t *)calloc(S->nc, sizeof(uint16_t));
+    if (C->n_mix) {
+        S->k1 = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
+        S->kprev1 = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
+        S->Lfx1 = (int64_t *)calloc(S->nc, sizeof(int64_t));
+        S->tidx1 = (uint16_t *)calloc(S->nc, sizeof(uint16_t));
+    }
     S->sed = (uint64_t *)calloc((size_t)C->ndir * C->nf, sizeof(uint64_t));
     S->sed_direct = (uint64_t *)calloc((size_t)C->ndir * C->nf, sizeof(uint64_t));
     return S;
@@ -827,6 +933,7 @@ void orc_state_destroy(orc_state *S)
 {
     if (!S) return;
     free(S->k); free(S->kprev); free(S->Lfx); free(S->Lsum); free(S->Lcmp); free(S->tidx);
+    free(S->k1); free(S->kprev1); free(S->Lfx1); free(S->tidx1);
     free(S->sed); free(S->sed_direct); free(S->sca_slot); free(S->sca_ev); free(S);
 }
 
@@ -835,6 +942,11 @@ static void zero_tallies(orc_state *S)
     memset(S->k, 0, S->nc * sizeof(uint64_t));
     memset(S->kprev, 0, S->nc * sizeof(uint64_t));
     memset(S->Lfx, 0, S->nc * sizeof(int64_t));
+    if (S->k1) {
+        memset(S->k1, 0, S->nc * sizeof(uint64_t));
+        memset(S->kprev1, 0, S->nc * sizeof(uint64_t));
+        memset(S->Lfx1, 0, S->nc * sizeof(int64_t));
+    }
     if (S->Lsum) { memset(S->Lsum, 0, S->nc * sizeof(double)); memset(S->Lcmp, 0, S->nc * sizeof(double)); }
     memset(S->sed, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
     memset(S->sed_direct, 0, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
@@ -880,12 +992,30 @@ static void epoch_update(orc_state *S, int first_epoch, double ratio, double cel
                 double pred = 0.5 * (double)(kk - S->kprev[ci]) * ratio;
                 kt = (double)kk + ((pred > 1.0) ? pred : 1.0);
             }
-            double x = kt * cellfac / rho_c;
-            S->tidx[ci] = (uint16_t)t_index(C, C->sp[ci], x);
+            /* (a mixture: Eq. 4 with the component's own mass rho f_c V, reading Q36) */
+            double x = kt * cellfac / (C->n_mix ? rho_c * C->mx_frac[2 * C->sp[ci]] : rho_c);
+            S->tidx[ci] = (uint16_t)t_index(C, comp_mat(C, C->sp[ci], 0), x);
         } else {
             S->tidx[ci] = 0;
         }
         S->kprev[ci] = kk;
+        if (S->k1) {    /* the second component: the same rule on its own count */
+            const int xm = C->sp[ci];
+            uint64_t k1 = S->k1[ci];
+            if (rho_c > 0.0 && C->mx_ncomp[xm] == 2) {
+                double kt;
+                if (first_epoch) kt = (double)k1 + 1.0;
+                else {
+                    double pred = 0.5 * (double)(k1 - S->kprev1[ci]) * ratio;
+                    kt = (double)k1 + ((pred > 1.0) ? pred : 1.0);
+                }
+                double x = kt * cellfac / (rho_c * C->mx_frac[2 * xm + 1]);
+                S->tidx1[ci] = (uint16_t)t_index(C, C->mx_mat[2 * xm + 1], x);
+            } else {
+                S->tidx1[ci] = 0;
+            }
+            S->kprev1[ci] = k1;
+        }
     }
 }
 
@@ -898,10 +1028,20 @@ static void sweep_update(orc_state *S, int from_lucy, double cellfac, int fx_of_
         double rho_c = (double)C->rho[ci];
         if (rho_c > 0.0) {
             double e = from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
-            double x = e * cellfac / rho_c;
-            S->tidx[ci] = (uint16_t)t_index(C, C->sp[ci], x);
+            double x = e * cellfac / (C->n_mix ? rho_c * C->mx_frac[2 * C->sp[ci]] : rho_c);
+            S->tidx[ci] = (uint16_t)t_index(C, comp_mat(C, C->sp[ci], 0), x);
         } else {
             S->tidx[ci] = 0;
+        }
+        if (S->k1) {
+            const int xm = C->sp[ci];
+            if (rho_c > 0.0 && C->mx_ncomp[xm] == 2) {
+                double e = from_lucy ? (double)S->Lfx1[ci] * inv_fx : (double)S->k1[ci];
+                double x = e * cellfac / (rho_c * C->mx_frac[2 * xm + 1]);
+                S->tidx1[ci] = (uint16_t)t_index(C, C->mx_mat[2 * xm + 1], x);
+            } else {
+                S->tidx1[ci] = 0;
+            }
         }
     }
 }
@@ -933,14 +1073,19 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
     double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h); /* xi / (4 pi V), Eq. 4 */
     /* Eq. 4 for the first sweep: k and L were counted in packets of the PREVIOUS run's energy */
     double prev_cellfac = prev_xi / (ORC_FOUR_PI * C->h * C->h * C->h);
-    size_t nsf = (size_t)C->ns * C->nf;
+    size_t nsf = (size_t)C->ntab * C->nf;
     R.C = C; R.k = S->k; R.kprev = S->kprev; R.Lfx = S->Lfx; R.tidx = S->tidx;
+    R.k1 = S->k1; R.Lfx1 = S->Lfx1; R.tidx1 = S->tidx1;
     R.Lsum = o->keep_fp64_lucy ? S->Lsum : NULL; R.Lcmp = S->Lcmp;
     R.sed = S->sed; R.sed_direct = S->sed_direct; R.dig = digests; R.seed = seed; R.fx = S->fx; R.o = o;
     R.pid0_digest = o->pid0;
     R.sca_slot = S->sca_slot; R.sca_ev = S->sca_ev; R.sca_cap = S->sca_cap; R.sca_n = &S->sca_n;
     R.kabs_fx = (double *)malloc(nsf * sizeof(double));
     for (size_t i = 0; i < nsf; ++i) R.kabs_fx[i] = ldexp(C->kabs_h[i], S->fx);
+    if (C->n_mix) {
+        R.kabs1_fx = (double *)malloc(nsf * sizeof(double));
+        for (size_t i = 0; i < nsf; ++i) R.kabs1_fx[i] = ldexp(C->mx_kabs1_h[i], S->fx);
+    }
     st.fx_bits = S->fx;
 
     if (o->mode == ORC_MODE_BW_EPOCH) {
@@ -1000,10 +1145,14 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
             st.epochs++;
         }
     }
-    free(R.kabs_fx);
+    free(R.kabs_fx); free(R.kabs1_fx);
     for (size_t ci = 0; ci < S->nc; ++ci) {
         int64_t v = S->Lfx[ci];
         if (v > ((int64_t)1 << 62) || v < -((int64_t)1 << 62)) st.overflow = 1;
+        if (S->Lfx1) {
+            v = S->Lfx1[ci];
+            if (v > ((int64_t)1 << 62) || v < -((int64_t)1 << 62)) st.overflow = 1;
+        }
     }
     if (stats) *stats = st;
     return st.overflow ? -5 : 0;
@@ -1019,6 +1168,16 @@ void orc_read_raw(const orc_state *S, uint64_t *k, int64_t *Lfx, uint64_t *sed, 
     if (sed_direct) memcpy(sed_direct, S->sed_direct, (size_t)S->C->ndir * S->C->nf * sizeof(uint64_t));
     if (tidx) memcpy(tidx, S->tidx, S->nc * sizeof(uint16_t));
     if (Lsum && S->Lsum) memcpy(Lsum, S->Lsum, S->nc * sizeof(double));
+}
+
+/* raw tallies of the second component of a mixture (NEXT-3) */
+int orc_read_raw_comp1(const orc_state *S, uint64_t *k, int64_t *Lfx, uint16_t *tidx)
+{
+    if (!S->k1) return -1;
+    if (k) memcpy(k, S->k1, S->nc * sizeof(uint64_t));
+    if (Lfx) memcpy(Lfx, S->Lfx1, S->nc * sizeof(int64_t));
+    if (tidx) memcpy(tidx, S->tidx1, S->nc * sizeof(uint16_t));
+    return 0;
 }
 
 /* invert J[s](T) = x by log-log interpolation (O12; Eq. 4; clamp per reading Q16) */
@@ -1053,7 +1212,8 @@ void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int
             double rho_c = (double)C->rho[ci];
             if (rho_c > 0.0) {
                 double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
-                T[ci] = (float)orc_T_of_x(C, C->sp[ci], e * cellfac / rho_c);
+                double mass = C->n_mix ? rho_c * C->mx_frac[2 * C->sp[ci]] : rho_c;
+                T[ci] = (float)orc_T_of_x(C, comp_mat(C, C->sp[ci], 0), e * cellfac / mass);
             } else T[ci] = 0.0f;
         }
     }
@@ -1063,6 +1223,29 @@ void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int
                 double dom = ORC_FOUR_PI * (C->mu_edges[b + 1] - C->mu_edges[b]);
                 SED[(size_t)b * C->nf + j] = (double)S->sed[(size_t)b * C->nf + j] * S->xi / (C->dnu[j] * dom);
             }
+}
+
+/* the same outputs for the second component of a mixture (NEXT-3, reading Q36): energy absorbed by that component and
+ * its temperature (0 in cells whose mixture has one component) */
+int orc_read_comp1(const orc_state *S, double *E_count, double *E_lucy, float *T, int T_from_lucy)
+{
+    const orc_ctx *C = S->C;
+    if (!S->k1) return -1;
+    double inv_fx = ldexp(1.0, -S->fx);
+    double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h);
+    for (size_t ci = 0; ci < S->nc; ++ci) {
+        if (E_count) E_count[ci] = (double)S->k1[ci] * S->xi;
+        if (E_lucy) E_lucy[ci] = (double)S->Lfx1[ci] * inv_fx * S->xi;
+        if (T) {
+            double rho_c = (double)C->rho[ci];
+            const int xm = C->sp[ci];
+            if (rho_c > 0.0 && C->mx_ncomp[xm] == 2) {
+                double e = T_from_lucy ? (double)S->Lfx1[ci] * inv_fx : (double)S->k1[ci];
+                T[ci] = (float)orc_T_of_x(C, C->mx_mat[2 * xm + 1], e * cellfac / (rho_c * C->mx_frac[2 * xm + 1]));
+            } else T[ci] = 0.0f;
+        }
+    }
+    return 0;
 }
 
 /* ------------------------------------------------------------------------------------------------
@@ -1115,6 +1298,7 @@ int orc_ray_trace(const orc_state *S, const double ez_in[3], const double ex_in[
 {
     const orc_ctx *C = S->C;
     if (j < 0 || j >= C->nf || nx < 1 || ny < 1 || !(pix > 0.0) || !(D > 0.0)) return -1;
+    if (C->n_mix) return -1;    /* images of mixtures are not defined here */
     const int n[3] = { C->nx, C->ny, C->nz };
     double ez[3], ex[3], ey[3];
     double nz_ = sqrt(ez_in[0] * ez_in[0] + ez_in[1] * ez_in[1] + ez_in[2] * ez_in[2]);

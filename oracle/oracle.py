@@ -64,6 +64,12 @@ def lib():
         L.orc_read_raw.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.orc_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_get_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        L.orc_set_mixtures.restype = C.c_int
+        L.orc_set_mixtures.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_read_raw_comp1.restype = C.c_int
+        L.orc_read_raw_comp1.argtypes = [C.c_void_p] + [C.c_void_p] * 3
+        L.orc_read_comp1.restype = C.c_int
+        L.orc_read_comp1.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int]
         L.orc_philox4x32_10.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_void_p]
         L.orc_planck.restype = C.c_double
@@ -192,7 +198,7 @@ class Oracle:
     """One problem (grid + dust + source + escape bins) and its tally state."""
 
     def __init__(self, nx, ny, nz, h, rho, species, n_species, nu, kabs, ksca, g, Tgrid, L, Tstar, Lnu_w,
-                 pos_cm, mu_edges):
+                 pos_cm, mu_edges, mixtures=None):
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.nc = self.nx * self.ny * self.nz
         self.ns, self.nf, self.nT = int(n_species), len(nu), len(Tgrid)
@@ -208,6 +214,14 @@ class Oracle:
         self._ctx = lib().orc_create(self.nx, self.ny, self.nz, float(h), _p(k[0]), _p(k[1]), self.ns, self.nf,
                                      _p(k[2]), _p(k[3]), _p(k[4]), _p(k[5]), self.nT, _p(k[6]), float(L),
                                      float(Tstar), _p(k[7]), _p(k[8]), self.ndir, _p(k[9]))
+        self.mixtures = mixtures
+        if mixtures is not None:
+            # NEXT-3: the species byte of a cell names a mixture: (ncomp[n_mix], material[n_mix][2], fraction[n_mix][2])
+            nc_, mat_, fr_ = (np.ascontiguousarray(mixtures[0], np.int32), np.ascontiguousarray(mixtures[1], np.int32),
+                              np.ascontiguousarray(mixtures[2], np.float64))
+            assert mat_.shape == (len(nc_), 2) and fr_.shape == (len(nc_), 2)
+            rc = lib().orc_set_mixtures(self._ctx, len(nc_), _p(nc_), _p(mat_), _p(fr_))
+            assert rc == 0, "bad mixture table"
         self._state = lib().orc_state_create(self._ctx)
         self.last_n = 0
 
@@ -215,7 +229,7 @@ class Oracle:
     def from_workload(cls, w):
         return cls(w.nx, w.ny, w.nz, w.cell_size_cm, w.rho, w.species, w.n_species, w.nu_hz, w.kappa_abs,
                    w.kappa_sca, w.g, w.T_grid, w.L_erg_s, w.T_star_K, w.L_nu_weights, w.source_pos_cm,
-                   w.abs_mu_edges)
+                   w.abs_mu_edges, mixtures=getattr(w, "mixtures", None))
 
     def close(self):
         if self._state:
@@ -271,6 +285,21 @@ class Oracle:
         if fp64_lucy:
             out["lucy_fp64"] = Ls
         return out
+
+    def read_raw_comp1(self):
+        """Raw tallies of the second component of the mixtures (NEXT-3)."""
+        k = np.zeros(self.nc, np.uint64)
+        L = np.zeros(self.nc, np.int64)
+        tidx = np.zeros(self.nc, np.uint16)
+        assert lib().orc_read_raw_comp1(self._state, _p(k), _p(L), _p(tidx)) == 0
+        return {"k": k, "lucy_fx": L, "tidx": tidx}
+
+    def read_comp1(self, T_from_lucy=False):
+        Ec = np.zeros(self.nc)
+        El = np.zeros(self.nc)
+        T = np.zeros(self.nc, np.float32)
+        assert lib().orc_read_comp1(self._state, _p(Ec), _p(El), _p(T), int(T_from_lucy)) == 0
+        return {"E_count": Ec, "E_lucy": El, "T": T}
 
     def scatter_store(self, nu_bins, capacity):
         b = np.ascontiguousarray(nu_bins, np.int32)

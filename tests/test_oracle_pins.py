@@ -891,3 +891,177 @@ def test_p21_stratified_source_frequencies(orc):
     cnt1 = o.read_raw()["sed"].sum(axis=0).astype(np.int64)
     big = N * p > 2000
     assert np.all(np.abs(cnt1 - N * p)[big] < 0.35 * np.sqrt(N * p)[big] + 15)
+
+
+# ------------------------------------------------------------------------------------------ P22 dust mixtures (NEXT-3)
+def test_p22_one_component_mixtures_and_identical_halves(orc):
+    """Readings Q34-Q36: (i) a mixture table that names every material as its own one-component mixture is the run
+    without mixtures, bit for bit (digests, tallies); (ii) two halves (f = 1/2 each: scaling by 1/2 is exact) of the
+    SAME material give the same trajectories as that material alone when absorbed packets end, the absorptions are
+    split between the halves cell by cell (k0 + k1 = k), binomially, and each half's Lucy tally is half the
+    material's up to the rounding of the fixed-point adds."""
+    w = W.uniform_cube(12, tau_edge_V=3.0, albedo=0.6, g_const=0.5, n_nu=12, slope=1.0)
+    N = 40_000
+    a = orc.Oracle.from_workload(w)
+    ra = a.run(N, seed=221, digests=True, n_threads=NTH)
+    w.mixtures = ([1], [[0, 0]], [[1.0, 0.0]])
+    b = orc.Oracle.from_workload(w)
+    rb = b.run(N, seed=221, digests=True, n_threads=NTH)
+    assert np.array_equal(ra["digests"], rb["digests"])
+    A, B = a.read_raw(), b.read_raw()
+    for key in ("k", "lucy_fx", "sed", "tidx"):
+        assert np.array_equal(A[key], B[key]), key
+    assert not b.read_raw_comp1()["k"].any()
+    # (ii)
+    a2 = orc.Oracle.from_workload(W.uniform_cube(12, tau_edge_V=3.0, albedo=0.6, g_const=0.5, n_nu=12, slope=1.0))
+    r1 = a2.run(N, seed=222, digests=True, absorb_and_stop=True, n_threads=NTH)
+    w.mixtures = ([2], [[0, 0]], [[0.5, 0.5]])
+    c = orc.Oracle.from_workload(w)
+    r2 = c.run(N, seed=222, digests=True, absorb_and_stop=True, n_threads=NTH)
+    assert np.array_equal(r1["digests"], r2["digests"])
+    k = a2.read_raw()["k"].astype(np.int64)
+    k0, k1 = c.read_raw()["k"].astype(np.int64), c.read_raw_comp1()["k"].astype(np.int64)
+    assert np.array_equal(k0 + k1, k)
+    K = int(k.sum())
+    assert abs(int(k1.sum()) - K / 2) < 4 * math.sqrt(K / 4) and k1.sum() > 0
+    L, L0, L1 = a2.read_raw()["lucy_fx"], c.read_raw()["lucy_fx"], c.read_raw_comp1()["lucy_fx"]
+    assert np.array_equal(L0, L1)
+    assert np.abs(2 * L0 - L).max() <= r1["lucy_adds"] and L.max() > 1e6   # at most one unit per add
+
+
+def test_p22_thin_mixture_component_temperatures(orc):
+    """Reading Q36 against radiative balance: in an optically thin sphere around a blackbody source two power-law
+    materials (kappa ~ nu^beta_c) mixed 30 % / 70 % by mass each reach THEIR OWN temperature
+    T_c = T* (R*/2r)^(2/(4+beta_c)), whatever the other one does; and each component's Lucy tally per unit of its own
+    mass, times 16 pi^2 r^2 / L, is the source-weighted mean of its own kappa.  Fails when a component is tallied
+    with the other's opacity, when Eq. 4 uses the cell's whole mass, or when the fractions are swapped."""
+    betas, fr, Tstar, n, N = (1.0, 2.0), (0.3, 0.7), 1500.0, 24, 600_000
+    lam = W.wavelength_grid_um(160, 0.2, 1e5)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = np.stack([100.0 * (nu / nu[-1]) ** b for b in betas])
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    rho0 = 1e-3 / (kabs.max() * n / 2 * h)
+    rho = np.where(r < n / 2, rho0, 0.0).astype(np.float32)
+    L = W.LSUN_ERG_S
+    c = n / 2 * h
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 2, nu, kabs, np.zeros((2, len(nu))),
+                   np.zeros((2, len(nu))), W.temperature_grid(1000, 2.0, 2000.0), L, Tstar, None, [c, c, c],
+                   [0.0, 1.0], mixtures=([2], [[0, 1]], [list(fr)]))
+    res = o.run(N, seed=8, n_threads=NTH)
+    assert res["absorptions"] < 0.01 * N
+    T = [o.read(T_from_lucy=True)["T"].reshape(n, n, n).astype(np.float64),
+         o.read_comp1(T_from_lucy=True)["T"].reshape(n, n, n).astype(np.float64)]
+    E = [o.read()["E_lucy"].reshape(n, n, n), o.read_comp1()["E_lucy"].reshape(n, n, n)]
+    Rstar = math.sqrt(L / (4 * math.pi * SIGMA_SB * Tstar ** 4))
+    pj = np.diff(np.concatenate([[0.0], o.tables()["srccdf"]]))
+    for comp in (0, 1):
+        for r_lo in (4.0, 7.0, 10.0):
+            sel = (r >= r_lo) & (r < r_lo + 1.0)
+            T_exp = Tstar * (Rstar / (2 * r[sel] * h)) ** (2 / (4 + betas[comp]))
+            assert abs((T[comp][sel] / T_exp).mean() - 1) < 0.01, (comp, r_lo)
+        sel = (r >= 5.0) & (r < 9.0)
+        xcell = E[comp][sel] / (4 * math.pi * rho0 * fr[comp] * h ** 3)
+        got = (xcell * (r[sel] * h) ** 2).mean() * 16 * math.pi ** 2 / L
+        assert abs(got / (kabs[comp] * pj).sum() - 1) < 0.01, comp
+    sel = (r >= 4.0) & (r < 5.0)
+    assert T[1][sel].mean() / T[0][sel].mean() > 1.2      # the two laws are far apart: (R*/2r)^(2/6 - 2/5), R* << r
+
+
+def test_p22_mixture_random_flight_and_absorption_split(orc):
+    """Reading Q35 against the random-flight closed form of P18: in an infinite uniform grey medium made of a forward
+    scattering material (g = 0.8) and an isotropic one (g = 0), with different albedos and mixed 40 % / 60 %, the
+    packets end at <R^2> = 2 l^2 / [(1 - a)(1 - a g)] with l = 1/(kext_x rho), a the mixture's albedo and g the
+    mean cosine over all scatterings, g = (f0 ks0 g0 + f1 ks1 g1) / (f0 ks0 + f1 ks1); the absorptions go to the
+    components in the ratio f0 ka0 : f1 ka1.  Fails when the scattering component's g is taken from the other
+    material, when the thresholds are in the wrong order, or when the fractions do not enter kext."""
+    n, N = 160, 200_000
+    f = (0.4, 0.6)
+    ka, ks, gg = (30.0, 90.0), (210.0, 60.0), (0.8, 0.0)
+    nf = 4
+    lam = W.wavelength_grid_um(nf, 0.1, 1000.0)
+    nu = W.nu_from_lambda_um(lam)
+    kext = f[0] * (ka[0] + ks[0]) + f[1] * (ka[1] + ks[1])
+    h = W.AU_CM
+    ell = 2.0                                             # mean free path in cells
+    rho0 = 1.0 / (kext * ell * h)
+    rho = np.full((n, n, n), rho0, np.float32)
+    kabs = np.stack([np.full(nf, ka[0]), np.full(nf, ka[1])])
+    ksca = np.stack([np.full(nf, ks[0]), np.full(nf, ks[1])])
+    g = np.stack([np.full(nf, gg[0]), np.full(nf, gg[1])])
+    c = n / 2 * h
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 2, nu, kabs, ksca, g, W.temperature_grid(),
+                   W.LSUN_ERG_S, 5800.0, None, [c, c, c], [0.0, 1.0], mixtures=([2], [[0, 1]], [list(f)]))
+    r = o.run(N, seed=2203, absorb_and_stop=True, B0=N, Bmax=N, n_threads=NTH)
+    assert r["escapes"] <= 2e-4 * N and r["absorptions"] + r["escapes"] == N
+    ell = 1.0 / (kext * float(rho.flat[0]) * h)
+    a = (f[0] * ks[0] + f[1] * ks[1]) / kext
+    gbar = (f[0] * ks[0] * gg[0] + f[1] * ks[1] * gg[1]) / (f[0] * ks[0] + f[1] * ks[1])
+    assert abs(r["scatterings"] / (r["scatterings"] + r["absorptions"]) - a) < 4 * math.sqrt(a * (1 - a) / r["flights"])
+    k0 = o.read_raw()["k"].reshape(n, n, n).astype(np.float64)
+    k1 = o.read_raw_comp1()["k"].reshape(n, n, n).astype(np.float64)
+    K = k0.sum() + k1.sum()
+    p1 = f[1] * ka[1] / (f[0] * ka[0] + f[1] * ka[1])
+    assert abs(k1.sum() / K - p1) < 4 * math.sqrt(p1 * (1 - p1) / K)
+    k = k0 + k1
+    d = (np.arange(n) + 0.5) - n / 2
+    X, Y, Z = np.meshgrid(d, d, d, indexing="ij")
+    rr2 = Z ** 2 + Y ** 2 + X ** 2
+    tot = (k * rr2).sum() / K
+    sig = math.sqrt(((k * rr2 ** 2).sum() / K - tot ** 2) / K)
+    r2_true = 2 * ell ** 2 / ((1 - a) * (1 - a * gbar))
+    assert abs(tot - (r2_true + 0.25)) < 4 * sig, (tot, r2_true + 0.25, sig)
+    r2_swapped = 2 * ell ** 2 / ((1 - a) * (1 - a * (f[0] * ks[0] * gg[1] + f[1] * ks[1] * gg[0]) / (f[0] * ks[0] + f[1] * ks[1])))
+    assert abs(r2_swapped - r2_true) > 20 * sig           # the pin can tell the two assignments apart
+
+
+def test_p22_mixture_component_order_is_a_relabelling(orc):
+    """Readings Q35/Q36, the second component's share of the path (its frozen temperature index and the row it
+    re-emits from): listing a mixture's components in the other order changes nothing physical.  A moderately thick
+    sphere (tau ~ 4 at the source's peak) of a grey material and a kappa ~ nu^2 material, 30 % / 70 %: the escaping
+    spectrum and both materials' radial temperature profiles of the run with the order (grey, nu^2) agree with those
+    of the run with the order (nu^2, grey) within the counting noise.  Together with the pins of the one-material
+    path (which component 0 is, bit for bit: P22 (i)) this pins component 1: a wrong mass in its Eq. 4 or a row of
+    the other material moves its re-emission by 25 % in frequency."""
+    n, N, Tstar = 16, 300_000, 2500.0
+    lam = W.wavelength_grid_um(60, 0.1, 3000.0)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = np.stack([np.full(len(nu), 40.0), 400.0 * (nu / nu[-1]) ** 2])
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    nu_peak = 2.82 * K_BOLTZ * Tstar / H_PLANCK
+    k_peak = 0.3 * 40.0 + 0.7 * 400.0 * (nu_peak / nu[-1]) ** 2
+    rho0 = 4.0 / (k_peak * n / 2 * h)
+    rho = np.where(r < n / 2, rho0, 0.0).astype(np.float32)
+    c = n / 2 * h
+    zeros = np.zeros((2, len(nu)))
+    runs = []
+    for order, seed in (((0, 1), 2210), ((1, 0), 2211)):
+        fr = [(0.3, 0.7)[m] for m in order]
+        o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 2, nu, kabs, zeros, zeros,
+                       W.temperature_grid(1000, 2.0, 3000.0), W.LSUN_ERG_S, Tstar, None, [c, c, c], [0.0, 1.0],
+                       mixtures=([2], [list(order)], [fr]))
+        res = o.run(N, seed=seed, n_threads=NTH)
+        assert res["absorptions"] > 2 * N
+        sed = o.read_raw()["sed"][0].astype(np.float64)
+        T = [o.read(T_from_lucy=True)["T"].reshape(n, n, n).astype(np.float64),
+             o.read_comp1(T_from_lucy=True)["T"].reshape(n, n, n).astype(np.float64)]
+        Tm = {order[0]: T[0], order[1]: T[1]}               # by MATERIAL
+        # ... and a frozen-temperature sweep (S12) at the Lucy temperatures of that run: its escaping spectrum
+        o.run(N, seed=seed + 10, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, sweep_T_from_lucy=1, reset=False, n_threads=NTH)
+        sed_sweep = o.read_raw()["sed"][0].astype(np.float64)
+        runs.append((sed, Tm, sed_sweep))
+    (sA, TA, wA), (sB, TB, wB) = runs
+    for a_, b_ in ((sA, sB), (wA, wB)):
+        sel = (a_ + b_) >= 50
+        chi2 = ((a_[sel] - b_[sel]) ** 2 / (a_[sel] + b_[sel])).sum()
+        ndf = int(sel.sum())
+        assert ndf >= 25 and chi2 < ndf + 5 * math.sqrt(2 * ndf), (chi2, ndf)
+    for m in (0, 1):
+        for r_lo in (2.0, 4.0, 6.0):
+            s = (r >= r_lo) & (r < r_lo + 1.0)
+            assert abs(TA[m][s].mean() / TB[m][s].mean() - 1) < 0.01, (m, r_lo, TA[m][s].mean(), TB[m][s].mean())
+    s = (r >= 4.0) & (r < 5.0)
+    assert TA[1][s].mean() / TA[0][s].mean() > 1.1        # the two materials' temperatures differ: the pin has teeth
