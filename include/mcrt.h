@@ -151,6 +151,24 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
 int mcrt_dust_tables(mcrt_ctx *ctx, int n_nu, const double *nu_hz, const double *kappa_abs,
                      const double *kappa_sca, const double *g, int n_T, const double *T_grid);
 
+/* Dust mixtures with per-material temperatures ("two populations of large grains",
+ * PAPER.md:43 "different grain materials", "the total number of absorbed photon packets per particle and
+ * cell is used to calculate the temperature of each material").  After mcrt_dust_tables, before the first run, once
+ * per context: redefines cell species x (the byte of the grid's species array, x < n_species) as a MIXTURE of
+ * n_components[x] = 1 or 2 of the n_species materials of mcrt_dust_tables: component c of x is material
+ * material[2x+c] with mass fraction fraction[2x+c] > 0 of the cell's density (the fractions of x add up to 1).
+ * Host pointers, [n_species], [n_species][2], [n_species][2].  The paper has no formulas for this; the readings
+ * (Q34-Q36): extinction adds up, kext_x = (f0 kabs0 + f0 ksca0) + (f1 kabs1 + f1 ksca1); the ONE uniform
+ * number z that decides scattering against absorption also picks the component, in proportion to its
+ * share of kext_x -- z < f0 ksca0/kext_x: scattered by component 0 (its g), z < albedo_x: by component 1,
+ * z < albedo_x + f0 kabs0/kext_x: absorbed by component 0, else by component 1; every component keeps its own
+ * absorption count, Lucy tally (f_c kabs_c rho ds per traversal) and temperature (Eq. 4 with its material and its
+ * mass rho f_c V), and re-emits what it absorbed from its own Eq. 10 / Eq. 5 row.  mcrt_read / mcrt_read_raw return
+ * component 0, mcrt_read_component either.  A one-component mixture is that material, bit for bit.
+ * Not available with MCRT_MODE_LIVE_BW, in partitioned runs and for mcrt_ray_trace (MCRT_EINVAL); such runs use
+ * the kernel instantiation of the rarely used features and no per-CTA hot-cell copies. */
+int mcrt_dust_mixtures(mcrt_ctx *ctx, const int32_t *n_components, const int32_t *material, const double *fraction);
+
 /* Point source: luminosity L_erg_s split into equal-energy packets xi = L/N.
  *  T_star_K > 0: blackbody spectrum; otherwise L_nu_weights [n_nu] gives the spectral shape L_nu at the
  *  grid frequencies (any normalisation, >= 0, not all zero).  pos_cm strictly inside the grid. */
@@ -240,6 +258,12 @@ int mcrt_read(mcrt_ctx *ctx, double *E_abs_count, double *E_abs_lucy, float *T_c
 /* Raw integer tallies (parity tests), [where]: k_abs uint64 [cells]; lucy_fx int64 [cells];
  * sed_counts, sed_direct uint64 [n_dir][n_nu]; tidx uint16 [cells] (temperature index of the last
  * epoch); digests [n_packets of the last run] (only if recorded). */
+/* Outputs of one component of the mixtures (mcrt_dust_mixtures; component 0 or 1): the arrays of mcrt_read and the
+ * raw tallies of mcrt_read_raw for that component, [cells] each, any pointer may be NULL.  T is 0 where the cell's
+ * mixture has no such component.  MCRT_ESTATE without mixtures. */
+int mcrt_read_component(mcrt_ctx *ctx, int component, double *E_abs_count, double *E_abs_lucy, float *T_count,
+                        float *T_lucy, uint64_t *k_abs, int64_t *lucy_fx, uint16_t *tidx, mcrt_mem where);
+
 int mcrt_read_raw(mcrt_ctx *ctx, uint64_t *k_abs, int64_t *lucy_fx, uint64_t *sed_counts,
                   uint64_t *sed_direct, uint16_t *tidx, mcrt_digest *digests, mcrt_mem where);
 

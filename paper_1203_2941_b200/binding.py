@@ -21,10 +21,10 @@ MCRT_OK, MCRT_EINVAL, MCRT_ESTATE, MCRT_ENOMEM, MCRT_ECUDA, MCRT_EOVERFLOW = 0, 
 MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP, MCRT_MODE_LIVE_BW = 0, 1, 2
 
 EXPORTS = [
-    "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_source", "mcrt_escape_bins",
+    "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_dust_mixtures", "mcrt_source", "mcrt_escape_bins",
     "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
     "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_epoch_schedule", "mcrt_part_slice",
-    "mcrt_measure_read_bandwidth", "mcrt_scatter_store", "mcrt_scatter_events", "mcrt_ray_trace", "mcrt_get_stats", "mcrt_read", "mcrt_read_raw", "mcrt_read_tables",
+    "mcrt_measure_read_bandwidth", "mcrt_scatter_store", "mcrt_scatter_events", "mcrt_ray_trace", "mcrt_get_stats", "mcrt_read", "mcrt_read_component", "mcrt_read_raw", "mcrt_read_tables",
     "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
@@ -109,6 +109,8 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_get_stats.argtypes = [vp, C.POINTER(RunStats)]
     L.mcrt_read.argtypes = [vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
+    L.mcrt_read_component.argtypes = [vp, i, vp, vp, vp, vp, vp, vp, vp, i]
+    L.mcrt_dust_mixtures.argtypes = [vp, vp, vp, vp]
     L.mcrt_read_tables.argtypes = [vp] + [vp] * 6
     L.mcrt_philox_device.argtypes = [vp, vp, vp, u64]
     L.mcrt_traj_math_device.argtypes = [vp, vp, vp, vp, u64]
@@ -294,6 +296,20 @@ def mcrt_read(ctx, E_abs_count=None, E_abs_lucy=None, T_count=None, T_lucy=None,
                                     where), ctx)
 
 
+def mcrt_dust_mixtures(ctx, n_components, material, fraction):
+    nc_ = np.ascontiguousarray(n_components, np.int32)
+    mat = np.ascontiguousarray(material, np.int32)
+    fr = np.ascontiguousarray(fraction, np.float64)
+    assert mat.shape == (len(nc_), 2) and fr.shape == (len(nc_), 2)
+    _check(load_library().mcrt_dust_mixtures(ctx, _ptr(nc_), _ptr(mat), _ptr(fr)), ctx)
+
+
+def mcrt_read_component(ctx, component, E_abs_count=None, E_abs_lucy=None, T_count=None, T_lucy=None, k_abs=None,
+                        lucy_fx=None, tidx=None, where=MCRT_HOST):
+    _check(load_library().mcrt_read_component(ctx, int(component), _ptr(E_abs_count), _ptr(E_abs_lucy), _ptr(T_count),
+                                              _ptr(T_lucy), _ptr(k_abs), _ptr(lucy_fx), _ptr(tidx), where), ctx)
+
+
 def mcrt_read_raw(ctx, k_abs=None, lucy_fx=None, sed_counts=None, sed_direct=None, tidx=None, digests=None,
                   where=MCRT_HOST):
     _check(load_library().mcrt_read_raw(ctx, _ptr(k_abs), _ptr(lucy_fx), _ptr(sed_counts), _ptr(sed_direct), _ptr(tidx),
@@ -372,6 +388,8 @@ class Context:
             self.stream = torch.cuda.current_stream(self.device)
             mcrt_set_stream(self.ctx, self.stream.cuda_stream)
         mcrt_dust_tables(self.ctx, w.nu_hz, w.kappa_abs, w.kappa_sca, w.g, w.T_grid)
+        if getattr(w, "mixtures", None) is not None:
+            mcrt_dust_mixtures(self.ctx, *w.mixtures)
         mcrt_source(self.ctx, w.L_erg_s, w.T_star_K, w.L_nu_weights, w.source_pos_cm)
         mcrt_escape_bins(self.ctx, w.abs_mu_edges)
         self.last_n = 0
@@ -419,6 +437,14 @@ class Context:
         if digests:
             out["digests"] = dig
         return out
+
+    def read_component(self, component):
+        """Outputs and raw tallies of one component of the mixtures (mcrt_dust_mixtures)."""
+        Ec, El = np.zeros(self.nc), np.zeros(self.nc)
+        Tc, Tl = np.zeros(self.nc, np.float32), np.zeros(self.nc, np.float32)
+        k, L, tidx = np.zeros(self.nc, np.uint64), np.zeros(self.nc, np.int64), np.zeros(self.nc, np.uint16)
+        mcrt_read_component(self.ctx, component, Ec, El, Tc, Tl, k, L, tidx)
+        return {"E_count": Ec, "E_lucy": El, "T_count": Tc, "T_lucy": Tl, "k": k, "lucy_fx": L, "tidx": tidx}
 
     def read(self):
         Ec, El = np.zeros(self.nc), np.zeros(self.nc)

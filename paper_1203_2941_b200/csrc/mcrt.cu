@@ -120,6 +120,15 @@ struct mcrt_ctx {
     CarryRec *carry_buf[2] = {nullptr, nullptr};   // carried packets: read by this epoch / written for the next (cudaMalloc)
     size_t carry_cap[2] = {0, 0};
     int carry_cur = 0;
+    // dust mixtures (mcrt_dust_mixtures; NEXT-3): the species byte of a cell names a mixture of one or two materials
+    bool mix = false;
+    std::vector<int> mx_ncomp, mx_mat;             // [ns], [ns][2]
+    std::vector<double> mx_frac, mx_S0, mx_A0, kabs1_h;   // [ns][2]; [ns*nf] event thresholds, f_1 kabs_1 h
+    int *d_mx_ncomp = nullptr, *d_mx_mat = nullptr;       // device copies and the second component's per-cell arrays (cudaMalloc)
+    double *d_mx_frac = nullptr, *d_mx_thr = nullptr, *d_kabs1_fx = nullptr;   // d_mx_thr: [ns*nf] {S0, A0}
+    long long *lfx1 = nullptr;
+    unsigned long long *kcnt1 = nullptr, *kprev1 = nullptr;
+    uint16_t *tidx1 = nullptr;
     // run in progress (mcrt_run_begin .. mcrt_run_end)
     struct Run {
         bool active = false;
@@ -479,6 +488,13 @@ struct TransportParams {
     const int8_t *__restrict__ sca_slot;       // [nf] slot of a stored frequency bin (-1: not stored), or NULL
     mcrt_scatter_event *__restrict__ sca_ev;   // the event list and its capacity; counters[CNT_SCAEV] counts
     unsigned long long sca_cap;
+    // dust mixtures (NEXT-3; readings Q34-Q36): NULL lfx1 = the species byte names a material
+    long long *__restrict__ lfx1;              // Lucy tally, absorption count and temperature index of the second component
+    unsigned long long *__restrict__ kcnt1;
+    const uint16_t *__restrict__ tidx1;
+    const double *__restrict__ kabs1_fx;       // [ns][nf] f_1 kabs_1 h 2^FX (0 for a one-component mixture)
+    const double2 *__restrict__ mx_thr;        // [ns][nf] {S0, A0}: thresholds of the event uniform
+    const int *__restrict__ mx_mat;            // [ns][2] material of each component
     uint32_t seed_lo, seed_hi, pass;
 };
 
@@ -782,6 +798,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             double2 kq = make_double2(0.0, 0.0);                // {kext_h, kabs_fx} of species kq_sp at the packet's frequency
             uint32_t kq_sp = 0u;
             const double2 *kq_row = s_kk;                       // s_kk + j
+            const double *k1_row = P.kabs1_fx;                  // mixtures: the second component's kabs_fx at frequency j
+            double kq1 = 0.0;
             // words of cells n .. n+kDepth-1, in registers
             unsigned long long cwr[kDepth];
             unsigned long long wstop = 0ull;             // cell word of the cell this lane's packet stopped in (MCRT_STOP_RELOAD)
@@ -890,6 +908,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         for (int i = 0; i < kDepth - 2; ++i) { tq[i] = t; cq[i] = 0u; }
                         kq_row = s_kk + j;
                         kq_sp = 0u; kq = kq_row[0];
+                        if (XTRA && P.lfx1) { k1_row = P.kabs1_fx + j; kq1 = k1_row[0]; }
                         state = ST_FLY;
                     }
                     mFly.remove(take, slot);
@@ -946,6 +965,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq_sp = cw_species(cw);                                                                             \
                         MCRT_CHK(!fly || kq_sp < (uint32_t)P.ns, "walk: species of the cell word");                         \
                         kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
+                        if (XTRA && P.lfx1) kq1 = k1_row[fly ? kq_sp * nf_r : 0u];   /* second component of a mixture */     \
                     }                                                                                                       \
                     const double dtau = kq.x * rho_c * ds;            /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */ \
                     const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
@@ -972,6 +992,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         MCRT_CHK(!(fly && stop) || (uint32_t)slot < (uint32_t)kSlots, "walk: slot of the stopped packet");   \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
                                      ::"l"(lfx_r + kCS * ciA), "l"(q), "r"(HOT ? cold : dusty) : "memory");                 \
+                        if (XTRA && P.lfx1) {       /* the second component's tally (reading Q36) */                         \
+                            const unsigned long long q1 = lucy_round(kq1 * rho_c * ds);                                     \
+                            if (dusty && kq1 != 0.0) lucy_add_raw(P.lfx1, ciA, q1);                                         \
+                        }                                                                                                   \
                         if (HOT && __any_sync(kFull, dusty && hid != 0u)) {                                                 \
                             if (dusty && hid != 0u) hot_add(s_hot, hid, q);                                    \
                         }                                                                                                   \
@@ -1166,6 +1190,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             if (act && !dead) {
                 double px, py, pz, z0, z1;
                 bool scatter = false;
+                double gmix = 0.0;                          // mixtures: g of the scattering component's material
                 int sj = 0;
                 unsigned long long cw;
                 uint32_t cidx;
@@ -1202,6 +1227,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;
                     if (hid) hot_add(s_hot, hid, lucy_round(kq.y * rho_c * sint));
                     else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
+                    // mixtures (NEXT-3, readings Q34-Q36): the second component's tally; which component interacts
+                    double2 thr = make_double2(2.0, 2.0);      // {S0, A0}; a uniform is < 2: one component = always component 0
+                    if (XTRA && P.lfx1) {
+                        const double k1 = P.kabs1_fx[sj];
+                        if (k1 != 0.0) lucy_add(P.lfx1, cidx, k1 * rho_c * sint);
+                        if (P.mx_mat[2 * cw_species(cw) + 1] >= 0) thr = P.mx_thr[sj];
+                    }
                     const double tint = t + sint;
                     double q;
                     q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
@@ -1224,13 +1256,20 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             }
                         }
                         if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
+                        if (XTRA && P.lfx1) gmix = P.g[P.mx_mat[2 * cw_species(cw) + (!(ztype < thr.x) ? 1 : 0)] * nf + j];
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
                         nabs++;
                         MCRT_CHK(cidx < P.ncp, "absorption: storage index of the cell");
-                        const int s = cw_species(cw);
+                        int s = cw_species(cw);
                         int m = cw_tidx(cw, P.tidx_mask);
+                        bool second = false;                   // absorbed by the second component of a mixture
+                        if (XTRA && P.lfx1) {
+                            second = !(ztype < thr.y);
+                            s = P.mx_mat[2 * s + (second ? 1 : 0)];    // the material whose row re-emits
+                            if (second) m = (int)P.tidx1[cidx];
+                        }
                         if (XTRA && P.live_bw) {
                             // Bjorkman & Wood as printed: the temperature is adjusted after each
                             // absorption -- T_{i,k} from the count including this one (Eq. 4).  The count a packet sees
@@ -1238,6 +1277,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             const unsigned long long kn = atomicAdd(&P.kcnt[cidx], 1ull) + 1ull;
                             m = t_index(P.J + s * P.nT, P.nT, (double)kn * P.cellfac / rho_c);
                         } else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
+                        else if (XTRA && second) atomicAdd(&P.kcnt1[cidx], 1ull);
                         else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                         MCRT_CHK(s >= 0 && s < P.ns && m >= 0 && m < P.nT, "absorption: CDF row");
@@ -1250,7 +1290,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                 double mu = 1.0 - 2.0 * z0;
                 if (scatter) {
-                    const double gg = s_ag[sj].y;
+                    const double gg = (XTRA && P.lfx1) ? gmix : s_ag[sj].y;
                     if (fabs(gg) > 1e-6) {
                         const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
                         mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
@@ -1441,6 +1481,57 @@ __global__ void __launch_bounds__(256) k_sweep_update(unsigned long long *__rest
     }
 }
 
+// The same two updates for a grid of dust mixtures (NEXT-3; reading Q36): every component has its own count, tally
+// and temperature index -- Eq. 4 with the component's material and its own mass rho f_c V.  Component 0's index
+// lives in the cell word, component 1's in tidx1.  sweep = 0: epoch rule (S11), 1: frozen-T sweep (S12, zeroes the tallies).
+struct MixArrays {
+    unsigned long long *kcnt[2], *kprev[2];
+    long long *lfx[2];
+    uint16_t *tidx1;
+    const int *ncomp, *mat;
+    const double *frac;
+};
+__global__ void __launch_bounds__(256) k_mix_update(unsigned long long *__restrict__ cellw, MixArrays A, const double *__restrict__ J,
+                                                    int nT, int ns, size_t ncp, int sweep, int first_epoch, double ratio,
+                                                    int from_lucy, double inv_fx, double cellfac,
+                                                    unsigned long long *__restrict__ counters, uint32_t tmask)
+{
+    extern __shared__ double s_J[];
+    for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters[CNT_NEXT] = 0ull; if (!sweep) counters[CNT_CARRY] = 0ull; }
+    bool ovf = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
+        const unsigned long long cw = cellw[kCS * i];
+        const double rho_c = cw_rho(cw);
+        const bool dusty = cw_dusty(cw);
+        const int x = (int)cw_species(cw);
+        uint32_t mi[2] = {0u, 0u};
+        for (int c = 0; c < 2; ++c) {
+            const unsigned long long kc = A.kcnt[c][i];
+            if (dusty && c < A.ncomp[x]) {
+                const long long v = A.lfx[c][kCS * i];
+                double e;
+                if (sweep) e = from_lucy ? (double)v * inv_fx : (double)kc;
+                else if (first_epoch) e = (double)kc + 1.0;
+                else {
+                    const double pred = 0.5 * (double)(kc - A.kprev[c][i]) * ratio;
+                    e = (double)kc + ((pred > 1.0) ? pred : 1.0);
+                }
+                const double xx = e * cellfac / (rho_c * A.frac[2 * x + c]);
+                mi[c] = (uint32_t)t_index(s_J + A.mat[2 * x + c] * nT, nT, xx);
+                ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
+            }
+            if (sweep) { A.kcnt[c][i] = 0ull; A.kprev[c][i] = 0ull; A.lfx[c][kCS * i] = 0ll; }
+            else A.kprev[c][i] = kc;
+        }
+        const uint32_t lo = (uint32_t)cw, nlo = (lo & ~(tmask << 8)) | (mi[0] << 8);
+        if (nlo != lo && dusty) reinterpret_cast<uint32_t *>(cellw + kCS * i)[0] = nlo;
+        A.tidx1[i] = (uint16_t)mi[1];
+    }
+    if (ovf && !sweep) counters[CNT_OVERFLOW] = 1ull;
+}
+
 // Partitioned runs: between epochs a part's absorption counts are exchanged as this epoch's own
 // increments, k - k_prev (k_prev = the global counts at the start of the epoch), and restored afterwards.
 __global__ void __launch_bounds__(256) k_count_delta(unsigned long long *__restrict__ kcnt, const unsigned long long *__restrict__ kprev,
@@ -1627,8 +1718,11 @@ __device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int 
 __global__ void k_gather(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
                          const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
                          const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
-                         int px, int pxy, double xi, double inv_fx, double cellfac, uint32_t tmask)
+                         int px, int pxy, double xi, double inv_fx, double cellfac, uint32_t tmask,
+                         const int *__restrict__ mx_mat, const double *__restrict__ mx_frac, int comp,
+                         const uint16_t *__restrict__ tidx1)
 {
+    // (mixtures, NEXT-3: kcnt / lfx are those of component `comp`, whose material and mass fraction enter Eq. 4)
     const size_t nc = (size_t)nx * ny * nz;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
         const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
@@ -1636,7 +1730,7 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
         switch (what) {
         case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
         case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[bs]; break;
-        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = (uint16_t)cw_tidx(cellw[bs], tmask); break;
+        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = comp ? tidx1[b] : (uint16_t)cw_tidx(cellw[bs], tmask); break;
         case G_ECOUNT: reinterpret_cast<double *>(out)[i] = (double)kcnt[b] * xi; break;
         case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[bs] * inv_fx * xi; break;
         default: {
@@ -1645,7 +1739,11 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
             float T = 0.0f;
             if (cw_dusty(cw)) {
                 const double e = (what == G_TLUCY) ? (double)lfx[bs] * inv_fx : (double)kcnt[b];
-                T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
+                if (!mx_mat) T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
+                else {
+                    const int m = mx_mat[2 * cw_species(cw) + comp];
+                    if (m >= 0) T = (float)T_of_x(J + m * nT, Tg, nT, e * cellfac / (rho_c * mx_frac[2 * cw_species(cw) + comp]));
+                }
             }
             reinterpret_cast<float *>(out)[i] = T;
         }
@@ -2194,6 +2292,80 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
     return MCRT_OK;
 }
 
+int mcrt_dust_mixtures(mcrt_ctx *c, const int32_t *n_components, const int32_t *material, const double *fraction)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->have_tables) return fail(c, MCRT_ESTATE, "call mcrt_dust_tables before mcrt_dust_mixtures");
+    if (c->mix) return fail(c, MCRT_ESTATE, "mcrt_dust_mixtures may be called once per context");
+    if (c->last_n || c->run.active) return fail(c, MCRT_ESTATE, "mcrt_dust_mixtures after a run");
+    if (!n_components || !material || !fraction) return fail(c, MCRT_EINVAL, "NULL mixture table");
+    const int ns = c->ns, nf = c->nf;
+    for (int x = 0; x < ns; ++x) {
+        if (n_components[x] < 1 || n_components[x] > 2) return fail(c, MCRT_EINVAL, "a mixture has 1 or 2 components");
+        double tot = 0.0;
+        for (int k = 0; k < n_components[x]; ++k) {
+            if (material[2 * x + k] < 0 || material[2 * x + k] >= ns) return fail(c, MCRT_EINVAL, "material index out of range");
+            if (!(fraction[2 * x + k] > 0.0) || !isfinite(fraction[2 * x + k])) return fail(c, MCRT_EINVAL, "mass fractions must be > 0");
+            tot += fraction[2 * x + k];
+        }
+        if (fabs(tot - 1.0) > 1e-12) return fail(c, MCRT_EINVAL, "the mass fractions of a mixture must add up to 1");
+    }
+    const size_t nsf = (size_t)ns * nf;
+    c->mx_ncomp.assign(n_components, n_components + ns);
+    c->mx_mat.assign(2 * (size_t)ns, -1);
+    c->mx_frac.assign(2 * (size_t)ns, 0.0);
+    c->mx_S0.assign(nsf, 0.0); c->mx_A0.assign(nsf, 1.0); c->kabs1_h.assign(nsf, 0.0);
+    std::vector<double> thr(2 * nsf);
+    // readings Q34 / Q35: extinction adds up in component order; the event uniform's thresholds
+    for (int x = 0; x < ns; ++x) {
+        for (int k = 0; k < n_components[x]; ++k) { c->mx_mat[2 * x + k] = material[2 * x + k]; c->mx_frac[2 * x + k] = fraction[2 * x + k]; }
+        const int m0 = material[2 * x];
+        for (int j = 0; j < nf; ++j) {
+            const size_t i = (size_t)x * nf + j, i0 = (size_t)m0 * nf + j;
+            if (n_components[x] == 1) {       // the material itself: the arithmetic of mcrt_dust_tables
+                const double kext = c->kabs[i0] + c->ksca[i0];
+                c->kext_h[i] = kext * c->h;
+                c->kabs_h[i] = c->kabs[i0] * c->h;
+                c->albedo[i] = c->ksca[i0] / kext;
+                c->mx_S0[i] = c->albedo[i]; c->mx_A0[i] = 1.0;
+            } else {
+                const size_t i1 = (size_t)material[2 * x + 1] * nf + j;
+                const double f0 = fraction[2 * x], f1 = fraction[2 * x + 1];
+                const double ka0 = f0 * c->kabs[i0], ks0 = f0 * c->ksca[i0], ka1 = f1 * c->kabs[i1], ks1 = f1 * c->ksca[i1];
+                const double kext = (ka0 + ks0) + (ka1 + ks1);
+                c->kext_h[i] = kext * c->h;
+                c->kabs_h[i] = ka0 * c->h;
+                c->kabs1_h[i] = ka1 * c->h;
+                c->mx_S0[i] = ks0 / kext;
+                c->albedo[i] = (ks0 + ks1) / kext;
+                c->mx_A0[i] = ((ks0 + ks1) + ka0) / kext;
+            }
+            thr[2 * i] = c->mx_S0[i]; thr[2 * i + 1] = c->mx_A0[i];
+        }
+    }
+    // NB: c->kabs / c->ksca / c->g stay the MATERIALS' tables; kext_h, kabs_h and albedo are now the mixtures'
+    const size_t cells = c->ncp * (size_t)kCS;
+    if (cudaMalloc((void **)&c->d_mx_ncomp, ns * sizeof(int)) != cudaSuccess || cudaMalloc((void **)&c->d_mx_mat, 2 * ns * sizeof(int)) != cudaSuccess ||
+        cudaMalloc((void **)&c->d_mx_frac, 2 * ns * 8) != cudaSuccess || cudaMalloc((void **)&c->d_mx_thr, 2 * nsf * 8) != cudaSuccess ||
+        cudaMalloc((void **)&c->d_kabs1_fx, nsf * 8) != cudaSuccess || cudaMalloc((void **)&c->lfx1, cells * 8) != cudaSuccess ||
+        cudaMalloc((void **)&c->kcnt1, c->ncp * 8) != cudaSuccess || cudaMalloc((void **)&c->kprev1, c->ncp * 8) != cudaSuccess ||
+        cudaMalloc((void **)&c->tidx1, c->ncp * 2) != cudaSuccess)
+        return fail(c, MCRT_ENOMEM, "cudaMalloc of the second component's arrays failed");
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_mx_ncomp, c->mx_ncomp.data(), ns * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_mx_mat, c->mx_mat.data(), 2 * ns * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_mx_frac, c->mx_frac.data(), 2 * ns * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_mx_thr, thr.data(), 2 * nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_kext_h, c->kext_h.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemcpyAsync(c->d_albedo, c->albedo.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->lfx1, 0, cells * 8, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->kcnt1, 0, c->ncp * 8, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->kprev1, 0, c->ncp * 8, c->stream));
+    CUDA_TRY(c, cudaMemsetAsync(c->tidx1, 0, c->ncp * 2, c->stream));
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));   // thr and the host vectors must outlive the copies
+    c->mix = true;
+    return MCRT_OK;
+}
+
 // Number the first n_use candidates (nearest first) as hot cells 1..n_use in their cell words, after clearing the
 // numbering in force.
 static int apply_hot(mcrt_ctx *c, int n_use)
@@ -2355,7 +2527,7 @@ static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, in
             if (smem_carveout(transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, t, record, 0)) <= 164 * 1024) { *threads = t; break; }
     const size_t base = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0);
     // ... and as many hot cells as the carve-out these need leaves room for (live B&W needs every count in global memory)
-    int nh = (o && (o->no_hot_cells || o->mode == MCRT_MODE_LIVE_BW)) ? 0 : (int)c->hot_cand.size();
+    int nh = (c->mix || (o && (o->no_hot_cells || o->mode == MCRT_MODE_LIVE_BW))) ? 0 : (int)c->hot_cand.size();
     const size_t cap = smem_carveout(base) - kSmemOverhead;
     while (nh > 0 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh) > cap) --nh;
     if (nh < 8) nh = 0;
@@ -2419,6 +2591,15 @@ static void launch_transport(mcrt_ctx *c, const TransportParams &P)
     transport_kernel(R.o.record_digests != 0, R.hot, R.xtra)<<<R.blocks, R.threads, R.smem, c->stream>>>(P);
 }
 
+static MixArrays mix_arrays(mcrt_ctx *c)
+{
+    MixArrays A;
+    A.kcnt[0] = c->kabs_cnt; A.kcnt[1] = c->kcnt1; A.kprev[0] = c->kprev; A.kprev[1] = c->kprev1;
+    A.lfx[0] = c->lfx; A.lfx[1] = c->lfx1; A.tidx1 = c->tidx1;
+    A.ncomp = c->d_mx_ncomp; A.mat = c->d_mx_mat; A.frac = c->d_mx_frac;
+    return A;
+}
+
 static void fill_params(mcrt_ctx *c, TransportParams &P)
 {
     memset(&P, 0, sizeof(P));
@@ -2429,6 +2610,10 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
     P.source_strata = c->run.o.source_strata; P.live_bw = c->run.o.mode == MCRT_MODE_LIVE_BW; P.J = c->d_J; P.cellfac = c->run.cellfac;
     P.sca_slot = c->sca_ev ? c->d_sca_slot : nullptr; P.sca_ev = c->sca_ev; P.sca_cap = c->sca_cap;
     P.hot_idx = c->d_hot_idx; P.hot_shift = c->hot_shift; P.hot_mask = c->hot_mask; P.tidx_mask = c->tidx_mask; P.n_hot = c->n_hot;
+    if (c->mix) {
+        P.lfx1 = c->lfx1; P.kcnt1 = c->kcnt1; P.tidx1 = c->tidx1; P.kabs1_fx = c->d_kabs1_fx;
+        P.mx_thr = reinterpret_cast<const double2 *>(c->d_mx_thr); P.mx_mat = c->d_mx_mat;
+    }
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base; P.dig_n = c->dig_n;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
@@ -2547,13 +2732,15 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (!(o.epoch_growth >= 1.0) || !isfinite(o.epoch_growth)) return fail(c, MCRT_EINVAL, "epoch_growth must be >= 1");
     if (o.n_total && o.n_total < n_packets) return fail(c, MCRT_EINVAL, "n_total must be >= n_packets");
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
+    if (c->mix && (o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
+        return fail(c, MCRT_EINVAL, "dust mixtures are not available in live B&W or partitioned runs");
     int rc = ensure_histograms(c);
     if (rc) return rc;
     mcrt_ctx::Run &R = c->run;
     int n_hot = 0;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
     if ((rc = apply_hot(c, n_hot))) return rc;
-    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW;
+    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix;
     R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
@@ -2580,6 +2767,11 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         CUDA_TRY(c, cudaMemset2DAsync(c->lfx, 8 * kCS, 0, 8, c->ncp, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
+        if (c->mix) {
+            CUDA_TRY(c, cudaMemsetAsync(c->lfx1, 0, c->ncp * (size_t)kCS * 8, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->kcnt1, 0, c->ncp * 8, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->kprev1, 0, c->ncp * 8, c->stream));
+        }
         CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_N * 8, c->stream));
@@ -2600,11 +2792,17 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         for (size_t i = 0; i < nsf; ++i) kfx[i] = ldexp(c->kabs_h[i], c->fx);
         CUDA_TRY(c, cudaMemcpyAsync(c->d_kabs_fx, kfx.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        if (c->mix) {
+            for (size_t i = 0; i < nsf; ++i) kfx[i] = ldexp(c->kabs1_h[i], c->fx);
+            CUDA_TRY(c, cudaMemcpyAsync(c->d_kabs1_fx, kfx.data(), nsf * 8, cudaMemcpyHostToDevice, c->stream));
+            CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+        }
     }
     const size_t j_smem = (size_t)c->ns * c->nT * 8;
     if (j_smem > 48 * 1024) {
         CUDA_TRY(c, cudaFuncSetAttribute(k_epoch_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_sweep_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
+        CUDA_TRY(c, cudaFuncSetAttribute(k_mix_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
     }
     R.o = o; R.n = n_packets; R.seed = seed; R.done = 0; R.Bprev = 0; R.e = 0; R.sweep = 0; R.finished = false;
     R.carry_K = (o.mode == MCRT_MODE_BW_EPOCH) ? o.carry_interactions : 0u; R.n_carry = 0;
@@ -2656,6 +2854,11 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
             P.n_carry_in = (uint32_t)R.n_carry; P.carry_K = R.carry_K;
         }
         mark(c, timing);
+        if (c->mix)
+            k_mix_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, mix_arrays(c), c->d_J, c->nT, c->ns, c->ncp, 0, R.e == 0,
+                                                           (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev, 0, 0.0,
+                                                           R.cellfac, c->counters, c->tidx_mask);
+        else
         k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          R.e == 0, (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev,
                                                          R.cellfac, c->counters, c->tidx_mask);
@@ -2687,6 +2890,11 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         P.cdf = c->d_cdfB;
         // temperatures of the previous pass (its own packet energy and fixed-point scale), then zero and re-run all N packets
         mark(c, timing);
+        if (c->mix)
+            k_mix_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, mix_arrays(c), c->d_J, c->nT, c->ns, c->ncp, 1, 0, 1.0,
+                                                           o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
+                                                           sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
+        else
         k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
                                                          sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
@@ -2725,7 +2933,8 @@ int mcrt_run_end(mcrt_ctx *c, mcrt_run_stats *stats_out)
     if (!R.finished) return fail(c, MCRT_ESTATE, "mcrt_run_end before the last mcrt_run_step");
     if (c->need_exchange) return fail(c, MCRT_ESTATE, "partitioned run: exchange the last step's tallies before mcrt_run_end");
     k_range_check<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx, c->ncp, c->counters);
-    c->launches += 1;
+    if (c->mix) k_range_check<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx1, c->ncp, c->counters);
+    c->launches += c->mix ? 2 : 1;
     R.active = false;
     CUDA_TRY(c, cudaGetLastError());
     if (stats_out) {
@@ -2837,13 +3046,15 @@ int mcrt_exchange_local(mcrt_ctx *const *parts, int n_parts)
     return MCRT_OK;
 }
 
-static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem where)
+static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem where, int comp = 0)
 {
     if (!dst) return MCRT_OK;
     void *dev = (where == MCRT_DEVICE) ? dst : c->scratch;
     const double cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
-    k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, c->kabs_cnt, c->lfx, c->d_J, c->d_Tg, c->nT, c->nx,
-                                                       c->ny, c->nz, c->px, c->pxy, c->xi, ldexp(1.0, -c->fx), cellfac, c->tidx_mask);
+    k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, comp ? c->kcnt1 : c->kabs_cnt, comp ? c->lfx1 : c->lfx,
+                                                       c->d_J, c->d_Tg, c->nT, c->nx, c->ny, c->nz, c->px, c->pxy, c->xi,
+                                                       ldexp(1.0, -c->fx), cellfac, c->tidx_mask, c->mix ? c->d_mx_mat : nullptr,
+                                                       c->d_mx_frac, comp, c->tidx1);
     CUDA_TRY(c, cudaGetLastError());
     if (where == MCRT_HOST) {
         CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
@@ -2881,6 +3092,27 @@ int mcrt_read(mcrt_ctx *c, double *E_abs_count, double *E_abs_lucy, float *T_cou
             CUDA_TRY(c, cudaMemcpyAsync(SED, dev, (size_t)n * 8, cudaMemcpyDeviceToHost, c->stream));
         }
     }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
+int mcrt_read_component(mcrt_ctx *c, int component, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy,
+                        uint64_t *k_abs, int64_t *lucy_fx, uint16_t *tidx, mcrt_mem where)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->mix) return fail(c, MCRT_ESTATE, "mcrt_read_component without mcrt_dust_mixtures");
+    if (component < 0 || component > 1) return fail(c, MCRT_EINVAL, "component must be 0 or 1");
+    if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read_component before mcrt_run");
+    if (c->run.active) return fail(c, MCRT_ESTATE, "mcrt_read_component inside mcrt_run_begin .. mcrt_run_end");
+    int rc;
+    if ((rc = check_overflow(c))) return rc;
+    if ((rc = gather_out(c, G_ECOUNT, E_abs_count, 8, where, component))) return rc;
+    if ((rc = gather_out(c, G_ELUCY, E_abs_lucy, 8, where, component))) return rc;
+    if ((rc = gather_out(c, G_TCOUNT, T_count, 4, where, component))) return rc;
+    if ((rc = gather_out(c, G_TLUCY, T_lucy, 4, where, component))) return rc;
+    if ((rc = gather_out(c, G_K, k_abs, 8, where, component))) return rc;
+    if ((rc = gather_out(c, G_LFX, lucy_fx, 8, where, component))) return rc;
+    if ((rc = gather_out(c, G_TIDX, tidx, 2, where, component))) return rc;
     CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     return MCRT_OK;
 }
@@ -2953,6 +3185,7 @@ int mcrt_ray_trace(mcrt_ctx *c, const mcrt_image_opts *io, double *F_emission, d
 {
     if (!c || !io || !F_emission) return MCRT_EINVAL;
     if (!c->last_n || c->run.active) return fail(c, MCRT_ESTATE, "mcrt_ray_trace needs a finished run");
+    if (c->mix) return fail(c, MCRT_EINVAL, "mcrt_ray_trace: images of dust mixtures are not defined");
     if (io->nx < 1 || io->ny < 1 || (size_t)io->nx * io->ny > ((size_t)1 << 28) || !(io->pixel_cm > 0.0) || !(io->distance_cm > 0.0) ||
         io->nu_bin < 0 || io->nu_bin >= c->nf)
         return fail(c, MCRT_EINVAL, "mcrt_ray_trace: bad image options");
@@ -3090,6 +3323,9 @@ void mcrt_destroy(mcrt_ctx *c)
     if (c->d_sca_slot) cudaFree(c->d_sca_slot);
     if (c->sca_ev) cudaFree(c->sca_ev);
     if (c->img_buf) cudaFree(c->img_buf);
+    for (void *p : {(void *)c->d_mx_ncomp, (void *)c->d_mx_mat, (void *)c->d_mx_frac, (void *)c->d_mx_thr, (void *)c->d_kabs1_fx,
+                    (void *)c->lfx1, (void *)c->kcnt1, (void *)c->kprev1, (void *)c->tidx1})
+        if (p) cudaFree(p);
     delete c;
 }
 

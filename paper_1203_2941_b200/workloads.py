@@ -56,6 +56,9 @@ class Workload:
     n_packets: int  # the configuration's full packet count
     seed: int
     meta: dict = dataclasses.field(default_factory=dict)
+    # NEXT-3: (n_components[n_species], material[n_species][2], mass fraction[n_species][2]): cell species x is a mixture
+    # of one or two of the n_species materials (None: species x is material x)
+    mixtures: tuple | None = None
 
     @property
     def n_cells(self) -> int:

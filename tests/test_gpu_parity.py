@@ -663,3 +663,63 @@ def test_partitioned_run_across_processes(B, mode):
                         "--master-addr", "127.0.0.1", "--master-port", str(port), worker, mode],
                        capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "PARTITION_OK" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
+
+
+@pytest.mark.parametrize("case", ["torus", "identity", "sweeps_carry"])
+def test_parity_dust_mixtures(B, orc, case):
+    """NEXT-3 (readings Q34-Q36; oracle pins P22): cell species are mixtures of one or two of the
+    materials, every component with its own absorption count, Lucy tally and temperature index.  Bit-equal to the
+    oracle: digests, both components' counts / tallies / temperature indices, escape histograms."""
+    if case == "torus":
+        w = W.torus256(n_clumps=400, n=64)               # 3 materials -> 3 mixtures, one of them a single material
+        w.mixtures = ([2, 1, 2], [[0, 1], [1, -1], [2, 0]], [[0.3, 0.7], [1.0, 0.0], [0.55, 0.45]])
+        N, kw = 150_000, {}
+    elif case == "identity":
+        w = W.torus256(n_clumps=50, n=16)                # every species its own material: the run without mixtures
+        w.mixtures = ([1, 1, 1], [[0, -1], [1, -1], [2, -1]], [[1.0, 0.0]] * 3)
+        N, kw = 40_000, {}
+    else:
+        w = W.sphere32(tau_V=20.0, n=16)                 # 1 material cannot mix: give the sphere a second one
+        lam_slope = (w.nu_hz / w.nu_hz[-1])
+        w.kappa_abs = np.vstack([w.kappa_abs, w.kappa_abs[:1] * lam_slope])
+        w.kappa_sca = np.vstack([w.kappa_sca, 0.5 * w.kappa_sca[:1]])
+        w.g = np.vstack([w.g, 0.0 * w.g[:1] + 0.2])
+        w.n_species = 2
+        w.mixtures = ([2, 2], [[0, 1], [1, 0]], [[0.6, 0.4], [0.5, 0.5]])
+        N, kw = 50_000, {"carry_K": 30}
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 77, n_threads=NTH, digests=True, **kw)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 77, record_digests=1, **({"carry_interactions": 30} if kw else {}))
+    for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+        assert ro[key] == rg[key], key
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    o1, g1 = o.read_raw_comp1(), c.read_component(1)
+    for key in ("k", "lucy_fx", "tidx"):
+        assert np.array_equal(o1[key], g1[key]), key
+    g0 = c.read_component(0)
+    assert np.array_equal(g0["k"], raw_g["k"]) and np.array_equal(g0["lucy_fx"], raw_g["lucy_fx"])
+    if case != "identity":
+        assert o1["k"].sum() > 100 and (o1["lucy_fx"] != 0).sum() > 100
+    else:
+        assert not g1["k"].any()
+        o_plain = orc.Oracle.from_workload(W.torus256(n_clumps=50, n=16))
+        r_plain = o_plain.run(N, 77, n_threads=NTH, digests=True)
+        assert np.array_equal(r_plain["digests"], raw_g["digests"])
+    # physical outputs of both components (T by inverting Eq. 4 with the component's material and mass)
+    for comp, (oo, gg) in enumerate(((o.read(), g0), (o.read_comp1(), g1))):
+        assert np.allclose(oo["E_lucy"], gg["E_lucy"], rtol=1e-13, atol=0.0), comp
+        assert np.allclose(oo["T"], gg["T_count"], rtol=2e-6, atol=0.0), comp
+    if case == "sweeps_carry":
+        o.run(N, 78, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=2, sweep_T_from_lucy=1, reset=False, n_threads=NTH, digests=True)
+        c.run(N, 78, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=2, sweep_T_from_lucy=1, record_digests=1)
+        raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+        for key in RAW_KEYS:
+            assert np.array_equal(raw_o[key], raw_g[key]), key
+        o1, g1 = o.read_raw_comp1(), c.read_component(1)
+        for key in ("k", "lucy_fx", "tidx"):
+            assert np.array_equal(o1[key], g1[key]), key
+    c.close()
