@@ -559,7 +559,21 @@ typedef struct {
     double growth;           /* epoch e+1 has min(floor(B_e * growth), Bmax) packets; 0 = 2 (O11) */
     uint32_t carry_K;        /* > 0: a packet is carried over to the next epoch after this many interactions in one epoch */
     uint32_t source_strata;  /* > 0: the source frequency is drawn stratified (Eq. 1): stratum = packet id mod source_strata */
+    int32_t lucy_hybrid;     /* 1: the thresholded estimator of Sect. 3.1 / Eq. 9 (see orc_thin_cell, lucy_add) */
 } orc_opts;
+
+/* Sect. 3.1: "It is applied whenever the maximal optical depth of a cell i is smaller than 10^-2."
+ * Reading Q37: the maximal optical depth of a cell is that of its longest chord, the diagonal, at the frequency of
+ * its largest extinction: tau_max = sqrt(3) h rho_i max_nu (kabs + ksca). */
+#define ORC_THIN_TAU 1e-2
+static inline int orc_thin_cell(double rho_c, double kmax_diag) { return rho_c > 0.0 && rho_c * kmax_diag < ORC_THIN_TAU; }
+/* Eq. 9: E_abs = (1 - e^-tau) xi for one traversal, tau the absorption optical depth of the chord (reading Q38: the
+ * energy ABSORBED, so kabs only).  tau < 10^-2 here, and 1 - e^-tau is DEFINED as its series up to tau^5 in this
+ * fixed order (truncation < 2 10^-13 relative), so that every implementation gets the same bits. */
+static inline double orc_eq9(double tau)
+{
+    return tau * (1.0 - tau * (0.5 - tau * (1.0 / 6.0 - tau * (1.0 / 24.0 - tau * (1.0 / 120.0)))));
+}
 
 /* One stored scattering event ("The index of the cell, the frequency of the scattered photon and the
  * incoming direction is stored"): cell in [nz][ny][nx] order, slot of the frequency bin among the recorded ones,
@@ -594,6 +608,7 @@ typedef struct {
     int64_t *Lfx1;
     uint16_t *tidx1;
     double *kabs1_fx;
+    const double *kmax_diag; /* lucy_hybrid: [ns] sqrt(3) h max_nu (kabs + ksca) per species, else NULL */
     uint64_t *sed, *sed_direct; /* [ndir][nf] */
     orc_digest *dig;         /* [n_packets] or NULL */
     double *kabs_fx;         /* kabs_h * 2^FX */
@@ -625,6 +640,15 @@ static inline uint64_t event_word(int type, int j, uint64_t cell)
  * integer so that the sum does not depend on the order of additions (integer atomics). */
 static inline void lucy_add(orc_run_t *R, size_t ci, int sj, double rho_c, double ds, orc_stats *st)
 {
+    if (R->kmax_diag) {
+        /* Sect. 3.1 as printed: only cells below the threshold are tallied, with Eq. 9 per traversal (readings Q37, Q38) */
+        if (!orc_thin_cell(rho_c, R->kmax_diag[sj / R->C->nf])) return;
+        double tau = R->kabs_fx[sj] * rho_c * ds * ldexp(1.0, -R->fx);
+        int64_t q = (int64_t)llrint(ldexp(orc_eq9(tau), R->fx));
+        __atomic_fetch_add(&R->Lfx[ci], q, __ATOMIC_RELAXED);
+        st->lucy_adds++;
+        return;
+    }
     if (rho_c > 0.0) {
         double x = R->kabs_fx[sj] * rho_c * ds;
         int64_t q = (int64_t)llrint(x);
@@ -901,6 +925,8 @@ typedef struct {
     uint16_t *tidx1;
     uint64_t *sed, *sed_direct;
     int fx;
+    int hybrid;              /* the stored tallies were made with lucy_hybrid */
+    double *kmax_diag;       /* [ns] sqrt(3) h max_nu (kabs + ksca), reading Q37 */
     double xi;               /* packet energy L/N of the run that produced the stored tallies */
     int32_t *sca_slot;       /* [nf] slot of a recorded frequency bin, -1 otherwise; NULL = nothing is recorded */
     int n_sca_bins;
@@ -933,7 +959,7 @@ void orc_state_destroy(orc_state *S)
 {
     if (!S) return;
     free(S->k); free(S->kprev); free(S->Lfx); free(S->Lsum); free(S->Lcmp); free(S->tidx);
-    free(S->k1); free(S->kprev1); free(S->Lfx1); free(S->tidx1);
+    free(S->k1); free(S->kprev1); free(S->Lfx1); free(S->tidx1); free(S->kmax_diag);
     free(S->sed); free(S->sed_direct); free(S->sca_slot); free(S->sca_ev); free(S);
 }
 
@@ -982,9 +1008,19 @@ void orc_default_schedule(uint64_t n_packets, uint64_t *B0, uint64_t *Bmax)
 static void epoch_update(orc_state *S, int first_epoch, double ratio, double cellfac)
 {
     const orc_ctx *C = S->C;
+    const double inv_fx = ldexp(1.0, -S->fx);
     for (size_t ci = 0; ci < S->nc; ++ci) {
         double rho_c = (double)C->rho[ci];
         uint64_t kk = S->k[ci];
+        if (S->hybrid && orc_thin_cell(rho_c, S->kmax_diag[C->sp[ci]])) {
+            /* Sect. 3.1 (reading Q39): the temperature of a cell below the threshold comes from its Eq. 9 energy, Eq. 4
+             * with k xi replaced by E_abs; the same midpoint prediction, on the tally (k_prev keeps the tally here) */
+            double E = (double)S->Lfx[ci] * inv_fx, Ep = (double)(int64_t)S->kprev[ci] * inv_fx;
+            double Et = first_epoch ? E : E + 0.5 * (E - Ep) * ratio;
+            S->tidx[ci] = (uint16_t)t_index(C, C->sp[ci], Et * cellfac / rho_c);
+            S->kprev[ci] = (uint64_t)S->Lfx[ci];
+            continue;
+        }
         if (rho_c > 0.0) {
             double kt;
             if (first_epoch) kt = (double)kk + 1.0;
@@ -1028,6 +1064,7 @@ static void sweep_update(orc_state *S, int from_lucy, double cellfac, int fx_of_
         double rho_c = (double)C->rho[ci];
         if (rho_c > 0.0) {
             double e = from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+            if (S->hybrid) e = orc_thin_cell(rho_c, S->kmax_diag[C->sp[ci]]) ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
             double x = e * cellfac / (C->n_mix ? rho_c * C->mx_frac[2 * C->sp[ci]] : rho_c);
             S->tidx[ci] = (uint16_t)t_index(C, comp_mat(C, C->sp[ci], 0), x);
         } else {
@@ -1070,12 +1107,28 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
     S->xi = C->L / (double)n_xi;                         /* xi = L/N */
     if (!o->reset && o->mode == ORC_MODE_BW_EPOCH && prev_xi != 0.0 && (prev_xi != S->xi || prev_fx != S->fx))
         return -2;                                       /* tallies of another packet energy cannot be continued */
+    if (o->lucy_hybrid && C->n_mix) return -3;           /* not defined for mixtures */
+    if (!o->reset && prev_xi != 0.0 && (S->hybrid != 0) != (o->lucy_hybrid != 0))
+        return -2;                                       /* tallies of the other estimator cannot be continued */
+    if (o->lucy_hybrid && !S->kmax_diag) {
+        S->kmax_diag = (double *)malloc(C->ns * sizeof(double));
+        for (int s = 0; s < C->ns; ++s) {
+            double km = 0.0;
+            for (int j = 0; j < C->nf; ++j) {
+                double ke = C->kabs[s * C->nf + j] + C->ksca[s * C->nf + j];
+                if (ke > km) km = ke;
+            }
+            S->kmax_diag[s] = sqrt(3.0) * C->h * km;
+        }
+    }
+    S->hybrid = o->lucy_hybrid ? 1 : 0;
     double cellfac = S->xi / (ORC_FOUR_PI * C->h * C->h * C->h); /* xi / (4 pi V), Eq. 4 */
     /* Eq. 4 for the first sweep: k and L were counted in packets of the PREVIOUS run's energy */
     double prev_cellfac = prev_xi / (ORC_FOUR_PI * C->h * C->h * C->h);
     size_t nsf = (size_t)C->ntab * C->nf;
     R.C = C; R.k = S->k; R.kprev = S->kprev; R.Lfx = S->Lfx; R.tidx = S->tidx;
     R.k1 = S->k1; R.Lfx1 = S->Lfx1; R.tidx1 = S->tidx1;
+    R.kmax_diag = S->hybrid ? S->kmax_diag : NULL;
     R.Lsum = o->keep_fp64_lucy ? S->Lsum : NULL; R.Lcmp = S->Lcmp;
     R.sed = S->sed; R.sed_direct = S->sed_direct; R.dig = digests; R.seed = seed; R.fx = S->fx; R.o = o;
     R.pid0_digest = o->pid0;
@@ -1170,6 +1223,9 @@ void orc_read_raw(const orc_state *S, uint64_t *k, int64_t *Lfx, uint64_t *sed, 
     if (Lsum && S->Lsum) memcpy(Lsum, S->Lsum, S->nc * sizeof(double));
 }
 
+/* Eq. 9 as evaluated by lucy_add, for the pin that compares it with 1 - exp(-tau) */
+double orc_eq9_value(double tau) { return orc_eq9(tau); }
+
 /* raw tallies of the second component of a mixture (NEXT-3) */
 int orc_read_raw_comp1(const orc_state *S, uint64_t *k, int64_t *Lfx, uint16_t *tidx)
 {
@@ -1212,6 +1268,8 @@ void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int
             double rho_c = (double)C->rho[ci];
             if (rho_c > 0.0) {
                 double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+                if (T_from_lucy == 2)   /* Sect. 3.1: Eq. 9 energy below the threshold, counts above (reading Q39) */
+                    e = (S->kmax_diag && orc_thin_cell(rho_c, S->kmax_diag[C->sp[ci]])) ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
                 double mass = C->n_mix ? rho_c * C->mx_frac[2 * C->sp[ci]] : rho_c;
                 T[ci] = (float)orc_T_of_x(C, comp_mat(C, C->sp[ci], 0), e * cellfac / mass);
             } else T[ci] = 0.0f;

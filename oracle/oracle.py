@@ -34,7 +34,7 @@ class Opts(C.Structure):
     _fields_ = [("mode", C.c_int32), ("B0", C.c_uint64), ("Bmax", C.c_uint64), ("n_sweeps", C.c_int32),
                 ("sweep_T_from_lucy", C.c_int32), ("n_threads", C.c_int32), ("absorb_and_stop", C.c_int32),
                 ("per_cell_redraw", C.c_int32), ("keep_fp64_lucy", C.c_int32), ("reset", C.c_int32),
-                ("pass0", C.c_uint32), ("pid0", C.c_uint64), ("n_total", C.c_uint64), ("growth", C.c_double), ("carry_K", C.c_uint32), ("source_strata", C.c_uint32)]
+                ("pass0", C.c_uint32), ("pid0", C.c_uint64), ("n_total", C.c_uint64), ("growth", C.c_double), ("carry_K", C.c_uint32), ("source_strata", C.c_uint32), ("lucy_hybrid", C.c_int32)]
 
 
 SCA_EVENT_DTYPE = np.dtype([("cell", np.uint32), ("slot", np.uint16), ("q", np.int16, (3,))])
@@ -64,6 +64,8 @@ def lib():
         L.orc_read_raw.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.orc_read.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         L.orc_get_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
+        L.orc_eq9_value.restype = C.c_double
+        L.orc_eq9_value.argtypes = [C.c_double]
         L.orc_set_mixtures.restype = C.c_int
         L.orc_set_mixtures.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_read_raw_comp1.restype = C.c_int
@@ -190,6 +192,10 @@ def phase_hg(g, cos_beta):
     return lib().orc_phase_hg(float(g), float(cos_beta))
 
 
+def eq9_value(tau):
+    return lib().orc_eq9_value(float(tau))
+
+
 def max_threads():
     return lib().orc_max_threads()
 
@@ -260,9 +266,9 @@ class Oracle:
 
     def run(self, n_packets, seed, mode=MODE_BW_EPOCH, B0=0, Bmax=0, n_sweeps=0, sweep_T_from_lucy=1,
             n_threads=1, absorb_and_stop=False, per_cell_redraw=False, keep_fp64_lucy=False, reset=True,
-            pass0=0, digests=False, pid0=0, n_total=0, growth=0.0, carry_K=0, source_strata=0):
+            pass0=0, digests=False, pid0=0, n_total=0, growth=0.0, carry_K=0, source_strata=0, lucy_hybrid=False):
         o = Opts(mode, B0, Bmax, n_sweeps, int(sweep_T_from_lucy), n_threads, int(absorb_and_stop),
-                 int(per_cell_redraw), int(keep_fp64_lucy), int(reset), pass0, int(pid0), int(n_total), float(growth), int(carry_K), int(source_strata))
+                 int(per_cell_redraw), int(keep_fp64_lucy), int(reset), pass0, int(pid0), int(n_total), float(growth), int(carry_K), int(source_strata), int(lucy_hybrid))
         st = Stats()
         dig = np.zeros(n_packets, DIGEST_DTYPE) if digests else None
         rc = lib().orc_run(self._state, int(n_packets), int(seed), C.byref(o), C.byref(st), _p(dig))

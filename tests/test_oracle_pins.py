@@ -1065,3 +1065,85 @@ def test_p22_mixture_component_order_is_a_relabelling(orc):
             assert abs(TA[m][s].mean() / TB[m][s].mean() - 1) < 0.01, (m, r_lo, TA[m][s].mean(), TB[m][s].mean())
     s = (r >= 4.0) & (r < 5.0)
     assert TA[1][s].mean() / TA[0][s].mean() > 1.1        # the two materials' temperatures differ: the pin has teeth
+
+
+# ------------------------------------------------------------------------------------------ P23 Eq. 9 hybrid (NEXT-4)
+def test_p23_eq9_series_and_threshold(orc):
+    """Sect. 3.1, readings Q37 / Q38.  (i) Eq. 9's 1 - e^-tau as the oracle evaluates it (series to
+    tau^5) against -expm1(-tau) below the threshold; (ii) which cells are tallied: a slab of cells just below and one
+    just above tau_max = sqrt(3) h rho max_nu(kabs + ksca) = 10^-2, and one far above: only the first is tallied, with
+    every traversal's (1 - e^-tau_abs), which lies between the linear tally and the linear tally (1 - tau_max/2)."""
+    for tau in (1e-9, 1e-6, 1e-4, 3e-3, 9.99e-3):
+        assert abs(orc.eq9_value(tau) / -math.expm1(-tau) - 1) < 1e-12
+    n = 12
+    w = W.uniform_cube(n, tau_edge_V=1.0, albedo=0.4, g_const=0.3, n_nu=12, slope=1.0)
+    kmax = float((w.kappa_abs + w.kappa_sca).max())
+    rho_at = lambda tau: tau / (math.sqrt(3.0) * w.cell_size_cm * kmax)
+    rho = np.zeros((n, n, n), np.float32)
+    rho[:, :, 0:4] = rho_at(0.99e-2)
+    rho[:, :, 4:8] = rho_at(1.01e-2)
+    rho[:, :, 8:12] = rho_at(3.0)
+    w.rho = rho
+    N = 60_000
+    lin = orc.Oracle.from_workload(w)
+    lin.run(N, seed=230, absorb_and_stop=True, n_threads=NTH)
+    hyb = orc.Oracle.from_workload(w)
+    r = hyb.run(N, seed=230, absorb_and_stop=True, lucy_hybrid=True, n_threads=NTH)
+    Ll = lin.read_raw()["lucy_fx"].reshape(n, n, n).astype(np.float64)
+    Lh = hyb.read_raw()["lucy_fx"].reshape(n, n, n).astype(np.float64)
+    assert np.array_equal(lin.read_raw()["k"], hyb.read_raw()["k"])          # the estimator does not touch the transport
+    assert not Lh[:, :, 4:].any() and (Lh[:, :, 0:4] > 0).all()
+    ratio = Lh[:, :, 0:4] / Ll[:, :, 0:4]
+    assert (ratio < 1.0).all() and (ratio > 1.0 - 0.5e-2).all()
+    assert r["lucy_adds"] > 0
+
+
+def test_p23_hybrid_temperatures(orc):
+    """Reading Q39 against radiative balance (the closed form of P8): in an optically thin sphere every cell is below
+    the threshold, so in hybrid mode the Eq. 9 energy gives the output temperature AND the frozen per-epoch index
+    B&W re-emits from: both follow T = T* (R*/2r)^(2/(4+beta)), although hardly any packet is ever absorbed there
+    (the count-based index of those cells would sit at the bottom of the T grid).  A sphere 10^5 times denser next to
+    it in the same run is above the threshold: no tally, temperature from its counts."""
+    beta, Tstar, n, N = 1.0, 1500.0, 24, 600_000
+    lam = W.wavelength_grid_um(160, 0.2, 1e5)
+    nu = W.nu_from_lambda_um(lam)
+    kabs = 100.0 * (nu / nu[-1]) ** beta
+    h = W.AU_CM
+    x = (np.arange(n) + 0.5) - n / 2
+    r = np.sqrt(x[None, None, :] ** 2 + x[None, :, None] ** 2 + x[:, None, None] ** 2)
+    rho0 = 1e-3 / (kabs.max() * n / 2 * h)
+    rho = np.where(r < n / 2, rho0, 0.0).astype(np.float32)
+    L = W.LSUN_ERG_S
+    c = n / 2 * h
+    Tg = W.temperature_grid(1000, 2.0, 2000.0)
+    o = orc.Oracle(n, n, n, h, rho, np.zeros(n ** 3, np.uint8), 1, nu, kabs[None], np.zeros((1, len(nu))),
+                   np.zeros((1, len(nu))), Tg, L, Tstar, None, [c, c, c], [0.0, 1.0])
+    res = o.run(N, seed=8, lucy_hybrid=True, n_threads=NTH)
+    assert res["absorptions"] < 0.01 * N
+    T = lib_T = o.read(T_from_lucy=2)["T"].reshape(n, n, n).astype(np.float64)
+    tidx = o.read_raw()["tidx"].reshape(n, n, n)
+    Rstar = math.sqrt(L / (4 * math.pi * SIGMA_SB * Tstar ** 4))
+    for r_lo in (4.0, 7.0, 10.0):
+        sel = (r >= r_lo) & (r < r_lo + 1.0)
+        T_exp = Tstar * (Rstar / (2 * r[sel] * h)) ** (2 / (4 + beta))
+        assert abs((T[sel] / T_exp).mean() - 1) < 0.01, r_lo
+        # the index the LAST epoch re-emitted from (midpoint prediction of the tally at ~98 % of the run): first grid T above
+        assert abs((Tg[tidx[sel]] / T_exp).mean() - 1) < 0.02, r_lo
+    assert (o.read_raw()["k"].reshape(n, n, n)[(r >= 7.0) & (r < 8.0)] == 0).mean() > 0.9
+    # a thick cell in the same kind of run: no tally, T from counts
+    rho2 = rho.copy()
+    rho2[n // 2 - 2:n // 2 + 2, n // 2 - 2:n // 2 + 2, n // 2 - 2:n // 2 + 2] = rho0 * 1e5
+    o2 = orc.Oracle(n, n, n, h, rho2, np.zeros(n ** 3, np.uint8), 1, nu, kabs[None], np.zeros((1, len(nu))),
+                    np.zeros((1, len(nu))), Tg, L, Tstar, None, [c, c, c], [0.0, 1.0])
+    o2.run(60_000, seed=9, lucy_hybrid=True, n_threads=NTH)
+    core = (slice(n // 2 - 2, n // 2 + 2),) * 3
+    assert not o2.read_raw()["lucy_fx"].reshape(n, n, n)[core].any()
+    Th, Tc = o2.read(T_from_lucy=2)["T"].reshape(n, n, n)[core], o2.read(T_from_lucy=False)["T"].reshape(n, n, n)[core]
+    assert np.array_equal(Th, Tc) and (Tc > 0).all()
+    # ... and a frozen-T sweep in hybrid mode takes the core's index from its counts, the thin cells' from their tally
+    Tl = o2.read(T_from_lucy=2)["T"].reshape(n, n, n).astype(np.float64)
+    o2.run(20_000, seed=11, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, lucy_hybrid=True, reset=False, n_threads=NTH)
+    t2 = o2.read_raw()["tidx"].reshape(n, n, n)
+    assert (t2[core] > 0).all() and np.abs(Tg[t2[core]] / Tc - 1).max() < 0.02
+    shell = (r >= 7.0) & (r < 8.0)
+    assert abs((Tg[t2[shell]] / Tl[shell]).mean() - 1) < 0.02
