@@ -94,6 +94,12 @@ typedef struct {
                                   packets is allocated with cudaMalloc (88 bytes per packet of an epoch). */
     int32_t no_hot_cells;      /* launch tuning: 1 = do not keep per-CTA copies of the tallies of the cells around the
                                   source (default 0: kept; the sums are integers, so results do not depend on it) */
+    int32_t lucy_hybrid;       /* 1 = the thresholded estimator of Sect. 3.1 (readings Q37-Q39): only cells whose
+                                  maximal optical depth sqrt(3) h rho max_nu(kabs+ksca) is below 10^-2 are tallied, with Eq. 9's
+                                  (1 - e^-tau_abs) per traversal, and their temperature (per-epoch index, sweeps, the T_lucy of
+                                  mcrt_read) comes from that energy; all other cells' from their counts.  Default 0: the linear
+                                  path-length tally in every cell.  Not with mixtures, live B&W or partitioned runs; a run that
+                                  continues stored tallies (reset_tallies = 0, sweeps) must use the estimator that made them */
 } mcrt_run_opts;
 
 /* Counters of the runs since the last reset (all exact integers). */

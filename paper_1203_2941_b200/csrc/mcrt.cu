@@ -129,6 +129,9 @@ struct mcrt_ctx {
     long long *lfx1 = nullptr;
     unsigned long long *kcnt1 = nullptr, *kprev1 = nullptr;
     uint16_t *tidx1 = nullptr;
+    // thresholded Lucy estimator (mcrt_run_opts.lucy_hybrid; Sect. 3.1)
+    bool hybrid = false;                           // the stored tallies were made with it
+    double *d_kmax_diag = nullptr;                 // [ns] sqrt(3) h max_nu (kabs + ksca) (cudaMalloc)
     // run in progress (mcrt_run_begin .. mcrt_run_end)
     struct Run {
         bool active = false;
@@ -495,6 +498,9 @@ struct TransportParams {
     const double *__restrict__ kabs1_fx;       // [ns][nf] f_1 kabs_1 h 2^FX (0 for a one-component mixture)
     const double2 *__restrict__ mx_thr;        // [ns][nf] {S0, A0}: thresholds of the event uniform
     const int *__restrict__ mx_mat;            // [ns][2] material of each component
+    // thresholded Lucy estimator (Sect. 3.1, readings Q37 / Q38): NULL = the linear tally in every cell
+    const double *__restrict__ kmax_diag;      // [ns] sqrt(3) h max_nu (kabs + ksca): a cell is tallied if rho * this < 10^-2
+    double two_fx, inv_two_fx;                 // 2^FX, 2^-FX
     uint32_t seed_lo, seed_hi, pass;
 };
 
@@ -536,6 +542,14 @@ __device__ __forceinline__ unsigned long long lucy_round(double x)
 __device__ __forceinline__ void lucy_add_raw(long long *__restrict__ lfx, uint32_t cidx, unsigned long long q)
 {
     asm volatile("red.global.add.u64 [%0], %1;" ::"l"(lfx + (size_t)kCS * cidx), "l"(q) : "memory");
+}
+// Eq. 9, per traversal of a cell below the threshold of Sect. 3.1: (1 - e^-tau) 2^FX from the linear
+// tally value x = tau 2^FX; 1 - e^-tau is DEFINED as its series to tau^5 in this order (reading Q38; tau < 10^-2)
+constexpr double kThinTau = 1e-2;
+__device__ __forceinline__ double eq9_fx(double x, double two_fx, double inv_two_fx)
+{
+    const double tau = x * inv_two_fx;
+    return (tau * (1.0 - tau * (0.5 - tau * (1.0 / 6.0 - tau * (1.0 / 24.0 - tau * (1.0 / 120.0)))))) * two_fx;
 }
 __device__ __forceinline__ void lucy_add(long long *__restrict__ lfx, uint32_t cidx, double x)
 {
@@ -800,6 +814,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const double2 *kq_row = s_kk;                       // s_kk + j
             const double *k1_row = P.kabs1_fx;                  // mixtures: the second component's kabs_fx at frequency j
             double kq1 = 0.0;
+            double kmd = 0.0;                                   // thresholded estimator: kmax_diag of species kq_sp
             // words of cells n .. n+kDepth-1, in registers
             unsigned long long cwr[kDepth];
             unsigned long long wstop = 0ull;             // cell word of the cell this lane's packet stopped in (MCRT_STOP_RELOAD)
@@ -909,6 +924,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq_row = s_kk + j;
                         kq_sp = 0u; kq = kq_row[0];
                         if (XTRA && P.lfx1) { k1_row = P.kabs1_fx + j; kq1 = k1_row[0]; }
+                        if (XTRA && P.kmax_diag) kmd = P.kmax_diag[0];
                         state = ST_FLY;
                     }
                     mFly.remove(take, slot);
@@ -966,6 +982,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         MCRT_CHK(!fly || kq_sp < (uint32_t)P.ns, "walk: species of the cell word");                         \
                         kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
                         if (XTRA && P.lfx1) kq1 = k1_row[fly ? kq_sp * nf_r : 0u];   /* second component of a mixture */     \
+                        if (XTRA && P.kmax_diag) kmd = P.kmax_diag[fly ? kq_sp : 0u]; /* thresholded estimator */             \
                     }                                                                                                       \
                     const double dtau = kq.x * rho_c * ds;            /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */ \
                     const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
@@ -982,16 +999,18 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                                      : "+l"(wstop) : "l"(cellw_r + kCS * ciA), "r"((uint32_t)(fly && stop)));               \
                     /* S5: tally of a traversed dusty cell (a vacuum cell has nothing to add) */                           \
                     {                                                                                                       \
-                        const unsigned long long q = lucy_round(kq.y * rho_c * ds);                                         \
+                        const bool hyb = XTRA && P.kmax_diag;       /* Sect. 3.1: Eq. 9 in cells below the threshold only */ \
+                        const double xq = kq.y * rho_c * ds;                                                                \
+                        const unsigned long long q = lucy_round(hyb ? eq9_fx(xq, P.two_fx, P.inv_two_fx) : xq);             \
                         const bool go = fly && !stop;                                                                       \
                         const uint32_t dusty = (go && __double2hiint(rho_c) != 0) ? 1u : 0u;                                \
                         const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;   /* tallied in the CTA's own copy */ \
-                        const uint32_t cold = (dusty && hid == 0u) ? 1u : 0u;                                               \
+                        const uint32_t cold = (dusty && hid == 0u && !(hyb && !(rho_c * kmd < kThinTau))) ? 1u : 0u;        \
                         MCRT_CHK(!dusty || ciA < P.ncp, "walk: storage index of the tallied cell");                         \
                         MCRT_CHK(hid <= (uint32_t)P.n_hot, "walk: hot-cell number");                                        \
                         MCRT_CHK(!(fly && stop) || (uint32_t)slot < (uint32_t)kSlots, "walk: slot of the stopped packet");   \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
-                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"(HOT ? cold : dusty) : "memory");                 \
+                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA) ? cold : dusty) : "memory");       \
                         if (XTRA && P.lfx1) {       /* the second component's tally (reading Q36) */                         \
                             const unsigned long long q1 = lucy_round(kq1 * rho_c * ds);                                     \
                             if (dusty && kq1 != 0.0) lucy_add_raw(P.lfx1, ciA, q1);                                         \
@@ -1226,7 +1245,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double sint = tau / kk;
                     const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;
                     if (hid) hot_add(s_hot, hid, lucy_round(kq.y * rho_c * sint));
-                    else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
+                    else if (XTRA && P.kmax_diag) {           // Sect. 3.1: Eq. 9, cells below the threshold only
+                        if (rho_c * P.kmax_diag[cw_species(cw)] < kThinTau)
+                            lucy_add(P.lfx, cidx, eq9_fx(kq.y * rho_c * sint, P.two_fx, P.inv_two_fx));
+                    } else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
                     // mixtures (NEXT-3, readings Q34-Q36): the second component's tally; which component interacts
                     double2 thr = make_double2(2.0, 2.0);      // {S0, A0}; a uniform is < 2: one component = always component 0
                     if (XTRA && P.lfx1) {
@@ -1532,6 +1554,50 @@ __global__ void __launch_bounds__(256) k_mix_update(unsigned long long *__restri
     if (ovf && !sweep) counters[CNT_OVERFLOW] = 1ull;
 }
 
+// The two updates under the thresholded estimator of Sect. 3.1 (reading Q39): a cell below the threshold takes its
+// temperature from its Eq. 9 energy (the same midpoint prediction, on the tally; k_prev keeps the tally there), every
+// other cell from its count as above.  sweep = 0: epoch rule (S11), 1: frozen-T sweep (S12, zeroes the tallies).
+__global__ void __launch_bounds__(256) k_hybrid_update(unsigned long long *__restrict__ cellw, unsigned long long *__restrict__ kcnt,
+                                                       unsigned long long *__restrict__ kprev, long long *__restrict__ lfx,
+                                                       const double *__restrict__ J, const double *__restrict__ kmax_diag, int nT,
+                                                       int ns, size_t ncp, int sweep, int first_epoch, double ratio, double inv_fx,
+                                                       double cellfac, unsigned long long *__restrict__ counters, uint32_t tmask)
+{
+    extern __shared__ double s_J[];
+    for (int i = threadIdx.x; i < ns * nT; i += blockDim.x) s_J[i] = J[i];
+    __syncthreads();
+    if (blockIdx.x == 0 && threadIdx.x == 0) { counters[CNT_NEXT] = 0ull; if (!sweep) counters[CNT_CARRY] = 0ull; }
+    bool ovf = false;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < ncp; i += (size_t)gridDim.x * blockDim.x) {
+        const unsigned long long cw = cellw[kCS * i];
+        const double rho_c = cw_rho(cw);
+        const unsigned long long kc = kcnt[i];
+        const long long v = lfx[kCS * i];
+        uint32_t m = 0u;
+        bool thin = false;
+        if (cw_dusty(cw)) {
+            thin = rho_c * kmax_diag[cw_species(cw)] < kThinTau;
+            double e;
+            if (thin) {
+                const double E = (double)v * inv_fx, Ep = (double)(long long)kprev[i] * inv_fx;
+                e = (sweep || first_epoch) ? E : E + 0.5 * (E - Ep) * ratio;
+            } else if (sweep) e = (double)kc;
+            else if (first_epoch) e = (double)kc + 1.0;
+            else {
+                const double pred = 0.5 * (double)(kc - kprev[i]) * ratio;
+                e = (double)kc + ((pred > 1.0) ? pred : 1.0);
+            }
+            m = (uint32_t)t_index(s_J + cw_species(cw) * nT, nT, e * cellfac / rho_c);
+            ovf |= (v > (1ll << 62)) || (v < -(1ll << 62));
+        }
+        if (sweep) { kcnt[i] = 0ull; kprev[i] = 0ull; lfx[kCS * i] = 0ll; }
+        else kprev[i] = thin ? (unsigned long long)v : kc;
+        const uint32_t lo = (uint32_t)cw, nlo = (lo & ~(tmask << 8)) | (m << 8);
+        if (nlo != lo && cw_dusty(cw)) reinterpret_cast<uint32_t *>(cellw + kCS * i)[0] = nlo;
+    }
+    if (ovf && !sweep) counters[CNT_OVERFLOW] = 1ull;
+}
+
 // Partitioned runs: between epochs a part's absorption counts are exchanged as this epoch's own
 // increments, k - k_prev (k_prev = the global counts at the start of the epoch), and restored afterwards.
 __global__ void __launch_bounds__(256) k_count_delta(unsigned long long *__restrict__ kcnt, const unsigned long long *__restrict__ kprev,
@@ -1698,7 +1764,7 @@ __global__ void k_grow_boxes(const uint32_t *__restrict__ mask, const int *__res
     }
 }
 
-enum : int { G_K = 0, G_LFX = 1, G_TIDX = 2, G_ECOUNT = 3, G_ELUCY = 4, G_TCOUNT = 5, G_TLUCY = 6 };
+enum : int { G_K = 0, G_LFX = 1, G_TIDX = 2, G_ECOUNT = 3, G_ELUCY = 4, G_TCOUNT = 5, G_TLUCY = 6, G_THYBRID = 7 };
 
 __device__ __forceinline__ double T_of_x(const double *J, const double *Tg, int nT, double x)
 {
@@ -1720,7 +1786,7 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
                          const double *__restrict__ J, const double *__restrict__ Tg, int nT, int nx, int ny, int nz,
                          int px, int pxy, double xi, double inv_fx, double cellfac, uint32_t tmask,
                          const int *__restrict__ mx_mat, const double *__restrict__ mx_frac, int comp,
-                         const uint16_t *__restrict__ tidx1)
+                         const uint16_t *__restrict__ tidx1, const double *__restrict__ kmax_diag)
 {
     // (mixtures, NEXT-3: kcnt / lfx are those of component `comp`, whose material and mass fraction enter Eq. 4)
     const size_t nc = (size_t)nx * ny * nz;
@@ -1738,7 +1804,9 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
             const double rho_c = cw_rho(cw);
             float T = 0.0f;
             if (cw_dusty(cw)) {
-                const double e = (what == G_TLUCY) ? (double)lfx[bs] * inv_fx : (double)kcnt[b];
+                double e = (what == G_TLUCY) ? (double)lfx[bs] * inv_fx : (double)kcnt[b];
+                // Sect. 3.1 (reading Q39): the Eq. 9 energy below the threshold, the count above
+                if (what == G_THYBRID) e = (rho_c * kmax_diag[cw_species(cw)] < kThinTau) ? (double)lfx[bs] * inv_fx : (double)kcnt[b];
                 if (!mx_mat) T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / rho_c);
                 else {
                     const int m = mx_mat[2 * cw_species(cw) + comp];
@@ -2527,7 +2595,7 @@ static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, in
             if (smem_carveout(transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, t, record, 0)) <= 164 * 1024) { *threads = t; break; }
     const size_t base = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0);
     // ... and as many hot cells as the carve-out these need leaves room for (live B&W needs every count in global memory)
-    int nh = (c->mix || (o && (o->no_hot_cells || o->mode == MCRT_MODE_LIVE_BW))) ? 0 : (int)c->hot_cand.size();
+    int nh = (c->mix || (o && (o->no_hot_cells || o->lucy_hybrid || o->mode == MCRT_MODE_LIVE_BW))) ? 0 : (int)c->hot_cand.size();
     const size_t cap = smem_carveout(base) - kSmemOverhead;
     while (nh > 0 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh) > cap) --nh;
     if (nh < 8) nh = 0;
@@ -2614,6 +2682,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
         P.lfx1 = c->lfx1; P.kcnt1 = c->kcnt1; P.tidx1 = c->tidx1; P.kabs1_fx = c->d_kabs1_fx;
         P.mx_thr = reinterpret_cast<const double2 *>(c->d_mx_thr); P.mx_mat = c->d_mx_mat;
     }
+    if (c->run.o.lucy_hybrid) { P.kmax_diag = c->d_kmax_diag; P.two_fx = ldexp(1.0, c->fx); P.inv_two_fx = ldexp(1.0, -c->fx); }
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base; P.dig_n = c->dig_n;
     P.nx = c->nx; P.ny = c->ny; P.nz = c->nz; P.ns = c->ns; P.nf = c->nf; P.nT = c->nT; P.ndir = c->ndir;
@@ -2734,13 +2803,26 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
     if (c->mix && (o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
         return fail(c, MCRT_EINVAL, "dust mixtures are not available in live B&W or partitioned runs");
+    if (o.lucy_hybrid && (c->mix || o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
+        return fail(c, MCRT_EINVAL, "lucy_hybrid is not available with mixtures, in live B&W or partitioned runs");
+    if ((o.mode == MCRT_MODE_FROZEN_T_SWEEP || !o.reset_tallies) && c->last_n != 0 && c->hybrid != (o.lucy_hybrid != 0))
+        return fail(c, MCRT_ESTATE, "the stored tallies were made with the other Lucy estimator (lucy_hybrid)");
     int rc = ensure_histograms(c);
     if (rc) return rc;
+    if (o.lucy_hybrid && !c->d_kmax_diag) {
+        std::vector<double> km(c->ns, 0.0);     // reading Q37: the diagonal at the frequency of the largest extinction
+        for (int s_ = 0; s_ < c->ns; ++s_) {
+            for (int j = 0; j < c->nf; ++j) km[s_] = fmax(km[s_], c->kabs[(size_t)s_ * c->nf + j] + c->ksca[(size_t)s_ * c->nf + j]);
+            km[s_] = sqrt(3.0) * c->h * km[s_];
+        }
+        if (cudaMalloc((void **)&c->d_kmax_diag, c->ns * 8) != cudaSuccess) return fail(c, MCRT_ENOMEM, "cudaMalloc failed");
+        CUDA_TRY(c, cudaMemcpy(c->d_kmax_diag, km.data(), c->ns * 8, cudaMemcpyHostToDevice));
+    }
     mcrt_ctx::Run &R = c->run;
     int n_hot = 0;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
     if ((rc = apply_hot(c, n_hot))) return rc;
-    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix;
+    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid;
     R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
@@ -2784,6 +2866,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     R.prev_fx = c->fx;
     R.prev_cellfac = c->xi / (kFourPi * c->h * c->h * c->h);
     c->fx = fx; c->xi = xi;
+    c->hybrid = o.lucy_hybrid != 0;
     R.cellfac = xi / (kFourPi * c->h * c->h * c->h);             // xi / (4 pi V) of Eq. 4
     c->last_n = n_packets;
     {
@@ -2803,6 +2886,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         CUDA_TRY(c, cudaFuncSetAttribute(k_epoch_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_sweep_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
         CUDA_TRY(c, cudaFuncSetAttribute(k_mix_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
+        CUDA_TRY(c, cudaFuncSetAttribute(k_hybrid_update, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)j_smem));
     }
     R.o = o; R.n = n_packets; R.seed = seed; R.done = 0; R.Bprev = 0; R.e = 0; R.sweep = 0; R.finished = false;
     R.carry_K = (o.mode == MCRT_MODE_BW_EPOCH) ? o.carry_interactions : 0u; R.n_carry = 0;
@@ -2854,7 +2938,12 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
             P.n_carry_in = (uint32_t)R.n_carry; P.carry_K = R.carry_K;
         }
         mark(c, timing);
-        if (c->mix)
+        if (o.lucy_hybrid)
+            k_hybrid_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->d_kmax_diag, c->nT,
+                                                              c->ns, c->ncp, 0, R.e == 0,
+                                                              (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev,
+                                                              ldexp(1.0, -c->fx), R.cellfac, c->counters, c->tidx_mask);
+        else if (c->mix)
             k_mix_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, mix_arrays(c), c->d_J, c->nT, c->ns, c->ncp, 0, R.e == 0,
                                                            (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev, 0, 0.0,
                                                            R.cellfac, c->counters, c->tidx_mask);
@@ -2890,7 +2979,11 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         P.cdf = c->d_cdfB;
         // temperatures of the previous pass (its own packet energy and fixed-point scale), then zero and re-run all N packets
         mark(c, timing);
-        if (c->mix)
+        if (o.lucy_hybrid)
+            k_hybrid_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->d_kmax_diag, c->nT,
+                                                              c->ns, c->ncp, 1, 0, 1.0, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
+                                                              sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
+        else if (c->mix)
             k_mix_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, mix_arrays(c), c->d_J, c->nT, c->ns, c->ncp, 1, 0, 1.0,
                                                            o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
                                                            sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
@@ -3054,7 +3147,7 @@ static int gather_out(mcrt_ctx *c, int what, void *dst, size_t elem, mcrt_mem wh
     k_gather<<<stream_grid(c->nc), 256, 0, c->stream>>>(what, dev, c->cellw, comp ? c->kcnt1 : c->kabs_cnt, comp ? c->lfx1 : c->lfx,
                                                        c->d_J, c->d_Tg, c->nT, c->nx, c->ny, c->nz, c->px, c->pxy, c->xi,
                                                        ldexp(1.0, -c->fx), cellfac, c->tidx_mask, c->mix ? c->d_mx_mat : nullptr,
-                                                       c->d_mx_frac, comp, c->tidx1);
+                                                       c->d_mx_frac, comp, c->tidx1, c->d_kmax_diag);
     CUDA_TRY(c, cudaGetLastError());
     if (where == MCRT_HOST) {
         CUDA_TRY(c, cudaMemcpyAsync(dst, dev, c->nc * elem, cudaMemcpyDeviceToHost, c->stream));
@@ -3082,7 +3175,7 @@ int mcrt_read(mcrt_ctx *c, double *E_abs_count, double *E_abs_lucy, float *T_cou
     if ((rc = gather_out(c, G_ECOUNT, E_abs_count, 8, where))) return rc;
     if ((rc = gather_out(c, G_ELUCY, E_abs_lucy, 8, where))) return rc;
     if ((rc = gather_out(c, G_TCOUNT, T_count, 4, where))) return rc;
-    if ((rc = gather_out(c, G_TLUCY, T_lucy, 4, where))) return rc;
+    if ((rc = gather_out(c, c->hybrid ? G_THYBRID : G_TLUCY, T_lucy, 4, where))) return rc;
     if (SED) {
         const int n = c->ndir * c->nf;
         double *dev = (where == MCRT_DEVICE) ? SED : c->sed_stage;
@@ -3324,7 +3417,7 @@ void mcrt_destroy(mcrt_ctx *c)
     if (c->sca_ev) cudaFree(c->sca_ev);
     if (c->img_buf) cudaFree(c->img_buf);
     for (void *p : {(void *)c->d_mx_ncomp, (void *)c->d_mx_mat, (void *)c->d_mx_frac, (void *)c->d_mx_thr, (void *)c->d_kabs1_fx,
-                    (void *)c->lfx1, (void *)c->kcnt1, (void *)c->kprev1, (void *)c->tidx1})
+                    (void *)c->lfx1, (void *)c->kcnt1, (void *)c->kprev1, (void *)c->tidx1, (void *)c->d_kmax_diag})
         if (p) cudaFree(p);
     delete c;
 }

@@ -723,3 +723,40 @@ def test_parity_dust_mixtures(B, orc, case):
         for key in ("k", "lucy_fx", "tidx"):
             assert np.array_equal(o1[key], g1[key]), key
     c.close()
+
+
+def test_parity_thresholded_lucy_estimator(B, orc):
+    """NEXT-4, Sect. 3.1 / Eq. 9 (readings Q37-Q39; oracle pins P23): only cells below the optical
+    depth threshold are tallied, with (1 - e^-tau) per traversal, and take their temperature from that energy.  A
+    sphere whose cells' densities are spread over 7.5 decades (a good part of them below the threshold), B&W epochs and two
+    sweeps: digests, counts, tallies, temperature indices bit-equal to the oracle; the hybrid temperature output."""
+    w = W.sphere32(tau_V=30.0, n=16)
+    rng = np.random.default_rng(5)
+    w.rho = (w.rho * 10.0 ** rng.uniform(-7.0, 0.5, w.rho.shape)).astype(np.float32)
+    N = 60_000
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 91, n_threads=NTH, digests=True, lucy_hybrid=True)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 91, record_digests=1, lucy_hybrid=1)
+    for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+        assert ro[key] == rg[key], key
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    dusty = w.rho.reshape(-1) > 0
+    tallied = raw_g["lucy_fx"] != 0
+    assert 0.1 < tallied[dusty].mean() < 0.9                 # both kinds of cells are there
+    assert raw_g["k"][dusty & ~tallied].sum() > 1000           # the untallied ones are the thick ones
+    assert np.allclose(o.read(T_from_lucy=2)["T"], c.read()["T_lucy"], rtol=2e-6, atol=0.0)
+    plain = orc.Oracle.from_workload(w)
+    rp = plain.run(N, 91, n_threads=NTH, digests=True)
+    assert not np.array_equal(rp["digests"]["hash"], ro["digests"]["hash"])   # thin cells re-emit at another temperature
+    o.run(N, 92, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=2, lucy_hybrid=True, reset=False, n_threads=NTH, digests=True)
+    c.run(N, 92, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=2, lucy_hybrid=1, record_digests=1)
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    with pytest.raises(Exception):
+        c.run(N, 93, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1)      # the other estimator's tallies: refused
+    c.close()
