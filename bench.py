@@ -57,6 +57,7 @@ def parse():
                     help="N > 1: how the ranks' tallies are summed (auto = peer memory, NCCL if that cannot be set up)")
     ap.add_argument("--carry", type=int, default=0, help="experiment: carry packets over epoch boundaries after this many interactions in one epoch (0 = off, the configuration's definition)")
     ap.add_argument("--no-hot", action="store_true", help="experiment: no per-CTA copies of the tallies of the cells around the source")
+    ap.add_argument("--lucy-hybrid", action="store_true", help="experiment: the thresholded Lucy estimator of Sect. 3.1 (only thin cells tallied)")
     ap.add_argument("--threads", type=int, default=0, help="experiment: threads per CTA of the transport kernel (0 = as many warps as fit)")
     ap.add_argument("--sweeps", type=int, default=-1, help="frozen-T sweeps after the B&W pass (-1 = the configuration's: 3 for torus512)")
     return ap.parse_args()
@@ -275,7 +276,7 @@ def run_ours(args, workload_name=None):
         counters of every pass (a sweep counts its own packets: they are read after each sweep, a 120-byte D2H copy
         inside the timed region)."""
         kw = dict(epoch_Bmax=args.bmax, time_kernels=1 if timed else 0, no_hot_cells=1 if args.no_hot else 0,
-                  block_threads=args.threads)
+                  block_threads=args.threads, lucy_hybrid=1 if args.lucy_hybrid else 0)
         out = []
         sweep_kw = dict(mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=n_sweeps, **kw)
         if args.carry and world == 1:
