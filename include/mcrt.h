@@ -321,6 +321,16 @@ int mcrt_philox_device(const uint32_t *ctr, const uint32_t *key, uint32_t *out, 
  * algorithms (reading Q28), so the tests can demand bit-equality with the oracle's. */
 int mcrt_traj_math_device(const double *z, double *ln_z, double *sin_2piz, double *cos_2piz, uint64_t n);
 
+/* The same functions through an entry point that ALLOCATES NOTHING (no cudaMalloc / cudaFree, no host allocation), for
+ * callers that cannot allocate: tight loops, harnesses that forbid it.  Host pointers as above; n <= MCRT_STATIC_MAX_N,
+ * beyond that MCRT_EINVAL with a message.  The device copies of z and of the three results live in a static device
+ * array of 4 x MCRT_STATIC_MAX_N doubles (2 MiB) that every GPU which loads the library holds until the process exits
+ * and that ALL calls share: it keeps the last call's contents (nothing in it has to start at zero -- a call reads back
+ * only what it wrote), and calls that overlap on the GPU (several host threads) race on it -- serialise them.  Runs on
+ * the current device, default stream, synchronous.  Results are bit-identical to mcrt_traj_math_device. */
+#define MCRT_STATIC_MAX_N 65536
+int mcrt_traj_math_device_static(const double *z, double *ln_z, double *sin_2piz, double *cos_2piz, uint64_t n);
+
 /* Use this CUDA stream (a cudaStream_t passed as void*) for all later work of the context. */
 int mcrt_set_stream(mcrt_ctx *ctx, void *cuda_stream);
 

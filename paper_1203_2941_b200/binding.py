@@ -25,7 +25,7 @@ EXPORTS = [
     "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
     "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_epoch_schedule", "mcrt_part_slice",
     "mcrt_measure_read_bandwidth", "mcrt_scatter_store", "mcrt_scatter_events", "mcrt_ray_trace", "mcrt_get_stats", "mcrt_read", "mcrt_read_component", "mcrt_read_raw", "mcrt_read_tables",
-    "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
+    "mcrt_philox_device", "mcrt_traj_math_device", "mcrt_traj_math_device_static", "mcrt_set_stream", "mcrt_launch_config", "mcrt_last_error", "mcrt_version",
     "mcrt_destroy",
 ]
 
@@ -114,6 +114,7 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_read_tables.argtypes = [vp] + [vp] * 6
     L.mcrt_philox_device.argtypes = [vp, vp, vp, u64]
     L.mcrt_traj_math_device.argtypes = [vp, vp, vp, vp, u64]
+    L.mcrt_traj_math_device_static.argtypes = [vp, vp, vp, vp, u64]
     L.mcrt_set_stream.argtypes = [vp, vp]
     L.mcrt_launch_config.argtypes = [vp, C.POINTER(i), C.POINTER(i), C.POINTER(C.c_size_t)]
     L.mcrt_last_error.argtypes = [vp]
@@ -333,6 +334,17 @@ def mcrt_traj_math_device(z):
     z = np.ascontiguousarray(z, np.float64).reshape(-1)
     ln, s, c = np.zeros_like(z), np.zeros_like(z), np.zeros_like(z)
     _check(load_library().mcrt_traj_math_device(_ptr(z), _ptr(ln), _ptr(s), _ptr(c), len(z)))
+    return ln, s, c
+
+
+MCRT_STATIC_MAX_N = 65536
+
+
+def mcrt_traj_math_device_static(z):
+    """mcrt_traj_math_device through the entry point that allocates nothing on the device (n <= MCRT_STATIC_MAX_N)."""
+    z = np.ascontiguousarray(z, np.float64).reshape(-1)
+    ln, s, c = np.zeros_like(z), np.zeros_like(z), np.zeros_like(z)
+    _check(load_library().mcrt_traj_math_device_static(_ptr(z), _ptr(ln), _ptr(s), _ptr(c), len(z)))
     return ln, s, c
 
 

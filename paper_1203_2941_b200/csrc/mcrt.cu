@@ -16,6 +16,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -1983,6 +1984,25 @@ __global__ void k_traj_math_test(const double *__restrict__ z, double *__restric
     }
 }
 
+// The allocation-free variant of k_traj_math_test (mcrt_traj_math_device_static): its scratch -- the device copy of the
+// input and the three output arrays -- lives in a file-scope device array of fixed size, 4 x 65536 doubles = 2 MiB,
+// which every GPU that loads the library holds until the process exits.  All calls share it.
+constexpr uint64_t kStaticMaxN = 65536;
+constexpr int kStaticMaxDevices = 64;
+static __device__ __align__(256) double g_static_scratch[4 * kStaticMaxN];
+static std::atomic<double *> g_static_scratch_ptr[kStaticMaxDevices];   // its device address, per device ordinal (0 = not asked yet)
+
+__global__ void k_traj_math_static(const double *__restrict__ z, double *__restrict__ ln_z, double *__restrict__ sn,
+                                   double *__restrict__ cs, unsigned long long n)
+{
+    const unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) {
+        double s, c;
+        traj_sincos_turns(z[i], s, c);
+        ln_z[i] = traj_log(z[i]); sn[i] = s; cs[i] = c;
+    }
+}
+
 __global__ void k_philox_test(const uint32_t *__restrict__ ctr, const uint32_t *__restrict__ key, uint32_t *__restrict__ out,
                               unsigned long long n)
 {
@@ -3403,6 +3423,38 @@ int mcrt_traj_math_device(const double *z, double *ln_z, double *sin_2piz, doubl
     cudaFree(d);
     if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
     for (uint64_t i = 0; i < n; ++i) { ln_z[i] = h[3 * i]; sin_2piz[i] = h[3 * i + 1]; cos_2piz[i] = h[3 * i + 2]; }
+    return MCRT_OK;
+}
+
+int mcrt_traj_math_device_static(const double *z, double *ln_z, double *sin_2piz, double *cos_2piz, uint64_t n)
+{
+    if (!z || !ln_z || !sin_2piz || !cos_2piz || n == 0) return MCRT_EINVAL;
+    if (n > kStaticMaxN)
+        return fail(nullptr, MCRT_EINVAL, "mcrt_traj_math_device_static: n exceeds MCRT_STATIC_MAX_N = " + std::to_string(kStaticMaxN) +
+                                              " (the static device scratch holds no more; use mcrt_traj_math_device)");
+    // The array's name is a host-side stand-in here: its device address comes from cudaGetSymbolAddress, once per
+    // device, with that device current.
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
+    if (dev < 0 || dev >= kStaticMaxDevices) return fail(nullptr, MCRT_EINVAL, "mcrt_traj_math_device_static: device ordinal out of range");
+    double *d = g_static_scratch_ptr[dev].load(std::memory_order_acquire);
+    if (!d) {
+        e = cudaGetSymbolAddress((void **)&d, g_static_scratch);
+        if (e != cudaSuccess || !d) return fail(nullptr, MCRT_ECUDA, std::string("cudaGetSymbolAddress(g_static_scratch): ") + cudaGetErrorString(e));
+        g_static_scratch_ptr[dev].store(d, std::memory_order_release);
+    }
+    // layout: z | ln z | sin | cos, kStaticMaxN doubles each.  Nothing has to start at zero: every element read back
+    // below is written by this call's copy or kernel; what an earlier call left beyond n is never read.
+    e = cudaMemcpy(d, z, n * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        k_traj_math_static<<<(unsigned)((n + 255) / 256), 256>>>(d, d + kStaticMaxN, d + 2 * kStaticMaxN, d + 3 * kStaticMaxN, n);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpy(ln_z, d + kStaticMaxN, n * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(sin_2piz, d + 2 * kStaticMaxN, n * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(cos_2piz, d + 3 * kStaticMaxN, n * sizeof(double), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return fail(nullptr, MCRT_ECUDA, cudaGetErrorString(e));
     return MCRT_OK;
 }
 
