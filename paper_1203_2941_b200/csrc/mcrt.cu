@@ -617,7 +617,28 @@ enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, 
 #else
 enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, F_PID, F_HASH };
 #endif
+// MCRT_PACK_STOP = 1: what a stopping packet stores in the walk sits in adjacent words of its slot -- (t, tau) as one
+// 16-byte pair, (crossings, cell) as one 8-byte pair -- so that a stop is three shared-memory stores instead of five
+#ifndef MCRT_L2_HINT
+#define MCRT_L2_HINT 0              // 1: the walk's cell-word loads carry an L2 evict_last policy; 2: and its tally REDs evict_first
+#endif
+#ifndef MCRT_PF
+#define MCRT_PF 0                   // > 0: the walk prefetches into L2 a guessed cell this many iterations (of kDepth cells) ahead
+#endif
+#ifndef MCRT_VAC_SPECIES
+#define MCRT_VAC_SPECIES 0          // 1: vacuum cells inside dusty bricks take the species byte of the nearest dusty cell (k_vac_species)
+#endif
+#ifndef MCRT_VAC_KEEP
+#define MCRT_VAC_KEEP 0             // 1: a vacuum cell does not reload the walk's cached opacities (its species byte is irrelevant)
+#endif
+#ifndef MCRT_PACK_STOP
+#define MCRT_PACK_STOP 0
+#endif
+#if MCRT_PACK_STOP
+enum : int { U_DK = 0, U_NCROSS, U_W0, U_NSCA, U_NABS, U_W1 };   // DK = draw counter | kind << 30
+#else
 enum : int { U_DK = 0, U_NCROSS, U_NSCA, U_NABS, U_W0, U_W1 };   // DK = draw counter | kind << 30
+#endif
 enum : uint32_t { K_EMIT = 0u, K_INTERACT = 1u, K_ESCAPED = 2u };
 // cell coordinates packed in 32 bits: x, y < 2048, z < 1024
 __device__ __forceinline__ uint32_t pack_xyz(int x, int y, int z) { return (uint32_t)x | ((uint32_t)y << 11) | ((uint32_t)z << 22); }
@@ -775,8 +796,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     const int nf = P.nf, bsh = P.bsh, nbx = P.nbx, nby = P.nby, lpx = P.lpx, lpxy = P.lpxy;
     double *wf = s_pool + (size_t)(threadIdx.x >> 5) * kPoolF64;                  // this warp's pool, f64 fields
     uint32_t *wu = reinterpret_cast<uint32_t *>(wf + kNF64 * kSlots);             // its u32 fields
+#if MCRT_PACK_STOP
+    static_assert(F_TAU == F_T + 1 && U_W0 == U_NCROSS + 1, "the pairs stored at a stop are neighbouring fields");
+#define SF(f, s) wf[((f) == F_T || (f) == F_TAU) ? F_T * kSlots + 2 * (s) + ((f) - F_T) : (f) * kSlots + (s)]
+#define SU(f, s) wu[((f) == U_NCROSS || (f) == U_W0) ? U_NCROSS * kSlots + 2 * (s) + ((f) - U_NCROSS) : (f) * kSlots + (s)]
+#else
 #define SF(f, s) wf[(f) * kSlots + (s)]
 #define SU(f, s) wu[(f) * kSlots + (s)]
+#endif
 
     // every slot starts as "emit the next packet"
     for (int s = lane; s < kSlots; s += 32) SU(U_DK, s) = K_EMIT << 30;
@@ -829,6 +856,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const volatile unsigned long long *vpp = s_parp;
             const volatile uint32_t *vpi = s_pari;
             const unsigned long long *const cellw_r = reinterpret_cast<const unsigned long long *>(vpp[0]);
+            // L2 policies (MCRT_L2_HINT): cell words, which the walk waits for, stay in L2 longest; tally lines go first
+            unsigned long long l2_keep = 0ull, l2_stream = 0ull;
+            if (MCRT_L2_HINT) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(l2_keep));
+            if (MCRT_L2_HINT == 2) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(l2_stream));
             long long *const lfx_r = reinterpret_cast<long long *>(vpp[1]);
             const uint32_t px_r = vpi[5], pxy_r = vpi[6];
             const uint32_t nf_r = vpi[7];
@@ -962,6 +993,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     MCRT_CHK(!fly || gi < P.ncp, "walk: storage index of the prefetched cell");                             \
                     if (MCRT_ROT4) asm("ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];" : "=l"(WN) : "l"(cellw_r + kCS * gi));     \
                     else                                                                                                    \
+                    if (MCRT_L2_HINT)                                                                                       \
+                    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc" MCRT_CW_POLICY ".L2::cache_hint.u64 %0, [%1], %3;\n\t}" \
+                                 : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly), "l"(l2_keep));                   \
+                    else                                                                                                    \
                     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p ld.global.nc" MCRT_CW_POLICY ".u64 %0, [%1];\n\t}" \
                                  : "+l"(W) : "l"(cellw_r + kCS * gi), "r"((uint32_t)fly));                                 \
                     /* parameter of the face through which the entered cell will be left (reading Q8): the face          */ \
@@ -978,7 +1013,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     /* cell outside the grid) has rho = +inf, so dtau is +inf or (ds = 0) NaN                             */ \
                     const double ds = tnA - tprev;                                                                          \
                     const double rho_c = cw_rho(cw);                                                                        \
-                    if (cw_species(cw) != kq_sp) {   /* opacities of this species at the packet's frequency */              \
+                    /* opacities of this cell's species at the packet's frequency; a vacuum cell needs none (rho = 0  */    \
+                    /* makes every product 0 whatever kq holds), so it leaves the cached pair alone                    */    \
+                    if (cw_species(cw) != kq_sp && (!MCRT_VAC_KEEP || __double2hiint(rho_c) != 0)) {                        \
                         kq_sp = cw_species(cw);                                                                             \
                         MCRT_CHK(!fly || kq_sp < (uint32_t)P.ns, "walk: species of the cell word");                         \
                         kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
@@ -989,8 +1026,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
                     if (fly && stop) {                                                                                      \
                         state = ST_STOP;                                                                                    \
-                        SU(U_NCROSS, slot) = ncross; SU(U_W0, slot) = ciA;                                                  \
-                        SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau;                                                       \
+                        if (MCRT_PACK_STOP) {                                                                               \
+                            *reinterpret_cast<uint2 *>(&SU(U_NCROSS, slot)) = make_uint2(ncross, ciA);                      \
+                            *reinterpret_cast<double2 *>(&SF(F_T, slot)) = make_double2(tprev, tau);                        \
+                        } else {                                                                                            \
+                            SU(U_NCROSS, slot) = ncross; SU(U_W0, slot) = ciA;                                              \
+                            SF(F_T, slot) = tprev; SF(F_TAU, slot) = tau;                                                   \
+                        }                                                                                                   \
                         if (!MCRT_STOP_RELOAD) SF(F_CW, slot) = __longlong_as_double((long long)cw);                        \
                     }                                                                                                       \
                     /* the stopped packet's cell word is read again (rare; an L1 hit) instead of being kept: its register */ \
@@ -1010,6 +1052,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         MCRT_CHK(!dusty || ciA < P.ncp, "walk: storage index of the tallied cell");                         \
                         MCRT_CHK(hid <= (uint32_t)P.n_hot, "walk: hot-cell number");                                        \
                         MCRT_CHK(!(fly && stop) || (uint32_t)slot < (uint32_t)kSlots, "walk: slot of the stopped packet");   \
+                        if (MCRT_L2_HINT == 2)                                                                              \
+                        asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.L2::cache_hint.u64 [%0], %1, %3;\n\t}" \
+                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA) ? cold : dusty), "l"(l2_stream) : "memory"); \
+                        else                                                                                                \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
                                      ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA) ? cold : dusty) : "memory");       \
                         if (XTRA && P.lfx1) {       /* the second component's tally (reading Q36) */                         \
@@ -1048,8 +1094,17 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 }
 #else
                 do {
+                    const uint32_t g_before = gi;
 #pragma unroll
                     for (int i = 0; i < kDepth; ++i) WALK_STEP(cwr[i], cwr[i])
+                    if (MCRT_PF) {
+                        // A guess at where the ray will be MCRT_PF iterations on -- G's index moved on by the displacement
+                        // of this iteration, as if the next steps took the same axes -- fetched into L2 ahead of time.
+                        // Wrong guesses cost a sector of bandwidth and nothing else.
+                        const uint32_t gp = gi + (uint32_t)MCRT_PF * (gi - g_before);
+                        if (state == ST_FLY && gp < P.ncp)
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(cellw_r + kCS * gp));
+                    }
                 } while ((nnot = __popc(__ballot_sync(kFull, state != ST_FLY)), nnot - nidle < MCRT_SWAP_MIN && nnot != 32));
 #endif
 #undef WALK_STEP
@@ -1676,6 +1731,34 @@ __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__rest
     }
 }
 
+// The species byte of a vacuum cell means nothing (rho = 0 makes every product of the walk 0), but the walk reloads its
+// cached opacities whenever the byte changes.  So a vacuum cell inside a dusty brick takes the species of the nearest
+// dusty cell along the axes (fixed search order, up to kVacReach cells: deterministic; only dusty cells are read for
+// their species and those are never written): a ray that leaves a clump, crosses a gap and enters the next reloads
+// once instead of twice.  Run after k_build_mask0 (the cells of empty bricks are marker words by then and stay).
+constexpr int kVacReach = 4;
+__global__ void k_vac_species(unsigned long long *__restrict__ cellw, int nx, int ny, int nz, int px, int pxy)
+{
+    const size_t nc = (size_t)nx * ny * nz;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nc; i += (size_t)gridDim.x * blockDim.x) {
+        const int ix = (int)(i % nx), iy = (int)((i / nx) % ny), iz = (int)(i / ((size_t)nx * ny));
+        const size_t b = lin_index(ix, iy, iz, px, pxy);
+        const unsigned long long cw = cellw[kCS * b];
+        if ((cw >> 32) != 0ull) continue;                    // dusty or marker
+        const int step[6] = {-1, 1, -px, px, -pxy, pxy};
+        const int room[6] = {ix, nx - 1 - ix, iy, ny - 1 - iy, iz, nz - 1 - iz};
+        int found = -1;
+        for (int d = 1; d <= kVacReach && found < 0; ++d)
+            for (int a = 0; a < 6 && found < 0; ++a) {
+                if (d > room[a]) continue;
+                const unsigned long long w = cellw[kCS * (size_t)((long long)b + (long long)d * step[a])];
+                if (cw_dusty(w)) found = (int)cw_species(w);
+            }
+        if (found >= 0 && (uint32_t)found != cw_species(cw))
+            reinterpret_cast<uint32_t *>(cellw + kCS * b)[0] = ((uint32_t)cw & ~0xffu) | (uint32_t)found;
+    }
+}
+
 // Vacuum mask of one level: bit of box (bx, by, bz) is set when all its in-grid cells have rho == 0.
 // Level 0 is built from the packed cells, level l > 0 from level l - 1 (4x4x4 children per box).
 __global__ void k_build_mask0(unsigned long long *__restrict__ cellw, uint32_t *__restrict__ m, int nx, int ny, int nz,
@@ -2236,6 +2319,7 @@ int mcrt_grid_create(mcrt_ctx **out, int nx, int ny, int nz, double cell_size_cm
         const size_t nbr = (size_t)c->nbx * c->nby * c->nbz;
         k_build_mask0<<<stream_grid(nbr), 256, 0, c->stream>>>(c->cellw, c->vmask, nx, ny, nz, c->px, c->pxy, c->msh, c->nbx,
                                                              c->nby, c->nbz);
+        if (MCRT_VAC_SPECIES) k_vac_species<<<stream_grid(c->nc), 256, 0, c->stream>>>(c->cellw, nx, ny, nz, c->px, c->pxy);
         GC_CUDA(cudaMemsetAsync(c->vsat, 0, (size_t)(c->nbx + 1) * (c->nby + 1) * (c->nbz + 1) * sizeof(int), c->stream));
         k_sat_pass<<<stream_grid((size_t)c->nby * c->nbz), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 0);
         k_sat_pass<<<stream_grid((size_t)c->nbx * c->nbz), 256, 0, c->stream>>>(c->vmask, c->vsat, c->nbx, c->nby, c->nbz, 1);
