@@ -100,6 +100,11 @@ typedef struct {
                                   mcrt_read) comes from that energy; all other cells' from their counts.  Default 0: the linear
                                   path-length tally in every cell.  Not with mixtures, live B&W or partitioned runs; a run that
                                   continues stored tallies (reset_tallies = 0, sweeps) must use the estimator that made them */
+    int32_t tau_redraw_per_cell; /* 1 = the optical depth to the next interaction is drawn anew on entering every cell, the paper's
+                                  literal form (footnote 1, states its equivalence with one draw per
+                                  flight, which pin P11 confirms statistically): the cell reached after c crossings of a flight
+                                  uses Philox draw (flight's draw index + c).  Default 0: one draw per flight (reading Q4).
+                                  Trajectories differ from the default's; not with carry-over or live B&W */
 } mcrt_run_opts;
 
 /* Counters of the runs since the last reset (all exact integers). */

@@ -42,7 +42,7 @@ class RunOpts(C.Structure):
                 ("reset_tallies", C.c_int32), ("rng_pass", C.c_uint32), ("grid_blocks", C.c_int32),
                 ("block_threads", C.c_int32), ("time_kernels", C.c_int32), ("first_packet_id", C.c_uint64),
                 ("n_total", C.c_uint64), ("epoch_growth", C.c_double), ("part_index", C.c_int32),
-                ("part_count", C.c_int32), ("source_strata", C.c_uint32), ("carry_interactions", C.c_uint32), ("no_hot_cells", C.c_int32), ("lucy_hybrid", C.c_int32)]
+                ("part_count", C.c_int32), ("source_strata", C.c_uint32), ("carry_interactions", C.c_uint32), ("no_hot_cells", C.c_int32), ("lucy_hybrid", C.c_int32), ("tau_redraw_per_cell", C.c_int32)]
 
 
 class ImageOpts(C.Structure):

@@ -500,6 +500,7 @@ struct TransportParams {
     const double2 *__restrict__ mx_thr;        // [ns][nf] {S0, A0}: thresholds of the event uniform
     const int *__restrict__ mx_mat;            // [ns][2] material of each component
     // thresholded Lucy estimator (Sect. 3.1, readings Q37 / Q38): NULL = the linear tally in every cell
+    int redraw;                                // 1: a new optical depth is drawn on entering every cell (as printed)
     const double *__restrict__ kmax_diag;      // [ns] sqrt(3) h max_nu (kabs + ksca): a cell is tallied if rho * this < 10^-2
     double two_fx, inv_two_fx;                 // 2^FX, 2^-FX
     uint32_t seed_lo, seed_hi, pass;
@@ -843,6 +844,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             const double *k1_row = P.kabs1_fx;                  // mixtures: the second component's kabs_fx at frequency j
             double kq1 = 0.0;
             double kmd = 0.0;                                   // thresholded estimator: kmax_diag of species kq_sp
+            unsigned long long rd_pid = 0ull;                   // per-cell redraw: the packet's id and its draw index minus crossings
+            uint32_t rd_base = 0u;
             // words of cells n .. n+kDepth-1, in registers
             unsigned long long cwr[kDepth];
             unsigned long long wstop = 0ull;             // cell word of the cell this lane's packet stopped in (MCRT_STOP_RELOAD)
@@ -957,6 +960,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq_sp = 0u; kq = kq_row[0];
                         if (XTRA && P.lfx1) { k1_row = P.kabs1_fx + j; kq1 = k1_row[0]; }
                         if (XTRA && P.kmax_diag) kmd = P.kmax_diag[0];
+                        if (XTRA && P.redraw) {
+                            rd_pid = (unsigned long long)__double_as_longlong(SF(F_PID, slot));
+                            rd_base = SU(U_DK, slot) & 0x3fffffffu;
+                        }
                         state = ST_FLY;
                     }
                     mFly.remove(take, slot);
@@ -1021,6 +1028,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
                         if (XTRA && P.lfx1) kq1 = k1_row[fly ? kq_sp * nf_r : 0u];   /* second component of a mixture */     \
                         if (XTRA && P.kmax_diag) kmd = P.kmax_diag[fly ? kq_sp : 0u]; /* thresholded estimator */             \
+                    }                                                                                                       \
+                    if (XTRA && P.redraw && fly) {   /* a new random number on entering the cell */             \
+                        double zr0, zr1;                                                                                    \
+                        draw2(P.seed_lo, P.seed_hi, rd_pid, (rd_base + ncross) & 0x3fffffffu, P.pass, zr0, zr1);            \
+                        tau = -traj_log(zr0);                                                                               \
                     }                                                                                                       \
                     const double dtau = kq.x * rho_c * ds;            /* tau_i = (kabs+ksca) h rho ds (Eq. 2) */ \
                     const bool stop = !(dtau <= tau);                 /* interaction inside this cell: equality leaves (Q5) */ \
@@ -1198,6 +1210,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0);
                 j = (int)(SU(U_W1, slot) & 0xffffu); nint = SU(U_W1, slot) >> 16;
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+                // per-cell redraw: the slot holds (index of the flight's draw) - (crossings at its start); every cell
+                // entered since has used one more draw (see the walk), so the next free index is
+                if (XTRA && P.redraw) d = (d + ncross + 1u) & 0x3fffffffu;
             }
             {   // run counters of the packets that escape in this phase: summed over the warp, then added to the warp's
                 // own counters in shared memory by one lane (no atomics)
@@ -1439,7 +1454,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 SF(F_CW, slot) = __longlong_as_double((long long)cw);
                 SF(F_PID, slot) = __longlong_as_double((long long)pid);
                 if (RECORD) SF(F_HASH, slot) = __longlong_as_double((long long)hash);
-                SU(U_DK, slot) = d;    // kind is set when the walk stops
+                // (kind is set when the walk stops.)  Per-cell redraw: the cell reached after c crossings of
+                // this flight takes the draw of index (flight's draw) + c -- c = 0 is the flight's own draw, so the first
+                // cell needs no special case -- and the slot keeps that index minus the crossing count
+                SU(U_DK, slot) = (XTRA && P.redraw) ? ((d - 1u - ncross) & 0x3fffffffu) : d;
                 SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
                 SU(U_W0, slot) = pack_xyz(ix, iy, iz);
                 SU(U_W1, slot) = (uint32_t)j | (nint << 16);
@@ -2786,6 +2804,7 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
         P.lfx1 = c->lfx1; P.kcnt1 = c->kcnt1; P.tidx1 = c->tidx1; P.kabs1_fx = c->d_kabs1_fx;
         P.mx_thr = reinterpret_cast<const double2 *>(c->d_mx_thr); P.mx_mat = c->d_mx_mat;
     }
+    P.redraw = c->run.o.tau_redraw_per_cell ? 1 : 0;
     if (c->run.o.lucy_hybrid) { P.kmax_diag = c->d_kmax_diag; P.two_fx = ldexp(1.0, c->fx); P.inv_two_fx = ldexp(1.0, -c->fx); }
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base; P.dig_n = c->dig_n;
@@ -2907,6 +2926,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
     if (c->mix && (o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
         return fail(c, MCRT_EINVAL, "dust mixtures are not available in live B&W or partitioned runs");
+    if (o.tau_redraw_per_cell && (o.carry_interactions || o.mode == MCRT_MODE_LIVE_BW))
+        return fail(c, MCRT_EINVAL, "tau_redraw_per_cell is not available with carry-over or in live B&W");
     if (o.lucy_hybrid && (c->mix || o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
         return fail(c, MCRT_EINVAL, "lucy_hybrid is not available with mixtures, in live B&W or partitioned runs");
     if ((o.mode == MCRT_MODE_FROZEN_T_SWEEP || !o.reset_tallies) && c->last_n != 0 && c->hybrid != (o.lucy_hybrid != 0))
@@ -2926,7 +2947,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     int n_hot = 0;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
     if ((rc = apply_hot(c, n_hot))) return rc;
-    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid;
+    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid || o.tau_redraw_per_cell;
     R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 

@@ -760,3 +760,32 @@ def test_parity_thresholded_lucy_estimator(B, orc):
     with pytest.raises(Exception):
         c.run(N, 93, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1)      # the other estimator's tallies: refused
     c.close()
+
+
+@pytest.mark.parametrize("case", ["sphere", "torus"])
+def test_parity_tau_redraw_per_cell(B, orc, case):
+    """NEXT-4, PAPER.md:51 as printed (oracle pin P11): a new optical depth on entering every cell.  The cell reached
+    after c crossings of a flight uses draw (flight's index + c), through walk, jumps over empty bricks and parked
+    packets alike: digests and all tallies bit-equal to the oracle's per_cell_redraw, B&W epochs and a sweep."""
+    if case == "sphere":
+        w, N, kw = W.sphere32(tau_V=5.0, n=16), 50_000, {}
+    else:
+        w, N, kw = W.torus256(n_clumps=400, n=64), 150_000, dict(grid_blocks=3, block_threads=64)   # saturated pools
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 55, n_threads=NTH, digests=True, per_cell_redraw=True)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 55, record_digests=1, tau_redraw_per_cell=1, **kw)
+    for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+        assert ro[key] == rg[key], key
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    r1 = orc.Oracle.from_workload(w).run(N, 55, n_threads=NTH, digests=True)
+    assert not np.array_equal(r1["digests"]["hash"], ro["digests"]["hash"])      # other trajectories than one draw per flight
+    o.run(N, 56, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, per_cell_redraw=True, reset=False, n_threads=NTH, digests=True)
+    c.run(N, 56, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1, tau_redraw_per_cell=1, record_digests=1)
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    c.close()
