@@ -157,6 +157,11 @@ typedef struct {
     double *cdfB;          /* [ns][nT][nf], Eq. 5 */
     double *cdfdB;         /* [ns][nT][nf], Eq. 10 */
     double *srccdf;        /* [nf] */
+    /* NEXT-3 sub-cubes (orc_set_subgrid): refined cubes hold subR^3 sub-cubes each, numbered nc + block*subR^3 + local */
+    int subR, n_sub;
+    int32_t *sub_of_cell;  /* [nc] block number of a refined cube, -1 otherwise */
+    float *sub_rho;        /* [n_sub][subR^3] (z, y, x) */
+    uint8_t *sub_sp;
     /* NEXT-3 dust mixtures (orc_set_mixtures): with n_mix > 0 the species byte of a cell names a MIXTURE of one or
      * two of the ns materials, and kext_h / kabs_h / albedo above have n_mix rows (ntab = rows of those tables) */
     int ntab, n_mix;
@@ -227,6 +232,7 @@ void orc_destroy(orc_ctx *C)
     free(C->rho); free(C->sp); free(C->nu); free(C->dnu); free(C->kabs); free(C->ksca); free(C->g);
     free(C->Tg); free(C->mu_edges); free(C->kext_h); free(C->kabs_h); free(C->albedo); free(C->J);
     free(C->cdfB); free(C->cdfdB); free(C->srccdf);
+    free(C->sub_of_cell); free(C->sub_rho); free(C->sub_sp);
     free(C->mx_ncomp); free(C->mx_mat); free(C->mx_frac); free(C->mx_S0); free(C->mx_A0); free(C->mx_kabs1_h);
     free(C);
 }
@@ -299,6 +305,57 @@ int orc_set_mixtures(orc_ctx *C, int n_mix, const int32_t *ncomp, const int32_t 
         }
     }
     return 0;
+}
+
+/* NEXT-3, one level of refinement: "Each cube is divided into an arbitrary number of sub-cubes of volume
+ * V_i and constant density rho_i ... The subdivision of cubes allows a finer sampling whenever required".
+ * Reading Q40: a refined cube holds R x R x R equal sub-cubes, R = 2, 4 or 8 the same for all refined cubes
+ * of a grid, each with its own density and species; a packet crosses them with the same cell walk on the lattice of
+ * sub-cube faces (face coordinates c + k/R are exact doubles), every sub-cube is a cell of its own for optical depth,
+ * tallies, absorption counts and temperature (Eq. 4 with V = (h/R)^3).  Cell numbers of sub-cubes: nc + block R^3 +
+ * (gz R + gy) R + gx.  With every cube refined the run IS the run on the (n R)^3 uniform grid, bit for bit (pin P24).
+ * cube[n_sub]: cell index of every refined cube; rho_sub / sp_sub [n_sub][R^3].  Call before orc_state_create. */
+int orc_set_subgrid(orc_ctx *C, int R, int n_sub, const int64_t *cube, const float *rho_sub, const uint8_t *sp_sub)
+{
+    if ((R != 2 && R != 4 && R != 8) || n_sub < 1 || C->n_mix) return -1;
+    size_t nc = (size_t)C->nx * C->ny * C->nz, R3 = (size_t)R * R * R;
+    C->sub_of_cell = (int32_t *)malloc(nc * sizeof(int32_t));
+    for (size_t i = 0; i < nc; ++i) C->sub_of_cell[i] = -1;
+    for (int b = 0; b < n_sub; ++b) {
+        if (cube[b] < 0 || (size_t)cube[b] >= nc || C->sub_of_cell[cube[b]] >= 0) return -1;
+        C->sub_of_cell[cube[b]] = b;
+    }
+    for (size_t i = 0; i < n_sub * R3; ++i)
+        if (!(rho_sub[i] >= 0.0f) || sp_sub[i] >= C->ns) return -1;
+    C->sub_rho = (float *)malloc(n_sub * R3 * sizeof(float));  memcpy(C->sub_rho, rho_sub, n_sub * R3 * sizeof(float));
+    C->sub_sp = (uint8_t *)malloc(n_sub * R3);                 memcpy(C->sub_sp, sp_sub, n_sub * R3);
+    C->subR = R; C->n_sub = n_sub;
+    return 0;
+}
+/* all cells, sub-cubes included: count, density (0 for a refined cube itself: its dust is in its sub-cubes), species */
+static inline size_t cells_total(const orc_ctx *C)
+{
+    size_t nc = (size_t)C->nx * C->ny * C->nz;
+    return C->subR ? nc + (size_t)C->n_sub * C->subR * C->subR * C->subR : nc;
+}
+static inline double cell_rho(const orc_ctx *C, size_t ci)
+{
+    size_t nc = (size_t)C->nx * C->ny * C->nz;
+    if (ci >= nc) return (double)C->sub_rho[ci - nc];
+    if (C->subR && C->sub_of_cell[ci] >= 0) return 0.0;
+    return (double)C->rho[ci];
+}
+static inline int cell_sp(const orc_ctx *C, size_t ci)
+{
+    size_t nc = (size_t)C->nx * C->ny * C->nz;
+    return ci >= nc ? C->sub_sp[ci - nc] : C->sp[ci];
+}
+/* Eq. 4's xi / (4 pi V) for cell ci: V = h^3, or (h/R)^3 for a sub-cube (computed like the uniform grid of that cell size) */
+static inline double cell_fac(const orc_ctx *C, size_t ci, double xi)
+{
+    size_t nc = (size_t)C->nx * C->ny * C->nz;
+    double hh = ci >= nc ? C->h / (double)C->subR : C->h;
+    return xi / (ORC_FOUR_PI * hh * hh * hh);
 }
 
 /* material and mass fraction of component c of the cell species x (without mixtures: the material x itself) */
@@ -681,6 +738,10 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
     uint32_t ncross = 0, nsca = 0, nabs = 0, nint = 0;
     uint64_t hash = 0xCBF29CE484222325ull;
     int j;
+    /* sub-cubes (orc_set_subgrid): the sub-cube g of cube c the packet is in, if g_ok; the axis of the last crossing */
+    const int subR = C->subR;
+    const size_t nc0 = (size_t)n[0] * n[1] * n[2], R3 = (size_t)subR * subR * subR;
+    int g[3] = { 0, 0, 0 }, g_ok = 0, last_axis = 0;
 
     if (resume) {
         pid = resume->pid; hash = resume->hash; j = resume->j; d = resume->d;
@@ -701,6 +762,15 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
         orc_isotropic(z[0], z[1], u);
         p[0] = C->pos[0]; p[1] = C->pos[1]; p[2] = C->pos[2];
         start_cell(p, u, c);
+        if (subR) {     /* the same rule on the lattice of sub-cube faces: cube and sub-cube of the start point */
+            for (int a = 0; a < 3; ++a) {
+                double pf = p[a] * (double)subR, fl = floor(pf);
+                int G = (pf != fl) ? (int)fl : ((u[a] >= 0.0) ? (int)fl : (int)fl - 1);
+                c[a] = (G >= 0) ? G / subR : -((-G + subR - 1) / subR);
+                g[a] = G - c[a] * subR;
+            }
+            g_ok = 1;
+        }
         hash_mix(&hash, event_word(ORC_EV_EMIT, j, ((uint64_t)c[2] * n[1] + c[1]) * n[0] + c[0]));
         st->packets++;
     }
@@ -719,7 +789,65 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
         int s, sj;
         double rho_c, kk;
         int first_cell = 1;
+        int in_sub = 0;         /* the flight ends with an interaction inside sub-cube g */
         for (;;) {
+            int blk = subR ? C->sub_of_cell[((size_t)c[2] * n[1] + c[1]) * n[0] + c[0]] : -1;
+            if (blk < 0) g_ok = 0;
+            else {
+                /* a refined cube: the same walk on the lattice of its sub-cube faces, f = c + k/R (reading Q40) */
+                const double Rd = (double)subR;
+                if (!g_ok) {    /* entered from an unrefined cube: first / last layer along the crossed axis, else by the entry point */
+                    for (int a = 0; a < 3; ++a) {
+                        if (a == last_axis && !first_cell) g[a] = (D.step[a] > 0) ? 0 : subR - 1;
+                        else {
+                            double e = p[a] + u[a] * t;
+                            int q = (int)floor((e - (double)c[a]) * Rd);
+                            g[a] = q < 0 ? 0 : (q > subR - 1 ? subR - 1 : q);
+                        }
+                    }
+                    g_ok = 1;
+                }
+                double ftm[3];
+                for (int a = 0; a < 3; ++a)
+                    ftm[a] = (D.step[a] == 0) ? INFINITY
+                                              : (((double)c[a] + (double)(g[a] + (D.step[a] > 0 ? 1 : 0)) / Rd) - D.p[a]) * D.inv[a];
+                int left = 0;
+                while (!left) {
+                    int a = (ftm[0] <= ftm[1] && ftm[0] <= ftm[2]) ? 0 : ((ftm[1] <= ftm[2]) ? 1 : 2);
+                    double tn = ftm[a];
+                    double ds = tn - t;
+                    ci = nc0 + (size_t)blk * R3 + ((size_t)g[2] * subR + g[1]) * subR + g[0];
+                    rho_c = (double)C->sub_rho[ci - nc0];
+                    s = C->sub_sp[ci - nc0];
+                    sj = s * nf + j;
+                    if (R->o->per_cell_redraw && !first_cell) {
+                        orc_uniforms(R->seed, pid, d++, R->pass, z);
+                        tau = -orc_det_log(z[0]);
+                    }
+                    first_cell = 0;
+                    kk = C->kext_h[sj] * rho_c;
+                    double dtau = kk * ds;
+                    if (dtau > tau) { in_sub = 1; break; }
+                    tau -= dtau;
+                    lucy_add(R, ci, sj, rho_c, ds, st);
+                    t = tn;
+                    g[a] += D.step[a];
+                    ncross++;
+                    st->crossings++;
+                    if (rho_c > 0.0) st->dusty_crossings++;
+                    if (g[a] < 0 || g[a] >= subR) {     /* through a face of the cube: the neighbouring cube, same sub-cube row */
+                        g[a] = (D.step[a] > 0) ? 0 : subR - 1;
+                        last_axis = a;
+                        dda_advance(&D, a, c);
+                        if (c[a] < 0 || c[a] >= n[a]) goto escaped;
+                        left = 1;
+                    } else {
+                        ftm[a] = (((double)c[a] + (double)(g[a] + (D.step[a] > 0 ? 1 : 0)) / Rd) - D.p[a]) * D.inv[a];
+                    }
+                }
+                if (in_sub) break;
+                continue;
+            }
             int a = dda_axis(&D);
             double tn = D.tmax[a];
             double ds = tn - t;
@@ -739,6 +867,7 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
             lucy_add(R, ci, sj, rho_c, ds, st);
             t = tn;
             dda_advance(&D, a, c);
+            last_axis = a;
             ncross++;
             st->crossings++;
             if (rho_c > 0.0) st->dusty_crossings++;
@@ -752,6 +881,10 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
             for (int a = 0; a < 3; ++a) {
                 double q = p[a] + u[a] * tint;
                 double lo = (double)c[a], hi = (double)(c[a] + 1);
+                if (in_sub) {   /* the interaction point stays inside its sub-cube */
+                    lo = (double)c[a] + (double)g[a] / (double)subR;
+                    hi = (double)c[a] + (double)(g[a] + 1) / (double)subR;
+                }
                 if (q < lo) q = lo;
                 if (q > hi) q = hi;
                 p[a] = q;
@@ -939,7 +1072,7 @@ orc_state *orc_state_create(const orc_ctx *C)
 {
     orc_state *S = (orc_state *)calloc(1, sizeof(orc_state));
     S->C = C;
-    S->nc = (size_t)C->nx * C->ny * C->nz;
+    S->nc = cells_total(C);          /* sub-cubes (NEXT-3) are cells of their own, behind the grid's */
     S->k = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
     S->kprev = (uint64_t *)calloc(S->nc, sizeof(uint64_t));
     S->Lfx = (int64_t *)calloc(S->nc, sizeof(int64_t));
@@ -1009,9 +1142,25 @@ static void epoch_update(orc_state *S, int first_epoch, double ratio, double cel
 {
     const orc_ctx *C = S->C;
     const double inv_fx = ldexp(1.0, -S->fx);
+    const size_t nc0 = (size_t)C->nx * C->ny * C->nz;
+    const double cellfac0 = cellfac, cellfac_sub = cellfac * (double)(C->subR * C->subR * C->subR);   /* V = (h/R)^3 */
     for (size_t ci = 0; ci < S->nc; ++ci) {
-        double rho_c = (double)C->rho[ci];
+        double rho_c = cell_rho(C, ci);
         uint64_t kk = S->k[ci];
+        if (ci >= nc0) cellfac = cellfac_sub; else cellfac = cellfac0;
+        if (ci >= nc0 || (C->subR && C->sub_of_cell[ci] >= 0)) {      /* a sub-cube, or a refined cube (no dust of its own) */
+            if (rho_c > 0.0) {
+                double kt;
+                if (first_epoch) kt = (double)kk + 1.0;
+                else {
+                    double pred = 0.5 * (double)(kk - S->kprev[ci]) * ratio;
+                    kt = (double)kk + ((pred > 1.0) ? pred : 1.0);
+                }
+                S->tidx[ci] = (uint16_t)t_index(C, cell_sp(C, ci), kt * cellfac / rho_c);
+            } else S->tidx[ci] = 0;
+            S->kprev[ci] = kk;
+            continue;
+        }
         if (S->hybrid && orc_thin_cell(rho_c, S->kmax_diag[C->sp[ci]])) {
             /* Sect. 3.1 (reading Q39): the temperature of a cell below the threshold comes from its Eq. 9 energy, Eq. 4
              * with k xi replaced by E_abs; the same midpoint prediction, on the tally (k_prev keeps the tally here) */
@@ -1060,8 +1209,17 @@ static void sweep_update(orc_state *S, int from_lucy, double cellfac, int fx_of_
 {
     const orc_ctx *C = S->C;
     double inv_fx = ldexp(1.0, -fx_of_tallies);
+    const size_t nc0 = (size_t)C->nx * C->ny * C->nz;
+    const double cellfac_sub = cellfac * (double)(C->subR * C->subR * C->subR);
     for (size_t ci = 0; ci < S->nc; ++ci) {
-        double rho_c = (double)C->rho[ci];
+        double rho_c = cell_rho(C, ci);
+        if (ci >= nc0 || (C->subR && C->sub_of_cell[ci] >= 0)) {
+            if (rho_c > 0.0) {
+                double e = from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+                S->tidx[ci] = (uint16_t)t_index(C, cell_sp(C, ci), e * (ci >= nc0 ? cellfac_sub : cellfac) / rho_c);
+            } else S->tidx[ci] = 0;
+            continue;
+        }
         if (rho_c > 0.0) {
             double e = from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
             if (S->hybrid) e = orc_thin_cell(rho_c, S->kmax_diag[C->sp[ci]]) ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
@@ -1107,7 +1265,8 @@ int orc_run(orc_state *S, uint64_t n_packets, uint64_t seed, const orc_opts *o, 
     S->xi = C->L / (double)n_xi;                         /* xi = L/N */
     if (!o->reset && o->mode == ORC_MODE_BW_EPOCH && prev_xi != 0.0 && (prev_xi != S->xi || prev_fx != S->fx))
         return -2;                                       /* tallies of another packet energy cannot be continued */
-    if (o->lucy_hybrid && C->n_mix) return -3;           /* not defined for mixtures */
+    if (o->lucy_hybrid && (C->n_mix || C->subR)) return -3; /* not defined for mixtures / sub-cubes */
+    if (C->subR && o->carry_K) return -3;
     if (!o->reset && prev_xi != 0.0 && (S->hybrid != 0) != (o->lucy_hybrid != 0))
         return -2;                                       /* tallies of the other estimator cannot be continued */
     if (o->lucy_hybrid && !S->kmax_diag) {
@@ -1264,7 +1423,11 @@ void orc_read(const orc_state *S, double *E_count, double *E_lucy, float *T, int
         double el = (double)S->Lfx[ci] * inv_fx * S->xi;
         if (E_count) E_count[ci] = ec;
         if (E_lucy) E_lucy[ci] = el;
-        if (T) {
+        if (T && C->subR) {          /* grids with sub-cubes: every cell with its own volume */
+            double rho_c = cell_rho(C, ci);
+            double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
+            T[ci] = rho_c > 0.0 ? (float)orc_T_of_x(C, cell_sp(C, ci), e * cell_fac(C, ci, S->xi) / rho_c) : 0.0f;
+        } else if (T) {
             double rho_c = (double)C->rho[ci];
             if (rho_c > 0.0) {
                 double e = T_from_lucy ? (double)S->Lfx[ci] * inv_fx : (double)S->k[ci];
@@ -1356,7 +1519,7 @@ int orc_ray_trace(const orc_state *S, const double ez_in[3], const double ex_in[
 {
     const orc_ctx *C = S->C;
     if (j < 0 || j >= C->nf || nx < 1 || ny < 1 || !(pix > 0.0) || !(D > 0.0)) return -1;
-    if (C->n_mix) return -1;    /* images of mixtures are not defined here */
+    if (C->n_mix || C->subR) return -1;    /* images of mixtures / refined grids are not defined here */
     const int n[3] = { C->nx, C->ny, C->nz };
     double ez[3], ex[3], ey[3];
     double nz_ = sqrt(ez_in[0] * ez_in[0] + ez_in[1] * ez_in[1] + ez_in[2] * ez_in[2]);

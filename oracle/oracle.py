@@ -66,6 +66,8 @@ def lib():
         L.orc_get_tables.argtypes = [C.c_void_p] + [C.c_void_p] * 6
         L.orc_eq9_value.restype = C.c_double
         L.orc_eq9_value.argtypes = [C.c_double]
+        L.orc_set_subgrid.restype = C.c_int
+        L.orc_set_subgrid.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_set_mixtures.restype = C.c_int
         L.orc_set_mixtures.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_read_raw_comp1.restype = C.c_int
@@ -204,7 +206,7 @@ class Oracle:
     """One problem (grid + dust + source + escape bins) and its tally state."""
 
     def __init__(self, nx, ny, nz, h, rho, species, n_species, nu, kabs, ksca, g, Tgrid, L, Tstar, Lnu_w,
-                 pos_cm, mu_edges, mixtures=None):
+                 pos_cm, mu_edges, mixtures=None, subgrid=None):
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.nc = self.nx * self.ny * self.nz
         self.ns, self.nf, self.nT = int(n_species), len(nu), len(Tgrid)
@@ -228,6 +230,18 @@ class Oracle:
             assert mat_.shape == (len(nc_), 2) and fr_.shape == (len(nc_), 2)
             rc = lib().orc_set_mixtures(self._ctx, len(nc_), _p(nc_), _p(mat_), _p(fr_))
             assert rc == 0, "bad mixture table"
+        self.subgrid = subgrid
+        if subgrid is not None:
+            # NEXT-3: (R, cube[n_sub] cell indices of the refined cubes, rho_sub[n_sub][R^3], species_sub[n_sub][R^3]);
+            # the sub-cubes are cells nc .. nc + n_sub R^3 - 1 of every per-cell output
+            Rr, cube, rs, ss = subgrid
+            cube = np.ascontiguousarray(cube, np.int64)
+            rs = np.ascontiguousarray(rs, np.float32).reshape(len(cube), -1)
+            ss = np.ascontiguousarray(ss, np.uint8).reshape(len(cube), -1)
+            assert rs.shape == (len(cube), Rr ** 3) and ss.shape == rs.shape
+            rc = lib().orc_set_subgrid(self._ctx, int(Rr), len(cube), _p(cube), _p(rs), _p(ss))
+            assert rc == 0, "bad sub-grid"
+            self.nc0, self.nc = self.nc, self.nc + len(cube) * Rr ** 3
         self._state = lib().orc_state_create(self._ctx)
         self.last_n = 0
 
@@ -235,7 +249,7 @@ class Oracle:
     def from_workload(cls, w):
         return cls(w.nx, w.ny, w.nz, w.cell_size_cm, w.rho, w.species, w.n_species, w.nu_hz, w.kappa_abs,
                    w.kappa_sca, w.g, w.T_grid, w.L_erg_s, w.T_star_K, w.L_nu_weights, w.source_pos_cm,
-                   w.abs_mu_edges, mixtures=getattr(w, "mixtures", None))
+                   w.abs_mu_edges, mixtures=getattr(w, "mixtures", None), subgrid=getattr(w, "subgrid", None))
 
     def close(self):
         if self._state:

@@ -59,6 +59,9 @@ class Workload:
     # NEXT-3: (n_components[n_species], material[n_species][2], mass fraction[n_species][2]): cell species x is a mixture
     # of one or two of the n_species materials (None: species x is material x)
     mixtures: tuple | None = None
+    # NEXT-3: (R, cube[n_sub], rho_sub[n_sub][R^3], species_sub[n_sub][R^3]): the cubes with these cell indices are divided
+    # into R^3 sub-cubes (z, y, x order) with their own densities and species; rho of such a cube must be > 0 (a placeholder)
+    subgrid: tuple | None = None
 
     @property
     def n_cells(self) -> int:

@@ -1147,3 +1147,116 @@ def test_p23_hybrid_temperatures(orc):
     assert (t2[core] > 0).all() and np.abs(Tg[t2[core]] / Tc - 1).max() < 0.02
     shell = (r >= 7.0) & (r < 8.0)
     assert abs((Tg[t2[shell]] / Tl[shell]).mean() - 1) < 0.02
+
+
+# ------------------------------------------------------------------------------------------ P24 sub-cubes (NEXT-3)
+def _fine_medium(nf_cells, seed, n_species=2):
+    """A random clumpy medium on a fine grid: densities over two decades, a quarter of the cells empty."""
+    rng = np.random.default_rng(seed)
+    rho = (10.0 ** rng.uniform(-1.5, 0.5, (nf_cells,) * 3)).astype(np.float32)
+    rho[rng.random((nf_cells,) * 3) < 0.25] = 0.0
+    sp = rng.integers(0, n_species, (nf_cells,) * 3).astype(np.uint8)
+    return rho, sp
+
+
+def _two_species_cube(n, tau_edge):
+    w = W.uniform_cube(n, tau_edge_V=tau_edge, albedo=0.5, g_const=0.4, n_nu=16, slope=1.0, source_offset_cells=(0.3, -0.2, 0.1))
+    w.kappa_abs = np.vstack([w.kappa_abs, 0.5 * w.kappa_abs[:1]])
+    w.kappa_sca = np.vstack([w.kappa_sca, 2.0 * w.kappa_sca[:1]])
+    w.g = np.vstack([w.g, 0.0 * w.g[:1] - 0.2])
+    w.n_species = 2
+    return w
+
+
+def _to_blocks(fine, n, R):
+    """[nR]^3 array -> [n^3 cubes][R^3] in cube order (z, y, x) and sub-cube order (z, y, x)."""
+    return fine.reshape(n, R, n, R, n, R).transpose(0, 2, 4, 1, 3, 5).reshape(n ** 3, R ** 3)
+
+
+@pytest.mark.parametrize("R", [2, 4])
+def test_p24_fully_refined_grid_is_the_fine_uniform_grid(orc, R):
+    """Reading Q40 against the uniform-grid path (itself pinned by P2-P18): with EVERY cube divided into R^3 sub-cubes
+    the run is the run on the (n R)^3 uniform grid of cell size h/R -- face coordinates c + k/R, chord lengths and
+    volumes differ from the fine grid's by exact powers of two -- so every packet makes the same crossings, scatterings
+    and absorptions and escapes into the same bin, and every sub-cube has the fine cell's count, tally and temperature
+    index, bit for bit, through B&W epochs and a sweep."""
+    n, N = 6, 20_000
+    nfc = n * R
+    fine = _two_species_cube(nfc, tau_edge=1.5)
+    rho_f, sp_f = _fine_medium(nfc, 240 + R)
+    rho_f *= np.float32(fine.rho.flat[0])
+    fine.rho, fine.species = rho_f, sp_f
+    coarse = _two_species_cube(n, tau_edge=1.5)
+    coarse.cell_size_cm = fine.cell_size_cm * R
+    coarse.source_pos_cm = fine.source_pos_cm
+    coarse.rho = np.ones((n, n, n), np.float32)
+    coarse.species = np.zeros((n, n, n), np.uint8)
+    coarse.subgrid = (R, np.arange(n ** 3), _to_blocks(rho_f, n, R), _to_blocks(sp_f, n, R))
+    of, oc = orc.Oracle.from_workload(fine), orc.Oracle.from_workload(coarse)
+    for step in range(2):
+        kw = dict(n_threads=NTH, digests=True) if step == 0 else dict(n_threads=NTH, digests=True, mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, reset=False)
+        rf, rc = of.run(N, 2400 + step, **kw), oc.run(N, 2400 + step, **kw)
+        for key in ("crossings", "dusty_crossings", "scatterings", "absorptions", "escapes", "direct_escapes", "lucy_adds"):
+            assert rf[key] == rc[key], key
+        for key in ("crossings", "scatterings", "absorptions", "escape_bin"):
+            assert np.array_equal(rf["digests"][key], rc["digests"][key]), key
+        F, Cc = of.read_raw(), oc.read_raw()
+        assert np.array_equal(F["sed"], Cc["sed"])
+        for key in ("k", "lucy_fx", "tidx"):
+            assert not Cc[key][:n ** 3].any()                               # refined cubes hold nothing themselves
+            assert np.array_equal(_to_blocks(F[key].reshape(nfc, nfc, nfc), n, R).reshape(-1), Cc[key][n ** 3:]), (step, key)
+        assert F["k"].sum() > N / 4
+    assert np.array_equal(_to_blocks(of.read()["T"].reshape(nfc, nfc, nfc), n, R).reshape(-1), oc.read()["T"][n ** 3:])
+
+
+def test_p24_partly_refined_grid(orc):
+    """Cubes of a coarse grid divided here and there (a third of them, R = 4), the others not: the medium is the same
+    as the fine uniform grid's in which an undivided cube is R^3 equal cells, so the statistics agree -- absorptions
+    per coarse cube, their split over the sub-cubes of the divided cubes (this is what a wrong sub-cube at the entry
+    from an undivided cube, or a wrong row kept from a divided one, changes), and the escaping spectrum -- and the
+    temperature of a sub-cube comes from its own volume (h/R)^3."""
+    n, R, N = 6, 4, 200_000
+    nfc = n * R
+    rng = np.random.default_rng(77)
+    refined = rng.random(n ** 3) < 0.35
+    refined[(n ** 3) // 2 + n // 2] = True
+    rho_f, sp_f = _fine_medium(nfc, 99)
+    base = _two_species_cube(nfc, tau_edge=1.5)
+    rho_f *= np.float32(base.rho.flat[0])
+    rb, sb = _to_blocks(rho_f, n, R), _to_blocks(sp_f, n, R)
+    rb[~refined] = rb[~refined][:, :1]                  # an undivided cube: one density, one species
+    sb[~refined] = sb[~refined][:, :1]
+    back = lambda blocks: blocks.reshape(n, n, n, R, R, R).transpose(0, 3, 1, 4, 2, 5).reshape(nfc, nfc, nfc)
+    base.rho, base.species = np.ascontiguousarray(back(rb)), np.ascontiguousarray(back(sb))
+    coarse = _two_species_cube(n, tau_edge=1.5)
+    coarse.cell_size_cm = base.cell_size_cm * R
+    coarse.source_pos_cm = base.source_pos_cm
+    coarse.rho = np.where(refined, 1.0, rb[:, 0]).astype(np.float32).reshape(n, n, n)
+    coarse.species = sb[:, 0].reshape(n, n, n).copy()
+    idx = np.flatnonzero(refined)
+    coarse.subgrid = (R, idx, rb[idx], sb[idx])
+    of, oc = orc.Oracle.from_workload(base), orc.Oracle.from_workload(coarse)
+    rf = of.run(N, 2411, n_threads=NTH, absorb_and_stop=True)
+    rc = oc.run(N, 2412, n_threads=NTH, absorb_and_stop=True)
+    assert rc["crossings"] < rf["crossings"]            # undivided cubes are crossed in one step
+    kf = _to_blocks(of.read_raw()["k"].reshape(nfc, nfc, nfc), n, R).astype(np.float64)
+    kc_raw = oc.read_raw()["k"].astype(np.float64)
+    kc = np.zeros_like(kf)
+    kc[~refined, 0] = kc_raw[:n ** 3][~refined]
+    kc[idx] = kc_raw[n ** 3:].reshape(len(idx), R ** 3)
+    a, b = kf.sum(axis=1), kc.sum(axis=1)               # per coarse cube
+    sel = (a + b) >= 40
+    chi2 = ((a[sel] - b[sel]) ** 2 / (a[sel] + b[sel])).sum()
+    assert sel.sum() > 100 and chi2 < sel.sum() + 5 * math.sqrt(2 * sel.sum()), (chi2, sel.sum())
+    a, b = kf[idx].reshape(-1), kc[idx].reshape(-1)     # per sub-cube of the divided cubes
+    sel = (a + b) >= 30
+    chi2 = ((a[sel] - b[sel]) ** 2 / (a[sel] + b[sel])).sum()
+    assert sel.sum() > 300 and chi2 < sel.sum() + 5 * math.sqrt(2 * sel.sum()), (chi2, sel.sum())
+    assert abs(rf["absorptions"] - rc["absorptions"]) < 5 * math.sqrt(2 * rf["absorptions"])
+    # temperatures (full B&W runs): a divided cube's sub-cubes against the fine grid's cells (a wrong volume in Eq. 4,
+    # h^3 for (h/R)^3, would shift every one of them by a factor 64^(1/5) or so)
+    of.run(60_000, 2413, n_threads=NTH); oc.run(60_000, 2414, n_threads=NTH)
+    Tf = _to_blocks(of.read(T_from_lucy=True)["T"].reshape(nfc, nfc, nfc).astype(np.float64), n, R)[idx].reshape(-1)
+    Tc = oc.read(T_from_lucy=True)["T"][n ** 3:].astype(np.float64)
+    ok = (Tf > 0) & (Tc > 0)
+    assert ok.sum() > 1000 and abs(np.log(Tc[ok] / Tf[ok]).mean()) < 0.01 and abs(np.median(np.log(Tc[ok] / Tf[ok]))) < 0.01
