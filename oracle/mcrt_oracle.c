@@ -738,10 +738,10 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
     uint32_t ncross = 0, nsca = 0, nabs = 0, nint = 0;
     uint64_t hash = 0xCBF29CE484222325ull;
     int j;
-    /* sub-cubes (orc_set_subgrid): the sub-cube g of cube c the packet is in, if g_ok; the axis of the last crossing */
+    /* sub-cubes (orc_set_subgrid): the sub-cube g of cube c the packet is in, if g_ok */
     const int subR = C->subR;
     const size_t nc0 = (size_t)n[0] * n[1] * n[2], R3 = (size_t)subR * subR * subR;
-    int g[3] = { 0, 0, 0 }, g_ok = 0, last_axis = 0;
+    int g[3] = { 0, 0, 0 }, g_ok = 0;
 
     if (resume) {
         pid = resume->pid; hash = resume->hash; j = resume->j; d = resume->d;
@@ -796,14 +796,13 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
             else {
                 /* a refined cube: the same walk on the lattice of its sub-cube faces, f = c + k/R (reading Q40) */
                 const double Rd = (double)subR;
-                if (!g_ok) {    /* entered from an unrefined cube: first / last layer along the crossed axis, else by the entry point */
+                if (!g_ok) {    /* entered from an unrefined cube: the sub-cube that holds the entry point p + u t.  Along the
+                                 * crossed axis the point lies on the cube's face up to rounding, and the clamp makes that the
+                                 * first or the last layer */
                     for (int a = 0; a < 3; ++a) {
-                        if (a == last_axis && !first_cell) g[a] = (D.step[a] > 0) ? 0 : subR - 1;
-                        else {
-                            double e = p[a] + u[a] * t;
-                            int q = (int)floor((e - (double)c[a]) * Rd);
-                            g[a] = q < 0 ? 0 : (q > subR - 1 ? subR - 1 : q);
-                        }
+                        double e = p[a] + u[a] * t;
+                        int q = (int)floor((e - (double)c[a]) * Rd);
+                        g[a] = q < 0 ? 0 : (q > subR - 1 ? subR - 1 : q);
                     }
                     g_ok = 1;
                 }
@@ -837,7 +836,6 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
                     if (rho_c > 0.0) st->dusty_crossings++;
                     if (g[a] < 0 || g[a] >= subR) {     /* through a face of the cube: the neighbouring cube, same sub-cube row */
                         g[a] = (D.step[a] > 0) ? 0 : subR - 1;
-                        last_axis = a;
                         dda_advance(&D, a, c);
                         if (c[a] < 0 || c[a] >= n[a]) goto escaped;
                         left = 1;
@@ -867,7 +865,6 @@ static int run_packet(orc_run_t *R, uint64_t pid, orc_stats *st, const orc_carry
             lucy_add(R, ci, sj, rho_c, ds, st);
             t = tn;
             dda_advance(&D, a, c);
-            last_axis = a;
             ncross++;
             st->crossings++;
             if (rho_c > 0.0) st->dusty_crossings++;
