@@ -180,6 +180,26 @@ int mcrt_dust_tables(mcrt_ctx *ctx, int n_nu, const double *nu_hz, const double 
  * the kernel instantiation of the rarely used features and no per-CTA hot-cell copies. */
 int mcrt_dust_mixtures(mcrt_ctx *ctx, const int32_t *n_components, const int32_t *material, const double *fraction);
 
+/* One level of refinement ("Each cube is divided into an arbitrary number of sub-cubes
+ * of volume V_i and constant density rho_i ... a finer sampling whenever required").  Reading Q40: the n_sub
+ * cubes with the cell indices cube[n_sub] ((iz ny + iy) nx + ix; each at most once; their own density in the grid must
+ * be > 0, a placeholder) are divided into R x R x R equal sub-cubes, R = 2, 4 or 8, with the densities rho_sub
+ * [n_sub][R^3] (g cm^-3, >= 0; order z, y, x) and species species_sub [n_sub][R^3].  Packets cross them with the same
+ * cell walk on the lattice of sub-cube faces; every sub-cube is a cell of its own for optical depth, Lucy tally,
+ * absorption count and temperature (Eq. 4 with V = (h/R)^3); in digests its cell number is nx ny nz + b R^3 +
+ * (gz R + gy) R + gx for sub-cube (gx, gy, gz) of cube cube[b].  With every cube divided the run is the run on the
+ * (n R)^3 uniform grid, bit for bit.  Host pointers.  After mcrt_grid_create, before the first run, once per context
+ * (after a failure the context must be destroyed).  mcrt_read / mcrt_read_raw return 0 for a divided cube itself;
+ * mcrt_read_subcells returns the sub-cubes' outputs.  Not with mixtures, carry-over, the thresholded estimator, live
+ * B&W, partitioned runs or mcrt_ray_trace; such runs use the kernel instantiation of the rarely used features. */
+int mcrt_subgrid(mcrt_ctx *ctx, int R, uint64_t n_sub, const int64_t *cube, const float *rho_sub,
+                 const uint8_t *species_sub);
+
+/* The arrays of mcrt_read and mcrt_read_raw for the sub-cubes, [n_sub R^3] each in the order of mcrt_subgrid; any
+ * pointer may be NULL. */
+int mcrt_read_subcells(mcrt_ctx *ctx, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy,
+                       uint64_t *k_abs, int64_t *lucy_fx, uint16_t *tidx, mcrt_mem where);
+
 /* Point source: luminosity L_erg_s split into equal-energy packets xi = L/N.
  *  T_star_K > 0: blackbody spectrum; otherwise L_nu_weights [n_nu] gives the spectral shape L_nu at the
  *  grid frequencies (any normalisation, >= 0, not all zero).  pos_cm strictly inside the grid. */

@@ -21,7 +21,7 @@ MCRT_OK, MCRT_EINVAL, MCRT_ESTATE, MCRT_ENOMEM, MCRT_ECUDA, MCRT_EOVERFLOW = 0, 
 MCRT_MODE_BW_EPOCH, MCRT_MODE_FROZEN_T_SWEEP, MCRT_MODE_LIVE_BW = 0, 1, 2
 
 EXPORTS = [
-    "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_dust_mixtures", "mcrt_source", "mcrt_escape_bins",
+    "mcrt_workspace_bytes", "mcrt_grid_create", "mcrt_dust_tables", "mcrt_dust_mixtures", "mcrt_subgrid", "mcrt_read_subcells", "mcrt_source", "mcrt_escape_bins",
     "mcrt_default_opts", "mcrt_run", "mcrt_run_begin", "mcrt_run_step", "mcrt_run_end", "mcrt_exchange_begin",
     "mcrt_exchange_end", "mcrt_exchange_peer_sum", "mcrt_exchange_local", "mcrt_epoch_schedule", "mcrt_part_slice",
     "mcrt_measure_read_bandwidth", "mcrt_scatter_store", "mcrt_scatter_events", "mcrt_ray_trace", "mcrt_get_stats", "mcrt_read", "mcrt_read_component", "mcrt_read_raw", "mcrt_read_tables",
@@ -111,6 +111,8 @@ def load_library(path: str = LIB_PATH):
     L.mcrt_read_raw.argtypes = [vp, vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_component.argtypes = [vp, i, vp, vp, vp, vp, vp, vp, vp, i]
     L.mcrt_dust_mixtures.argtypes = [vp, vp, vp, vp]
+    L.mcrt_subgrid.argtypes = [vp, i, u64, vp, vp, vp]
+    L.mcrt_read_subcells.argtypes = [vp, vp, vp, vp, vp, vp, vp, vp, i]
     L.mcrt_read_tables.argtypes = [vp] + [vp] * 6
     L.mcrt_philox_device.argtypes = [vp, vp, vp, u64]
     L.mcrt_traj_math_device.argtypes = [vp, vp, vp, vp, u64]
@@ -305,6 +307,20 @@ def mcrt_dust_mixtures(ctx, n_components, material, fraction):
     _check(load_library().mcrt_dust_mixtures(ctx, _ptr(nc_), _ptr(mat), _ptr(fr)), ctx)
 
 
+def mcrt_subgrid(ctx, R, cube, rho_sub, species_sub):
+    cube = np.ascontiguousarray(cube, np.int64).reshape(-1)
+    rs = np.ascontiguousarray(rho_sub, np.float32).reshape(len(cube), -1)
+    ss = np.ascontiguousarray(species_sub, np.uint8).reshape(len(cube), -1)
+    assert rs.shape == (len(cube), int(R) ** 3) and ss.shape == rs.shape
+    _check(load_library().mcrt_subgrid(ctx, int(R), len(cube), _ptr(cube), _ptr(rs), _ptr(ss)), ctx)
+
+
+def mcrt_read_subcells(ctx, E_abs_count=None, E_abs_lucy=None, T_count=None, T_lucy=None, k_abs=None, lucy_fx=None,
+                       tidx=None, where=MCRT_HOST):
+    _check(load_library().mcrt_read_subcells(ctx, _ptr(E_abs_count), _ptr(E_abs_lucy), _ptr(T_count), _ptr(T_lucy),
+                                             _ptr(k_abs), _ptr(lucy_fx), _ptr(tidx), where), ctx)
+
+
 def mcrt_read_component(ctx, component, E_abs_count=None, E_abs_lucy=None, T_count=None, T_lucy=None, k_abs=None,
                         lucy_fx=None, tidx=None, where=MCRT_HOST):
     _check(load_library().mcrt_read_component(ctx, int(component), _ptr(E_abs_count), _ptr(E_abs_lucy), _ptr(T_count),
@@ -402,6 +418,10 @@ class Context:
         mcrt_dust_tables(self.ctx, w.nu_hz, w.kappa_abs, w.kappa_sca, w.g, w.T_grid)
         if getattr(w, "mixtures", None) is not None:
             mcrt_dust_mixtures(self.ctx, *w.mixtures)
+        self.n_subcells = 0
+        if getattr(w, "subgrid", None) is not None:
+            mcrt_subgrid(self.ctx, *w.subgrid)
+            self.n_subcells = len(w.subgrid[1]) * int(w.subgrid[0]) ** 3
         mcrt_source(self.ctx, w.L_erg_s, w.T_star_K, w.L_nu_weights, w.source_pos_cm)
         mcrt_escape_bins(self.ctx, w.abs_mu_edges)
         self.last_n = 0
@@ -449,6 +469,15 @@ class Context:
         if digests:
             out["digests"] = dig
         return out
+
+    def read_subcells(self):
+        """Outputs and raw tallies of the sub-cubes (mcrt_subgrid), in its order."""
+        n = self.n_subcells
+        Ec, El = np.zeros(n), np.zeros(n)
+        Tc, Tl = np.zeros(n, np.float32), np.zeros(n, np.float32)
+        k, L, tidx = np.zeros(n, np.uint64), np.zeros(n, np.int64), np.zeros(n, np.uint16)
+        mcrt_read_subcells(self.ctx, Ec, El, Tc, Tl, k, L, tidx)
+        return {"E_count": Ec, "E_lucy": El, "T_count": Tc, "T_lucy": Tl, "k": k, "lucy_fx": L, "tidx": tidx}
 
     def read_component(self, component):
         """Outputs and raw tallies of one component of the mixtures (mcrt_dust_mixtures)."""

@@ -38,7 +38,7 @@ constexpr double kFourPi = 12.566370614359172953850573533118;
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kHot = 511;            // most hot cells around the source (see cw_hot)
 
-enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4, ST_STOP = 5 };
+enum : int { ST_IDLE = 0, ST_JUMP = 1, ST_INTERACT = 2, ST_FLY = 3, ST_DONE = 4, ST_STOP = 5, ST_SUB = 6 };
 enum : int { EV_EMIT = 0, EV_SCATTER = 1, EV_ABSORB = 2, EV_ESCAPE = 3 };
 
 // device counters (unsigned long long each)
@@ -130,6 +130,11 @@ struct mcrt_ctx {
     long long *lfx1 = nullptr;
     unsigned long long *kcnt1 = nullptr, *kprev1 = nullptr;
     uint16_t *tidx1 = nullptr;
+    // sub-cubes (mcrt_subgrid; NEXT-3): refined cubes carry a marker word with their block number; their sub-cubes' arrays (cudaMalloc)
+    int subR = 0, sub_shift = 0;
+    size_t n_sub = 0, n_subcells = 0;
+    unsigned long long *sub_cellw = nullptr, *sub_kcnt = nullptr, *sub_kprev = nullptr;
+    long long *sub_lfx = nullptr;
     // thresholded Lucy estimator (mcrt_run_opts.lucy_hybrid; Sect. 3.1)
     bool hybrid = false;                           // the stored tallies were made with it
     double *d_kmax_diag = nullptr;                 // [ns] sqrt(3) h max_nu (kabs + ksca) (cudaMalloc)
@@ -500,6 +505,14 @@ struct TransportParams {
     const double2 *__restrict__ mx_thr;        // [ns][nf] {S0, A0}: thresholds of the event uniform
     const int *__restrict__ mx_mat;            // [ns][2] material of each component
     // thresholded Lucy estimator (Sect. 3.1, readings Q37 / Q38): NULL = the linear tally in every cell
+    // sub-cubes (NEXT-3, reading Q40): subR = 0 none.  A refined cube's cell word is a marker with kSubFlag and its block
+    // number << kSubShift; sub-cube (gx, gy, gz) of block b is cell b R^3 + (gz R + gy) R + gx of the sub arrays
+    int subR, sub_shift;
+    const unsigned long long *__restrict__ sub_cellw;
+    long long *__restrict__ sub_lfx;
+    unsigned long long *__restrict__ sub_kcnt;
+    unsigned long long sub_n;                  // number of sub-cubes
+    unsigned long long nc_grid;                // cells of the grid: a sub-cube's number in digests is nc_grid + its index
     int redraw;                                // 1: a new optical depth is drawn on entering every cell (as printed)
     const double *__restrict__ kmax_diag;      // [ns] sqrt(3) h max_nu (kabs + ksca): a cell is tallied if rho * this < 10^-2
     double two_fx, inv_two_fx;                 // 2^FX, 2^-FX
@@ -652,6 +665,12 @@ __device__ __forceinline__ int unpack_z(uint32_t w) { return (int)(w >> 22); }
 constexpr unsigned long long kJumpWord = 0x7FF0000000000000ull;
 constexpr uint32_t kMarkHi = 0x7FF00000u, kOutFlag = 0x100u;
 constexpr unsigned long long kOutWord = kJumpWord | kOutFlag;
+// ... and so does the word of a cube that is divided into sub-cubes (mcrt_subgrid): kSubFlag and its block number
+constexpr uint32_t kSubFlag = 0x200u;
+constexpr int kSubShift = 10;
+// state of a packet inside a divided cube, kept in the upper half of slot word U_W1: sub-cube coordinates, "valid"
+constexpr uint32_t kSubOk = 1u << 25;
+__device__ __forceinline__ uint32_t sub_pack(int gx, int gy, int gz) { return kSubOk | ((uint32_t)gx << 16) | ((uint32_t)gy << 19) | ((uint32_t)gz << 22); }
 // Storage order of the per-cell arrays (cell words, Lucy tally, absorption counts): linear, x fastest, with a shell
 // of kGuard cells around the grid that hold the "outside the grid" marker word:
 //     index(ix, iy, iz) = ((iz + kGuard) * PY + (iy + kGuard)) * PX + (ix + kGuard),  PX = nx + 2 kGuard, PY = ny + 2 kGuard.
@@ -811,13 +830,15 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
     __syncwarp();
     // warp-uniform slot sets: parked flying packets / packets inside a run of empty bricks / packets waiting for an event
     SlotSet mFly, mJ, mEv;
+    SlotSet mSub;                                  // packets inside a cube divided into sub-cubes (XTRA kernels only)
+    mSub.clear();
     mFly.clear(); mJ.clear(); mEv.fill();
     bool exhausted = false;                        // the epoch counter has run out (warp-uniform)
     uint32_t ndusty_acc = 0u;                      // dusty crossings stepped by this lane
 
     for (;;) {
-        const int nfly = mFly.count(), njmp = mJ.count(), nevt = mEv.count();
-        if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0)) {
+        const int nfly = mFly.count(), njmp = mJ.count(), nevt = mEv.count(), nsub = XTRA ? mSub.count() : 0;
+        if (nfly >= MCRT_S_ENTER || (nfly > 0 && njmp == 0 && nevt == 0 && nsub == 0)) {
             // =========================================================== S phase: S4/S5 cell walk
             // Software pipeline.  The path of a flight does not depend on the cells' contents, so the geometry
             // (G: axis choice, next cell, exit parameter) runs ahead of the physics: in the step that handles cell n,
@@ -882,6 +903,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 #endif
                         const bool mk = (uint32_t)(scw >> 32) == kMarkHi;
                         state = mk ? (((uint32_t)scw & kOutFlag) ? ST_DONE : ST_JUMP) : ST_INTERACT;
+                        if (XTRA && mk && ((uint32_t)scw & kSubFlag)) state = ST_SUB;   // a cube divided into sub-cubes
                         if (state == ST_DONE) SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
                         else {
                             SU(U_W0, slot) = index_to_packed(SU(U_W0, slot), px_r, pxy_r, P.inv_lpx, P.inv_lpxy);   // the walk stored the index
@@ -889,12 +911,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         }
                     }
                     mJ.add(state == ST_JUMP, slot);
+                    if (XTRA) mSub.add(state == ST_SUB, slot);
                     mEv.add(state == ST_DONE || state == ST_INTERACT, slot);
                     if (state != ST_FLY) state = ST_IDLE;
                     const unsigned idle = __ballot_sync(kFull, state == ST_IDLE);
                     const int nfl = 32 - __popc(idle);
                     // nothing left to refill with and many lanes idle: let the other phases make flying packets
-                    if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty())))) {
+                    if (mFly.empty() && (nfl == 0 || (nfl <= 32 - MCRT_S_LEAVE && !(mJ.empty() && mEv.empty() && mSub.empty())))) {
                         // park mid-flight: cell n, entered at tprev.  A packet still behind its no-op cell has not
                         // started: its slot is as the refill found it
                         // (its crossing count is still below the slot's)
@@ -1122,6 +1145,132 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
 #undef WALK_STEP
             }
             __syncwarp();
+        } else if (XTRA && nsub > 0 && nsub >= nevt && nsub >= njmp) {
+            // =========================================================== R phase: cubes divided into sub-cubes (NEXT-3)
+            // Each lane takes one packet that stands in a divided cube and walks its sub-cubes one by one -- the same
+            // walk on the lattice of sub-cube faces f = c + k/R (reading Q40), not pipelined -- through any further
+            // divided cubes, until it interacts (E phase), reaches an undivided cube (back to the pool) or escapes.
+            const int nr = min(nsub, 32);
+            const bool act = lane < nr;
+            const int slot = act ? mSub.nth(lane) : 0;
+            const int R = P.subR, R3 = R * R * R;
+            const double Rd = (double)R;
+            bool busy = act, escaped = false, hit = false;
+            double px = 0.0, py = 0.0, pz = 0.0, ux = 0.0, uy = 0.0, uz = 0.0, ivx = 0.0, ivy = 0.0, ivz = 0.0;
+            double t = 0.0, tau = 0.0, fx = 0.0, fy = 0.0, fz = 0.0;
+            int ix = 0, iy = 0, iz = 0, gx = 0, gy = 0, gz = 0, stx = 0, sty = 0, stz = 0, j = 0;
+            uint32_t ncross = 0u, blk = 0u, rbase = 0u;
+            unsigned long long rpid = 0ull, fw = 0ull, pw = 0ull;
+            bool g_ok = false, need_cube = true;
+            if (act) {
+                px = SF(F_PX, slot); py = SF(F_PY, slot); pz = SF(F_PZ, slot);
+                ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
+                ivx = (ux != 0.0) ? 1.0 / ux : CUDART_INF;
+                ivy = (uy != 0.0) ? 1.0 / uy : CUDART_INF;
+                ivz = (uz != 0.0) ? 1.0 / uz : CUDART_INF;
+                stx = (ux > 0.0) ? 1 : ((ux < 0.0) ? -1 : 0);
+                sty = (uy > 0.0) ? 1 : ((uy < 0.0) ? -1 : 0);
+                stz = (uz > 0.0) ? 1 : ((uz < 0.0) ? -1 : 0);
+                t = SF(F_T, slot); tau = SF(F_TAU, slot);
+                const uint32_t w0 = SU(U_W0, slot), w1 = SU(U_W1, slot);
+                ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0);
+                ncross = SU(U_NCROSS, slot);
+                j = (int)(w1 & 0xffffu);
+                g_ok = (w1 & kSubOk) != 0u;
+                gx = (int)((w1 >> 16) & 7u); gy = (int)((w1 >> 19) & 7u); gz = (int)((w1 >> 22) & 7u);
+                if (P.redraw) { rpid = (unsigned long long)__double_as_longlong(SF(F_PID, slot)); rbase = SU(U_DK, slot) & 0x3fffffffu; }
+            }
+            do {
+                if (busy) {
+                    if (need_cube) {
+                        pw = __ldg(P.cellw + (size_t)kCS * lin_index(ix, iy, iz, lpx, lpxy));
+                        if (!((uint32_t)(pw >> 32) == kMarkHi && ((uint32_t)pw & kSubFlag))) { busy = false; g_ok = false; }
+                        else {
+                            blk = (uint32_t)pw >> kSubShift;
+                            if (!g_ok) {   // entered from an undivided cube: the sub-cube that holds the entry point p + u t
+                                int q;
+                                q = (int)floor(((px + ux * t) - (double)ix) * Rd); gx = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                                q = (int)floor(((py + uy * t) - (double)iy) * Rd); gy = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                                q = (int)floor(((pz + uz * t) - (double)iz) * Rd); gz = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                                g_ok = true;
+                            }
+                            fx = stx ? (((double)ix + (double)(gx + (stx > 0 ? 1 : 0)) / Rd) - px) * ivx : CUDART_INF;
+                            fy = sty ? (((double)iy + (double)(gy + (sty > 0 ? 1 : 0)) / Rd) - py) * ivy : CUDART_INF;
+                            fz = stz ? (((double)iz + (double)(gz + (stz > 0 ? 1 : 0)) / Rd) - pz) * ivz : CUDART_INF;
+                            need_cube = false;
+                        }
+                    }
+                    if (busy) {
+                        const bool selx = (fx <= fy) && (fx <= fz), sely = !selx && (fy <= fz);
+                        const double tn = selx ? fx : (sely ? fy : fz);
+                        const double ds = tn - t;
+                        const uint32_t fidx = blk * (uint32_t)R3 + (uint32_t)((gz * R + gy) * R + gx);
+                        MCRT_CHK(fidx < (uint32_t)P.sub_n, "sub-cube index");
+                        fw = __ldg(P.sub_cellw + (size_t)kCS * fidx);
+                        const double rho_c = cw_rho(fw);
+                        const double2 kq = s_kk[cw_species(fw) * nf + j];
+                        if (P.redraw) {
+                            double zr0, zr1;
+                            draw2(P.seed_lo, P.seed_hi, rpid, (rbase + ncross) & 0x3fffffffu, P.pass, zr0, zr1);
+                            tau = -traj_log(zr0);
+                        }
+                        const double dtau = kq.x * rho_c * ds;
+                        if (!(dtau <= tau)) { hit = true; busy = false; }
+                        else {
+                            tau -= dtau;
+                            if (__double2hiint(rho_c) != 0) { lucy_add(P.sub_lfx, fidx, kq.y * rho_c * ds); ndusty_acc++; }
+                            t = tn;
+                            ncross++;
+                            if (selx) {
+                                gx += stx;
+                                if ((unsigned)gx >= (unsigned)R) { gx = stx > 0 ? 0 : R - 1; ix += stx; need_cube = true; }
+                                else fx = (((double)ix + (double)(gx + (stx > 0 ? 1 : 0)) / Rd) - px) * ivx;
+                            } else if (sely) {
+                                gy += sty;
+                                if ((unsigned)gy >= (unsigned)R) { gy = sty > 0 ? 0 : R - 1; iy += sty; need_cube = true; }
+                                else fy = (((double)iy + (double)(gy + (sty > 0 ? 1 : 0)) / Rd) - py) * ivy;
+                            } else {
+                                gz += stz;
+                                if ((unsigned)gz >= (unsigned)R) { gz = stz > 0 ? 0 : R - 1; iz += stz; need_cube = true; }
+                                else fz = (((double)iz + (double)(gz + (stz > 0 ? 1 : 0)) / Rd) - pz) * ivz;
+                            }
+                            if (need_cube) {
+                                escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) | ((unsigned)iz >= (unsigned)P.nz);
+                                if (escaped) busy = false;
+                            }
+                        }
+                    }
+                }
+            } while (__popc(__ballot_sync(kFull, busy)) >= max(min(nr, MCRT_J_MIN), 1));
+            bool to_jump = false;
+            if (act) {
+                SF(F_T, slot) = t; SF(F_TAU, slot) = tau;
+                SU(U_NCROSS, slot) = ncross;
+                const uint32_t w1 = SU(U_W1, slot) & 0xffffu;
+                if (escaped) {
+                    SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_ESCAPED << 30);
+                    SU(U_W1, slot) = w1;
+                } else {
+                    SU(U_W0, slot) = pack_xyz(ix, iy, iz);
+                    if (hit) {              // interaction inside sub-cube g: the E phase finds it by the flag in U_W1
+                        SU(U_DK, slot) = (SU(U_DK, slot) & 0x3fffffffu) | (K_INTERACT << 30);
+                        SF(F_CW, slot) = __longlong_as_double((long long)fw);
+                        SU(U_W1, slot) = w1 | sub_pack(gx, gy, gz);
+                    } else if (busy) {      // still inside: stays in the set
+                        SU(U_W1, slot) = w1 | (need_cube ? (g_ok ? sub_pack(gx, gy, gz) : 0u) : sub_pack(gx, gy, gz));
+                    } else {                // an undivided cube: back to the walk (or to the jumps, if its brick is empty)
+                        SF(F_CW, slot) = __longlong_as_double((long long)pw);
+                        SU(U_W1, slot) = w1;
+                        to_jump = brick_empty(s_m0, brick_of(ix, iy, iz, nbx, nby, bsh));
+                    }
+                }
+            }
+            const bool mine = act && !busy;
+            mSub.remove(mine, slot);
+            mEv.add(mine && (escaped || hit), slot);
+            mFly.add(mine && !escaped && !hit && !to_jump, slot);
+            mJ.add(mine && !escaped && !hit && to_jump, slot);
+            __syncwarp();
         } else if (njmp > 0 && njmp >= nevt) {
             // =========================================================== J phase: runs of empty bricks
             // Each lane takes one packet whose current cell lies in an empty brick and crosses, one box per
@@ -1202,6 +1351,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             uint32_t ncross = 0u, nsca = 0u, nabs = 0u, nint = 0u;
             int ix = 0, iy = 0, iz = 0, j = 0;
             double ux = 0.0, uy = 0.0, uz = 1.0;
+            bool insub = false;                         // the event happened / the new flight starts inside sub-cube (sgx, sgy, sgz)
+            int sgx = 0, sgy = 0, sgz = 0;
             if (act && kind != K_EMIT) {
                 pid = (unsigned long long)__double_as_longlong(SF(F_PID, slot));
                 if (RECORD) hash = (unsigned long long)__double_as_longlong(SF(F_HASH, slot));
@@ -1209,6 +1360,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 const uint32_t w0 = SU(U_W0, slot);
                 ix = unpack_x(w0); iy = unpack_y(w0); iz = unpack_z(w0);
                 j = (int)(SU(U_W1, slot) & 0xffffu); nint = SU(U_W1, slot) >> 16;
+                if (XTRA && P.subR) {       // (no carry-over on divided grids: the upper half of U_W1 is the sub-cube state)
+                    insub = kind == K_INTERACT && (SU(U_W1, slot) & kSubOk) != 0u;
+                    sgx = (int)(nint & 7u); sgy = (int)((nint >> 3) & 7u); sgz = (int)((nint >> 6) & 7u);
+                    nint = 0u;
+                }
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
                 // per-cell redraw: the slot holds (index of the flight's draw) - (crossings at its start); every cell
                 // entered since has used one more draw (see the walk), so the next free index is
@@ -1315,6 +1471,12 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const double kk = kq.x * rho_c;
                     const double sint = tau / kk;
                     const uint32_t hid = HOT ? cw_hot(cw, P.hot_shift, P.hot_mask) : 0u;
+                    uint32_t fidx = 0u;                        // the sub-cube's index in the sub arrays
+                    if (XTRA && insub) {
+                        const unsigned long long pw = __ldg(P.cellw + (size_t)kCS * cidx);     // the divided cube's marker: its block
+                        fidx = ((uint32_t)pw >> kSubShift) * (uint32_t)(P.subR * P.subR * P.subR) + (uint32_t)((sgz * P.subR + sgy) * P.subR + sgx);
+                        lucy_add(P.sub_lfx, fidx, kq.y * rho_c * sint);
+                    } else
                     if (hid) hot_add(s_hot, hid, lucy_round(kq.y * rho_c * sint));
                     else if (XTRA && P.kmax_diag) {           // Sect. 3.1: Eq. 9, cells below the threshold only
                         if (rho_c * P.kmax_diag[cw_species(cw)] < kThinTau)
@@ -1329,10 +1491,17 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }
                     const double tint = t + sint;
                     double q;
+                    if (XTRA && insub) {    // the interaction point stays inside its sub-cube
+                        const double Rd = (double)P.subR;
+                        q = px + ux * tint; q = fmax(q, (double)ix + (double)sgx / Rd); q = fmin(q, (double)ix + (double)(sgx + 1) / Rd); px = q;
+                        q = py + uy * tint; q = fmax(q, (double)iy + (double)sgy / Rd); q = fmin(q, (double)iy + (double)(sgy + 1) / Rd); py = q;
+                        q = pz + uz * tint; q = fmax(q, (double)iz + (double)sgz / Rd); q = fmin(q, (double)iz + (double)(sgz + 1) / Rd); pz = q;
+                    } else {
                     q = px + ux * tint; q = fmax(q, (double)ix); q = fmin(q, (double)(ix + 1)); px = q;
                     q = py + uy * tint; q = fmax(q, (double)iy); q = fmin(q, (double)(iy + 1)); py = q;
                     q = pz + uz * tint; q = fmax(q, (double)iz); q = fmin(q, (double)(iz + 1)); pz = q;
-                    const unsigned long long cell = ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
+                    }
+                    const unsigned long long cell = (XTRA && insub) ? P.nc_grid + fidx : ((unsigned long long)iz * P.ny + iy) * P.nx + ix;
                     // S6 scatter with probability albedo
                     if (ztype < s_ag[sj].x) {
                         scatter = true;
@@ -1369,7 +1538,8 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             // depends on the order of the atomics: results are reproducible only statistically.
                             const unsigned long long kn = atomicAdd(&P.kcnt[cidx], 1ull) + 1ull;
                             m = t_index(P.J + s * P.nT, P.nT, (double)kn * P.cellfac / rho_c);
-                        } else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
+                        } else if (XTRA && insub) atomicAdd(&P.sub_kcnt[fidx], 1ull);
+                        else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
                         else if (XTRA && second) atomicAdd(&P.kcnt1[cidx], 1ull);
                         else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
@@ -1424,6 +1594,15 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     cidx = lin_index(ix, iy, iz, lpx, lpxy);
                     to_jump = brick_empty(s_m0, brick);
                     cw = to_jump ? 0ull : __ldg(P.cellw + (size_t)kCS * cidx);
+                    if (XTRA && P.subR && (uint32_t)(cw >> 32) == kMarkHi && ((uint32_t)cw & kSubFlag)) {
+                        // the source stands in a divided cube: the same start rule on the lattice of sub-cube faces
+                        const double Rd = (double)P.subR;
+                        double pf;
+                        pf = px * Rd; f = floor(pf); sgx = ((pf != f) ? (int)f : ((ux >= 0.0) ? (int)f : (int)f - 1)) - ix * P.subR;
+                        pf = py * Rd; f = floor(pf); sgy = ((pf != f) ? (int)f : ((uy >= 0.0) ? (int)f : (int)f - 1)) - iy * P.subR;
+                        pf = pz * Rd; f = floor(pf); sgz = ((pf != f) ? (int)f : ((uz >= 0.0) ? (int)f : (int)f - 1)) - iz * P.subR;
+                        insub = true;
+                    }
                     if (RECORD)
                         hash_mix(hash, event_word(EV_EMIT, j, ((unsigned long long)iz * P.ny + iy) * P.nx + ix));
                 } else if (XTRA && P.carry_K && ++nint >= P.carry_K) {
@@ -1460,11 +1639,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 SU(U_DK, slot) = (XTRA && P.redraw) ? ((d - 1u - ncross) & 0x3fffffffu) : d;
                 SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
                 SU(U_W0, slot) = pack_xyz(ix, iy, iz);
-                SU(U_W1, slot) = (uint32_t)j | (nint << 16);
+                SU(U_W1, slot) = (uint32_t)j | (nint << 16) | ((XTRA && insub) ? sub_pack(sgx, sgy, sgz) : 0u);
                 }   // !carried
             }
             mEv.remove(act && !carried, slot);             // taken: now flying, jumping, or dead (no packets left)
-            mFly.add(act && !dead && !to_jump && !carried, slot);
+            const bool to_sub = XTRA && insub && act && !dead && !carried;      // the new flight starts inside a sub-cube
+            if (XTRA) mSub.add(to_sub, slot);
+            mFly.add(act && !dead && !to_jump && !carried && !to_sub, slot);
             mJ.add(act && !dead && to_jump && !carried, slot);
             __syncwarp();
         } else {
@@ -1749,6 +1930,36 @@ __global__ void k_pack_grid(const float *__restrict__ rho, const uint8_t *__rest
     }
 }
 
+// mcrt_subgrid: packs the sub-cubes' cell words and turns the divided cubes' words into markers with their block number.
+// bad[0] counts divided cubes whose own density is not > 0 (their brick would count as empty), bad[1] bad sub-cubes.
+__global__ void k_pack_sub(unsigned long long *__restrict__ cellw, unsigned long long *__restrict__ sub_cellw,
+                           const long long *__restrict__ cube, const float *__restrict__ rho, const uint8_t *__restrict__ sp,
+                           size_t n_sub, int R3, int nx, int ny, int nz, int px, int pxy, int ns, unsigned long long *__restrict__ bad)
+{
+    const size_t n = n_sub * (size_t)R3;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float r = rho[i];
+        const uint32_t s = sp[i];
+        if (!(r >= 0.0f) || isinf(r) || s >= (uint32_t)ns) atomicAdd(&bad[1], 1ull);
+        const double rd = (r > 0.0f && !isinf(r)) ? (double)r : 0.0;
+        sub_cellw[kCS * i] = ((unsigned long long)__double_as_longlong(rd) & kRhoMask) | (unsigned long long)(s & 0xffu);
+        if (i % (size_t)R3 == 0) {
+            const size_t b = i / (size_t)R3;
+            const long long ci = cube[b];
+            const int ix = (int)(ci % nx), iy = (int)((ci / nx) % ny), iz = (int)(ci / ((long long)nx * ny));
+            unsigned long long *w = cellw + (size_t)kCS * lin_index(ix, iy, iz, px, pxy);
+            if (!cw_dusty(*w)) atomicAdd(&bad[0], 1ull);
+            *w = kJumpWord | kSubFlag | ((unsigned long long)b << kSubShift);
+        }
+    }
+}
+
+// the outputs of mcrt_read / mcrt_read_raw for the sub-cubes (identity order; Eq. 4 with V = (h/R)^3 through cellfac)
+__global__ void k_gather_sub(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
+                             const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
+                             const double *__restrict__ J, const double *__restrict__ Tg, int nT, size_t off, size_t n, double xi,
+                             double inv_fx, double cellfac, uint32_t tmask);
+
 // The species byte of a vacuum cell means nothing (rho = 0 makes every product of the walk 0), but the walk reloads its
 // cached opacities whenever the byte changes.  So a vacuum cell inside a dusty brick takes the species of the nearest
 // dusty cell along the axes (fixed search order, up to kVacReach cells: deterministic; only dusty cells are read for
@@ -1898,7 +2109,9 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
         switch (what) {
         case G_K: reinterpret_cast<unsigned long long *>(out)[i] = kcnt[b]; break;
         case G_LFX: reinterpret_cast<long long *>(out)[i] = lfx[bs]; break;
-        case G_TIDX: reinterpret_cast<uint16_t *>(out)[i] = comp ? tidx1[b] : (uint16_t)cw_tidx(cellw[bs], tmask); break;
+        case G_TIDX:    // (a marker word -- the cube is divided into sub-cubes -- has no temperature index)
+            reinterpret_cast<uint16_t *>(out)[i] = comp ? tidx1[b] : (cw_dusty(cellw[bs]) ? (uint16_t)cw_tidx(cellw[bs], tmask) : (uint16_t)0);
+            break;
         case G_ECOUNT: reinterpret_cast<double *>(out)[i] = (double)kcnt[b] * xi; break;
         case G_ELUCY: reinterpret_cast<double *>(out)[i] = (double)lfx[bs] * inv_fx * xi; break;
         default: {
@@ -1916,6 +2129,33 @@ __global__ void k_gather(int what, void *__restrict__ out, const unsigned long l
                 }
             }
             reinterpret_cast<float *>(out)[i] = T;
+        }
+        }
+    }
+}
+
+__global__ void k_gather_sub(int what, void *__restrict__ out, const unsigned long long *__restrict__ cellw,
+                             const unsigned long long *__restrict__ kcnt, const long long *__restrict__ lfx,
+                             const double *__restrict__ J, const double *__restrict__ Tg, int nT, size_t off, size_t n, double xi,
+                             double inv_fx, double cellfac, uint32_t tmask)
+{
+    // sub-cubes off .. off + n - 1 to out[0 .. n - 1]
+    for (size_t o = (size_t)blockIdx.x * blockDim.x + threadIdx.x; o < n; o += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = off + o, bs = (size_t)kCS * i;
+        switch (what) {
+        case G_K: reinterpret_cast<unsigned long long *>(out)[o] = kcnt[i]; break;
+        case G_LFX: reinterpret_cast<long long *>(out)[o] = lfx[bs]; break;
+        case G_TIDX: reinterpret_cast<uint16_t *>(out)[o] = (uint16_t)cw_tidx(cellw[bs], tmask); break;
+        case G_ECOUNT: reinterpret_cast<double *>(out)[o] = (double)kcnt[i] * xi; break;
+        case G_ELUCY: reinterpret_cast<double *>(out)[o] = (double)lfx[bs] * inv_fx * xi; break;
+        default: {
+            const unsigned long long cw = cellw[bs];
+            float T = 0.0f;
+            if (cw_dusty(cw)) {
+                const double e = (what == G_TLUCY) ? (double)lfx[bs] * inv_fx : (double)kcnt[i];
+                T = (float)T_of_x(J + cw_species(cw) * nT, Tg, nT, e * cellfac / cw_rho(cw));
+            }
+            reinterpret_cast<float *>(out)[o] = T;
         }
         }
     }
@@ -2482,6 +2722,96 @@ int mcrt_dust_tables(mcrt_ctx *c, int n_nu, const double *nu_hz, const double *k
     return MCRT_OK;
 }
 
+static int apply_hot(mcrt_ctx *c, int n_use);
+static int check_overflow(mcrt_ctx *c);
+
+int mcrt_subgrid(mcrt_ctx *c, int R, uint64_t n_sub, const int64_t *cube, const float *rho_sub, const uint8_t *species_sub)
+{
+    if (!c) return MCRT_EINVAL;
+    if (c->subR) return fail(c, MCRT_ESTATE, "mcrt_subgrid may be called once per context");
+    if (c->last_n || c->run.active) return fail(c, MCRT_ESTATE, "mcrt_subgrid after a run");
+    if (c->mix) return fail(c, MCRT_EINVAL, "mcrt_subgrid is not available with dust mixtures");
+    if (R != 2 && R != 4 && R != 8) return fail(c, MCRT_EINVAL, "R must be 2, 4 or 8");
+    if (n_sub < 1 || n_sub > ((uint64_t)1 << 22) || !cube || !rho_sub || !species_sub) return fail(c, MCRT_EINVAL, "1 <= n_sub <= 2^22 divided cubes");
+    const size_t R3 = (size_t)R * R * R, n = (size_t)n_sub * R3;
+    {
+        std::vector<int64_t> sorted(cube, cube + n_sub);
+        std::sort(sorted.begin(), sorted.end());
+        if (sorted.front() < 0 || (uint64_t)sorted.back() >= c->nc) return fail(c, MCRT_EINVAL, "cube index out of range");
+        for (size_t i = 1; i < sorted.size(); ++i)
+            if (sorted[i] == sorted[i - 1]) return fail(c, MCRT_EINVAL, "a cube is listed twice");
+    }
+    long long *d_cube = nullptr; float *d_rho = nullptr; uint8_t *d_sp = nullptr;
+    bool ok = cudaMalloc((void **)&c->sub_cellw, n * kCS * 8) == cudaSuccess && cudaMalloc((void **)&c->sub_lfx, n * kCS * 8) == cudaSuccess &&
+              cudaMalloc((void **)&c->sub_kcnt, n * 8) == cudaSuccess && cudaMalloc((void **)&c->sub_kprev, n * 8) == cudaSuccess &&
+              cudaMalloc((void **)&d_cube, n_sub * 8) == cudaSuccess && cudaMalloc((void **)&d_rho, n * 4) == cudaSuccess &&
+              cudaMalloc((void **)&d_sp, n) == cudaSuccess;
+    int rc = MCRT_OK;
+    unsigned long long bad[2] = {0ull, 0ull};
+    unsigned long long *d_bad = c->counters + CNT_N;
+    cudaError_t e = cudaSuccess;
+    if (!ok) rc = fail(c, MCRT_ENOMEM, "cudaMalloc of the sub-cube arrays failed");
+    if (!rc) {
+        e = cudaMemcpyAsync(d_cube, cube, n_sub * 8, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_rho, rho_sub, n * 4, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_sp, species_sub, n, cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(d_bad, 0, 16, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->sub_lfx, 0, n * kCS * 8, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->sub_kcnt, 0, n * 8, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->sub_kprev, 0, n * 8, c->stream);
+        if (e == cudaSuccess) {
+            k_pack_sub<<<stream_grid(n), 256, 0, c->stream>>>(c->cellw, c->sub_cellw, d_cube, d_rho, d_sp, (size_t)n_sub, (int)R3, c->nx, c->ny,
+                                                             c->nz, c->px, c->pxy, c->ns, d_bad);
+            e = cudaGetLastError();
+        }
+        if (e == cudaSuccess) e = cudaMemcpyAsync(bad, d_bad, 16, cudaMemcpyDeviceToHost, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = fail(c, MCRT_ECUDA, cudaGetErrorString(e));
+    }
+    cudaFree(d_cube); cudaFree(d_rho); cudaFree(d_sp);
+    if (!rc && bad[0]) rc = fail(c, MCRT_EINVAL, "a divided cube must have a density > 0 in the grid (a placeholder: its dust is in its sub-cubes)");
+    if (!rc && bad[1]) rc = fail(c, MCRT_EINVAL, "sub-cube densities must be finite and >= 0, species < n_species");
+    if (rc) return rc;      // (the context is unusable after a failure that has already rewritten cell words: destroy it)
+    c->subR = R; c->sub_shift = R == 2 ? 1 : (R == 4 ? 2 : 3); c->n_sub = (size_t)n_sub; c->n_subcells = n;
+    // no per-CTA copies of tallies on divided grids (a cell near the source may be a divided cube)
+    if ((rc = apply_hot(c, 0))) return rc;
+    c->hot_cand.clear();
+    return MCRT_OK;
+}
+
+int mcrt_read_subcells(mcrt_ctx *c, double *E_abs_count, double *E_abs_lucy, float *T_count, float *T_lucy, uint64_t *k_abs,
+                       int64_t *lucy_fx, uint16_t *tidx, mcrt_mem where)
+{
+    if (!c) return MCRT_EINVAL;
+    if (!c->subR) return fail(c, MCRT_ESTATE, "mcrt_read_subcells without mcrt_subgrid");
+    if (!c->last_n) return fail(c, MCRT_ESTATE, "mcrt_read_subcells before mcrt_run");
+    if (c->run.active) return fail(c, MCRT_ESTATE, "mcrt_read_subcells inside mcrt_run_begin .. mcrt_run_end");
+    int rc = check_overflow(c);
+    if (rc) return rc;
+    const double hs = c->h / (double)c->subR;
+    const double cellfac = c->xi / (kFourPi * hs * hs * hs);
+    struct { int what; void *dst; size_t elem; } outs[7] = {{G_ECOUNT, E_abs_count, 8}, {G_ELUCY, E_abs_lucy, 8}, {G_TCOUNT, T_count, 4},
+                                                            {G_TLUCY, T_lucy, 4}, {G_K, k_abs, 8}, {G_LFX, lucy_fx, 8}, {G_TIDX, tidx, 2}};
+    for (auto &o : outs) {
+        if (!o.dst) continue;
+        // host reads are staged through the context's scratch array (one value per grid cell), a piece at a time
+        const size_t piece = (where == MCRT_DEVICE) ? c->n_subcells : std::min(c->n_subcells, c->nc);
+        for (size_t off = 0; off < c->n_subcells; off += piece) {
+            const size_t n = std::min(piece, c->n_subcells - off);
+            void *dev = (where == MCRT_DEVICE) ? o.dst : c->scratch;
+            k_gather_sub<<<stream_grid(n), 256, 0, c->stream>>>(o.what, dev, c->sub_cellw, c->sub_kcnt, c->sub_lfx, c->d_J, c->d_Tg, c->nT, off,
+                                                               n, c->xi, ldexp(1.0, -c->fx), cellfac, c->tidx_mask);
+            CUDA_TRY(c, cudaGetLastError());
+            if (where == MCRT_HOST) {
+                CUDA_TRY(c, cudaMemcpyAsync((char *)o.dst + off * o.elem, dev, n * o.elem, cudaMemcpyDeviceToHost, c->stream));
+                CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+            }
+        }
+    }
+    CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    return MCRT_OK;
+}
+
 int mcrt_dust_mixtures(mcrt_ctx *c, const int32_t *n_components, const int32_t *material, const double *fraction)
 {
     if (!c) return MCRT_EINVAL;
@@ -2717,7 +3047,7 @@ static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, in
             if (smem_carveout(transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, t, record, 0)) <= 164 * 1024) { *threads = t; break; }
     const size_t base = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, 0);
     // ... and as many hot cells as the carve-out these need leaves room for (live B&W needs every count in global memory)
-    int nh = (c->mix || (o && (o->no_hot_cells || o->lucy_hybrid || o->mode == MCRT_MODE_LIVE_BW))) ? 0 : (int)c->hot_cand.size();
+    int nh = (c->mix || c->subR || (o && (o->no_hot_cells || o->lucy_hybrid || o->mode == MCRT_MODE_LIVE_BW))) ? 0 : (int)c->hot_cand.size();
     const size_t cap = smem_carveout(base) - kSmemOverhead;
     while (nh > 0 && transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh) > cap) --nh;
     if (nh < 8) nh = 0;
@@ -2805,6 +3135,8 @@ static void fill_params(mcrt_ctx *c, TransportParams &P)
         P.mx_thr = reinterpret_cast<const double2 *>(c->d_mx_thr); P.mx_mat = c->d_mx_mat;
     }
     P.redraw = c->run.o.tau_redraw_per_cell ? 1 : 0;
+    P.subR = c->subR; P.sub_shift = c->sub_shift; P.sub_cellw = c->sub_cellw; P.sub_lfx = c->sub_lfx; P.sub_kcnt = c->sub_kcnt;
+    P.sub_n = c->n_subcells; P.nc_grid = c->nc;
     if (c->run.o.lucy_hybrid) { P.kmax_diag = c->d_kmax_diag; P.two_fx = ldexp(1.0, c->fx); P.inv_two_fx = ldexp(1.0, -c->fx); }
     P.dig = c->run.o.record_digests ? c->dig : nullptr;
     P.dig_base = c->dig_base; P.dig_n = c->dig_n;
@@ -2926,6 +3258,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     if (o.first_packet_id + n_packets < o.first_packet_id) return fail(c, MCRT_EINVAL, "packet ids overflow 64 bits");
     if (c->mix && (o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
         return fail(c, MCRT_EINVAL, "dust mixtures are not available in live B&W or partitioned runs");
+    if (c->subR && (o.carry_interactions || o.lucy_hybrid || o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
+        return fail(c, MCRT_EINVAL, "grids with sub-cubes: no carry-over, thresholded estimator, live B&W or partitioned runs");
     if (o.tau_redraw_per_cell && (o.carry_interactions || o.mode == MCRT_MODE_LIVE_BW))
         return fail(c, MCRT_EINVAL, "tau_redraw_per_cell is not available with carry-over or in live B&W");
     if (o.lucy_hybrid && (c->mix || o.mode == MCRT_MODE_LIVE_BW || o.part_count > 1))
@@ -2947,7 +3281,7 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     int n_hot = 0;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
     if ((rc = apply_hot(c, n_hot))) return rc;
-    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid || o.tau_redraw_per_cell;
+    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid || o.tau_redraw_per_cell || c->subR;
     R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
@@ -2974,6 +3308,11 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
         CUDA_TRY(c, cudaMemset2DAsync(c->lfx, 8 * kCS, 0, 8, c->ncp, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kabs_cnt, 0, c->ncp * 8, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->kprev, 0, c->ncp * 8, c->stream));
+        if (c->subR) {
+            CUDA_TRY(c, cudaMemsetAsync(c->sub_lfx, 0, c->n_subcells * (size_t)kCS * 8, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->sub_kcnt, 0, c->n_subcells * 8, c->stream));
+            CUDA_TRY(c, cudaMemsetAsync(c->sub_kprev, 0, c->n_subcells * 8, c->stream));
+        }
         if (c->mix) {
             CUDA_TRY(c, cudaMemsetAsync(c->lfx1, 0, c->ncp * (size_t)kCS * 8, c->stream));
             CUDA_TRY(c, cudaMemsetAsync(c->kcnt1, 0, c->ncp * 8, c->stream));
@@ -3076,6 +3415,12 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         k_epoch_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          R.e == 0, (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev,
                                                          R.cellfac, c->counters, c->tidx_mask);
+        if (c->subR)    // the sub-cubes: the same rule, Eq. 4 with V = (h/R)^3
+            k_epoch_update<<<stream_grid(c->n_subcells), 256, j_smem, c->stream>>>(c->sub_cellw, c->sub_kcnt, c->sub_kprev, c->sub_lfx, c->d_J,
+                                                                                  c->nT, c->ns, c->n_subcells, R.e == 0,
+                                                                                  (R.e == 0 || drain) ? 1.0 : (double)Be / (double)R.Bprev,
+                                                                                  R.cellfac * (double)(c->subR * c->subR * c->subR), c->counters,
+                                                                                  c->tidx_mask);
         part_slice(o, Be, &lo, &hi);
         P.pid0 = o.first_packet_id + R.done + lo; P.count = hi - lo;
         mark(c, timing);
@@ -3116,6 +3461,12 @@ int mcrt_run_step(mcrt_ctx *c, int *done_out)
         k_sweep_update<<<ugrid, 256, j_smem, c->stream>>>(c->cellw, c->kabs_cnt, c->kprev, c->lfx, c->d_J, c->nT, c->ns, c->ncp,
                                                          o.sweep_T_from_lucy, ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
                                                          sw == 1 ? R.prev_cellfac : R.cellfac, c->counters, c->tidx_mask);
+        if (c->subR)
+            k_sweep_update<<<stream_grid(c->n_subcells), 256, j_smem, c->stream>>>(c->sub_cellw, c->sub_kcnt, c->sub_kprev, c->sub_lfx, c->d_J,
+                                                                                  c->nT, c->ns, c->n_subcells, o.sweep_T_from_lucy,
+                                                                                  ldexp(1.0, -(sw == 1 ? R.prev_fx : c->fx)),
+                                                                                  (sw == 1 ? R.prev_cellfac : R.cellfac) * (double)(c->subR * c->subR * c->subR),
+                                                                                  c->counters, c->tidx_mask);
         CUDA_TRY(c, cudaMemsetAsync(c->sed, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->sed_direct, 0, hist_bytes, c->stream));
         CUDA_TRY(c, cudaMemsetAsync(c->counters, 0, CNT_NEXT * 8, c->stream));
@@ -3152,6 +3503,7 @@ int mcrt_run_end(mcrt_ctx *c, mcrt_run_stats *stats_out)
     if (c->need_exchange) return fail(c, MCRT_ESTATE, "partitioned run: exchange the last step's tallies before mcrt_run_end");
     k_range_check<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx, c->ncp, c->counters);
     if (c->mix) k_range_check<<<stream_grid(c->ncp), 256, 0, c->stream>>>(c->lfx1, c->ncp, c->counters);
+    if (c->subR) k_range_check<<<stream_grid(c->n_subcells), 256, 0, c->stream>>>(c->sub_lfx, c->n_subcells, c->counters);
     c->launches += c->mix ? 2 : 1;
     R.active = false;
     CUDA_TRY(c, cudaGetLastError());
@@ -3403,7 +3755,7 @@ int mcrt_ray_trace(mcrt_ctx *c, const mcrt_image_opts *io, double *F_emission, d
 {
     if (!c || !io || !F_emission) return MCRT_EINVAL;
     if (!c->last_n || c->run.active) return fail(c, MCRT_ESTATE, "mcrt_ray_trace needs a finished run");
-    if (c->mix) return fail(c, MCRT_EINVAL, "mcrt_ray_trace: images of dust mixtures are not defined");
+    if (c->mix || c->subR) return fail(c, MCRT_EINVAL, "mcrt_ray_trace: images of dust mixtures / divided grids are not defined");
     if (io->nx < 1 || io->ny < 1 || (size_t)io->nx * io->ny > ((size_t)1 << 28) || !(io->pixel_cm > 0.0) || !(io->distance_cm > 0.0) ||
         io->nu_bin < 0 || io->nu_bin >= c->nf)
         return fail(c, MCRT_EINVAL, "mcrt_ray_trace: bad image options");
@@ -3574,7 +3926,7 @@ void mcrt_destroy(mcrt_ctx *c)
     if (c->sca_ev) cudaFree(c->sca_ev);
     if (c->img_buf) cudaFree(c->img_buf);
     for (void *p : {(void *)c->d_mx_ncomp, (void *)c->d_mx_mat, (void *)c->d_mx_frac, (void *)c->d_mx_thr, (void *)c->d_kabs1_fx,
-                    (void *)c->lfx1, (void *)c->kcnt1, (void *)c->kprev1, (void *)c->tidx1, (void *)c->d_kmax_diag})
+                    (void *)c->lfx1, (void *)c->kcnt1, (void *)c->kprev1, (void *)c->tidx1, (void *)c->d_kmax_diag, (void *)c->sub_cellw, (void *)c->sub_lfx, (void *)c->sub_kcnt, (void *)c->sub_kprev})
         if (p) cudaFree(p);
     delete c;
 }

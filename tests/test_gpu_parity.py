@@ -789,3 +789,54 @@ def test_parity_tau_redraw_per_cell(B, orc, case):
     for key in RAW_KEYS:
         assert np.array_equal(raw_o[key], raw_g[key]), key
     c.close()
+
+
+@pytest.mark.parametrize("case", ["partly", "fully", "torus"])
+def test_parity_sub_cubes(B, orc, case):
+    """NEXT-3, one level of refinement (reading Q40; oracle pins P24): cubes divided into R^3 sub-cubes,
+    each a cell of its own.  Digests (with the sub-cubes' cell numbers in them), the grid's and the sub-cubes' counts,
+    tallies and temperature indices, escape histograms: bit-equal to the oracle, B&W epochs and a sweep, with the
+    source inside a divided cube and with per-cell redraw as well."""
+    rng = np.random.default_rng(31)
+    kw = {}
+    if case == "torus":
+        w = W.torus256(n_clumps=400, n=64)
+        R, N = 2, 120_000
+        dusty = np.flatnonzero(w.rho.reshape(-1) > 0)
+        cube = np.sort(rng.choice(dusty, size=len(dusty) // 5, replace=False))
+        kw = dict(grid_blocks=3, block_threads=64)                      # saturated pools
+    else:
+        w = W.sphere32(tau_V=8.0, n=12)
+        R, N = 4, 60_000
+        w.rho = np.where(w.rho > 0, w.rho, np.float32(w.rho.max() * 0.05)).astype(np.float32)   # dust everywhere
+        nc = w.rho.size
+        cube = np.arange(nc) if case == "fully" else np.sort(rng.choice(nc, size=nc // 3, replace=False))
+        centre = (nc // 2) + (12 * 12 // 2) * 0 + 6 * 12 + 6             # the source's cube
+        if case == "partly" and centre not in cube:
+            cube = np.sort(np.append(cube, centre))
+    rho_par = w.rho.reshape(-1)[cube].astype(np.float64)
+    rho_sub = (rho_par[:, None] * 10.0 ** rng.uniform(-1.0, 0.6, (len(cube), R ** 3))).astype(np.float32)
+    rho_sub[rng.random(rho_sub.shape) < 0.2] = 0.0
+    sp_sub = rng.integers(0, w.n_species, (len(cube), R ** 3)).astype(np.uint8)
+    w.subgrid = (R, cube, rho_sub, sp_sub)
+    nc0 = w.rho.size
+    o = orc.Oracle.from_workload(w)
+    c = B.Context(w, n_digests=N)
+    for step, okw, gkw in ((0, {}, {}), (1, dict(mode=orc.MODE_FROZEN_SWEEP, n_sweeps=1, reset=False),
+                                         dict(mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1)),
+                           (2, dict(per_cell_redraw=True), dict(tau_redraw_per_cell=1))):
+        ro = o.run(N, 61 + step, n_threads=NTH, digests=True, **okw)
+        rg = c.run(N, 61 + step, record_digests=1, **gkw, **kw)
+        for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+            assert ro[key] == rg[key], (step, key)
+        raw_o, raw_g, sub_g = o.read_raw(), c.read_raw(digests=True), c.read_subcells()
+        assert np.array_equal(ro["digests"], raw_g["digests"]), step
+        for key in ("sed", "sed_direct"):
+            assert np.array_equal(raw_o[key], raw_g[key]), (step, key)
+        for key in ("k", "lucy_fx", "tidx"):
+            assert np.array_equal(raw_o[key][:nc0], raw_g[key]), (step, key)
+            assert np.array_equal(raw_o[key][nc0:], sub_g[key]), (step, "sub", key)
+        assert sub_g["k"].sum() > 1000 and not raw_g["k"][cube].any()
+        To = o.read()["T"]
+        assert np.allclose(To[nc0:], sub_g["T_count"], rtol=2e-6, atol=0.0) and np.allclose(To[:nc0], c.read()["T_count"], rtol=2e-6, atol=0.0)
+    c.close()
