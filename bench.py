@@ -57,6 +57,9 @@ def parse():
                     help="N > 1: how the ranks' tallies are summed (auto = peer memory, NCCL if that cannot be set up)")
     ap.add_argument("--carry", type=int, default=0, help="experiment: carry packets over epoch boundaries after this many interactions in one epoch (0 = off, the configuration's definition)")
     ap.add_argument("--no-hot", action="store_true", help="experiment: no per-CTA copies of the tallies of the cells around the source")
+    ap.add_argument("--redraw", action="store_true", help="experiment: optical depth redrawn on entering every cell (PAPER.md:51)")
+    ap.add_argument("--mix", action="store_true", help="experiment: every species a 60/40 mixture of two materials (mcrt_dust_mixtures)")
+    ap.add_argument("--subgrid", type=float, default=0.0, help="experiment: this fraction of the dusty cubes divided into 2^3 sub-cubes (mcrt_subgrid)")
     ap.add_argument("--lucy-hybrid", action="store_true", help="experiment: the thresholded Lucy estimator of Sect. 3.1 (only thin cells tallied)")
     ap.add_argument("--threads", type=int, default=0, help="experiment: threads per CTA of the transport kernel (0 = as many warps as fit)")
     ap.add_argument("--sweeps", type=int, default=-1, help="frozen-T sweeps after the B&W pass (-1 = the configuration's: 3 for torus512)")
@@ -71,6 +74,18 @@ def make_workload(args):
         kw["n_clumps"] = args.clumps if args.workload == "torus256" else 20000
     w = W.make(args.workload, **kw)
     n = args.packets if args.packets > 0 else w.n_packets
+    # experiments with the rarely used features (not BASELINE configurations; the line's config names them)
+    if args.mix and w.n_species >= 2:
+        import numpy as np
+        ns = w.n_species      # species x becomes a 60 / 40 mixture of materials x and x + 1
+        w.mixtures = ([2] * ns, [[x, (x + 1) % ns] for x in range(ns)], [[0.6, 0.4]] * ns)
+    if args.subgrid > 0.0:
+        import numpy as np
+        rng = np.random.default_rng(12)
+        dusty = np.flatnonzero(w.rho.reshape(-1) > 0)
+        cube = np.sort(rng.choice(dusty, size=max(1, int(args.subgrid * len(dusty))), replace=False))
+        rho_sub = np.repeat(w.rho.reshape(-1)[cube][:, None], 8, axis=1) * rng.uniform(0.5, 1.5, (len(cube), 8)).astype(np.float32)
+        w.subgrid = (2, cube, rho_sub.astype(np.float32), np.repeat(w.species.reshape(-1)[cube][:, None], 8, axis=1))
     return w, n
 
 
@@ -276,7 +291,8 @@ def run_ours(args, workload_name=None):
         counters of every pass (a sweep counts its own packets: they are read after each sweep, a 120-byte D2H copy
         inside the timed region)."""
         kw = dict(epoch_Bmax=args.bmax, time_kernels=1 if timed else 0, no_hot_cells=1 if args.no_hot else 0,
-                  block_threads=args.threads, lucy_hybrid=1 if args.lucy_hybrid else 0)
+                  block_threads=args.threads, lucy_hybrid=1 if args.lucy_hybrid else 0,
+                  tau_redraw_per_cell=1 if args.redraw else 0)
         out = []
         sweep_kw = dict(mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=n_sweeps, **kw)
         if args.carry and world == 1:
@@ -470,6 +486,9 @@ def run_ours(args, workload_name=None):
                              "L2 read bandwidth; the tallies are reset and every cell is rewritten between launches"
                              % (res_b / 1e6),
                        "epoch_Bmax": args.bmax if args.bmax else "default 2^22",
+                       "experiment": {k: v for k, v in (("carry", args.carry), ("no_hot", args.no_hot), ("lucy_hybrid", args.lucy_hybrid),
+                                                        ("redraw", args.redraw), ("mix", args.mix), ("subgrid", args.subgrid),
+                                                        ("threads", args.threads)) if v} or None,
                        "parallelism": (f"1 run partitioned over {world} GPUs by packet id, integer tallies summed per epoch "
                                        f"({exchange_mode})") if world > 1 else "single"},
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e,

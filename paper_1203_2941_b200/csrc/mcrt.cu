@@ -149,7 +149,7 @@ struct mcrt_ctx {
         bool finished = false;            // every step has been issued
         uint32_t carry_K = 0;             // interaction budget of the current epoch (0 = no carry-over)
         uint64_t n_carry = 0;             // packets carried into the next epoch
-        bool xtra = false;                // carry-over / event store / stratified source / live B&W in use
+        int xtra = 0;                     // which rarely used features are in use (template argument XTRA of k_transport)
         bool hot = false;                 // hot cells tallied per CTA
     } run;
     bool need_exchange = false;           // partitioned run: a step's tallies are still per-part
@@ -761,7 +761,10 @@ __device__ __forceinline__ void hot_add(unsigned int *hot, uint32_t id, unsigned
 __host__ __device__ constexpr int hot_smem_words(int n_hot) { return (3 * (n_hot + 1) + 3) & ~3; }
 constexpr int kPermSmem = 1024;
 
-template <bool RECORD, bool HOT, bool XTRA>
+// XTRA: 0 = none of the rarely used features; 1 = those that live outside the walk loop (carry-over, event store, stratified
+// source, live B&W, sub-cubes); 2 = those of 1 and the ones inside it (mixtures, thresholded estimator); 3 = those of 2
+// and the per-cell redraw of the optical depth (a Philox block and a logarithm in every step)
+template <bool RECORD, bool HOT, int XTRA>
 __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const TransportParams P)
 {
     constexpr int kDepth = kDepthReg;
@@ -981,9 +984,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         for (int i = 0; i < kDepth - 2; ++i) { tq[i] = t; cq[i] = 0u; }
                         kq_row = s_kk + j;
                         kq_sp = 0u; kq = kq_row[0];
-                        if (XTRA && P.lfx1) { k1_row = P.kabs1_fx + j; kq1 = k1_row[0]; }
-                        if (XTRA && P.kmax_diag) kmd = P.kmax_diag[0];
-                        if (XTRA && P.redraw) {
+                        if (XTRA >= 2 && P.lfx1) { k1_row = P.kabs1_fx + j; kq1 = k1_row[0]; }
+                        if (XTRA >= 2 && P.kmax_diag) kmd = P.kmax_diag[0];
+                        if (XTRA >= 3 && P.redraw) {
                             rd_pid = (unsigned long long)__double_as_longlong(SF(F_PID, slot));
                             rd_base = SU(U_DK, slot) & 0x3fffffffu;
                         }
@@ -1049,10 +1052,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         kq_sp = cw_species(cw);                                                                             \
                         MCRT_CHK(!fly || kq_sp < (uint32_t)P.ns, "walk: species of the cell word");                         \
                         kq = kq_row[(fly || !MCRT_CHECK) ? kq_sp * nf_r : 0u];                                              \
-                        if (XTRA && P.lfx1) kq1 = k1_row[fly ? kq_sp * nf_r : 0u];   /* second component of a mixture */     \
-                        if (XTRA && P.kmax_diag) kmd = P.kmax_diag[fly ? kq_sp : 0u]; /* thresholded estimator */             \
+                        if (XTRA >= 2 && P.lfx1) kq1 = k1_row[fly ? kq_sp * nf_r : 0u];   /* second component of a mixture */     \
+                        if (XTRA >= 2 && P.kmax_diag) kmd = P.kmax_diag[fly ? kq_sp : 0u]; /* thresholded estimator */             \
                     }                                                                                                       \
-                    if (XTRA && P.redraw && fly) {   /* a new random number on entering the cell */             \
+                    if (XTRA >= 3 && P.redraw && fly) {   /* a new random number on entering the cell */             \
                         double zr0, zr1;                                                                                    \
                         draw2(P.seed_lo, P.seed_hi, rd_pid, (rd_base + ncross) & 0x3fffffffu, P.pass, zr0, zr1);            \
                         tau = -traj_log(zr0);                                                                               \
@@ -1077,7 +1080,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                                      : "+l"(wstop) : "l"(cellw_r + kCS * ciA), "r"((uint32_t)(fly && stop)));               \
                     /* S5: tally of a traversed dusty cell (a vacuum cell has nothing to add) */                           \
                     {                                                                                                       \
-                        const bool hyb = XTRA && P.kmax_diag;       /* Sect. 3.1: Eq. 9 in cells below the threshold only */ \
+                        const bool hyb = XTRA >= 2 && P.kmax_diag;       /* Sect. 3.1: Eq. 9 in cells below the threshold only */ \
                         const double xq = kq.y * rho_c * ds;                                                                \
                         const unsigned long long q = lucy_round(hyb ? eq9_fx(xq, P.two_fx, P.inv_two_fx) : xq);             \
                         const bool go = fly && !stop;                                                                       \
@@ -1089,11 +1092,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         MCRT_CHK(!(fly && stop) || (uint32_t)slot < (uint32_t)kSlots, "walk: slot of the stopped packet");   \
                         if (MCRT_L2_HINT == 2)                                                                              \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.L2::cache_hint.u64 [%0], %1, %3;\n\t}" \
-                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA) ? cold : dusty), "l"(l2_stream) : "memory"); \
+                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA >= 2) ? cold : dusty), "l"(l2_stream) : "memory"); \
                         else                                                                                                \
                         asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p red.global.add.u64 [%0], %1;\n\t}"  \
-                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA) ? cold : dusty) : "memory");       \
-                        if (XTRA && P.lfx1) {       /* the second component's tally (reading Q36) */                         \
+                                     ::"l"(lfx_r + kCS * ciA), "l"(q), "r"((HOT || XTRA >= 2) ? cold : dusty) : "memory");       \
+                        if (XTRA >= 2 && P.lfx1) {       /* the second component's tally (reading Q36) */                         \
                             const unsigned long long q1 = lucy_round(kq1 * rho_c * ds);                                     \
                             if (dusty && kq1 != 0.0) lucy_add_raw(P.lfx1, ciA, q1);                                         \
                         }                                                                                                   \
@@ -1178,7 +1181,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 j = (int)(w1 & 0xffffu);
                 g_ok = (w1 & kSubOk) != 0u;
                 gx = (int)((w1 >> 16) & 7u); gy = (int)((w1 >> 19) & 7u); gz = (int)((w1 >> 22) & 7u);
-                if (P.redraw) { rpid = (unsigned long long)__double_as_longlong(SF(F_PID, slot)); rbase = SU(U_DK, slot) & 0x3fffffffu; }
+                if (XTRA >= 3 && P.redraw) { rpid = (unsigned long long)__double_as_longlong(SF(F_PID, slot)); rbase = SU(U_DK, slot) & 0x3fffffffu; }
             }
             do {
                 if (busy) {
@@ -1209,7 +1212,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         fw = __ldg(P.sub_cellw + (size_t)kCS * fidx);
                         const double rho_c = cw_rho(fw);
                         const double2 kq = s_kk[cw_species(fw) * nf + j];
-                        if (P.redraw) {
+                        if (XTRA >= 3 && P.redraw) {
                             double zr0, zr1;
                             draw2(P.seed_lo, P.seed_hi, rpid, (rbase + ncross) & 0x3fffffffu, P.pass, zr0, zr1);
                             tau = -traj_log(zr0);
@@ -1368,7 +1371,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 ux = SF(F_UX, slot); uy = SF(F_UY, slot); uz = SF(F_UZ, slot);
                 // per-cell redraw: the slot holds (index of the flight's draw) - (crossings at its start); every cell
                 // entered since has used one more draw (see the walk), so the next free index is
-                if (XTRA && P.redraw) d = (d + ncross + 1u) & 0x3fffffffu;
+                if (XTRA >= 3 && P.redraw) d = (d + ncross + 1u) & 0x3fffffffu;
             }
             {   // run counters of the packets that escape in this phase: summed over the warp, then added to the warp's
                 // own counters in shared memory by one lane (no atomics)
@@ -1478,13 +1481,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         lucy_add(P.sub_lfx, fidx, kq.y * rho_c * sint);
                     } else
                     if (hid) hot_add(s_hot, hid, lucy_round(kq.y * rho_c * sint));
-                    else if (XTRA && P.kmax_diag) {           // Sect. 3.1: Eq. 9, cells below the threshold only
+                    else if (XTRA >= 2 && P.kmax_diag) {           // Sect. 3.1: Eq. 9, cells below the threshold only
                         if (rho_c * P.kmax_diag[cw_species(cw)] < kThinTau)
                             lucy_add(P.lfx, cidx, eq9_fx(kq.y * rho_c * sint, P.two_fx, P.inv_two_fx));
                     } else lucy_add(P.lfx, cidx, kq.y * rho_c * sint);
                     // mixtures (NEXT-3, readings Q34-Q36): the second component's tally; which component interacts
                     double2 thr = make_double2(2.0, 2.0);      // {S0, A0}; a uniform is < 2: one component = always component 0
-                    if (XTRA && P.lfx1) {
+                    if (XTRA >= 2 && P.lfx1) {
                         const double k1 = P.kabs1_fx[sj];
                         if (k1 != 0.0) lucy_add(P.lfx1, cidx, k1 * rho_c * sint);
                         if (P.mx_mat[2 * cw_species(cw) + 1] >= 0) thr = P.mx_thr[sj];
@@ -1518,7 +1521,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             }
                         }
                         if (RECORD) hash_mix(hash, event_word(EV_SCATTER, j, cell));
-                        if (XTRA && P.lfx1) gmix = P.g[P.mx_mat[2 * cw_species(cw) + (!(ztype < thr.x) ? 1 : 0)] * nf + j];
+                        if (XTRA >= 2 && P.lfx1) gmix = P.g[P.mx_mat[2 * cw_species(cw) + (!(ztype < thr.x) ? 1 : 0)] * nf + j];
                     } else {
                         // S8/S9 absorb: count, re-emit at once at a frequency drawn from the
                         // cell's frozen-epoch temperature row of Eq. 10 or Eq. 5 (sweeps)
@@ -1527,7 +1530,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         int s = cw_species(cw);
                         int m = cw_tidx(cw, P.tidx_mask);
                         bool second = false;                   // absorbed by the second component of a mixture
-                        if (XTRA && P.lfx1) {
+                        if (XTRA >= 2 && P.lfx1) {
                             second = !(ztype < thr.y);
                             s = P.mx_mat[2 * s + (second ? 1 : 0)];    // the material whose row re-emits
                             if (second) m = (int)P.tidx1[cidx];
@@ -1540,7 +1543,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                             m = t_index(P.J + s * P.nT, P.nT, (double)kn * P.cellfac / rho_c);
                         } else if (XTRA && insub) atomicAdd(&P.sub_kcnt[fidx], 1ull);
                         else if (hid) atomicAdd(&s_hot[3u * hid + 2u], 1u);
-                        else if (XTRA && second) atomicAdd(&P.kcnt1[cidx], 1ull);
+                        else if (XTRA >= 2 && second) atomicAdd(&P.kcnt1[cidx], 1ull);
                         else atomicAdd(&P.kcnt[cidx], 1ull);
                         draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                         MCRT_CHK(s >= 0 && s < P.ns && m >= 0 && m < P.nT, "absorption: CDF row");
@@ -1553,7 +1556,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 draw2(P.seed_lo, P.seed_hi, pid, d++, P.pass, z0, z1);
                 double mu = 1.0 - 2.0 * z0;
                 if (scatter) {
-                    const double gg = (XTRA && P.lfx1) ? gmix : s_ag[sj].y;
+                    const double gg = (XTRA >= 2 && P.lfx1) ? gmix : s_ag[sj].y;
                     if (fabs(gg) > 1e-6) {
                         const double q = (1.0 - gg * gg) / (1.0 - gg + 2.0 * gg * z0);
                         mu = (1.0 + gg * gg - q * q) / (2.0 * gg);
@@ -1636,7 +1639,7 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 // (kind is set when the walk stops.)  Per-cell redraw: the cell reached after c crossings of
                 // this flight takes the draw of index (flight's draw) + c -- c = 0 is the flight's own draw, so the first
                 // cell needs no special case -- and the slot keeps that index minus the crossing count
-                SU(U_DK, slot) = (XTRA && P.redraw) ? ((d - 1u - ncross) & 0x3fffffffu) : d;
+                SU(U_DK, slot) = (XTRA >= 3 && P.redraw) ? ((d - 1u - ncross) & 0x3fffffffu) : d;
                 SU(U_NCROSS, slot) = ncross; SU(U_NSCA, slot) = nsca; SU(U_NABS, slot) = nabs;
                 SU(U_W0, slot) = pack_xyz(ix, iy, iz);
                 SU(U_W1, slot) = (uint32_t)j | (nint << 16) | ((XTRA && insub) ? sub_pack(sgx, sgy, sgz) : 0u);
@@ -3018,18 +3021,17 @@ static int ensure_histograms(mcrt_ctx *c)
     return MCRT_OK;
 }
 
-// the eight instantiations of the transport kernel
+// the sixteen instantiations of the transport kernel
 typedef void (*transport_fn)(const TransportParams);
-// (digests recorded, hot cells tallied per CTA, any of the rarely used extras: carry-over, scattering-event store,
-// stratified source, live B&W -- compiled out of the default kernels: the kernel's code has to fit the instruction
-// cache, and every feature inlined into the event phase cost 1-4 % of the default path's throughput)
-static transport_fn transport_kernel(bool record, bool hot, bool xtra)
+// (digests recorded, hot cells tallied per CTA, level of the rarely used extras -- compiled out of the default kernels:
+// the kernel's code has to fit the instruction cache, and every feature inlined into the event phase cost 1-4 % of the
+// default path's throughput; the features that sit inside the walk loop halve it and have a level of their own)
+static transport_fn transport_kernel(bool record, bool hot, int xtra)
 {
-    static const transport_fn tab[8] = {k_transport<false, false, false>, k_transport<true, false, false>,
-                                        k_transport<false, true, false>,  k_transport<true, true, false>,
-                                        k_transport<false, false, true>,  k_transport<true, false, true>,
-                                        k_transport<false, true, true>,   k_transport<true, true, true>};
-    return tab[(record ? 1 : 0) | (hot ? 2 : 0) | (xtra ? 4 : 0)];
+#define MCRT_KT(x) k_transport<false, false, x>, k_transport<true, false, x>, k_transport<false, true, x>, k_transport<true, true, x>
+    static const transport_fn tab[16] = {MCRT_KT(0), MCRT_KT(1), MCRT_KT(2), MCRT_KT(3)};
+#undef MCRT_KT
+    return tab[(record ? 1 : 0) | (hot ? 2 : 0) | (4 * xtra)];
 }
 
 static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, int *threads, size_t *smem, int *n_hot)
@@ -3054,12 +3056,12 @@ static int transport_config(mcrt_ctx *c, const mcrt_run_opts *o, int *blocks, in
     *n_hot = nh;
     *smem = transport_smem_bytes(c->ns, c->nf, c->ndir, c->mwords, *threads, record, nh);
     if (*smem > 48 * 1024) {
-        for (int v = 0; v < 8; ++v)
-            CUDA_TRY(c, cudaFuncSetAttribute(transport_kernel(v & 1, v & 2, v & 4), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
+        for (int v = 0; v < 16; ++v)
+            CUDA_TRY(c, cudaFuncSetAttribute(transport_kernel(v & 1, v & 2, v >> 2), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)*smem));
     }
     int nsm = 148, occ = 1;
     CUDA_TRY(c, cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, c->device));
-    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, transport_kernel(false, true, true), *threads, *smem));
+    CUDA_TRY(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, transport_kernel(false, true, 3), *threads, *smem));
     if (occ < 1) return fail(c, MCRT_EINVAL, "transport kernel does not fit on an SM with these table sizes");
     c->occ_blocks = occ;
     *blocks = (o && o->grid_blocks > 0) ? o->grid_blocks : nsm * occ;  // persistent: every CTA resident
@@ -3281,7 +3283,8 @@ int mcrt_run_begin(mcrt_ctx *c, uint64_t n_packets, uint64_t seed, const mcrt_ru
     int n_hot = 0;
     if ((rc = transport_config(c, &o, &R.blocks, &R.threads, &R.smem, &n_hot))) return rc;
     if ((rc = apply_hot(c, n_hot))) return rc;
-    R.xtra = o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->mix || o.lucy_hybrid || o.tau_redraw_per_cell || c->subR;
+    R.xtra = o.tau_redraw_per_cell ? 3 : (c->mix || o.lucy_hybrid) ? 2
+             : ((o.carry_interactions || c->sca_ev || o.source_strata || o.mode == MCRT_MODE_LIVE_BW || c->subR) ? 1 : 0);
     R.hot = c->n_hot > 0;
     const size_t hist_bytes = (size_t)c->ndir * c->nf * 8;
 
