@@ -633,6 +633,9 @@ enum : int { F_PX = 0, F_PY, F_PZ, F_UX, F_UY, F_UZ, F_T, F_TAU, F_ZTYPE, F_CW, 
 #endif
 // MCRT_PACK_STOP = 1: what a stopping packet stores in the walk sits in adjacent words of its slot -- (t, tau) as one
 // 16-byte pair, (crossings, cell) as one 8-byte pair -- so that a stop is three shared-memory stores instead of five
+#ifndef MCRT_J_ONELOAD
+#define MCRT_J_ONELOAD 1            // 1: the jump loop reads the landing brick's box entry (its fourth word says "empty") instead of
+#endif                              //    the mask bit and then the box: one dependent load per jump instead of two
 #ifndef MCRT_L2_HINT
 #define MCRT_L2_HINT 0              // 1: the walk's cell-word loads carry an L2 evict_last policy; 2: and its tally REDs evict_first
 #endif
@@ -1310,11 +1313,13 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 tmz = mcrt::face_t(iz, stz, pz, ivz);
             }
             const int jmin = min(nj, MCRT_J_MIN);
+            uint4 bb = make_uint4(0u, 0u, 0u, 0u);
+            if (MCRT_J_ONELOAD && busy) bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
             do {
                 if (busy) {
                     // the precomputed box of empty bricks around this brick, in cells, clipped to the grid
                     MCRT_CHK(ix >= 0 && iy >= 0 && iz >= 0 && ix < P.nx && iy < P.ny && iz < P.nz, "jump: cell coordinates");
-                    const uint4 bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
+                    if (!MCRT_J_ONELOAD) bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh));
                     const int lox = (int)(bb.x & 0xffffu) << bsh, loy = (int)(bb.x >> 16) << bsh, loz = (int)(bb.y & 0xffffu) << bsh;
                     const int hix = min((int)(bb.y >> 16) << bsh, P.nx), hiy = min((int)(bb.z & 0xffffu) << bsh, P.ny),
                               hiz = min((int)(bb.z >> 16) << bsh, P.nz);
@@ -1322,6 +1327,11 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                                              stx, sty, stz, lox, loy, loz, hix, hiy, hiz);
                     escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) |
                               ((unsigned)iz >= (unsigned)P.nz);
+                    if (MCRT_J_ONELOAD) {
+                        // the landing brick's entry: whether it is empty as well and, if so, its box -- one load per jump
+                        busy = false;
+                        if (!escaped) { bb = ldg_table(P.vbox + brick_of(ix, iy, iz, nbx, nby, bsh)); busy = bb.w != 0u; }
+                    } else
                     busy = !escaped && brick_empty(s_m0, brick_of(ix, iy, iz, nbx, nby, bsh));
                 }
             } while (__popc(__ballot_sync(kFull, busy)) >= max(jmin, 1));
@@ -2075,8 +2085,9 @@ __global__ void k_grow_boxes(const uint32_t *__restrict__ mask, const int *__res
                 if (z1 < nbz && sat_count(sat, sx, sy, x0, y0, z1, x1, y1, z1 + 1) == 0) { ++z1; grew = true; }
             }
         }
+        // (fourth word: 1 = the brick is empty -- the jump loop reads "is the landing brick empty" and its box in one load)
         box[b] = make_uint4((uint32_t)x0 | ((uint32_t)y0 << 16), (uint32_t)z0 | ((uint32_t)x1 << 16),
-                            (uint32_t)y1 | ((uint32_t)z1 << 16), 0u);
+                            (uint32_t)y1 | ((uint32_t)z1 << 16), ((mask[b >> 5] >> (b & 31)) & 1u));
     }
 }
 
