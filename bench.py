@@ -83,7 +83,11 @@ def make_workload(args):
         import numpy as np
         rng = np.random.default_rng(12)
         dusty = np.flatnonzero(w.rho.reshape(-1) > 0)
-        cube = np.sort(rng.choice(dusty, size=max(1, int(args.subgrid * len(dusty))), replace=False))
+        # the dusty cubes nearest to the source ("close to the dust evaporation zone")
+        iz, iy, ix = np.unravel_index(dusty, w.rho.shape)
+        src = np.asarray(w.source_pos_cm) / w.cell_size_cm
+        d2 = (ix + 0.5 - src[0]) ** 2 + (iy + 0.5 - src[1]) ** 2 + (iz + 0.5 - src[2]) ** 2
+        cube = np.sort(dusty[np.argsort(d2, kind="stable")[:max(1, min(1 << 22, int(args.subgrid * len(dusty))))]])
         rho_sub = np.repeat(w.rho.reshape(-1)[cube][:, None], 8, axis=1) * rng.uniform(0.5, 1.5, (len(cube), 8)).astype(np.float32)
         w.subgrid = (2, cube, rho_sub.astype(np.float32), np.repeat(w.species.reshape(-1)[cube][:, None], 8, axis=1))
     return w, n

@@ -1186,64 +1186,61 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                 gx = (int)((w1 >> 16) & 7u); gy = (int)((w1 >> 19) & 7u); gz = (int)((w1 >> 22) & 7u);
                 if (XTRA >= 3 && P.redraw) { rpid = (unsigned long long)__double_as_longlong(SF(F_PID, slot)); rbase = SU(U_DK, slot) & 0x3fffffffu; }
             }
+            // (1/R is a power of two: the products below are the oracle's quotients (g + 1) / R, exactly.  The step is
+            // written without branches on the axis: lanes of a warp take different axes, and a branch per axis made the
+            // compiler's software division and the face arithmetic run lane by lane)
+            const double invR = 1.0 / Rd;
+            const int upx = stx > 0 ? 1 : 0, upy = sty > 0 ? 1 : 0, upz = stz > 0 ? 1 : 0;
             do {
-                if (busy) {
-                    if (need_cube) {
-                        pw = __ldg(P.cellw + (size_t)kCS * lin_index(ix, iy, iz, lpx, lpxy));
-                        if (!((uint32_t)(pw >> 32) == kMarkHi && ((uint32_t)pw & kSubFlag))) { busy = false; g_ok = false; }
-                        else {
-                            blk = (uint32_t)pw >> kSubShift;
-                            if (!g_ok) {   // entered from an undivided cube: the sub-cube that holds the entry point p + u t
-                                int q;
-                                q = (int)floor(((px + ux * t) - (double)ix) * Rd); gx = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
-                                q = (int)floor(((py + uy * t) - (double)iy) * Rd); gy = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
-                                q = (int)floor(((pz + uz * t) - (double)iz) * Rd); gz = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
-                                g_ok = true;
-                            }
-                            fx = stx ? (((double)ix + (double)(gx + (stx > 0 ? 1 : 0)) / Rd) - px) * ivx : CUDART_INF;
-                            fy = sty ? (((double)iy + (double)(gy + (sty > 0 ? 1 : 0)) / Rd) - py) * ivy : CUDART_INF;
-                            fz = stz ? (((double)iz + (double)(gz + (stz > 0 ? 1 : 0)) / Rd) - pz) * ivz : CUDART_INF;
-                            need_cube = false;
+                if (busy && need_cube) {
+                    pw = __ldg(P.cellw + (size_t)kCS * lin_index(ix, iy, iz, lpx, lpxy));
+                    if (!((uint32_t)(pw >> 32) == kMarkHi && ((uint32_t)pw & kSubFlag))) { busy = false; g_ok = false; }
+                    else {
+                        blk = (uint32_t)pw >> kSubShift;
+                        if (!g_ok) {   // entered from an undivided cube: the sub-cube that holds the entry point p + u t
+                            int q;
+                            q = (int)floor(((px + ux * t) - (double)ix) * Rd); gx = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                            q = (int)floor(((py + uy * t) - (double)iy) * Rd); gy = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                            q = (int)floor(((pz + uz * t) - (double)iz) * Rd); gz = q < 0 ? 0 : (q > R - 1 ? R - 1 : q);
+                            g_ok = true;
                         }
+                        need_cube = false;
                     }
-                    if (busy) {
-                        const bool selx = (fx <= fy) && (fx <= fz), sely = !selx && (fy <= fz);
-                        const double tn = selx ? fx : (sely ? fy : fz);
-                        const double ds = tn - t;
-                        const uint32_t fidx = blk * (uint32_t)R3 + (uint32_t)((gz * R + gy) * R + gx);
-                        MCRT_CHK(fidx < (uint32_t)P.sub_n, "sub-cube index");
-                        fw = __ldg(P.sub_cellw + (size_t)kCS * fidx);
-                        const double rho_c = cw_rho(fw);
-                        const double2 kq = s_kk[cw_species(fw) * nf + j];
-                        if (XTRA >= 3 && P.redraw) {
-                            double zr0, zr1;
-                            draw2(P.seed_lo, P.seed_hi, rpid, (rbase + ncross) & 0x3fffffffu, P.pass, zr0, zr1);
-                            tau = -traj_log(zr0);
-                        }
-                        const double dtau = kq.x * rho_c * ds;
-                        if (!(dtau <= tau)) { hit = true; busy = false; }
-                        else {
-                            tau -= dtau;
-                            if (__double2hiint(rho_c) != 0) { lucy_add(P.sub_lfx, fidx, kq.y * rho_c * ds); ndusty_acc++; }
-                            t = tn;
-                            ncross++;
-                            if (selx) {
-                                gx += stx;
-                                if ((unsigned)gx >= (unsigned)R) { gx = stx > 0 ? 0 : R - 1; ix += stx; need_cube = true; }
-                                else fx = (((double)ix + (double)(gx + (stx > 0 ? 1 : 0)) / Rd) - px) * ivx;
-                            } else if (sely) {
-                                gy += sty;
-                                if ((unsigned)gy >= (unsigned)R) { gy = sty > 0 ? 0 : R - 1; iy += sty; need_cube = true; }
-                                else fy = (((double)iy + (double)(gy + (sty > 0 ? 1 : 0)) / Rd) - py) * ivy;
-                            } else {
-                                gz += stz;
-                                if ((unsigned)gz >= (unsigned)R) { gz = stz > 0 ? 0 : R - 1; iz += stz; need_cube = true; }
-                                else fz = (((double)iz + (double)(gz + (stz > 0 ? 1 : 0)) / Rd) - pz) * ivz;
-                            }
-                            if (need_cube) {
-                                escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) | ((unsigned)iz >= (unsigned)P.nz);
-                                if (escaped) busy = false;
-                            }
+                }
+                if (busy) {
+                    // parameters of the faces through which sub-cube g is left: f = c + (g + [u > 0]) / R
+                    fx = stx ? (((double)ix + (double)(gx + upx) * invR) - px) * ivx : CUDART_INF;
+                    fy = sty ? (((double)iy + (double)(gy + upy) * invR) - py) * ivy : CUDART_INF;
+                    fz = stz ? (((double)iz + (double)(gz + upz) * invR) - pz) * ivz : CUDART_INF;
+                    const bool selx = (fx <= fy) && (fx <= fz), sely = !selx && (fy <= fz), selz = !selx && !sely;
+                    const double tn = selx ? fx : (sely ? fy : fz);
+                    const double ds = tn - t;
+                    const uint32_t fidx = blk * (uint32_t)R3 + (uint32_t)((gz * R + gy) * R + gx);
+                    MCRT_CHK(fidx < (uint32_t)P.sub_n, "sub-cube index");
+                    fw = __ldg(P.sub_cellw + (size_t)kCS * fidx);
+                    const double rho_c = cw_rho(fw);
+                    const double2 kq = s_kk[cw_species(fw) * nf + j];
+                    if (XTRA >= 3 && P.redraw) {
+                        double zr0, zr1;
+                        draw2(P.seed_lo, P.seed_hi, rpid, (rbase + ncross) & 0x3fffffffu, P.pass, zr0, zr1);
+                        tau = -traj_log(zr0);
+                    }
+                    const double dtau = kq.x * rho_c * ds;
+                    if (!(dtau <= tau)) { hit = true; busy = false; }
+                    else {
+                        tau -= dtau;
+                        if (__double2hiint(rho_c) != 0) { lucy_add(P.sub_lfx, fidx, kq.y * rho_c * ds); ndusty_acc++; }
+                        t = tn;
+                        ncross++;
+                        // the neighbouring sub-cube along the selected axis; through a face of the cube: the next cube, same row
+                        gx += selx ? stx : 0; gy += sely ? sty : 0; gz += selz ? stz : 0;
+                        const bool ox = (unsigned)gx >= (unsigned)R, oy = (unsigned)gy >= (unsigned)R, oz = (unsigned)gz >= (unsigned)R;
+                        gx = ox ? (upx ? 0 : R - 1) : gx; gy = oy ? (upy ? 0 : R - 1) : gy; gz = oz ? (upz ? 0 : R - 1) : gz;
+                        ix += ox ? stx : 0; iy += oy ? sty : 0; iz += oz ? stz : 0;
+                        need_cube = ox || oy || oz;
+                        if (need_cube) {
+                            escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) | ((unsigned)iz >= (unsigned)P.nz);
+                            if (escaped) busy = false;
                         }
                     }
                 }
