@@ -840,3 +840,40 @@ def test_parity_sub_cubes(B, orc, case):
         To = o.read()["T"]
         assert np.allclose(To[nc0:], sub_g["T_count"], rtol=2e-6, atol=0.0) and np.allclose(To[:nc0], c.read()["T_count"], rtol=2e-6, atol=0.0)
     c.close()
+
+
+def test_new_entry_points_reject_bad_arguments(B):
+    """Error behaviour of the NEXT-3 / NEXT-4 additions stated in include/mcrt.h: bad tables and conflicting options
+    are refused with MCRT_EINVAL / MCRT_ESTATE and a message, and a refused run leaves the context usable."""
+    w = W.torus256(n_clumps=50, n=16)
+    dusty = np.flatnonzero(w.rho.reshape(-1) > 0)
+    vac = np.flatnonzero(w.rho.reshape(-1) == 0)
+    ones8, zeros8 = np.ones((1, 8), np.float32), np.zeros((1, 8), np.uint8)
+    for bad in ((3, dusty[:1], np.ones((1, 27), np.float32), np.zeros((1, 27), np.uint8)),      # R not 2, 4, 8
+                (2, np.array([dusty[0], dusty[0]]), np.ones((2, 8), np.float32), np.zeros((2, 8), np.uint8)),   # listed twice
+                (2, np.array([w.rho.size]), ones8, zeros8),                                        # out of range
+                (2, vac[:1], ones8, zeros8),                                                       # the cube itself holds no dust
+                (2, dusty[:1], ones8, zeros8 + 9)):                                                # species out of range
+        c = B.Context(w)
+        with pytest.raises(B.McrtError):
+            B.mcrt_subgrid(c.ctx, *bad)
+        c.close()
+    c = B.Context(w)
+    for bad in (([3, 1, 1], [[0, 1], [1, -1], [2, -1]], [[0.5, 0.5], [1, 0], [1, 0]]),            # three components
+                ([2, 1, 1], [[0, 7], [1, -1], [2, -1]], [[0.5, 0.5], [1, 0], [1, 0]]),            # material out of range
+                ([2, 1, 1], [[0, 1], [1, -1], [2, -1]], [[0.5, 0.4], [1, 0], [1, 0]])):           # fractions do not add up
+        with pytest.raises(B.McrtError):
+            B.mcrt_dust_mixtures(c.ctx, *bad)
+    with pytest.raises(B.McrtError):
+        B.mcrt_read_component(c.ctx, 1)                                                           # no mixtures set
+    with pytest.raises(B.McrtError):
+        B.mcrt_read_subcells(c.ctx)                                                               # no sub-grid set
+    for kw in (dict(tau_redraw_per_cell=1, carry_interactions=10), dict(lucy_hybrid=1, part_count=2, part_index=0),
+               dict(tau_redraw_per_cell=1, mode=B.MCRT_MODE_LIVE_BW)):
+        with pytest.raises(B.McrtError):
+            c.run(1000, 1, **kw)
+    r = c.run(2000, 1)                                                                            # still usable
+    assert r["packets"] == 2000
+    with pytest.raises(B.McrtError):
+        c.run(2000, 2, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1, lucy_hybrid=1)                # the other estimator's tallies
+    c.close()
