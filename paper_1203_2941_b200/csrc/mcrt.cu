@@ -1191,9 +1191,14 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
             // compiler's software division and the face arithmetic run lane by lane)
             const double invR = 1.0 / Rd;
             const int upx = stx > 0 ? 1 : 0, upy = sty > 0 ? 1 : 0, upz = stz > 0 ? 1 : 0;
+            // The word of the NEXT position -- the next sub-cube's, or the next cube's when the step leaves this one -- is
+            // loaded one step ahead (which position that is does not depend on what the sub-cubes hold): nw, valid if nw_ok.
+            unsigned long long nw = 0ull;
+            bool nw_ok = false;
             do {
                 if (busy && need_cube) {
-                    pw = __ldg(P.cellw + (size_t)kCS * lin_index(ix, iy, iz, lpx, lpxy));
+                    pw = nw_ok ? nw : __ldg(P.cellw + (size_t)kCS * lin_index(ix, iy, iz, lpx, lpxy));
+                    nw_ok = false;
                     if (!((uint32_t)(pw >> 32) == kMarkHi && ((uint32_t)pw & kSubFlag))) { busy = false; g_ok = false; }
                     else {
                         blk = (uint32_t)pw >> kSubShift;
@@ -1208,6 +1213,10 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     }
                 }
                 if (busy) {
+                    const uint32_t fidx = blk * (uint32_t)R3 + (uint32_t)((gz * R + gy) * R + gx);
+                    MCRT_CHK(fidx < (uint32_t)P.sub_n, "sub-cube index");
+                    fw = nw_ok ? nw : __ldg(P.sub_cellw + (size_t)kCS * fidx);
+                    nw_ok = false;
                     // parameters of the faces through which sub-cube g is left: f = c + (g + [u > 0]) / R
                     fx = stx ? (((double)ix + (double)(gx + upx) * invR) - px) * ivx : CUDART_INF;
                     fy = sty ? (((double)iy + (double)(gy + upy) * invR) - py) * ivy : CUDART_INF;
@@ -1215,9 +1224,17 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                     const bool selx = (fx <= fy) && (fx <= fz), sely = !selx && (fy <= fz), selz = !selx && !sely;
                     const double tn = selx ? fx : (sely ? fy : fz);
                     const double ds = tn - t;
-                    const uint32_t fidx = blk * (uint32_t)R3 + (uint32_t)((gz * R + gy) * R + gx);
-                    MCRT_CHK(fidx < (uint32_t)P.sub_n, "sub-cube index");
-                    fw = __ldg(P.sub_cellw + (size_t)kCS * fidx);
+                    // where the packet goes if it does not stop here: the neighbouring sub-cube along the selected axis;
+                    // through a face of the cube: the next cube, same row
+                    int ngx = gx + (selx ? stx : 0), ngy = gy + (sely ? sty : 0), ngz = gz + (selz ? stz : 0);
+                    const bool ox = (unsigned)ngx >= (unsigned)R, oy = (unsigned)ngy >= (unsigned)R, oz = (unsigned)ngz >= (unsigned)R;
+                    ngx = ox ? (upx ? 0 : R - 1) : ngx; ngy = oy ? (upy ? 0 : R - 1) : ngy; ngz = oz ? (upz ? 0 : R - 1) : ngz;
+                    const int nix = ix + (ox ? stx : 0), niy = iy + (oy ? sty : 0), niz = iz + (oz ? stz : 0);
+                    const bool out = ox || oy || oz;
+                    const bool esc = out && (((unsigned)nix >= (unsigned)P.nx) | ((unsigned)niy >= (unsigned)P.ny) | ((unsigned)niz >= (unsigned)P.nz));
+                    if (!out) { nw = __ldg(P.sub_cellw + (size_t)kCS * (blk * (uint32_t)R3 + (uint32_t)((ngz * R + ngy) * R + ngx))); nw_ok = true; }
+                    else if (!esc) { nw = __ldg(P.cellw + (size_t)kCS * lin_index(nix, niy, niz, lpx, lpxy)); nw_ok = true; }
+                    // physics of this sub-cube
                     const double rho_c = cw_rho(fw);
                     const double2 kq = s_kk[cw_species(fw) * nf + j];
                     if (XTRA >= 3 && P.redraw) {
@@ -1232,16 +1249,9 @@ __global__ void __launch_bounds__(MCRT_MAX_THREADS, 1) k_transport(const Transpo
                         if (__double2hiint(rho_c) != 0) { lucy_add(P.sub_lfx, fidx, kq.y * rho_c * ds); ndusty_acc++; }
                         t = tn;
                         ncross++;
-                        // the neighbouring sub-cube along the selected axis; through a face of the cube: the next cube, same row
-                        gx += selx ? stx : 0; gy += sely ? sty : 0; gz += selz ? stz : 0;
-                        const bool ox = (unsigned)gx >= (unsigned)R, oy = (unsigned)gy >= (unsigned)R, oz = (unsigned)gz >= (unsigned)R;
-                        gx = ox ? (upx ? 0 : R - 1) : gx; gy = oy ? (upy ? 0 : R - 1) : gy; gz = oz ? (upz ? 0 : R - 1) : gz;
-                        ix += ox ? stx : 0; iy += oy ? sty : 0; iz += oz ? stz : 0;
-                        need_cube = ox || oy || oz;
-                        if (need_cube) {
-                            escaped = ((unsigned)ix >= (unsigned)P.nx) | ((unsigned)iy >= (unsigned)P.ny) | ((unsigned)iz >= (unsigned)P.nz);
-                            if (escaped) busy = false;
-                        }
+                        gx = ngx; gy = ngy; gz = ngz; ix = nix; iy = niy; iz = niz;
+                        need_cube = out;
+                        if (esc) { escaped = true; busy = false; }
                     }
                 }
             } while (__popc(__ballot_sync(kFull, busy)) >= max(min(nr, MCRT_J_MIN), 1));
