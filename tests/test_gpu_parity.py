@@ -877,3 +877,47 @@ def test_new_entry_points_reject_bad_arguments(B):
     with pytest.raises(B.McrtError):
         c.run(2000, 2, mode=B.MCRT_MODE_FROZEN_T_SWEEP, n_sweeps=1, lucy_hybrid=1)                # the other estimator's tallies
     c.close()
+
+
+@pytest.mark.parametrize("feature", ["mixtures", "sub_cubes"])
+def test_parity_next3_features_on_the_full_256_grid(B, orc, feature):
+    """NEXT-3 at BASELINE config 4's full grid size (256^3, 5000 clumps) in the default launch configuration: mixtures of
+    two materials in every species / the 1.2e6 dusty cubes nearest the source divided into 2^3 sub-cubes (block numbers
+    and sub-cube indices far beyond what the small grids reach).  3e5 packets, bit-equal to the oracle."""
+    w = W.torus256(n_clumps=5000)
+    N = 300_000
+    if feature == "mixtures":
+        w.mixtures = ([2, 2, 1], [[0, 2], [1, 0], [2, -1]], [[0.7, 0.3], [0.45, 0.55], [1.0, 0.0]])
+    else:
+        rng = np.random.default_rng(8)
+        dusty = np.flatnonzero(w.rho.reshape(-1) > 0)
+        iz, iy, ix = np.unravel_index(dusty, w.rho.shape)
+        d2 = (ix - 127.5) ** 2 + (iy - 127.5) ** 2 + (iz - 127.5) ** 2
+        cube = np.sort(dusty[np.argsort(d2, kind="stable")[:1_200_000]])
+        rho_sub = (w.rho.reshape(-1)[cube][:, None] * rng.uniform(0.3, 1.7, (len(cube), 8))).astype(np.float32)
+        rho_sub[rng.random(rho_sub.shape) < 0.1] = 0.0
+        w.subgrid = (2, cube, rho_sub, rng.integers(0, 3, (len(cube), 8)).astype(np.uint8))
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 404, n_threads=NTH, digests=True)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 404, record_digests=1)
+    for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+        assert ro[key] == rg[key], key
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    nc0 = w.rho.size
+    for key in ("sed", "sed_direct"):
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    for key in ("k", "lucy_fx", "tidx"):
+        assert np.array_equal(raw_o[key][:nc0], raw_g[key]), key
+    if feature == "mixtures":
+        o1, g1 = o.read_raw_comp1(), c.read_component(1)
+        for key in ("k", "lucy_fx", "tidx"):
+            assert np.array_equal(o1[key], g1[key]), key
+        assert g1["k"].sum() > 10_000
+    else:
+        sub = c.read_subcells()
+        for key in ("k", "lucy_fx", "tidx"):
+            assert np.array_equal(raw_o[key][nc0:], sub[key]), key
+        assert sub["k"].sum() > 10_000
+    c.close()
