@@ -921,3 +921,26 @@ def test_parity_next3_features_on_the_full_256_grid(B, orc, feature):
             assert np.array_equal(raw_o[key][nc0:], sub[key]), key
         assert sub["k"].sum() > 10_000
     c.close()
+
+
+@pytest.mark.parametrize("option", ["lucy_hybrid", "tau_redraw_per_cell", "source_strata", "carry_interactions"])
+def test_parity_run_options_on_the_full_256_grid(B, orc, option):
+    """The rarely used run options (kernel instantiations XTRA = 1, 2, 3) at config 4's full grid in the default launch
+    configuration, 3e5 packets: digests and all tallies bit-equal to the oracle."""
+    w = W.torus256(n_clumps=5000)
+    N = 300_000
+    okw, gkw = {"lucy_hybrid": (dict(lucy_hybrid=True), dict(lucy_hybrid=1)),
+                "tau_redraw_per_cell": (dict(per_cell_redraw=True), dict(tau_redraw_per_cell=1)),
+                "source_strata": (dict(source_strata=1000), dict(source_strata=1000)),
+                "carry_interactions": (dict(carry_K=20), dict(carry_interactions=20))}[option]
+    o = orc.Oracle.from_workload(w)
+    ro = o.run(N, 505, n_threads=NTH, digests=True, **okw)
+    c = B.Context(w, n_digests=N)
+    rg = c.run(N, 505, record_digests=1, **gkw)
+    for key in ("packets", "crossings", "dusty_crossings", "scatterings", "absorptions", "direct_escapes"):
+        assert ro[key] == rg[key], key
+    raw_o, raw_g = o.read_raw(), c.read_raw(digests=True)
+    assert np.array_equal(ro["digests"], raw_g["digests"])
+    for key in RAW_KEYS:
+        assert np.array_equal(raw_o[key], raw_g[key]), key
+    c.close()
